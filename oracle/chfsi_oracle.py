@@ -1,0 +1,378 @@
+"""CPU ORACLE for the Chebyshev-filter hot path of DFT-FE (arxiv 2203.07820).  TEST INFRASTRUCTURE ONLY.
+
+This file is a plain, slow, obviously-correct float64 NumPy statement of what the path computes, written
+from the paper (citations are `PAPER.md:<line>` = /root/reference/PAPER.md plus the section / equation).
+It shares NO code with the CUDA path (`paper_2203_07820_b200/`): its own GLL / Gauss tables, its own shape
+functions, its own cell matrices, its own loops.  Only `tests/`, `__graft_entry__.smoke()` and `bench.py`'s
+`cpu_baseline` / `--impl reference` leg may import it; the product never does.
+
+What the path computes:
+
+    H~ = M^-1/2 ( 1/2 K + V + sum_a C_a D_a C_a^T ) M^-1/2          Eq. 30 (terms 1-2), 33, 34
+    Y  = T_m((H~ - c)/e) X / T_m((a0 - c)/e),  e=(b-a)/2, c=(b+a)/2   Eq. 37 + scaled form of ref. [86]
+
+The cell-level batched form (Eq. 47) and Algorithm 4 are exact
+re-bracketings of that global product, so the oracle follows them literally:  extraction -> per-cell dense
+product -> assembly, and  C^T X -> assemble P -> scale by D -> C P -> assemble.
+
+Parity pins (tests/test_oracle_*.py, all `-m "not gpu"`): every function below is pinned to a closed form,
+an invariant, a textbook/library special case or brute force -- see DESIGN.md Sec. 6.  Parity unpinned: none.
+
+Readings of the paper taken here: U1 scaled recurrence, U2 (p+2)^3 Gauss points for K
+and V, U3 P_Ip = N_j N_k, U4 M^-1/2 applied at the vector level, U5 h_lp = D, U6 x-fastest orderings and
+trilinear cells.
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass
+from typing import Optional
+
+import numpy as np
+
+# ---------------------------------------------------------------------------------------------------------
+# 1-D tables
+# ---------------------------------------------------------------------------------------------------------
+
+
+def legendre(n: int, x):
+    """(P_n(x), P_n'(x)) by the three-term recurrence (k+1)P_{k+1} = (2k+1) x P_k - k P_{k-1}."""
+    x = np.asarray(x, dtype=np.float64)
+    p0, p1 = np.ones_like(x), x.copy()
+    if n == 0:
+        return p0, np.zeros_like(x)
+    for k in range(1, n):
+        p0, p1 = p1, ((2 * k + 1) * x * p1 - k * p0) / (k + 1)
+    # (1 - x^2) P_n' = n (P_{n-1} - x P_n)
+    with np.errstate(divide="ignore", invalid="ignore"):
+        dp = n * (p0 - x * p1) / (1 - x * x)
+    return p1, dp
+
+
+def gauss_legendre(nq: int):
+    """Gauss-Legendre nodes (ascending) and weights on [-1,1]: roots of P_nq, w = 2/((1-x^2) P_nq'(x)^2)."""
+    k = np.arange(1, nq + 1)
+    x = -np.cos(np.pi * (k - 0.25) / (nq + 0.5))           # Chebyshev-like initial guess, ascending
+    for _ in range(100):
+        pn, dpn = legendre(nq, x)
+        dx = pn / dpn
+        x = x - dx
+        if np.max(np.abs(dx)) < 1e-16:
+            break
+    _, dpn = legendre(nq, x)
+    w = 2.0 / ((1 - x * x) * dpn * dpn)
+    return x, w
+
+
+def gauss_lobatto_legendre(p: int):
+    """GLL nodes (ascending, p+1 of them) and weights: end points +-1 and the roots of P_p'(x);
+    w_i = 2 / (p (p+1) P_p(x_i)^2).  Spectral FE nodes, PAPER.md:301 (Sec. 2.3)."""
+    if p < 1:
+        raise ValueError("p >= 1")
+    x = -np.cos(np.pi * np.arange(p + 1) / p)               # Chebyshev-Gauss-Lobatto initial guess
+    xi = x[1:-1].copy()
+    for _ in range(100):
+        # Newton on q(x) = P_p'(x); q'(x) from Legendre's ODE: (1-x^2) P'' = 2x P' - p(p+1) P
+        pn, dpn = legendre(p, xi)
+        d2 = (2 * xi * dpn - p * (p + 1) * pn) / (1 - xi * xi)
+        dx = dpn / d2
+        xi = xi - dx
+        if xi.size == 0 or np.max(np.abs(dx)) < 1e-16:
+            break
+    x[1:-1] = xi
+    x[0], x[-1] = -1.0, 1.0
+    pn, _ = legendre(p, x)
+    w = 2.0 / (p * (p + 1) * pn * pn)
+    return x, w
+
+
+def lagrange_basis(nodes, x):
+    """Values and first derivatives of the Lagrange polynomials l_i through `nodes`, at points `x`.
+    Returns (L, dL), both [len(x), len(nodes)].  Direct product formula, O(p^3) per point."""
+    nodes = np.asarray(nodes, dtype=np.float64)
+    x = np.asarray(x, dtype=np.float64)
+    n = nodes.size
+    L = np.ones((x.size, n))
+    dL = np.zeros((x.size, n))
+    for i in range(n):
+        for j in range(n):
+            if j != i:
+                L[:, i] *= (x - nodes[j]) / (nodes[i] - nodes[j])
+        for k in range(n):
+            if k == i:
+                continue
+            term = np.full(x.size, 1.0 / (nodes[i] - nodes[k]))
+            for j in range(n):
+                if j != i and j != k:
+                    term *= (x - nodes[j]) / (nodes[i] - nodes[j])
+            dL[:, i] += term
+    return L, dL
+
+
+# ---------------------------------------------------------------------------------------------------------
+# reference-cell tables in 3-D (x fastest: l = a + (p+1)(b + (p+1)c), q = qa + nq1 (qb + nq1 qc))
+# ---------------------------------------------------------------------------------------------------------
+
+
+@dataclass
+class RefCell:
+    p: int
+    gll_x: np.ndarray      # [p+1]
+    gll_w: np.ndarray
+    gq_x: np.ndarray       # [p+2]
+    gq_w: np.ndarray
+    N: np.ndarray          # [nq, M_cell]      shape-function values at the Gauss points
+    dN: np.ndarray         # [nq, 3, M_cell]   reference-coordinate gradients at the Gauss points
+    wq: np.ndarray         # [nq]              tensor-product Gauss weights
+    ref_q: np.ndarray      # [nq, 3]
+    ref_nodes: np.ndarray  # [M_cell, 3]
+    w_nodes: np.ndarray    # [M_cell]          tensor-product GLL weights
+
+
+def reference_cell(p: int) -> RefCell:
+    gx, gw = gauss_lobatto_legendre(p)
+    qx, qw = gauss_legendre(p + 2)                           # reading U2: (p+2)^3 Gauss points
+    l1, d1 = lagrange_basis(gx, qx)                          # [p+2, p+1]
+    n1, nq1 = p + 1, p + 2
+    M, nq = n1 ** 3, nq1 ** 3
+    N = np.zeros((nq, M))
+    dN = np.zeros((nq, 3, M))
+    wq = np.zeros(nq)
+    ref_q = np.zeros((nq, 3))
+    for qc in range(nq1):
+        for qb in range(nq1):
+            for qa in range(nq1):
+                q = qa + nq1 * (qb + nq1 * qc)
+                wq[q] = qw[qa] * qw[qb] * qw[qc]
+                ref_q[q] = (qx[qa], qx[qb], qx[qc])
+                for c in range(n1):
+                    for b in range(n1):
+                        for a in range(n1):
+                            l = a + n1 * (b + n1 * c)
+                            N[q, l] = l1[qa, a] * l1[qb, b] * l1[qc, c]
+                            dN[q, 0, l] = d1[qa, a] * l1[qb, b] * l1[qc, c]
+                            dN[q, 1, l] = l1[qa, a] * d1[qb, b] * l1[qc, c]
+                            dN[q, 2, l] = l1[qa, a] * l1[qb, b] * d1[qc, c]
+    ref_nodes = np.zeros((M, 3))
+    w_nodes = np.zeros(M)
+    for c in range(n1):
+        for b in range(n1):
+            for a in range(n1):
+                l = a + n1 * (b + n1 * c)
+                ref_nodes[l] = (gx[a], gx[b], gx[c])
+                w_nodes[l] = gw[a] * gw[b] * gw[c]
+    return RefCell(p, gx, gw, qx, qw, N, dN, wq, ref_q, ref_nodes, w_nodes)
+
+
+def trilinear_jacobian(vertices, ref_pts):
+    """Jacobian J[pt, i, d] = d x_i / d xi_d of the trilinear map of one cell (vertices [8,3], vertex
+    v = vx + 2 vy + 4 vz) at reference points [npt, 3]."""
+    J = np.zeros((ref_pts.shape[0], 3, 3))
+    for v in range(8):
+        s = [2 * ((v >> d) & 1) - 1 for d in range(3)]
+        f = [(1 + s[d] * ref_pts[:, d]) / 2 for d in range(3)]
+        df = [s[d] / 2.0 for d in range(3)]
+        grads = [df[0] * f[1] * f[2], f[0] * df[1] * f[2], f[0] * f[1] * df[2]]
+        for i in range(3):
+            for d in range(3):
+                J[:, i, d] += vertices[v, i] * grads[d]
+    return J
+
+
+# ---------------------------------------------------------------------------------------------------------
+# the operator
+# ---------------------------------------------------------------------------------------------------------
+
+
+@dataclass
+class Operator:
+    p: int
+    n_cells: int
+    n_dofs: int
+    cell_dofs: np.ndarray              # [n_cells, M_cell]
+    M: np.ndarray                      # [n_dofs]     diagonal GLL mass matrix
+    He: np.ndarray                     # [n_cells, M_cell, M_cell]   1/2 K^e + V^e   (NOT Loewdin-scaled)
+    n_proj: int
+    D: np.ndarray                      # [n_proj]
+    proj_cell_ptr: np.ndarray          # CSR projector -> cells
+    proj_cell_idx: np.ndarray
+    Cc: np.ndarray                     # [nnz, M_cell]  C^c_{l,j} for the (j, c) pair k of the CSR
+
+
+def mass_diagonal(p, cell_dofs, cell_vertices, n_dofs, ref: Optional[RefCell] = None):
+    """M_g = sum over cells containing g of  w_a w_b w_c det J(node):  the overlap matrix integrated with
+    the GLL rule whose points coincide with the FE nodes, which makes it diagonal.  PAPER.md:336."""
+    ref = ref or reference_cell(p)
+    M = np.zeros(n_dofs)
+    for c in range(cell_dofs.shape[0]):
+        J = trilinear_jacobian(cell_vertices[c], ref.ref_nodes)
+        detJ = np.linalg.det(J)
+        if np.any(detJ <= 0):
+            raise ValueError(f"cell {c}: non-positive Jacobian")
+        M[cell_dofs[c]] += ref.w_nodes * detJ              # dofs are distinct inside one cell
+    return M
+
+
+def cell_hamiltonian(ref: RefCell, vertices, veff_q):
+    """H^e = 1/2 K^e + V^e for one cell (Eq. 30 terms 1-2; quadrature form Eq. 40,
+    PAPER.md:462, with P_Ip = N_j(q_p) N_k(q_p), reading U3):
+        K^e_jk = sum_q w_q detJ_q (J_q^-T grad N_j)(q) . (J_q^-T grad N_k)(q)
+        V^e_jk = sum_q w_q detJ_q V(q) N_j(q) N_k(q)."""
+    J = trilinear_jacobian(vertices, ref.ref_q)              # [nq, 3, 3]
+    detJ = np.linalg.det(J)
+    if np.any(detJ <= 0):
+        raise ValueError("non-positive Jacobian")
+    Jinv = np.linalg.inv(J)                                  # Jinv[q, d, i] = d xi_d / d x_i
+    # physical gradient of N_l: g[q, i, l] = sum_d Jinv[q, d, i] dN[q, d, l]
+    g = np.einsum("qdi,qdl->qil", Jinv, ref.dN)
+    wj = ref.wq * detJ
+    K = np.einsum("q,qij,qik->jk", wj, g, g, optimize=True)
+    V = (ref.N * (wj * veff_q)[:, None]).T @ ref.N
+    return 0.5 * K + V, K, V
+
+
+def projector_cell_vector(ref: RefCell, vertices, chi_q):
+    """C^c_{l} = sum_q w_q detJ_q chi(q) N_l(q)   (Eq. 33; Gamma point: phase factors 1)."""
+    detJ = np.linalg.det(trilinear_jacobian(vertices, ref.ref_q))
+    return ref.N.T @ (ref.wq * detJ * chi_q)
+
+
+def build_operator(p, cell_dofs, cell_vertices, n_dofs, veff_q, n_proj=0, D=None, proj_cell_ptr=None,
+                   proj_cell_idx=None, chi_q=None) -> Operator:
+    ref = reference_cell(p)
+    n_cells, m_cell = cell_dofs.shape
+    assert m_cell == (p + 1) ** 3
+    for c in range(n_cells):
+        if np.unique(cell_dofs[c]).size != m_cell:
+            raise ValueError(f"cell {c}: repeated dof inside one cell")
+    M = mass_diagonal(p, cell_dofs, cell_vertices, n_dofs, ref)
+    He = np.zeros((n_cells, m_cell, m_cell))
+    for c in range(n_cells):
+        He[c] = cell_hamiltonian(ref, cell_vertices[c], veff_q[c])[0]
+    if n_proj:
+        nnz = int(proj_cell_ptr[-1])
+        Cc = np.zeros((nnz, m_cell))
+        for j in range(n_proj):
+            for k in range(int(proj_cell_ptr[j]), int(proj_cell_ptr[j + 1])):
+                Cc[k] = projector_cell_vector(ref, cell_vertices[proj_cell_idx[k]], chi_q[k])
+        return Operator(p, n_cells, n_dofs, cell_dofs, M, He, n_proj, np.asarray(D, dtype=np.float64),
+                        np.asarray(proj_cell_ptr), np.asarray(proj_cell_idx), Cc)
+    return Operator(p, n_cells, n_dofs, cell_dofs, M, He, 0, np.zeros(0), np.zeros(1, dtype=np.int64),
+                    np.zeros(0, dtype=np.int32), np.zeros((0, m_cell)))
+
+
+def operator_from_workload(wl) -> Operator:
+    return build_operator(wl.p, wl.cell_dofs, wl.cell_vertices, wl.n_dofs, wl.veff_q, wl.n_proj, wl.D,
+                          wl.proj_cell_ptr, wl.proj_cell_idx, wl.chi_q)
+
+
+def apply_H(op: Operator, X):
+    """Y = H~ X for a block X [n_dofs, B] of Loewdin-space vectors (Eq. 34).
+
+    Local part, Eq. 47: (i) extraction X -> X^c, (ii) H^c X^c, (iii) assembly.
+    Non-local part, Algorithm 4: 1 extraction, 2 P^c = C^cT X^c, 3 P = ASEMB_NLP{P^c},
+    4 scale by h_lp (= D, reading U5), 5 Y^c = C^c P^c, 6 ASEMB_FEM."""
+    X = np.asarray(X, dtype=np.float64)
+    if X.ndim == 1:
+        return apply_H(op, X[:, None])[:, 0]
+    s = 1.0 / np.sqrt(op.M)
+    U = s[:, None] * X                                        # M^-1/2 X (reading U4)
+    W = np.zeros_like(U)
+    for c in range(op.n_cells):
+        g = op.cell_dofs[c]
+        W[g] += op.He[c] @ U[g]                               # extraction, dense product, assembly
+    if op.n_proj:
+        P = np.zeros((op.n_proj, X.shape[1]))
+        for j in range(op.n_proj):
+            for k in range(int(op.proj_cell_ptr[j]), int(op.proj_cell_ptr[j + 1])):
+                g = op.cell_dofs[op.proj_cell_idx[k]]
+                P[j] += op.Cc[k] @ U[g]                       # Alg. 4 steps 1-3
+        P *= op.D[:, None]                                    # step 4
+        for j in range(op.n_proj):
+            for k in range(int(op.proj_cell_ptr[j]), int(op.proj_cell_ptr[j + 1])):
+                g = op.cell_dofs[op.proj_cell_idx[k]]
+                W[g] += np.outer(op.Cc[k], P[j])              # steps 5-6
+    return s[:, None] * W
+
+
+def chebyshev_filter(op: Operator, X, m: int, a: float, b: float, a0: float):
+    """Degree-m scaled Chebyshev filter (Eq. 37, in the scaled three-term form of ref. [86]
+    (Zhou, Saad, Tiago, Chelikowsky); reading U1):
+
+        e = (b-a)/2, c = (b+a)/2, sigma_1 = e/(a0-c)
+        Y_1 = (sigma_1/e) (H~ X - c X)
+        sigma_k = 1/(2/sigma_1 - sigma_{k-1});  Y_k = (2 sigma_k/e)(H~ Y_{k-1} - c Y_{k-1}) - sigma_{k-1} sigma_k Y_{k-2}
+
+    which equals T_m((H~-c)/e) X / T_m((a0-c)/e)."""
+    if m < 1 or not (a0 <= a < b):
+        raise ValueError("need m >= 1 and a0 <= a < b")
+    X = np.asarray(X, dtype=np.float64)
+    e, c = (b - a) / 2, (b + a) / 2
+    sigma1 = e / (a0 - c)
+    sigma = sigma1
+    Ym2 = X
+    Ym1 = (sigma1 / e) * (apply_H(op, X) - c * X)
+    for _ in range(2, m + 1):
+        sigma_new = 1.0 / (2.0 / sigma1 - sigma)
+        Y = (2 * sigma_new / e) * (apply_H(op, Ym1) - c * Ym1) - (sigma * sigma_new) * Ym2
+        Ym2, Ym1, sigma = Ym1, Y, sigma_new
+    return Ym1
+
+
+# ---------------------------------------------------------------------------------------------------------
+# harness-level helpers (bounds a0, a, b and the Rayleigh-Ritz parity measure; reading U7)
+# ---------------------------------------------------------------------------------------------------------
+
+
+def lanczos_upper_bound(op: Operator, v0, k: int = 20):
+    """k-step Lanczos on H~ from start vector v0; returns (upper bound lambda_max(T_k) + |f_k|, lambda_min(T_k)).
+    The safeguarded estimator used with Chebyshev filtering in ref. [86]."""
+    n = op.n_dofs
+    v = np.asarray(v0, dtype=np.float64) / np.linalg.norm(v0)
+    alpha, beta = [], []
+    v_prev = np.zeros(n)
+    f = apply_H(op, v)
+    a_ = float(f @ v)
+    f = f - a_ * v
+    alpha.append(a_)
+    for _ in range(1, k):
+        b_ = float(np.linalg.norm(f))
+        if b_ < 1e-14:
+            break
+        v_prev, v = v, f / b_
+        f = apply_H(op, v) - b_ * v_prev
+        a_ = float(f @ v)
+        f = f - a_ * v
+        alpha.append(a_)
+        beta.append(b_)
+    T = np.diag(alpha) + np.diag(beta, 1) + np.diag(beta, -1)
+    ev = np.linalg.eigvalsh(T)
+    return float(ev[-1] + np.linalg.norm(f)), float(ev[0])
+
+
+def rayleigh_ritz(op: Operator, Y, HY=None, rel_cut: float = 1e-12):
+    """Ritz values of H~ in span(Y) (Algorithm 2: S = Y^T Y, H^ = Y^T H~ Y, generalised
+    eigenproblem), after column normalisation; directions with S-eigenvalue < rel_cut * max are discarded."""
+    Y = np.asarray(Y, dtype=np.float64)
+    Y = Y / np.linalg.norm(Y, axis=0, keepdims=True)
+    HY = apply_H(op, Y) if HY is None else HY
+    S = Y.T @ Y
+    Hh = Y.T @ HY
+    Hh = 0.5 * (Hh + Hh.T)
+    w, Q = np.linalg.eigh(S)
+    keep = w > rel_cut * w[-1]
+    Qk = Q[:, keep] / np.sqrt(w[keep])[None, :]
+    return np.linalg.eigvalsh(Qk.T @ Hh @ Qk)
+
+
+def ritz_values_of_block(Y, HY, rel_cut: float = 1e-12):
+    """Same as rayleigh_ritz but for a given pair (Y, H~Y) (used to compare GPU and oracle blocks with the
+    SAME H~Y provider).  Columns are normalised with the norms of Y."""
+    nrm = np.linalg.norm(Y, axis=0, keepdims=True)
+    Y, HY = Y / nrm, HY / nrm
+    S = Y.T @ Y
+    Hh = Y.T @ HY
+    Hh = 0.5 * (Hh + Hh.T)
+    w, Q = np.linalg.eigh(S)
+    keep = w > rel_cut * w[-1]
+    Qk = Q[:, keep] / np.sqrt(w[keep])[None, :]
+    return np.linalg.eigvalsh(Qk.T @ Hh @ Qk)
