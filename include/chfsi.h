@@ -1,0 +1,143 @@
+/* chfsi.h -- C ABI of the B200-native Chebyshev-filter hot path of DFT-FE (arxiv 2203.07820).
+ *
+ * Citations are PAPER.md:<line> (= /root/reference/PAPER.md) plus the section / equation / algorithm.
+ *
+ * What the library computes
+ * -------------------------
+ *   H~ = M^-1/2 ( 1/2 K + V_eff + sum_a C_a D_a C_a^T ) M^-1/2           Eq. 30 terms 1-2,
+ *                                                                         Eq. 33, Eq. 34
+ *   apply_H :          Y = H~ X                                           Eq. 47, Alg. 4
+ *   chebyshev_filter : X <- T_m((H~ - c)/e) X / T_m((a0 - c)/e),  e=(b-a)/2, c=(b+a)/2
+ *                      Eq. 37 in the scaled three-term form of ref. [86]:
+ *                        sigma_1 = e/(a0-c);  Y_1 = (sigma_1/e)(H~ X - c X)
+ *                        sigma_k = 1/(2/sigma_1 - sigma_{k-1})
+ *                        Y_k = (2 sigma_k/e)(H~ Y_{k-1} - c Y_{k-1}) - sigma_{k-1} sigma_k Y_{k-2},  k = 2..m
+ *
+ * on a hexahedral spectral-element mesh (GLL nodes) with the diagonal GLL mass matrix M
+ * (PAPER.md:336), K and V_eff integrated with (p+2)^3 Gauss-Legendre points, cell by cell:
+ * extraction -> per-cell dense product with the Loewdin-scaled cell matrix -> assembly.
+ *
+ * Conventions
+ * -----------
+ *  - Every call returns an int: CHFSI_OK (0) or a negative chfsi_status.  Nothing throws or aborts across
+ *    the ABI.  chfsi_last_error() gives a human-readable message for the last failing call on a handle
+ *    (or for a failed chfsi_create when passed NULL).
+ *  - Vectors live in the Loewdin space x~ = M^{1/2} x^.  A block of vectors is a row-major
+ *    array [n_dofs][ld] with the VECTOR INDEX FASTEST; ld >= B, so a chunk of B columns of a
+ *    wider array is addressed by passing a pointer to its first column and the wide array's ld.
+ *    Element type is double (precision 64) or float (precision 32).
+ *  - "_dev" pointers are device pointers owned by the CALLER (PyTorch allocates them); "_host"/plain struct
+ *    members are host pointers.  The library copies everything it needs from the host inputs of
+ *    chfsi_create during that call; the caller may free them afterwards.  The library owns its device
+ *    copies (cell matrices, maps) until chfsi_destroy.
+ *  - All device work of the *_dev entry points is enqueued on the caller's cudaStream_t (passed as void*,
+ *    NULL = default stream).  They never synchronise the host.  chfsi_create and the *_host entry points
+ *    synchronise before returning.
+ *  - There is no CPU fallback: without a CUDA device chfsi_create returns CHFSI_ERR_CUDA.
+ *  - Alignment: X_dev / Y_dev / workspace_dev must be 16-byte aligned and ld*sizeof(element) a multiple of
+ *    16 for the tensor-core path; other shapes take a slower generic CUDA path (never the CPU).
+ */
+#ifndef CHFSI_H_
+#define CHFSI_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  CHFSI_OK = 0,
+  CHFSI_ERR_BAD_ARGUMENT = -1, /* NULL pointer, B < 1, ld < B, m < 1, !(a0 <= a && a < b), bad precision ... */
+  CHFSI_ERR_BAD_MESH = -2,     /* dof out of range / repeated inside one cell / non-positive Jacobian         */
+  CHFSI_ERR_OUT_OF_MEMORY = -3,
+  CHFSI_ERR_CUDA = -4,         /* any CUDA runtime failure, including "no device"                              */
+  CHFSI_ERR_UNSUPPORTED = -5   /* p outside 1..8, precision not 32/64                                          */
+} chfsi_status;
+
+typedef struct chfsi_op chfsi_op; /* opaque operator handle */
+
+/* Mesh: "cell connectivity, FE degree" (north_star; Sec. 2.3).  All host pointers. */
+typedef struct {
+  int32_t p;                    /* FE degree 1..8; (p+1)^3 GLL nodes per cell                               */
+  int64_t n_cells;
+  int64_t n_dofs;
+  const int32_t* cell_dofs;     /* [n_cells][(p+1)^3]; local node l = a + (p+1)(b + (p+1)c), x fastest;
+                                   periodic identification already applied; dofs distinct inside a cell   */
+  const double* cell_vertices;  /* [n_cells][8][3]; vertex v = vx + 2 vy + 4 vz; unwrapped coordinates;
+                                   the cell is the trilinear image of [-1,1]^3                             */
+} chfsi_mesh;
+
+/* Local potential: V_eff sampled at the (p+2)^3 Gauss-Legendre points of every cell (Eq. 40). */
+typedef struct {
+  const double* veff_q;         /* [n_cells][(p+2)^3], q = qa + (p+2)(qb + (p+2)qc), x fastest              */
+} chfsi_potential;
+
+/* Non-local projectors (Eq. 33).  NULL pointer or n_proj == 0: no such term. */
+typedef struct {
+  int64_t n_proj;
+  const double* D;              /* [n_proj] coupling h_lp (Alg. 4 step 4)                     */
+  const int64_t* proj_cell_ptr; /* [n_proj+1] CSR: projector j lives on cells proj_cell_idx[ptr[j]..ptr[j+1]) */
+  const int32_t* proj_cell_idx; /* [nnz] cell ids, distinct within one projector                            */
+  const double* chi_q;          /* [nnz][(p+2)^3] projector function at the Gauss points of that cell       */
+} chfsi_nonlocal;
+
+/* Sizes and the algorithmic work of one H~ application, for benchmarks and tests. */
+typedef struct {
+  int32_t p, m_cell, n_q, precision, assembly, n_colors;
+  int64_t n_cells, n_dofs, n_proj;
+  int64_t nnz_cell_proj;        /* sum over cells of N_psp^c (projectors touching the cell)                 */
+  int64_t cells_with_proj;
+  double flops_per_vector_apply;/* n_cells*2*m_cell^2 + 4*m_cell*nnz_cell_proj + 7*n_dofs  */
+  int64_t matrix_bytes;         /* device bytes of the Loewdin-scaled cell matrices (incl. padding)         */
+} chfsi_info;
+
+/* assembly: 0 = deterministic (graph colouring of cells that share a dof; one launch per colour, the
+ *               recurrence is fused into the first write of every dof),
+ *           1 = atomic (one launch, red.global.add; result depends on summation order within rounding). */
+int chfsi_create(chfsi_op** out, const chfsi_mesh* mesh, const chfsi_potential* pot,
+                 const chfsi_nonlocal* nl /* nullable */, int precision /* 64 | 32 */,
+                 int assembly /* 0 | 1 */, void* cuda_stream);
+int chfsi_destroy(chfsi_op* op);
+int chfsi_get_info(const chfsi_op* op, chfsi_info* info);
+
+/* Device workspace (bytes) that chfsi_apply_H / chfsi_chebyshev_filter need for a block of B columns. */
+int chfsi_workspace_bytes(const chfsi_op* op, int64_t B, size_t* bytes);
+
+/* Diagonal GLL mass matrix, FP64, copied to a device array [n_dofs] (for the harness:
+ * x~ = M^{1/2} x^). */
+int chfsi_mass_diag(const chfsi_op* op, double* M_dev, void* cuda_stream);
+
+/* Y = H~ X for a block of B columns.  X_dev and Y_dev must not overlap. */
+int chfsi_apply_H(chfsi_op* op, const void* X_dev, int64_t ldx, void* Y_dev, int64_t ldy, int64_t B,
+                  void* workspace_dev, void* cuda_stream);
+
+/* In place: X <- scaled Chebyshev filter of degree m applied to the B columns of X_dev. */
+int chfsi_chebyshev_filter(chfsi_op* op, void* X_dev, int64_t ldx, int64_t B, int32_t m, double a, double b,
+                           double a0, void* workspace_dev, void* cuda_stream);
+
+/* The same for N columns filtered in sequential chunks of at most B columns ("blocks of B_f
+ * vectors filtered sequentially"); workspace sized for B. */
+int chfsi_chebyshev_filter_chunked(chfsi_op* op, void* X_dev, int64_t ldx, int64_t N, int64_t B, int32_t m,
+                                   double a, double b, double a0, void* workspace_dev, void* cuda_stream);
+
+/* End-to-end variant with HOST buffers: X_host is [n_dofs][ldx] (element type per precision); the call
+ * allocates device staging for one chunk, copies each chunk host->device, filters it, copies it back, and
+ * synchronises before returning. */
+int chfsi_chebyshev_filter_host(chfsi_op* op, void* X_host, int64_t ldx, int64_t N, int64_t B, int32_t m,
+                                double a, double b, double a0);
+
+/* Number of kernel launches enqueued by this handle since creation (for benchmark bookkeeping). */
+int64_t chfsi_launch_count(const chfsi_op* op);
+
+/* Selects the kernel used for the per-cell contraction: 0 = automatic (tensor-core path when the shape
+ * allows), 1 = force the generic path.  For tests and A/B measurements. */
+int chfsi_set_kernel_variant(chfsi_op* op, int variant);
+
+const char* chfsi_last_error(const chfsi_op* op /* NULL: last failed chfsi_create of this thread */);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CHFSI_H_ */

@@ -1,0 +1,416 @@
+// Hot-path kernels of libchfsi: one fused launch sequence per H~ application + Chebyshev recurrence update.
+//
+//   step 1  cell extraction          X^e = rows of X through the cell->dof map      PAPER.md:513 (i), :515
+//   step 2  per-cell contraction     Y^e = H~^e X^e    (FP64: mma.sync m8n8k4 DMMA)   Eq. 47
+//   step 3  non-local                P^c = C~^cT X^e ; P = D sum_c P^c ; Y^e += C~^c P   Alg. 4
+//   step 4  assembly                 T[g] += Y^e[l]    (coloured or atomic)           PAPER.md:513 (iii)
+//   step 5  recurrence               Y_k = alpha (H~ Y_{k-1} - c Y_{k-1}) - beta Y_{k-2}   Eq. 37
+//
+// Steps 1, 2, 3d (as extra contraction rows), 4 and 5 run inside ONE kernel (k_apply_dmma / k_apply_generic);
+// steps 3a-3c are two small kernels in front of it because P needs every cell of a projector's support.
+// M^-1/2 is folded into the cell matrices at setup, so no scaling appears here.
+#include <cstdio>
+
+#include "common.h"
+
+namespace chfsi {
+
+namespace {
+
+template <typename T>
+struct ApplyDev {
+  const T* __restrict__ mat;
+  const int64_t* __restrict__ mat_off;
+  const int64_t* __restrict__ idx_off;
+  const int32_t* __restrict__ ktot;
+  const int32_t* __restrict__ gidx;
+  const int32_t* __restrict__ cells;   // cells of this launch
+  int n_launch_cells;
+  int n_col_tiles;
+  int m_cell, lda;
+  const T* __restrict__ X; int64_t ldx;
+  T* __restrict__ Tg; int64_t ldt;
+  const T* __restrict__ P; int64_t ldp;
+  int B;
+  T alpha, beta, ac;                   // ac = alpha * cshift
+  int atomic;                          // 1: red.add into a pre-filled target
+};
+
+__device__ __forceinline__ void red_add(double* p, double v) { atomicAdd(p, v); }
+__device__ __forceinline__ void red_add(float* p, float v) { atomicAdd(p, v); }
+
+// -------------------------------------------------------------------------------------------------------------
+// Generic path: any B, any alignment, any p, double or float.  One CTA = (cell, 32 columns); lane = column.
+// -------------------------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(256) k_apply_generic(ApplyDev<T> a) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  T* Xs = reinterpret_cast<T*>(smem_raw);          // [kt][32]
+  const int cell = a.cells[blockIdx.x / a.n_col_tiles];
+  const int col = (blockIdx.x % a.n_col_tiles) * 32 + (threadIdx.x & 31);
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int kt = a.ktot[cell], mc = a.m_cell;
+  const int32_t* gi = a.gidx + a.idx_off[cell];
+  const T* M = a.mat + a.mat_off[cell];
+  const bool colok = col < a.B;
+  for (int k = warp; k < kt; k += 8) {
+    int idx = gi[k];
+    const T* src = (k < mc) ? a.X + (int64_t)(idx & 0x7fffffff) * a.ldx : a.P + (int64_t)idx * a.ldp;
+    Xs[k * 32 + lane] = colok ? src[col] : (T)0;
+  }
+  __syncthreads();
+  const int n_rt = (mc + 7) / 8;
+  for (int rt = warp; rt < n_rt; rt += 8) {
+    T acc[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) acc[i] = (T)0;
+    const T* Mr = M + rt * 8;
+    for (int k = 0; k < kt; ++k) {
+      T x = Xs[k * 32 + lane];
+#pragma unroll
+      for (int i = 0; i < 8; ++i) acc[i] = fma(Mr[(int64_t)k * a.lda + i], x, acc[i]);
+    }
+    if (!colok) continue;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      int r = rt * 8 + i;
+      if (r >= mc) break;
+      int idx = gi[r];
+      int64_t g = idx & 0x7fffffff;
+      T* tp = a.Tg + g * a.ldt + col;
+      T v = a.alpha * acc[i];
+      if (a.atomic) {
+        red_add(tp, v);
+      } else if (idx < 0) {   // first contribution to this dof: carries the recurrence terms
+        if (a.ac != (T)0) v -= a.ac * a.X[g * a.ldx + col];
+        if (a.beta != (T)0) v -= a.beta * *tp;
+        *tp = v;
+      } else {
+        *tp += v;
+      }
+    }
+  }
+}
+
+// -------------------------------------------------------------------------------------------------------------
+// Steps 3a-3c
+// -------------------------------------------------------------------------------------------------------------
+// P^c[i][col] = sum_l C~^c[l][i] X[dof_l][col]       (Alg. 4 step 2).  grid = (cells with projectors, col tiles of 128)
+template <typename T>
+__global__ void __launch_bounds__(128) k_proj_partial(const T* __restrict__ mat, const int64_t* __restrict__ mat_off,
+                                                      const int64_t* __restrict__ idx_off, const int32_t* __restrict__ gidx,
+                                                      const int32_t* __restrict__ pc_cells,
+                                                      const int64_t* __restrict__ cell_proj_ptr, int m_cell, int lda,
+                                                      const T* __restrict__ X, int64_t ldx, T* __restrict__ Pc, int B) {
+  extern __shared__ int32_t dofs[];
+  const int cell = pc_cells[blockIdx.x];
+  const int col = blockIdx.y * 128 + threadIdx.x;
+  const int32_t* gi = gidx + idx_off[cell];
+  for (int l = threadIdx.x; l < m_cell; l += 128) dofs[l] = gi[l] & 0x7fffffff;
+  __syncthreads();
+  if (col >= B) return;
+  const int64_t r0 = cell_proj_ptr[cell];
+  const int np = (int)(cell_proj_ptr[cell + 1] - r0);
+  const T* C = mat + mat_off[cell] + (int64_t)m_cell * lda;   // rows = projectors of this cell, columns = nodes
+  for (int i0 = 0; i0 < np; i0 += 8) {
+    T acc[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) acc[i] = (T)0;
+    const int ni = min(8, np - i0);
+    for (int l = 0; l < m_cell; ++l) {
+      T x = X[(int64_t)dofs[l] * ldx + col];
+#pragma unroll
+      for (int i = 0; i < 8; ++i)
+        if (i < ni) acc[i] = fma(C[(int64_t)(i0 + i) * lda + l], x, acc[i]);
+    }
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+      if (i < ni) Pc[(r0 + i0 + i) * B + col] = acc[i];
+  }
+}
+
+// P[j][col] = D_j sum_{c in supp(j)} P^c[j][col], fixed CSR order (Alg. 4 steps 3-4); row n_proj = 0 (padding target)
+template <typename T>
+__global__ void __launch_bounds__(128) k_proj_reduce(const T* __restrict__ Pc, const int64_t* __restrict__ proj_ptr,
+                                                     const int64_t* __restrict__ proj_pcrow, const double* __restrict__ D,
+                                                     int64_t n_proj, T* __restrict__ P, int B) {
+  const int64_t j = blockIdx.x;
+  const int col = blockIdx.y * 128 + threadIdx.x;
+  if (col >= B) return;
+  T s = (T)0;
+  if (j < n_proj) {
+    for (int64_t k = proj_ptr[j]; k < proj_ptr[j + 1]; ++k) s += Pc[proj_pcrow[k] * B + col];
+    s *= (T)D[j];
+  }
+  P[j * B + col] = s;
+}
+
+// Atomic assembly needs the recurrence terms in place first:  T <- -alpha c X - beta T
+template <typename T>
+__global__ void __launch_bounds__(256) k_prefill(const T* __restrict__ X, int64_t ldx, T* __restrict__ Tg, int64_t ldt,
+                                                 int64_t n_dofs, int B, T ac, T beta) {
+  int64_t n = n_dofs * B;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    int64_t g = i / B; int col = (int)(i % B);
+    T v = (T)0;
+    if (ac != (T)0) v -= ac * X[g * ldx + col];
+    if (beta != (T)0) v -= beta * Tg[g * ldt + col];
+    Tg[g * ldt + col] = v;
+  }
+}
+
+// -------------------------------------------------------------------------------------------------------------
+// Tensor-core path (FP64): CTA = (cell, 64 columns), 16 warps as 4 (m) x 4 (n); warp tile = MT m-tiles x 2 n-tiles
+// of mma.sync.m8n8k4.f64.  The cell matrix is streamed in 16-row K-panels by cp.async.bulk (one bulk copy per
+// panel; the HBM image of the matrix IS the padded shared-memory image), X^e rows are gathered by one bulk copy per
+// row through the cell->dof map, both landing on an mbarrier; 3-stage ring.
+// -------------------------------------------------------------------------------------------------------------
+constexpr int kPanelK = 16;
+constexpr int kTileN = 64;
+constexpr int kLdXs = kTileN + 4;    // 68: 68 mod 16 == 4 -> conflict-free 64-bit fragment loads
+constexpr int kStages = 3;
+constexpr int kMaxKtot = 1024;
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_LOOP:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra WAIT_DONE;\n"
+      "bra WAIT_LOOP;\n"
+      "WAIT_DONE:\n"
+      "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+               "l"(src), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
+  asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+template <int MT>
+__global__ void __launch_bounds__(512, 1) k_apply_dmma(ApplyDev<double> a) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int lda = a.lda;
+  const int a_panel_elems = kPanelK * lda;
+  const int stage_elems = a_panel_elems + kPanelK * kLdXs;
+  double* stage0 = reinterpret_cast<double*>(smem_raw);
+  uint64_t* full = reinterpret_cast<uint64_t*>(stage0 + kStages * stage_elems);
+  int32_t* idx_s = reinterpret_cast<int32_t*>(full + kStages);
+
+  const int cell = a.cells[blockIdx.x / a.n_col_tiles];
+  const int col0 = (blockIdx.x % a.n_col_tiles) * kTileN;
+  const int ncols = min(kTileN, a.B - col0);             // multiple of 8
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int warp_m = warp >> 2, warp_n = warp & 3;
+  const int kt = a.ktot[cell], mc = a.m_cell;
+  const int32_t* gi = a.gidx + a.idx_off[cell];
+  const double* M = a.mat + a.mat_off[cell];
+
+  for (int k = tid; k < kt; k += 512) idx_s[k] = gi[k];
+  if (tid == 0) {
+    for (int s = 0; s < kStages; ++s) mbar_init(&full[s], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+
+  const int npanel = (kt + kPanelK - 1) / kPanelK;
+  const uint32_t row_bytes = (uint32_t)ncols * 8u;
+  auto issue = [&](int pi) {   // called by warp 0, all lanes
+    const int s = pi % kStages;
+    const int rows = min(kPanelK, kt - pi * kPanelK);
+    double* As = stage0 + s * stage_elems;
+    double* Xs = As + a_panel_elems;
+    if (lane == 0) mbar_expect_tx(&full[s], (uint32_t)rows * ((uint32_t)lda * 8u + row_bytes));
+    __syncwarp();
+    if (lane < rows) {
+      const int k = pi * kPanelK + lane;
+      const int idx = idx_s[k];
+      const double* src = (k < mc) ? a.X + (int64_t)(idx & 0x7fffffff) * a.ldx + col0 : a.P + (int64_t)idx * a.ldp + col0;
+      bulk_g2s(Xs + lane * kLdXs, src, row_bytes, &full[s]);
+    } else if (lane == 16) {
+      bulk_g2s(As, M + (int64_t)pi * a_panel_elems, (uint32_t)rows * (uint32_t)lda * 8u, &full[s]);
+    }
+  };
+  if (warp == 0)
+    for (int pi = 0; pi < kStages - 1 && pi < npanel; ++pi) issue(pi);
+
+  // warp tile
+  const int n_mtiles = (mc + 7) / 8;
+  const int mt0 = warp_m * MT;
+  const int nmt = max(0, min(MT, n_mtiles - mt0));
+  const int nt0 = warp_n * 2;
+  const int nnt = max(0, min(2, ncols / 8 - nt0));
+  double acc[MT][2][2];
+#pragma unroll
+  for (int i = 0; i < MT; ++i)
+#pragma unroll
+    for (int j = 0; j < 2; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+  const int fk = lane & 3, fm = lane >> 2;
+  for (int pi = 0; pi < npanel; ++pi) {
+    const int s = pi % kStages;
+    mbar_wait(&full[s], (uint32_t)((pi / kStages) & 1));
+    __syncthreads();   // every warp is done with panel pi-1: its ring slot may be refilled
+    if (warp == 0 && pi + kStages - 1 < npanel) issue(pi + kStages - 1);
+    if (nnt == 0 || nmt == 0) continue;
+    const double* As = stage0 + s * stage_elems;
+    const double* Xs = As + a_panel_elems;
+    const int ksteps = min(kPanelK, kt - pi * kPanelK) / 4;
+    const double* Ap = As + fk * lda + mt0 * 8 + fm;
+    const double* Xp = Xs + fk * kLdXs + nt0 * 8 + fm;
+    for (int ks = 0; ks < ksteps; ++ks) {
+      double b0 = Xp[0], b1 = (nnt > 1) ? Xp[8] : 0.0;
+#pragma unroll
+      for (int i = 0; i < MT; ++i) {
+        if (i < nmt) {
+          double av = Ap[i * 8];
+          dmma884(acc[i][0][0], acc[i][0][1], av, b0);
+          dmma884(acc[i][1][0], acc[i][1][1], av, b1);
+        }
+      }
+      Ap += 4 * lda;
+      Xp += 4 * kLdXs;
+    }
+  }
+
+  // epilogue: assembly + recurrence (steps 4-5).  C fragment: row = lane/4, columns 2*(lane%4) + {0,1}
+  const double alpha = a.alpha, beta = a.beta, ac = a.ac;
+#pragma unroll
+  for (int i = 0; i < MT; ++i) {
+    if (i >= nmt) continue;
+    const int r = (mt0 + i) * 8 + fm;
+    if (r >= mc) continue;
+    const int idx = idx_s[r];
+    const int64_t g = idx & 0x7fffffff;
+#pragma unroll
+    for (int j = 0; j < 2; ++j) {
+      if (j >= nnt) continue;
+      const int col = col0 + (nt0 + j) * 8 + fk * 2;
+      double2* tp = reinterpret_cast<double2*>(a.Tg + g * a.ldt + col);
+      double v0 = alpha * acc[i][j][0], v1 = alpha * acc[i][j][1];
+      if (a.atomic) {
+        atomicAdd(&tp->x, v0);
+        atomicAdd(&tp->y, v1);
+      } else if (idx < 0) {
+        if (ac != 0.0) {
+          double2 x = *reinterpret_cast<const double2*>(a.X + g * a.ldx + col);
+          v0 -= ac * x.x; v1 -= ac * x.y;
+        }
+        if (beta != 0.0) {
+          double2 t = *tp;
+          v0 -= beta * t.x; v1 -= beta * t.y;
+        }
+        *tp = make_double2(v0, v1);
+      } else {
+        double2 t = *tp;
+        *tp = make_double2(t.x + v0, t.y + v1);
+      }
+    }
+  }
+}
+
+template <typename T>
+cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
+  const int B = (int)g.B;
+  T* P = reinterpret_cast<T*>(g.P);
+  T* Pc = reinterpret_cast<T*>(g.Pc);
+  const T* X = reinterpret_cast<const T*>(g.X);
+  T* Tg = reinterpret_cast<T*>(g.T);
+  const T* mat = reinterpret_cast<const T*>(op->mat);
+  // steps 3a-3c
+  if (op->n_proj > 0) {
+    dim3 g1((unsigned)op->n_pc_cells, (unsigned)((B + 127) / 128));
+    k_proj_partial<T><<<g1, 128, op->m_cell * sizeof(int32_t), st>>>(mat, op->mat_off, op->idx_off, op->gidx, op->pc_cells,
+                                                                    op->cell_proj_ptr, op->m_cell, op->lda, X, g.ldx, Pc, B);
+    op->launches++;
+  }
+  {
+    dim3 g2((unsigned)(op->n_proj + 1), (unsigned)((B + 127) / 128));
+    k_proj_reduce<T><<<g2, 128, 0, st>>>(Pc, op->proj_ptr, op->proj_pcrow, op->D, op->n_proj, P, B);
+    op->launches++;
+  }
+  ApplyDev<T> a;
+  a.mat = mat; a.mat_off = op->mat_off; a.idx_off = op->idx_off; a.ktot = op->ktot; a.gidx = op->gidx;
+  a.m_cell = op->m_cell; a.lda = op->lda;
+  a.X = X; a.ldx = g.ldx; a.Tg = Tg; a.ldt = g.ldt; a.P = P; a.ldp = B; a.B = B;
+  a.alpha = (T)g.alpha; a.beta = (T)g.beta; a.ac = (T)(g.alpha * g.cshift);
+  a.atomic = op->assembly;
+
+  bool fast = false;
+  int MT = 0;
+  if (sizeof(T) == 8 && op->variant == 0 && B % 8 == 0 && g.ldx % 2 == 0 && g.ldt % 2 == 0 &&
+      ((uintptr_t)g.X % 16 == 0) && ((uintptr_t)g.T % 16 == 0) && ((uintptr_t)g.P % 16 == 0) && op->max_ktot <= kMaxKtot) {
+    int n_mtiles = (op->m_cell + 7) / 8;
+    MT = (n_mtiles + 3) / 4;
+    fast = (MT == 11 || MT == 4 || MT == 2 || MT == 7);
+  }
+  size_t smem_fast = (size_t)kStages * (kPanelK * op->lda + kPanelK * kLdXs) * sizeof(double) + kStages * sizeof(uint64_t) +
+                     (size_t)op->max_ktot * sizeof(int32_t);
+  if (fast && smem_fast > 227 * 1024) fast = false;
+
+  if (op->assembly == 1) {
+    k_prefill<T><<<148 * 8, 256, 0, st>>>(X, g.ldx, Tg, g.ldt, op->n_dofs, B, a.ac, a.beta);
+    op->launches++;
+  }
+  const int n_launch = op->assembly == 1 ? 1 : op->n_colors;
+  for (int c = 0; c < n_launch; ++c) {
+    if (op->assembly == 1) { a.cells = op->all_cells; a.n_launch_cells = (int)op->n_cells; }
+    else { a.cells = op->color_cells + op->color_ptr[c]; a.n_launch_cells = op->color_ptr[c + 1] - op->color_ptr[c]; }
+    if (a.n_launch_cells == 0) continue;
+    if (fast) {
+      if constexpr (sizeof(T) == 8) {
+        a.n_col_tiles = (B + kTileN - 1) / kTileN;
+        unsigned grid = (unsigned)a.n_launch_cells * (unsigned)a.n_col_tiles;
+        ApplyDev<double> ad = *reinterpret_cast<ApplyDev<double>*>(&a);
+        switch (MT) {
+          case 11: k_apply_dmma<11><<<grid, 512, smem_fast, st>>>(ad); break;
+          case 7: k_apply_dmma<7><<<grid, 512, smem_fast, st>>>(ad); break;
+          case 4: k_apply_dmma<4><<<grid, 512, smem_fast, st>>>(ad); break;
+          case 2: k_apply_dmma<2><<<grid, 512, smem_fast, st>>>(ad); break;
+        }
+      }
+    } else {
+      a.n_col_tiles = (B + 31) / 32;
+      unsigned grid = (unsigned)a.n_launch_cells * (unsigned)a.n_col_tiles;
+      k_apply_generic<T><<<grid, 256, (size_t)op->max_ktot * 32 * sizeof(T), st>>>(a);
+    }
+    op->launches++;
+  }
+  return cudaGetLastError();
+}
+
+}  // namespace
+
+cudaError_t init_apply_kernels(Op* op) {
+  cudaError_t e;
+  size_t smem_fast = (size_t)kStages * (kPanelK * op->lda + kPanelK * kLdXs) * sizeof(double) + kStages * sizeof(uint64_t) +
+                     (size_t)op->max_ktot * sizeof(int32_t);
+  if (smem_fast <= 227 * 1024) {
+    if ((e = cudaFuncSetAttribute(k_apply_dmma<11>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_fast))) return e;
+    if ((e = cudaFuncSetAttribute(k_apply_dmma<7>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_fast))) return e;
+    if ((e = cudaFuncSetAttribute(k_apply_dmma<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_fast))) return e;
+    if ((e = cudaFuncSetAttribute(k_apply_dmma<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_fast))) return e;
+  }
+  size_t smem_gen = (size_t)op->max_ktot * 32 * 8;
+  if (smem_gen > 227 * 1024) return cudaErrorInvalidValue;
+  if ((e = cudaFuncSetAttribute(k_apply_generic<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_gen))) return e;
+  if ((e = cudaFuncSetAttribute(k_apply_generic<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_gen))) return e;
+  return cudaSuccess;
+}
+
+cudaError_t launch_apply(Op* op, const ApplyArgs& a, cudaStream_t stream) {
+  return op->precision == 64 ? launch_apply_t<double>(op, a, stream) : launch_apply_t<float>(op, a, stream);
+}
+
+}  // namespace chfsi

@@ -1,0 +1,110 @@
+// Internal declarations shared by the translation units of libchfsi (not part of the ABI).
+//
+// Device data layout:
+//   mat   [cell c]  : K_c rows x LDA columns, element type T (double | float), row k = CONTRACTION index,
+//                     column m = OUTPUT node.  Rows 0..M_cell-1 hold the Loewdin-scaled cell Hamiltonian
+//                     s_k H^e_km s_m (symmetric, "H~^{loc,c_i}"); rows M_cell..M_cell+N_psp^c-1
+//                     hold s_m C^c_{m,j} for the projectors j touching the cell; remaining
+//                     rows/columns are zero padding.  K_c is a multiple of 8, LDA = round8(M_cell) + 4 so that
+//                     FP64 mma fragments read shared memory without bank conflicts (LDA mod 16 in {4, 12}).
+//   gidx  [cell c]  : K_c int32.  k < M_cell: global dof of local node k, bit 31 set when this (cell, node) is
+//                     the FIRST contribution to that dof in colour order (it then carries the recurrence
+//                     terms); k >= M_cell: row of the projector-coefficient block P (padding rows point at
+//                     the all-zero row n_proj).
+//   X, Y  blocks    : [n_dofs][ld], vector index fastest.
+//   P               : [n_proj + 1][B]   (Alg. 4 steps 3-4: assembled and D-scaled projector coefficients)
+//   Pc              : [nnz_cell_proj][B] (Alg. 4 step 2: per-cell partial coefficients C^cT X^c)
+#pragma once
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include <cuda_runtime.h>
+
+#include "../../include/chfsi.h"
+
+namespace chfsi {
+
+constexpr uint32_t kFirstBit = 0x80000000u;
+
+// ---- host-side tables and mesh analysis (host_setup.cpp) -------------------------------------------------
+struct Tables1D {
+  int p = 0, n1 = 0, nq1 = 0;
+  std::vector<double> gll_x, gll_w;   // [n1]
+  std::vector<double> gq_x, gq_w;     // [nq1]
+  std::vector<double> phi, dphi;      // [nq1][n1]  Lagrange (GLL) basis and derivative at the Gauss points
+};
+void build_tables(int p, Tables1D* t);
+
+struct HostPlan {
+  // colouring
+  int n_colors = 0;
+  std::vector<int32_t> color_cells;      // cells sorted by colour
+  std::vector<int32_t> color_ptr;        // [n_colors+1]
+  // cell-centric projector lists
+  std::vector<int64_t> cell_proj_ptr;    // [n_cells+1]
+  std::vector<int32_t> cell_proj_idx;    // [nnz] projector id
+  std::vector<int64_t> cell_proj_src;    // [nnz] index k into the caller's (projector,cell) CSR (chi_q row)
+  // per-cell layout
+  std::vector<int32_t> ktot;             // [n_cells]
+  std::vector<int64_t> mat_off;          // [n_cells+1] element offsets into mat
+  std::vector<int64_t> idx_off;          // [n_cells+1] offsets into gidx
+  std::vector<int32_t> gidx;
+  // projector-centric reduction lists (Alg. 4 step 3)
+  std::vector<int64_t> proj_ptr;         // [n_proj+1]
+  std::vector<int64_t> proj_pcrow;       // [nnz] row of Pc
+  std::vector<int32_t> pc_cells;         // cells that have projectors
+  std::vector<double> mass;              // [n_dofs] diagonal GLL mass
+};
+// Returns "" on success, else an error message (bad mesh).
+std::string analyse_mesh(const chfsi_mesh& mesh, const chfsi_nonlocal* nl, const Tables1D& tab, int lda,
+                         HostPlan* plan);
+
+// ---- device operator ----------------------------------------------------------------------------------------
+struct Op {
+  int p = 0, n1 = 0, nq1 = 0, m_cell = 0, n_q = 0, mpad = 0, lda = 0;
+  int precision = 64, assembly = 0, variant = 0;
+  int64_t n_cells = 0, n_dofs = 0, n_proj = 0, nnz_cp = 0, n_pc_cells = 0;
+  int n_colors = 0;
+  std::vector<int32_t> color_ptr;        // host copy
+  int max_ktot = 0;
+  int64_t mat_elems = 0;
+  // device arrays
+  void* mat = nullptr;                   // T
+  int64_t* mat_off = nullptr;
+  int64_t* idx_off = nullptr;
+  int32_t* ktot = nullptr;
+  int32_t* gidx = nullptr;
+  int32_t* color_cells = nullptr;
+  int32_t* all_cells = nullptr;          // 0..n_cells-1 (atomic mode launches every cell at once)
+  int32_t* pc_cells = nullptr;
+  int64_t* cell_proj_ptr = nullptr;      // [n_cells+1]  (row offsets into Pc)
+  int64_t* proj_ptr = nullptr;
+  int64_t* proj_pcrow = nullptr;
+  double* D = nullptr;
+  double* mass = nullptr;
+  int64_t launches = 0;
+  std::string err;
+};
+
+// ---- setup kernels (setup_kernels.cu) ------------------------------------------------------------------------
+// Fills op->mat (element type per op->precision) from the mesh geometry, V_eff and projector samples.
+// All pointer arguments are HOST pointers except op's device arrays.  Returns cudaSuccess or the failing code;
+// *bad_jacobian is set when some quadrature point has det J <= 0.
+cudaError_t build_cell_matrices(Op* op, const HostPlan& plan, const Tables1D& tab, const chfsi_mesh& mesh,
+                                const chfsi_potential& pot, const chfsi_nonlocal* nl, cudaStream_t stream,
+                                bool* bad_jacobian);
+
+// ---- apply kernels (apply_kernels.cu) ----------------------------------------------------------------------
+struct ApplyArgs {
+  const void* X = nullptr;  int64_t ldx = 0;     // input block Y_{k-1}
+  void* T = nullptr;        int64_t ldt = 0;     // target block: holds Y_{k-2} on entry, Y_k on exit
+  int64_t B = 0;
+  double alpha = 1.0, beta = 0.0, cshift = 0.0;  // Y_k = alpha (H~ X - cshift X) - beta T
+  void* P = nullptr;                             // [n_proj+1][B]
+  void* Pc = nullptr;                            // [nnz_cp][B]
+};
+// Enqueues one fused H~ application + recurrence update.  Returns cudaGetLastError().
+cudaError_t launch_apply(Op* op, const ApplyArgs& a, cudaStream_t stream);
+
+}  // namespace chfsi
