@@ -1,0 +1,265 @@
+"""ctypes binding of libchfsi (include/chfsi.h).  Argument marshalling only.
+
+`Operator` mirrors the C entry points one to one:
+    chfsi_create / chfsi_destroy / chfsi_get_info / chfsi_workspace_bytes / chfsi_mass_diag /
+    chfsi_apply_H / chfsi_chebyshev_filter / chfsi_chebyshev_filter_chunked / chfsi_chebyshev_filter_host /
+    chfsi_launch_count / chfsi_set_kernel_variant / chfsi_last_error
+Vector blocks are torch CUDA tensors of shape [n_dofs, ld] (row-major, vector index fastest);
+a chunk of columns is passed as a column slice `X[:, j0:j0+B]` (stride(0) = ld, stride(1) = 1).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libchfsi.so")
+
+EXPORTED_SYMBOLS = [
+    "chfsi_create", "chfsi_destroy", "chfsi_get_info", "chfsi_workspace_bytes", "chfsi_mass_diag",
+    "chfsi_apply_H", "chfsi_chebyshev_filter", "chfsi_chebyshev_filter_chunked", "chfsi_chebyshev_filter_host",
+    "chfsi_launch_count", "chfsi_set_kernel_variant", "chfsi_last_error",
+]
+
+
+class ChfsiError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"libchfsi error {code}: {msg}")
+        self.code = code
+
+
+class _Mesh(C.Structure):
+    _fields_ = [("p", C.c_int32), ("n_cells", C.c_int64), ("n_dofs", C.c_int64),
+                ("cell_dofs", C.c_void_p), ("cell_vertices", C.c_void_p)]
+
+
+class _Potential(C.Structure):
+    _fields_ = [("veff_q", C.c_void_p)]
+
+
+class _Nonlocal(C.Structure):
+    _fields_ = [("n_proj", C.c_int64), ("D", C.c_void_p), ("proj_cell_ptr", C.c_void_p),
+                ("proj_cell_idx", C.c_void_p), ("chi_q", C.c_void_p)]
+
+
+class _Info(C.Structure):
+    _fields_ = [("p", C.c_int32), ("m_cell", C.c_int32), ("n_q", C.c_int32), ("precision", C.c_int32),
+                ("assembly", C.c_int32), ("n_colors", C.c_int32),
+                ("n_cells", C.c_int64), ("n_dofs", C.c_int64), ("n_proj", C.c_int64),
+                ("nnz_cell_proj", C.c_int64), ("cells_with_proj", C.c_int64),
+                ("flops_per_vector_apply", C.c_double), ("matrix_bytes", C.c_int64)]
+
+
+_lib = None
+
+
+def load_library(build_if_missing: bool = True):
+    """dlopen libchfsi.so (building it in-tree with nvcc first if it is missing or stale)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if build_if_missing:
+        from .build import build
+        build()
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_2203_07820_b200.build` "
+                           "(there is no CPU fallback)")
+    lib_ = C.CDLL(LIB_PATH)
+    vp, i64, i32, dbl = C.c_void_p, C.c_int64, C.c_int32, C.c_double
+    lib_.chfsi_create.argtypes = [C.POINTER(vp), C.POINTER(_Mesh), C.POINTER(_Potential), C.POINTER(_Nonlocal),
+                                  C.c_int, C.c_int, vp]
+    lib_.chfsi_create.restype = C.c_int
+    lib_.chfsi_destroy.argtypes = [vp]
+    lib_.chfsi_destroy.restype = C.c_int
+    lib_.chfsi_get_info.argtypes = [vp, C.POINTER(_Info)]
+    lib_.chfsi_get_info.restype = C.c_int
+    lib_.chfsi_workspace_bytes.argtypes = [vp, i64, C.POINTER(C.c_size_t)]
+    lib_.chfsi_workspace_bytes.restype = C.c_int
+    lib_.chfsi_mass_diag.argtypes = [vp, vp, vp]
+    lib_.chfsi_mass_diag.restype = C.c_int
+    lib_.chfsi_apply_H.argtypes = [vp, vp, i64, vp, i64, i64, vp, vp]
+    lib_.chfsi_apply_H.restype = C.c_int
+    lib_.chfsi_chebyshev_filter.argtypes = [vp, vp, i64, i64, i32, dbl, dbl, dbl, vp, vp]
+    lib_.chfsi_chebyshev_filter.restype = C.c_int
+    lib_.chfsi_chebyshev_filter_chunked.argtypes = [vp, vp, i64, i64, i64, i32, dbl, dbl, dbl, vp, vp]
+    lib_.chfsi_chebyshev_filter_chunked.restype = C.c_int
+    lib_.chfsi_chebyshev_filter_host.argtypes = [vp, vp, i64, i64, i64, i32, dbl, dbl, dbl]
+    lib_.chfsi_chebyshev_filter_host.restype = C.c_int
+    lib_.chfsi_launch_count.argtypes = [vp]
+    lib_.chfsi_launch_count.restype = i64
+    lib_.chfsi_set_kernel_variant.argtypes = [vp, C.c_int]
+    lib_.chfsi_set_kernel_variant.restype = C.c_int
+    lib_.chfsi_last_error.argtypes = [vp]
+    lib_.chfsi_last_error.restype = C.c_char_p
+    _lib = lib_
+    return _lib
+
+
+def lib():
+    return load_library()
+
+
+def _np_ptr(a: np.ndarray) -> int:
+    return a.ctypes.data
+
+
+def _stream_ptr(stream) -> Optional[int]:
+    import torch
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return C.c_void_p(s.cuda_stream)
+
+
+class Operator:
+    """Owns one `chfsi_op` handle.  Inputs are host NumPy arrays (copied by the library during the call)."""
+
+    def __init__(self, p, cell_dofs, cell_vertices, n_dofs, veff_q, n_proj=0, D=None, proj_cell_ptr=None,
+                 proj_cell_idx=None, chi_q=None, precision=64, assembly=0, stream=None):
+        self._h = None
+        L = load_library()
+        import torch
+        if not torch.cuda.is_available():
+            raise ChfsiError(-4, "no CUDA device: libchfsi has no CPU fallback")
+        cell_dofs = np.ascontiguousarray(cell_dofs, dtype=np.int32)
+        cell_vertices = np.ascontiguousarray(cell_vertices, dtype=np.float64)
+        veff_q = np.ascontiguousarray(veff_q, dtype=np.float64)
+        mesh = _Mesh(int(p), int(cell_dofs.shape[0]), int(n_dofs), _np_ptr(cell_dofs), _np_ptr(cell_vertices))
+        pot = _Potential(_np_ptr(veff_q))
+        keep = [cell_dofs, cell_vertices, veff_q]
+        nlp = None
+        if n_proj:
+            D = np.ascontiguousarray(D, dtype=np.float64)
+            ptr = np.ascontiguousarray(proj_cell_ptr, dtype=np.int64)
+            idx = np.ascontiguousarray(proj_cell_idx, dtype=np.int32)
+            chi = np.ascontiguousarray(chi_q, dtype=np.float64)
+            keep += [D, ptr, idx, chi]
+            nlp = C.pointer(_Nonlocal(int(n_proj), _np_ptr(D), _np_ptr(ptr), _np_ptr(idx), _np_ptr(chi)))
+        h = C.c_void_p()
+        rc = L.chfsi_create(C.byref(h), C.byref(mesh), C.byref(pot), nlp, int(precision), int(assembly),
+                            _stream_ptr(stream))
+        if rc != 0:
+            raise ChfsiError(rc, (L.chfsi_last_error(None) or b"").decode())
+        self._h = h
+        self.precision = int(precision)
+        info = _Info()
+        self._check(L.chfsi_get_info(self._h, C.byref(info)))
+        self.info = {k: getattr(info, k) for k, _ in _Info._fields_}
+        self.n_dofs = int(info.n_dofs)
+        self._ws = None
+        self._ws_B = 0
+
+    @classmethod
+    def from_workload(cls, wl, precision=64, assembly=0, stream=None):
+        return cls(wl.p, wl.cell_dofs, wl.cell_vertices, wl.n_dofs, wl.veff_q, wl.n_proj, wl.D, wl.proj_cell_ptr,
+                   wl.proj_cell_idx, wl.chi_q, precision=precision, assembly=assembly, stream=stream)
+
+    # -- helpers ------------------------------------------------------------------------------------------
+    def _check(self, rc: int):
+        if rc != 0:
+            raise ChfsiError(rc, (load_library().chfsi_last_error(self._h) or b"").decode())
+
+    @property
+    def dtype(self):
+        import torch
+        return torch.float64 if self.precision == 64 else torch.float32
+
+    def _block(self, X, name):
+        import torch
+        if not (isinstance(X, torch.Tensor) and X.is_cuda and X.dim() == 2):
+            raise TypeError(f"{name}: expected a 2-D CUDA tensor [n_dofs, B]")
+        if X.dtype != self.dtype:
+            raise TypeError(f"{name}: dtype {X.dtype} does not match operator precision {self.precision}")
+        if X.shape[0] != self.n_dofs or X.stride(1) != 1 or X.stride(0) < X.shape[1]:
+            raise ValueError(f"{name}: need shape [n_dofs, B] with the vector index fastest")
+        return C.c_void_p(X.data_ptr()), int(X.stride(0)), int(X.shape[1])
+
+    def workspace_bytes(self, B: int) -> int:
+        n = C.c_size_t()
+        self._check(load_library().chfsi_workspace_bytes(self._h, int(B), C.byref(n)))
+        return int(n.value)
+
+    def workspace(self, B: int):
+        """A cached torch-allocated device workspace for blocks of B columns."""
+        import torch
+        if self._ws is None or self._ws_B != B:
+            self._ws = None
+            self._ws = torch.empty(self.workspace_bytes(B), dtype=torch.uint8, device="cuda")
+            self._ws_B = B
+        return self._ws
+
+    # -- the ABI calls ------------------------------------------------------------------------------------
+    def mass_diag(self, stream=None):
+        import torch
+        M = torch.empty(self.n_dofs, dtype=torch.float64, device="cuda")
+        self._check(load_library().chfsi_mass_diag(self._h, C.c_void_p(M.data_ptr()), _stream_ptr(stream)))
+        return M
+
+    def apply_H(self, X, Y=None, workspace=None, stream=None):
+        import torch
+        xp, ldx, B = self._block(X, "X")
+        if Y is None:
+            Y = torch.empty((self.n_dofs, B), dtype=self.dtype, device="cuda")
+        yp, ldy, By = self._block(Y, "Y")
+        if By != B:
+            raise ValueError("X and Y must have the same number of columns")
+        ws = workspace if workspace is not None else self.workspace(B)
+        self._check(load_library().chfsi_apply_H(self._h, xp, ldx, yp, ldy, B, C.c_void_p(ws.data_ptr()),
+                                                 _stream_ptr(stream)))
+        return Y
+
+    def chebyshev_filter(self, X, m, a, b, a0, workspace=None, stream=None):
+        """In place on the columns of X."""
+        xp, ldx, B = self._block(X, "X")
+        ws = workspace if workspace is not None else self.workspace(B)
+        self._check(load_library().chfsi_chebyshev_filter(self._h, xp, ldx, B, int(m), float(a), float(b),
+                                                          float(a0), C.c_void_p(ws.data_ptr()),
+                                                          _stream_ptr(stream)))
+        return X
+
+    def chebyshev_filter_chunked(self, X, B, m, a, b, a0, workspace=None, stream=None):
+        """In place on all N columns of X, filtered in sequential chunks of B columns."""
+        xp, ldx, N = self._block(X, "X")
+        B = min(int(B), N)
+        ws = workspace if workspace is not None else self.workspace(B)
+        self._check(load_library().chfsi_chebyshev_filter_chunked(self._h, xp, ldx, N, B, int(m), float(a),
+                                                                  float(b), float(a0),
+                                                                  C.c_void_p(ws.data_ptr()), _stream_ptr(stream)))
+        return X
+
+    def chebyshev_filter_host(self, X_host, B, m, a, b, a0):
+        """End-to-end variant on a HOST block (NumPy array or CPU torch tensor, ideally pinned), in place."""
+        import torch
+        if isinstance(X_host, torch.Tensor):
+            if X_host.is_cuda or X_host.dim() != 2 or X_host.stride(1) != 1 or X_host.dtype != self.dtype:
+                raise TypeError("X_host: expected a 2-D CPU tensor of the operator's precision, vector index fastest")
+            ptr, ld, N, rows = X_host.data_ptr(), X_host.stride(0), X_host.shape[1], X_host.shape[0]
+        else:
+            want = np.float64 if self.precision == 64 else np.float32
+            if X_host.dtype != want or X_host.ndim != 2 or X_host.strides[1] != X_host.itemsize:
+                raise TypeError("X_host: expected a 2-D array of the operator's precision, vector index fastest")
+            ptr, ld, N, rows = X_host.ctypes.data, X_host.strides[0] // X_host.itemsize, X_host.shape[1], X_host.shape[0]
+        if rows != self.n_dofs:
+            raise ValueError("X_host: wrong number of rows")
+        self._check(load_library().chfsi_chebyshev_filter_host(self._h, C.c_void_p(ptr), int(ld), int(N), int(B),
+                                                               int(m), float(a), float(b), float(a0)))
+        return X_host
+
+    def launch_count(self) -> int:
+        return int(load_library().chfsi_launch_count(self._h))
+
+    def set_kernel_variant(self, variant: int):
+        self._check(load_library().chfsi_set_kernel_variant(self._h, int(variant)))
+
+    def close(self):
+        if self._h is not None and _lib is not None:
+            _lib.chfsi_destroy(self._h)
+        self._h = None
+        self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

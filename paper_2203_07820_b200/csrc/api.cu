@@ -1,0 +1,348 @@
+// C ABI of libchfsi (include/chfsi.h): argument checking, operator construction, the Chebyshev host loop.
+//
+// The filter loop (Eq. 37, scaled form of ref. [86]) only computes the FP64 scalars
+// sigma_k on the host and enqueues one fused "H~ apply + recurrence" launch sequence per degree on the caller's
+// stream; it never synchronises.  Two blocks ping-pong: the caller's X and one workspace block W
+//     k = 1 :  W <- (sigma_1/e)(H~ X - c X)
+//     k = 2 :  X <- (2 sigma_2/e)(H~ W - c W) - sigma_1 sigma_2 X        (target holds Y_{k-2}, becomes Y_k)
+//     ...
+// and for odd m the result is copied from W back to X.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "common.h"
+
+using namespace chfsi;
+
+struct chfsi_op : public Op {};
+
+namespace {
+
+thread_local std::string g_create_error;
+
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+int fail(chfsi_op* op, int code, const std::string& msg) {
+  if (op) op->err = msg; else g_create_error = msg;
+  return code;
+}
+int cuda_fail(chfsi_op* op, cudaError_t e, const char* where) {
+  return fail(op, e == cudaErrorMemoryAllocation ? CHFSI_ERR_OUT_OF_MEMORY : CHFSI_ERR_CUDA,
+              std::string(where) + ": " + cudaGetErrorString(e));
+}
+
+template <typename U>
+cudaError_t upload_vec(U** dst, const std::vector<U>& v, cudaStream_t st) {
+  *dst = nullptr;
+  size_t n = v.empty() ? 1 : v.size();
+  cudaError_t e = cudaMalloc((void**)dst, n * sizeof(U));
+  if (e != cudaSuccess) return e;
+  if (!v.empty()) e = cudaMemcpyAsync(*dst, v.data(), v.size() * sizeof(U), cudaMemcpyHostToDevice, st);
+  return e;
+}
+
+void free_op(chfsi_op* op) {
+  if (!op) return;
+  cudaFree(op->mat); cudaFree(op->mat_off); cudaFree(op->idx_off); cudaFree(op->ktot); cudaFree(op->gidx);
+  cudaFree(op->color_cells); cudaFree(op->all_cells); cudaFree(op->pc_cells); cudaFree(op->cell_proj_ptr);
+  cudaFree(op->proj_ptr); cudaFree(op->proj_pcrow); cudaFree(op->D); cudaFree(op->mass);
+  delete op;
+}
+
+struct WsLayout {
+  size_t elt, block_off, p_off, pc_off, total;
+  int64_t ldw;
+};
+WsLayout ws_layout(const Op* op, int64_t B) {
+  WsLayout w;
+  w.elt = op->precision == 64 ? 8 : 4;
+  w.ldw = (B + 7) / 8 * 8;                                  // rows of the workspace block stay 32/64-byte aligned
+  w.block_off = 0;
+  w.p_off = align_up((size_t)op->n_dofs * w.ldw * w.elt, 256);
+  w.pc_off = w.p_off + align_up((size_t)(op->n_proj + 1) * B * w.elt, 256);
+  w.total = w.pc_off + align_up((size_t)(op->nnz_cp > 0 ? op->nnz_cp : 1) * B * w.elt, 256);
+  return w;
+}
+
+int check_block_args(chfsi_op* op, const void* X, int64_t ldx, int64_t B, const void* ws) {
+  if (!op) return CHFSI_ERR_BAD_ARGUMENT;
+  if (!X) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "NULL vector block");
+  if (B < 1) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "B < 1");
+  if (B > (1 << 20)) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "B too large");
+  if (ldx < B) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "ld < B");
+  if (!ws) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "NULL workspace");
+  if ((uintptr_t)ws % 16 != 0) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "workspace must be 16-byte aligned");
+  return CHFSI_OK;
+}
+
+int filter_block(chfsi_op* op, void* X, int64_t ldx, int64_t B, int32_t m, double a, double b, double a0,
+                 void* ws, cudaStream_t st) {
+  const WsLayout w = ws_layout(op, B);
+  char* base = reinterpret_cast<char*>(ws);
+  void* W = base + w.block_off;
+  ApplyArgs g;
+  g.B = B; g.P = base + w.p_off; g.Pc = base + w.pc_off;
+  const double e = 0.5 * (b - a), c = 0.5 * (b + a);
+  const double sigma1 = e / (a0 - c);
+  double sigma = sigma1;
+  void* cur = X; int64_t ldcur = ldx;      // Y_{k-1}
+  void* tgt = W; int64_t ldtgt = w.ldw;    // Y_{k-2} -> Y_k
+  for (int k = 1; k <= m; ++k) {
+    g.X = cur; g.ldx = ldcur; g.T = tgt; g.ldt = ldtgt; g.cshift = c;
+    if (k == 1) { g.alpha = sigma1 / e; g.beta = 0.0; }
+    else {
+      const double sigma_new = 1.0 / (2.0 / sigma1 - sigma);
+      g.alpha = 2.0 * sigma_new / e; g.beta = sigma * sigma_new; sigma = sigma_new;
+    }
+    cudaError_t ce = launch_apply(op, g, st);
+    if (ce != cudaSuccess) return cuda_fail(op, ce, "chebyshev_filter launch");
+    std::swap(cur, tgt); std::swap(ldcur, ldtgt);
+  }
+  if (cur != X) {   // odd m: result sits in the workspace block
+    cudaError_t ce = cudaMemcpy2DAsync(X, (size_t)ldx * w.elt, W, (size_t)w.ldw * w.elt, (size_t)B * w.elt,
+                                       (size_t)op->n_dofs, cudaMemcpyDeviceToDevice, st);
+    if (ce != cudaSuccess) return cuda_fail(op, ce, "chebyshev_filter copy-back");
+    op->launches++;
+  }
+  return CHFSI_OK;
+}
+
+int check_filter_scalars(chfsi_op* op, int32_t m, double a, double b, double a0) {
+  if (m < 1) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "m < 1");
+  if (!(a0 <= a && a < b) || !std::isfinite(a0) || !std::isfinite(b))
+    return fail(op, CHFSI_ERR_BAD_ARGUMENT, "need finite a0 <= a < b");
+  return CHFSI_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int chfsi_create(chfsi_op** out, const chfsi_mesh* mesh, const chfsi_potential* pot, const chfsi_nonlocal* nl,
+                 int precision, int assembly, void* cuda_stream) {
+  if (!out) return fail(nullptr, CHFSI_ERR_BAD_ARGUMENT, "out == NULL");
+  *out = nullptr;
+  if (!mesh || !pot || !mesh->cell_dofs || !mesh->cell_vertices || !pot->veff_q)
+    return fail(nullptr, CHFSI_ERR_BAD_ARGUMENT, "NULL mesh / potential pointer");
+  if (mesh->p < 1 || mesh->p > 8) return fail(nullptr, CHFSI_ERR_UNSUPPORTED, "FE degree p must be in 1..8");
+  if (precision != 64 && precision != 32) return fail(nullptr, CHFSI_ERR_UNSUPPORTED, "precision must be 64 or 32");
+  if (assembly != 0 && assembly != 1) return fail(nullptr, CHFSI_ERR_BAD_ARGUMENT, "assembly must be 0 or 1");
+  if (mesh->n_cells < 1 || mesh->n_dofs < 1 || mesh->n_cells > INT32_MAX / 2 || mesh->n_dofs > INT32_MAX / 2)
+    return fail(nullptr, CHFSI_ERR_BAD_ARGUMENT, "n_cells / n_dofs out of range");
+  const bool has_nl = nl && nl->n_proj > 0;
+  if (has_nl && (!nl->D || !nl->proj_cell_ptr || !nl->proj_cell_idx || !nl->chi_q))
+    return fail(nullptr, CHFSI_ERR_BAD_ARGUMENT, "NULL projector pointer");
+
+  int ndev = 0;
+  cudaError_t ce = cudaGetDeviceCount(&ndev);
+  if (ce != cudaSuccess || ndev == 0)
+    return fail(nullptr, CHFSI_ERR_CUDA, std::string("no CUDA device (there is no CPU fallback): ") +
+                                             (ce != cudaSuccess ? cudaGetErrorString(ce) : "device count 0"));
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+
+  chfsi_op* op = new (std::nothrow) chfsi_op();
+  if (!op) return fail(nullptr, CHFSI_ERR_OUT_OF_MEMORY, "host allocation failed");
+  op->p = mesh->p; op->n1 = mesh->p + 1; op->nq1 = mesh->p + 2;
+  op->m_cell = op->n1 * op->n1 * op->n1; op->n_q = op->nq1 * op->nq1 * op->nq1;
+  op->mpad = (op->m_cell + 7) / 8 * 8; op->lda = op->mpad + 4;
+  op->precision = precision; op->assembly = assembly;
+  op->n_cells = mesh->n_cells; op->n_dofs = mesh->n_dofs; op->n_proj = has_nl ? nl->n_proj : 0;
+
+  Tables1D tab;
+  build_tables(op->p, &tab);
+  HostPlan plan;
+  std::string msg;
+  try {
+    msg = analyse_mesh(*mesh, has_nl ? nl : nullptr, tab, op->lda, &plan);
+  } catch (const std::bad_alloc&) {
+    delete op;
+    return fail(nullptr, CHFSI_ERR_OUT_OF_MEMORY, "host allocation failed in mesh analysis");
+  }
+  if (!msg.empty()) { delete op; return fail(nullptr, CHFSI_ERR_BAD_MESH, msg); }
+
+  op->n_colors = plan.n_colors; op->color_ptr = plan.color_ptr;
+  op->nnz_cp = (int64_t)plan.cell_proj_idx.size();
+  op->n_pc_cells = (int64_t)plan.pc_cells.size();
+  op->max_ktot = 0;
+  for (int32_t k : plan.ktot) op->max_ktot = std::max(op->max_ktot, (int)k);
+  op->mat_elems = plan.mat_off[op->n_cells];
+
+#define CKC(x, what) do { ce = (x); if (ce != cudaSuccess) { int rc_ = cuda_fail(nullptr, ce, what); free_op(op); return rc_; } } while (0)
+  const size_t elt = precision == 64 ? 8 : 4;
+  CKC(cudaMalloc(&op->mat, (size_t)op->mat_elems * elt), "cudaMalloc(cell matrices)");
+  CKC(upload_vec(&op->mat_off, plan.mat_off, st), "upload");
+  CKC(upload_vec(&op->idx_off, plan.idx_off, st), "upload");
+  CKC(upload_vec(&op->ktot, plan.ktot, st), "upload");
+  CKC(upload_vec(&op->gidx, plan.gidx, st), "upload");
+  CKC(upload_vec(&op->color_cells, plan.color_cells, st), "upload");
+  {
+    std::vector<int32_t> all(op->n_cells);
+    for (int64_t c = 0; c < op->n_cells; ++c) all[c] = (int32_t)c;
+    CKC(upload_vec(&op->all_cells, all, st), "upload");
+    CKC(cudaStreamSynchronize(st), "sync");
+  }
+  CKC(upload_vec(&op->pc_cells, plan.pc_cells, st), "upload");
+  CKC(upload_vec(&op->cell_proj_ptr, plan.cell_proj_ptr, st), "upload");
+  CKC(upload_vec(&op->proj_ptr, plan.proj_ptr, st), "upload");
+  CKC(upload_vec(&op->proj_pcrow, plan.proj_pcrow, st), "upload");
+  {
+    std::vector<double> D(has_nl ? nl->D : nullptr, has_nl ? nl->D + nl->n_proj : nullptr);
+    CKC(upload_vec(&op->D, D, st), "upload");
+    CKC(cudaStreamSynchronize(st), "sync");
+  }
+  CKC(upload_vec(&op->mass, plan.mass, st), "upload");
+  bool bad_jac = false;
+  CKC(build_cell_matrices(op, plan, tab, *mesh, *pot, has_nl ? nl : nullptr, st, &bad_jac), "cell-matrix setup");
+  if (bad_jac) { free_op(op); return fail(nullptr, CHFSI_ERR_BAD_MESH, "non-positive Jacobian at a quadrature point"); }
+  CKC(init_apply_kernels(op), "kernel attribute setup");
+  CKC(cudaStreamSynchronize(st), "sync");
+#undef CKC
+  *out = op;
+  return CHFSI_OK;
+}
+
+int chfsi_destroy(chfsi_op* op) {
+  if (!op) return CHFSI_ERR_BAD_ARGUMENT;
+  free_op(op);
+  return CHFSI_OK;
+}
+
+int chfsi_get_info(const chfsi_op* op, chfsi_info* info) {
+  if (!op || !info) return CHFSI_ERR_BAD_ARGUMENT;
+  info->p = op->p; info->m_cell = op->m_cell; info->n_q = op->n_q; info->precision = op->precision;
+  info->assembly = op->assembly; info->n_colors = op->n_colors;
+  info->n_cells = op->n_cells; info->n_dofs = op->n_dofs; info->n_proj = op->n_proj;
+  info->nnz_cell_proj = op->nnz_cp; info->cells_with_proj = op->n_pc_cells;
+  info->flops_per_vector_apply = (double)op->n_cells * 2.0 * op->m_cell * op->m_cell +
+                                 4.0 * op->m_cell * (double)op->nnz_cp + 7.0 * (double)op->n_dofs;
+  info->matrix_bytes = op->mat_elems * (op->precision == 64 ? 8 : 4);
+  return CHFSI_OK;
+}
+
+int chfsi_workspace_bytes(const chfsi_op* op, int64_t B, size_t* bytes) {
+  if (!op || !bytes || B < 1) return CHFSI_ERR_BAD_ARGUMENT;
+  *bytes = ws_layout(op, B).total;
+  return CHFSI_OK;
+}
+
+int chfsi_mass_diag(const chfsi_op* op, double* M_dev, void* cuda_stream) {
+  if (!op || !M_dev) return CHFSI_ERR_BAD_ARGUMENT;
+  cudaError_t ce = cudaMemcpyAsync(M_dev, op->mass, (size_t)op->n_dofs * sizeof(double), cudaMemcpyDeviceToDevice,
+                                   reinterpret_cast<cudaStream_t>(cuda_stream));
+  return ce == cudaSuccess ? CHFSI_OK : CHFSI_ERR_CUDA;
+}
+
+int chfsi_apply_H(chfsi_op* op, const void* X_dev, int64_t ldx, void* Y_dev, int64_t ldy, int64_t B,
+                  void* workspace_dev, void* cuda_stream) {
+  int rc = check_block_args(op, X_dev, ldx, B, workspace_dev);
+  if (rc) return rc;
+  if (!Y_dev) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "NULL output block");
+  if (ldy < B) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "ldy < B");
+  if (X_dev == Y_dev) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "X and Y must not overlap");
+  const WsLayout w = ws_layout(op, B);
+  char* base = reinterpret_cast<char*>(workspace_dev);
+  ApplyArgs g;
+  g.X = X_dev; g.ldx = ldx; g.T = Y_dev; g.ldt = ldy; g.B = B;
+  g.alpha = 1.0; g.beta = 0.0; g.cshift = 0.0;
+  g.P = base + w.p_off; g.Pc = base + w.pc_off;
+  cudaError_t ce = launch_apply(op, g, reinterpret_cast<cudaStream_t>(cuda_stream));
+  if (ce != cudaSuccess) return cuda_fail(op, ce, "apply_H launch");
+  return CHFSI_OK;
+}
+
+int chfsi_chebyshev_filter(chfsi_op* op, void* X_dev, int64_t ldx, int64_t B, int32_t m, double a, double b,
+                           double a0, void* workspace_dev, void* cuda_stream) {
+  int rc = check_block_args(op, X_dev, ldx, B, workspace_dev);
+  if (rc) return rc;
+  if ((rc = check_filter_scalars(op, m, a, b, a0))) return rc;
+  return filter_block(op, X_dev, ldx, B, m, a, b, a0, workspace_dev, reinterpret_cast<cudaStream_t>(cuda_stream));
+}
+
+int chfsi_chebyshev_filter_chunked(chfsi_op* op, void* X_dev, int64_t ldx, int64_t N, int64_t B, int32_t m,
+                                   double a, double b, double a0, void* workspace_dev, void* cuda_stream) {
+  int rc = check_block_args(op, X_dev, ldx, B, workspace_dev);
+  if (rc) return rc;
+  if (N < 1 || ldx < N) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "need 1 <= N <= ld");
+  if ((rc = check_filter_scalars(op, m, a, b, a0))) return rc;
+  const size_t elt = op->precision == 64 ? 8 : 4;
+  for (int64_t j0 = 0; j0 < N; j0 += B) {
+    const int64_t bw = std::min(B, N - j0);
+    rc = filter_block(op, reinterpret_cast<char*>(X_dev) + (size_t)j0 * elt, ldx, bw, m, a, b, a0, workspace_dev,
+                      reinterpret_cast<cudaStream_t>(cuda_stream));
+    if (rc) return rc;
+  }
+  return CHFSI_OK;
+}
+
+int chfsi_chebyshev_filter_host(chfsi_op* op, void* X_host, int64_t ldx, int64_t N, int64_t B, int32_t m, double a,
+                                double b, double a0) {
+  if (!op) return CHFSI_ERR_BAD_ARGUMENT;
+  if (!X_host) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "NULL host block");
+  if (B < 1 || N < 1 || ldx < N) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "need B >= 1 and 1 <= N <= ld");
+  int rc = check_filter_scalars(op, m, a, b, a0);
+  if (rc) return rc;
+  const size_t elt = op->precision == 64 ? 8 : 4;
+  const int64_t Bc = std::min(B, N);
+  const int64_t ldd = (Bc + 7) / 8 * 8;
+  const WsLayout w = ws_layout(op, Bc);
+  // Two staging blocks and two streams: the copies of chunk i+1 / i-1 overlap the filter of chunk i.
+  void* stage[2] = {nullptr, nullptr};
+  void* ws = nullptr;
+  cudaStream_t st[2] = {nullptr, nullptr};
+  cudaEvent_t done[2] = {nullptr, nullptr};
+  cudaError_t ce = cudaSuccess;
+  rc = CHFSI_OK;
+  const int nbuf = (N > Bc) ? 2 : 1;
+  for (int i = 0; i < nbuf && ce == cudaSuccess; ++i) {
+    ce = cudaMalloc(&stage[i], (size_t)op->n_dofs * ldd * elt);
+    if (ce == cudaSuccess) ce = cudaStreamCreateWithFlags(&st[i], cudaStreamNonBlocking);
+    if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&done[i], cudaEventDisableTiming);
+  }
+  if (ce == cudaSuccess) ce = cudaMalloc(&ws, w.total);
+  if (ce != cudaSuccess) rc = cuda_fail(op, ce, "chebyshev_filter_host allocation");
+  // The filters themselves are serialised through the single workspace by the `done` events.
+  int64_t chunk = 0;
+  for (int64_t j0 = 0; j0 < N && rc == CHFSI_OK; j0 += Bc, ++chunk) {
+    const int s = (int)(chunk % nbuf);
+    const int64_t bw = std::min(Bc, N - j0);
+    char* hp = reinterpret_cast<char*>(X_host) + (size_t)j0 * elt;
+    ce = cudaMemcpy2DAsync(stage[s], (size_t)ldd * elt, hp, (size_t)ldx * elt, (size_t)bw * elt, (size_t)op->n_dofs,
+                           cudaMemcpyHostToDevice, st[s]);
+    if (ce == cudaSuccess && chunk > 0) ce = cudaStreamWaitEvent(st[s], done[(chunk - 1) % nbuf], 0);
+    if (ce != cudaSuccess) { rc = cuda_fail(op, ce, "chebyshev_filter_host H2D"); break; }
+    rc = filter_block(op, stage[s], ldd, bw, m, a, b, a0, ws, st[s]);
+    if (rc) break;
+    ce = cudaEventRecord(done[s], st[s]);
+    if (ce == cudaSuccess)
+      ce = cudaMemcpy2DAsync(hp, (size_t)ldx * elt, stage[s], (size_t)ldd * elt, (size_t)bw * elt, (size_t)op->n_dofs,
+                             cudaMemcpyDeviceToHost, st[s]);
+    if (ce != cudaSuccess) { rc = cuda_fail(op, ce, "chebyshev_filter_host D2H"); break; }
+  }
+  for (int i = 0; i < nbuf; ++i)
+    if (st[i]) {
+      ce = cudaStreamSynchronize(st[i]);
+      if (ce != cudaSuccess && rc == CHFSI_OK) rc = cuda_fail(op, ce, "chebyshev_filter_host sync");
+    }
+  for (int i = 0; i < 2; ++i) {
+    if (done[i]) cudaEventDestroy(done[i]);
+    if (st[i]) cudaStreamDestroy(st[i]);
+    cudaFree(stage[i]);
+  }
+  cudaFree(ws);
+  return rc;
+}
+
+int64_t chfsi_launch_count(const chfsi_op* op) { return op ? op->launches : -1; }
+
+int chfsi_set_kernel_variant(chfsi_op* op, int variant) {
+  if (!op) return CHFSI_ERR_BAD_ARGUMENT;
+  if (variant != 0 && variant != 1) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "variant must be 0 or 1");
+  op->variant = variant;
+  return CHFSI_OK;
+}
+
+const char* chfsi_last_error(const chfsi_op* op) { return op ? op->err.c_str() : g_create_error.c_str(); }
+
+}  // extern "C"

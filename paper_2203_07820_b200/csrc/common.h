@@ -106,5 +106,7 @@ struct ApplyArgs {
 };
 // Enqueues one fused H~ application + recurrence update.  Returns cudaGetLastError().
 cudaError_t launch_apply(Op* op, const ApplyArgs& a, cudaStream_t stream);
+// Opts the kernels into the shared memory they need for this operator (once, at create).
+cudaError_t init_apply_kernels(Op* op);
 
 }  // namespace chfsi

@@ -19,7 +19,6 @@ namespace chfsi {
 
 namespace {
 
-constexpr int kMaxN1 = 9;    // p <= 8
 constexpr int kMaxNq1 = 10;
 
 struct Geom {
