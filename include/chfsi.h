@@ -135,6 +135,27 @@ int64_t chfsi_launch_count(const chfsi_op* op);
  * allows), 1 = force the generic path.  For tests and A/B measurements. */
 int chfsi_set_kernel_variant(chfsi_op* op, int variant);
 
+/* Per-kernel device timing for the roofline report.  While enabled, every H~ application records one CUDA
+ * event pair on the launching stream around its per-cell contraction launches (the dominant kernel; steps 1,
+ * 2, 3d, 4, 5 of the path) and one around its projector launches (steps 3a-3c).  chfsi_get_profile waits for
+ * the recorded events, returns the accumulated device time and launch counts since profiling was enabled (or
+ * last read), and resets the accumulators. */
+typedef struct {
+  double contraction_ms;        /* summed device time of the contraction launches                           */
+  int64_t contraction_launches; /* number of those launches (one per colour, or one in atomic mode)          */
+  double projector_ms;          /* summed device time of the projector launches (incl. atomic-mode pre-fill) */
+  int64_t projector_launches;
+  int64_t applies;              /* H~ applications covered                                                   */
+} chfsi_profile;
+int chfsi_set_profiling(chfsi_op* op, int enabled);
+int chfsi_get_profile(chfsi_op* op, chfsi_profile* prof);
+
+/* FP64 peak of the current device in TFLOP/s, measured with register-resident loops of mma.sync m8n8k4 f64
+ * (the tensor pipe used by the per-cell contraction) and of plain DFMA; best of 5 launches of ~10 ms each.
+ * This is the roofline denominator of the contraction kernel (MEASURED_PEAKS.json has no FP64 figure).
+ * Synchronises the host. */
+int chfsi_measure_fp64_peak(double* dmma_tflops, double* dfma_tflops, void* cuda_stream);
+
 const char* chfsi_last_error(const chfsi_op* op /* NULL: last failed chfsi_create of this thread */);
 
 #ifdef __cplusplus

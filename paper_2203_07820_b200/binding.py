@@ -21,7 +21,8 @@ LIB_PATH = os.path.join(HERE, "libchfsi.so")
 EXPORTED_SYMBOLS = [
     "chfsi_create", "chfsi_destroy", "chfsi_get_info", "chfsi_workspace_bytes", "chfsi_mass_diag",
     "chfsi_apply_H", "chfsi_chebyshev_filter", "chfsi_chebyshev_filter_chunked", "chfsi_chebyshev_filter_host",
-    "chfsi_launch_count", "chfsi_set_kernel_variant", "chfsi_last_error",
+    "chfsi_launch_count", "chfsi_set_kernel_variant", "chfsi_set_profiling", "chfsi_get_profile",
+    "chfsi_measure_fp64_peak", "chfsi_last_error",
 ]
 
 
@@ -51,6 +52,11 @@ class _Info(C.Structure):
                 ("n_cells", C.c_int64), ("n_dofs", C.c_int64), ("n_proj", C.c_int64),
                 ("nnz_cell_proj", C.c_int64), ("cells_with_proj", C.c_int64),
                 ("flops_per_vector_apply", C.c_double), ("matrix_bytes", C.c_int64)]
+
+
+class _Profile(C.Structure):
+    _fields_ = [("contraction_ms", C.c_double), ("contraction_launches", C.c_int64),
+                ("projector_ms", C.c_double), ("projector_launches", C.c_int64), ("applies", C.c_int64)]
 
 
 _lib = None
@@ -92,6 +98,12 @@ def load_library(build_if_missing: bool = True):
     lib_.chfsi_launch_count.restype = i64
     lib_.chfsi_set_kernel_variant.argtypes = [vp, C.c_int]
     lib_.chfsi_set_kernel_variant.restype = C.c_int
+    lib_.chfsi_set_profiling.argtypes = [vp, C.c_int]
+    lib_.chfsi_set_profiling.restype = C.c_int
+    lib_.chfsi_get_profile.argtypes = [vp, C.POINTER(_Profile)]
+    lib_.chfsi_get_profile.restype = C.c_int
+    lib_.chfsi_measure_fp64_peak.argtypes = [C.POINTER(dbl), C.POINTER(dbl), vp]
+    lib_.chfsi_measure_fp64_peak.restype = C.c_int
     lib_.chfsi_last_error.argtypes = [vp]
     lib_.chfsi_last_error.restype = C.c_char_p
     _lib = lib_
@@ -110,6 +122,15 @@ def _stream_ptr(stream) -> Optional[int]:
     import torch
     s = stream if stream is not None else torch.cuda.current_stream()
     return C.c_void_p(s.cuda_stream)
+
+
+def measure_fp64_peak(stream=None) -> dict:
+    """{'dmma_tflops', 'dfma_tflops'} of the current device (chfsi_measure_fp64_peak)."""
+    a, b = C.c_double(), C.c_double()
+    rc = load_library().chfsi_measure_fp64_peak(C.byref(a), C.byref(b), _stream_ptr(stream))
+    if rc != 0:
+        raise ChfsiError(rc, "chfsi_measure_fp64_peak failed")
+    return {"dmma_tflops": a.value, "dfma_tflops": b.value}
 
 
 class Operator:
@@ -251,6 +272,14 @@ class Operator:
 
     def set_kernel_variant(self, variant: int):
         self._check(load_library().chfsi_set_kernel_variant(self._h, int(variant)))
+
+    def set_profiling(self, enabled: bool):
+        self._check(load_library().chfsi_set_profiling(self._h, int(bool(enabled))))
+
+    def get_profile(self) -> dict:
+        pr = _Profile()
+        self._check(load_library().chfsi_get_profile(self._h, C.byref(pr)))
+        return {k: getattr(pr, k) for k, _ in _Profile._fields_}
 
     def close(self):
         if self._h is not None and _lib is not None:

@@ -48,6 +48,7 @@ void free_op(chfsi_op* op) {
   cudaFree(op->mat); cudaFree(op->mat_off); cudaFree(op->idx_off); cudaFree(op->ktot); cudaFree(op->gidx);
   cudaFree(op->color_cells); cudaFree(op->all_cells); cudaFree(op->pc_cells); cudaFree(op->cell_proj_ptr);
   cudaFree(op->proj_ptr); cudaFree(op->proj_pcrow); cudaFree(op->D); cudaFree(op->mass);
+  for (cudaEvent_t e : op->prof_events) cudaEventDestroy(e);
   delete op;
 }
 
@@ -340,6 +341,29 @@ int chfsi_set_kernel_variant(chfsi_op* op, int variant) {
   if (!op) return CHFSI_ERR_BAD_ARGUMENT;
   if (variant != 0 && variant != 1) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "variant must be 0 or 1");
   op->variant = variant;
+  return CHFSI_OK;
+}
+
+int chfsi_set_profiling(chfsi_op* op, int enabled) {
+  if (!op) return CHFSI_ERR_BAD_ARGUMENT;
+  op->profiling = enabled != 0;
+  op->prof_used = 0; op->prof_main_launches = 0; op->prof_proj_launches = 0;
+  return CHFSI_OK;
+}
+
+int chfsi_get_profile(chfsi_op* op, chfsi_profile* prof) {
+  if (!op || !prof) return CHFSI_ERR_BAD_ARGUMENT;
+  std::memset(prof, 0, sizeof(*prof));
+  for (size_t i = 0; i + 3 <= op->prof_used; i += 3) {
+    cudaError_t ce = cudaEventSynchronize(op->prof_events[i + 2]);
+    if (ce != cudaSuccess) return cuda_fail(op, ce, "get_profile");
+    float ms_p = 0.f, ms_m = 0.f;
+    cudaEventElapsedTime(&ms_p, op->prof_events[i], op->prof_events[i + 1]);
+    cudaEventElapsedTime(&ms_m, op->prof_events[i + 1], op->prof_events[i + 2]);
+    prof->projector_ms += ms_p; prof->contraction_ms += ms_m; prof->applies++;
+  }
+  prof->contraction_launches = op->prof_main_launches; prof->projector_launches = op->prof_proj_launches;
+  op->prof_used = 0; op->prof_main_launches = 0; op->prof_proj_launches = 0;
   return CHFSI_OK;
 }
 

@@ -331,6 +331,21 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
   const T* X = reinterpret_cast<const T*>(g.X);
   T* Tg = reinterpret_cast<T*>(g.T);
   const T* mat = reinterpret_cast<const T*>(op->mat);
+  cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
+  if (op->profiling) {
+    if (op->prof_used + 3 > op->prof_events.size()) {
+      for (int i = 0; i < 3; ++i) {
+        cudaEvent_t e;
+        cudaError_t ce = cudaEventCreate(&e);
+        if (ce != cudaSuccess) return ce;
+        op->prof_events.push_back(e);
+      }
+    }
+    for (int i = 0; i < 3; ++i) ev[i] = op->prof_events[op->prof_used + i];
+    op->prof_used += 3;
+    cudaEventRecord(ev[0], st);
+  }
+  const int64_t launches_before = op->launches;
   // steps 3a-3c
   if (op->n_proj > 0) {
     dim3 g1((unsigned)op->n_pc_cells, (unsigned)((B + 127) / 128));
@@ -366,6 +381,11 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
     k_prefill<T><<<148 * 8, 256, 0, st>>>(X, g.ldx, Tg, g.ldt, op->n_dofs, B, a.ac, a.beta);
     op->launches++;
   }
+  if (op->profiling) {
+    cudaEventRecord(ev[1], st);
+    op->prof_proj_launches += op->launches - launches_before;
+  }
+  const int64_t launches_mid = op->launches;
   const int n_launch = op->assembly == 1 ? 1 : op->n_colors;
   for (int c = 0; c < n_launch; ++c) {
     if (op->assembly == 1) { a.cells = op->all_cells; a.n_launch_cells = (int)op->n_cells; }
@@ -389,6 +409,10 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
       k_apply_generic<T><<<grid, 256, (size_t)op->max_ktot * 32 * sizeof(T), st>>>(a);
     }
     op->launches++;
+  }
+  if (op->profiling) {
+    cudaEventRecord(ev[2], st);
+    op->prof_main_launches += op->launches - launches_mid;
   }
   return cudaGetLastError();
 }

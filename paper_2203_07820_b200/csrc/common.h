@@ -84,6 +84,11 @@ struct Op {
   double* D = nullptr;
   double* mass = nullptr;
   int64_t launches = 0;
+  // optional per-kernel timing (chfsi_set_profiling): event triples (start, after projector kernels, end)
+  bool profiling = false;
+  std::vector<cudaEvent_t> prof_events;
+  size_t prof_used = 0;
+  int64_t prof_main_launches = 0, prof_proj_launches = 0;
   std::string err;
 };
 
