@@ -376,3 +376,49 @@ def ritz_values_of_block(Y, HY, rel_cut: float = 1e-12):
     keep = w > rel_cut * w[-1]
     Qk = Q[:, keep] / np.sqrt(w[keep])[None, :]
     return np.linalg.eigvalsh(Qk.T @ Hh @ Qk)
+
+
+def apply_H_rows(wl, M, X, rows):
+    """Rows `rows` of Y = H~ X computed ONE BY ONE from the definition, without building the whole operator
+    (for spot checks at sizes where `build_operator` takes minutes).  `wl` carries the raw inputs (p, cell_dofs,
+    cell_vertices, veff_q and the projector CSR / chi_q), `M` is `mass_diagonal(...)`.
+
+        Y[g] = M_g^-1/2 ( sum_{(c,l): dof(c,l)=g} ( H^c[l,:] U^c + sum_{j on c} C^c_{l,j} D_j P_j ) ),  U = M^-1/2 X,
+        P_j = sum_{c' in supp(j)} C^{c'}_{:,j} . U^{c'}
+
+    i.e. Eq. 47 and Algorithm 4 restricted to the cells that contain g.
+    Pinned in tests/test_oracle_filter.py against `apply_H` (itself pinned to the brute-force dense operator)."""
+    X = np.asarray(X, dtype=np.float64)
+    ref = reference_cell(wl.p)
+    s = 1.0 / np.sqrt(M)
+    out = np.zeros((len(rows), X.shape[1]))
+    # projector -> cells lists, and cell -> (projector, CSR position) lists for the cells we touch
+    P_cache = {}
+
+    def P_of(j):
+        if j not in P_cache:
+            acc = np.zeros(X.shape[1])
+            for k in range(int(wl.proj_cell_ptr[j]), int(wl.proj_cell_ptr[j + 1])):
+                c2 = int(wl.proj_cell_idx[k])
+                g2 = wl.cell_dofs[c2]
+                Cv = projector_cell_vector(ref, wl.cell_vertices[c2], wl.chi_q[k])
+                acc += Cv @ (s[g2, None] * X[g2])
+            P_cache[j] = acc
+        return P_cache[j]
+
+    for r, g in enumerate(rows):
+        cells, locs = np.nonzero(wl.cell_dofs == g)
+        acc = np.zeros(X.shape[1])
+        for c, l in zip(cells, locs):
+            gd = wl.cell_dofs[c]
+            He = cell_hamiltonian(ref, wl.cell_vertices[c], wl.veff_q[c])[0]
+            acc += He[l] @ (s[gd, None] * X[gd])
+            if wl.n_proj:
+                for j in range(wl.n_proj):
+                    k0, k1 = int(wl.proj_cell_ptr[j]), int(wl.proj_cell_ptr[j + 1])
+                    hit = np.nonzero(wl.proj_cell_idx[k0:k1] == c)[0]
+                    if hit.size:
+                        Cv = projector_cell_vector(ref, wl.cell_vertices[c], wl.chi_q[k0 + int(hit[0])])
+                        acc += Cv[l] * wl.D[j] * P_of(j)
+        out[r] = s[g] * acc
+    return out

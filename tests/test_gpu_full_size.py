@@ -1,0 +1,161 @@
+"""GPU <-> oracle parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (chunk width B,
+degree m, stored bounds recipe B, default coloured assembly), through the C ABI.  `-m gpu`.
+
+ * config 2: the whole 110,592 x 256 block against the oracle, plus the Rayleigh-Ritz values.
+ * configs 3 / 4 / 5: the GPU filters one full chunk (B = 256 / 512 / 400 columns); the oracle filters SAMPLED
+   columns of that chunk one by one (columns are independent, and every column of the seeded block
+   has its own random stream), and sampled ROWS of H~X are recomputed from the definition (oracle.apply_H_rows).
+ * properties that hold at any size: the fused filter equals the three-term recurrence driven by separate
+   apply_H calls; a column filtered inside the wide chunk (tensor-core kernel) equals the same column filtered
+   alone (generic kernel).
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+
+def _imports():
+    import torch
+    from oracle import chfsi_oracle as orc
+    from paper_2203_07820_b200 import Operator
+    from workloads.generate import CONFIGS, SEED_X, load_bounds, make_workload, random_block
+    return torch, orc, Operator, CONFIGS, SEED_X, load_bounds, make_workload, random_block
+
+
+def rel_fro(a, b):
+    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+def device_block(torch, random_block, n_dofs, B, seed, dtype):
+    """The first B columns of the config's seeded N(0,1) block, on the device."""
+    X = torch.empty((n_dofs, B), dtype=dtype, device="cuda")
+    for j0 in range(0, B, 64):
+        j1 = min(B, j0 + 64)
+        X[:, j0:j1] = torch.from_numpy(random_block(n_dofs, range(j0, j1), seed)).to("cuda", dtype)
+    return X
+
+
+def recurrence_from_apply_H(torch, op, X, m, a, b, a0):
+    """Eq. 37 / scaled form (include/chfsi.h) with chfsi_apply_H as the only library call."""
+    e, c = (b - a) / 2, (b + a) / 2
+    s1 = e / (a0 - c)
+    s = s1
+    Ym2 = X
+    Ym1 = (op.apply_H(X) - c * X) * (s1 / e)
+    for _ in range(2, m + 1):
+        sn = 1.0 / (2.0 / s1 - s)
+        Y = (op.apply_H(Ym1) - c * Ym1) * (2 * sn / e) - (s * sn) * Ym2
+        Ym2, Ym1, s = Ym1, Y, sn
+    return Ym1
+
+
+def test_config2_whole_block_and_ritz_values():
+    torch, orc, Operator, CONFIGS, SEED_X, load_bounds, make_workload, random_block = _imports()
+    spec = CONFIGS[2]
+    wl = make_workload(2)
+    a0, a, b = load_bounds(spec.bounds_key, "B")
+    oop = orc.operator_from_workload(wl)
+    X = random_block(wl.n_dofs, range(spec.B), spec.seed_base + SEED_X)
+    Fo = orc.chebyshev_filter(oop, X, spec.m, a, b, a0)
+    for assembly in (0, 1):
+        op = Operator.from_workload(wl, assembly=assembly)
+        Xd = torch.tensor(X, device="cuda")
+        Y = op.apply_H(Xd).cpu().numpy()
+        assert rel_fro(Y, orc.apply_H(oop, X)) <= 1e-10
+        op.chebyshev_filter_chunked(Xd, spec.B, spec.m, a, b, a0)
+        F = Xd.cpu().numpy()
+        err = rel_fro(F, Fo)
+        assert err <= 1e-10, f"config 2 assembly {assembly}: {err:.3e}"
+        assert np.max(np.abs(F - Fo)) <= 1e-10 * np.max(np.abs(Fo))
+        th_g = orc.ritz_values_of_block(F, orc.apply_H(oop, F))
+        th_o = orc.ritz_values_of_block(Fo, orc.apply_H(oop, Fo))
+        assert th_g.shape == th_o.shape and np.max(np.abs(th_g - th_o)) <= 1e-8
+        op.close()
+
+
+@pytest.fixture(scope="module")
+def config3_oracle():
+    torch, orc, Operator, CONFIGS, SEED_X, load_bounds, make_workload, random_block = _imports()
+    wl = make_workload(3)
+    return wl, orc.operator_from_workload(wl)
+
+
+SAMPLE_COLS = {3: [0, 131, 255], 4: [0, 300, 511], 5: [0, 399]}
+
+
+@pytest.mark.parametrize("config", [3, 4])
+def test_config3_and_4_one_chunk_sampled_columns(config, config3_oracle):
+    torch, orc, Operator, CONFIGS, SEED_X, load_bounds, make_workload, random_block = _imports()
+    spec = CONFIGS[config]
+    wl, oop = config3_oracle
+    a0, a, b = load_bounds(spec.bounds_key, "B")
+    tol, tol_ritz = (1e-10, 1e-8) if spec.precision == 64 else (1e-4, 1e-5)
+    op = Operator.from_workload(wl, precision=spec.precision)
+    Xd = device_block(torch, random_block, wl.n_dofs, spec.B, spec.seed_base + SEED_X, op.dtype)
+    cols = SAMPLE_COLS[config]
+    Xs = Xd[:, cols].double().cpu().numpy()                  # FP32 variant: the input rounded once to FP32
+    if spec.precision == 64:
+        assert np.array_equal(Xs, random_block(wl.n_dofs, cols, spec.seed_base + SEED_X))
+    Y = op.apply_H(Xd)
+    Yr = orc.apply_H(oop, Xs)
+    assert rel_fro(Y[:, cols].double().cpu().numpy(), Yr) <= tol
+    # the fused filter == the recurrence built from apply_H (any size), then the oracle on the sampled columns
+    F = Xd.clone()
+    op.chebyshev_filter_chunked(F, spec.B, spec.m, a, b, a0)
+    R = recurrence_from_apply_H(torch, op, Xd, spec.m, a, b, a0)
+    assert float((F - R).norm() / R.norm()) <= (1e-12 if spec.precision == 64 else 1e-5)
+    del R, Y
+    Fo = orc.chebyshev_filter(oop, Xs, spec.m, a, b, a0)
+    Fs = F[:, cols].double().cpu().numpy()
+    for k, j in enumerate(cols):
+        err = rel_fro(Fs[:, k], Fo[:, k])
+        assert err <= tol, f"config {config} column {j}: {err:.3e}"
+        assert np.max(np.abs(Fs[:, k] - Fo[:, k])) <= tol * np.max(np.abs(Fo[:, k]))
+    th_g = orc.ritz_values_of_block(Fs, orc.apply_H(oop, Fs))
+    th_o = orc.ritz_values_of_block(Fo, orc.apply_H(oop, Fo))
+    assert np.max(np.abs(th_g - th_o)) <= tol_ritz
+    # a column filtered alone (generic kernel, B = 1) == the same column inside the wide chunk
+    one = Xd[:, cols[1]:cols[1] + 1].clone()
+    op.chebyshev_filter(one, spec.m, a, b, a0)
+    assert float((one[:, 0] - F[:, cols[1]]).norm() / one.norm()) <= (1e-12 if spec.precision == 64 else 1e-5)
+    op.close()
+
+
+def test_config5_one_chunk_sampled_rows_columns_and_properties():
+    torch, orc, Operator, CONFIGS, SEED_X, load_bounds, make_workload, random_block = _imports()
+    spec = CONFIGS[5]
+    wl = make_workload(5)
+    a0, a, b = load_bounds(spec.bounds_key, "B")
+    op = Operator.from_workload(wl)
+    assert op.info["n_dofs"] == 1728000 and op.info["n_proj"] == 1728
+    Xd = device_block(torch, random_block, wl.n_dofs, spec.B, spec.seed_base + SEED_X, op.dtype)
+    cols = SAMPLE_COLS[5]
+    Xs = Xd[:, cols].cpu().numpy()
+    # (1) sampled rows of H~X recomputed one by one from the definition, without the whole oracle operator
+    M = orc.mass_diagonal(wl.p, wl.cell_dofs, wl.cell_vertices, wl.n_dofs)
+    assert np.allclose(op.mass_diag().cpu().numpy(), M, rtol=1e-12)
+    near_atom = int(wl.cell_dofs[int(wl.proj_cell_idx[0]), 171])          # a dof inside a projector's support
+    rows = [0, 3, 120 * 5 + 2, near_atom, wl.n_dofs - 1]
+    Y = op.apply_H(Xd)
+    Yr = orc.apply_H_rows(wl, M, Xs, rows)
+    Yg = Y[rows][:, cols].cpu().numpy()
+    assert np.max(np.abs(Yg - Yr)) <= 1e-10 * float(Y.abs().max())
+    del Y
+    # (2) fused filter == recurrence from apply_H calls, at the full chunk width and degree
+    F = Xd.clone()
+    op.chebyshev_filter_chunked(F, spec.B, spec.m, a, b, a0)
+    R = recurrence_from_apply_H(torch, op, Xd, spec.m, a, b, a0)
+    assert float((F - R).norm() / R.norm()) <= 1e-12
+    del R
+    # (3) the oracle proper on sampled columns of the chunk
+    oop = orc.operator_from_workload(wl)
+    Fo = orc.chebyshev_filter(oop, Xs, spec.m, a, b, a0)
+    Fs = F[:, cols].cpu().numpy()
+    for k, j in enumerate(cols):
+        err = rel_fro(Fs[:, k], Fo[:, k])
+        assert err <= 1e-10, f"config 5 column {j}: {err:.3e}"
+    th_g = orc.ritz_values_of_block(Fs, orc.apply_H(oop, Fs))
+    th_o = orc.ritz_values_of_block(Fo, orc.apply_H(oop, Fo))
+    assert np.max(np.abs(th_g - th_o)) <= 1e-8
+    op.close()

@@ -1,0 +1,208 @@
+"""GPU <-> oracle parity of the CUDA path, element by element, through the C ABI (ctypes binding).  `-m gpu`.
+
+Sizes: the oracle finishes in seconds, yet every case spans several (cell, column-tile) CTAs, several K panels
+and a ragged tail (B not a multiple of the 64-column tile, M_cell = 343 not a multiple of 8, odd B on the generic
+kernel).  Tolerances are north_star's (BASELINE.json): FP64 relative Frobenius error <= 1e-10 and Rayleigh-Ritz
+values within 1e-8 Ha; FP32 variant <= 1e-4 and 1e-5 Ha.  The element-wise bound used on top of that is
+|dY_ij| <= tol * max|Y| (same tolerance, max-norm instead of Frobenius).
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL = {64: (1e-10, 1e-8), 32: (1e-4, 1e-5)}
+
+
+def _imports():
+    import torch
+    from oracle import chfsi_oracle as orc
+    from paper_2203_07820_b200 import ChfsiError, Operator
+    from workloads.generate import load_bounds, make_workload, random_block
+    return torch, orc, Operator, ChfsiError, make_workload, random_block, load_bounds
+
+
+def rel_fro(a, b):
+    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+def assert_block_close(Y, Yo, tol, what):
+    assert Y.shape == Yo.shape
+    assert np.all(np.isfinite(Y)), what
+    err = rel_fro(Y, Yo)
+    emax = float(np.max(np.abs(Y - Yo)) / np.max(np.abs(Yo)))
+    assert err <= tol and emax <= tol, f"{what}: rel Frobenius {err:.3e}, max-norm {emax:.3e} > {tol:g}"
+    return err
+
+
+CASES = {
+    # name: (workload kwargs | config number, B, m, precision)
+    "config1": (1, 32, 10, 64),
+    "p6_nonlocal_ragged": (dict(n=3, p=6, L=6.0, atoms_per_side=1, n_gaussians=0, nonlocal_=True, smooth_field=0.05,
+                                seed_base=77), 72, 7, 64),
+    "p6_distorted_cells": (dict(n=2, p=6, L=4.0, mesh_jitter=0.15, atoms_per_side=1, n_gaussians=0, nonlocal_=True,
+                                smooth_field=0.05, seed_base=78, r_cut=1.9), 40, 6, 64),
+    "p3_odd_B": (dict(n=3, p=3, L=6.0, atoms_per_side=1, n_gaussians=0, nonlocal_=True, smooth_field=0.05,
+                      seed_base=79), 13, 5, 64),
+    "p2_nonperiodic": (dict(n=3, p=2, L=6.0, periodic=False, atoms_per_side=1, n_gaussians=0, nonlocal_=True,
+                            smooth_field=0.05, seed_base=80, r_cut=2.5), 8, 4, 64),
+    "p6_fp32": (dict(n=3, p=6, L=6.0, atoms_per_side=1, n_gaussians=0, nonlocal_=True, smooth_field=0.05,
+                     seed_base=77), 64, 7, 32),
+    "p4_fp32_odd_B": (dict(n=3, p=4, L=6.0, atoms_per_side=1, n_gaussians=0, nonlocal_=True, smooth_field=0.05,
+                           seed_base=81), 21, 6, 32),
+}
+
+_cache = {}
+
+
+def oracle_case(name):
+    """Oracle operator, inputs, bounds and expected blocks of a case (computed once per session)."""
+    if name in _cache:
+        return _cache[name]
+    torch, orc, Operator, _, make_workload, random_block, load_bounds = _imports()
+    spec, B, m, precision = CASES[name]
+    wl = make_workload(spec) if isinstance(spec, int) else make_workload(None, **spec)
+    oop = orc.operator_from_workload(wl)
+    X = random_block(wl.n_dofs, range(B), 7)
+    if precision == 32:
+        X = X.astype(np.float32).astype(np.float64)     # the FP64-generated input rounded once to FP32 (reading U9)
+    if isinstance(spec, int):
+        a0, a, b = load_bounds(str(spec), "B")
+    else:
+        b, lmin = orc.lanczos_upper_bound(oop, np.random.default_rng(5).standard_normal(wl.n_dofs), 20)
+        a0, a = lmin, lmin + 0.1 * (b - lmin)
+    Yo = orc.apply_H(oop, X)
+    Fo = orc.chebyshev_filter(oop, X, m, a, b, a0)
+    _cache[name] = (wl, oop, X, (a0, a, b), Yo, Fo)
+    return _cache[name]
+
+
+@pytest.mark.parametrize("assembly", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("name", list(CASES))
+def test_apply_H_and_filter_match_the_oracle(name, assembly, variant):
+    torch, orc, Operator, _, _, _, _ = _imports()
+    _, B, m, precision = CASES[name]
+    wl, oop, X, (a0, a, b), Yo, Fo = oracle_case(name)
+    tol, tol_ritz = TOL[precision]
+    op = Operator.from_workload(wl, precision=precision, assembly=assembly)
+    op.set_kernel_variant(variant)
+    Xd = torch.tensor(X, dtype=op.dtype, device="cuda")
+    n0 = op.launch_count()
+    Y = op.apply_H(Xd).double().cpu().numpy()
+    assert op.launch_count() > n0, "no kernel was launched"
+    assert_block_close(Y, Yo, tol, f"{name} apply_H")
+    F = Xd.clone()
+    op.chebyshev_filter(F, m, a, b, a0)
+    F = F.double().cpu().numpy()
+    assert_block_close(F, Fo, tol, f"{name} filter m={m}")
+    # Rayleigh-Ritz values of the filtered subspace (Algorithm 2), same H~Y provider on both sides
+    th_g = orc.ritz_values_of_block(F, orc.apply_H(oop, F))
+    th_o = orc.ritz_values_of_block(Fo, orc.apply_H(oop, Fo))
+    assert th_g.shape == th_o.shape
+    assert np.max(np.abs(th_g - th_o)) <= tol_ritz, f"{name}: Ritz values differ by {np.max(np.abs(th_g - th_o)):.3e} Ha"
+    op.close()
+
+
+def test_mass_diagonal_matches_the_oracle():
+    torch, orc, Operator, *_ = _imports()
+    wl, oop, *_ = oracle_case("p6_distorted_cells")
+    op = Operator.from_workload(wl)
+    M = op.mass_diag().cpu().numpy()
+    assert np.allclose(M, oop.M, rtol=1e-12, atol=0)
+
+
+def test_coloured_assembly_is_bit_reproducible_and_atomic_is_within_tolerance():
+    torch, orc, Operator, *_ = _imports()
+    wl, oop, X, (a0, a, b), Yo, Fo = oracle_case("p6_nonlocal_ragged")
+    op = Operator.from_workload(wl, assembly=0)
+    Xd = torch.tensor(X, device="cuda")
+    runs = []
+    for _ in range(3):
+        F = Xd.clone()
+        op.chebyshev_filter(F, 7, a, b, a0)
+        runs.append(F.clone())
+    assert torch.equal(runs[0], runs[1]) and torch.equal(runs[0], runs[2])
+    opa = Operator.from_workload(wl, assembly=1)
+    Fa = Xd.clone()
+    opa.chebyshev_filter(Fa, 7, a, b, a0)
+    assert rel_fro(Fa.cpu().numpy(), runs[0].cpu().numpy()) <= 1e-12
+
+
+def test_chunked_wide_array_strided_columns_and_odd_degree():
+    """A chunk of a wider array is filtered in place through ld > B; chunked == all at once == column by column
+    (column independence); odd m exercises the copy-back from the workspace block."""
+    torch, orc, Operator, *_ = _imports()
+    wl, oop, X, (a0, a, b), _, _ = oracle_case("p6_nonlocal_ragged")
+    op = Operator.from_workload(wl)
+    N = X.shape[1]                                         # 72
+    for m in (1, 2, 5):
+        Fo = orc.chebyshev_filter(oop, X, m, a, b, a0)
+        wide = torch.full((wl.n_dofs, N + 24), 123.0, dtype=torch.float64, device="cuda")
+        wide[:, 8:8 + N] = torch.tensor(X, device="cuda")
+        op.chebyshev_filter_chunked(wide[:, 8:8 + N], 32, m, a, b, a0)       # chunks 32 + 32 + 8
+        assert_block_close(wide[:, 8:8 + N].cpu().numpy(), Fo, 1e-10, f"chunked m={m}")
+        assert torch.all(wide[:, :8] == 123.0) and torch.all(wide[:, 8 + N:] == 123.0), "columns outside the chunk touched"
+    one = torch.tensor(X[:, 5:6].copy(), device="cuda")
+    op.chebyshev_filter(one, 5, a, b, a0)
+    assert_block_close(one.cpu().numpy(), orc.chebyshev_filter(oop, X[:, 5:6], 5, a, b, a0), 1e-10, "B=1")
+
+
+def test_host_buffer_entry_point_matches_device_entry_point():
+    torch, orc, Operator, *_ = _imports()
+    wl, oop, X, (a0, a, b), _, _ = oracle_case("p6_nonlocal_ragged")
+    op = Operator.from_workload(wl)
+    Fo = orc.chebyshev_filter(oop, X, 4, a, b, a0)
+    Xh = torch.tensor(X).pin_memory()
+    op.chebyshev_filter_host(Xh, 32, 4, a, b, a0)
+    assert_block_close(Xh.numpy(), Fo, 1e-10, "host entry point")
+    Xn = np.ascontiguousarray(X)
+    op.chebyshev_filter_host(Xn, 100, 4, a, b, a0)        # pageable NumPy memory, B > N
+    assert_block_close(Xn, Fo, 1e-10, "host entry point (NumPy)")
+
+
+def test_degenerate_inputs():
+    torch, orc, Operator, ChfsiError, make_workload, random_block, _ = _imports()
+    # no projectors at all, a0 == a, the smallest periodic mesh (n = 2) and p = 1
+    wl = make_workload(None, n=2, p=1, L=2.0, atoms_per_side=1, n_gaussians=0, nonlocal_=False, smooth_field=0.1,
+                       seed_base=5)
+    oop = orc.operator_from_workload(wl)
+    X = random_block(wl.n_dofs, range(3), 1)
+    op = Operator.from_workload(wl)
+    F = torch.tensor(X, device="cuda")
+    op.chebyshev_filter(F, 3, 0.5, 9.0, 0.5)
+    assert_block_close(F.cpu().numpy(), orc.chebyshev_filter(oop, X, 3, 0.5, 9.0, 0.5), 1e-10, "a0 == a")
+    # an all-zero block stays zero; V_eff = 0 constant mode is annihilated by apply_H
+    Z = torch.zeros((wl.n_dofs, 4), dtype=torch.float64, device="cuda")
+    op.chebyshev_filter(Z, 4, 0.5, 9.0, 0.1)
+    assert torch.all(Z == 0)
+    wl0 = make_workload(None, n=3, p=4, L=6.0, atoms_per_side=0, n_gaussians=0, nonlocal_=False, smooth_field=0.0,
+                        seed_base=5)
+    op0 = Operator.from_workload(wl0)
+    v = torch.sqrt(op0.mass_diag())[:, None].repeat(1, 8).contiguous()
+    assert float(op0.apply_H(v).abs().max()) <= 1e-11 * float(v.abs().max()) * 60.0   # ||H~|| ~ 60 Ha here
+
+
+def test_argument_errors_on_the_device_entry_points():
+    torch, orc, Operator, ChfsiError, *_ = _imports()
+    wl, *_ = oracle_case("p3_odd_B")
+    op = Operator.from_workload(wl)
+    X = torch.zeros((wl.n_dofs, 8), dtype=torch.float64, device="cuda")
+    for args in [(0, 1.0, 2.0, 0.5), (3, 2.0, 1.0, 0.5), (3, 1.0, 2.0, 1.5), (3, 1.0, float("inf"), 0.5)]:
+        with pytest.raises(ChfsiError) as ei:
+            op.chebyshev_filter(X, *args)
+        assert ei.value.code == -1
+    with pytest.raises(ChfsiError):
+        op.apply_H(X, X)                                    # aliasing
+    with pytest.raises(TypeError):
+        op.apply_H(X.float())
+    bad = wl.cell_dofs.copy()
+    bad[0, 1] = bad[0, 0]                                   # dof repeated inside one cell
+    with pytest.raises(ChfsiError) as ei:
+        Operator(wl.p, bad, wl.cell_vertices, wl.n_dofs, wl.veff_q)
+    assert ei.value.code == -2
+    verts = wl.cell_vertices.copy()
+    verts[0, [0, 1]] = verts[0, [1, 0]]                     # inverted cell
+    with pytest.raises(ChfsiError) as ei:
+        Operator(wl.p, wl.cell_dofs, verts, wl.n_dofs, wl.veff_q)
+    assert ei.value.code == -2
