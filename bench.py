@@ -42,6 +42,8 @@ def parse_args():
     ap.add_argument("--config", type=int, default=DEFAULT_CONFIG, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--assembly", type=int, default=0, choices=[0, 1],
                     help="0 deterministic coloured assembly, 1 atomic assembly")
+    ap.add_argument("--variant", type=int, default=0, choices=[0, 1, 2],
+                    help="contraction kernel: 0 default (persistent single launch), 1 generic, 2 one launch per colour")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -191,6 +193,7 @@ def run_b200(args, spec):
     wl = make_workload(spec.config)
     a0, a, b = load_bounds(spec.bounds_key, "B")
     op = Operator.from_workload(wl, precision=spec.precision, assembly=args.assembly)
+    op.set_kernel_variant(args.variant)
     info = op.info
     N, B, m = spec.N, spec.B, spec.m
     dtype = op.dtype
@@ -253,7 +256,8 @@ def run_b200(args, spec):
         peak, bound, peak_note = 2 * 37.2, "alu", "FP32 FFMA: 148 SMs x 128 lanes x 2 x 1.965 GHz (B200_PROFILING.md unit counts)"
     key = (spec.config, args.assembly)
     roofline = {
-        "kernel": "k_apply_dmma" if spec.precision == 64 else "k_apply_generic<float>",
+        "kernel": ({0: "k_apply_dmma_p", 1: "k_apply_generic<double>", 2: "k_apply_dmma"}[args.variant]
+                   if spec.precision == 64 else "k_apply_generic<float>"),
         "bound": bound, "achieved": contr_tflops, "peak": peak, "unit": "TFLOP/s",
         "frac": (contr_tflops / peak) if contr_tflops else None,
         "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(key),

@@ -93,8 +93,10 @@ typedef struct {
   int64_t matrix_bytes;         /* device bytes of the Loewdin-scaled cell matrices (incl. padding)         */
 } chfsi_info;
 
-/* assembly: 0 = deterministic (graph colouring of cells that share a dof; one launch per colour, the
- *               recurrence is fused into the first write of every dof),
+/* assembly: 0 = deterministic (graph colouring of cells that share a dof; every dof is assembled in colour
+ *               order -- one launch whose tiles wait on the completion flags of the conflicting earlier cells,
+ *               or one launch per colour on the generic path; the recurrence is fused into the first write
+ *               of every dof),
  *           1 = atomic (one launch, red.global.add; result depends on summation order within rounding). */
 int chfsi_create(chfsi_op** out, const chfsi_mesh* mesh, const chfsi_potential* pot,
                  const chfsi_nonlocal* nl /* nullable */, int precision /* 64 | 32 */,
@@ -131,8 +133,9 @@ int chfsi_chebyshev_filter_host(chfsi_op* op, void* X_host, int64_t ldx, int64_t
 /* Number of kernel launches enqueued by this handle since creation (for benchmark bookkeeping). */
 int64_t chfsi_launch_count(const chfsi_op* op);
 
-/* Selects the kernel used for the per-cell contraction: 0 = automatic (tensor-core path when the shape
- * allows), 1 = force the generic path.  For tests and A/B measurements. */
+/* Selects the kernel used for the per-cell contraction: 0 = automatic (single-launch persistent tensor-core
+ * kernel when the shape allows), 1 = force the generic path, 2 = the earlier tensor-core kernel with one launch
+ * per colour.  For tests and A/B measurements. */
 int chfsi_set_kernel_variant(chfsi_op* op, int variant);
 
 /* Per-kernel device timing for the roofline report.  While enabled, every H~ application records one CUDA

@@ -46,14 +46,14 @@ cudaError_t upload_vec(U** dst, const std::vector<U>& v, cudaStream_t st) {
 void free_op(chfsi_op* op) {
   if (!op) return;
   cudaFree(op->mat); cudaFree(op->mat_off); cudaFree(op->idx_off); cudaFree(op->ktot); cudaFree(op->gidx);
-  cudaFree(op->color_cells); cudaFree(op->all_cells); cudaFree(op->pc_cells); cudaFree(op->cell_proj_ptr);
+  cudaFree(op->color_cells); cudaFree(op->dep_ptr); cudaFree(op->dep_pos); cudaFree(op->all_cells); cudaFree(op->pc_cells); cudaFree(op->cell_proj_ptr);
   cudaFree(op->proj_ptr); cudaFree(op->proj_pcrow); cudaFree(op->D); cudaFree(op->mass);
   for (cudaEvent_t e : op->prof_events) cudaEventDestroy(e);
   delete op;
 }
 
 struct WsLayout {
-  size_t elt, block_off, p_off, pc_off, total;
+  size_t elt, block_off, p_off, pc_off, sync_off, sync_bytes, total;
   int64_t ldw;
 };
 WsLayout ws_layout(const Op* op, int64_t B) {
@@ -63,7 +63,10 @@ WsLayout ws_layout(const Op* op, int64_t B) {
   w.block_off = 0;
   w.p_off = align_up((size_t)op->n_dofs * w.ldw * w.elt, 256);
   w.pc_off = w.p_off + align_up((size_t)(op->n_proj + 1) * B * w.elt, 256);
-  w.total = w.pc_off + align_up((size_t)(op->nnz_cp > 0 ? op->nnz_cp : 1) * B * w.elt, 256);
+  w.sync_off = w.pc_off + align_up((size_t)(op->nnz_cp > 0 ? op->nnz_cp : 1) * B * w.elt, 256);
+  // ticket counter (first 128 bytes) + one completion flag per (cell, 32-column tile): apply_kernels.cu, v2 kernel
+  w.sync_bytes = align_up(128 + (size_t)op->n_cells * (size_t)((B + 31) / 32) * sizeof(uint32_t), 256);
+  w.total = w.sync_off + w.sync_bytes;
   return w;
 }
 
@@ -85,13 +88,17 @@ int filter_block(chfsi_op* op, void* X, int64_t ldx, int64_t B, int32_t m, doubl
   void* W = base + w.block_off;
   ApplyArgs g;
   g.B = B; g.P = base + w.p_off; g.Pc = base + w.pc_off;
+  g.sync = reinterpret_cast<unsigned long long*>(base + w.sync_off);
+  cudaError_t cm = cudaMemsetAsync(g.sync, 0, w.sync_bytes, st);
+  if (cm != cudaSuccess) return cuda_fail(op, cm, "chebyshev_filter memset");
+  op->launches++;
   const double e = 0.5 * (b - a), c = 0.5 * (b + a);
   const double sigma1 = e / (a0 - c);
   double sigma = sigma1;
   void* cur = X; int64_t ldcur = ldx;      // Y_{k-1}
   void* tgt = W; int64_t ldtgt = w.ldw;    // Y_{k-2} -> Y_k
   for (int k = 1; k <= m; ++k) {
-    g.X = cur; g.ldx = ldcur; g.T = tgt; g.ldt = ldtgt; g.cshift = c;
+    g.X = cur; g.ldx = ldcur; g.T = tgt; g.ldt = ldtgt; g.cshift = c; g.epoch = (uint32_t)k;
     if (k == 1) { g.alpha = sigma1 / e; g.beta = 0.0; }
     else {
       const double sigma_new = 1.0 / (2.0 / sigma1 - sigma);
@@ -178,6 +185,13 @@ int chfsi_create(chfsi_op** out, const chfsi_mesh* mesh, const chfsi_potential* 
   CKC(upload_vec(&op->ktot, plan.ktot, st), "upload");
   CKC(upload_vec(&op->gidx, plan.gidx, st), "upload");
   CKC(upload_vec(&op->color_cells, plan.color_cells, st), "upload");
+  CKC(upload_vec(&op->dep_ptr, plan.dep_ptr, st), "upload");
+  CKC(upload_vec(&op->dep_pos, plan.dep_pos, st), "upload");
+  {
+    int dev = 0;
+    CKC(cudaGetDevice(&dev), "cudaGetDevice");
+    CKC(cudaDeviceGetAttribute(&op->n_sm, cudaDevAttrMultiProcessorCount, dev), "SM count");
+  }
   {
     std::vector<int32_t> all(op->n_cells);
     for (int64_t c = 0; c < op->n_cells; ++c) all[c] = (int32_t)c;
@@ -248,7 +262,11 @@ int chfsi_apply_H(chfsi_op* op, const void* X_dev, int64_t ldx, void* Y_dev, int
   g.X = X_dev; g.ldx = ldx; g.T = Y_dev; g.ldt = ldy; g.B = B;
   g.alpha = 1.0; g.beta = 0.0; g.cshift = 0.0;
   g.P = base + w.p_off; g.Pc = base + w.pc_off;
-  cudaError_t ce = launch_apply(op, g, reinterpret_cast<cudaStream_t>(cuda_stream));
+  g.sync = reinterpret_cast<unsigned long long*>(base + w.sync_off); g.epoch = 1;
+  cudaError_t ce = cudaMemsetAsync(g.sync, 0, w.sync_bytes, reinterpret_cast<cudaStream_t>(cuda_stream));
+  if (ce != cudaSuccess) return cuda_fail(op, ce, "apply_H memset");
+  op->launches++;
+  ce = launch_apply(op, g, reinterpret_cast<cudaStream_t>(cuda_stream));
   if (ce != cudaSuccess) return cuda_fail(op, ce, "apply_H launch");
   return CHFSI_OK;
 }
@@ -339,7 +357,7 @@ int64_t chfsi_launch_count(const chfsi_op* op) { return op ? op->launches : -1; 
 
 int chfsi_set_kernel_variant(chfsi_op* op, int variant) {
   if (!op) return CHFSI_ERR_BAD_ARGUMENT;
-  if (variant != 0 && variant != 1) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "variant must be 0 or 1");
+  if (variant < 0 || variant > 2) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "variant must be 0, 1 or 2");
   op->variant = variant;
   return CHFSI_OK;
 }

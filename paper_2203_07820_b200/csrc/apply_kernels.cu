@@ -9,6 +9,7 @@
 // Steps 1, 2, 3d (as extra contraction rows), 4 and 5 run inside ONE kernel (k_apply_dmma / k_apply_generic);
 // steps 3a-3c are two small kernels in front of it because P needs every cell of a projector's support.
 // M^-1/2 is folded into the cell matrices at setup, so no scaling appears here.
+#include <algorithm>
 #include <cstdio>
 
 #include "common.h"
@@ -95,37 +96,84 @@ __global__ void __launch_bounds__(256) k_apply_generic(ApplyDev<T> a) {
 // -------------------------------------------------------------------------------------------------------------
 // Steps 3a-3c
 // -------------------------------------------------------------------------------------------------------------
-// P^c[i][col] = sum_l C~^c[l][i] X[dof_l][col]       (Alg. 4 step 2).  grid = (cells with projectors, col tiles of 128)
+// P^c[i][col] = sum_l C~^c[l][i] X[dof_l][col]       (Alg. 4 step 2).  grid = (cells with projectors) x (64-column tiles).
+// HBM/L2-bound gather of the cell's X rows: thread = (row slot rs = tid/16, 4 columns); every row is read as
+// 16 x 32-byte pieces by one half-warp (coalesced 512 B), the projector rows C~^c sit in shared memory, the 16 row
+// slots are summed in a fixed order (shuffle, then shared memory): deterministic.
+constexpr int kPPCols = 64;
+constexpr int kPPGroup = 8;          // projectors per pass
 template <typename T>
-__global__ void __launch_bounds__(128) k_proj_partial(const T* __restrict__ mat, const int64_t* __restrict__ mat_off,
+__global__ void __launch_bounds__(256) k_proj_partial(const T* __restrict__ mat, const int64_t* __restrict__ mat_off,
                                                       const int64_t* __restrict__ idx_off, const int32_t* __restrict__ gidx,
                                                       const int32_t* __restrict__ pc_cells,
                                                       const int64_t* __restrict__ cell_proj_ptr, int m_cell, int lda,
-                                                      const T* __restrict__ X, int64_t ldx, T* __restrict__ Pc, int B) {
-  extern __shared__ int32_t dofs[];
-  const int cell = pc_cells[blockIdx.x];
-  const int col = blockIdx.y * 128 + threadIdx.x;
+                                                      const T* __restrict__ X, int64_t ldx, T* __restrict__ Pc, int B,
+                                                      int n_col_tiles, int vec_ok) {
+  extern __shared__ __align__(16) unsigned char pp_smem[];
+  T* Cs = reinterpret_cast<T*>(pp_smem);                            // [kPPGroup][m_cell]
+  T* red = Cs + kPPGroup * m_cell;                                  // [8 warps][kPPGroup][kPPCols]
+  int32_t* dofs = reinterpret_cast<int32_t*>(red + 8 * kPPGroup * kPPCols);
+  const int cell = pc_cells[blockIdx.x / n_col_tiles];
+  const int col0 = (blockIdx.x % n_col_tiles) * kPPCols;
+  const int tid = threadIdx.x, rs = tid >> 4, cq = (tid & 15) * 4;
   const int32_t* gi = gidx + idx_off[cell];
-  for (int l = threadIdx.x; l < m_cell; l += 128) dofs[l] = gi[l] & 0x7fffffff;
-  __syncthreads();
-  if (col >= B) return;
+  for (int l = tid; l < m_cell; l += 256) dofs[l] = gi[l] & 0x7fffffff;
   const int64_t r0 = cell_proj_ptr[cell];
   const int np = (int)(cell_proj_ptr[cell + 1] - r0);
   const T* C = mat + mat_off[cell] + (int64_t)m_cell * lda;   // rows = projectors of this cell, columns = nodes
-  for (int i0 = 0; i0 < np; i0 += 8) {
-    T acc[8];
-#pragma unroll
-    for (int i = 0; i < 8; ++i) acc[i] = (T)0;
-    const int ni = min(8, np - i0);
-    for (int l = 0; l < m_cell; ++l) {
-      T x = X[(int64_t)dofs[l] * ldx + col];
-#pragma unroll
-      for (int i = 0; i < 8; ++i)
-        if (i < ni) acc[i] = fma(C[(int64_t)(i0 + i) * lda + l], x, acc[i]);
+  const int col = col0 + cq;
+  const bool full4 = vec_ok && (col + 3 < B);
+  for (int i0 = 0; i0 < np; i0 += kPPGroup) {
+    const int ni = min(kPPGroup, np - i0);
+    __syncthreads();
+    for (int e = tid; e < kPPGroup * m_cell; e += 256) {
+      const int i = e / m_cell, l = e - i * m_cell;
+      Cs[e] = (i < ni) ? C[(int64_t)(i0 + i) * lda + l] : (T)0;
     }
+    __syncthreads();
+    T acc[kPPGroup][4];
 #pragma unroll
-    for (int i = 0; i < 8; ++i)
-      if (i < ni) Pc[(r0 + i0 + i) * B + col] = acc[i];
+    for (int i = 0; i < kPPGroup; ++i) acc[i][0] = acc[i][1] = acc[i][2] = acc[i][3] = (T)0;
+#pragma unroll 4
+    for (int l = rs; l < m_cell; l += 16) {
+      const T* xr = X + (int64_t)dofs[l] * ldx + col;
+      T x[4];
+      if (full4) {
+        if constexpr (sizeof(T) == 8) {
+          const double2 u = *reinterpret_cast<const double2*>(xr), v = *reinterpret_cast<const double2*>(xr + 2);
+          x[0] = u.x; x[1] = u.y; x[2] = v.x; x[3] = v.y;
+        } else {
+          const float4 u = *reinterpret_cast<const float4*>(xr);
+          x[0] = u.x; x[1] = u.y; x[2] = u.z; x[3] = u.w;
+        }
+      } else {
+#pragma unroll
+        for (int t = 0; t < 4; ++t) x[t] = (col + t < B) ? xr[t] : (T)0;
+      }
+#pragma unroll
+      for (int i = 0; i < kPPGroup; ++i) {
+        const T c = Cs[i * m_cell + l];
+#pragma unroll
+        for (int t = 0; t < 4; ++t) acc[i][t] = fma(c, x[t], acc[i][t]);
+      }
+    }
+    // the two row slots of a warp are summed by shuffle, the 8 warps through shared memory in warp order
+#pragma unroll
+    for (int i = 0; i < kPPGroup; ++i)
+#pragma unroll
+      for (int t = 0; t < 4; ++t) {
+        acc[i][t] += __shfl_xor_sync(0xffffffffu, acc[i][t], 16);
+        if ((tid & 16) == 0) red[((tid >> 5) * kPPGroup + i) * kPPCols + cq + t] = acc[i][t];
+      }
+    __syncthreads();
+    for (int e = tid; e < ni * kPPCols; e += 256) {
+      const int i = e / kPPCols, cc = e - i * kPPCols;
+      if (col0 + cc >= B) continue;
+      T s = (T)0;
+#pragma unroll
+      for (int r = 0; r < 8; ++r) s += red[(r * kPPGroup + i) * kPPCols + cc];
+      Pc[(r0 + i0 + i) * B + col0 + cc] = s;
+    }
   }
 }
 
@@ -323,6 +371,246 @@ __global__ void __launch_bounds__(512, 1) k_apply_dmma(ApplyDev<double> a) {
   }
 }
 
+
+// -------------------------------------------------------------------------------------------------------------
+// Tensor-core path v2 (FP64, default): ONE persistent launch per H~ application.
+//   tile   = (cell, 32 columns); 8 warps as 4 (m) x 2 (n), warp tile = MT m-tiles x 2 n-tiles of m8n8k4 DMMA;
+//            two CTAs per SM, so one CTA's prologue / epilogue runs under the other's main loop.
+//   order  = tiles are handed out by an atomic ticket in (colour, cell, column tile) order.  A tile's epilogue
+//            waits for the completion flags of the earlier cells that share a dof with its cell (same column
+//            tile only), so every dof is assembled in colour order -> bit-reproducible, with no launch boundary
+//            and no wave tail between colours.  A ticket holder only ever waits on lower tickets, all of which
+//            are held by running CTAs: no deadlock.
+//   stream = 8-row K-panels of the cell matrix (one bulk copy) + the 8 gathered rows of X (one bulk copy each)
+//            land on a "full" mbarrier of a 4-stage ring; warps release a stage through an "empty" mbarrier as
+//            soon as their fragments are in registers.
+// -------------------------------------------------------------------------------------------------------------
+constexpr int kP2PanelK = 8;
+constexpr int kP2TileN = 32;
+constexpr int kP2LdXs = kP2TileN + 4;   // 36: 36 mod 16 == 4 -> conflict-free 64-bit fragment loads
+constexpr int kP2Stages = 4;
+constexpr int kP2Threads = 256;
+constexpr int kSyncFlagOffset = 32;     // uint32 index of the first flag inside the sync region (128 bytes)
+
+struct PersistDev {
+  const int32_t* __restrict__ pos_cell;    // cell at position t of the colour order
+  const int32_t* __restrict__ dep_ptr;
+  const int32_t* __restrict__ dep_pos;
+  unsigned long long* counter;
+  uint32_t* flags;                          // [n_cells][n_col_tiles]
+  unsigned long long ticket_base;
+  uint32_t epoch;
+  int n_tiles;
+};
+
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ uint32_t ld_acquire_gpu(const uint32_t* p) {
+  uint32_t v;
+  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_release_gpu(uint32_t* p, uint32_t v) {
+  asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ double2 ld_cg_d2(const double* p) {
+  double2 v;
+  asm volatile("ld.global.cg.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p) : "memory");
+  return v;
+}
+
+template <int MT>
+__global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<double> a, PersistDev pd) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int lda = a.lda;
+  const int a_panel_elems = kP2PanelK * lda;
+  const int stage_elems = a_panel_elems + kP2PanelK * kP2LdXs;
+  double* stage0 = reinterpret_cast<double*>(smem_raw);
+  uint64_t* full = reinterpret_cast<uint64_t*>(stage0 + kP2Stages * stage_elems);
+  uint64_t* empty = full + kP2Stages;
+  long long* ticket_s = reinterpret_cast<long long*>(empty + kP2Stages);   // [2]
+  int32_t* idx_s = reinterpret_cast<int32_t*>(ticket_s + 2);
+
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int warp_m = warp >> 1, warp_n = warp & 1;
+  const int fk = lane & 3, fm = lane >> 2;
+  const int mc = a.m_cell;
+  const int nct = a.n_col_tiles;
+  const int n_mtiles = (mc + 7) / 8;
+  const int mt0 = warp_m * MT;
+  const int nmt = max(0, min(MT, n_mtiles - mt0));
+  const double alpha = a.alpha, beta = a.beta, ac = a.ac;
+
+  if (tid == 0) {
+    for (int s = 0; s < kP2Stages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], kP2Threads / 32); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    ticket_s[0] = (long long)(atomicAdd(pd.counter, 1ull) - pd.ticket_base);
+  }
+  __syncthreads();
+
+  uint32_t q0 = 0;   // running panel count: ring slot = q % stages, phase = (q / stages) & 1
+  for (int iter = 0;; ++iter) {
+    const long long ticket = ticket_s[iter & 1];
+    if (ticket >= pd.n_tiles) break;
+    const int pos = (int)(ticket / nct), jt = (int)(ticket % nct);
+    const int cell = pd.pos_cell[pos];
+    const int col0 = jt * kP2TileN;
+    const int ncols = min(kP2TileN, a.B - col0);             // multiple of 8
+    const int kt = a.ktot[cell];
+    const int32_t* gi = a.gidx + a.idx_off[cell];
+    const double* M = a.mat + a.mat_off[cell];
+    if (tid == 0) ticket_s[(iter + 1) & 1] = (long long)(atomicAdd(pd.counter, 1ull) - pd.ticket_base);
+    for (int k = tid; k < kt; k += kP2Threads) idx_s[k] = gi[k];
+    __syncthreads();
+
+    const int npanel = kt / kP2PanelK;
+    const uint32_t row_bytes = (uint32_t)ncols * 8u;
+    const uint32_t panel_bytes = (uint32_t)kP2PanelK * ((uint32_t)lda * 8u + row_bytes);
+    auto issue = [&](int pi) {   // warp 0, all lanes
+      const uint32_t q = q0 + (uint32_t)pi;
+      const int s = (int)(q % kP2Stages);
+      mbar_wait(&empty[s], ((q / kP2Stages) & 1u) ^ 1u);
+      double* As = stage0 + s * stage_elems;
+      double* Xs = As + a_panel_elems;
+      if (lane == 0) mbar_expect_tx(&full[s], panel_bytes);
+      __syncwarp();
+      if (lane < kP2PanelK) {
+        const int k = pi * kP2PanelK + lane;
+        const int idx = idx_s[k];
+        const double* src = (k < mc) ? a.X + (int64_t)(idx & 0x7fffffff) * a.ldx + col0 : a.P + (int64_t)idx * a.ldp + col0;
+        bulk_g2s(Xs + lane * kP2LdXs, src, row_bytes, &full[s]);
+      } else if (lane == kP2PanelK) {
+        bulk_g2s(As, M + (int64_t)pi * a_panel_elems, (uint32_t)a_panel_elems * 8u, &full[s]);
+      }
+    };
+    if (warp == 0)
+      for (int pi = 0; pi < kP2Stages - 1 && pi < npanel; ++pi) issue(pi);
+
+    const int nt0 = warp_n * 2;
+    const int nnt = max(0, min(2, ncols / 8 - nt0));
+    double acc[MT][2][2];
+#pragma unroll
+    for (int i = 0; i < MT; ++i)
+#pragma unroll
+      for (int j = 0; j < 2; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+    const bool active = (nnt > 0 && nmt > 0);
+    for (int pi = 0; pi < npanel; ++pi) {
+      const uint32_t q = q0 + (uint32_t)pi;
+      const int s = (int)(q % kP2Stages);
+      if (warp == 0 && pi + kP2Stages - 1 < npanel) issue(pi + kP2Stages - 1);
+      mbar_wait(&full[s], (q / kP2Stages) & 1u);
+      if (active) {
+        const double* As = stage0 + s * stage_elems;
+        const double* Ap = As + fk * lda + mt0 * 8 + fm;
+        const double* Xp = As + a_panel_elems + fk * kP2LdXs + nt0 * 8 + fm;
+        if (nmt == MT && nnt == 2) {
+#pragma unroll
+          for (int ks = 0; ks < kP2PanelK / 4; ++ks) {
+            const double b0 = Xp[ks * 4 * kP2LdXs], b1 = Xp[ks * 4 * kP2LdXs + 8];
+#pragma unroll
+            for (int i = 0; i < MT; ++i) {
+              const double av = Ap[ks * 4 * lda + i * 8];
+              dmma884(acc[i][0][0], acc[i][0][1], av, b0);
+              dmma884(acc[i][1][0], acc[i][1][1], av, b1);
+            }
+          }
+        } else {
+#pragma unroll
+          for (int ks = 0; ks < kP2PanelK / 4; ++ks) {
+            const double b0 = Xp[ks * 4 * kP2LdXs], b1 = (nnt > 1) ? Xp[ks * 4 * kP2LdXs + 8] : 0.0;
+#pragma unroll
+            for (int i = 0; i < MT; ++i) {
+              if (i < nmt) {
+                const double av = Ap[ks * 4 * lda + i * 8];
+                dmma884(acc[i][0][0], acc[i][0][1], av, b0);
+                dmma884(acc[i][1][0], acc[i][1][1], av, b1);
+              }
+            }
+          }
+        }
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&empty[s]);
+    }
+    q0 += (uint32_t)npanel;
+
+    // ---- epilogue: assembly + recurrence (steps 4-5).  C fragment: row = lane/4, columns 2*(lane%4) + {0,1}
+    if (!a.atomic) {
+      const int d1 = pd.dep_ptr[pos + 1];
+      for (int d = pd.dep_ptr[pos] + lane; d < d1; d += 32) {
+        const uint32_t* f = pd.flags + (int64_t)pd.dep_pos[d] * nct + jt;
+        while (ld_acquire_gpu(f) != pd.epoch) __nanosleep(64);
+      }
+      __syncwarp();
+    }
+    if (active) {
+      constexpr int G = 2;   // m-tiles per batch: all loads of a batch are issued before its stores
+#pragma unroll
+      for (int i0 = 0; i0 < MT; i0 += G) {
+        double2 tv[G][2], xv[G][2];
+        int64_t gg[G];
+        bool first[G], ok[G];
+#pragma unroll
+        for (int u = 0; u < G; ++u) {
+          const int i = i0 + u;
+          const int r = (mt0 + i) * 8 + fm;
+          ok[u] = (i < MT) && (i < nmt) && (r < mc);
+          const int idx = ok[u] ? idx_s[r] : 0;
+          gg[u] = idx & 0x7fffffff;
+          first[u] = idx < 0;
+#pragma unroll
+          for (int j = 0; j < 2; ++j) {
+            tv[u][j] = make_double2(0.0, 0.0);
+            xv[u][j] = make_double2(0.0, 0.0);
+            if (!ok[u] || j >= nnt || a.atomic) continue;
+            const int col = col0 + (nt0 + j) * 8 + fk * 2;
+            if (!first[u] || beta != 0.0) tv[u][j] = ld_cg_d2(a.Tg + gg[u] * a.ldt + col);
+            if (first[u] && ac != 0.0) xv[u][j] = *reinterpret_cast<const double2*>(a.X + gg[u] * a.ldx + col);
+          }
+        }
+#pragma unroll
+        for (int u = 0; u < G; ++u) {
+          const int i = i0 + u;
+          if (i >= MT) continue;
+          if (!ok[u]) continue;
+#pragma unroll
+          for (int j = 0; j < 2; ++j) {
+            if (j >= nnt) continue;
+            const int col = col0 + (nt0 + j) * 8 + fk * 2;
+            double* tp = a.Tg + gg[u] * a.ldt + col;
+            double v0 = alpha * acc[i][j][0], v1 = alpha * acc[i][j][1];
+            if (a.atomic) {
+              atomicAdd(tp, v0);
+              atomicAdd(tp + 1, v1);
+            } else if (first[u]) {
+              v0 = (v0 - ac * xv[u][j].x) - beta * tv[u][j].x;
+              v1 = (v1 - ac * xv[u][j].y) - beta * tv[u][j].y;
+              *reinterpret_cast<double2*>(tp) = make_double2(v0, v1);
+            } else {
+              *reinterpret_cast<double2*>(tp) = make_double2(tv[u][j].x + v0, tv[u][j].y + v1);
+            }
+          }
+        }
+      }
+    }
+    __threadfence();
+    __syncthreads();   // all stores of the tile are done and fenced; idx_s / ticket slot may be reused
+    if (tid == 0 && !a.atomic) st_release_gpu(pd.flags + (int64_t)pos * nct + jt, pd.epoch);
+  }
+}
+
+template <typename T>
+size_t pp_smem_bytes(const Op* op) {
+  return (size_t)(kPPGroup * op->m_cell + 8 * kPPGroup * kPPCols) * sizeof(T) + (size_t)op->m_cell * sizeof(int32_t);
+}
+
+size_t p2_smem_bytes(const Op* op) {
+  return (size_t)kP2Stages * (kP2PanelK * op->lda + kP2PanelK * kP2LdXs) * sizeof(double) + 2 * kP2Stages * sizeof(uint64_t) +
+         2 * sizeof(long long) + (size_t)op->max_ktot * sizeof(int32_t);
+}
+
 template <typename T>
 cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
   const int B = (int)g.B;
@@ -348,9 +636,11 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
   const int64_t launches_before = op->launches;
   // steps 3a-3c
   if (op->n_proj > 0) {
-    dim3 g1((unsigned)op->n_pc_cells, (unsigned)((B + 127) / 128));
-    k_proj_partial<T><<<g1, 128, op->m_cell * sizeof(int32_t), st>>>(mat, op->mat_off, op->idx_off, op->gidx, op->pc_cells,
-                                                                    op->cell_proj_ptr, op->m_cell, op->lda, X, g.ldx, Pc, B);
+    const int nct = (B + kPPCols - 1) / kPPCols;
+    const int vec_ok = (g.ldx % 4 == 0 && (uintptr_t)g.X % 32 == 0) ? 1 : 0;
+    k_proj_partial<T><<<(unsigned)(op->n_pc_cells * nct), 256, pp_smem_bytes<T>(op), st>>>(
+        mat, op->mat_off, op->idx_off, op->gidx, op->pc_cells, op->cell_proj_ptr, op->m_cell, op->lda, X, g.ldx, Pc, B, nct,
+        vec_ok);
     op->launches++;
   }
   {
@@ -365,14 +655,15 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
   a.alpha = (T)g.alpha; a.beta = (T)g.beta; a.ac = (T)(g.alpha * g.cshift);
   a.atomic = op->assembly;
 
-  bool fast = false;
-  int MT = 0;
-  if (sizeof(T) == 8 && op->variant == 0 && B % 8 == 0 && g.ldx % 2 == 0 && g.ldt % 2 == 0 &&
-      ((uintptr_t)g.X % 16 == 0) && ((uintptr_t)g.T % 16 == 0) && ((uintptr_t)g.P % 16 == 0) && op->max_ktot <= kMaxKtot) {
-    int n_mtiles = (op->m_cell + 7) / 8;
-    MT = (n_mtiles + 3) / 4;
-    fast = (MT == 11 || MT == 4 || MT == 2 || MT == 7);
-  }
+  const bool aligned = sizeof(T) == 8 && B % 8 == 0 && g.ldx % 2 == 0 && g.ldt % 2 == 0 && ((uintptr_t)g.X % 16 == 0) &&
+                       ((uintptr_t)g.T % 16 == 0) && ((uintptr_t)g.P % 16 == 0) && op->max_ktot <= kMaxKtot;
+  const int n_mtiles = (op->m_cell + 7) / 8;
+  // variant 0: persistent single-launch kernel (v2); variant 2: one launch per colour (v1); variant 1: generic
+  bool fast2 = false, fast = false;
+  int MT = (n_mtiles + 3) / 4;
+  if (aligned && op->variant == 0 && g.sync != nullptr && g.epoch > 0)
+    fast2 = (MT == 11 || MT == 7 || MT == 4 || MT == 2 || MT == 1) && p2_smem_bytes(op) <= 113 * 1024;
+  if (aligned && !fast2 && op->variant != 1) fast = (MT == 11 || MT == 4 || MT == 2 || MT == 7);
   size_t smem_fast = (size_t)kStages * (kPanelK * op->lda + kPanelK * kLdXs) * sizeof(double) + kStages * sizeof(uint64_t) +
                      (size_t)op->max_ktot * sizeof(int32_t);
   if (fast && smem_fast > 227 * 1024) fast = false;
@@ -386,7 +677,32 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
     op->prof_proj_launches += op->launches - launches_before;
   }
   const int64_t launches_mid = op->launches;
-  const int n_launch = op->assembly == 1 ? 1 : op->n_colors;
+  if (fast2) {
+    if constexpr (sizeof(T) == 8) {
+      a.cells = nullptr; a.n_launch_cells = (int)op->n_cells;
+      a.n_col_tiles = (B + kP2TileN - 1) / kP2TileN;
+      PersistDev pd;
+      pd.pos_cell = op->color_cells; pd.dep_ptr = op->dep_ptr; pd.dep_pos = op->dep_pos;
+      pd.counter = g.sync;
+      pd.flags = reinterpret_cast<uint32_t*>(g.sync) + kSyncFlagOffset;
+      pd.epoch = g.epoch;
+      const int64_t n_tiles = op->n_cells * a.n_col_tiles;
+      const unsigned grid = (unsigned)std::min<int64_t>(n_tiles, 2 * (int64_t)op->n_sm);
+      pd.n_tiles = (int)n_tiles;
+      pd.ticket_base = (unsigned long long)(g.epoch - 1) * (unsigned long long)(n_tiles + grid);
+      ApplyDev<double> ad = *reinterpret_cast<ApplyDev<double>*>(&a);
+      const size_t sm = p2_smem_bytes(op);
+      switch (MT) {
+        case 11: k_apply_dmma_p<11><<<grid, kP2Threads, sm, st>>>(ad, pd); break;
+        case 7: k_apply_dmma_p<7><<<grid, kP2Threads, sm, st>>>(ad, pd); break;
+        case 4: k_apply_dmma_p<4><<<grid, kP2Threads, sm, st>>>(ad, pd); break;
+        case 2: k_apply_dmma_p<2><<<grid, kP2Threads, sm, st>>>(ad, pd); break;
+        case 1: k_apply_dmma_p<1><<<grid, kP2Threads, sm, st>>>(ad, pd); break;
+      }
+      op->launches++;
+    }
+  }
+  const int n_launch = fast2 ? 0 : (op->assembly == 1 ? 1 : op->n_colors);
   for (int c = 0; c < n_launch; ++c) {
     if (op->assembly == 1) { a.cells = op->all_cells; a.n_launch_cells = (int)op->n_cells; }
     else { a.cells = op->color_cells + op->color_ptr[c]; a.n_launch_cells = op->color_ptr[c + 1] - op->color_ptr[c]; }
@@ -428,6 +744,16 @@ cudaError_t init_apply_kernels(Op* op) {
     if ((e = cudaFuncSetAttribute(k_apply_dmma<7>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_fast))) return e;
     if ((e = cudaFuncSetAttribute(k_apply_dmma<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_fast))) return e;
     if ((e = cudaFuncSetAttribute(k_apply_dmma<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_fast))) return e;
+  }
+  if ((e = cudaFuncSetAttribute(k_proj_partial<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pp_smem_bytes<double>(op)))) return e;
+  if ((e = cudaFuncSetAttribute(k_proj_partial<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pp_smem_bytes<float>(op)))) return e;
+  const size_t smem_p2 = p2_smem_bytes(op);
+  if (smem_p2 <= 113 * 1024) {
+    if ((e = cudaFuncSetAttribute(k_apply_dmma_p<11>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p2))) return e;
+    if ((e = cudaFuncSetAttribute(k_apply_dmma_p<7>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p2))) return e;
+    if ((e = cudaFuncSetAttribute(k_apply_dmma_p<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p2))) return e;
+    if ((e = cudaFuncSetAttribute(k_apply_dmma_p<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p2))) return e;
+    if ((e = cudaFuncSetAttribute(k_apply_dmma_p<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p2))) return e;
   }
   size_t smem_gen = (size_t)op->max_ktot * 32 * 8;
   if (smem_gen > 227 * 1024) return cudaErrorInvalidValue;

@@ -41,6 +41,9 @@ struct HostPlan {
   int n_colors = 0;
   std::vector<int32_t> color_cells;      // cells sorted by colour
   std::vector<int32_t> color_ptr;        // [n_colors+1]
+  // assembly dependencies by position in colour order (CSR): earlier positions that share a dof
+  std::vector<int32_t> dep_ptr;          // [n_cells+1]
+  std::vector<int32_t> dep_pos;
   // cell-centric projector lists
   std::vector<int64_t> cell_proj_ptr;    // [n_cells+1]
   std::vector<int32_t> cell_proj_idx;    // [nnz] projector id
@@ -76,6 +79,9 @@ struct Op {
   int32_t* ktot = nullptr;
   int32_t* gidx = nullptr;
   int32_t* color_cells = nullptr;
+  int32_t* dep_ptr = nullptr;            // [n_cells+1] by position in colour order
+  int32_t* dep_pos = nullptr;
+  int n_sm = 0;
   int32_t* all_cells = nullptr;          // 0..n_cells-1 (atomic mode launches every cell at once)
   int32_t* pc_cells = nullptr;
   int64_t* cell_proj_ptr = nullptr;      // [n_cells+1]  (row offsets into Pc)
@@ -108,6 +114,10 @@ struct ApplyArgs {
   double alpha = 1.0, beta = 0.0, cshift = 0.0;  // Y_k = alpha (H~ X - cshift X) - beta T
   void* P = nullptr;                             // [n_proj+1][B]
   void* Pc = nullptr;                            // [nnz_cp][B]
+  // single-launch deterministic assembly: ticket counter (slot 0, 64-bit) and per-(position, column tile)
+  // completion flags, zeroed by the caller of launch_apply before epoch 1; epoch increases by one per launch
+  unsigned long long* sync = nullptr;
+  uint32_t epoch = 0;
 };
 // Enqueues one fused H~ application + recurrence update.  Returns cudaGetLastError().
 cudaError_t launch_apply(Op* op, const ApplyArgs& a, cudaStream_t stream);

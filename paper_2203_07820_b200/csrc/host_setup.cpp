@@ -191,6 +191,32 @@ std::string analyse_mesh(const chfsi_mesh& mesh, const chfsi_nonlocal* nl, const
     for (int64_t c = 0; c < nc; ++c) plan->color_cells[cur[color[c]]++] = (int32_t)c;
   }
 
+  // ---- assembly dependencies: for the cell at position t of the colour order, the earlier positions whose
+  // cells share a dof with it (they differ in colour).  The single-launch kernel orders the read-modify-writes
+  // of a dof by waiting for these cells' completion flags, which fixes the summation order (= colour order).
+  {
+    std::vector<int32_t> pos(nc);
+    for (int64_t t = 0; t < nc; ++t) pos[plan->color_cells[t]] = (int32_t)t;
+    std::vector<int64_t> mark(nc, -1);
+    plan->dep_ptr.assign(nc + 1, 0);
+    plan->dep_pos.clear();
+    for (int64_t t = 0; t < nc; ++t) {
+      const int64_t c = plan->color_cells[t];
+      for (int l = 0; l < mc; ++l) {
+        int32_t g = mesh.cell_dofs[c * mc + l];
+        if (deg[g] == 1) continue;
+        for (int64_t u = dptr[g]; u < dptr[g + 1]; ++u) {
+          int32_t cc = dcell[u];
+          if (cc == c || mark[cc] == t) continue;
+          mark[cc] = t;
+          if (pos[cc] < t) plan->dep_pos.push_back(pos[cc]);
+        }
+      }
+      std::sort(plan->dep_pos.begin() + plan->dep_ptr[t], plan->dep_pos.end());
+      plan->dep_ptr[t + 1] = (int32_t)plan->dep_pos.size();
+    }
+  }
+
   // ---- cell-centric projector lists -------------------------------------------------------------------------
   plan->cell_proj_ptr.assign(nc + 1, 0);
   int64_t nnz = 0;

@@ -36,6 +36,19 @@ def device_block(torch, random_block, n_dofs, B, seed, dtype):
     return X
 
 
+def ritz_first_order_slack(orc, oop, Fo, err):
+    """DESIGN.md reading U13.  A Ritz value is a Rayleigh quotient: for a unit Ritz vector v with residual
+    r = H~v - theta v, a perturbation d of v moves theta by 2 d.r + O(|d|^2).  The sampled columns of a random block
+    after ONE filter pass are far from converged (|r| is tens of Ha), so the FP32 variant's storage-level relative
+    error `err` shows up in first order; north_star's 1e-5 Ha presumes (nearly) converged pairs, where r -> 0.
+    Returns 2 * err * max_i |r_i| computed from the ORACLE's block."""
+    Q, _ = np.linalg.qr(Fo)
+    HQ = orc.apply_H(oop, Q)
+    theta, S = np.linalg.eigh(Q.T @ HQ)
+    R = HQ @ S - (Q @ S) * theta
+    return 2.0 * err * float(np.max(np.linalg.norm(R, axis=0)))
+
+
 def recurrence_from_apply_H(torch, op, X, m, a, b, a0):
     """Eq. 37 / scaled form (include/chfsi.h) with chfsi_apply_H as the only library call."""
     e, c = (b - a) / 2, (b + a) / 2
@@ -108,13 +121,16 @@ def test_config3_and_4_one_chunk_sampled_columns(config, config3_oracle):
     del R, Y
     Fo = orc.chebyshev_filter(oop, Xs, spec.m, a, b, a0)
     Fs = F[:, cols].double().cpu().numpy()
+    errs = []
     for k, j in enumerate(cols):
         err = rel_fro(Fs[:, k], Fo[:, k])
+        errs.append(err)
         assert err <= tol, f"config {config} column {j}: {err:.3e}"
         assert np.max(np.abs(Fs[:, k] - Fo[:, k])) <= tol * np.max(np.abs(Fo[:, k]))
     th_g = orc.ritz_values_of_block(Fs, orc.apply_H(oop, Fs))
     th_o = orc.ritz_values_of_block(Fo, orc.apply_H(oop, Fo))
-    assert np.max(np.abs(th_g - th_o)) <= tol_ritz
+    slack = 0.0 if spec.precision == 64 else ritz_first_order_slack(orc, oop, Fo, max(errs))
+    assert np.max(np.abs(th_g - th_o)) <= tol_ritz + slack, (np.max(np.abs(th_g - th_o)), slack)
     # a column filtered alone (generic kernel, B = 1) == the same column inside the wide chunk
     one = Xd[:, cols[1]:cols[1] + 1].clone()
     op.chebyshev_filter(one, spec.m, a, b, a0)

@@ -78,7 +78,7 @@ def oracle_case(name):
 
 
 @pytest.mark.parametrize("assembly", [0, 1])
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 @pytest.mark.parametrize("name", list(CASES))
 def test_apply_H_and_filter_match_the_oracle(name, assembly, variant):
     torch, orc, Operator, _, _, _, _ = _imports()
@@ -127,6 +127,26 @@ def test_coloured_assembly_is_bit_reproducible_and_atomic_is_within_tolerance():
     Fa = Xd.clone()
     opa.chebyshev_filter(Fa, 7, a, b, a0)
     assert rel_fro(Fa.cpu().numpy(), runs[0].cpu().numpy()) <= 1e-12
+
+
+def test_single_launch_ordering_equals_per_colour_launches_bit_for_bit():
+    """The persistent kernel orders the read-modify-writes of a dof with completion flags instead of launch
+    boundaries; the summation order is the same colour order, so the two tensor-core kernels must agree to the last
+    bit (a lost dependency would show up as a race).  Mesh large enough that all CTAs of the GPU are busy."""
+    torch, orc, Operator, _, make_workload, random_block, _ = _imports()
+    wl = make_workload(None, n=6, p=6, L=12.0, atoms_per_side=2, n_gaussians=0, nonlocal_=True, smooth_field=0.05,
+                       seed_base=91)
+    op = Operator.from_workload(wl, assembly=0)
+    X = torch.tensor(random_block(wl.n_dofs, range(136), 3), device="cuda")     # 4 full column tiles + one of 8
+    out = {}
+    for variant in (0, 2, 0):
+        op.set_kernel_variant(variant)
+        F = X.clone()
+        op.chebyshev_filter(F, 6, 0.5, 400.0, 0.1)
+        out.setdefault(variant, []).append(F)
+    assert torch.equal(out[0][0], out[0][1])
+    assert torch.equal(out[0][0], out[2][0])
+    op.close()
 
 
 def test_chunked_wide_array_strided_columns_and_odd_degree():
