@@ -47,6 +47,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         obj = os.path.join(HERE, "build", s + ".o")
         cmd = [nvcc, "-O3", "-std=c++17", "-lineinfo", *ARCH, "-Xcompiler", "-fPIC", "-x", "cu",
                "-c", os.path.join(CSRC, s), "-o", obj]
+        cmd[1:1] = os.environ.get("CHFSI_NVCC_FLAGS", "").split()     # e.g. -DCHFSI_TRACE (debug time stamps)
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
         procs.append((s, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))

@@ -11,6 +11,7 @@
 // M^-1/2 is folded into the cell matrices at setup, so no scaling appears here.
 #include <algorithm>
 #include <cstdio>
+#include <cstdlib>
 
 #include "common.h"
 
@@ -390,6 +391,9 @@ constexpr int kP2TileN = 32;
 constexpr int kP2LdXs = kP2TileN + 4;   // 36: 36 mod 16 == 4 -> conflict-free 64-bit fragment loads
 constexpr int kP2Stages = 4;
 constexpr int kP2Threads = 256;
+constexpr int kP2Ahead = kP2Stages - 2;   // panels in flight; one slot of slack so that a producer never waits for
+                                          // the previous producer (which lags by its own issue time)
+constexpr int kP2L2Ahead = 6;           // cell-matrix panels prefetched into L2 beyond the ring
 constexpr int kSyncFlagOffset = 32;     // uint32 index of the first flag inside the sync region (128 bytes)
 
 struct PersistDev {
@@ -401,10 +405,43 @@ struct PersistDev {
   unsigned long long ticket_base;
   uint32_t epoch;
   int n_tiles;
+#ifdef CHFSI_TRACE
+  long long* trace;                         // [grid][64 tiles][2 warps][8] clock64 stamps (debug builds only)
+#endif
 };
+#ifdef CHFSI_TRACE
+#define TRACE_STAMP(slot) do { if (tr) tr[slot] = clock64(); } while (0)
+#define TRACE_ADD(slot, v) do { if (tr) tr[slot] += (v); } while (0)
+#else
+#define TRACE_STAMP(slot) do { } while (0)
+#define TRACE_ADD(slot, v) do { } while (0)
+#endif
 
 __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ uint32_t mbar_test(uint64_t* bar, uint32_t parity) {
+  uint32_t done;
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+      "selp.u32 %0, 1, 0, p;\n"
+      "}\n"
+      : "=r"(done)
+      : "r"(smem_u32(bar)), "r"(parity)
+      : "memory");
+  return done;
+}
+__device__ __forceinline__ void bulk_prefetch_l2(const void* src, uint32_t bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async16(void* dst, const void* src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
+}
+// one pending arrival on `bar` that fires when all earlier cp.async of this thread have landed
+__device__ __forceinline__ void cp_async_arrive(uint64_t* bar) {
+  asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 __device__ __forceinline__ uint32_t ld_acquire_gpu(const uint32_t* p) {
   uint32_t v;
@@ -443,7 +480,7 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<double>
   const double alpha = a.alpha, beta = a.beta, ac = a.ac;
 
   if (tid == 0) {
-    for (int s = 0; s < kP2Stages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], kP2Threads / 32); }
+    for (int s = 0; s < kP2Stages; ++s) { mbar_init(&full[s], 1 + 32); mbar_init(&empty[s], kP2Threads / 32); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     ticket_s[0] = (long long)(atomicAdd(pd.counter, 1ull) - pd.ticket_base);
   }
@@ -453,6 +490,13 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<double>
   for (int iter = 0;; ++iter) {
     const long long ticket = ticket_s[iter & 1];
     if (ticket >= pd.n_tiles) break;
+#ifdef CHFSI_TRACE
+    long long* tr = nullptr;
+    if (pd.trace && lane == 0 && (warp == 0 || warp == 7) && iter < 64)
+      tr = pd.trace + (((long long)blockIdx.x * 64 + iter) * 2 + (warp ? 1 : 0)) * 16;
+    if (tr) { for (int z = 6; z < 16; ++z) tr[z] = 0; }
+    TRACE_STAMP(0);
+#endif
     const int pos = (int)(ticket / nct), jt = (int)(ticket % nct);
     const int cell = pd.pos_cell[pos];
     const int col0 = jt * kP2TileN;
@@ -465,27 +509,72 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<double>
     __syncthreads();
 
     const int npanel = kt / kP2PanelK;
-    const uint32_t row_bytes = (uint32_t)ncols * 8u;
-    const uint32_t panel_bytes = (uint32_t)kP2PanelK * ((uint32_t)lda * 8u + row_bytes);
-    auto issue = [&](int pi) {   // warp 0, all lanes
+#ifdef CHFSI_TRACE
+    long long* tr_p = tr;
+    if (tr) tr[4] = 0;
+#endif
+    auto issue = [&](int pi) {   // one warp, all lanes
       const uint32_t q = q0 + (uint32_t)pi;
       const int s = (int)(q % kP2Stages);
-      mbar_wait(&empty[s], ((q / kP2Stages) & 1u) ^ 1u);
       double* As = stage0 + s * stage_elems;
       double* Xs = As + a_panel_elems;
-      if (lane == 0) mbar_expect_tx(&full[s], panel_bytes);
-      __syncwarp();
-      if (lane < kP2PanelK) {
-        const int k = pi * kP2PanelK + lane;
-        const int idx = idx_s[k];
-        const double* src = (k < mc) ? a.X + (int64_t)(idx & 0x7fffffff) * a.ldx + col0 : a.P + (int64_t)idx * a.ldp + col0;
-        bulk_g2s(Xs + lane * kP2LdXs, src, row_bytes, &full[s]);
-      } else if (lane == kP2PanelK) {
+      // the matrix panel: ONE bulk copy (each UBLKCP costs the SM's copy engine ~200 cycles of service, so the
+      // 8 gathered rows of X do not go through it: they are 16-byte cp.async pieces, 4 per lane)
+#ifdef CHFSI_TRACE
+      long long ti0 = clock64();
+#endif
+      if (lane == 0) {
+        mbar_expect_tx(&full[s], (uint32_t)a_panel_elems * 8u);
         bulk_g2s(As, M + (int64_t)pi * a_panel_elems, (uint32_t)a_panel_elems * 8u, &full[s]);
       }
+#ifdef CHFSI_TRACE
+      long long ti1 = clock64();
+      if (tr_p) tr_p[8] += ti1 - ti0;
+#endif
+      const int chunk = lane & 15;
+      if (chunk * 2 < ncols) {
+#pragma unroll
+        for (int j = 0; j < kP2PanelK / 2; ++j) {
+          const int r = j * 2 + (lane >> 4);
+          const int k = pi * kP2PanelK + r;
+          const int idx = idx_s[k];
+          const double* src = (k < mc) ? a.X + (int64_t)(idx & 0x7fffffff) * a.ldx + col0 : a.P + (int64_t)idx * a.ldp + col0;
+          cp_async16(Xs + r * kP2LdXs + chunk * 2, src + chunk * 2);
+        }
+      }
+#ifdef CHFSI_TRACE
+      long long ti2 = clock64();
+      if (tr_p) tr_p[9] += ti2 - ti1;
+#endif
+      cp_async_arrive(&full[s]);
+#ifdef CHFSI_TRACE
+      if (tr_p) tr_p[10] += clock64() - ti2;
+#endif
     };
-    if (warp == 0)
-      for (int pi = 0; pi < kP2Stages - 1 && pi < npanel; ++pi) issue(pi);
+    TRACE_STAMP(1);
+    // Producer duty rotates over the 8 warps (panel j is issued by warp j % 8 at its iteration j - stages + 1): the
+    // empty-slot wait, the expect_tx / bulk copy / cp.async sequence and the L2 prefetch cost several hundred cycles
+    // per panel, which would make a fixed producer warp the slowest consumer of the ring.
+    auto produce = [&](int pj) {
+      const uint32_t q = q0 + (uint32_t)pj;
+#ifdef CHFSI_TRACE
+      long long te0 = clock64();
+#endif
+      mbar_wait(&empty[q % kP2Stages], ((q / kP2Stages) & 1u) ^ 1u);
+#ifdef CHFSI_TRACE
+      if (tr_p) tr_p[4] += clock64() - te0;
+#endif
+      issue(pj);
+      const int pf = pj + kP2L2Ahead;   // pull a later panel of the cell matrix into L2 ahead of the ring
+#ifdef CHFSI_TRACE
+      long long tp0 = clock64();
+#endif
+      if (lane == 0 && pf < npanel) bulk_prefetch_l2(M + (int64_t)pf * a_panel_elems, (uint32_t)a_panel_elems * 8u);
+#ifdef CHFSI_TRACE
+      if (tr_p) tr_p[11] += clock64() - tp0;
+#endif
+    };
+    if (warp < kP2Ahead && warp < npanel) produce(warp);
 
     const int nt0 = warp_n * 2;
     const int nnt = max(0, min(2, ncols / 8 - nt0));
@@ -499,8 +588,20 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<double>
     for (int pi = 0; pi < npanel; ++pi) {
       const uint32_t q = q0 + (uint32_t)pi;
       const int s = (int)(q % kP2Stages);
-      if (warp == 0 && pi + kP2Stages - 1 < npanel) issue(pi + kP2Stages - 1);
+#ifdef CHFSI_TRACE
+      long long tw0 = tr ? clock64() : 0;
+#endif
+      {
+        const int pj = pi + kP2Ahead;
+        if (pj < npanel && (pj & 7) == warp) produce(pj);
+      }
+#ifdef CHFSI_TRACE
+      long long tw1 = tr ? clock64() : 0;
+#endif
       mbar_wait(&full[s], (q / kP2Stages) & 1u);
+#ifdef CHFSI_TRACE
+      if (tr) { long long tw2 = clock64(); if (pi == 0) tr[2] = tw2; else { tr[6] += tw2 - tw1; } tr[7] += tw1 - tw0; }
+#endif
       if (active) {
         const double* As = stage0 + s * stage_elems;
         const double* Ap = As + fk * lda + mt0 * 8 + fm;
@@ -535,6 +636,7 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<double>
       if (lane == 0) mbar_arrive(&empty[s]);
     }
     q0 += (uint32_t)npanel;
+    TRACE_STAMP(3);
 
     // ---- epilogue: assembly + recurrence (steps 4-5).  C fragment: row = lane/4, columns 2*(lane%4) + {0,1}
     if (!a.atomic) {
@@ -595,8 +697,12 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<double>
         }
       }
     }
+    TRACE_STAMP(5);
     __threadfence();
     __syncthreads();   // all stores of the tile are done and fenced; idx_s / ticket slot may be reused
+#ifdef CHFSI_TRACE
+    if (tr) tr[5] = clock64() - tr[5];   // fence + barrier time
+#endif
     if (tid == 0 && !a.atomic) st_release_gpu(pd.flags + (int64_t)pos * nct + jt, pd.epoch);
   }
 }
@@ -605,6 +711,10 @@ template <typename T>
 size_t pp_smem_bytes(const Op* op) {
   return (size_t)(kPPGroup * op->m_cell + 8 * kPPGroup * kPPCols) * sizeof(T) + (size_t)op->m_cell * sizeof(int32_t);
 }
+
+#ifdef CHFSI_TRACE
+long long* g_trace_buffer = nullptr;
+#endif
 
 size_t p2_smem_bytes(const Op* op) {
   return (size_t)kP2Stages * (kP2PanelK * op->lda + kP2PanelK * kP2LdXs) * sizeof(double) + 2 * kP2Stages * sizeof(uint64_t) +
@@ -687,9 +797,15 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
       pd.flags = reinterpret_cast<uint32_t*>(g.sync) + kSyncFlagOffset;
       pd.epoch = g.epoch;
       const int64_t n_tiles = op->n_cells * a.n_col_tiles;
-      const unsigned grid = (unsigned)std::min<int64_t>(n_tiles, 2 * (int64_t)op->n_sm);
+      unsigned grid = (unsigned)std::min<int64_t>(n_tiles, 2 * (int64_t)op->n_sm);
+#ifdef CHFSI_TRACE
+      if (const char* eg = getenv("CHFSI_DEBUG_GRID")) grid = (unsigned)std::min<int64_t>(n_tiles, atoi(eg));
+#endif
       pd.n_tiles = (int)n_tiles;
       pd.ticket_base = (unsigned long long)(g.epoch - 1) * (unsigned long long)(n_tiles + grid);
+#ifdef CHFSI_TRACE
+      pd.trace = g_trace_buffer;
+#endif
       ApplyDev<double> ad = *reinterpret_cast<ApplyDev<double>*>(&a);
       const size_t sm = p2_smem_bytes(op);
       switch (MT) {
@@ -761,6 +877,10 @@ cudaError_t init_apply_kernels(Op* op) {
   if ((e = cudaFuncSetAttribute(k_apply_generic<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_gen))) return e;
   return cudaSuccess;
 }
+
+#ifdef CHFSI_TRACE
+extern "C" void chfsi_debug_set_trace(long long* dev_buffer) { g_trace_buffer = dev_buffer; }
+#endif
 
 cudaError_t launch_apply(Op* op, const ApplyArgs& a, cudaStream_t stream) {
   return op->precision == 64 ? launch_apply_t<double>(op, a, stream) : launch_apply_t<float>(op, a, stream);
