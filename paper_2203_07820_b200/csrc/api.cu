@@ -47,7 +47,7 @@ void free_op(chfsi_op* op) {
   if (!op) return;
   cudaFree(op->mat); cudaFree(op->mat_off); cudaFree(op->idx_off); cudaFree(op->ktot); cudaFree(op->gidx);
   cudaFree(op->color_cells); cudaFree(op->dep_ptr); cudaFree(op->dep_pos); cudaFree(op->all_cells); cudaFree(op->pc_cells); cudaFree(op->cell_proj_ptr);
-  cudaFree(op->proj_ptr); cudaFree(op->proj_pcrow); cudaFree(op->D); cudaFree(op->mass);
+  cudaFree(op->proj_ptr); cudaFree(op->proj_pcrow); cudaFree(op->D); cudaFree(op->mass); cudaFree(op->diag0);
   for (cudaEvent_t e : op->prof_events) cudaEventDestroy(e);
   delete op;
 }
@@ -211,6 +211,8 @@ int chfsi_create(chfsi_op** out, const chfsi_mesh* mesh, const chfsi_potential* 
   bool bad_jac = false;
   CKC(build_cell_matrices(op, plan, tab, *mesh, *pot, has_nl ? nl : nullptr, st, &bad_jac), "cell-matrix setup");
   if (bad_jac) { free_op(op); return fail(nullptr, CHFSI_ERR_BAD_MESH, "non-positive Jacobian at a quadrature point"); }
+  CKC(cudaMalloc((void**)&op->diag0, (size_t)op->n_cells * op->m_cell * sizeof(double)), "cudaMalloc(diagonal)");
+  CKC(capture_diagonal(op, st), "diagonal capture");
   CKC(init_apply_kernels(op), "kernel attribute setup");
   CKC(cudaStreamSynchronize(st), "sync");
 #undef CKC

@@ -34,7 +34,7 @@ struct ApplyDev {
   T* __restrict__ Tg; int64_t ldt;
   const T* __restrict__ P; int64_t ldp;
   int B;
-  T alpha, beta, ac;                   // ac = alpha * cshift
+  T alpha, beta;                       // T <- alpha (H~ - c) X - beta T ; the shift c sits on the matrix diagonals
   int atomic;                          // 1: red.add into a pre-filled target
 };
 
@@ -83,9 +83,8 @@ __global__ void __launch_bounds__(256) k_apply_generic(ApplyDev<T> a) {
       T v = a.alpha * acc[i];
       if (a.atomic) {
         red_add(tp, v);
-      } else if (idx < 0) {   // first contribution to this dof: carries the recurrence terms
-        if (a.ac != (T)0) v -= a.ac * a.X[g * a.ldx + col];
-        if (a.beta != (T)0) v -= a.beta * *tp;
+      } else if (idx < 0) {   // first contribution to this dof: carries the recurrence term -beta Y_{k-2}
+        if (a.beta != (T)0) v = fma(-a.beta, *tp, v);
         *tp = v;
       } else {
         *tp += v;
@@ -194,18 +193,40 @@ __global__ void __launch_bounds__(128) k_proj_reduce(const T* __restrict__ Pc, c
   P[j * B + col] = s;
 }
 
-// Atomic assembly needs the recurrence terms in place first:  T <- -alpha c X - beta T
+// Atomic assembly needs the recurrence term in place first:  T <- -beta T
 template <typename T>
-__global__ void __launch_bounds__(256) k_prefill(const T* __restrict__ X, int64_t ldx, T* __restrict__ Tg, int64_t ldt,
-                                                 int64_t n_dofs, int B, T ac, T beta) {
+__global__ void __launch_bounds__(256) k_prefill(T* __restrict__ Tg, int64_t ldt, int64_t n_dofs, int B, T beta) {
   int64_t n = n_dofs * B;
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
     int64_t g = i / B; int col = (int)(i % B);
     T v = (T)0;
-    if (ac != (T)0) v -= ac * X[g * ldx + col];
-    if (beta != (T)0) v -= beta * Tg[g * ldt + col];
+    if (beta != (T)0) v = -beta * Tg[g * ldt + col];
     Tg[g * ldt + col] = v;
   }
+}
+
+// The spectral shift c of the filter lives on the diagonals of the cell matrices (common.h, Op::diag0): the
+// (cell, node) that makes the first contribution to a dof carries -c for that dof.
+template <typename T>
+__global__ void __launch_bounds__(256) k_set_diag_shift(T* __restrict__ mat, const int64_t* __restrict__ mat_off,
+                                                        const int64_t* __restrict__ idx_off, const int32_t* __restrict__ gidx,
+                                                        const double* __restrict__ diag0, int m_cell, int lda,
+                                                        int64_t n_cells, double shift) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n_cells * m_cell) return;
+  const int64_t c = i / m_cell;
+  const int k = (int)(i - c * m_cell);
+  const bool first = gidx[idx_off[c] + k] < 0;
+  mat[mat_off[c] + (int64_t)k * lda + k] = (T)(diag0[i] - (first ? shift : 0.0));
+}
+template <typename T>
+__global__ void __launch_bounds__(256) k_capture_diag(const T* __restrict__ mat, const int64_t* __restrict__ mat_off,
+                                                      double* __restrict__ diag0, int m_cell, int lda, int64_t n_cells) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n_cells * m_cell) return;
+  const int64_t c = i / m_cell;
+  const int k = (int)(i - c * m_cell);
+  diag0[i] = (double)mat[mat_off[c] + (int64_t)k * lda + k];
 }
 
 // -------------------------------------------------------------------------------------------------------------
@@ -337,7 +358,7 @@ __global__ void __launch_bounds__(512, 1) k_apply_dmma(ApplyDev<double> a) {
   }
 
   // epilogue: assembly + recurrence (steps 4-5).  C fragment: row = lane/4, columns 2*(lane%4) + {0,1}
-  const double alpha = a.alpha, beta = a.beta, ac = a.ac;
+  const double alpha = a.alpha, beta = a.beta;
 #pragma unroll
   for (int i = 0; i < MT; ++i) {
     if (i >= nmt) continue;
@@ -355,13 +376,9 @@ __global__ void __launch_bounds__(512, 1) k_apply_dmma(ApplyDev<double> a) {
         atomicAdd(&tp->x, v0);
         atomicAdd(&tp->y, v1);
       } else if (idx < 0) {
-        if (ac != 0.0) {
-          double2 x = *reinterpret_cast<const double2*>(a.X + g * a.ldx + col);
-          v0 -= ac * x.x; v1 -= ac * x.y;
-        }
         if (beta != 0.0) {
           double2 t = *tp;
-          v0 -= beta * t.x; v1 -= beta * t.y;
+          v0 = fma(-beta, t.x, v0); v1 = fma(-beta, t.y, v1);
         }
         *tp = make_double2(v0, v1);
       } else {
@@ -406,7 +423,8 @@ struct PersistDev {
   uint32_t epoch;
   int n_tiles;
 #ifdef CHFSI_TRACE
-  long long* trace;                         // [grid][64 tiles][2 warps][8] clock64 stamps (debug builds only)
+  long long* trace;                         // [grid][64 tiles][2 warps][16] clock64 stamps (debug builds only)
+  int debug_flags;                          // bit 0: skip the epilogue (timing experiments only; results are wrong)
 #endif
 };
 #ifdef CHFSI_TRACE
@@ -477,7 +495,7 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<double>
   const int n_mtiles = (mc + 7) / 8;
   const int mt0 = warp_m * MT;
   const int nmt = max(0, min(MT, n_mtiles - mt0));
-  const double alpha = a.alpha, beta = a.beta, ac = a.ac;
+  const double alpha = a.alpha, beta = a.beta;
 
   if (tid == 0) {
     for (int s = 0; s < kP2Stages; ++s) { mbar_init(&full[s], 1 + 32); mbar_init(&empty[s], kP2Threads / 32); }
@@ -505,7 +523,14 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<double>
     const int32_t* gi = a.gidx + a.idx_off[cell];
     const double* M = a.mat + a.mat_off[cell];
     if (tid == 0) ticket_s[(iter + 1) & 1] = (long long)(atomicAdd(pd.counter, 1ull) - pd.ticket_base);
-    for (int k = tid; k < kt; k += kP2Threads) idx_s[k] = gi[k];
+    for (int k = tid; k < kt; k += kP2Threads) {
+      const int idx = gi[k];
+      idx_s[k] = idx;
+      // the epilogue reads Y_{k-2} only where this tile makes the first contribution: pull those row segments
+      // into L2 now, a whole main loop ahead of their use
+      if (idx < 0 && k < mc && beta != 0.0 && !a.atomic)
+        bulk_prefetch_l2(a.Tg + (int64_t)(idx & 0x7fffffff) * a.ldt + col0, (uint32_t)ncols * 8u);
+    }
     __syncthreads();
 
     const int npanel = kt / kP2PanelK;
@@ -639,7 +664,12 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<double>
     TRACE_STAMP(3);
 
     // ---- epilogue: assembly + recurrence (steps 4-5).  C fragment: row = lane/4, columns 2*(lane%4) + {0,1}
-    if (!a.atomic) {
+#ifdef CHFSI_TRACE
+    const bool skip_epi = (pd.debug_flags & 1) != 0;
+#else
+    constexpr bool skip_epi = false;
+#endif
+    if (!a.atomic && !skip_epi) {
       const int d1 = pd.dep_ptr[pos + 1];
       for (int d = pd.dep_ptr[pos] + lane; d < d1; d += 32) {
         const uint32_t* f = pd.flags + (int64_t)pd.dep_pos[d] * nct + jt;
@@ -647,11 +677,14 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<double>
       }
       __syncwarp();
     }
-    if (active) {
-      constexpr int G = 2;   // m-tiles per batch: all loads of a batch are issued before its stores
+    TRACE_STAMP(12);
+    if (active && !skip_epi) {
+      // first contribution to a dof: T <- alpha acc - beta T (T holds Y_{k-2}); later contributions are added by
+      // red.global.add.f64 (fire and forget: no load, no register staging); their order is fixed by the flags.
+      constexpr int G = 4;   // m-tiles per batch: all loads of a batch are issued before its stores
 #pragma unroll
       for (int i0 = 0; i0 < MT; i0 += G) {
-        double2 tv[G][2], xv[G][2];
+        double2 tv[G][2];
         int64_t gg[G];
         bool first[G], ok[G];
 #pragma unroll
@@ -665,11 +698,8 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<double>
 #pragma unroll
           for (int j = 0; j < 2; ++j) {
             tv[u][j] = make_double2(0.0, 0.0);
-            xv[u][j] = make_double2(0.0, 0.0);
-            if (!ok[u] || j >= nnt || a.atomic) continue;
-            const int col = col0 + (nt0 + j) * 8 + fk * 2;
-            if (!first[u] || beta != 0.0) tv[u][j] = ld_cg_d2(a.Tg + gg[u] * a.ldt + col);
-            if (first[u] && ac != 0.0) xv[u][j] = *reinterpret_cast<const double2*>(a.X + gg[u] * a.ldx + col);
+            if (!ok[u] || j >= nnt || a.atomic || !first[u] || beta == 0.0) continue;
+            tv[u][j] = ld_cg_d2(a.Tg + gg[u] * a.ldt + col0 + (nt0 + j) * 8 + fk * 2);
           }
         }
 #pragma unroll
@@ -682,27 +712,21 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<double>
             if (j >= nnt) continue;
             const int col = col0 + (nt0 + j) * 8 + fk * 2;
             double* tp = a.Tg + gg[u] * a.ldt + col;
-            double v0 = alpha * acc[i][j][0], v1 = alpha * acc[i][j][1];
-            if (a.atomic) {
+            const double v0 = alpha * acc[i][j][0], v1 = alpha * acc[i][j][1];
+            if (a.atomic || !first[u]) {
               atomicAdd(tp, v0);
               atomicAdd(tp + 1, v1);
-            } else if (first[u]) {
-              v0 = (v0 - ac * xv[u][j].x) - beta * tv[u][j].x;
-              v1 = (v1 - ac * xv[u][j].y) - beta * tv[u][j].y;
-              *reinterpret_cast<double2*>(tp) = make_double2(v0, v1);
             } else {
-              *reinterpret_cast<double2*>(tp) = make_double2(tv[u][j].x + v0, tv[u][j].y + v1);
+              *reinterpret_cast<double2*>(tp) = make_double2(fma(-beta, tv[u][j].x, v0), fma(-beta, tv[u][j].y, v1));
             }
           }
         }
       }
     }
-    TRACE_STAMP(5);
+    TRACE_STAMP(13);
     __threadfence();
     __syncthreads();   // all stores of the tile are done and fenced; idx_s / ticket slot may be reused
-#ifdef CHFSI_TRACE
-    if (tr) tr[5] = clock64() - tr[5];   // fence + barrier time
-#endif
+    TRACE_STAMP(14);
     if (tid == 0 && !a.atomic) st_release_gpu(pd.flags + (int64_t)pos * nct + jt, pd.epoch);
   }
 }
@@ -743,6 +767,14 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
     op->prof_used += 3;
     cudaEventRecord(ev[0], st);
   }
+  if (g.cshift != op->cur_shift) {   // once per filter call: move the spectral shift onto the matrix diagonals
+    const int64_t n = op->n_cells * op->m_cell;
+    k_set_diag_shift<T><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(reinterpret_cast<T*>(op->mat), op->mat_off, op->idx_off,
+                                                                    op->gidx, op->diag0, op->m_cell, op->lda, op->n_cells,
+                                                                    g.cshift);
+    op->cur_shift = g.cshift;
+    op->launches++;
+  }
   const int64_t launches_before = op->launches;
   // steps 3a-3c
   if (op->n_proj > 0) {
@@ -762,7 +794,7 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
   a.mat = mat; a.mat_off = op->mat_off; a.idx_off = op->idx_off; a.ktot = op->ktot; a.gidx = op->gidx;
   a.m_cell = op->m_cell; a.lda = op->lda;
   a.X = X; a.ldx = g.ldx; a.Tg = Tg; a.ldt = g.ldt; a.P = P; a.ldp = B; a.B = B;
-  a.alpha = (T)g.alpha; a.beta = (T)g.beta; a.ac = (T)(g.alpha * g.cshift);
+  a.alpha = (T)g.alpha; a.beta = (T)g.beta;
   a.atomic = op->assembly;
 
   const bool aligned = sizeof(T) == 8 && B % 8 == 0 && g.ldx % 2 == 0 && g.ldt % 2 == 0 && ((uintptr_t)g.X % 16 == 0) &&
@@ -779,7 +811,7 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
   if (fast && smem_fast > 227 * 1024) fast = false;
 
   if (op->assembly == 1) {
-    k_prefill<T><<<148 * 8, 256, 0, st>>>(X, g.ldx, Tg, g.ldt, op->n_dofs, B, a.ac, a.beta);
+    k_prefill<T><<<148 * 8, 256, 0, st>>>(Tg, g.ldt, op->n_dofs, B, a.beta);
     op->launches++;
   }
   if (op->profiling) {
@@ -805,6 +837,7 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
       pd.ticket_base = (unsigned long long)(g.epoch - 1) * (unsigned long long)(n_tiles + grid);
 #ifdef CHFSI_TRACE
       pd.trace = g_trace_buffer;
+      pd.debug_flags = getenv("CHFSI_DEBUG_FLAGS") ? atoi(getenv("CHFSI_DEBUG_FLAGS")) : 0;
 #endif
       ApplyDev<double> ad = *reinterpret_cast<ApplyDev<double>*>(&a);
       const size_t sm = p2_smem_bytes(op);
@@ -881,6 +914,19 @@ cudaError_t init_apply_kernels(Op* op) {
 #ifdef CHFSI_TRACE
 extern "C" void chfsi_debug_set_trace(long long* dev_buffer) { g_trace_buffer = dev_buffer; }
 #endif
+
+cudaError_t capture_diagonal(Op* op, cudaStream_t st) {
+  const int64_t n = op->n_cells * op->m_cell;
+  const unsigned grid = (unsigned)((n + 255) / 256);
+  if (op->precision == 64)
+    k_capture_diag<double><<<grid, 256, 0, st>>>(reinterpret_cast<const double*>(op->mat), op->mat_off, op->diag0, op->m_cell,
+                                                 op->lda, op->n_cells);
+  else
+    k_capture_diag<float><<<grid, 256, 0, st>>>(reinterpret_cast<const float*>(op->mat), op->mat_off, op->diag0, op->m_cell,
+                                                op->lda, op->n_cells);
+  op->cur_shift = 0.0;
+  return cudaGetLastError();
+}
 
 cudaError_t launch_apply(Op* op, const ApplyArgs& a, cudaStream_t stream) {
   return op->precision == 64 ? launch_apply_t<double>(op, a, stream) : launch_apply_t<float>(op, a, stream);

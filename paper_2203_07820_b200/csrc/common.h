@@ -89,6 +89,12 @@ struct Op {
   int64_t* proj_pcrow = nullptr;
   double* D = nullptr;
   double* mass = nullptr;
+  // Spectral shift folded into the cell matrices: diag0 [n_cells][m_cell] keeps the unshifted diagonal entries
+  // mat[c][k][k]; while a filter runs, the diagonal entry of the (cell, node) that makes the FIRST contribution
+  // to its dof holds diag0 - cur_shift, so that the contraction itself yields (H~ - c I) X  (Eq. 37's
+  // "c1 H~ + c2") and the recurrence epilogue never re-reads X.
+  double* diag0 = nullptr;
+  double cur_shift = 0.0;
   int64_t launches = 0;
   // optional per-kernel timing (chfsi_set_profiling): event triples (start, after projector kernels, end)
   bool profiling = false;
@@ -121,6 +127,8 @@ struct ApplyArgs {
 };
 // Enqueues one fused H~ application + recurrence update.  Returns cudaGetLastError().
 cudaError_t launch_apply(Op* op, const ApplyArgs& a, cudaStream_t stream);
+// Copies the diagonal of every cell matrix into op->diag0 (once, at create, after build_cell_matrices).
+cudaError_t capture_diagonal(Op* op, cudaStream_t stream);
 // Opts the kernels into the shared memory they need for this operator (once, at create).
 cudaError_t init_apply_kernels(Op* op);
 
