@@ -454,6 +454,7 @@ __device__ __forceinline__ uint32_t mbar_test(uint64_t* bar, uint32_t parity) {
 __device__ __forceinline__ void bulk_prefetch_l2(const void* src, uint32_t bytes) {
   asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 __device__ __forceinline__ void cp_async16(void* dst, const void* src) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
 }
@@ -523,13 +524,10 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<double>
     const int32_t* gi = a.gidx + a.idx_off[cell];
     const double* M = a.mat + a.mat_off[cell];
     if (tid == 0) ticket_s[(iter + 1) & 1] = (long long)(atomicAdd(pd.counter, 1ull) - pd.ticket_base);
+    const bool use_t = (beta != 0.0) && !a.atomic;   // the -beta Y_{k-2} term seeds the accumulators (below)
     for (int k = tid; k < kt; k += kP2Threads) {
       const int idx = gi[k];
       idx_s[k] = idx;
-      // the epilogue reads Y_{k-2} only where this tile makes the first contribution: pull those row segments
-      // into L2 now, a whole main loop ahead of their use
-      if (idx < 0 && k < mc && beta != 0.0 && !a.atomic)
-        bulk_prefetch_l2(a.Tg + (int64_t)(idx & 0x7fffffff) * a.ldt + col0, (uint32_t)ncols * 8u);
     }
     __syncthreads();
 
@@ -603,13 +601,33 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<double>
 
     const int nt0 = warp_n * 2;
     const int nnt = max(0, min(2, ncols / 8 - nt0));
+    const bool active = (nnt > 0 && nmt > 0);
+    // Recurrence term -beta Y_{k-2} (Eq. 37): the accumulators of the first-contribution nodes START at
+    // (-beta/alpha) Y_{k-2} (the target block still holds Y_{k-2}); the loads land straight in the accumulator
+    // registers while the first panels are in flight, and the epilogue has no loads left.
     double acc[MT][2][2];
 #pragma unroll
     for (int i = 0; i < MT; ++i)
 #pragma unroll
       for (int j = 0; j < 2; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
-
-    const bool active = (nnt > 0 && nmt > 0);
+    if (use_t && active) {
+      const double nb = -beta / alpha;
+#pragma unroll
+      for (int i = 0; i < MT; ++i) {
+        const int r = (mt0 + i) * 8 + fm;
+        const int idx = (i < nmt && r < mc) ? idx_s[r] : 0;
+        if (idx < 0) {
+          const double* tp = a.Tg + (int64_t)(idx & 0x7fffffff) * a.ldt + col0 + nt0 * 8 + fk * 2;
+          const double2 u = ld_cg_d2(tp);
+          acc[i][0][0] = u.x; acc[i][0][1] = u.y;
+          if (nnt > 1) { const double2 v = ld_cg_d2(tp + 8); acc[i][1][0] = v.x; acc[i][1][1] = v.y; }
+        }
+      }
+#pragma unroll
+      for (int i = 0; i < MT; ++i)
+#pragma unroll
+        for (int j = 0; j < 2; ++j) { acc[i][j][0] *= nb; acc[i][j][1] *= nb; }
+    }
     for (int pi = 0; pi < npanel; ++pi) {
       const uint32_t q = q0 + (uint32_t)pi;
       const int s = (int)(q % kP2Stages);
@@ -679,46 +697,24 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<double>
     }
     TRACE_STAMP(12);
     if (active && !skip_epi) {
-      // first contribution to a dof: T <- alpha acc - beta T (T holds Y_{k-2}); later contributions are added by
-      // red.global.add.f64 (fire and forget: no load, no register staging); their order is fixed by the flags.
-      constexpr int G = 4;   // m-tiles per batch: all loads of a batch are issued before its stores
+      // first contribution to a dof: plain store of alpha acc (the -beta Y_{k-2} term is already in acc); later
+      // contributions: red.global.add.f64 (fire and forget); their order is fixed by the completion flags.
 #pragma unroll
-      for (int i0 = 0; i0 < MT; i0 += G) {
-        double2 tv[G][2];
-        int64_t gg[G];
-        bool first[G], ok[G];
+      for (int i = 0; i < MT; ++i) {
+        const int r = (mt0 + i) * 8 + fm;
+        if (i >= nmt || r >= mc) continue;
+        const int idx = idx_s[r];
+        double* trow = a.Tg + (int64_t)(idx & 0x7fffffff) * a.ldt + col0 + nt0 * 8 + fk * 2;
+        const bool add = a.atomic || idx >= 0;
 #pragma unroll
-        for (int u = 0; u < G; ++u) {
-          const int i = i0 + u;
-          const int r = (mt0 + i) * 8 + fm;
-          ok[u] = (i < MT) && (i < nmt) && (r < mc);
-          const int idx = ok[u] ? idx_s[r] : 0;
-          gg[u] = idx & 0x7fffffff;
-          first[u] = idx < 0;
-#pragma unroll
-          for (int j = 0; j < 2; ++j) {
-            tv[u][j] = make_double2(0.0, 0.0);
-            if (!ok[u] || j >= nnt || a.atomic || !first[u] || beta == 0.0) continue;
-            tv[u][j] = ld_cg_d2(a.Tg + gg[u] * a.ldt + col0 + (nt0 + j) * 8 + fk * 2);
-          }
-        }
-#pragma unroll
-        for (int u = 0; u < G; ++u) {
-          const int i = i0 + u;
-          if (i >= MT) continue;
-          if (!ok[u]) continue;
-#pragma unroll
-          for (int j = 0; j < 2; ++j) {
-            if (j >= nnt) continue;
-            const int col = col0 + (nt0 + j) * 8 + fk * 2;
-            double* tp = a.Tg + gg[u] * a.ldt + col;
-            const double v0 = alpha * acc[i][j][0], v1 = alpha * acc[i][j][1];
-            if (a.atomic || !first[u]) {
-              atomicAdd(tp, v0);
-              atomicAdd(tp + 1, v1);
-            } else {
-              *reinterpret_cast<double2*>(tp) = make_double2(fma(-beta, tv[u][j].x, v0), fma(-beta, tv[u][j].y, v1));
-            }
+        for (int j = 0; j < 2; ++j) {
+          if (j >= nnt) continue;
+          const double v0 = alpha * acc[i][j][0], v1 = alpha * acc[i][j][1];
+          if (add) {
+            atomicAdd(trow + j * 8, v0);
+            atomicAdd(trow + j * 8 + 1, v1);
+          } else {
+            *reinterpret_cast<double2*>(trow + j * 8) = make_double2(v0, v1);
           }
         }
       }
