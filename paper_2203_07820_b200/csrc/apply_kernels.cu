@@ -13,6 +13,8 @@
 #include <cstdio>
 #include <cstdlib>
 
+#include <cuda.h>   // CUtensorMap (types only; the encoder is fetched through cudaGetDriverEntryPoint)
+
 #include "common.h"
 
 namespace chfsi {
@@ -29,7 +31,7 @@ struct ApplyDev {
   const int32_t* __restrict__ cells;   // cells of this launch
   int n_launch_cells;
   int n_col_tiles;
-  int m_cell, lda;
+  int m_cell, mpad, lda;               // mpad = round8(m_cell): projector rows of the contraction start there
   const T* __restrict__ X; int64_t ldx;
   T* __restrict__ Tg; int64_t ldt;
   const T* __restrict__ P; int64_t ldp;
@@ -57,7 +59,7 @@ __global__ void __launch_bounds__(256) k_apply_generic(ApplyDev<T> a) {
   const bool colok = col < a.B;
   for (int k = warp; k < kt; k += 8) {
     int idx = gi[k];
-    const T* src = (k < mc) ? a.X + (int64_t)(idx & 0x7fffffff) * a.ldx : a.P + (int64_t)idx * a.ldp;
+    const T* src = (k < a.mpad) ? a.X + (int64_t)(idx & 0x7fffffff) * a.ldx : a.P + (int64_t)idx * a.ldp;
     Xs[k * 32 + lane] = colok ? src[col] : (T)0;
   }
   __syncthreads();
@@ -120,7 +122,7 @@ __global__ void __launch_bounds__(256) k_proj_partial(const T* __restrict__ mat,
   for (int l = tid; l < m_cell; l += 256) dofs[l] = gi[l] & 0x7fffffff;
   const int64_t r0 = cell_proj_ptr[cell];
   const int np = (int)(cell_proj_ptr[cell + 1] - r0);
-  const T* C = mat + mat_off[cell] + (int64_t)m_cell * lda;   // rows = projectors of this cell, columns = nodes
+  const T* C = mat + mat_off[cell] + (int64_t)((m_cell + 7) / 8 * 8) * lda;   // rows = projectors of this cell, columns = nodes
   const int col = col0 + cq;
   const bool full4 = vec_ok && (col + 3 < B);
   for (int i0 = 0; i0 < np; i0 += kPPGroup) {
@@ -309,7 +311,7 @@ __global__ void __launch_bounds__(512, 1) k_apply_dmma(ApplyDev<double> a) {
     if (lane < rows) {
       const int k = pi * kPanelK + lane;
       const int idx = idx_s[k];
-      const double* src = (k < mc) ? a.X + (int64_t)(idx & 0x7fffffff) * a.ldx + col0 : a.P + (int64_t)idx * a.ldp + col0;
+      const double* src = (k < a.mpad) ? a.X + (int64_t)(idx & 0x7fffffff) * a.ldx + col0 : a.P + (int64_t)idx * a.ldp + col0;
       bulk_g2s(Xs + lane * kLdXs, src, row_bytes, &full[s]);
     } else if (lane == 16) {
       bulk_g2s(As, M + (int64_t)pi * a_panel_elems, (uint32_t)rows * (uint32_t)lda * 8u, &full[s]);
@@ -399,13 +401,15 @@ __global__ void __launch_bounds__(512, 1) k_apply_dmma(ApplyDev<double> a) {
 //            tile only), so every dof is assembled in colour order -> bit-reproducible, with no launch boundary
 //            and no wave tail between colours.  A ticket holder only ever waits on lower tickets, all of which
 //            are held by running CTAs: no deadlock.
-//   stream = 8-row K-panels of the cell matrix (one bulk copy) + the 8 gathered rows of X (one bulk copy each)
-//            land on a "full" mbarrier of a 4-stage ring; warps release a stage through an "empty" mbarrier as
-//            soon as their fragments are in registers.
+//   stream = 8-row K-panels of the cell matrix (one bulk copy, UBLKCP) + the 8 matching rows of X gathered through
+//            the cell->dof map by two TMA row gathers (cp.async.bulk.tensor.2d.tile::gather4, UTMALDG.2D.GATHER4:
+//            four arbitrary rows of the [n_dofs x B] block per instruction) land on a "full" mbarrier of a
+//            4-stage ring; ONE lane issues the three copies of a panel, nobody touches the data on the way;
+//            warps release a stage through an "empty" mbarrier as soon as their fragments are in registers.
 // -------------------------------------------------------------------------------------------------------------
 constexpr int kP2PanelK = 8;
 constexpr int kP2TileN = 32;
-constexpr int kP2LdXs = kP2TileN + 4;   // 36: 36 mod 16 == 4 -> conflict-free 64-bit fragment loads
+constexpr int kP2LdXs = kP2TileN;       // the TMA row gather packs the rows densely (256 B each)
 constexpr int kP2Stages = 4;
 constexpr int kP2Threads = 256;
 constexpr int kP2Ahead = kP2Stages - 2;   // panels in flight; one slot of slack so that a producer never waits for
@@ -438,29 +442,16 @@ struct PersistDev {
 __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
-__device__ __forceinline__ uint32_t mbar_test(uint64_t* bar, uint32_t parity) {
-  uint32_t done;
-  asm volatile(
-      "{\n"
-      ".reg .pred p;\n"
-      "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n"
-      "selp.u32 %0, 1, 0, p;\n"
-      "}\n"
-      : "=r"(done)
-      : "r"(smem_u32(bar)), "r"(parity)
-      : "memory");
-  return done;
-}
 __device__ __forceinline__ void bulk_prefetch_l2(const void* src, uint32_t bytes) {
   asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
-__device__ __forceinline__ void cp_async16(void* dst, const void* src) {
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
-}
-// one pending arrival on `bar` that fires when all earlier cp.async of this thread have landed
-__device__ __forceinline__ void cp_async_arrive(uint64_t* bar) {
-  asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+// four rows r0..r3 of a 2-D tensor (columns c0 .. c0+box-1) -> four consecutive box-wide rows at dst
+__device__ __forceinline__ void tma_gather4(void* dst, const CUtensorMap* tm, int c0, int r0, int r1, int r2, int r3,
+                                            uint64_t* bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.tile::gather4.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6, %7}], [%2];"
+      ::"r"(smem_u32(dst)), "l"(tm), "r"(smem_u32(bar)), "r"(c0), "r"(r0), "r"(r1), "r"(r2), "r"(r3)
+      : "memory");
 }
 __device__ __forceinline__ uint32_t ld_acquire_gpu(const uint32_t* p) {
   uint32_t v;
@@ -477,7 +468,9 @@ __device__ __forceinline__ double2 ld_cg_d2(const double* p) {
 }
 
 template <int MT>
-__global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<double> a, PersistDev pd) {
+__global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<double> a, PersistDev pd,
+                                                                const __grid_constant__ CUtensorMap tmX,
+                                                                const __grid_constant__ CUtensorMap tmP) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int lda = a.lda;
   const int a_panel_elems = kP2PanelK * lda;
@@ -499,7 +492,7 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<double>
   const double alpha = a.alpha, beta = a.beta;
 
   if (tid == 0) {
-    for (int s = 0; s < kP2Stages; ++s) { mbar_init(&full[s], 1 + 32); mbar_init(&empty[s], kP2Threads / 32); }
+    for (int s = 0; s < kP2Stages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], kP2Threads / 32); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     ticket_s[0] = (long long)(atomicAdd(pd.counter, 1ull) - pd.ticket_base);
   }
@@ -536,65 +529,36 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<double>
     long long* tr_p = tr;
     if (tr) tr[4] = 0;
 #endif
-    auto issue = [&](int pi) {   // one warp, all lanes
-      const uint32_t q = q0 + (uint32_t)pi;
-      const int s = (int)(q % kP2Stages);
-      double* As = stage0 + s * stage_elems;
-      double* Xs = As + a_panel_elems;
-      // the matrix panel: ONE bulk copy (each UBLKCP costs the SM's copy engine ~200 cycles of service, so the
-      // 8 gathered rows of X do not go through it: they are 16-byte cp.async pieces, 4 per lane)
-#ifdef CHFSI_TRACE
-      long long ti0 = clock64();
-#endif
-      if (lane == 0) {
-        mbar_expect_tx(&full[s], (uint32_t)a_panel_elems * 8u);
-        bulk_g2s(As, M + (int64_t)pi * a_panel_elems, (uint32_t)a_panel_elems * 8u, &full[s]);
-      }
-#ifdef CHFSI_TRACE
-      long long ti1 = clock64();
-      if (tr_p) tr_p[8] += ti1 - ti0;
-#endif
-      const int chunk = lane & 15;
-      if (chunk * 2 < ncols) {
-#pragma unroll
-        for (int j = 0; j < kP2PanelK / 2; ++j) {
-          const int r = j * 2 + (lane >> 4);
-          const int k = pi * kP2PanelK + r;
-          const int idx = idx_s[k];
-          const double* src = (k < mc) ? a.X + (int64_t)(idx & 0x7fffffff) * a.ldx + col0 : a.P + (int64_t)idx * a.ldp + col0;
-          cp_async16(Xs + r * kP2LdXs + chunk * 2, src + chunk * 2);
-        }
-      }
-#ifdef CHFSI_TRACE
-      long long ti2 = clock64();
-      if (tr_p) tr_p[9] += ti2 - ti1;
-#endif
-      cp_async_arrive(&full[s]);
-#ifdef CHFSI_TRACE
-      if (tr_p) tr_p[10] += clock64() - ti2;
-#endif
-    };
     TRACE_STAMP(1);
-    // Producer duty rotates over the 8 warps (panel j is issued by warp j % 8 at its iteration j - stages + 1): the
-    // empty-slot wait, the expect_tx / bulk copy / cp.async sequence and the L2 prefetch cost several hundred cycles
-    // per panel, which would make a fixed producer warp the slowest consumer of the ring.
+    // Producer duty rotates over the 8 warps (panel j is issued by lane 0 of warp j % 8, kP2Ahead iterations ahead):
+    // wait for the ring slot, then one expect_tx, one bulk copy (matrix panel) and two TMA row gathers (X or P rows).
     auto produce = [&](int pj) {
+      if (lane != 0) return;
       const uint32_t q = q0 + (uint32_t)pj;
+      const int s = (int)(q % kP2Stages);
 #ifdef CHFSI_TRACE
       long long te0 = clock64();
 #endif
-      mbar_wait(&empty[q % kP2Stages], ((q / kP2Stages) & 1u) ^ 1u);
+      mbar_wait(&empty[s], ((q / kP2Stages) & 1u) ^ 1u);
 #ifdef CHFSI_TRACE
-      if (tr_p) tr_p[4] += clock64() - te0;
+      long long te1 = clock64();
+      if (tr_p) tr_p[4] += te1 - te0;
 #endif
-      issue(pj);
+      double* As = stage0 + s * stage_elems;
+      double* Xs = As + a_panel_elems;
+      const uint32_t a_bytes = (uint32_t)a_panel_elems * 8u;
+      mbar_expect_tx(&full[s], a_bytes + (uint32_t)(kP2PanelK * kP2LdXs * 8));
+      bulk_g2s(As, M + (int64_t)pj * a_panel_elems, a_bytes, &full[s]);
+      const int k0 = pj * kP2PanelK;
+      const CUtensorMap* tm = (k0 < a.mpad) ? &tmX : &tmP;
+      tma_gather4(Xs, tm, col0, idx_s[k0] & 0x7fffffff, idx_s[k0 + 1] & 0x7fffffff, idx_s[k0 + 2] & 0x7fffffff,
+                  idx_s[k0 + 3] & 0x7fffffff, &full[s]);
+      tma_gather4(Xs + 4 * kP2LdXs, tm, col0, idx_s[k0 + 4] & 0x7fffffff, idx_s[k0 + 5] & 0x7fffffff,
+                  idx_s[k0 + 6] & 0x7fffffff, idx_s[k0 + 7] & 0x7fffffff, &full[s]);
       const int pf = pj + kP2L2Ahead;   // pull a later panel of the cell matrix into L2 ahead of the ring
+      if (pf < npanel) bulk_prefetch_l2(M + (int64_t)pf * a_panel_elems, a_bytes);
 #ifdef CHFSI_TRACE
-      long long tp0 = clock64();
-#endif
-      if (lane == 0 && pf < npanel) bulk_prefetch_l2(M + (int64_t)pf * a_panel_elems, (uint32_t)a_panel_elems * 8u);
-#ifdef CHFSI_TRACE
-      if (tr_p) tr_p[11] += clock64() - tp0;
+      if (tr_p) tr_p[8] += clock64() - te1;
 #endif
     };
     if (warp < kP2Ahead && warp < npanel) produce(warp);
@@ -727,6 +691,34 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<double>
   }
 }
 
+// Tensor map of a row-major FP64 block [rows][ld] restricted to its first `cols` columns, box = kP2TileN x 1
+// (tile::gather4 picks four such rows per instruction); columns beyond `cols` read as zero.
+using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_tiled_fn() {
+  static EncodeTiledFn fn = [] {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess)
+      p = nullptr;
+    return reinterpret_cast<EncodeTiledFn>(p);
+  }();
+  return fn;
+}
+bool make_row_gather_map(CUtensorMap* tm, const void* base, int64_t rows, int64_t cols, int64_t ld) {
+  EncodeTiledFn enc = encode_tiled_fn();
+  if (!enc || rows < 1 || cols < 1 || (ld * 8) % 16 != 0 || (uintptr_t)base % 16 != 0) return false;
+  const cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
+  const cuuint64_t strides[1] = {(cuuint64_t)ld * 8};
+  const cuuint32_t box[2] = {(cuuint32_t)kP2TileN, 1};
+  const cuuint32_t estr[2] = {1, 1};
+  return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<void*>(base), dims, strides, box, estr,
+             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 template <typename T>
 size_t pp_smem_bytes(const Op* op) {
   return (size_t)(kPPGroup * op->m_cell + 8 * kPPGroup * kPPCols) * sizeof(T) + (size_t)op->m_cell * sizeof(int32_t);
@@ -788,7 +780,7 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
   }
   ApplyDev<T> a;
   a.mat = mat; a.mat_off = op->mat_off; a.idx_off = op->idx_off; a.ktot = op->ktot; a.gidx = op->gidx;
-  a.m_cell = op->m_cell; a.lda = op->lda;
+  a.m_cell = op->m_cell; a.mpad = op->mpad; a.lda = op->lda;
   a.X = X; a.ldx = g.ldx; a.Tg = Tg; a.ldt = g.ldt; a.P = P; a.ldp = B; a.B = B;
   a.alpha = (T)g.alpha; a.beta = (T)g.beta;
   a.atomic = op->assembly;
@@ -799,8 +791,10 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
   // variant 0: persistent single-launch kernel (v2); variant 2: one launch per colour (v1); variant 1: generic
   bool fast2 = false, fast = false;
   int MT = (n_mtiles + 3) / 4;
+  CUtensorMap tmX, tmP;
   if (aligned && op->variant == 0 && g.sync != nullptr && g.epoch > 0)
-    fast2 = (MT == 11 || MT == 7 || MT == 4 || MT == 2 || MT == 1) && p2_smem_bytes(op) <= 113 * 1024;
+    fast2 = (MT == 11 || MT == 7 || MT == 4 || MT == 2 || MT == 1) && p2_smem_bytes(op) <= 113 * 1024 &&
+            make_row_gather_map(&tmX, g.X, op->n_dofs, B, g.ldx) && make_row_gather_map(&tmP, g.P, op->n_proj + 1, B, B);
   if (aligned && !fast2 && op->variant != 1) fast = (MT == 11 || MT == 4 || MT == 2 || MT == 7);
   size_t smem_fast = (size_t)kStages * (kPanelK * op->lda + kPanelK * kLdXs) * sizeof(double) + kStages * sizeof(uint64_t) +
                      (size_t)op->max_ktot * sizeof(int32_t);
@@ -838,11 +832,11 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
       ApplyDev<double> ad = *reinterpret_cast<ApplyDev<double>*>(&a);
       const size_t sm = p2_smem_bytes(op);
       switch (MT) {
-        case 11: k_apply_dmma_p<11><<<grid, kP2Threads, sm, st>>>(ad, pd); break;
-        case 7: k_apply_dmma_p<7><<<grid, kP2Threads, sm, st>>>(ad, pd); break;
-        case 4: k_apply_dmma_p<4><<<grid, kP2Threads, sm, st>>>(ad, pd); break;
-        case 2: k_apply_dmma_p<2><<<grid, kP2Threads, sm, st>>>(ad, pd); break;
-        case 1: k_apply_dmma_p<1><<<grid, kP2Threads, sm, st>>>(ad, pd); break;
+        case 11: k_apply_dmma_p<11><<<grid, kP2Threads, sm, st>>>(ad, pd, tmX, tmP); break;
+        case 7: k_apply_dmma_p<7><<<grid, kP2Threads, sm, st>>>(ad, pd, tmX, tmP); break;
+        case 4: k_apply_dmma_p<4><<<grid, kP2Threads, sm, st>>>(ad, pd, tmX, tmP); break;
+        case 2: k_apply_dmma_p<2><<<grid, kP2Threads, sm, st>>>(ad, pd, tmX, tmP); break;
+        case 1: k_apply_dmma_p<1><<<grid, kP2Threads, sm, st>>>(ad, pd, tmX, tmP); break;
       }
       op->launches++;
     }

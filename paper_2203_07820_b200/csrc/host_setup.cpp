@@ -259,12 +259,16 @@ std::string analyse_mesh(const chfsi_mesh& mesh, const chfsi_nonlocal* nl, const
     if (plan->cell_proj_ptr[c + 1] > plan->cell_proj_ptr[c]) plan->pc_cells.push_back((int32_t)c);
 
   // ---- per-cell layout: K_c, matrix offsets, gather/scatter index lists with first-contribution flags --------
+  // rows 0..mc-1: nodes; rows mc..mpad-1: padding (zero matrix rows, gather any valid dof); rows mpad..: projectors.
+  // Node rows and projector rows never share a group of 4 (or a panel of 8) rows, so every TMA row gather of the
+  // contraction kernel reads from ONE array (X or P).
+  const int mpad = (mc + 7) / 8 * 8;
   plan->ktot.resize(nc);
   plan->mat_off.assign(nc + 1, 0);
   plan->idx_off.assign(nc + 1, 0);
   for (int64_t c = 0; c < nc; ++c) {
     int64_t np = plan->cell_proj_ptr[c + 1] - plan->cell_proj_ptr[c];
-    int kt = (int)((mc + np + 7) / 8 * 8);
+    int kt = (int)(mpad + (np + 7) / 8 * 8);
     plan->ktot[c] = kt;
     plan->mat_off[c + 1] = plan->mat_off[c] + (int64_t)kt * lda;
     plan->idx_off[c + 1] = plan->idx_off[c] + kt;
@@ -273,8 +277,9 @@ std::string analyse_mesh(const chfsi_mesh& mesh, const chfsi_nonlocal* nl, const
   for (int64_t c = 0; c < nc; ++c) {
     int32_t* gi = plan->gidx.data() + plan->idx_off[c];
     for (int l = 0; l < mc; ++l) gi[l] = mesh.cell_dofs[c * mc + l];
+    for (int l = mc; l < mpad; ++l) gi[l] = mesh.cell_dofs[c * mc];
     int64_t np = plan->cell_proj_ptr[c + 1] - plan->cell_proj_ptr[c];
-    for (int64_t i = 0; i < np; ++i) gi[mc + i] = plan->cell_proj_idx[plan->cell_proj_ptr[c] + i];
+    for (int64_t i = 0; i < np; ++i) gi[mpad + i] = plan->cell_proj_idx[plan->cell_proj_ptr[c] + i];
   }
   std::vector<uint8_t> seen(nd, 0);
   for (int64_t t = 0; t < nc; ++t) {

@@ -196,7 +196,7 @@ __global__ void __launch_bounds__(256) k_cell_projector(int n1, int nq1, SetupTa
   }
   __syncthreads();
   const int32_t* gi = gidx + idx_off[c];
-  T* row = mat + mat_off[c] + (int64_t)(mc + (r - cell_proj_ptr[c])) * lda;
+  T* row = mat + mat_off[c] + (int64_t)((mc + 7) / 8 * 8 + (r - cell_proj_ptr[c])) * lda;
   for (int m = threadIdx.x; m < lda; m += blockDim.x) {
     double v = 0.0;
     if (m < mc) {
