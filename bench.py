@@ -209,7 +209,7 @@ def run_b200(args, spec):
     X0 = X_host.to("cuda")
     X = torch.empty_like(X0)
     ws = op.workspace(min(B, N))
-    peaks = measure_fp64_peak() if spec.precision == 64 else None
+    peaks = measure_fp64_peak()
 
     def barrier():
         torch.cuda.synchronize()
@@ -250,15 +250,16 @@ def run_b200(args, spec):
     n_apply = prof["applies"]
     cols_total = N * m * args.steps                           # column-applies covered by the profile
     contr_tflops = contr_flops_per_apply * cols_total / (prof["contraction_ms"] * 1e-3) * 1e-12 if prof["contraction_ms"] > 0 else None
-    if spec.precision == 64:
+    if spec.precision == 64 or args.variant == 0:
+        # the FP32 variant stores matrices and vectors in FP32 and contracts them on the same FP64 tensor pipe
         peak, bound, peak_note = peaks["dmma_tflops"], "tensor", \
             "FP64 mma.sync m8n8k4 (DMMA) rate measured in this run by chfsi_measure_fp64_peak; MEASURED_PEAKS.json has no FP64 figure"
     else:
         peak, bound, peak_note = 2 * 37.2, "alu", "FP32 FFMA: 148 SMs x 128 lanes x 2 x 1.965 GHz (B200_PROFILING.md unit counts)"
     key = (spec.config, args.assembly)
     roofline = {
-        "kernel": ({0: "k_apply_dmma_p", 1: "k_apply_generic<double>", 2: "k_apply_dmma"}[args.variant]
-                   if spec.precision == 64 else "k_apply_generic<float>"),
+        "kernel": ({0: "k_apply_dmma_p<double>", 1: "k_apply_generic<double>", 2: "k_apply_dmma"}[args.variant]
+                   if spec.precision == 64 else {0: "k_apply_dmma_p<float>"}.get(args.variant, "k_apply_generic<float>")),
         "bound": bound, "achieved": contr_tflops, "peak": peak, "unit": "TFLOP/s",
         "frac": (contr_tflops / peak) if contr_tflops else None,
         "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(key),
@@ -305,7 +306,9 @@ def run_b200(args, spec):
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f64" if spec.precision == 64 else "f32", "data": "synthetic",
+            "vs_baseline": None,
+            "dtype": "f64" if spec.precision == 64 else "f64 accumulate on f32-stored matrices and vectors",
+            "data": "synthetic",
             "config": {"workload": workload_name(spec), "assembly": "coloured" if args.assembly == 0 else "atomic",
                        "n_colors": info["n_colors"], "bounds": {"a0": a0, "a": a, "b": b},
                        "parallelism": f"band-parallel x{world} (operator replicated, no collective)",

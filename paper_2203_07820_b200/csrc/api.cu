@@ -154,7 +154,10 @@ int chfsi_create(chfsi_op** out, const chfsi_mesh* mesh, const chfsi_potential* 
   if (!op) return fail(nullptr, CHFSI_ERR_OUT_OF_MEMORY, "host allocation failed");
   op->p = mesh->p; op->n1 = mesh->p + 1; op->nq1 = mesh->p + 2;
   op->m_cell = op->n1 * op->n1 * op->n1; op->n_q = op->nq1 * op->nq1 * op->nq1;
-  op->mpad = (op->m_cell + 7) / 8 * 8; op->lda = op->mpad + 4;
+  op->mpad = (op->m_cell + 7) / 8 * 8;
+  // leading dimension of the cell matrices = their shared-memory row pitch: the four k-rows of an mma A fragment
+  // must fall into different bank groups.  FP64: LDA mod 16 in {4, 12}; FP32: LDA mod 32 in {8, 24}.
+  op->lda = precision == 64 ? op->mpad + 4 : op->mpad + (op->mpad % 16 == 0 ? 8 : 0);
   op->precision = precision; op->assembly = assembly;
   op->n_cells = mesh->n_cells; op->n_dofs = mesh->n_dofs; op->n_proj = has_nl ? nl->n_proj : 0;
 

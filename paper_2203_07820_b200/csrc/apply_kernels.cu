@@ -410,10 +410,10 @@ __global__ void __launch_bounds__(512, 1) k_apply_dmma(ApplyDev<double> a) {
 constexpr int kP2PanelK = 8;
 constexpr int kP2TileN = 32;
 constexpr int kP2LdXs = kP2TileN;       // the TMA row gather packs the rows densely (256 B each)
-constexpr int kP2Stages = 4;
 constexpr int kP2Threads = 256;
-constexpr int kP2Ahead = kP2Stages - 2;   // panels in flight; one slot of slack so that a producer never waits for
-                                          // the previous producer (which lags by its own issue time)
+// ring depth: 4 stages of 24 KB for FP64 storage, 8 stages of 12 KB for FP32 storage; panels in flight = stages - 2
+// (one slot of slack so that a producer never waits for the previous producer, which lags by its own issue time)
+template <typename S> __host__ __device__ constexpr int p2_stages() { return sizeof(S) == 8 ? 4 : 8; }
 constexpr int kP2L2Ahead = 6;           // cell-matrix panels prefetched into L2 beyond the ring
 constexpr int kSyncFlagOffset = 32;     // uint32 index of the first flag inside the sync region (128 bytes)
 
@@ -467,15 +467,28 @@ __device__ __forceinline__ double2 ld_cg_d2(const double* p) {
   return v;
 }
 
-template <int MT>
-__global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<double> a, PersistDev pd,
+__device__ __forceinline__ double2 ld_cg_pair(const double* p) { return ld_cg_d2(p); }
+__device__ __forceinline__ double2 ld_cg_pair(const float* p) {
+  float x, y;
+  asm volatile("ld.global.cg.v2.f32 {%0,%1}, [%2];" : "=f"(x), "=f"(y) : "l"(p) : "memory");
+  return make_double2((double)x, (double)y);
+}
+__device__ __forceinline__ void st_pair(double* p, double v0, double v1) { *reinterpret_cast<double2*>(p) = make_double2(v0, v1); }
+__device__ __forceinline__ void st_pair(float* p, double v0, double v1) { *reinterpret_cast<float2*>(p) = make_float2((float)v0, (float)v1); }
+
+// S = storage type of the cell matrices and the vector blocks (double, or float for the FP32 variant: the fragments
+// are widened to FP64 in registers and the contraction still runs on the FP64 tensor pipe with FP64 accumulators).
+template <int MT, typename S>
+__global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<S> a, PersistDev pd,
                                                                 const __grid_constant__ CUtensorMap tmX,
                                                                 const __grid_constant__ CUtensorMap tmP) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int lda = a.lda;
   const int a_panel_elems = kP2PanelK * lda;
   const int stage_elems = a_panel_elems + kP2PanelK * kP2LdXs;
-  double* stage0 = reinterpret_cast<double*>(smem_raw);
+  constexpr int kP2Stages = p2_stages<S>();
+  constexpr int kP2Ahead = kP2Stages - 2;
+  S* stage0 = reinterpret_cast<S*>(smem_raw);
   uint64_t* full = reinterpret_cast<uint64_t*>(stage0 + kP2Stages * stage_elems);
   uint64_t* empty = full + kP2Stages;
   long long* ticket_s = reinterpret_cast<long long*>(empty + kP2Stages);   // [2]
@@ -515,7 +528,7 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<double>
     const int ncols = min(kP2TileN, a.B - col0);             // multiple of 8
     const int kt = a.ktot[cell];
     const int32_t* gi = a.gidx + a.idx_off[cell];
-    const double* M = a.mat + a.mat_off[cell];
+    const S* M = a.mat + a.mat_off[cell];
     if (tid == 0) ticket_s[(iter + 1) & 1] = (long long)(atomicAdd(pd.counter, 1ull) - pd.ticket_base);
     const bool use_t = (beta != 0.0) && !a.atomic;   // the -beta Y_{k-2} term seeds the accumulators (below)
     for (int k = tid; k < kt; k += kP2Threads) {
@@ -544,10 +557,10 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<double>
       long long te1 = clock64();
       if (tr_p) tr_p[4] += te1 - te0;
 #endif
-      double* As = stage0 + s * stage_elems;
-      double* Xs = As + a_panel_elems;
-      const uint32_t a_bytes = (uint32_t)a_panel_elems * 8u;
-      mbar_expect_tx(&full[s], a_bytes + (uint32_t)(kP2PanelK * kP2LdXs * 8));
+      S* As = stage0 + s * stage_elems;
+      S* Xs = As + a_panel_elems;
+      const uint32_t a_bytes = (uint32_t)a_panel_elems * (uint32_t)sizeof(S);
+      mbar_expect_tx(&full[s], a_bytes + (uint32_t)(kP2PanelK * kP2LdXs * sizeof(S)));
       bulk_g2s(As, M + (int64_t)pj * a_panel_elems, a_bytes, &full[s]);
       const int k0 = pj * kP2PanelK;
       const CUtensorMap* tm = (k0 < a.mpad) ? &tmX : &tmP;
@@ -581,10 +594,10 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<double>
         const int r = (mt0 + i) * 8 + fm;
         const int idx = (i < nmt && r < mc) ? idx_s[r] : 0;
         if (idx < 0) {
-          const double* tp = a.Tg + (int64_t)(idx & 0x7fffffff) * a.ldt + col0 + nt0 * 8 + fk * 2;
-          const double2 u = ld_cg_d2(tp);
+          const S* tp = a.Tg + (int64_t)(idx & 0x7fffffff) * a.ldt + col0 + nt0 * 8 + fk * 2;
+          const double2 u = ld_cg_pair(tp);
           acc[i][0][0] = u.x; acc[i][0][1] = u.y;
-          if (nnt > 1) { const double2 v = ld_cg_d2(tp + 8); acc[i][1][0] = v.x; acc[i][1][1] = v.y; }
+          if (nnt > 1) { const double2 v = ld_cg_pair(tp + 8); acc[i][1][0] = v.x; acc[i][1][1] = v.y; }
         }
       }
 #pragma unroll
@@ -610,16 +623,16 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<double>
       if (tr) { long long tw2 = clock64(); if (pi == 0) tr[2] = tw2; else { tr[6] += tw2 - tw1; } tr[7] += tw1 - tw0; }
 #endif
       if (active) {
-        const double* As = stage0 + s * stage_elems;
-        const double* Ap = As + fk * lda + mt0 * 8 + fm;
-        const double* Xp = As + a_panel_elems + fk * kP2LdXs + nt0 * 8 + fm;
+        const S* As = stage0 + s * stage_elems;
+        const S* Ap = As + fk * lda + mt0 * 8 + fm;
+        const S* Xp = As + a_panel_elems + fk * kP2LdXs + nt0 * 8 + fm;
         if (nmt == MT && nnt == 2) {
 #pragma unroll
           for (int ks = 0; ks < kP2PanelK / 4; ++ks) {
-            const double b0 = Xp[ks * 4 * kP2LdXs], b1 = Xp[ks * 4 * kP2LdXs + 8];
+            const double b0 = (double)Xp[ks * 4 * kP2LdXs], b1 = (double)Xp[ks * 4 * kP2LdXs + 8];
 #pragma unroll
             for (int i = 0; i < MT; ++i) {
-              const double av = Ap[ks * 4 * lda + i * 8];
+              const double av = (double)Ap[ks * 4 * lda + i * 8];
               dmma884(acc[i][0][0], acc[i][0][1], av, b0);
               dmma884(acc[i][1][0], acc[i][1][1], av, b1);
             }
@@ -627,11 +640,11 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<double>
         } else {
 #pragma unroll
           for (int ks = 0; ks < kP2PanelK / 4; ++ks) {
-            const double b0 = Xp[ks * 4 * kP2LdXs], b1 = (nnt > 1) ? Xp[ks * 4 * kP2LdXs + 8] : 0.0;
+            const double b0 = (double)Xp[ks * 4 * kP2LdXs], b1 = (nnt > 1) ? (double)Xp[ks * 4 * kP2LdXs + 8] : 0.0;
 #pragma unroll
             for (int i = 0; i < MT; ++i) {
               if (i < nmt) {
-                const double av = Ap[ks * 4 * lda + i * 8];
+                const double av = (double)Ap[ks * 4 * lda + i * 8];
                 dmma884(acc[i][0][0], acc[i][0][1], av, b0);
                 dmma884(acc[i][1][0], acc[i][1][1], av, b1);
               }
@@ -668,17 +681,17 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<double>
         const int r = (mt0 + i) * 8 + fm;
         if (i >= nmt || r >= mc) continue;
         const int idx = idx_s[r];
-        double* trow = a.Tg + (int64_t)(idx & 0x7fffffff) * a.ldt + col0 + nt0 * 8 + fk * 2;
+        S* trow = a.Tg + (int64_t)(idx & 0x7fffffff) * a.ldt + col0 + nt0 * 8 + fk * 2;
         const bool add = a.atomic || idx >= 0;
 #pragma unroll
         for (int j = 0; j < 2; ++j) {
           if (j >= nnt) continue;
           const double v0 = alpha * acc[i][j][0], v1 = alpha * acc[i][j][1];
           if (add) {
-            atomicAdd(trow + j * 8, v0);
-            atomicAdd(trow + j * 8 + 1, v1);
+            atomicAdd(trow + j * 8, (S)v0);
+            atomicAdd(trow + j * 8 + 1, (S)v1);
           } else {
-            *reinterpret_cast<double2*>(trow + j * 8) = make_double2(v0, v1);
+            st_pair(trow + j * 8, v0, v1);
           }
         }
       }
@@ -691,7 +704,7 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<double>
   }
 }
 
-// Tensor map of a row-major FP64 block [rows][ld] restricted to its first `cols` columns, box = kP2TileN x 1
+// Tensor map of a row-major FP64 / FP32 block [rows][ld] restricted to its first `cols` columns, box = kP2TileN x 1
 // (tile::gather4 picks four such rows per instruction); columns beyond `cols` read as zero.
 using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                    const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -707,14 +720,14 @@ EncodeTiledFn encode_tiled_fn() {
   }();
   return fn;
 }
-bool make_row_gather_map(CUtensorMap* tm, const void* base, int64_t rows, int64_t cols, int64_t ld) {
+bool make_row_gather_map(CUtensorMap* tm, const void* base, int64_t rows, int64_t cols, int64_t ld, int elt) {
   EncodeTiledFn enc = encode_tiled_fn();
-  if (!enc || rows < 1 || cols < 1 || (ld * 8) % 16 != 0 || (uintptr_t)base % 16 != 0) return false;
+  if (!enc || rows < 1 || cols < 1 || (ld * elt) % 16 != 0 || (uintptr_t)base % 16 != 0) return false;
   const cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
-  const cuuint64_t strides[1] = {(cuuint64_t)ld * 8};
+  const cuuint64_t strides[1] = {(cuuint64_t)ld * (cuuint64_t)elt};
   const cuuint32_t box[2] = {(cuuint32_t)kP2TileN, 1};
   const cuuint32_t estr[2] = {1, 1};
-  return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<void*>(base), dims, strides, box, estr,
+  return enc(tm, elt == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<void*>(base), dims, strides, box, estr,
              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
@@ -728,9 +741,10 @@ size_t pp_smem_bytes(const Op* op) {
 long long* g_trace_buffer = nullptr;
 #endif
 
+template <typename S>
 size_t p2_smem_bytes(const Op* op) {
-  return (size_t)kP2Stages * (kP2PanelK * op->lda + kP2PanelK * kP2LdXs) * sizeof(double) + 2 * kP2Stages * sizeof(uint64_t) +
-         2 * sizeof(long long) + (size_t)op->max_ktot * sizeof(int32_t);
+  return (size_t)p2_stages<S>() * (kP2PanelK * op->lda + kP2PanelK * kP2LdXs) * sizeof(S) +
+         2 * p2_stages<S>() * sizeof(uint64_t) + 2 * sizeof(long long) + (size_t)op->max_ktot * sizeof(int32_t);
 }
 
 template <typename T>
@@ -785,7 +799,9 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
   a.alpha = (T)g.alpha; a.beta = (T)g.beta;
   a.atomic = op->assembly;
 
-  const bool aligned = sizeof(T) == 8 && B % 8 == 0 && g.ldx % 2 == 0 && g.ldt % 2 == 0 && ((uintptr_t)g.X % 16 == 0) &&
+  // row segments of a chunk start 16-byte aligned (TMA, vector loads / stores of the fragments)
+  constexpr int kPer16 = 16 / (int)sizeof(T);
+  const bool aligned = B % 8 == 0 && g.ldx % kPer16 == 0 && g.ldt % kPer16 == 0 && ((uintptr_t)g.X % 16 == 0) &&
                        ((uintptr_t)g.T % 16 == 0) && ((uintptr_t)g.P % 16 == 0) && op->max_ktot <= kMaxKtot;
   const int n_mtiles = (op->m_cell + 7) / 8;
   // variant 0: persistent single-launch kernel (v2); variant 2: one launch per colour (v1); variant 1: generic
@@ -793,9 +809,10 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
   int MT = (n_mtiles + 3) / 4;
   CUtensorMap tmX, tmP;
   if (aligned && op->variant == 0 && g.sync != nullptr && g.epoch > 0)
-    fast2 = (MT == 11 || MT == 7 || MT == 4 || MT == 2 || MT == 1) && p2_smem_bytes(op) <= 113 * 1024 &&
-            make_row_gather_map(&tmX, g.X, op->n_dofs, B, g.ldx) && make_row_gather_map(&tmP, g.P, op->n_proj + 1, B, B);
-  if (aligned && !fast2 && op->variant != 1) fast = (MT == 11 || MT == 4 || MT == 2 || MT == 7);
+    fast2 = (MT == 11 || MT == 7 || MT == 4 || MT == 2 || MT == 1) && p2_smem_bytes<T>(op) <= 113 * 1024 &&
+            make_row_gather_map(&tmX, g.X, op->n_dofs, B, g.ldx, (int)sizeof(T)) &&
+            make_row_gather_map(&tmP, g.P, op->n_proj + 1, B, B, (int)sizeof(T));
+  if (sizeof(T) == 8 && aligned && !fast2 && op->variant != 1) fast = (MT == 11 || MT == 4 || MT == 2 || MT == 7);
   size_t smem_fast = (size_t)kStages * (kPanelK * op->lda + kPanelK * kLdXs) * sizeof(double) + kStages * sizeof(uint64_t) +
                      (size_t)op->max_ktot * sizeof(int32_t);
   if (fast && smem_fast > 227 * 1024) fast = false;
@@ -810,7 +827,7 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
   }
   const int64_t launches_mid = op->launches;
   if (fast2) {
-    if constexpr (sizeof(T) == 8) {
+    {
       a.cells = nullptr; a.n_launch_cells = (int)op->n_cells;
       a.n_col_tiles = (B + kP2TileN - 1) / kP2TileN;
       PersistDev pd;
@@ -829,14 +846,13 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
       pd.trace = g_trace_buffer;
       pd.debug_flags = getenv("CHFSI_DEBUG_FLAGS") ? atoi(getenv("CHFSI_DEBUG_FLAGS")) : 0;
 #endif
-      ApplyDev<double> ad = *reinterpret_cast<ApplyDev<double>*>(&a);
-      const size_t sm = p2_smem_bytes(op);
+      const size_t sm = p2_smem_bytes<T>(op);
       switch (MT) {
-        case 11: k_apply_dmma_p<11><<<grid, kP2Threads, sm, st>>>(ad, pd, tmX, tmP); break;
-        case 7: k_apply_dmma_p<7><<<grid, kP2Threads, sm, st>>>(ad, pd, tmX, tmP); break;
-        case 4: k_apply_dmma_p<4><<<grid, kP2Threads, sm, st>>>(ad, pd, tmX, tmP); break;
-        case 2: k_apply_dmma_p<2><<<grid, kP2Threads, sm, st>>>(ad, pd, tmX, tmP); break;
-        case 1: k_apply_dmma_p<1><<<grid, kP2Threads, sm, st>>>(ad, pd, tmX, tmP); break;
+        case 11: k_apply_dmma_p<11, T><<<grid, kP2Threads, sm, st>>>(a, pd, tmX, tmP); break;
+        case 7: k_apply_dmma_p<7, T><<<grid, kP2Threads, sm, st>>>(a, pd, tmX, tmP); break;
+        case 4: k_apply_dmma_p<4, T><<<grid, kP2Threads, sm, st>>>(a, pd, tmX, tmP); break;
+        case 2: k_apply_dmma_p<2, T><<<grid, kP2Threads, sm, st>>>(a, pd, tmX, tmP); break;
+        case 1: k_apply_dmma_p<1, T><<<grid, kP2Threads, sm, st>>>(a, pd, tmX, tmP); break;
       }
       op->launches++;
     }
@@ -886,13 +902,24 @@ cudaError_t init_apply_kernels(Op* op) {
   }
   if ((e = cudaFuncSetAttribute(k_proj_partial<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pp_smem_bytes<double>(op)))) return e;
   if ((e = cudaFuncSetAttribute(k_proj_partial<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pp_smem_bytes<float>(op)))) return e;
-  const size_t smem_p2 = p2_smem_bytes(op);
-  if (smem_p2 <= 113 * 1024) {
-    if ((e = cudaFuncSetAttribute(k_apply_dmma_p<11>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p2))) return e;
-    if ((e = cudaFuncSetAttribute(k_apply_dmma_p<7>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p2))) return e;
-    if ((e = cudaFuncSetAttribute(k_apply_dmma_p<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p2))) return e;
-    if ((e = cudaFuncSetAttribute(k_apply_dmma_p<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p2))) return e;
-    if ((e = cudaFuncSetAttribute(k_apply_dmma_p<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p2))) return e;
+  if (op->precision == 64) {
+    const size_t smem_p2 = p2_smem_bytes<double>(op);
+    if (smem_p2 <= 113 * 1024) {
+      if ((e = cudaFuncSetAttribute(k_apply_dmma_p<11, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p2))) return e;
+      if ((e = cudaFuncSetAttribute(k_apply_dmma_p<7, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p2))) return e;
+      if ((e = cudaFuncSetAttribute(k_apply_dmma_p<4, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p2))) return e;
+      if ((e = cudaFuncSetAttribute(k_apply_dmma_p<2, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p2))) return e;
+      if ((e = cudaFuncSetAttribute(k_apply_dmma_p<1, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p2))) return e;
+    }
+  } else {
+    const size_t smem_p2 = p2_smem_bytes<float>(op);
+    if (smem_p2 <= 113 * 1024) {
+      if ((e = cudaFuncSetAttribute(k_apply_dmma_p<11, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p2))) return e;
+      if ((e = cudaFuncSetAttribute(k_apply_dmma_p<7, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p2))) return e;
+      if ((e = cudaFuncSetAttribute(k_apply_dmma_p<4, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p2))) return e;
+      if ((e = cudaFuncSetAttribute(k_apply_dmma_p<2, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p2))) return e;
+      if ((e = cudaFuncSetAttribute(k_apply_dmma_p<1, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p2))) return e;
+    }
   }
   size_t smem_gen = (size_t)op->max_ktot * 32 * 8;
   if (smem_gen > 227 * 1024) return cudaErrorInvalidValue;
