@@ -47,7 +47,8 @@ void free_op(chfsi_op* op) {
   if (!op) return;
   cudaFree(op->mat); cudaFree(op->mat_off); cudaFree(op->idx_off); cudaFree(op->ktot); cudaFree(op->gidx);
   cudaFree(op->color_cells); cudaFree(op->dep_ptr); cudaFree(op->dep_pos); cudaFree(op->all_cells); cudaFree(op->pc_cells); cudaFree(op->cell_proj_ptr);
-  cudaFree(op->proj_ptr); cudaFree(op->proj_pcrow); cudaFree(op->D); cudaFree(op->mass); cudaFree(op->diag0);
+  cudaFree(op->proj_ptr); cudaFree(op->proj_pcrow); cudaFree(op->seg_ptr); cudaFree(op->grow_dof); cudaFree(op->pcoef);
+  cudaFree(op->grp_seg_ptr); cudaFree(op->proj_grp); cudaFree(op->proj_slot); cudaFree(op->D); cudaFree(op->mass); cudaFree(op->diag0);
   for (cudaEvent_t e : op->prof_events) cudaEventDestroy(e);
   delete op;
 }
@@ -63,7 +64,7 @@ WsLayout ws_layout(const Op* op, int64_t B) {
   w.block_off = 0;
   w.p_off = align_up((size_t)op->n_dofs * w.ldw * w.elt, 256);
   w.pc_off = w.p_off + align_up((size_t)(op->n_proj + 1) * B * w.elt, 256);
-  w.sync_off = w.pc_off + align_up((size_t)(op->nnz_cp > 0 ? op->nnz_cp : 1) * B * w.elt, 256);
+  w.sync_off = w.pc_off + align_up((size_t)(op->n_pseg > 0 ? op->n_pseg : 1) * kProjGroup * B * sizeof(double), 256);
   // ticket counter (first 128 bytes) + one completion flag per (cell, 32-column tile): apply_kernels.cu, v2 kernel
   w.sync_bytes = align_up(128 + (size_t)op->n_cells * (size_t)((B + 31) / 32) * sizeof(uint32_t), 256);
   w.total = w.sync_off + w.sync_bytes;
@@ -205,6 +206,11 @@ int chfsi_create(chfsi_op** out, const chfsi_mesh* mesh, const chfsi_potential* 
   CKC(upload_vec(&op->cell_proj_ptr, plan.cell_proj_ptr, st), "upload");
   CKC(upload_vec(&op->proj_ptr, plan.proj_ptr, st), "upload");
   CKC(upload_vec(&op->proj_pcrow, plan.proj_pcrow, st), "upload");
+  CKC(upload_vec(&op->seg_ptr, plan.seg_ptr, st), "upload");
+  CKC(upload_vec(&op->grow_dof, plan.grow_dof, st), "upload");
+  CKC(upload_vec(&op->grp_seg_ptr, plan.grp_seg_ptr, st), "upload");
+  CKC(upload_vec(&op->proj_grp, plan.proj_grp, st), "upload");
+  CKC(upload_vec(&op->proj_slot, plan.proj_slot, st), "upload");
   {
     std::vector<double> D(has_nl ? nl->D : nullptr, has_nl ? nl->D + nl->n_proj : nullptr);
     CKC(upload_vec(&op->D, D, st), "upload");
@@ -214,6 +220,12 @@ int chfsi_create(chfsi_op** out, const chfsi_mesh* mesh, const chfsi_potential* 
   bool bad_jac = false;
   CKC(build_cell_matrices(op, plan, tab, *mesh, *pot, has_nl ? nl : nullptr, st, &bad_jac), "cell-matrix setup");
   if (bad_jac) { free_op(op); return fail(nullptr, CHFSI_ERR_BAD_MESH, "non-positive Jacobian at a quadrature point"); }
+  try {
+    CKC(assemble_projector_rows(op, plan, *mesh, st), "projector-row assembly");
+  } catch (const std::bad_alloc&) {
+    free_op(op);
+    return fail(nullptr, CHFSI_ERR_OUT_OF_MEMORY, "host allocation failed in projector-row assembly");
+  }
   CKC(cudaMalloc((void**)&op->diag0, (size_t)op->n_cells * op->m_cell * sizeof(double)), "cudaMalloc(diagonal)");
   CKC(capture_diagonal(op, st), "diagonal capture");
   CKC(init_apply_kernels(op), "kernel attribute setup");

@@ -96,103 +96,102 @@ __global__ void __launch_bounds__(256) k_apply_generic(ApplyDev<T> a) {
 }
 
 // -------------------------------------------------------------------------------------------------------------
-// Steps 3a-3c
+// Steps 3a-3c.  Alg. 4 steps 2-3 compute P = sum_c C^cT X^c cell by cell and assemble over the cells of each
+// projector.  C is constant, so that assembly is applied to C once at setup
+// (assemble_projector_rows: coefficient of dof g = s_g sum_{c containing g} C^c[l(g)][j]) and per apply
+// P[j] = sum_g coef[g][j] X[g]: every dof row of X in the support of an atom is read ONCE (not once per cell) for
+// all of the atom's <= 8 projectors.  HBM-bound row stream.
 // -------------------------------------------------------------------------------------------------------------
-// P^c[i][col] = sum_l C~^c[l][i] X[dof_l][col]       (Alg. 4 step 2).  grid = (cells with projectors) x (64-column tiles).
-// HBM/L2-bound gather of the cell's X rows: thread = (row slot rs = tid/16, 4 columns); every row is read as
-// 16 x 32-byte pieces by one half-warp (coalesced 512 B), the projector rows C~^c sit in shared memory, the 16 row
-// slots are summed in a fixed order (shuffle, then shared memory): deterministic.
-constexpr int kPPCols = 64;
-constexpr int kPPGroup = 8;          // projectors per pass
+// grid = (row segments of <= 128 dofs) x (256-column tiles); thread = (row slot rs = tid/128, 2 columns): a row is
+// read as 128 x 16-byte pieces (coalesced), its 8 coefficients come from shared memory (broadcast), the two row
+// slots are summed in slot order through shared memory: deterministic.  64 registers -> 4 CTAs/SM with 8 rows in
+// flight per thread: the kernel lives on memory-level parallelism.  Partial sums are FP64 for both precisions.
+constexpr int kPRCols = 256;
 template <typename T>
-__global__ void __launch_bounds__(256) k_proj_partial(const T* __restrict__ mat, const int64_t* __restrict__ mat_off,
-                                                      const int64_t* __restrict__ idx_off, const int32_t* __restrict__ gidx,
-                                                      const int32_t* __restrict__ pc_cells,
-                                                      const int64_t* __restrict__ cell_proj_ptr, int m_cell, int lda,
-                                                      const T* __restrict__ X, int64_t ldx, T* __restrict__ Pc, int B,
-                                                      int n_col_tiles, int vec_ok) {
-  extern __shared__ __align__(16) unsigned char pp_smem[];
-  T* Cs = reinterpret_cast<T*>(pp_smem);                            // [kPPGroup][m_cell]
-  T* red = Cs + kPPGroup * m_cell;                                  // [8 warps][kPPGroup][kPPCols]
-  int32_t* dofs = reinterpret_cast<int32_t*>(red + 8 * kPPGroup * kPPCols);
-  const int cell = pc_cells[blockIdx.x / n_col_tiles];
-  const int col0 = (blockIdx.x % n_col_tiles) * kPPCols;
-  const int tid = threadIdx.x, rs = tid >> 4, cq = (tid & 15) * 4;
-  const int32_t* gi = gidx + idx_off[cell];
-  for (int l = tid; l < m_cell; l += 256) dofs[l] = gi[l] & 0x7fffffff;
-  const int64_t r0 = cell_proj_ptr[cell];
-  const int np = (int)(cell_proj_ptr[cell + 1] - r0);
-  const T* C = mat + mat_off[cell] + (int64_t)((m_cell + 7) / 8 * 8) * lda;   // rows = projectors of this cell, columns = nodes
-  const int col = col0 + cq;
-  const bool full4 = vec_ok && (col + 3 < B);
-  for (int i0 = 0; i0 < np; i0 += kPPGroup) {
-    const int ni = min(kPPGroup, np - i0);
-    __syncthreads();
-    for (int e = tid; e < kPPGroup * m_cell; e += 256) {
-      const int i = e / m_cell, l = e - i * m_cell;
-      Cs[e] = (i < ni) ? C[(int64_t)(i0 + i) * lda + l] : (T)0;
-    }
-    __syncthreads();
-    T acc[kPPGroup][4];
+__global__ void __launch_bounds__(256, 4) k_proj_rows(const int32_t* __restrict__ seg_ptr, const int32_t* __restrict__ grow_dof,
+                                                      const T* __restrict__ pcoef, const T* __restrict__ X, int64_t ldx,
+                                                      double* __restrict__ Pc, int B, int vec_ok) {
+  __shared__ double red[kProjGroup][kPRCols];
+  __shared__ __align__(16) T cs[kProjSegRows * kProjGroup];
+  __shared__ int32_t dofs[kProjSegRows];
+  const int seg = blockIdx.x;
+  const int r0 = seg_ptr[seg], nr = seg_ptr[seg + 1] - r0;
+  const int tid = threadIdx.x, cg = tid & 127, rs = tid >> 7;
+  const int col = blockIdx.y * kPRCols + cg * 2;
+  for (int e = tid; e < nr * kProjGroup; e += 256) cs[e] = pcoef[(int64_t)r0 * kProjGroup + e];
+  for (int e = tid; e < nr; e += 256) dofs[e] = grow_dof[r0 + e];
+  __syncthreads();
+  double acc[kProjGroup][2];
 #pragma unroll
-    for (int i = 0; i < kPPGroup; ++i) acc[i][0] = acc[i][1] = acc[i][2] = acc[i][3] = (T)0;
-#pragma unroll 4
-    for (int l = rs; l < m_cell; l += 16) {
-      const T* xr = X + (int64_t)dofs[l] * ldx + col;
-      T x[4];
-      if (full4) {
+  for (int i = 0; i < kProjGroup; ++i) acc[i][0] = acc[i][1] = 0.0;
+  const bool full2 = vec_ok && (col + 1 < B);
+  if (col < B) {
+#pragma unroll 8
+    for (int r = rs; r < nr; r += 2) {
+      const T* xr = X + (int64_t)dofs[r] * ldx + col;
+      double x0, x1;
+      if (full2) {
         if constexpr (sizeof(T) == 8) {
-          const double2 u = *reinterpret_cast<const double2*>(xr), v = *reinterpret_cast<const double2*>(xr + 2);
-          x[0] = u.x; x[1] = u.y; x[2] = v.x; x[3] = v.y;
+          const double2 u = *reinterpret_cast<const double2*>(xr);
+          x0 = u.x; x1 = u.y;
         } else {
-          const float4 u = *reinterpret_cast<const float4*>(xr);
-          x[0] = u.x; x[1] = u.y; x[2] = u.z; x[3] = u.w;
+          const float2 u = *reinterpret_cast<const float2*>(xr);
+          x0 = u.x; x1 = u.y;
         }
       } else {
-#pragma unroll
-        for (int t = 0; t < 4; ++t) x[t] = (col + t < B) ? xr[t] : (T)0;
+        x0 = (double)xr[0]; x1 = (col + 1 < B) ? (double)xr[1] : 0.0;
       }
 #pragma unroll
-      for (int i = 0; i < kPPGroup; ++i) {
-        const T c = Cs[i * m_cell + l];
-#pragma unroll
-        for (int t = 0; t < 4; ++t) acc[i][t] = fma(c, x[t], acc[i][t]);
+      for (int i = 0; i < kProjGroup; ++i) {
+        const double c = (double)cs[r * kProjGroup + i];
+        acc[i][0] = fma(c, x0, acc[i][0]);
+        acc[i][1] = fma(c, x1, acc[i][1]);
       }
     }
-    // the two row slots of a warp are summed by shuffle, the 8 warps through shared memory in warp order
+  }
+  if (rs == 1) {
 #pragma unroll
-    for (int i = 0; i < kPPGroup; ++i)
+    for (int i = 0; i < kProjGroup; ++i) { red[i][cg * 2] = acc[i][0]; red[i][cg * 2 + 1] = acc[i][1]; }
+  }
+  __syncthreads();
+  if (rs == 0 && col < B) {
 #pragma unroll
-      for (int t = 0; t < 4; ++t) {
-        acc[i][t] += __shfl_xor_sync(0xffffffffu, acc[i][t], 16);
-        if ((tid & 16) == 0) red[((tid >> 5) * kPPGroup + i) * kPPCols + cq + t] = acc[i][t];
-      }
-    __syncthreads();
-    for (int e = tid; e < ni * kPPCols; e += 256) {
-      const int i = e / kPPCols, cc = e - i * kPPCols;
-      if (col0 + cc >= B) continue;
-      T s = (T)0;
-#pragma unroll
-      for (int r = 0; r < 8; ++r) s += red[(r * kPPGroup + i) * kPPCols + cc];
-      Pc[(r0 + i0 + i) * B + col0 + cc] = s;
+    for (int i = 0; i < kProjGroup; ++i) {
+      double* out = Pc + ((int64_t)seg * kProjGroup + i) * B + col;
+      out[0] = acc[i][0] + red[i][cg * 2];
+      if (col + 1 < B) out[1] = acc[i][1] + red[i][cg * 2 + 1];
     }
   }
 }
 
-// P[j][col] = D_j sum_{c in supp(j)} P^c[j][col], fixed CSR order (Alg. 4 steps 3-4); row n_proj = 0 (padding target)
+// P[j][col] = D_j sum_{segments of j's group} Pc[seg][slot_j][col], segment order (Alg. 4 step 4 is the D scaling,
+// PAPER.md:527); row n_proj = 0 (target of the padding rows of the contraction)
 template <typename T>
-__global__ void __launch_bounds__(128) k_proj_reduce(const T* __restrict__ Pc, const int64_t* __restrict__ proj_ptr,
-                                                     const int64_t* __restrict__ proj_pcrow, const double* __restrict__ D,
-                                                     int64_t n_proj, T* __restrict__ P, int B) {
+__global__ void __launch_bounds__(128) k_proj_reduce(const double* __restrict__ Pc, const int32_t* __restrict__ grp_seg_ptr,
+                                                     const int32_t* __restrict__ proj_grp, const int32_t* __restrict__ proj_slot,
+                                                     const double* __restrict__ D, int64_t n_proj, T* __restrict__ P, int B) {
   const int64_t j = blockIdx.x;
   const int col = blockIdx.y * 128 + threadIdx.x;
   if (col >= B) return;
-  T s = (T)0;
-  if (j < n_proj) {
-    for (int64_t k = proj_ptr[j]; k < proj_ptr[j + 1]; ++k) s += Pc[proj_pcrow[k] * B + col];
-    s *= (T)D[j];
+  double s = 0.0;
+  if (j < n_proj && proj_grp[j] >= 0) {
+    const int g = proj_grp[j], slot = proj_slot[j];
+    for (int seg = grp_seg_ptr[g]; seg < grp_seg_ptr[g + 1]; ++seg) s += Pc[((int64_t)seg * kProjGroup + slot) * B + col];
+    s *= D[j];
   }
-  P[j * B + col] = s;
+  P[j * B + col] = (T)s;
+}
+
+// setup: projector rows of the cell matrices -> compact FP64 rows [nnz_cp][m_cell]
+template <typename T>
+__global__ void __launch_bounds__(128) k_extract_proj_rows(const T* __restrict__ mat, const int64_t* __restrict__ mat_off,
+                                                           const int64_t* __restrict__ cell_proj_ptr,
+                                                           const int32_t* __restrict__ row_cell, int m_cell, int mpad, int lda,
+                                                           double* __restrict__ out) {
+  const int64_t r = blockIdx.x;
+  const int c = row_cell[r];
+  const T* row = mat + mat_off[c] + (int64_t)(mpad + (r - cell_proj_ptr[c])) * lda;
+  for (int l = threadIdx.x; l < m_cell; l += 128) out[r * m_cell + l] = (double)row[l];
 }
 
 // Atomic assembly needs the recurrence term in place first:  T <- -beta T
@@ -732,10 +731,6 @@ bool make_row_gather_map(CUtensorMap* tm, const void* base, int64_t rows, int64_
              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-template <typename T>
-size_t pp_smem_bytes(const Op* op) {
-  return (size_t)(kPPGroup * op->m_cell + 8 * kPPGroup * kPPCols) * sizeof(T) + (size_t)op->m_cell * sizeof(int32_t);
-}
 
 #ifdef CHFSI_TRACE
 long long* g_trace_buffer = nullptr;
@@ -751,7 +746,6 @@ template <typename T>
 cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
   const int B = (int)g.B;
   T* P = reinterpret_cast<T*>(g.P);
-  T* Pc = reinterpret_cast<T*>(g.Pc);
   const T* X = reinterpret_cast<const T*>(g.X);
   T* Tg = reinterpret_cast<T*>(g.T);
   const T* mat = reinterpret_cast<const T*>(op->mat);
@@ -779,17 +773,16 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
   }
   const int64_t launches_before = op->launches;
   // steps 3a-3c
-  if (op->n_proj > 0) {
-    const int nct = (B + kPPCols - 1) / kPPCols;
-    const int vec_ok = (g.ldx % 4 == 0 && (uintptr_t)g.X % 32 == 0) ? 1 : 0;
-    k_proj_partial<T><<<(unsigned)(op->n_pc_cells * nct), 256, pp_smem_bytes<T>(op), st>>>(
-        mat, op->mat_off, op->idx_off, op->gidx, op->pc_cells, op->cell_proj_ptr, op->m_cell, op->lda, X, g.ldx, Pc, B, nct,
-        vec_ok);
+  double* Pc = reinterpret_cast<double*>(g.Pc);
+  if (op->n_pseg > 0) {
+    dim3 g1((unsigned)op->n_pseg, (unsigned)((B + kPRCols - 1) / kPRCols));
+    const int vec_ok = (g.ldx % 2 == 0 && (uintptr_t)g.X % 16 == 0) ? 1 : 0;
+    k_proj_rows<T><<<g1, 256, 0, st>>>(op->seg_ptr, op->grow_dof, reinterpret_cast<const T*>(op->pcoef), X, g.ldx, Pc, B, vec_ok);
     op->launches++;
   }
   {
     dim3 g2((unsigned)(op->n_proj + 1), (unsigned)((B + 127) / 128));
-    k_proj_reduce<T><<<g2, 128, 0, st>>>(Pc, op->proj_ptr, op->proj_pcrow, op->D, op->n_proj, P, B);
+    k_proj_reduce<T><<<g2, 128, 0, st>>>(Pc, op->grp_seg_ptr, op->proj_grp, op->proj_slot, op->D, op->n_proj, P, B);
     op->launches++;
   }
   ApplyDev<T> a;
@@ -900,8 +893,6 @@ cudaError_t init_apply_kernels(Op* op) {
     if ((e = cudaFuncSetAttribute(k_apply_dmma<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_fast))) return e;
     if ((e = cudaFuncSetAttribute(k_apply_dmma<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_fast))) return e;
   }
-  if ((e = cudaFuncSetAttribute(k_proj_partial<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pp_smem_bytes<double>(op)))) return e;
-  if ((e = cudaFuncSetAttribute(k_proj_partial<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pp_smem_bytes<float>(op)))) return e;
   if (op->precision == 64) {
     const size_t smem_p2 = p2_smem_bytes<double>(op);
     if (smem_p2 <= 113 * 1024) {
@@ -931,6 +922,64 @@ cudaError_t init_apply_kernels(Op* op) {
 #ifdef CHFSI_TRACE
 extern "C" void chfsi_debug_set_trace(long long* dev_buffer) { g_trace_buffer = dev_buffer; }
 #endif
+
+cudaError_t assemble_projector_rows(Op* op, const HostPlan& plan, const chfsi_mesh& mesh, cudaStream_t st) {
+  op->n_pseg = 0; op->n_prow = (int64_t)plan.grow_dof.size();
+  const size_t elt = op->precision == 64 ? 8 : 4;
+  cudaError_t e;
+  if (op->n_proj == 0 || op->n_prow == 0 || op->nnz_cp == 0) return cudaSuccess;
+  const int mc = op->m_cell;
+  // 1. compact FP64 copy of the projector rows of the cell matrices, on the host
+  std::vector<int32_t> row_cell((size_t)op->nnz_cp);
+  for (int64_t c = 0; c < op->n_cells; ++c)
+    for (int64_t r = plan.cell_proj_ptr[c]; r < plan.cell_proj_ptr[c + 1]; ++r) row_cell[r] = (int32_t)c;
+  int32_t* d_row_cell = nullptr; double* d_rows = nullptr;
+  if ((e = cudaMalloc((void**)&d_row_cell, row_cell.size() * sizeof(int32_t)))) return e;
+  if ((e = cudaMalloc((void**)&d_rows, (size_t)op->nnz_cp * mc * sizeof(double)))) { cudaFree(d_row_cell); return e; }
+  std::vector<double> rows((size_t)op->nnz_cp * mc);
+  e = cudaMemcpyAsync(d_row_cell, row_cell.data(), row_cell.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st);
+  if (e == cudaSuccess) {
+    if (op->precision == 64)
+      k_extract_proj_rows<double><<<(unsigned)op->nnz_cp, 128, 0, st>>>(reinterpret_cast<const double*>(op->mat), op->mat_off,
+                                                                       op->cell_proj_ptr, d_row_cell, mc, op->mpad, op->lda, d_rows);
+    else
+      k_extract_proj_rows<float><<<(unsigned)op->nnz_cp, 128, 0, st>>>(reinterpret_cast<const float*>(op->mat), op->mat_off,
+                                                                      op->cell_proj_ptr, d_row_cell, mc, op->mpad, op->lda, d_rows);
+    e = cudaGetLastError();
+  }
+  if (e == cudaSuccess) e = cudaMemcpyAsync(rows.data(), d_rows, rows.size() * sizeof(double), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  cudaFree(d_row_cell); cudaFree(d_rows);
+  if (e != cudaSuccess) return e;
+  // 2. assembly over the cells of each projector, in the caller's CSR order (deterministic)
+  std::vector<double> coef((size_t)op->n_prow * kProjGroup, 0.0);
+  std::vector<int32_t> loc((size_t)op->n_dofs, -1);
+  for (int grp = 0; grp < plan.n_groups; ++grp) {
+    for (int32_t r = plan.grp_row_ptr[grp]; r < plan.grp_row_ptr[grp + 1]; ++r) loc[plan.grow_dof[r]] = r;
+    for (int i = 0; i < kProjGroup; ++i) {
+      const int32_t j = plan.grp_proj[(size_t)grp * kProjGroup + i];
+      if (j < 0) continue;
+      for (int64_t k = plan.proj_ptr[j]; k < plan.proj_ptr[j + 1]; ++k) {
+        const int64_t pr = plan.proj_pcrow[k];
+        const int64_t c = row_cell[pr];
+        for (int l = 0; l < mc; ++l) coef[(size_t)loc[mesh.cell_dofs[c * mc + l]] * kProjGroup + i] += rows[(size_t)pr * mc + l];
+      }
+    }
+  }
+  // 3. upload in the operator's storage type
+  if ((e = cudaMalloc(&op->pcoef, coef.size() * elt))) return e;
+  if (op->precision == 64) {
+    e = cudaMemcpyAsync(op->pcoef, coef.data(), coef.size() * sizeof(double), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  } else {
+    std::vector<float> cf(coef.begin(), coef.end());
+    e = cudaMemcpyAsync(op->pcoef, cf.data(), cf.size() * sizeof(float), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  }
+  if (e != cudaSuccess) return e;
+  op->n_pseg = (int64_t)plan.seg_ptr.size() - 1;
+  return cudaSuccess;
+}
 
 cudaError_t capture_diagonal(Op* op, cudaStream_t st) {
   const int64_t n = op->n_cells * op->m_cell;

@@ -26,6 +26,8 @@
 namespace chfsi {
 
 constexpr uint32_t kFirstBit = 0x80000000u;
+constexpr int kProjGroup = 8;            // projectors per group (slots of a coefficient row)
+constexpr int kProjSegRows = 128;        // dof rows per CTA of the projector-coefficient kernel
 
 // ---- host-side tables and mesh analysis (host_setup.cpp) -------------------------------------------------
 struct Tables1D {
@@ -57,6 +59,17 @@ struct HostPlan {
   std::vector<int64_t> proj_ptr;         // [n_proj+1]
   std::vector<int64_t> proj_pcrow;       // [nnz] row of Pc
   std::vector<int32_t> pc_cells;         // cells that have projectors
+  // dof-centric projector lists: projectors with the same support (one atom's) form a group of <= 8; the rows of a
+  // group are the dofs of its support cells; the assembly over cells of Alg. 4 step 3 is applied to
+  // C ONCE at setup (coefficients s_g sum_c C^c[l(g)][j]), so that per apply every dof row of X is read once per
+  // group instead of once per (cell, group).  Segments of <= kProjSegRows rows are the CTAs of k_proj_rows.
+  int n_groups = 0;
+  std::vector<int32_t> grp_row_ptr;      // [n_groups+1]
+  std::vector<int32_t> grow_dof;         // [n_rows] global dof, ascending inside a group
+  std::vector<int32_t> grp_proj;         // [n_groups][8] projector ids, -1 = unused slot
+  std::vector<int32_t> seg_ptr;          // [n_seg+1] row ranges; a segment never straddles two groups
+  std::vector<int32_t> grp_seg_ptr;      // [n_groups+1]
+  std::vector<int32_t> proj_grp, proj_slot;   // [n_proj]
   std::vector<double> mass;              // [n_dofs] diagonal GLL mass
 };
 // Returns "" on success, else an error message (bad mesh).
@@ -87,6 +100,14 @@ struct Op {
   int64_t* cell_proj_ptr = nullptr;      // [n_cells+1]  (row offsets into Pc)
   int64_t* proj_ptr = nullptr;
   int64_t* proj_pcrow = nullptr;
+  // dof-centric projector data (HostPlan): segments, rows, assembled coefficients [n_prow][8] (element type T)
+  int64_t n_pseg = 0, n_prow = 0;
+  int32_t* seg_ptr = nullptr;
+  int32_t* grow_dof = nullptr;
+  void* pcoef = nullptr;
+  int32_t* grp_seg_ptr = nullptr;
+  int32_t* proj_grp = nullptr;
+  int32_t* proj_slot = nullptr;
   double* D = nullptr;
   double* mass = nullptr;
   // Spectral shift folded into the cell matrices: diag0 [n_cells][m_cell] keeps the unshifted diagonal entries
@@ -119,7 +140,7 @@ struct ApplyArgs {
   int64_t B = 0;
   double alpha = 1.0, beta = 0.0, cshift = 0.0;  // Y_k = alpha (H~ X - cshift X) - beta T
   void* P = nullptr;                             // [n_proj+1][B]
-  void* Pc = nullptr;                            // [nnz_cp][B]
+  void* Pc = nullptr;                            // [n_pseg][8][B] FP64 partial coefficients of the row segments
   // single-launch deterministic assembly: ticket counter (slot 0, 64-bit) and per-(position, column tile)
   // completion flags, zeroed by the caller of launch_apply before epoch 1; epoch increases by one per launch
   unsigned long long* sync = nullptr;
@@ -127,6 +148,9 @@ struct ApplyArgs {
 };
 // Enqueues one fused H~ application + recurrence update.  Returns cudaGetLastError().
 cudaError_t launch_apply(Op* op, const ApplyArgs& a, cudaStream_t stream);
+// Builds op->pcoef: the projector rows of the cell matrices summed over the cells of each dof (once, at create,
+// after build_cell_matrices; deterministic host summation in the caller's CSR order).
+cudaError_t assemble_projector_rows(Op* op, const HostPlan& plan, const chfsi_mesh& mesh, cudaStream_t stream);
 // Copies the diagonal of every cell matrix into op->diag0 (once, at create, after build_cell_matrices).
 cudaError_t capture_diagonal(Op* op, cudaStream_t stream);
 // Opts the kernels into the shared memory they need for this operator (once, at create).

@@ -7,6 +7,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstring>
+#include <map>
 
 #include "common.h"
 
@@ -257,6 +258,49 @@ std::string analyse_mesh(const chfsi_mesh& mesh, const chfsi_nonlocal* nl, const
   plan->pc_cells.clear();
   for (int64_t c = 0; c < nc; ++c)
     if (plan->cell_proj_ptr[c + 1] > plan->cell_proj_ptr[c]) plan->pc_cells.push_back((int32_t)c);
+
+  // ---- dof-centric projector groups (same support = same atom), their dof rows and the CTA segments --------
+  plan->n_groups = 0;
+  plan->grp_row_ptr.assign(1, 0);
+  plan->grow_dof.clear(); plan->grp_proj.clear();
+  plan->seg_ptr.assign(1, 0); plan->grp_seg_ptr.assign(1, 0);
+  plan->proj_grp.assign(n_proj, 0); plan->proj_slot.assign(n_proj, 0);
+  if (n_proj) {
+    std::map<std::vector<int32_t>, std::vector<int32_t>> by_support;   // ordered: deterministic group numbering
+    for (int64_t j = 0; j < n_proj; ++j) {
+      std::vector<int32_t> cells(nl->proj_cell_idx + nl->proj_cell_ptr[j], nl->proj_cell_idx + nl->proj_cell_ptr[j + 1]);
+      std::sort(cells.begin(), cells.end());
+      by_support[cells].push_back((int32_t)j);
+    }
+    std::vector<uint8_t> in_grp(nd, 0);
+    for (const auto& kv : by_support) {
+      const std::vector<int32_t>& cells = kv.first;
+      if (cells.empty()) {   // projector without support: its coefficient is zero; give it an empty group
+        for (int32_t j : kv.second) { plan->proj_grp[j] = -1; plan->proj_slot[j] = 0; }
+        continue;
+      }
+      std::vector<int32_t> dofs;
+      for (int32_t c : cells)
+        for (int l = 0; l < mc; ++l) {
+          int32_t g = mesh.cell_dofs[(int64_t)c * mc + l];
+          if (!in_grp[g]) { in_grp[g] = 1; dofs.push_back(g); }
+        }
+      std::sort(dofs.begin(), dofs.end());
+      for (int32_t g : dofs) in_grp[g] = 0;
+      for (size_t i0 = 0; i0 < kv.second.size(); i0 += kProjGroup) {
+        const int grp = plan->n_groups++;
+        const size_t ni = std::min<size_t>(kProjGroup, kv.second.size() - i0);
+        for (int i = 0; i < kProjGroup; ++i) plan->grp_proj.push_back((size_t)i < ni ? kv.second[i0 + i] : -1);
+        for (size_t i = 0; i < ni; ++i) { plan->proj_grp[kv.second[i0 + i]] = grp; plan->proj_slot[kv.second[i0 + i]] = (int32_t)i; }
+        const int32_t r0 = (int32_t)plan->grow_dof.size();
+        plan->grow_dof.insert(plan->grow_dof.end(), dofs.begin(), dofs.end());
+        const int32_t r1 = (int32_t)plan->grow_dof.size();
+        plan->grp_row_ptr.push_back(r1);
+        for (int32_t r = r0; r < r1; r += kProjSegRows) plan->seg_ptr.push_back(std::min(r1, r + kProjSegRows));
+        plan->grp_seg_ptr.push_back((int32_t)plan->seg_ptr.size() - 1);
+      }
+    }
+  }
 
   // ---- per-cell layout: K_c, matrix offsets, gather/scatter index lists with first-contribution flags --------
   // rows 0..mc-1: nodes; rows mc..mpad-1: padding (zero matrix rows, gather any valid dof); rows mpad..: projectors.
