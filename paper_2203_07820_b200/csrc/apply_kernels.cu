@@ -413,7 +413,6 @@ constexpr int kP2Threads = 256;
 // ring depth: 4 stages of 24 KB for FP64 storage, 8 stages of 12 KB for FP32 storage; panels in flight = stages - 2
 // (one slot of slack so that a producer never waits for the previous producer, which lags by its own issue time)
 template <typename S> __host__ __device__ constexpr int p2_stages() { return sizeof(S) == 8 ? 4 : 8; }
-constexpr int kP2L2Ahead = 6;           // cell-matrix panels prefetched into L2 beyond the ring
 constexpr int kSyncFlagOffset = 32;     // uint32 index of the first flag inside the sync region (128 bytes)
 
 struct PersistDev {
@@ -440,9 +439,6 @@ struct PersistDev {
 
 __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void bulk_prefetch_l2(const void* src, uint32_t bytes) {
-  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
 }
 // four rows r0..r3 of a 2-D tensor (columns c0 .. c0+box-1) -> four consecutive box-wide rows at dst
 __device__ __forceinline__ void tma_gather4(void* dst, const CUtensorMap* tm, int c0, int r0, int r1, int r2, int r3,
@@ -567,8 +563,6 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<S> a, P
                   idx_s[k0 + 3] & 0x7fffffff, &full[s]);
       tma_gather4(Xs + 4 * kP2LdXs, tm, col0, idx_s[k0 + 4] & 0x7fffffff, idx_s[k0 + 5] & 0x7fffffff,
                   idx_s[k0 + 6] & 0x7fffffff, idx_s[k0 + 7] & 0x7fffffff, &full[s]);
-      const int pf = pj + kP2L2Ahead;   // pull a later panel of the cell matrix into L2 ahead of the ring
-      if (pf < npanel) bulk_prefetch_l2(M + (int64_t)pf * a_panel_elems, a_bytes);
 #ifdef CHFSI_TRACE
       if (tr_p) tr_p[8] += clock64() - te1;
 #endif
