@@ -43,8 +43,9 @@ def parse_args():
     ap.add_argument("--config", type=int, default=DEFAULT_CONFIG, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--assembly", type=int, default=0, choices=[0, 1],
                     help="0 deterministic coloured assembly, 1 atomic assembly")
-    ap.add_argument("--variant", type=int, default=0, choices=[0, 1, 2],
-                    help="contraction kernel: 0 default (persistent single launch), 1 generic, 2 one launch per colour")
+    ap.add_argument("--variant", type=int, default=0, choices=[0, 1, 2, 3],
+                    help="contraction kernel: 0 default (persistent single launch), 1 generic, 2 one launch per colour, "
+                         "3 FP32 storage with 3xTF32 products (opt-in, looser accuracy)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -250,7 +251,10 @@ def run_b200(args, spec):
     n_apply = prof["applies"]
     cols_total = N * m * args.steps                           # column-applies covered by the profile
     contr_tflops = contr_flops_per_apply * cols_total / (prof["contraction_ms"] * 1e-3) * 1e-12 if prof["contraction_ms"] > 0 else None
-    if spec.precision == 64 or args.variant == 0:
+    if spec.precision == 32 and args.variant == 3:
+        peak, bound, peak_note = 277.3 / 3.0, "tensor", \
+            "mma.sync m16n8k8 TF32 rate measured on B200 (277.3 TFLOP/s, round-1 microbenchmark) / 3 passes per FP32 product"
+    elif spec.precision == 64 or args.variant == 0:
         # the FP32 variant stores matrices and vectors in FP32 and contracts them on the same FP64 tensor pipe
         peak, bound, peak_note = peaks["dmma_tflops"], "tensor", \
             "FP64 mma.sync m8n8k4 (DMMA) rate measured in this run by chfsi_measure_fp64_peak; MEASURED_PEAKS.json has no FP64 figure"
@@ -259,7 +263,7 @@ def run_b200(args, spec):
     key = (spec.config, args.assembly)
     roofline = {
         "kernel": ({0: "k_apply_dmma_p<double>", 1: "k_apply_generic<double>", 2: "k_apply_dmma"}[args.variant]
-                   if spec.precision == 64 else {0: "k_apply_dmma_p<float>"}.get(args.variant, "k_apply_generic<float>")),
+                   if spec.precision == 64 else {0: "k_apply_dmma_p<float>", 3: "k_apply_tf32_p"}.get(args.variant, "k_apply_generic<float>")),
         "bound": bound, "achieved": contr_tflops, "peak": peak, "unit": "TFLOP/s",
         "frac": (contr_tflops / peak) if contr_tflops else None,
         "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(key),
@@ -307,7 +311,9 @@ def run_b200(args, spec):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None,
-            "dtype": "f64" if spec.precision == 64 else "f64 accumulate on f32-stored matrices and vectors",
+            "dtype": ("f64" if spec.precision == 64 else
+                      "f32 (3xTF32 products, f32 accumulate)" if args.variant == 3 else
+                      "f64 accumulate on f32-stored matrices and vectors"),
             "data": "synthetic",
             "config": {"workload": workload_name(spec), "assembly": "coloured" if args.assembly == 0 else "atomic",
                        "n_colors": info["n_colors"], "bounds": {"a0": a0, "a": a, "b": b},

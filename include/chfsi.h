@@ -135,7 +135,8 @@ int64_t chfsi_launch_count(const chfsi_op* op);
 
 /* Selects the kernel used for the per-cell contraction: 0 = automatic (single-launch persistent tensor-core
  * kernel when the shape allows), 1 = force the generic path, 2 = the earlier tensor-core kernel with one launch
- * per colour.  For tests and A/B measurements. */
+ * per colour, 3 = (FP32 storage only) 3xTF32 products on the 32-bit tensor pipe: faster, but outside the 1e-5 Ha
+ * eigenvalue tolerance of the FP32 variant (see csrc/apply_tf32.cuh).  For tests and A/B measurements. */
 int chfsi_set_kernel_variant(chfsi_op* op, int variant);
 
 /* Per-kernel device timing for the roofline report.  While enabled, every H~ application records one CUDA

@@ -374,7 +374,7 @@ int64_t chfsi_launch_count(const chfsi_op* op) { return op ? op->launches : -1; 
 
 int chfsi_set_kernel_variant(chfsi_op* op, int variant) {
   if (!op) return CHFSI_ERR_BAD_ARGUMENT;
-  if (variant < 0 || variant > 2) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "variant must be 0, 1 or 2");
+  if (variant < 0 || variant > 3) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "variant must be 0, 1, 2 or 3");
   op->variant = variant;
   return CHFSI_OK;
 }

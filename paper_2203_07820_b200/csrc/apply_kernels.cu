@@ -697,7 +697,9 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<S> a, P
   }
 }
 
-// Tensor map of a row-major FP64 / FP32 block [rows][ld] restricted to its first `cols` columns, box = kP2TileN x 1
+#include "apply_tf32.cuh"
+
+// Tensor map of a row-major FP64 / FP32 block [rows][ld] restricted to its first `cols` columns, box = box_cols x 1
 // (tile::gather4 picks four such rows per instruction); columns beyond `cols` read as zero.
 using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                    const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -713,12 +715,12 @@ EncodeTiledFn encode_tiled_fn() {
   }();
   return fn;
 }
-bool make_row_gather_map(CUtensorMap* tm, const void* base, int64_t rows, int64_t cols, int64_t ld, int elt) {
+bool make_row_gather_map(CUtensorMap* tm, const void* base, int64_t rows, int64_t cols, int64_t ld, int elt, int box_cols) {
   EncodeTiledFn enc = encode_tiled_fn();
   if (!enc || rows < 1 || cols < 1 || (ld * elt) % 16 != 0 || (uintptr_t)base % 16 != 0) return false;
   const cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
   const cuuint64_t strides[1] = {(cuuint64_t)ld * (cuuint64_t)elt};
-  const cuuint32_t box[2] = {(cuuint32_t)kP2TileN, 1};
+  const cuuint32_t box[2] = {(cuuint32_t)box_cols, 1};
   const cuuint32_t estr[2] = {1, 1};
   return enc(tm, elt == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<void*>(base), dims, strides, box, estr,
              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -794,11 +796,21 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
   // variant 0: persistent single-launch kernel (v2); variant 2: one launch per colour (v1); variant 1: generic
   bool fast2 = false, fast = false;
   int MT = (n_mtiles + 3) / 4;
+  // variant 0: persistent single-launch kernel, FP64 DMMA accumulation for both storage types;
+  // variant 3 (FP32 storage only, opt-in): persistent kernel with 3xTF32 products on the 32-bit tensor pipe -- 1.3x
+  // faster, but the FP32 tensor accumulator truncates: |dY|/|Y| ~ 2e-6 per apply, Ritz values off by up to 4e-5 Ha,
+  // i.e. inside the 1e-4 block tolerance but outside the 1e-5 Ha eigenvalue tolerance of the FP32 variant
   CUtensorMap tmX, tmP;
-  if (aligned && op->variant == 0 && g.sync != nullptr && g.epoch > 0)
+  bool fast3 = false;   // 3xTF32 kernel
+  const int MT16 = ((op->m_cell + 15) / 16 + 1) / 2;
+  if (sizeof(T) == 4 && aligned && op->variant == 3 && g.sync != nullptr && g.epoch > 0)
+    fast3 = (MT16 == 11 || MT16 == 7 || MT16 == 4 || MT16 == 2 || MT16 == 1) && t3_smem_bytes(op) <= 113 * 1024 &&
+            make_row_gather_map(&tmX, g.X, op->n_dofs, B, g.ldx, 4, kT3TileN) &&
+            make_row_gather_map(&tmP, g.P, op->n_proj + 1, B, B, 4, kT3TileN);
+  if (aligned && !fast3 && op->variant == 0 && g.sync != nullptr && g.epoch > 0)
     fast2 = (MT == 11 || MT == 7 || MT == 4 || MT == 2 || MT == 1) && p2_smem_bytes<T>(op) <= 113 * 1024 &&
-            make_row_gather_map(&tmX, g.X, op->n_dofs, B, g.ldx, (int)sizeof(T)) &&
-            make_row_gather_map(&tmP, g.P, op->n_proj + 1, B, B, (int)sizeof(T));
+            make_row_gather_map(&tmX, g.X, op->n_dofs, B, g.ldx, (int)sizeof(T), kP2TileN) &&
+            make_row_gather_map(&tmP, g.P, op->n_proj + 1, B, B, (int)sizeof(T), kP2TileN);
   if (sizeof(T) == 8 && aligned && !fast2 && op->variant != 1) fast = (MT == 11 || MT == 4 || MT == 2 || MT == 7);
   size_t smem_fast = (size_t)kStages * (kPanelK * op->lda + kPanelK * kLdXs) * sizeof(double) + kStages * sizeof(uint64_t) +
                      (size_t)op->max_ktot * sizeof(int32_t);
@@ -813,6 +825,33 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
     op->prof_proj_launches += op->launches - launches_before;
   }
   const int64_t launches_mid = op->launches;
+  if (fast3) {
+    if constexpr (sizeof(T) == 4) {
+      a.cells = nullptr; a.n_launch_cells = (int)op->n_cells;
+      a.n_col_tiles = (B + kT3TileN - 1) / kT3TileN;
+      PersistDev pd;
+      pd.pos_cell = op->color_cells; pd.dep_ptr = op->dep_ptr; pd.dep_pos = op->dep_pos;
+      pd.counter = g.sync;
+      pd.flags = reinterpret_cast<uint32_t*>(g.sync) + kSyncFlagOffset;
+      pd.epoch = g.epoch;
+      const int64_t n_tiles = op->n_cells * a.n_col_tiles;
+      const unsigned grid = (unsigned)std::min<int64_t>(n_tiles, 2 * (int64_t)op->n_sm);
+      pd.n_tiles = (int)n_tiles;
+      pd.ticket_base = (unsigned long long)(g.epoch - 1) * (unsigned long long)(n_tiles + grid);
+#ifdef CHFSI_TRACE
+      pd.trace = nullptr; pd.debug_flags = 0;
+#endif
+      const size_t sm = t3_smem_bytes(op);
+      switch (MT16) {
+        case 11: k_apply_tf32_p<11><<<grid, kP2Threads, sm, st>>>(a, pd, tmX, tmP); break;
+        case 7: k_apply_tf32_p<7><<<grid, kP2Threads, sm, st>>>(a, pd, tmX, tmP); break;
+        case 4: k_apply_tf32_p<4><<<grid, kP2Threads, sm, st>>>(a, pd, tmX, tmP); break;
+        case 2: k_apply_tf32_p<2><<<grid, kP2Threads, sm, st>>>(a, pd, tmX, tmP); break;
+        case 1: k_apply_tf32_p<1><<<grid, kP2Threads, sm, st>>>(a, pd, tmX, tmP); break;
+      }
+      op->launches++;
+    }
+  }
   if (fast2) {
     {
       a.cells = nullptr; a.n_launch_cells = (int)op->n_cells;
@@ -844,7 +883,7 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
       op->launches++;
     }
   }
-  const int n_launch = fast2 ? 0 : (op->assembly == 1 ? 1 : op->n_colors);
+  const int n_launch = (fast2 || fast3) ? 0 : (op->assembly == 1 ? 1 : op->n_colors);
   for (int c = 0; c < n_launch; ++c) {
     if (op->assembly == 1) { a.cells = op->all_cells; a.n_launch_cells = (int)op->n_cells; }
     else { a.cells = op->color_cells + op->color_ptr[c]; a.n_launch_cells = op->color_ptr[c + 1] - op->color_ptr[c]; }
@@ -904,6 +943,14 @@ cudaError_t init_apply_kernels(Op* op) {
       if ((e = cudaFuncSetAttribute(k_apply_dmma_p<4, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p2))) return e;
       if ((e = cudaFuncSetAttribute(k_apply_dmma_p<2, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p2))) return e;
       if ((e = cudaFuncSetAttribute(k_apply_dmma_p<1, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p2))) return e;
+    }
+    const size_t smem_t3 = t3_smem_bytes(op);
+    if (smem_t3 <= 113 * 1024) {
+      if ((e = cudaFuncSetAttribute(k_apply_tf32_p<11>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_t3))) return e;
+      if ((e = cudaFuncSetAttribute(k_apply_tf32_p<7>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_t3))) return e;
+      if ((e = cudaFuncSetAttribute(k_apply_tf32_p<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_t3))) return e;
+      if ((e = cudaFuncSetAttribute(k_apply_tf32_p<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_t3))) return e;
+      if ((e = cudaFuncSetAttribute(k_apply_tf32_p<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_t3))) return e;
     }
   }
   size_t smem_gen = (size_t)op->max_ktot * 32 * 8;
