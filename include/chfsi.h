@@ -102,6 +102,16 @@ int chfsi_create(chfsi_op** out, const chfsi_mesh* mesh, const chfsi_potential* 
                  const chfsi_nonlocal* nl /* nullable */, int precision /* 64 | 32 */,
                  int assembly /* 0 | 1 */, void* cuda_stream);
 int chfsi_destroy(chfsi_op* op);
+
+/* New V_eff on the same mesh and projectors: recomputes the Hamiltonian part of every cell matrix,
+ *   H^e_jk = 1/2 K^e_jk + sum_q w_q detJ_q V_eff(q) N_j(q) N_k(q)     (Eq. 30 terms 1-2; Eq. 40,
+ *   PAPER.md:462-464), Loewdin-scaled (Eq. 34),
+ * which is the DHM step of every SCF iteration (Algorithm 1 step 4: V_eff changes with the density).
+ * pot->veff_q is a HOST pointer [n_cells][(p+2)^3] (x fastest), copied during the call; projector rows, mesh
+ * analysis, colouring and all buffers are reused.  The work is enqueued on cuda_stream and the call returns after
+ * synchronising it (the host array may be released).  Must not overlap an apply / filter running on the same
+ * handle.  Errors: CHFSI_ERR_BAD_ARGUMENT (NULL), CHFSI_ERR_OUT_OF_MEMORY / CHFSI_ERR_CUDA (temporary buffers). */
+int chfsi_update_potential(chfsi_op* op, const chfsi_potential* pot, void* cuda_stream);
 int chfsi_get_info(const chfsi_op* op, chfsi_info* info);
 
 /* Device workspace (bytes) that chfsi_apply_H / chfsi_chebyshev_filter need for a block of B columns. */

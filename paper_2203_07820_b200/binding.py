@@ -19,7 +19,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libchfsi.so")
 
 EXPORTED_SYMBOLS = [
-    "chfsi_create", "chfsi_destroy", "chfsi_get_info", "chfsi_workspace_bytes", "chfsi_mass_diag",
+    "chfsi_create", "chfsi_destroy", "chfsi_update_potential", "chfsi_get_info", "chfsi_workspace_bytes", "chfsi_mass_diag",
     "chfsi_apply_H", "chfsi_chebyshev_filter", "chfsi_chebyshev_filter_chunked", "chfsi_chebyshev_filter_host",
     "chfsi_launch_count", "chfsi_set_kernel_variant", "chfsi_set_profiling", "chfsi_get_profile",
     "chfsi_measure_fp64_peak", "chfsi_last_error",
@@ -80,6 +80,8 @@ def load_library(build_if_missing: bool = True):
     lib_.chfsi_create.restype = C.c_int
     lib_.chfsi_destroy.argtypes = [vp]
     lib_.chfsi_destroy.restype = C.c_int
+    lib_.chfsi_update_potential.argtypes = [vp, C.POINTER(_Potential), vp]
+    lib_.chfsi_update_potential.restype = C.c_int
     lib_.chfsi_get_info.argtypes = [vp, C.POINTER(_Info)]
     lib_.chfsi_get_info.restype = C.c_int
     lib_.chfsi_workspace_bytes.argtypes = [vp, i64, C.POINTER(C.c_size_t)]
@@ -269,6 +271,12 @@ class Operator:
 
     def launch_count(self) -> int:
         return int(load_library().chfsi_launch_count(self._h))
+
+    def update_potential(self, veff_q, stream=None):
+        """chfsi_update_potential: new V_eff samples [n_cells][(p+2)^3] (host array) on the same mesh/projectors."""
+        v = np.ascontiguousarray(veff_q, dtype=np.float64)
+        pot = _Potential(_np_ptr(v))
+        self._check(load_library().chfsi_update_potential(self._h, C.byref(pot), _stream_ptr(stream)))
 
     def set_kernel_variant(self, variant: int):
         self._check(load_library().chfsi_set_kernel_variant(self._h, int(variant)))

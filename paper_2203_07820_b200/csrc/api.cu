@@ -48,7 +48,8 @@ void free_op(chfsi_op* op) {
   cudaFree(op->mat); cudaFree(op->mat_off); cudaFree(op->idx_off); cudaFree(op->ktot); cudaFree(op->gidx);
   cudaFree(op->color_cells); cudaFree(op->dep_ptr); cudaFree(op->dep_pos); cudaFree(op->all_cells); cudaFree(op->pc_cells); cudaFree(op->cell_proj_ptr);
   cudaFree(op->proj_ptr); cudaFree(op->proj_pcrow); cudaFree(op->seg_ptr); cudaFree(op->grow_dof); cudaFree(op->pcoef);
-  cudaFree(op->grp_seg_ptr); cudaFree(op->proj_grp); cudaFree(op->proj_slot); cudaFree(op->D); cudaFree(op->mass); cudaFree(op->diag0);
+  cudaFree(op->grp_seg_ptr); cudaFree(op->proj_grp); cudaFree(op->proj_slot);
+  cudaFree(op->setup_verts); cudaFree(op->setup_pp); cudaFree(op->setup_phi); cudaFree(op->setup_gx); cudaFree(op->setup_gw); cudaFree(op->D); cudaFree(op->mass); cudaFree(op->diag0);
   for (cudaEvent_t e : op->prof_events) cudaEventDestroy(e);
   delete op;
 }
@@ -238,6 +239,19 @@ int chfsi_create(chfsi_op** out, const chfsi_mesh* mesh, const chfsi_potential* 
 int chfsi_destroy(chfsi_op* op) {
   if (!op) return CHFSI_ERR_BAD_ARGUMENT;
   free_op(op);
+  return CHFSI_OK;
+}
+
+int chfsi_update_potential(chfsi_op* op, const chfsi_potential* pot, void* cuda_stream) {
+  if (!op) return CHFSI_ERR_BAD_ARGUMENT;
+  if (!pot || !pot->veff_q) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "NULL potential pointer");
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  cudaError_t ce = rebuild_local_matrices(op, pot->veff_q, st);
+  if (ce != cudaSuccess) return cuda_fail(op, ce, "update_potential (cell matrices)");
+  ce = capture_diagonal(op, st);      // new unshifted diagonals; the spectral shift of the last filter is gone
+  if (ce == cudaSuccess) ce = cudaStreamSynchronize(st);
+  if (ce != cudaSuccess) return cuda_fail(op, ce, "update_potential (diagonal)");
+  op->launches += 2;
   return CHFSI_OK;
 }
 

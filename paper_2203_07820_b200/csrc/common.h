@@ -116,6 +116,12 @@ struct Op {
   // "c1 H~ + c2") and the recurrence epilogue never re-reads X.
   double* diag0 = nullptr;
   double cur_shift = 0.0;
+  // kept from create for chfsi_update_potential: cell vertices and the 1-D tables of the setup kernels
+  double* setup_verts = nullptr;         // [n_cells][24]
+  double* setup_pp = nullptr;            // [4][nq1][n1*n1]
+  double* setup_phi = nullptr;           // [nq1][n1]
+  double* setup_gx = nullptr;            // [nq1]
+  double* setup_gw = nullptr;            // [nq1]
   int64_t launches = 0;
   // optional per-kernel timing (chfsi_set_profiling): event triples (start, after projector kernels, end)
   bool profiling = false;
@@ -132,6 +138,9 @@ struct Op {
 cudaError_t build_cell_matrices(Op* op, const HostPlan& plan, const Tables1D& tab, const chfsi_mesh& mesh,
                                 const chfsi_potential& pot, const chfsi_nonlocal* nl, cudaStream_t stream,
                                 bool* bad_jacobian);
+// Recomputes the Hamiltonian rows (rows 0..M_cell-1) of every cell matrix for a new V_eff (HOST pointer
+// [n_cells][(p+2)^3]); projector rows, layout and colouring are untouched.  Synchronises the stream.
+cudaError_t rebuild_local_matrices(Op* op, const double* veff_q_host, cudaStream_t stream);
 
 // ---- apply kernels (apply_kernels.cu) ----------------------------------------------------------------------
 struct ApplyArgs {

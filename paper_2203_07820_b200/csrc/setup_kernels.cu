@@ -75,7 +75,8 @@ __global__ void __launch_bounds__(256) k_cell_matrix(int n1, int nq1, int64_t n_
                                                      const int32_t* __restrict__ gidx, const int64_t* __restrict__ idx_off,
                                                      const int64_t* __restrict__ mat_off, const int32_t* __restrict__ ktot,
                                                      const double* __restrict__ mass, int lda, T* __restrict__ mat,
-                                                     double* __restrict__ scratch64, int* __restrict__ bad_flag) {
+                                                     double* __restrict__ scratch64, int* __restrict__ bad_flag,
+                                                     int zero_tail) {
   extern __shared__ double smem[];
   const int nn = n1 * n1, nq2 = nq1 * nq1, nq = nq1 * nq2, mc = n1 * nn;
   double* Wf = smem;                    // [10][nq]
@@ -149,7 +150,8 @@ __global__ void __launch_bounds__(256) k_cell_matrix(int n1, int nq1, int64_t n_
       M[o] = (T)v;
     }
     // padding rows beyond the projector rows (and the projector rows themselves, filled later) start at zero
-    for (int o = mc * lda + threadIdx.x; o < ktot[c] * lda; o += blockDim.x) M[o] = (T)0;
+    if (zero_tail)
+      for (int o = mc * lda + threadIdx.x; o < ktot[c] * lda; o += blockDim.x) M[o] = (T)0;
   }
 }
 
@@ -222,16 +224,56 @@ cudaError_t upload(U** dst, const U* src, size_t n, cudaStream_t st) {
 
 #define CK(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) { err = e_; goto done; } } while (0)
 
+namespace {
+// Hamiltonian rows of all cell matrices from V_eff at the Gauss points (host pointer); op->setup_* must exist.
+cudaError_t launch_local_matrices(Op* op, const double* veff_host, cudaStream_t stream, int zero_tail, bool* bad_jacobian) {
+  cudaError_t err = cudaSuccess;
+  const int n1 = op->n1, nq1 = op->nq1, nn = n1 * n1, nq = nq1 * nq1 * nq1, mc = n1 * nn;
+  const int64_t nc = op->n_cells;
+  double *d_veff = nullptr, *d_scratch = nullptr;
+  int* d_bad = nullptr;
+  int h_bad = 0;
+  CK(upload(&d_veff, veff_host, (size_t)nc * nq, stream));
+  CK(upload(&d_bad, &h_bad, 1, stream));
+  {
+    SetupTables tb{op->setup_pp, op->setup_phi, op->setup_gx, op->setup_gw};
+    int grid = (int)std::min<int64_t>(nc, 296);
+    CK(cudaMalloc((void**)&d_scratch, (size_t)grid * mc * mc * sizeof(double)));
+    size_t smem = ((size_t)10 * nq + (size_t)nn * nq1 * nq1 + (size_t)4 * nq1 * nn + 24) * sizeof(double);
+    if (op->precision == 64) {
+      CK(cudaFuncSetAttribute(k_cell_matrix<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      k_cell_matrix<double><<<grid, 256, smem, stream>>>(n1, nq1, nc, tb, op->setup_verts, d_veff, op->gidx, op->idx_off,
+                                                         op->mat_off, op->ktot, op->mass, op->lda, (double*)op->mat,
+                                                         d_scratch, d_bad, zero_tail);
+    } else {
+      CK(cudaFuncSetAttribute(k_cell_matrix<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      k_cell_matrix<float><<<grid, 256, smem, stream>>>(n1, nq1, nc, tb, op->setup_verts, d_veff, op->gidx, op->idx_off,
+                                                        op->mat_off, op->ktot, op->mass, op->lda, (float*)op->mat,
+                                                        d_scratch, d_bad, zero_tail);
+    }
+    CK(cudaGetLastError());
+    CK(cudaMemcpyAsync(&h_bad, d_bad, sizeof(int), cudaMemcpyDeviceToHost, stream));
+    CK(cudaStreamSynchronize(stream));
+    if (bad_jacobian) *bad_jacobian = (h_bad != 0);
+  }
+done:
+  cudaFree(d_veff); cudaFree(d_scratch); cudaFree(d_bad);
+  return err;
+}
+}  // namespace
+
+cudaError_t rebuild_local_matrices(Op* op, const double* veff_q_host, cudaStream_t stream) {
+  return launch_local_matrices(op, veff_q_host, stream, /*zero_tail=*/0, nullptr);
+}
+
 cudaError_t build_cell_matrices(Op* op, const HostPlan& plan, const Tables1D& tab, const chfsi_mesh& mesh,
                                 const chfsi_potential& pot, const chfsi_nonlocal* nl, cudaStream_t stream,
                                 bool* bad_jacobian) {
   cudaError_t err = cudaSuccess;
-  const int n1 = tab.n1, nq1 = tab.nq1, nn = n1 * n1, nq = nq1 * nq1 * nq1, mc = n1 * nn;
+  const int n1 = tab.n1, nq1 = tab.nq1, nn = n1 * n1, nq = nq1 * nq1 * nq1;
   const int64_t nc = op->n_cells;
-  double *d_pp = nullptr, *d_phi = nullptr, *d_gx = nullptr, *d_gw = nullptr, *d_verts = nullptr, *d_veff = nullptr;
-  double *d_chi = nullptr, *d_scratch = nullptr;
-  int64_t* d_row_src = nullptr; int32_t* d_row_cell = nullptr; int* d_bad = nullptr;
-  int h_bad = 0;
+  double* d_chi = nullptr;
+  int64_t* d_row_src = nullptr; int32_t* d_row_cell = nullptr;
   std::vector<double> pp((size_t)4 * nq1 * nn);
   for (int idx = 0; idx < 4; ++idx)
     for (int q = 0; q < nq1; ++q)
@@ -245,52 +287,31 @@ cudaError_t build_cell_matrices(Op* op, const HostPlan& plan, const Tables1D& ta
   for (int64_t c = 0; c < nc; ++c)
     for (int64_t r = plan.cell_proj_ptr[c]; r < plan.cell_proj_ptr[c + 1]; ++r) row_cell[r] = (int32_t)c;
 
-  CK(upload(&d_pp, pp.data(), pp.size(), stream));
-  CK(upload(&d_phi, tab.phi.data(), tab.phi.size(), stream));
-  CK(upload(&d_gx, tab.gq_x.data(), tab.gq_x.size(), stream));
-  CK(upload(&d_gw, tab.gq_w.data(), tab.gq_w.size(), stream));
-  CK(upload(&d_verts, mesh.cell_vertices, (size_t)nc * 24, stream));
-  CK(upload(&d_veff, pot.veff_q, (size_t)nc * nq, stream));
-  CK(upload(&d_bad, &h_bad, 1, stream));
-  {
-    SetupTables tb{d_pp, d_phi, d_gx, d_gw};
-    int grid = (int)std::min<int64_t>(nc, 296);
-    CK(cudaMalloc((void**)&d_scratch, (size_t)grid * mc * mc * sizeof(double)));
-    size_t smem = ((size_t)10 * nq + (size_t)nn * nq1 * nq1 + (size_t)4 * nq1 * nn + 24) * sizeof(double);
-    if (op->precision == 64) {
-      CK(cudaFuncSetAttribute(k_cell_matrix<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-      k_cell_matrix<double><<<grid, 256, smem, stream>>>(n1, nq1, nc, tb, d_verts, d_veff, op->gidx, op->idx_off,
-                                                         op->mat_off, op->ktot, op->mass, op->lda, (double*)op->mat,
-                                                         d_scratch, d_bad);
-    } else {
-      CK(cudaFuncSetAttribute(k_cell_matrix<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-      k_cell_matrix<float><<<grid, 256, smem, stream>>>(n1, nq1, nc, tb, d_verts, d_veff, op->gidx, op->idx_off,
-                                                        op->mat_off, op->ktot, op->mass, op->lda, (float*)op->mat,
-                                                        d_scratch, d_bad);
-    }
+  CK(upload(&op->setup_pp, pp.data(), pp.size(), stream));
+  CK(upload(&op->setup_phi, tab.phi.data(), tab.phi.size(), stream));
+  CK(upload(&op->setup_gx, tab.gq_x.data(), tab.gq_x.size(), stream));
+  CK(upload(&op->setup_gw, tab.gq_w.data(), tab.gq_w.size(), stream));
+  CK(upload(&op->setup_verts, mesh.cell_vertices, (size_t)nc * 24, stream));
+  CK(launch_local_matrices(op, pot.veff_q, stream, /*zero_tail=*/1, bad_jacobian));
+  if (op->nnz_cp > 0) {
+    SetupTables tb{op->setup_pp, op->setup_phi, op->setup_gx, op->setup_gw};
+    CK(upload(&d_chi, nl->chi_q, (size_t)op->nnz_cp * nq, stream));
+    CK(upload(&d_row_src, plan.cell_proj_src.data(), plan.cell_proj_src.size(), stream));
+    CK(upload(&d_row_cell, row_cell.data(), row_cell.size(), stream));
+    size_t smem2 = ((size_t)nq + (size_t)n1 * nq1 * nq1 + (size_t)nn * nq1 + (size_t)nq1 * n1 + 24) * sizeof(double);
+    if (op->precision == 64)
+      k_cell_projector<double><<<(unsigned)op->nnz_cp, 256, smem2, stream>>>(
+          n1, nq1, tb, op->setup_verts, d_chi, d_row_src, d_row_cell, op->cell_proj_ptr, op->gidx, op->idx_off, op->mat_off,
+          op->mass, op->lda, (double*)op->mat);
+    else
+      k_cell_projector<float><<<(unsigned)op->nnz_cp, 256, smem2, stream>>>(
+          n1, nq1, tb, op->setup_verts, d_chi, d_row_src, d_row_cell, op->cell_proj_ptr, op->gidx, op->idx_off, op->mat_off,
+          op->mass, op->lda, (float*)op->mat);
     CK(cudaGetLastError());
-    if (op->nnz_cp > 0) {
-      CK(upload(&d_chi, nl->chi_q, (size_t)op->nnz_cp * nq, stream));
-      CK(upload(&d_row_src, plan.cell_proj_src.data(), plan.cell_proj_src.size(), stream));
-      CK(upload(&d_row_cell, row_cell.data(), row_cell.size(), stream));
-      size_t smem2 = ((size_t)nq + (size_t)n1 * nq1 * nq1 + (size_t)nn * nq1 + (size_t)nq1 * n1 + 24) * sizeof(double);
-      if (op->precision == 64)
-        k_cell_projector<double><<<(unsigned)op->nnz_cp, 256, smem2, stream>>>(
-            n1, nq1, tb, d_verts, d_chi, d_row_src, d_row_cell, op->cell_proj_ptr, op->gidx, op->idx_off, op->mat_off,
-            op->mass, op->lda, (double*)op->mat);
-      else
-        k_cell_projector<float><<<(unsigned)op->nnz_cp, 256, smem2, stream>>>(
-            n1, nq1, tb, d_verts, d_chi, d_row_src, d_row_cell, op->cell_proj_ptr, op->gidx, op->idx_off, op->mat_off,
-            op->mass, op->lda, (float*)op->mat);
-      CK(cudaGetLastError());
-    }
-    CK(cudaMemcpyAsync(&h_bad, d_bad, sizeof(int), cudaMemcpyDeviceToHost, stream));
     CK(cudaStreamSynchronize(stream));
-    *bad_jacobian = (h_bad != 0);
   }
 done:
-  cudaFree(d_pp); cudaFree(d_phi); cudaFree(d_gx); cudaFree(d_gw); cudaFree(d_verts); cudaFree(d_veff);
-  cudaFree(d_chi); cudaFree(d_scratch); cudaFree(d_row_src); cudaFree(d_row_cell); cudaFree(d_bad);
+  cudaFree(d_chi); cudaFree(d_row_src); cudaFree(d_row_cell);
   return err;
 }
 

@@ -133,6 +133,36 @@ def test_fp32_3xtf32_variant_is_within_the_block_tolerance_and_reproducible():
         op.close()
 
 
+def test_update_potential_equals_a_fresh_operator_and_the_oracle():
+    """chfsi_update_potential (the per-SCF-iteration DHM step, Alg. 1 step 4): after the update the
+    operator is bit-identical to one created with the new V_eff, matches the oracle built from the new V_eff, and a
+    filter run BEFORE the update (which leaves its spectral shift on the matrix diagonals) does not leak into it."""
+    import dataclasses
+    torch, orc, Operator, _, _, _, _ = _imports()
+    wl, oop, X, (a0, a, b), Yo, Fo = oracle_case("p6_distorted_cells")
+    rng = np.random.default_rng(123)
+    veff2 = 0.6 * wl.veff_q - 0.25 + 0.05 * rng.standard_normal(wl.veff_q.shape)
+    wl2 = dataclasses.replace(wl, veff_q=veff2)
+    oop2 = orc.operator_from_workload(wl2)
+    for precision, tol in ((64, 1e-10), (32, 1e-4)):
+        Xr = X.astype(np.float32).astype(np.float64) if precision == 32 else X
+        op = Operator.from_workload(wl, precision=precision)
+        Xd = torch.tensor(Xr, dtype=op.dtype, device="cuda")
+        F = Xd.clone()
+        op.chebyshev_filter(F, 4, a, b, a0)                   # leaves the shift c on the diagonals
+        op.update_potential(veff2)
+        Y_upd = op.apply_H(Xd)
+        fresh = Operator.from_workload(wl2, precision=precision)
+        Y_new = fresh.apply_H(Xd)
+        assert torch.equal(Y_upd, Y_new)
+        assert_block_close(Y_upd.double().cpu().numpy(), orc.apply_H(oop2, Xr), tol, f"update_potential FP{precision}")
+        F1, F2 = Xd.clone(), Xd.clone()
+        op.chebyshev_filter(F1, 5, a, b + 1.0, a0)
+        fresh.chebyshev_filter(F2, 5, a, b + 1.0, a0)
+        assert torch.equal(F1, F2)
+        op.close(); fresh.close()
+
+
 def test_mass_diagonal_matches_the_oracle():
     torch, orc, Operator, *_ = _imports()
     wl, oop, *_ = oracle_case("p6_distorted_cells")
