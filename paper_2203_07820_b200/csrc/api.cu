@@ -67,7 +67,7 @@ WsLayout ws_layout(const Op* op, int64_t B) {
   w.pc_off = w.p_off + align_up((size_t)(op->n_proj + 1) * B * w.elt, 256);
   w.sync_off = w.pc_off + align_up((size_t)(op->n_pseg > 0 ? op->n_pseg : 1) * kProjGroup * B * sizeof(double), 256);
   // ticket counter (first 128 bytes) + one completion flag per (cell, 32-column tile): apply_kernels.cu, v2 kernel
-  w.sync_bytes = align_up(128 + (size_t)op->n_cells * (size_t)((B + 31) / 32) * sizeof(uint32_t), 256);
+  w.sync_bytes = align_up(128 + (size_t)op->n_cells * op->n_parts * (size_t)((B + 31) / 32) * sizeof(uint32_t), 256);
   w.total = w.sync_off + w.sync_bytes;
   return w;
 }
@@ -159,7 +159,12 @@ int chfsi_create(chfsi_op** out, const chfsi_mesh* mesh, const chfsi_potential* 
   op->mpad = (op->m_cell + 7) / 8 * 8;
   // leading dimension of the cell matrices = their shared-memory row pitch: the four k-rows of an mma A fragment
   // must fall into different bank groups.  FP64: LDA mod 16 in {4, 12}; FP32: LDA mod 32 in {8, 24}.
-  op->lda = precision == 64 ? op->mpad + 4 : op->mpad + (op->mpad % 16 == 0 ? 8 : 0);
+  {
+    const int n_mtiles = op->mpad / 8;
+    op->n_parts = (n_mtiles + kMaxPartMTiles - 1) / kMaxPartMTiles;
+    op->mw = 8 * ((n_mtiles + op->n_parts - 1) / op->n_parts);
+  }
+  op->lda = precision == 64 ? op->mw + 4 : op->mw + (op->mw % 16 == 0 ? 8 : 0);
   op->precision = precision; op->assembly = assembly;
   op->n_cells = mesh->n_cells; op->n_dofs = mesh->n_dofs; op->n_proj = has_nl ? nl->n_proj : 0;
 
@@ -168,7 +173,7 @@ int chfsi_create(chfsi_op** out, const chfsi_mesh* mesh, const chfsi_potential* 
   HostPlan plan;
   std::string msg;
   try {
-    msg = analyse_mesh(*mesh, has_nl ? nl : nullptr, tab, op->lda, &plan);
+    msg = analyse_mesh(*mesh, has_nl ? nl : nullptr, tab, op->lda, op->n_parts, &plan);
   } catch (const std::bad_alloc&) {
     delete op;
     return fail(nullptr, CHFSI_ERR_OUT_OF_MEMORY, "host allocation failed in mesh analysis");

@@ -32,6 +32,7 @@ struct ApplyDev {
   int n_launch_cells;
   int n_col_tiles;
   int m_cell, mpad, lda;               // mpad = round8(m_cell): projector rows of the contraction start there
+  int mw, n_parts;                     // output columns per matrix block / blocks per cell (common.h, Op::n_parts)
   const T* __restrict__ X; int64_t ldx;
   T* __restrict__ Tg; int64_t ldt;
   const T* __restrict__ P; int64_t ldp;
@@ -68,7 +69,7 @@ __global__ void __launch_bounds__(256) k_apply_generic(ApplyDev<T> a) {
     T acc[8];
 #pragma unroll
     for (int i = 0; i < 8; ++i) acc[i] = (T)0;
-    const T* Mr = M + rt * 8;
+    const T* Mr = M + mat_elem(0, rt * 8, a.mw, a.lda, kt);   // the 8 rows of an output tile sit in one block
     for (int k = 0; k < kt; ++k) {
       T x = Xs[k * 32 + lane];
 #pragma unroll
@@ -186,12 +187,14 @@ __global__ void __launch_bounds__(128) k_proj_reduce(const double* __restrict__ 
 template <typename T>
 __global__ void __launch_bounds__(128) k_extract_proj_rows(const T* __restrict__ mat, const int64_t* __restrict__ mat_off,
                                                            const int64_t* __restrict__ cell_proj_ptr,
-                                                           const int32_t* __restrict__ row_cell, int m_cell, int mpad, int lda,
-                                                           double* __restrict__ out) {
+                                                           const int32_t* __restrict__ row_cell,
+                                                           const int32_t* __restrict__ ktot, int m_cell, int mpad, int lda,
+                                                           int mw, double* __restrict__ out) {
   const int64_t r = blockIdx.x;
   const int c = row_cell[r];
-  const T* row = mat + mat_off[c] + (int64_t)(mpad + (r - cell_proj_ptr[c])) * lda;
-  for (int l = threadIdx.x; l < m_cell; l += 128) out[r * m_cell + l] = (double)row[l];
+  const int krow = mpad + (int)(r - cell_proj_ptr[c]);
+  const T* M = mat + mat_off[c];
+  for (int l = threadIdx.x; l < m_cell; l += 128) out[r * m_cell + l] = (double)M[mat_elem(krow, l, mw, lda, ktot[c])];
 }
 
 // Atomic assembly needs the recurrence term in place first:  T <- -beta T
@@ -211,23 +214,24 @@ __global__ void __launch_bounds__(256) k_prefill(T* __restrict__ Tg, int64_t ldt
 template <typename T>
 __global__ void __launch_bounds__(256) k_set_diag_shift(T* __restrict__ mat, const int64_t* __restrict__ mat_off,
                                                         const int64_t* __restrict__ idx_off, const int32_t* __restrict__ gidx,
-                                                        const double* __restrict__ diag0, int m_cell, int lda,
-                                                        int64_t n_cells, double shift) {
+                                                        const int32_t* __restrict__ ktot, const double* __restrict__ diag0,
+                                                        int m_cell, int lda, int mw, int64_t n_cells, double shift) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n_cells * m_cell) return;
   const int64_t c = i / m_cell;
   const int k = (int)(i - c * m_cell);
   const bool first = gidx[idx_off[c] + k] < 0;
-  mat[mat_off[c] + (int64_t)k * lda + k] = (T)(diag0[i] - (first ? shift : 0.0));
+  mat[mat_off[c] + mat_elem(k, k, mw, lda, ktot[c])] = (T)(diag0[i] - (first ? shift : 0.0));
 }
 template <typename T>
 __global__ void __launch_bounds__(256) k_capture_diag(const T* __restrict__ mat, const int64_t* __restrict__ mat_off,
-                                                      double* __restrict__ diag0, int m_cell, int lda, int64_t n_cells) {
+                                                      const int32_t* __restrict__ ktot, double* __restrict__ diag0,
+                                                      int m_cell, int lda, int mw, int64_t n_cells) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n_cells * m_cell) return;
   const int64_t c = i / m_cell;
   const int k = (int)(i - c * m_cell);
-  diag0[i] = (double)mat[mat_off[c] + (int64_t)k * lda + k];
+  diag0[i] = (double)mat[mat_off[c] + mat_elem(k, k, mw, lda, ktot[c])];
 }
 
 // -------------------------------------------------------------------------------------------------------------
@@ -495,8 +499,9 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<S> a, P
   const int mc = a.m_cell;
   const int nct = a.n_col_tiles;
   const int n_mtiles = (mc + 7) / 8;
+  const int mtp = a.mw / 8;            // 8-row output tiles per matrix block (= per tile of this kernel)
+  const int np = a.n_parts;
   const int mt0 = warp_m * MT;
-  const int nmt = max(0, min(MT, n_mtiles - mt0));
   const double alpha = a.alpha, beta = a.beta;
 
   if (tid == 0) {
@@ -517,13 +522,15 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<S> a, P
     if (tr) { for (int z = 6; z < 16; ++z) tr[z] = 0; }
     TRACE_STAMP(0);
 #endif
-    const int pos = (int)(ticket / nct), jt = (int)(ticket % nct);
+    const int pos = (int)(ticket / (np * nct)), part = (int)((ticket / nct) % np), jt = (int)(ticket % nct);
     const int cell = pd.pos_cell[pos];
+    const int row0 = part * a.mw;                                        // first output node of this tile
+    const int nmt = max(0, min(MT, min(mtp, n_mtiles - part * mtp) - mt0));
     const int col0 = jt * kP2TileN;
     const int ncols = min(kP2TileN, a.B - col0);             // multiple of 8
     const int kt = a.ktot[cell];
     const int32_t* gi = a.gidx + a.idx_off[cell];
-    const S* M = a.mat + a.mat_off[cell];
+    const S* M = a.mat + a.mat_off[cell] + (int64_t)part * kt * lda;
     if (tid == 0) ticket_s[(iter + 1) & 1] = (long long)(atomicAdd(pd.counter, 1ull) - pd.ticket_base);
     const bool use_t = (beta != 0.0) && !a.atomic;   // the -beta Y_{k-2} term seeds the accumulators (below)
     for (int k = tid; k < kt; k += kP2Threads) {
@@ -584,7 +591,7 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<S> a, P
       const double nb = -beta / alpha;
 #pragma unroll
       for (int i = 0; i < MT; ++i) {
-        const int r = (mt0 + i) * 8 + fm;
+        const int r = row0 + (mt0 + i) * 8 + fm;
         const int idx = (i < nmt && r < mc) ? idx_s[r] : 0;
         if (idx < 0) {
           const S* tp = a.Tg + (int64_t)(idx & 0x7fffffff) * a.ldt + col0 + nt0 * 8 + fk * 2;
@@ -658,9 +665,9 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<S> a, P
     constexpr bool skip_epi = false;
 #endif
     if (!a.atomic && !skip_epi) {
-      const int d1 = pd.dep_ptr[pos + 1];
-      for (int d = pd.dep_ptr[pos] + lane; d < d1; d += 32) {
-        const uint32_t* f = pd.flags + (int64_t)pd.dep_pos[d] * nct + jt;
+      const int d0 = pd.dep_ptr[pos], nd = (pd.dep_ptr[pos + 1] - d0) * np;   // every block of every earlier neighbour
+      for (int d = lane; d < nd; d += 32) {
+        const uint32_t* f = pd.flags + ((int64_t)pd.dep_pos[d0 + d / np] * np + d % np) * nct + jt;
         while (ld_acquire_gpu(f) != pd.epoch) __nanosleep(64);
       }
       __syncwarp();
@@ -671,7 +678,7 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<S> a, P
       // contributions: red.global.add.f64 (fire and forget); their order is fixed by the completion flags.
 #pragma unroll
       for (int i = 0; i < MT; ++i) {
-        const int r = (mt0 + i) * 8 + fm;
+        const int r = row0 + (mt0 + i) * 8 + fm;
         if (i >= nmt || r >= mc) continue;
         const int idx = idx_s[r];
         S* trow = a.Tg + (int64_t)(idx & 0x7fffffff) * a.ldt + col0 + nt0 * 8 + fk * 2;
@@ -693,7 +700,7 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<S> a, P
     __threadfence();
     __syncthreads();   // all stores of the tile are done and fenced; idx_s / ticket slot may be reused
     TRACE_STAMP(14);
-    if (tid == 0 && !a.atomic) st_release_gpu(pd.flags + (int64_t)pos * nct + jt, pd.epoch);
+    if (tid == 0 && !a.atomic) st_release_gpu(pd.flags + ((int64_t)pos * np + part) * nct + jt, pd.epoch);
   }
 }
 
@@ -762,8 +769,8 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
   if (g.cshift != op->cur_shift) {   // once per filter call: move the spectral shift onto the matrix diagonals
     const int64_t n = op->n_cells * op->m_cell;
     k_set_diag_shift<T><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(reinterpret_cast<T*>(op->mat), op->mat_off, op->idx_off,
-                                                                    op->gidx, op->diag0, op->m_cell, op->lda, op->n_cells,
-                                                                    g.cshift);
+                                                                    op->gidx, op->ktot, op->diag0, op->m_cell, op->lda, op->mw,
+                                                                    op->n_cells, g.cshift);
     op->cur_shift = g.cshift;
     op->launches++;
   }
@@ -783,7 +790,7 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
   }
   ApplyDev<T> a;
   a.mat = mat; a.mat_off = op->mat_off; a.idx_off = op->idx_off; a.ktot = op->ktot; a.gidx = op->gidx;
-  a.m_cell = op->m_cell; a.mpad = op->mpad; a.lda = op->lda;
+  a.m_cell = op->m_cell; a.mpad = op->mpad; a.lda = op->lda; a.mw = op->mw; a.n_parts = op->n_parts;
   a.X = X; a.ldx = g.ldx; a.Tg = Tg; a.ldt = g.ldt; a.P = P; a.ldp = B; a.B = B;
   a.alpha = (T)g.alpha; a.beta = (T)g.beta;
   a.atomic = op->assembly;
@@ -792,10 +799,9 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
   constexpr int kPer16 = 16 / (int)sizeof(T);
   const bool aligned = B % 8 == 0 && g.ldx % kPer16 == 0 && g.ldt % kPer16 == 0 && ((uintptr_t)g.X % 16 == 0) &&
                        ((uintptr_t)g.T % 16 == 0) && ((uintptr_t)g.P % 16 == 0) && op->max_ktot <= kMaxKtot;
-  const int n_mtiles = (op->m_cell + 7) / 8;
   // variant 0: persistent single-launch kernel (v2); variant 2: one launch per colour (v1); variant 1: generic
   bool fast2 = false, fast = false;
-  int MT = (n_mtiles + 3) / 4;
+  int MT = (op->mw / 8 + 3) / 4;   // 8-row tiles per warp row: 11 (p=6), 8 (p=7, 8), 7, 4, 2, 1
   // variant 0: persistent single-launch kernel, FP64 DMMA accumulation for both storage types;
   // variant 3 (FP32 storage only, opt-in): persistent kernel with 3xTF32 products on the 32-bit tensor pipe -- 1.3x
   // faster, but the FP32 tensor accumulator truncates: |dY|/|Y| ~ 2e-6 per apply, Ritz values off by up to 4e-5 Ha,
@@ -803,15 +809,15 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
   CUtensorMap tmX, tmP;
   bool fast3 = false;   // 3xTF32 kernel
   const int MT16 = ((op->m_cell + 15) / 16 + 1) / 2;
-  if (sizeof(T) == 4 && aligned && op->variant == 3 && g.sync != nullptr && g.epoch > 0)
+  if (sizeof(T) == 4 && aligned && op->variant == 3 && op->n_parts == 1 && g.sync != nullptr && g.epoch > 0)
     fast3 = (MT16 == 11 || MT16 == 7 || MT16 == 4 || MT16 == 2 || MT16 == 1) && t3_smem_bytes(op) <= 113 * 1024 &&
             make_row_gather_map(&tmX, g.X, op->n_dofs, B, g.ldx, 4, kT3TileN) &&
             make_row_gather_map(&tmP, g.P, op->n_proj + 1, B, B, 4, kT3TileN);
   if (aligned && !fast3 && op->variant == 0 && g.sync != nullptr && g.epoch > 0)
-    fast2 = (MT == 11 || MT == 7 || MT == 4 || MT == 2 || MT == 1) && p2_smem_bytes<T>(op) <= 113 * 1024 &&
+    fast2 = (MT == 11 || MT == 8 || MT == 7 || MT == 4 || MT == 2 || MT == 1) && p2_smem_bytes<T>(op) <= 113 * 1024 &&
             make_row_gather_map(&tmX, g.X, op->n_dofs, B, g.ldx, (int)sizeof(T), kP2TileN) &&
             make_row_gather_map(&tmP, g.P, op->n_proj + 1, B, B, (int)sizeof(T), kP2TileN);
-  if (sizeof(T) == 8 && aligned && !fast2 && op->variant != 1) fast = (MT == 11 || MT == 4 || MT == 2 || MT == 7);
+  if (sizeof(T) == 8 && aligned && !fast2 && op->variant != 1 && op->n_parts == 1) fast = (MT == 11 || MT == 4 || MT == 2 || MT == 7);
   size_t smem_fast = (size_t)kStages * (kPanelK * op->lda + kPanelK * kLdXs) * sizeof(double) + kStages * sizeof(uint64_t) +
                      (size_t)op->max_ktot * sizeof(int32_t);
   if (fast && smem_fast > 227 * 1024) fast = false;
@@ -861,7 +867,7 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
       pd.counter = g.sync;
       pd.flags = reinterpret_cast<uint32_t*>(g.sync) + kSyncFlagOffset;
       pd.epoch = g.epoch;
-      const int64_t n_tiles = op->n_cells * a.n_col_tiles;
+      const int64_t n_tiles = op->n_cells * op->n_parts * a.n_col_tiles;
       unsigned grid = (unsigned)std::min<int64_t>(n_tiles, 2 * (int64_t)op->n_sm);
 #ifdef CHFSI_TRACE
       if (const char* eg = getenv("CHFSI_DEBUG_GRID")) grid = (unsigned)std::min<int64_t>(n_tiles, atoi(eg));
@@ -875,6 +881,7 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
       const size_t sm = p2_smem_bytes<T>(op);
       switch (MT) {
         case 11: k_apply_dmma_p<11, T><<<grid, kP2Threads, sm, st>>>(a, pd, tmX, tmP); break;
+        case 8: k_apply_dmma_p<8, T><<<grid, kP2Threads, sm, st>>>(a, pd, tmX, tmP); break;
         case 7: k_apply_dmma_p<7, T><<<grid, kP2Threads, sm, st>>>(a, pd, tmX, tmP); break;
         case 4: k_apply_dmma_p<4, T><<<grid, kP2Threads, sm, st>>>(a, pd, tmX, tmP); break;
         case 2: k_apply_dmma_p<2, T><<<grid, kP2Threads, sm, st>>>(a, pd, tmX, tmP); break;
@@ -930,6 +937,7 @@ cudaError_t init_apply_kernels(Op* op) {
     const size_t smem_p2 = p2_smem_bytes<double>(op);
     if (smem_p2 <= 113 * 1024) {
       if ((e = cudaFuncSetAttribute(k_apply_dmma_p<11, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p2))) return e;
+      if ((e = cudaFuncSetAttribute(k_apply_dmma_p<8, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p2))) return e;
       if ((e = cudaFuncSetAttribute(k_apply_dmma_p<7, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p2))) return e;
       if ((e = cudaFuncSetAttribute(k_apply_dmma_p<4, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p2))) return e;
       if ((e = cudaFuncSetAttribute(k_apply_dmma_p<2, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p2))) return e;
@@ -939,6 +947,7 @@ cudaError_t init_apply_kernels(Op* op) {
     const size_t smem_p2 = p2_smem_bytes<float>(op);
     if (smem_p2 <= 113 * 1024) {
       if ((e = cudaFuncSetAttribute(k_apply_dmma_p<11, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p2))) return e;
+      if ((e = cudaFuncSetAttribute(k_apply_dmma_p<8, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p2))) return e;
       if ((e = cudaFuncSetAttribute(k_apply_dmma_p<7, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p2))) return e;
       if ((e = cudaFuncSetAttribute(k_apply_dmma_p<4, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p2))) return e;
       if ((e = cudaFuncSetAttribute(k_apply_dmma_p<2, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p2))) return e;
@@ -982,10 +991,10 @@ cudaError_t assemble_projector_rows(Op* op, const HostPlan& plan, const chfsi_me
   if (e == cudaSuccess) {
     if (op->precision == 64)
       k_extract_proj_rows<double><<<(unsigned)op->nnz_cp, 128, 0, st>>>(reinterpret_cast<const double*>(op->mat), op->mat_off,
-                                                                       op->cell_proj_ptr, d_row_cell, mc, op->mpad, op->lda, d_rows);
+                                                                       op->cell_proj_ptr, d_row_cell, op->ktot, mc, op->mpad, op->lda, op->mw, d_rows);
     else
       k_extract_proj_rows<float><<<(unsigned)op->nnz_cp, 128, 0, st>>>(reinterpret_cast<const float*>(op->mat), op->mat_off,
-                                                                      op->cell_proj_ptr, d_row_cell, mc, op->mpad, op->lda, d_rows);
+                                                                      op->cell_proj_ptr, d_row_cell, op->ktot, mc, op->mpad, op->lda, op->mw, d_rows);
     e = cudaGetLastError();
   }
   if (e == cudaSuccess) e = cudaMemcpyAsync(rows.data(), d_rows, rows.size() * sizeof(double), cudaMemcpyDeviceToHost, st);
@@ -1026,11 +1035,11 @@ cudaError_t capture_diagonal(Op* op, cudaStream_t st) {
   const int64_t n = op->n_cells * op->m_cell;
   const unsigned grid = (unsigned)((n + 255) / 256);
   if (op->precision == 64)
-    k_capture_diag<double><<<grid, 256, 0, st>>>(reinterpret_cast<const double*>(op->mat), op->mat_off, op->diag0, op->m_cell,
-                                                 op->lda, op->n_cells);
+    k_capture_diag<double><<<grid, 256, 0, st>>>(reinterpret_cast<const double*>(op->mat), op->mat_off, op->ktot, op->diag0,
+                                                 op->m_cell, op->lda, op->mw, op->n_cells);
   else
-    k_capture_diag<float><<<grid, 256, 0, st>>>(reinterpret_cast<const float*>(op->mat), op->mat_off, op->diag0, op->m_cell,
-                                                op->lda, op->n_cells);
+    k_capture_diag<float><<<grid, 256, 0, st>>>(reinterpret_cast<const float*>(op->mat), op->mat_off, op->ktot, op->diag0,
+                                                op->m_cell, op->lda, op->mw, op->n_cells);
   op->cur_shift = 0.0;
   return cudaGetLastError();
 }

@@ -1,7 +1,8 @@
 // Internal declarations shared by the translation units of libchfsi (not part of the ABI).
 //
 // Device data layout:
-//   mat   [cell c]  : K_c rows x LDA columns, element type T (double | float), row k = CONTRACTION index,
+//   mat   [cell c]  : [n_parts] blocks of K_c rows x LDA columns (block = mw consecutive output nodes; one block up to
+//                     p = 6); per block: K_c rows x LDA columns, element type T (double | float), row k = CONTRACTION index,
 //                     column m = OUTPUT node.  Rows 0..M_cell-1 hold the Loewdin-scaled cell Hamiltonian
 //                     s_k H^e_km s_m (symmetric, "H~^{loc,c_i}"); rows M_cell..M_cell+N_psp^c-1
 //                     hold s_m C^c_{m,j} for the projectors j touching the cell; remaining
@@ -26,6 +27,11 @@
 namespace chfsi {
 
 constexpr uint32_t kFirstBit = 0x80000000u;
+constexpr int kMaxPartMTiles = 44;       // 8-row output tiles per part (4 warp rows x 11)
+// element offset of (contraction row k, output column m) inside the matrix of a cell with K_c = kc rows
+__host__ __device__ inline int64_t mat_elem(int k, int m, int mw, int lda, int kc) {
+  return (int64_t)(m / mw) * kc * lda + (int64_t)k * lda + (m % mw);
+}
 constexpr int kProjGroup = 8;            // projectors per group (slots of a coefficient row)
 constexpr int kProjSegRows = 128;        // dof rows per CTA of the projector-coefficient kernel
 
@@ -73,12 +79,16 @@ struct HostPlan {
   std::vector<double> mass;              // [n_dofs] diagonal GLL mass
 };
 // Returns "" on success, else an error message (bad mesh).
-std::string analyse_mesh(const chfsi_mesh& mesh, const chfsi_nonlocal* nl, const Tables1D& tab, int lda,
+std::string analyse_mesh(const chfsi_mesh& mesh, const chfsi_nonlocal* nl, const Tables1D& tab, int lda, int n_parts,
                          HostPlan* plan);
 
 // ---- device operator ----------------------------------------------------------------------------------------
 struct Op {
   int p = 0, n1 = 0, nq1 = 0, m_cell = 0, n_q = 0, mpad = 0, lda = 0;
+  // output columns of a cell matrix are stored in n_parts blocks of mw columns: mat[c] = [part][K_c][lda]
+  // (one block, mw = mpad, up to p = 6; two blocks of 256 at p = 7, three of 248 at p = 8): a tile of the persistent
+  // kernel is (cell, part, column tile), so the accumulators of 8 warps always fit the register file.
+  int n_parts = 1, mw = 0;
   int precision = 64, assembly = 0, variant = 0;
   int64_t n_cells = 0, n_dofs = 0, n_proj = 0, nnz_cp = 0, n_pc_cells = 0;
   int n_colors = 0;

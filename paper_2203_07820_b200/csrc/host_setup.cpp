@@ -120,7 +120,7 @@ double trilinear_detJ(const double* verts, double x, double y, double z) {
 }
 }  // namespace
 
-std::string analyse_mesh(const chfsi_mesh& mesh, const chfsi_nonlocal* nl, const Tables1D& tab, int lda,
+std::string analyse_mesh(const chfsi_mesh& mesh, const chfsi_nonlocal* nl, const Tables1D& tab, int lda, int n_parts,
                          HostPlan* plan) {
   const int n1 = tab.n1, mc = n1 * n1 * n1;
   const int64_t nc = mesh.n_cells, nd = mesh.n_dofs;
@@ -314,7 +314,7 @@ std::string analyse_mesh(const chfsi_mesh& mesh, const chfsi_nonlocal* nl, const
     int64_t np = plan->cell_proj_ptr[c + 1] - plan->cell_proj_ptr[c];
     int kt = (int)(mpad + (np + 7) / 8 * 8);
     plan->ktot[c] = kt;
-    plan->mat_off[c + 1] = plan->mat_off[c] + (int64_t)kt * lda;
+    plan->mat_off[c + 1] = plan->mat_off[c] + (int64_t)n_parts * kt * lda;
     plan->idx_off[c + 1] = plan->idx_off[c] + kt;
   }
   plan->gidx.assign(plan->idx_off[nc], (int32_t)n_proj);

@@ -74,9 +74,9 @@ __global__ void __launch_bounds__(256) k_cell_matrix(int n1, int nq1, int64_t n_
                                                      const double* __restrict__ verts, const double* __restrict__ veff,
                                                      const int32_t* __restrict__ gidx, const int64_t* __restrict__ idx_off,
                                                      const int64_t* __restrict__ mat_off, const int32_t* __restrict__ ktot,
-                                                     const double* __restrict__ mass, int lda, T* __restrict__ mat,
-                                                     double* __restrict__ scratch64, int* __restrict__ bad_flag,
-                                                     int zero_tail) {
+                                                     const double* __restrict__ mass, int lda, int mw, int n_parts,
+                                                     T* __restrict__ mat, double* __restrict__ scratch64,
+                                                     int* __restrict__ bad_flag, int zero_tail) {
   extern __shared__ double smem[];
   const int nn = n1 * n1, nq2 = nq1 * nq1, nq = nq1 * nq2, mc = n1 * nn;
   double* Wf = smem;                    // [10][nq]
@@ -140,18 +140,22 @@ __global__ void __launch_bounds__(256) k_cell_matrix(int n1, int nq1, int64_t n_
     // Loewdin scaling (Eq. 34), conversion to T, zero padding of the Hamiltonian rows
     const int32_t* gi = gidx + idx_off[c];
     T* M = mat + mat_off[c];
-    for (int o = threadIdx.x; o < mc * lda; o += blockDim.x) {
-      int k = o / lda, m = o % lda;
-      double v = 0.0;
-      if (m < mc) {
-        double sk = 1.0 / sqrt(mass[gi[k] & 0x7fffffff]), sm = 1.0 / sqrt(mass[gi[m] & 0x7fffffff]);
-        v = H64[(size_t)k * mc + m] * sk * sm;
+    const int kc = ktot[c];
+    for (int part = 0; part < n_parts; ++part) {
+      T* Mp = M + (int64_t)part * kc * lda;
+      for (int o = threadIdx.x; o < mc * lda; o += blockDim.x) {
+        int k = o / lda, ml = o % lda, m = part * mw + ml;
+        double v = 0.0;
+        if (ml < mw && m < mc) {
+          double sk = 1.0 / sqrt(mass[gi[k] & 0x7fffffff]), sm = 1.0 / sqrt(mass[gi[m] & 0x7fffffff]);
+          v = H64[(size_t)k * mc + m] * sk * sm;
+        }
+        Mp[o] = (T)v;
       }
-      M[o] = (T)v;
+      // padding rows beyond the projector rows (and the projector rows themselves, filled later) start at zero
+      if (zero_tail)
+        for (int o = mc * lda + threadIdx.x; o < kc * lda; o += blockDim.x) Mp[o] = (T)0;
     }
-    // padding rows beyond the projector rows (and the projector rows themselves, filled later) start at zero
-    if (zero_tail)
-      for (int o = mc * lda + threadIdx.x; o < ktot[c] * lda; o += blockDim.x) M[o] = (T)0;
   }
 }
 
@@ -163,7 +167,8 @@ __global__ void __launch_bounds__(256) k_cell_projector(int n1, int nq1, SetupTa
                                                         const int64_t* __restrict__ cell_proj_ptr,
                                                         const int32_t* __restrict__ gidx, const int64_t* __restrict__ idx_off,
                                                         const int64_t* __restrict__ mat_off, const double* __restrict__ mass,
-                                                        int lda, T* __restrict__ mat) {
+                                                        const int32_t* __restrict__ ktot, int lda, int mw, int n_parts,
+                                                        T* __restrict__ mat) {
   extern __shared__ double smem[];
   const int nn = n1 * n1, nq2 = nq1 * nq1, nq = nq1 * nq2, mc = n1 * nn;
   double* W = smem;              // [nq]
@@ -198,15 +203,17 @@ __global__ void __launch_bounds__(256) k_cell_projector(int n1, int nq1, SetupTa
   }
   __syncthreads();
   const int32_t* gi = gidx + idx_off[c];
-  T* row = mat + mat_off[c] + (int64_t)((mc + 7) / 8 * 8 + (r - cell_proj_ptr[c])) * lda;
-  for (int m = threadIdx.x; m < lda; m += blockDim.x) {
+  const int krow = (mc + 7) / 8 * 8 + (int)(r - cell_proj_ptr[c]);
+  const int kc = ktot[c];
+  for (int o = threadIdx.x; o < n_parts * lda; o += blockDim.x) {
+    const int part = o / lda, ml = o % lda, m = part * mw + ml;
     double v = 0.0;
-    if (m < mc) {
+    if (ml < mw && m < mc) {
       int ab = m % nn, cz = m / nn;
       for (int qc = 0; qc < nq1; ++qc) v += Bt[ab * nq1 + qc] * ph[qc * n1 + cz];
       v *= 1.0 / sqrt(mass[gi[m] & 0x7fffffff]);
     }
-    row[m] = (T)v;
+    mat[mat_off[c] + ((int64_t)part * kc + krow) * lda + ml] = (T)v;
   }
 }
 
@@ -243,13 +250,13 @@ cudaError_t launch_local_matrices(Op* op, const double* veff_host, cudaStream_t 
     if (op->precision == 64) {
       CK(cudaFuncSetAttribute(k_cell_matrix<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
       k_cell_matrix<double><<<grid, 256, smem, stream>>>(n1, nq1, nc, tb, op->setup_verts, d_veff, op->gidx, op->idx_off,
-                                                         op->mat_off, op->ktot, op->mass, op->lda, (double*)op->mat,
-                                                         d_scratch, d_bad, zero_tail);
+                                                         op->mat_off, op->ktot, op->mass, op->lda, op->mw, op->n_parts,
+                                                         (double*)op->mat, d_scratch, d_bad, zero_tail);
     } else {
       CK(cudaFuncSetAttribute(k_cell_matrix<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
       k_cell_matrix<float><<<grid, 256, smem, stream>>>(n1, nq1, nc, tb, op->setup_verts, d_veff, op->gidx, op->idx_off,
-                                                        op->mat_off, op->ktot, op->mass, op->lda, (float*)op->mat,
-                                                        d_scratch, d_bad, zero_tail);
+                                                        op->mat_off, op->ktot, op->mass, op->lda, op->mw, op->n_parts,
+                                                        (float*)op->mat, d_scratch, d_bad, zero_tail);
     }
     CK(cudaGetLastError());
     CK(cudaMemcpyAsync(&h_bad, d_bad, sizeof(int), cudaMemcpyDeviceToHost, stream));
@@ -302,11 +309,11 @@ cudaError_t build_cell_matrices(Op* op, const HostPlan& plan, const Tables1D& ta
     if (op->precision == 64)
       k_cell_projector<double><<<(unsigned)op->nnz_cp, 256, smem2, stream>>>(
           n1, nq1, tb, op->setup_verts, d_chi, d_row_src, d_row_cell, op->cell_proj_ptr, op->gidx, op->idx_off, op->mat_off,
-          op->mass, op->lda, (double*)op->mat);
+          op->mass, op->ktot, op->lda, op->mw, op->n_parts, (double*)op->mat);
     else
       k_cell_projector<float><<<(unsigned)op->nnz_cp, 256, smem2, stream>>>(
           n1, nq1, tb, op->setup_verts, d_chi, d_row_src, d_row_cell, op->cell_proj_ptr, op->gidx, op->idx_off, op->mat_off,
-          op->mass, op->lda, (float*)op->mat);
+          op->mass, op->ktot, op->lda, op->mw, op->n_parts, (float*)op->mat);
     CK(cudaGetLastError());
     CK(cudaStreamSynchronize(stream));
   }

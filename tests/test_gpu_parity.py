@@ -46,6 +46,9 @@ CASES = {
                       seed_base=79), 13, 5, 64),
     "p2_nonperiodic": (dict(n=3, p=2, L=6.0, periodic=False, atoms_per_side=1, n_gaussians=0, nonlocal_=True,
                             smooth_field=0.05, seed_base=80, r_cut=2.5), 8, 4, 64),
+    # p = 7 (M_cell = 512): the output nodes of a cell are split over two tiles of the persistent kernel
+    "p7_two_blocks": (dict(n=2, p=7, L=4.0, atoms_per_side=1, n_gaussians=0, nonlocal_=True, smooth_field=0.05,
+                           seed_base=83, r_cut=1.9), 40, 5, 64),
     "p6_fp32": (dict(n=3, p=6, L=6.0, atoms_per_side=1, n_gaussians=0, nonlocal_=True, smooth_field=0.05,
                      seed_base=77), 64, 7, 32),
     "p4_fp32_odd_B": (dict(n=3, p=4, L=6.0, atoms_per_side=1, n_gaussians=0, nonlocal_=True, smooth_field=0.05,
