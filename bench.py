@@ -40,7 +40,8 @@ def parse_args():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=DEFAULT_CONFIG, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--config", type=int, default=DEFAULT_CONFIG, choices=[1, 2, 3, 4, 5, 6],
+                    help="BASELINE.json config 1..5; 6 = extra p=7 workload (config 2's box at FE degree 7)")
     ap.add_argument("--assembly", type=int, default=0, choices=[0, 1],
                     help="0 deterministic coloured assembly, 1 atomic assembly")
     ap.add_argument("--variant", type=int, default=0, choices=[0, 1, 2, 3],

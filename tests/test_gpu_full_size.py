@@ -94,14 +94,25 @@ def config3_oracle():
     return wl, orc.operator_from_workload(wl)
 
 
-SAMPLE_COLS = {3: [0, 131, 255], 4: [0, 300, 511], 5: [0, 399]}
+SAMPLE_COLS = {3: [0, 131, 255], 4: [0, 300, 511], 5: [0, 399], 6: [0, 131, 255]}
 
 
 @pytest.mark.parametrize("config", [3, 4])
 def test_config3_and_4_one_chunk_sampled_columns(config, config3_oracle):
+    _check_one_chunk_sampled_columns(config, *config3_oracle)
+
+
+def test_p7_workload_one_chunk_sampled_columns():
+    """Extra workload 6 (not in BASELINE.json): config 2's box at FE degree 7, where the persistent kernel processes
+    the 512 output nodes of a cell as two tiles of 256."""
+    torch, orc, Operator, CONFIGS, SEED_X, load_bounds, make_workload, random_block = _imports()
+    wl = make_workload(6)
+    _check_one_chunk_sampled_columns(6, wl, orc.operator_from_workload(wl))
+
+
+def _check_one_chunk_sampled_columns(config, wl, oop):
     torch, orc, Operator, CONFIGS, SEED_X, load_bounds, make_workload, random_block = _imports()
     spec = CONFIGS[config]
-    wl, oop = config3_oracle
     a0, a, b = load_bounds(spec.bounds_key, "B")
     tol, tol_ritz = (1e-10, 1e-8) if spec.precision == 64 else (1e-4, 1e-5)
     op = Operator.from_workload(wl, precision=spec.precision)

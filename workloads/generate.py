@@ -56,6 +56,9 @@ CONFIGS = {
     # config 4 = config 3's mesh and potential (same seeds), FP32 storage
     4: ConfigSpec(4, 16, 6, 32.0, 4, 0, True, 0.05, 4096, 512, 30, 32, 3000, "3"),
     5: ConfigSpec(5, 20, 6, 40.0, 6, 0, True, 0.0, 4000, 400, 40, 64, 5000, "5"),
+    # extra, NOT in BASELINE.json: config 2's box, atoms and block at FE degree 7 (the paper's other benchmark order,
+    # PAPER.md:586, 601-603; M_cell = 512, 175,616 dofs) -- the p = 7 tiling of the persistent kernel
+    6: ConfigSpec(6, 8, 7, 16.0, 2, 0, True, 0.0, 256, 256, 20, 64, 6000, "6"),
 }
 
 # seed offsets k: 0 V_eff centres/depths, 1 atom jitter, 2 D, 3 smooth field, 4 X,
