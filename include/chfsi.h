@@ -140,6 +140,20 @@ int chfsi_chebyshev_filter_chunked(chfsi_op* op, void* X_dev, int64_t ldx, int64
 int chfsi_chebyshev_filter_host(chfsi_op* op, void* X_host, int64_t ldx, int64_t N, int64_t B, int32_t m,
                                 double a, double b, double a0);
 
+/* Rayleigh-Ritz projection matrices of a (filtered) block Psi_f = Y [n_dofs][ldy], N columns -- Algorithm 2 step 1
+ * (RRGEP-OP; the blocked X^T Y products of PAPER.md:556-558), FP64 operators only:
+ *   chfsi_overlap_matrix:        S  = Y^T Y                     (step 1a, RRGEP-O)
+ *   chfsi_projected_hamiltonian: H^ = Y^T (H~ Y)                (step 1b, RRGEP-P; H~ Y is formed chunk by chunk, B
+ *                                                                columns at a time, in the workspace block)
+ * S_dev / H_dev are DEVICE arrays [N][N], row-major, FP64, owned by the caller.  N, ldy and B must be even and the
+ * pointers 16-byte aligned (CHFSI_ERR_UNSUPPORTED otherwise).  workspace_dev: chfsi_workspace_bytes(op, min(B, N)).
+ * Work is enqueued on cuda_stream; the row-split partial sums live in a library-owned scratch buffer that grows on
+ * demand (the call then synchronises the stream once).  Both matrices are computed in full (symmetric up to rounding:
+ * H^ is not symmetrised).  The Cholesky / eigen-decomposition of step 2 is left to the caller (N x N, dense). */
+int chfsi_overlap_matrix(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N, double* S_dev, void* cuda_stream);
+int chfsi_projected_hamiltonian(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N, int64_t B, double* H_dev,
+                                void* workspace_dev, void* cuda_stream);
+
 /* Number of kernel launches enqueued by this handle since creation (for benchmark bookkeeping). */
 int64_t chfsi_launch_count(const chfsi_op* op);
 

@@ -364,6 +364,13 @@ def rayleigh_ritz(op: Operator, Y, HY=None, rel_cut: float = 1e-12):
     return np.linalg.eigvalsh(Qk.T @ Hh @ Qk)
 
 
+def projection_matrices(op: Operator, Y):
+    """Algorithm 2 step 1 (RRGEP-OP) written out: the overlap matrix S = Y^T Y (step 1a) and the
+    projected Hamiltonian H^ = Y^T (H~ Y) (step 1b) of a block Y [n_dofs, N]; no normalisation, no symmetrisation."""
+    Y = np.asarray(Y, dtype=np.float64)
+    return Y.T @ Y, Y.T @ apply_H(op, Y)
+
+
 def ritz_values_of_block(Y, HY, rel_cut: float = 1e-12):
     """Same as rayleigh_ritz but for a given pair (Y, H~Y) (used to compare GPU and oracle blocks with the
     SAME H~Y provider).  Columns are normalised with the norms of Y."""

@@ -20,7 +20,7 @@ LIB_PATH = os.path.join(HERE, "libchfsi.so")
 
 EXPORTED_SYMBOLS = [
     "chfsi_create", "chfsi_destroy", "chfsi_update_potential", "chfsi_get_info", "chfsi_workspace_bytes", "chfsi_mass_diag",
-    "chfsi_apply_H", "chfsi_chebyshev_filter", "chfsi_chebyshev_filter_chunked", "chfsi_chebyshev_filter_host",
+    "chfsi_apply_H", "chfsi_overlap_matrix", "chfsi_projected_hamiltonian", "chfsi_chebyshev_filter", "chfsi_chebyshev_filter_chunked", "chfsi_chebyshev_filter_host",
     "chfsi_launch_count", "chfsi_set_kernel_variant", "chfsi_set_profiling", "chfsi_get_profile",
     "chfsi_measure_fp64_peak", "chfsi_last_error",
 ]
@@ -90,6 +90,10 @@ def load_library(build_if_missing: bool = True):
     lib_.chfsi_mass_diag.restype = C.c_int
     lib_.chfsi_apply_H.argtypes = [vp, vp, i64, vp, i64, i64, vp, vp]
     lib_.chfsi_apply_H.restype = C.c_int
+    lib_.chfsi_overlap_matrix.argtypes = [vp, vp, i64, i64, vp, vp]
+    lib_.chfsi_overlap_matrix.restype = C.c_int
+    lib_.chfsi_projected_hamiltonian.argtypes = [vp, vp, i64, i64, i64, vp, vp, vp]
+    lib_.chfsi_projected_hamiltonian.restype = C.c_int
     lib_.chfsi_chebyshev_filter.argtypes = [vp, vp, i64, i64, i32, dbl, dbl, dbl, vp, vp]
     lib_.chfsi_chebyshev_filter.restype = C.c_int
     lib_.chfsi_chebyshev_filter_chunked.argtypes = [vp, vp, i64, i64, i64, i32, dbl, dbl, dbl, vp, vp]
@@ -231,6 +235,26 @@ class Operator:
         self._check(load_library().chfsi_apply_H(self._h, xp, ldx, yp, ldy, B, C.c_void_p(ws.data_ptr()),
                                                  _stream_ptr(stream)))
         return Y
+
+    def overlap_matrix(self, Y, stream=None):
+        """S = Y^T Y (Algorithm 2 step 1a); returns a [N, N] FP64 device tensor."""
+        import torch
+        yp, ldy, N = self._block(Y, "Y")
+        S = torch.empty((N, N), dtype=torch.float64, device="cuda")
+        self._check(load_library().chfsi_overlap_matrix(self._h, yp, ldy, N, C.c_void_p(S.data_ptr()),
+                                                        _stream_ptr(stream)))
+        return S
+
+    def projected_hamiltonian(self, Y, B=None, workspace=None, stream=None):
+        """H^ = Y^T (H~ Y) (Algorithm 2 step 1b), H~ Y formed B columns at a time; returns [N, N] FP64."""
+        import torch
+        yp, ldy, N = self._block(Y, "Y")
+        B = int(B) if B is not None else min(N, 256)
+        ws = workspace if workspace is not None else self.workspace(min(B, N))
+        Hh = torch.empty((N, N), dtype=torch.float64, device="cuda")
+        self._check(load_library().chfsi_projected_hamiltonian(self._h, yp, ldy, N, B, C.c_void_p(Hh.data_ptr()),
+                                                               C.c_void_p(ws.data_ptr()), _stream_ptr(stream)))
+        return Hh
 
     def chebyshev_filter(self, X, m, a, b, a0, workspace=None, stream=None):
         """In place on the columns of X."""

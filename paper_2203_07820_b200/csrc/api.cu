@@ -49,6 +49,7 @@ void free_op(chfsi_op* op) {
   cudaFree(op->color_cells); cudaFree(op->dep_ptr); cudaFree(op->dep_pos); cudaFree(op->all_cells); cudaFree(op->pc_cells); cudaFree(op->cell_proj_ptr);
   cudaFree(op->proj_ptr); cudaFree(op->proj_pcrow); cudaFree(op->seg_ptr); cudaFree(op->grow_dof); cudaFree(op->pcoef);
   cudaFree(op->grp_seg_ptr); cudaFree(op->proj_grp); cudaFree(op->proj_slot);
+  cudaFree(op->rr_scratch);
   cudaFree(op->setup_verts); cudaFree(op->setup_pp); cudaFree(op->setup_phi); cudaFree(op->setup_gx); cudaFree(op->setup_gw); cudaFree(op->D); cudaFree(op->mass); cudaFree(op->diag0);
   for (cudaEvent_t e : op->prof_events) cudaEventDestroy(e);
   delete op;
@@ -387,6 +388,54 @@ int chfsi_chebyshev_filter_host(chfsi_op* op, void* X_host, int64_t ldx, int64_t
   }
   cudaFree(ws);
   return rc;
+}
+
+namespace {
+int check_rr_args(chfsi_op* op, const void* Y, int64_t ldy, int64_t N, const void* out) {
+  if (!op) return CHFSI_ERR_BAD_ARGUMENT;
+  if (!Y || !out) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "NULL block / output matrix");
+  if (N < 1 || ldy < N || N > (1 << 20)) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "need 1 <= N <= ld");
+  if (op->precision != 64) return fail(op, CHFSI_ERR_UNSUPPORTED, "Rayleigh-Ritz projection: FP64 operators only");
+  if (N % 2 != 0 || ldy % 2 != 0 || (uintptr_t)Y % 16 != 0 || (uintptr_t)out % 16 != 0)
+    return fail(op, CHFSI_ERR_UNSUPPORTED, "Rayleigh-Ritz projection: N and ld must be even, pointers 16-byte aligned");
+  return CHFSI_OK;
+}
+}  // namespace
+
+int chfsi_overlap_matrix(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N, double* S_dev, void* cuda_stream) {
+  int rc = check_rr_args(op, Y_dev, ldy, N, S_dev);
+  if (rc) return rc;
+  const double* Y = reinterpret_cast<const double*>(Y_dev);
+  cudaError_t ce = launch_xty(op, Y, ldy, Y, ldy, op->n_dofs, (int)N, (int)N, S_dev, N, reinterpret_cast<cudaStream_t>(cuda_stream));
+  return ce == cudaSuccess ? CHFSI_OK : cuda_fail(op, ce, "overlap_matrix");
+}
+
+int chfsi_projected_hamiltonian(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N, int64_t B, double* H_dev,
+                                void* workspace_dev, void* cuda_stream) {
+  int rc = check_rr_args(op, Y_dev, ldy, N, H_dev);
+  if (rc) return rc;
+  if (B < 2 || B % 2 != 0) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "chunk width B must be even and >= 2");
+  if (!workspace_dev || (uintptr_t)workspace_dev % 16 != 0) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "bad workspace");
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  const double* Y = reinterpret_cast<const double*>(Y_dev);
+  const int64_t Bc = std::min(B, N);
+  const WsLayout w = ws_layout(op, Bc);
+  char* base = reinterpret_cast<char*>(workspace_dev);
+  double* W = reinterpret_cast<double*>(base + w.block_off);
+  for (int64_t j0 = 0; j0 < N; j0 += Bc) {
+    const int64_t bw = std::min(Bc, N - j0);
+    ApplyArgs g;                                        // W <- H~ Y[:, j0 : j0 + bw]
+    g.X = Y + j0; g.ldx = ldy; g.T = W; g.ldt = w.ldw; g.B = bw;
+    g.alpha = 1.0; g.beta = 0.0; g.cshift = 0.0;
+    g.P = base + w.p_off; g.Pc = base + w.pc_off;
+    g.sync = reinterpret_cast<unsigned long long*>(base + w.sync_off); g.epoch = 1;
+    cudaError_t ce = cudaMemsetAsync(g.sync, 0, w.sync_bytes, st);
+    if (ce == cudaSuccess) { op->launches++; ce = launch_apply(op, g, st); }
+    // H^[:, j0 : j0 + bw] = Y^T W
+    if (ce == cudaSuccess) ce = launch_xty(op, Y, ldy, W, w.ldw, op->n_dofs, (int)N, (int)bw, H_dev + j0, N, st);
+    if (ce != cudaSuccess) return cuda_fail(op, ce, "projected_hamiltonian");
+  }
+  return CHFSI_OK;
 }
 
 int64_t chfsi_launch_count(const chfsi_op* op) { return op ? op->launches : -1; }

@@ -132,6 +132,9 @@ struct Op {
   double* setup_phi = nullptr;           // [nq1][n1]
   double* setup_gx = nullptr;            // [nq1]
   double* setup_gw = nullptr;            // [nq1]
+  // split-row partial tiles of the Rayleigh-Ritz projection products (rr_kernels.cu); grown on demand
+  void* rr_scratch = nullptr;
+  size_t rr_scratch_bytes = 0;
   int64_t launches = 0;
   // optional per-kernel timing (chfsi_set_profiling): event triples (start, after projector kernels, end)
   bool profiling = false;
@@ -172,6 +175,10 @@ cudaError_t launch_apply(Op* op, const ApplyArgs& a, cudaStream_t stream);
 cudaError_t assemble_projector_rows(Op* op, const HostPlan& plan, const chfsi_mesh& mesh, cudaStream_t stream);
 // Copies the diagonal of every cell matrix into op->diag0 (once, at create, after build_cell_matrices).
 cudaError_t capture_diagonal(Op* op, cudaStream_t stream);
+// C[N1][ldc] = A^T B over n_rows rows of two FP64 blocks [n_rows][ld] (Alg. 2 step 1); enqueued on
+// the stream; may grow op->rr_scratch (then it synchronises the stream once).
+cudaError_t launch_xty(Op* op, const double* A, int64_t lda, const double* B, int64_t ldb, int64_t n_rows, int N1, int N2,
+                       double* C, int64_t ldc, cudaStream_t stream);
 // Opts the kernels into the shared memory they need for this operator (once, at create).
 cudaError_t init_apply_kernels(Op* op);
 

@@ -166,6 +166,38 @@ def test_update_potential_equals_a_fresh_operator_and_the_oracle():
         op.close(); fresh.close()
 
 
+@pytest.mark.parametrize("name", ["p6_nonlocal_ragged", "config1"])
+def test_rayleigh_ritz_projection_matrices_match_the_oracle(name):
+    """chfsi_overlap_matrix / chfsi_projected_hamiltonian (Algorithm 2 step 1) on the filtered block:
+    element-wise against the oracle's S = Y^T Y and H^ = Y^T (H~ Y), chunked (B < N, ragged last chunk) and
+    unchunked, bit-reproducible, and the generalised eigenvalues of (H^, S) within 1e-8 Ha of the oracle's."""
+    import scipy.linalg
+    torch, orc, Operator, _, _, _, _ = _imports()
+    wl, oop, X, (a0, a, b), Yo, Fo = oracle_case(name)
+    Y = Fo / np.linalg.norm(Fo, axis=0, keepdims=True)          # the filtered block, column-normalised
+    So, Ho = orc.projection_matrices(oop, Y)
+    op = Operator.from_workload(wl)
+    Yd = torch.tensor(Y, device="cuda")
+    N = Y.shape[1]
+    S = op.overlap_matrix(Yd)
+    assert torch.equal(S, op.overlap_matrix(Yd))
+    assert np.max(np.abs(S.cpu().numpy() - So)) <= 1e-12 * np.max(np.abs(So))
+    for B in (N, 24 if N > 24 else 16):
+        Hh = op.projected_hamiltonian(Yd, B=B).cpu().numpy()
+        assert np.max(np.abs(Hh - Ho)) <= 1e-11 * np.max(np.abs(Ho)), (name, B)
+    Ss, Hs = S.cpu().numpy(), 0.5 * (Hh + Hh.T)
+    th_g = scipy.linalg.eigh(Hs, 0.5 * (Ss + Ss.T), eigvals_only=True)
+    th_o = scipy.linalg.eigh(0.5 * (Ho + Ho.T), 0.5 * (So + So.T), eigvals_only=True)
+    w = np.linalg.eigvalsh(0.5 * (So + So.T))
+    cond = w[-1] / max(w[0], 1e-300)        # generalised eigenvalues move by ~ cond(S) x the matrix error
+    assert np.max(np.abs(th_g - th_o)) <= max(1e-8, 1e-13 * cond * np.max(np.abs(Ho))), cond
+    # a wide array with ld > N and a column offset
+    wide = torch.zeros((wl.n_dofs, N + 10), dtype=torch.float64, device="cuda")
+    wide[:, 4:4 + N] = Yd
+    assert torch.equal(op.overlap_matrix(wide[:, 4:4 + N]), S)
+    op.close()
+
+
 def test_mass_diagonal_matches_the_oracle():
     torch, orc, Operator, *_ = _imports()
     wl, oop, *_ = oracle_case("p6_distorted_cells")

@@ -139,6 +139,23 @@ def test_lanczos_bound_and_rayleigh_ritz_against_dense_eigh(tiny_eig):
     assert np.all(th >= lam[:5] - 1e-10) and np.all(th <= lam[-5:] + 1e-10)
 
 
+def test_projection_matrices_closed_forms_on_eigenvectors(tiny_eig):
+    """Algorithm 2 step 1: on orthonormal eigenvectors S = I and H^ = diag(lambda); for a
+    mixture Y = V R of eigenvectors S = R^T R and H^ = R^T diag(lambda) R; S and H^ are symmetric; and the generalised
+    eigenvalues of (H^, S) are the eigenvalues of the invariant subspace (LAPACK via scipy)."""
+    import scipy.linalg
+    op, lam, V = tiny_eig
+    S, Hh = orc.projection_matrices(op, V[:, 3:10])
+    assert np.allclose(S, np.eye(7), atol=1e-12) and np.allclose(Hh, np.diag(lam[3:10]), atol=1e-10)
+    R = np.random.default_rng(8).standard_normal((7, 7))
+    S, Hh = orc.projection_matrices(op, V[:, 3:10] @ R)
+    assert np.allclose(S, R.T @ R, atol=1e-11)
+    assert np.allclose(Hh, R.T @ np.diag(lam[3:10]) @ R, atol=1e-9)
+    assert np.allclose(S, S.T, atol=1e-12) and np.allclose(Hh, Hh.T, atol=1e-10)
+    theta = scipy.linalg.eigh(0.5 * (Hh + Hh.T), S, eigvals_only=True)
+    assert np.allclose(theta, lam[3:10], atol=1e-9)
+
+
 def test_config1_stored_bounds_follow_the_recipe_and_bound_the_spectrum():
     """bounds.json (written by oracle/make_bounds.py) for config 1: b >= lambda_max and a0 <= a < b against a
     dense eigh of the 4096-dof operator, and both recipes reproduce from their seeds."""
