@@ -31,7 +31,8 @@ DEFAULT_CONFIG = 2          # BASELINE.json configs[1]
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the contraction kernel, from the `ncu --set full`
 # capture summarised in profiles/ (file named in the value); None until a capture exists for that key.
 NCU_TRAFFIC_BYTES_PER_LAUNCH = {
-    (2, 0): 1.827e9,        # profiles/r01_v3_config2.md: 1.497 GB read + 0.330 GB written per k_apply_dmma_p launch
+    (2, 0): 1.661e9,        # profiles/r01_v4_config2_config3.md: 1.334 GB read + 0.327 GB written per launch
+    (3, 0): 14.54e9,        # same file: 11.68 GB read + 2.86 GB written per launch
 }
 
 
