@@ -154,6 +154,16 @@ int chfsi_overlap_matrix(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N
 int chfsi_projected_hamiltonian(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N, int64_t B, double* H_dev,
                                 void* workspace_dev, void* cuda_stream);
 
+/* Subspace transformation  Out = Y Z  -- Algorithm 2 step 3 (RRGEP-ST; the blocked "X_p Z"
+ * products of PAPER.md:560): with Z = Q_fr it gives the Ritz vectors Psi_fr^R = Psi_f Q_fr (step 3a), with
+ * Z = L^-T (S = L L^T) the orthonormal basis Psi^o = Psi_f L^-T (step 3b).  FP64 operators only.
+ * Y_dev [n_dofs][ldy] (N columns), Z_dev [N][ldz] (N2 columns, row-major, DEVICE), Out_dev [n_dofs][ldo] (N2
+ * columns), all FP64, owned by the caller; Out must not overlap Y (CHFSI_ERR_BAD_ARGUMENT).  N, N2 and the leading
+ * dimensions must be even and the pointers 16-byte aligned (CHFSI_ERR_UNSUPPORTED otherwise).  Enqueued on
+ * cuda_stream, no synchronisation. */
+int chfsi_subspace_transform(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N, const double* Z_dev, int64_t ldz,
+                             int64_t N2, void* Out_dev, int64_t ldo, void* cuda_stream);
+
 /* Number of kernel launches enqueued by this handle since creation (for benchmark bookkeeping). */
 int64_t chfsi_launch_count(const chfsi_op* op);
 

@@ -20,7 +20,7 @@ LIB_PATH = os.path.join(HERE, "libchfsi.so")
 
 EXPORTED_SYMBOLS = [
     "chfsi_create", "chfsi_destroy", "chfsi_update_potential", "chfsi_get_info", "chfsi_workspace_bytes", "chfsi_mass_diag",
-    "chfsi_apply_H", "chfsi_overlap_matrix", "chfsi_projected_hamiltonian", "chfsi_chebyshev_filter", "chfsi_chebyshev_filter_chunked", "chfsi_chebyshev_filter_host",
+    "chfsi_apply_H", "chfsi_overlap_matrix", "chfsi_projected_hamiltonian", "chfsi_subspace_transform", "chfsi_chebyshev_filter", "chfsi_chebyshev_filter_chunked", "chfsi_chebyshev_filter_host",
     "chfsi_launch_count", "chfsi_set_kernel_variant", "chfsi_set_profiling", "chfsi_get_profile",
     "chfsi_measure_fp64_peak", "chfsi_last_error",
 ]
@@ -94,6 +94,8 @@ def load_library(build_if_missing: bool = True):
     lib_.chfsi_overlap_matrix.restype = C.c_int
     lib_.chfsi_projected_hamiltonian.argtypes = [vp, vp, i64, i64, i64, vp, vp, vp]
     lib_.chfsi_projected_hamiltonian.restype = C.c_int
+    lib_.chfsi_subspace_transform.argtypes = [vp, vp, i64, i64, vp, i64, i64, vp, i64, vp]
+    lib_.chfsi_subspace_transform.restype = C.c_int
     lib_.chfsi_chebyshev_filter.argtypes = [vp, vp, i64, i64, i32, dbl, dbl, dbl, vp, vp]
     lib_.chfsi_chebyshev_filter.restype = C.c_int
     lib_.chfsi_chebyshev_filter_chunked.argtypes = [vp, vp, i64, i64, i64, i32, dbl, dbl, dbl, vp, vp]
@@ -255,6 +257,22 @@ class Operator:
         self._check(load_library().chfsi_projected_hamiltonian(self._h, yp, ldy, N, B, C.c_void_p(Hh.data_ptr()),
                                                                C.c_void_p(ws.data_ptr()), _stream_ptr(stream)))
         return Hh
+
+    def subspace_transform(self, Y, Z, Out=None, stream=None):
+        """Out = Y Z (Algorithm 2 step 3); Z is a [N, N2] FP64 device tensor (row-major)."""
+        import torch
+        yp, ldy, N = self._block(Y, "Y")
+        if Z.dim() != 2 or Z.shape[0] != N or Z.dtype != torch.float64 or Z.stride(1) != 1 or not Z.is_cuda:
+            raise ValueError("Z must be a [N, N2] FP64 CUDA tensor with unit column stride")
+        N2 = int(Z.shape[1])
+        if Out is None:
+            Out = torch.empty((self.n_dofs, N2), dtype=torch.float64, device="cuda")
+        op_, ldo, No = self._block(Out, "Out")
+        if No != N2:
+            raise ValueError("Out must have N2 columns")
+        self._check(load_library().chfsi_subspace_transform(self._h, yp, ldy, N, C.c_void_p(Z.data_ptr()),
+                                                            int(Z.stride(0)), N2, op_, ldo, _stream_ptr(stream)))
+        return Out
 
     def chebyshev_filter(self, X, m, a, b, a0, workspace=None, stream=None):
         """In place on the columns of X."""

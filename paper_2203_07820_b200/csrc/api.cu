@@ -438,6 +438,23 @@ int chfsi_projected_hamiltonian(chfsi_op* op, const void* Y_dev, int64_t ldy, in
   return CHFSI_OK;
 }
 
+int chfsi_subspace_transform(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N, const double* Z_dev, int64_t ldz,
+                             int64_t N2, void* Out_dev, int64_t ldo, void* cuda_stream) {
+  int rc = check_rr_args(op, Y_dev, ldy, N, Out_dev);
+  if (rc) return rc;
+  if (!Z_dev) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "NULL transformation matrix");
+  if (N2 < 1 || ldz < N2 || ldo < N2 || N2 > (1 << 20)) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "need 1 <= N2 <= ldz, ldo");
+  if (N2 % 2 != 0 || ldz % 2 != 0 || ldo % 2 != 0 || (uintptr_t)Z_dev % 16 != 0)
+    return fail(op, CHFSI_ERR_UNSUPPORTED, "subspace_transform: N2, ldz, ldo must be even, pointers 16-byte aligned");
+  const char* y0 = reinterpret_cast<const char*>(Y_dev);
+  const char* o0 = reinterpret_cast<const char*>(Out_dev);
+  const size_t ybytes = (size_t)op->n_dofs * ldy * 8, obytes = (size_t)op->n_dofs * ldo * 8;
+  if (y0 < o0 + obytes && o0 < y0 + ybytes) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "Y and Out must not overlap");
+  cudaError_t ce = launch_xz(op, reinterpret_cast<const double*>(Y_dev), ldy, Z_dev, ldz, op->n_dofs, (int)N, (int)N2,
+                             reinterpret_cast<double*>(Out_dev), ldo, reinterpret_cast<cudaStream_t>(cuda_stream));
+  return ce == cudaSuccess ? CHFSI_OK : cuda_fail(op, ce, "subspace_transform");
+}
+
 int64_t chfsi_launch_count(const chfsi_op* op) { return op ? op->launches : -1; }
 
 int chfsi_set_kernel_variant(chfsi_op* op, int variant) {

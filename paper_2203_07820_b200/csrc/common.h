@@ -179,6 +179,9 @@ cudaError_t capture_diagonal(Op* op, cudaStream_t stream);
 // the stream; may grow op->rr_scratch (then it synchronises the stream once).
 cudaError_t launch_xty(Op* op, const double* A, int64_t lda, const double* B, int64_t ldb, int64_t n_rows, int N1, int N2,
                        double* C, int64_t ldc, cudaStream_t stream);
+// Out[n_rows][ldo] = Y Z, Y [n_rows][ldy] with N columns, Z [N][ldz] with N2 columns (Alg. 2 step 3)
+cudaError_t launch_xz(Op* op, const double* Y, int64_t ldy, const double* Z, int64_t ldz, int64_t n_rows, int N, int N2,
+                      double* Out, int64_t ldo, cudaStream_t stream);
 // Opts the kernels into the shared memory they need for this operator (once, at create).
 cudaError_t init_apply_kernels(Op* op);
 

@@ -114,7 +114,102 @@ __global__ void __launch_bounds__(256) k_xty_reduce(const double* __restrict__ C
   C[(e / N2) * ldc + (e % N2)] = s;
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// Subspace transformation (Algorithm 2 step 3, RRGEP-ST; the paper's blocked "X_p Z" products,
+// PAPER.md:560):   Out[g][j] = sum_i Y[g][i] Z[i][j]      Y: [n_rows][ldy] (N columns), Z: [N][ldz] (N2 columns)
+// Rows are independent, so there is no reduction across CTAs: CTA tile = 128 rows x 64 columns, K = N streamed in
+// 32-column panels of Y / 32-row panels of Z through a 2-stage cp.async ring; 8 warps as 4 x 2, 4 x 4 DMMA tiles each.
+// ---------------------------------------------------------------------------------------------------------------
+constexpr int kXzM = 128, kXzN = 64, kXzK = 32;
+constexpr int kXzLdA = kXzK + 4, kXzLdB = kXzN + 4;   // 36, 68: pitch mod 16 == 4
+
+__global__ void __launch_bounds__(256, 2) k_xz(const double* __restrict__ Y, int64_t ldy, const double* __restrict__ Z,
+                                               int64_t ldz, int64_t n_rows, int N, int N2, double* __restrict__ Out,
+                                               int64_t ldo) {
+  extern __shared__ __align__(16) double xs[];
+  constexpr int stage_elems = kXzM * kXzLdA + kXzK * kXzLdB;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int wm = warp >> 1, wn = warp & 1, fk = lane & 3, fm = lane >> 2;
+  const int j0 = blockIdx.x * kXzN;
+  const int64_t g0 = (int64_t)blockIdx.y * kXzM;
+  const int npanel = (N + kXzK - 1) / kXzK;
+
+  auto load_panel = [&](int pi) {
+    double* As = xs + (pi & 1) * stage_elems;
+    double* Bs = As + kXzM * kXzLdA;
+    const int k0 = pi * kXzK;
+#pragma unroll
+    for (int t = 0; t < 8; ++t) {                      // Y tile: 128 rows x 16 chunks of 16 B
+      const int e = tid + t * 256, r = e >> 4, c = (e & 15) * 2;
+      const bool ok = (g0 + r < n_rows) && (k0 + c < N);
+      cp_async16_zfill(As + r * kXzLdA + c, ok ? Y + (g0 + r) * ldy + k0 + c : Y, ok ? 16 : 0);
+    }
+#pragma unroll
+    for (int t = 0; t < 4; ++t) {                      // Z panel: 32 rows x 32 chunks
+      const int e = tid + t * 256, r = e >> 5, c = (e & 31) * 2;
+      const bool ok = (k0 + r < N) && (j0 + c < N2);
+      cp_async16_zfill(Bs + r * kXzLdB + c, ok ? Z + (int64_t)(k0 + r) * ldz + j0 + c : Z, ok ? 16 : 0);
+    }
+  };
+  load_panel(0);
+  asm volatile("cp.async.commit_group;" ::: "memory");
+
+  double acc[4][4][2];
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+#pragma unroll
+    for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+  for (int pi = 0; pi < npanel; ++pi) {
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    __syncthreads();                                   // panel pi has landed; everyone is done with panel pi-1
+    if (pi + 1 < npanel) load_panel(pi + 1);
+    asm volatile("cp.async.commit_group;" ::: "memory");
+    const double* As = xs + (pi & 1) * stage_elems;
+    const double* Ap = As + (wm * 32 + fm) * kXzLdA + fk;          // A fragment: row m = fm, k = fk
+    const double* Bp = As + kXzM * kXzLdA + fk * kXzLdB + wn * 32 + fm;
+#pragma unroll
+    for (int ks = 0; ks < kXzK / 4; ++ks) {
+      double b[4];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) b[j] = Bp[ks * 4 * kXzLdB + j * 8];
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        const double av = Ap[i * 8 * kXzLdA + ks * 4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) dmma884(acc[i][j][0], acc[i][j][1], av, b[j]);
+      }
+    }
+  }
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int64_t r = g0 + wm * 32 + i * 8 + fm;
+    if (r >= n_rows) continue;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      const int c = j0 + wn * 32 + j * 8 + fk * 2;
+      if (c + 1 < N2) *reinterpret_cast<double2*>(Out + r * ldo + c) = make_double2(acc[i][j][0], acc[i][j][1]);
+      else if (c < N2) Out[r * ldo + c] = acc[i][j][0];
+    }
+  }
+}
+
 }  // namespace
+
+cudaError_t launch_xz(Op* op, const double* Y, int64_t ldy, const double* Z, int64_t ldz, int64_t n_rows, int N, int N2,
+                      double* Out, int64_t ldo, cudaStream_t st) {
+  const size_t smem = (size_t)2 * (kXzM * kXzLdA + kXzK * kXzLdB) * sizeof(double);
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(k_xz, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  dim3 grid((unsigned)((N2 + kXzN - 1) / kXzN), (unsigned)((n_rows + kXzM - 1) / kXzM));
+  k_xz<<<grid, 256, smem, st>>>(Y, ldy, Z, ldz, n_rows, N, N2, Out, ldo);
+  op->launches++;
+  return cudaGetLastError();
+}
 
 cudaError_t launch_xty(Op* op, const double* A, int64_t lda, const double* B, int64_t ldb, int64_t n_rows, int N1, int N2,
                        double* C, int64_t ldc, cudaStream_t st) {

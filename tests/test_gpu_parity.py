@@ -198,6 +198,45 @@ def test_rayleigh_ritz_projection_matrices_match_the_oracle(name):
     op.close()
 
 
+def test_subspace_transform_and_a_full_rayleigh_ritz_step():
+    """chfsi_subspace_transform (Algorithm 2 step 3): Out = Y Z element-wise against Y @ Z (ragged
+    N, N2, ld > N), and the whole Rayleigh-Ritz step of Algorithm 2 assembled from the three device calls (S, H^ on
+    the device; Cholesky and the dense eigenproblem on the host; Psi^o = Y L^-T and Psi^R = Y Q on the device):
+    Psi^o is orthonormal, Psi^R diagonalises H~ in the subspace and its Ritz values equal the oracle's."""
+    import scipy.linalg
+    torch, orc, Operator, _, _, _, _ = _imports()
+    wl, oop, X, (a0, a, b), Yo, Fo = oracle_case("p6_nonlocal_ragged")
+    Y = Fo[:, :40] / np.linalg.norm(Fo[:, :40], axis=0, keepdims=True)
+    op = Operator.from_workload(wl)
+    wide = torch.zeros((wl.n_dofs, 50), dtype=torch.float64, device="cuda")
+    wide[:, 6:46] = torch.tensor(Y, device="cuda")
+    Yd = wide[:, 6:46]
+    Z = np.random.default_rng(4).standard_normal((40, 22))
+    Out = op.subspace_transform(Yd, torch.tensor(Z, device="cuda")).cpu().numpy()
+    ref = Y @ Z
+    assert np.max(np.abs(Out - ref)) <= 1e-13 * np.max(np.abs(ref))
+    # Algorithm 2, steps 1-3
+    S = op.overlap_matrix(Yd).cpu().numpy()
+    Hh = op.projected_hamiltonian(Yd, B=16).cpu().numpy()
+    L = np.linalg.cholesky(0.5 * (S + S.T))                               # step 2a
+    Linv = scipy.linalg.solve_triangular(L, np.eye(40), lower=True)
+    theta, Qp = np.linalg.eigh(Linv @ (0.5 * (Hh + Hh.T)) @ Linv.T)       # steps 2b, 2c
+    Q = Linv.T @ Qp
+    Po = op.subspace_transform(Yd, torch.tensor(np.ascontiguousarray(Linv.T), device="cuda"))      # step 3b
+    Pr = op.subspace_transform(Yd, torch.tensor(np.ascontiguousarray(Q), device="cuda"))           # step 3a
+    w = np.linalg.eigvalsh(0.5 * (S + S.T))
+    slack = 1e-13 * w[-1] / w[0]
+    assert np.max(np.abs(op.overlap_matrix(Po).cpu().numpy() - np.eye(40))) <= 1e-10 + slack
+    R = Pr.cpu().numpy()
+    G = R.T @ orc.apply_H(oop, R)
+    assert np.max(np.abs(G - np.diag(theta))) <= (1e-8 + slack) * max(1.0, np.max(np.abs(theta)))
+    th_o = orc.ritz_values_of_block(Y, orc.apply_H(oop, Y))
+    assert np.max(np.abs(theta - th_o)) <= 1e-8 + slack * np.max(np.abs(theta))
+    with pytest.raises(Exception):
+        op.subspace_transform(Yd, torch.tensor(Z, device="cuda"), Out=wide[:, 0:22])    # overlaps Y
+    op.close()
+
+
 def test_mass_diagonal_matches_the_oracle():
     torch, orc, Operator, *_ = _imports()
     wl, oop, *_ = oracle_case("p6_distorted_cells")
