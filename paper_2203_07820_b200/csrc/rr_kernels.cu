@@ -8,7 +8,7 @@
 // The stored layout is already "k-major" for both mma operands (row g = contraction index), so the fragments are
 // read exactly as in the contraction kernel.  CTA tile = 128 (i) x 64 (j); 8 warps as 4 x 2, warp tile = 4 x 4
 // tiles of mma.sync.m8n8k4.f64; the row range is split over gridDim.z CTAs whose partial tiles are summed in split
-// order by k_xty_reduce: deterministic.  Rows stream through a 4-stage cp.async ring of 8-row panels.
+// order by k_xty_reduce: deterministic.  Rows stream through a 2-stage cp.async ring of 32-row panels.
 #include <algorithm>
 
 #include "common.h"
@@ -17,7 +17,7 @@ namespace chfsi {
 
 namespace {
 
-constexpr int kXtM = 128, kXtN = 64, kXtK = 8, kXtStages = 4;
+constexpr int kXtM = 128, kXtN = 64, kXtK = 32, kXtStages = 2;
 constexpr int kXtLdA = kXtM + 4, kXtLdB = kXtN + 4;   // pitch mod 16 == 4: conflict-free 64-bit fragment loads
 
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
@@ -46,13 +46,14 @@ __global__ void __launch_bounds__(256, 2) k_xty(const double* __restrict__ A, in
     double* Bs = As + kXtK * kXtLdA;
     const int64_t g = g0 + (int64_t)pi * kXtK;
 #pragma unroll
-    for (int t = 0; t < 2; ++t) {                      // A panel: 8 rows x 64 chunks of 16 B
+    for (int t = 0; t < kXtK / 4; ++t) {               // A panel: kXtK rows x 64 chunks of 16 B
       const int e = tid + t * 256, r = e >> 6, c = (e & 63) * 2;
       const bool ok = (g + r < g1) && (i0 + c < N1);
       cp_async16_zfill(As + r * kXtLdA + c, ok ? A + (g + r) * lda + i0 + c : A, ok ? 16 : 0);
     }
-    {                                                  // B panel: 8 rows x 32 chunks
-      const int r = tid >> 5, c = (tid & 31) * 2;
+#pragma unroll
+    for (int t = 0; t < kXtK / 8; ++t) {               // B panel: kXtK rows x 32 chunks
+      const int e = tid + t * 256, r = e >> 5, c = (e & 31) * 2;
       const bool ok = (g + r < g1) && (j0 + c < N2);
       cp_async16_zfill(Bs + r * kXtLdB + c, ok ? B + (g + r) * ldb + j0 + c : B, ok ? 16 : 0);
     }
