@@ -50,6 +50,12 @@ void free_op(chfsi_op* op) {
   cudaFree(op->proj_ptr); cudaFree(op->proj_pcrow); cudaFree(op->seg_ptr); cudaFree(op->grow_dof); cudaFree(op->pcoef);
   cudaFree(op->grp_seg_ptr); cudaFree(op->proj_grp); cudaFree(op->proj_slot);
   cudaFree(op->rr_scratch);
+  for (int i = 0; i < 2; ++i) {
+    cudaFree(op->host_stage[i]);
+    if (op->host_done[i]) cudaEventDestroy(op->host_done[i]);
+    if (op->host_st[i]) cudaStreamDestroy(op->host_st[i]);
+  }
+  cudaFree(op->host_ws);
   cudaFree(op->setup_verts); cudaFree(op->setup_pp); cudaFree(op->setup_phi); cudaFree(op->setup_gx); cudaFree(op->setup_gw); cudaFree(op->D); cudaFree(op->mass); cudaFree(op->diag0);
   for (cudaEvent_t e : op->prof_events) cudaEventDestroy(e);
   delete op;
@@ -343,21 +349,31 @@ int chfsi_chebyshev_filter_host(chfsi_op* op, void* X_host, int64_t ldx, int64_t
   const int64_t Bc = std::min(B, N);
   const int64_t ldd = (Bc + 7) / 8 * 8;
   const WsLayout w = ws_layout(op, Bc);
-  // Two staging blocks and two streams: the copies of chunk i+1 / i-1 overlap the filter of chunk i.
-  void* stage[2] = {nullptr, nullptr};
-  void* ws = nullptr;
-  cudaStream_t st[2] = {nullptr, nullptr};
-  cudaEvent_t done[2] = {nullptr, nullptr};
+  // Two staging blocks and two streams: the copies of chunk i+1 / i-1 overlap the filter of chunk i.  The buffers,
+  // streams and events live in the handle and are reused by later calls (grown on demand).
   cudaError_t ce = cudaSuccess;
   rc = CHFSI_OK;
   const int nbuf = (N > Bc) ? 2 : 1;
+  const size_t stage_need = (size_t)op->n_dofs * ldd * elt;
   for (int i = 0; i < nbuf && ce == cudaSuccess; ++i) {
-    ce = cudaMalloc(&stage[i], (size_t)op->n_dofs * ldd * elt);
-    if (ce == cudaSuccess) ce = cudaStreamCreateWithFlags(&st[i], cudaStreamNonBlocking);
-    if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&done[i], cudaEventDisableTiming);
+    if (op->host_stage_bytes[i] < stage_need) {
+      cudaFree(op->host_stage[i]); op->host_stage[i] = nullptr; op->host_stage_bytes[i] = 0;
+      ce = cudaMalloc(&op->host_stage[i], stage_need);
+      if (ce == cudaSuccess) op->host_stage_bytes[i] = stage_need;
+    }
+    if (ce == cudaSuccess && !op->host_st[i]) ce = cudaStreamCreateWithFlags(&op->host_st[i], cudaStreamNonBlocking);
+    if (ce == cudaSuccess && !op->host_done[i]) ce = cudaEventCreateWithFlags(&op->host_done[i], cudaEventDisableTiming);
   }
-  if (ce == cudaSuccess) ce = cudaMalloc(&ws, w.total);
+  if (ce == cudaSuccess && op->host_ws_bytes < w.total) {
+    cudaFree(op->host_ws); op->host_ws = nullptr; op->host_ws_bytes = 0;
+    ce = cudaMalloc(&op->host_ws, w.total);
+    if (ce == cudaSuccess) op->host_ws_bytes = w.total;
+  }
   if (ce != cudaSuccess) rc = cuda_fail(op, ce, "chebyshev_filter_host allocation");
+  void** stage = op->host_stage;
+  void* ws = op->host_ws;
+  cudaStream_t* st = op->host_st;
+  cudaEvent_t* done = op->host_done;
   // The filters themselves are serialised through the single workspace by the `done` events.
   int64_t chunk = 0;
   for (int64_t j0 = 0; j0 < N && rc == CHFSI_OK; j0 += Bc, ++chunk) {
@@ -381,12 +397,6 @@ int chfsi_chebyshev_filter_host(chfsi_op* op, void* X_host, int64_t ldx, int64_t
       ce = cudaStreamSynchronize(st[i]);
       if (ce != cudaSuccess && rc == CHFSI_OK) rc = cuda_fail(op, ce, "chebyshev_filter_host sync");
     }
-  for (int i = 0; i < 2; ++i) {
-    if (done[i]) cudaEventDestroy(done[i]);
-    if (st[i]) cudaStreamDestroy(st[i]);
-    cudaFree(stage[i]);
-  }
-  cudaFree(ws);
   return rc;
 }
 

@@ -135,6 +135,13 @@ struct Op {
   // split-row partial tiles of the Rayleigh-Ritz projection products (rr_kernels.cu); grown on demand
   void* rr_scratch = nullptr;
   size_t rr_scratch_bytes = 0;
+  // device staging of chfsi_chebyshev_filter_host, kept between calls (grown on demand, freed at destroy)
+  void* host_stage[2] = {nullptr, nullptr};
+  size_t host_stage_bytes[2] = {0, 0};
+  void* host_ws = nullptr;
+  size_t host_ws_bytes = 0;
+  cudaStream_t host_st[2] = {nullptr, nullptr};
+  cudaEvent_t host_done[2] = {nullptr, nullptr};
   int64_t launches = 0;
   // optional per-kernel timing (chfsi_set_profiling): event triples (start, after projector kernels, end)
   bool profiling = false;
