@@ -215,8 +215,18 @@ cudaError_t launch_xz(Op* op, const double* Y, int64_t ldy, const double* Z, int
 cudaError_t launch_xty(Op* op, const double* A, int64_t lda, const double* B, int64_t ldb, int64_t n_rows, int N1, int N2,
                        double* C, int64_t ldc, cudaStream_t st) {
   const int ti = (N1 + kXtM - 1) / kXtM, tj = (N2 + kXtN - 1) / kXtN;
-  // enough CTAs for ~3 waves of 2 per SM, at least 512 rows per split
-  int n_split = (int)std::max<int64_t>(1, std::min<int64_t>((6 * op->n_sm + ti * tj - 1) / (ti * tj), (n_rows + 511) / 512));
+  // Row splits: at least ~3 waves of 2 CTAs per SM and at least 512 rows per split; among the candidates the one
+  // whose CTA count fills its last wave best (128 tiles x 7 splits = 3.03 waves would idle a quarter of the GPU).
+  const int cap = 2 * op->n_sm, tiles = ti * tj;
+  const int ns_max = (int)std::max<int64_t>(1, (n_rows + 511) / 512);
+  const int ns_lo = std::min(ns_max, std::max(1, (3 * cap + tiles - 1) / tiles));
+  int n_split = ns_lo;
+  double best = 0.0;
+  for (int ns = ns_lo; ns <= std::min(ns_max, 3 * ns_lo + 2); ++ns) {
+    const int64_t ctas = (int64_t)tiles * ns;
+    const double eff = (double)ctas / (double)(((ctas + cap - 1) / cap) * cap);
+    if (eff > best + 1e-9) { best = eff; n_split = ns; }
+  }
   int64_t rows_per_split = ((n_rows + n_split - 1) / n_split + kXtK - 1) / kXtK * kXtK;
   n_split = (int)((n_rows + rows_per_split - 1) / rows_per_split);
   const size_t need = (size_t)n_split * N1 * N2 * sizeof(double);
