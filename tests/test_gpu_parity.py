@@ -49,6 +49,11 @@ CASES = {
     # p = 7 (M_cell = 512): the output nodes of a cell are split over two tiles of the persistent kernel
     "p7_two_blocks": (dict(n=2, p=7, L=4.0, atoms_per_side=1, n_gaussians=0, nonlocal_=True, smooth_field=0.05,
                            seed_base=83, r_cut=1.9), 40, 5, 64),
+    # p = 8 (M_cell = 729): three blocks of 248 output nodes, the last one ragged; p = 5: 27 m-tiles (MT = 7)
+    "p8_three_blocks": (dict(n=2, p=8, L=4.0, atoms_per_side=1, n_gaussians=0, nonlocal_=True, smooth_field=0.05,
+                             seed_base=84, r_cut=1.9), 24, 4, 64),
+    "p5_nonlocal": (dict(n=3, p=5, L=6.0, atoms_per_side=1, n_gaussians=0, nonlocal_=True, smooth_field=0.05,
+                         seed_base=85), 48, 5, 64),
     "p6_fp32": (dict(n=3, p=6, L=6.0, atoms_per_side=1, n_gaussians=0, nonlocal_=True, smooth_field=0.05,
                      seed_base=77), 64, 7, 32),
     "p4_fp32_odd_B": (dict(n=3, p=4, L=6.0, atoms_per_side=1, n_gaussians=0, nonlocal_=True, smooth_field=0.05,
