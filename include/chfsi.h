@@ -34,8 +34,9 @@
  *    NULL = default stream).  They never synchronise the host.  chfsi_create and the *_host entry points
  *    synchronise before returning.
  *  - There is no CPU fallback: without a CUDA device chfsi_create returns CHFSI_ERR_CUDA.
- *  - Alignment: X_dev / Y_dev / workspace_dev must be 16-byte aligned and ld*sizeof(element) a multiple of
- *    16 for the tensor-core path; other shapes take a slower generic CUDA path (never the CPU).
+ *  - Alignment: X_dev / Y_dev / workspace_dev must be 16-byte aligned and B*sizeof(element), ld*sizeof(element)
+ *    multiples of 16 (B even for FP64, a multiple of 4 for FP32) for the tensor-core path; other shapes take a
+ *    slower generic CUDA path (never the CPU).
  */
 #ifndef CHFSI_H_
 #define CHFSI_H_

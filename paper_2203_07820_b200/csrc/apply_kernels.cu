@@ -527,7 +527,7 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<S> a, P
     const int row0 = part * a.mw;                                        // first output node of this tile
     const int nmt = max(0, min(MT, min(mtp, n_mtiles - part * mtp) - mt0));
     const int col0 = jt * kP2TileN;
-    const int ncols = min(kP2TileN, a.B - col0);             // multiple of 8
+    const int ncols = min(kP2TileN, a.B - col0);             // even (whole column pairs); the TMA zero-fills beyond B
     const int kt = a.ktot[cell];
     const int32_t* gi = a.gidx + a.idx_off[cell];
     const S* M = a.mat + a.mat_off[cell] + (int64_t)part * kt * lda;
@@ -577,7 +577,8 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<S> a, P
     if (warp < kP2Ahead && warp < npanel) produce(warp);
 
     const int nt0 = warp_n * 2;
-    const int nnt = max(0, min(2, ncols / 8 - nt0));
+    const int nnt = max(0, min(2, (ncols + 7) / 8 - nt0));
+    const bool ok0 = nt0 * 8 + fk * 2 < ncols, ok1 = nt0 * 8 + 8 + fk * 2 < ncols;   // this lane's two column pairs
     const bool active = (nnt > 0 && nmt > 0);
     // Recurrence term -beta Y_{k-2} (Eq. 37): the accumulators of the first-contribution nodes START at
     // (-beta/alpha) Y_{k-2} (the target block still holds Y_{k-2}); the loads land straight in the accumulator
@@ -595,9 +596,8 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<S> a, P
         const int idx = (i < nmt && r < mc) ? idx_s[r] : 0;
         if (idx < 0) {
           const S* tp = a.Tg + (int64_t)(idx & 0x7fffffff) * a.ldt + col0 + nt0 * 8 + fk * 2;
-          const double2 u = ld_cg_pair(tp);
-          acc[i][0][0] = u.x; acc[i][0][1] = u.y;
-          if (nnt > 1) { const double2 v = ld_cg_pair(tp + 8); acc[i][1][0] = v.x; acc[i][1][1] = v.y; }
+          if (ok0) { const double2 u = ld_cg_pair(tp); acc[i][0][0] = u.x; acc[i][0][1] = u.y; }
+          if (ok1) { const double2 v = ld_cg_pair(tp + 8); acc[i][1][0] = v.x; acc[i][1][1] = v.y; }
         }
       }
 #pragma unroll
@@ -685,7 +685,7 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<S> a, P
         const bool add = a.atomic || idx >= 0;
 #pragma unroll
         for (int j = 0; j < 2; ++j) {
-          if (j >= nnt) continue;
+          if (!(j ? ok1 : ok0)) continue;
           const double v0 = alpha * acc[i][j][0], v1 = alpha * acc[i][j][1];
           if (add) {
             atomicAdd(trow + j * 8, (S)v0);
@@ -797,7 +797,7 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
 
   // row segments of a chunk start 16-byte aligned (TMA, vector loads / stores of the fragments)
   constexpr int kPer16 = 16 / (int)sizeof(T);
-  const bool aligned = B % 8 == 0 && g.ldx % kPer16 == 0 && g.ldt % kPer16 == 0 && ((uintptr_t)g.X % 16 == 0) &&
+  const bool aligned = B % kPer16 == 0 && g.ldx % kPer16 == 0 && g.ldt % kPer16 == 0 && ((uintptr_t)g.X % 16 == 0) &&
                        ((uintptr_t)g.T % 16 == 0) && ((uintptr_t)g.P % 16 == 0) && op->max_ktot <= kMaxKtot;
   // variant 0: persistent single-launch kernel (v2); variant 2: one launch per colour (v1); variant 1: generic
   bool fast2 = false, fast = false;
@@ -809,7 +809,7 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
   CUtensorMap tmX, tmP;
   bool fast3 = false;   // 3xTF32 kernel
   const int MT16 = ((op->m_cell + 15) / 16 + 1) / 2;
-  if (sizeof(T) == 4 && aligned && op->variant == 3 && op->n_parts == 1 && g.sync != nullptr && g.epoch > 0)
+  if (sizeof(T) == 4 && aligned && B % 8 == 0 && op->variant == 3 && op->n_parts == 1 && g.sync != nullptr && g.epoch > 0)
     fast3 = (MT16 == 11 || MT16 == 7 || MT16 == 4 || MT16 == 2 || MT16 == 1) && t3_smem_bytes(op) <= 113 * 1024 &&
             make_row_gather_map(&tmX, g.X, op->n_dofs, B, g.ldx, 4, kT3TileN) &&
             make_row_gather_map(&tmP, g.P, op->n_proj + 1, B, B, 4, kT3TileN);
@@ -817,7 +817,7 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
     fast2 = (MT == 11 || MT == 8 || MT == 7 || MT == 4 || MT == 2 || MT == 1) && p2_smem_bytes<T>(op) <= 113 * 1024 &&
             make_row_gather_map(&tmX, g.X, op->n_dofs, B, g.ldx, (int)sizeof(T), kP2TileN) &&
             make_row_gather_map(&tmP, g.P, op->n_proj + 1, B, B, (int)sizeof(T), kP2TileN);
-  if (sizeof(T) == 8 && aligned && !fast2 && op->variant != 1 && op->n_parts == 1) fast = (MT == 11 || MT == 4 || MT == 2 || MT == 7);
+  if (sizeof(T) == 8 && aligned && B % 8 == 0 && !fast2 && op->variant != 1 && op->n_parts == 1) fast = (MT == 11 || MT == 4 || MT == 2 || MT == 7);
   size_t smem_fast = (size_t)kStages * (kPanelK * op->lda + kPanelK * kLdXs) * sizeof(double) + kStages * sizeof(uint64_t) +
                      (size_t)op->max_ktot * sizeof(int32_t);
   if (fast && smem_fast > 227 * 1024) fast = false;

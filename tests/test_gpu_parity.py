@@ -54,6 +54,11 @@ CASES = {
                              seed_base=84, r_cut=1.9), 24, 4, 64),
     "p5_nonlocal": (dict(n=3, p=5, L=6.0, atoms_per_side=1, n_gaussians=0, nonlocal_=True, smooth_field=0.05,
                          seed_base=85), 48, 5, 64),
+    # B = 50: not a multiple of 8 -- the persistent kernel masks the column pairs beyond B (last tile: 18 columns)
+    "p6_B50": (dict(n=3, p=6, L=6.0, atoms_per_side=1, n_gaussians=0, nonlocal_=True, smooth_field=0.05,
+                    seed_base=77), 50, 5, 64),
+    "p6_fp32_B44": (dict(n=3, p=6, L=6.0, atoms_per_side=1, n_gaussians=0, nonlocal_=True, smooth_field=0.05,
+                         seed_base=77), 44, 5, 32),
     "p6_fp32": (dict(n=3, p=6, L=6.0, atoms_per_side=1, n_gaussians=0, nonlocal_=True, smooth_field=0.05,
                      seed_base=77), 64, 7, 32),
     "p4_fp32_odd_B": (dict(n=3, p=4, L=6.0, atoms_per_side=1, n_gaussians=0, nonlocal_=True, smooth_field=0.05,
