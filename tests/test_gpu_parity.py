@@ -374,3 +374,18 @@ def test_argument_errors_on_the_device_entry_points():
     with pytest.raises(ChfsiError) as ei:
         Operator(wl.p, wl.cell_dofs, verts, wl.n_dofs, wl.veff_q)
     assert ei.value.code == -2
+    # Rayleigh-Ritz entry points: odd N is unsupported (-5), the output of a transform may not overlap its input (-1),
+    # FP32 operators are unsupported (-5)
+    Xo = torch.zeros((wl.n_dofs, 7), dtype=torch.float64, device="cuda")
+    with pytest.raises(ChfsiError) as ei:
+        op.overlap_matrix(Xo)
+    assert ei.value.code == -5
+    Z = torch.zeros((8, 8), dtype=torch.float64, device="cuda")
+    with pytest.raises(ChfsiError) as ei:
+        op.subspace_transform(X, Z, Out=X)
+    assert ei.value.code == -1
+    op32 = Operator.from_workload(wl, precision=32)
+    with pytest.raises(ChfsiError) as ei:
+        op32.overlap_matrix(torch.zeros((wl.n_dofs, 8), dtype=torch.float32, device="cuda"))
+    assert ei.value.code == -5
+    op32.close()
