@@ -704,6 +704,82 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<S> a, P
   }
 }
 
+// -------------------------------------------------------------------------------------------------------------
+// Steps 3a-3b as a TMA row stream (default when the block is 16-byte aligned; k_proj_rows above is the fallback).
+// CTA = (row segment of <= 128 dofs, 256-column tile); the rows are gathered by tile::gather4 (box = 256 columns)
+// into a 6-stage ring of 8 rows, 96 KB in flight per CTA and two CTAs per SM, so the stream does not depend on
+// per-thread loads in flight; thread t owns column t of the tile and accumulates the 8 projector coefficients of the
+// group over the rows of the segment in row order (no cross-thread reduction): deterministic.  HBM-bound.
+// -------------------------------------------------------------------------------------------------------------
+constexpr int kPTRows = 8, kPTStages = 6, kPTAhead = kPTStages - 2;
+template <typename T>
+size_t pt_smem_bytes() {
+  return (size_t)kPTStages * kPTRows * kPRCols * sizeof(T) + (size_t)kProjSegRows * kProjGroup * sizeof(T) +
+         (size_t)(kProjSegRows + 8) * sizeof(int32_t) + 2 * kPTStages * sizeof(uint64_t);
+}
+template <typename T>
+__global__ void __launch_bounds__(256, 2) k_proj_rows_tma(const int32_t* __restrict__ seg_ptr, const int32_t* __restrict__ grow_dof,
+                                                          const T* __restrict__ pcoef, double* __restrict__ Pc, int B,
+                                                          const __grid_constant__ CUtensorMap tmX) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  T* ring = reinterpret_cast<T*>(smem_raw);                                        // [stages][8 rows][256 columns]
+  T* cs = ring + kPTStages * kPTRows * kPRCols;                                    // [128][8]
+  int32_t* dofs = reinterpret_cast<int32_t*>(cs + kProjSegRows * kProjGroup);     // [128 + 8]
+  uint64_t* full = reinterpret_cast<uint64_t*>(dofs + kProjSegRows + 8);
+  uint64_t* empty = full + kPTStages;
+  const int seg = blockIdx.x;
+  const int r0 = seg_ptr[seg], nr = seg_ptr[seg + 1] - r0;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int col0 = blockIdx.y * kPRCols;
+  for (int e = tid; e < nr * kProjGroup; e += 256) cs[e] = pcoef[(int64_t)r0 * kProjGroup + e];
+  for (int e = tid; e < kProjSegRows + 8; e += 256) dofs[e] = grow_dof[r0 + min(e, nr - 1)];   // tail: any valid row
+  if (tid == 0) {
+    for (int s = 0; s < kPTStages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 8); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  const int npanel = (nr + kPTRows - 1) / kPTRows;
+  auto produce = [&](int pj) {
+    if (lane != 0) return;
+    const int s = pj % kPTStages;
+    mbar_wait(&empty[s], ((pj / kPTStages) & 1) ^ 1);
+    const int k0 = pj * kPTRows;
+    const int rows = min(kPTRows, (nr - k0 + 3) / 4 * 4);
+    mbar_expect_tx(&full[s], (uint32_t)(rows * kPRCols * sizeof(T)));
+    for (int r = 0; r < rows; r += 4)
+      tma_gather4(ring + (s * kPTRows + r) * kPRCols, &tmX, col0, dofs[k0 + r], dofs[k0 + r + 1], dofs[k0 + r + 2],
+                  dofs[k0 + r + 3], &full[s]);
+  };
+  if (warp < kPTAhead && warp < npanel) produce(warp);
+  double acc[kProjGroup];
+#pragma unroll
+  for (int i = 0; i < kProjGroup; ++i) acc[i] = 0.0;
+  for (int pi = 0; pi < npanel; ++pi) {
+    const int s = pi % kPTStages;
+    {
+      const int pj = pi + kPTAhead;
+      if (pj < npanel && (pj & 7) == warp) produce(pj);
+    }
+    mbar_wait(&full[s], (pi / kPTStages) & 1);
+    const int rows = min(kPTRows, nr - pi * kPTRows);
+    const T* xs = ring + s * kPTRows * kPRCols + tid;
+    const T* cp = cs + pi * kPTRows * kProjGroup;
+#pragma unroll 4
+    for (int r = 0; r < rows; ++r) {
+      const double x = (double)xs[r * kPRCols];
+#pragma unroll
+      for (int i = 0; i < kProjGroup; ++i) acc[i] = fma((double)cp[r * kProjGroup + i], x, acc[i]);
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&empty[s]);
+  }
+  const int col = col0 + tid;
+  if (col < B) {
+#pragma unroll
+    for (int i = 0; i < kProjGroup; ++i) Pc[((int64_t)seg * kProjGroup + i) * B + col] = acc[i];
+  }
+}
+
 #include "apply_tf32.cuh"
 
 // Tensor map of a row-major FP64 / FP32 block [rows][ld] restricted to its first `cols` columns, box = box_cols x 1
@@ -779,8 +855,14 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
   double* Pc = reinterpret_cast<double*>(g.Pc);
   if (op->n_pseg > 0) {
     dim3 g1((unsigned)op->n_pseg, (unsigned)((B + kPRCols - 1) / kPRCols));
-    const int vec_ok = (g.ldx % 2 == 0 && (uintptr_t)g.X % 16 == 0) ? 1 : 0;
-    k_proj_rows<T><<<g1, 256, 0, st>>>(op->seg_ptr, op->grow_dof, reinterpret_cast<const T*>(op->pcoef), X, g.ldx, Pc, B, vec_ok);
+    CUtensorMap tmXp;
+    if (op->variant != 1 && make_row_gather_map(&tmXp, g.X, op->n_dofs, B, g.ldx, (int)sizeof(T), kPRCols)) {
+      k_proj_rows_tma<T><<<g1, 256, pt_smem_bytes<T>(), st>>>(op->seg_ptr, op->grow_dof, reinterpret_cast<const T*>(op->pcoef), Pc,
+                                                             B, tmXp);
+    } else {
+      const int vec_ok = (g.ldx % 2 == 0 && (uintptr_t)g.X % 16 == 0) ? 1 : 0;
+      k_proj_rows<T><<<g1, 256, 0, st>>>(op->seg_ptr, op->grow_dof, reinterpret_cast<const T*>(op->pcoef), X, g.ldx, Pc, B, vec_ok);
+    }
     op->launches++;
   }
   {
@@ -962,6 +1044,8 @@ cudaError_t init_apply_kernels(Op* op) {
       if ((e = cudaFuncSetAttribute(k_apply_tf32_p<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_t3))) return e;
     }
   }
+  if ((e = cudaFuncSetAttribute(k_proj_rows_tma<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pt_smem_bytes<double>()))) return e;
+  if ((e = cudaFuncSetAttribute(k_proj_rows_tma<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pt_smem_bytes<float>()))) return e;
   size_t smem_gen = (size_t)op->max_ktot * 32 * 8;
   if (smem_gen > 227 * 1024) return cudaErrorInvalidValue;
   if ((e = cudaFuncSetAttribute(k_apply_generic<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_gen))) return e;
