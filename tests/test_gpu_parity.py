@@ -52,6 +52,8 @@ CASES = {
     # p = 8 (M_cell = 729): three blocks of 248 output nodes, the last one ragged; p = 5: 27 m-tiles (MT = 7)
     "p8_three_blocks": (dict(n=2, p=8, L=4.0, atoms_per_side=1, n_gaussians=0, nonlocal_=True, smooth_field=0.05,
                              seed_base=84, r_cut=1.9), 24, 4, 64),
+    "p1_linear_elements": (dict(n=6, p=1, L=6.0, atoms_per_side=1, n_gaussians=0, nonlocal_=True, smooth_field=0.05,
+                                seed_base=86, r_cut=2.5), 16, 4, 64),
     "p5_nonlocal": (dict(n=3, p=5, L=6.0, atoms_per_side=1, n_gaussians=0, nonlocal_=True, smooth_field=0.05,
                          seed_base=85), 48, 5, 64),
     # B = 50: not a multiple of 8 -- the persistent kernel masks the column pairs beyond B (last tile: 18 columns)
