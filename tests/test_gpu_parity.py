@@ -61,6 +61,8 @@ CASES = {
                     seed_base=77), 50, 5, 64),
     "p6_fp32_B44": (dict(n=3, p=6, L=6.0, atoms_per_side=1, n_gaussians=0, nonlocal_=True, smooth_field=0.05,
                          seed_base=77), 44, 5, 32),
+    "p7_fp32": (dict(n=2, p=7, L=4.0, atoms_per_side=1, n_gaussians=0, nonlocal_=True, smooth_field=0.05,
+                     seed_base=83, r_cut=1.9), 40, 5, 32),
     "p6_fp32": (dict(n=3, p=6, L=6.0, atoms_per_side=1, n_gaussians=0, nonlocal_=True, smooth_field=0.05,
                      seed_base=77), 64, 7, 32),
     "p4_fp32_odd_B": (dict(n=3, p=4, L=6.0, atoms_per_side=1, n_gaussians=0, nonlocal_=True, smooth_field=0.05,
