@@ -48,6 +48,9 @@ def parse_args():
     ap.add_argument("--variant", type=int, default=0, choices=[0, 1, 2, 3],
                     help="contraction kernel: 0 default (persistent single launch), 1 generic, 2 one launch per colour, "
                          "3 FP32 storage with 3xTF32 products (opt-in, looser accuracy)")
+    ap.add_argument("--block-width", type=int, default=0,
+                    help="override the chunk width B of the config (block-width sweep, the shape of the paper's Fig. 2a); "
+                         "N becomes one chunk of that width")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -336,6 +339,9 @@ def main():
     args = parse_args()
     from workloads.generate import CONFIGS
     spec = CONFIGS[args.config]
+    if args.block_width > 0:
+        import dataclasses
+        spec = dataclasses.replace(spec, B=args.block_width, N=args.block_width)
     if args.impl == "reference":
         run_reference(args, spec)
     else:
