@@ -33,6 +33,14 @@
  *  - All device work of the *_dev entry points is enqueued on the caller's cudaStream_t (passed as void*,
  *    NULL = default stream).  They never synchronise the host.  chfsi_create and the *_host entry points
  *    synchronise before returning.
+ *  - A handle is NOT re-entrant: it carries mutable state (the spectral shift of the running filter sits on the
+ *    diagonals of the stored cell matrices, scratch buffers of the Rayleigh-Ritz products, staging of the *_host
+ *    entry point, launch counters).  Host calls on one handle must therefore come from one thread at a time, and
+ *    the DEVICE work of successive calls on one handle never overlaps: when a call is enqueued on a different
+ *    stream than the previous call on that handle, the library makes the new stream wait (cudaStreamWaitEvent) for
+ *    the previous call's work first; the *_host entry point does the same for its internal streams.  Use one handle
+ *    per concurrent stream if overlap between filters is wanted.  The caller's workspace belongs to the call that
+ *    received it until that call's work has completed.
  *  - There is no CPU fallback: without a CUDA device chfsi_create returns CHFSI_ERR_CUDA.
  *  - Alignment: X_dev / Y_dev / workspace_dev must be 16-byte aligned and B*sizeof(element), ld*sizeof(element)
  *    multiples of 16 (B even for FP64, a multiple of 4 for FP32) for the tensor-core path; other shapes take a

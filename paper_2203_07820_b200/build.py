@@ -36,18 +36,32 @@ def _stale() -> bool:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    """Compile (if stale) and return the path of libchfsi.so."""
+    """Compile (if stale) and return the path of libchfsi.so.  Safe under torchrun: concurrent callers serialise on
+    a file lock (the first one builds, the others find a fresh library), and the library is moved into place
+    atomically, so no rank ever dlopens a half-written file."""
     if not force and not _stale():
         return LIB
+    import fcntl
+    os.makedirs(os.path.join(HERE, "build"), exist_ok=True)
+    with open(os.path.join(HERE, "build", ".lock"), "w") as lock:
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        try:
+            if not force and not _stale():          # another process built it while we waited
+                return LIB
+            return _build_locked(verbose)
+        finally:
+            fcntl.flock(lock, fcntl.LOCK_UN)
+
+
+def _build_locked(verbose: bool) -> str:
     nvcc = _nvcc()
     objs = []
     procs = []
-    os.makedirs(os.path.join(HERE, "build"), exist_ok=True)
     for s in SOURCES:
         obj = os.path.join(HERE, "build", s + ".o")
         cmd = [nvcc, "-O3", "-std=c++17", "-lineinfo", *ARCH, "-Xcompiler", "-fPIC", "-x", "cu",
                "-c", os.path.join(CSRC, s), "-o", obj]
-        cmd[1:1] = os.environ.get("CHFSI_NVCC_FLAGS", "").split()     # e.g. -DCHFSI_TRACE (debug time stamps)
+        cmd[1:1] = os.environ.get("CHFSI_NVCC_FLAGS", "").split()     # extra flags, e.g. -Xptxas=-v
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
         procs.append((s, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
@@ -62,8 +76,10 @@ def build(force: bool = False, verbose: bool = False) -> str:
             sys.stderr.write(f"--- {s}\n{out}\n")
     if failed:
         raise RuntimeError("libchfsi build failed")
-    cmd = [nvcc, "-shared", *ARCH, "-o", LIB, *objs, "-cudart", "shared"]
+    tmp = LIB + f".tmp{os.getpid()}"
+    cmd = [nvcc, "-shared", *ARCH, "-o", tmp, *objs, "-cudart", "shared"]
     subprocess.run(cmd, check=True)
+    os.replace(tmp, LIB)
     return LIB
 
 

@@ -10,6 +10,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <exception>
 #include <new>
 
 #include "common.h"
@@ -56,6 +57,7 @@ void free_op(chfsi_op* op) {
     if (op->host_st[i]) cudaStreamDestroy(op->host_st[i]);
   }
   cudaFree(op->host_ws);
+  if (op->order_ev) cudaEventDestroy(op->order_ev);
   cudaFree(op->setup_verts); cudaFree(op->setup_pp); cudaFree(op->setup_phi); cudaFree(op->setup_gx); cudaFree(op->setup_gw); cudaFree(op->D); cudaFree(op->mass); cudaFree(op->diag0);
   for (cudaEvent_t e : op->prof_events) cudaEventDestroy(e);
   delete op;
@@ -126,6 +128,30 @@ int filter_block(chfsi_op* op, void* X, int64_t ldx, int64_t B, int32_t m, doubl
   return CHFSI_OK;
 }
 
+// One handle carries mutable state (the spectral shift on the matrix diagonals, scratch buffers, counters), so the
+// device work of successive calls on one handle must not overlap.  Calls on DIFFERENT streams are therefore chained
+// through an event: each call first makes its stream wait for the previous call's work on this handle.
+cudaError_t order_enter(chfsi_op* op, cudaStream_t st) {
+  if (op->order_valid && st != op->order_stream) return cudaStreamWaitEvent(st, op->order_ev, 0);
+  return cudaSuccess;
+}
+cudaError_t order_leave(chfsi_op* op, cudaStream_t st) {
+  if (!op->order_ev) {
+    cudaError_t e = cudaEventCreateWithFlags(&op->order_ev, cudaEventDisableTiming);
+    if (e != cudaSuccess) return e;
+  }
+  cudaError_t e = cudaEventRecord(op->order_ev, st);
+  if (e == cudaSuccess) { op->order_stream = st; op->order_valid = true; }
+  return e;
+}
+
+// Nothing throws across the ABI: every entry point runs its body inside API_TRY / API_CATCH.
+#define API_TRY try {
+#define API_CATCH(op_)                                                                                        \
+  } catch (const std::bad_alloc&) { return fail(op_, CHFSI_ERR_OUT_OF_MEMORY, "host allocation failed"); }    \
+    catch (const std::exception& ex_) { return fail(op_, CHFSI_ERR_CUDA, std::string("internal error: ") + ex_.what()); } \
+    catch (...) { return fail(op_, CHFSI_ERR_CUDA, "internal error"); }
+
 int check_filter_scalars(chfsi_op* op, int32_t m, double a, double b, double a0) {
   if (m < 1) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "m < 1");
   if (!(a0 <= a && a < b) || !std::isfinite(a0) || !std::isfinite(b))
@@ -161,6 +187,7 @@ int chfsi_create(chfsi_op** out, const chfsi_mesh* mesh, const chfsi_potential* 
 
   chfsi_op* op = new (std::nothrow) chfsi_op();
   if (!op) return fail(nullptr, CHFSI_ERR_OUT_OF_MEMORY, "host allocation failed");
+  try {
   op->p = mesh->p; op->n1 = mesh->p + 1; op->nq1 = mesh->p + 2;
   op->m_cell = op->n1 * op->n1 * op->n1; op->n_q = op->nq1 * op->nq1 * op->nq1;
   op->mpad = (op->m_cell + 7) / 8 * 8;
@@ -178,14 +205,8 @@ int chfsi_create(chfsi_op** out, const chfsi_mesh* mesh, const chfsi_potential* 
   Tables1D tab;
   build_tables(op->p, &tab);
   HostPlan plan;
-  std::string msg;
-  try {
-    msg = analyse_mesh(*mesh, has_nl ? nl : nullptr, tab, op->lda, op->n_parts, &plan);
-  } catch (const std::bad_alloc&) {
-    delete op;
-    return fail(nullptr, CHFSI_ERR_OUT_OF_MEMORY, "host allocation failed in mesh analysis");
-  }
-  if (!msg.empty()) { delete op; return fail(nullptr, CHFSI_ERR_BAD_MESH, msg); }
+  std::string msg = analyse_mesh(*mesh, has_nl ? nl : nullptr, tab, op->lda, op->n_parts, &plan);
+  if (!msg.empty()) { free_op(op); return fail(nullptr, CHFSI_ERR_BAD_MESH, msg); }
 
   op->n_colors = plan.n_colors; op->color_ptr = plan.color_ptr;
   op->nnz_cp = (int64_t)plan.cell_proj_idx.size();
@@ -233,17 +254,19 @@ int chfsi_create(chfsi_op** out, const chfsi_mesh* mesh, const chfsi_potential* 
   bool bad_jac = false;
   CKC(build_cell_matrices(op, plan, tab, *mesh, *pot, has_nl ? nl : nullptr, st, &bad_jac), "cell-matrix setup");
   if (bad_jac) { free_op(op); return fail(nullptr, CHFSI_ERR_BAD_MESH, "non-positive Jacobian at a quadrature point"); }
-  try {
-    CKC(assemble_projector_rows(op, plan, *mesh, st), "projector-row assembly");
-  } catch (const std::bad_alloc&) {
-    free_op(op);
-    return fail(nullptr, CHFSI_ERR_OUT_OF_MEMORY, "host allocation failed in projector-row assembly");
-  }
+  CKC(assemble_projector_rows(op, plan, *mesh, st), "projector-row assembly");
   CKC(cudaMalloc((void**)&op->diag0, (size_t)op->n_cells * op->m_cell * sizeof(double)), "cudaMalloc(diagonal)");
   CKC(capture_diagonal(op, st), "diagonal capture");
   CKC(init_apply_kernels(op), "kernel attribute setup");
   CKC(cudaStreamSynchronize(st), "sync");
 #undef CKC
+  } catch (const std::bad_alloc&) {
+    free_op(op);
+    return fail(nullptr, CHFSI_ERR_OUT_OF_MEMORY, "host allocation failed in chfsi_create");
+  } catch (...) {
+    free_op(op);
+    return fail(nullptr, CHFSI_ERR_CUDA, "internal error in chfsi_create");
+  }
   *out = op;
   return CHFSI_OK;
 }
@@ -257,14 +280,18 @@ int chfsi_destroy(chfsi_op* op) {
 int chfsi_update_potential(chfsi_op* op, const chfsi_potential* pot, void* cuda_stream) {
   if (!op) return CHFSI_ERR_BAD_ARGUMENT;
   if (!pot || !pot->veff_q) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "NULL potential pointer");
+  API_TRY
   cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
-  cudaError_t ce = rebuild_local_matrices(op, pot->veff_q, st);
+  cudaError_t ce = order_enter(op, st);
+  if (ce == cudaSuccess) ce = rebuild_local_matrices(op, pot->veff_q, st);
   if (ce != cudaSuccess) return cuda_fail(op, ce, "update_potential (cell matrices)");
   ce = capture_diagonal(op, st);      // new unshifted diagonals; the spectral shift of the last filter is gone
   if (ce == cudaSuccess) ce = cudaStreamSynchronize(st);
   if (ce != cudaSuccess) return cuda_fail(op, ce, "update_potential (diagonal)");
   op->launches += 2;
+  op->order_valid = false;             // the stream was synchronised: nothing of this handle is in flight
   return CHFSI_OK;
+  API_CATCH(op)
 }
 
 int chfsi_get_info(const chfsi_op* op, chfsi_info* info) {
@@ -299,6 +326,8 @@ int chfsi_apply_H(chfsi_op* op, const void* X_dev, int64_t ldx, void* Y_dev, int
   if (!Y_dev) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "NULL output block");
   if (ldy < B) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "ldy < B");
   if (X_dev == Y_dev) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "X and Y must not overlap");
+  API_TRY
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
   const WsLayout w = ws_layout(op, B);
   char* base = reinterpret_cast<char*>(workspace_dev);
   ApplyArgs g;
@@ -306,12 +335,15 @@ int chfsi_apply_H(chfsi_op* op, const void* X_dev, int64_t ldx, void* Y_dev, int
   g.alpha = 1.0; g.beta = 0.0; g.cshift = 0.0;
   g.P = base + w.p_off; g.Pc = base + w.pc_off;
   g.sync = reinterpret_cast<unsigned long long*>(base + w.sync_off); g.epoch = 1;
-  cudaError_t ce = cudaMemsetAsync(g.sync, 0, w.sync_bytes, reinterpret_cast<cudaStream_t>(cuda_stream));
+  cudaError_t ce = order_enter(op, st);
+  if (ce == cudaSuccess) ce = cudaMemsetAsync(g.sync, 0, w.sync_bytes, st);
   if (ce != cudaSuccess) return cuda_fail(op, ce, "apply_H memset");
   op->launches++;
-  ce = launch_apply(op, g, reinterpret_cast<cudaStream_t>(cuda_stream));
+  ce = launch_apply(op, g, st);
+  if (ce == cudaSuccess) ce = order_leave(op, st);
   if (ce != cudaSuccess) return cuda_fail(op, ce, "apply_H launch");
   return CHFSI_OK;
+  API_CATCH(op)
 }
 
 int chfsi_chebyshev_filter(chfsi_op* op, void* X_dev, int64_t ldx, int64_t B, int32_t m, double a, double b,
@@ -319,7 +351,15 @@ int chfsi_chebyshev_filter(chfsi_op* op, void* X_dev, int64_t ldx, int64_t B, in
   int rc = check_block_args(op, X_dev, ldx, B, workspace_dev);
   if (rc) return rc;
   if ((rc = check_filter_scalars(op, m, a, b, a0))) return rc;
-  return filter_block(op, X_dev, ldx, B, m, a, b, a0, workspace_dev, reinterpret_cast<cudaStream_t>(cuda_stream));
+  API_TRY
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  cudaError_t ce = order_enter(op, st);
+  if (ce != cudaSuccess) return cuda_fail(op, ce, "chebyshev_filter");
+  rc = filter_block(op, X_dev, ldx, B, m, a, b, a0, workspace_dev, st);
+  if (rc) return rc;
+  ce = order_leave(op, st);
+  return ce == cudaSuccess ? CHFSI_OK : cuda_fail(op, ce, "chebyshev_filter");
+  API_CATCH(op)
 }
 
 int chfsi_chebyshev_filter_chunked(chfsi_op* op, void* X_dev, int64_t ldx, int64_t N, int64_t B, int32_t m,
@@ -328,14 +368,19 @@ int chfsi_chebyshev_filter_chunked(chfsi_op* op, void* X_dev, int64_t ldx, int64
   if (rc) return rc;
   if (N < 1 || ldx < N) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "need 1 <= N <= ld");
   if ((rc = check_filter_scalars(op, m, a, b, a0))) return rc;
+  API_TRY
   const size_t elt = op->precision == 64 ? 8 : 4;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  cudaError_t ce = order_enter(op, st);
+  if (ce != cudaSuccess) return cuda_fail(op, ce, "chebyshev_filter_chunked");
   for (int64_t j0 = 0; j0 < N; j0 += B) {
     const int64_t bw = std::min(B, N - j0);
-    rc = filter_block(op, reinterpret_cast<char*>(X_dev) + (size_t)j0 * elt, ldx, bw, m, a, b, a0, workspace_dev,
-                      reinterpret_cast<cudaStream_t>(cuda_stream));
+    rc = filter_block(op, reinterpret_cast<char*>(X_dev) + (size_t)j0 * elt, ldx, bw, m, a, b, a0, workspace_dev, st);
     if (rc) return rc;
   }
-  return CHFSI_OK;
+  ce = order_leave(op, st);
+  return ce == cudaSuccess ? CHFSI_OK : cuda_fail(op, ce, "chebyshev_filter_chunked");
+  API_CATCH(op)
 }
 
 int chfsi_chebyshev_filter_host(chfsi_op* op, void* X_host, int64_t ldx, int64_t N, int64_t B, int32_t m, double a,
@@ -345,12 +390,18 @@ int chfsi_chebyshev_filter_host(chfsi_op* op, void* X_host, int64_t ldx, int64_t
   if (B < 1 || N < 1 || ldx < N) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "need B >= 1 and 1 <= N <= ld");
   int rc = check_filter_scalars(op, m, a, b, a0);
   if (rc) return rc;
+  API_TRY
   const size_t elt = op->precision == 64 ? 8 : 4;
-  const int64_t Bc = std::min(B, N);
+  // Pipeline width: the copies of chunk i+1 / i-1 overlap the filter of chunk i on two streams.  A job of fewer than
+  // four chunks is cut into (up to) four narrower ones (multiples of 32 columns, at least 64) so that a single-chunk
+  // job overlaps its transfers too; columns are independent, so the result does not change.
+  int64_t Bc = std::min(B, N);
+  if (N < 4 * Bc) {
+    const int64_t quarter = ((N + 3) / 4 + 31) / 32 * 32;
+    Bc = std::min(Bc, std::max<int64_t>(64, quarter));
+  }
   const int64_t ldd = (Bc + 7) / 8 * 8;
   const WsLayout w = ws_layout(op, Bc);
-  // Two staging blocks and two streams: the copies of chunk i+1 / i-1 overlap the filter of chunk i.  The buffers,
-  // streams and events live in the handle and are reused by later calls (grown on demand).
   cudaError_t ce = cudaSuccess;
   rc = CHFSI_OK;
   const int nbuf = (N > Bc) ? 2 : 1;
@@ -363,6 +414,8 @@ int chfsi_chebyshev_filter_host(chfsi_op* op, void* X_host, int64_t ldx, int64_t
     }
     if (ce == cudaSuccess && !op->host_st[i]) ce = cudaStreamCreateWithFlags(&op->host_st[i], cudaStreamNonBlocking);
     if (ce == cudaSuccess && !op->host_done[i]) ce = cudaEventCreateWithFlags(&op->host_done[i], cudaEventDisableTiming);
+    // earlier asynchronous work on this handle (any stream) comes first
+    if (ce == cudaSuccess && op->order_valid) ce = cudaStreamWaitEvent(op->host_st[i], op->order_ev, 0);
   }
   if (ce == cudaSuccess && op->host_ws_bytes < w.total) {
     cudaFree(op->host_ws); op->host_ws = nullptr; op->host_ws_bytes = 0;
@@ -398,6 +451,7 @@ int chfsi_chebyshev_filter_host(chfsi_op* op, void* X_host, int64_t ldx, int64_t
       if (ce != cudaSuccess && rc == CHFSI_OK) rc = cuda_fail(op, ce, "chebyshev_filter_host sync");
     }
   return rc;
+  API_CATCH(op)
 }
 
 namespace {
@@ -415,9 +469,14 @@ int check_rr_args(chfsi_op* op, const void* Y, int64_t ldy, int64_t N, const voi
 int chfsi_overlap_matrix(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N, double* S_dev, void* cuda_stream) {
   int rc = check_rr_args(op, Y_dev, ldy, N, S_dev);
   if (rc) return rc;
+  API_TRY
   const double* Y = reinterpret_cast<const double*>(Y_dev);
-  cudaError_t ce = launch_xty(op, Y, ldy, Y, ldy, op->n_dofs, (int)N, (int)N, S_dev, N, reinterpret_cast<cudaStream_t>(cuda_stream));
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  cudaError_t ce = order_enter(op, st);
+  if (ce == cudaSuccess) ce = launch_xty(op, Y, ldy, Y, ldy, op->n_dofs, (int)N, (int)N, S_dev, N, st);
+  if (ce == cudaSuccess) ce = order_leave(op, st);
   return ce == cudaSuccess ? CHFSI_OK : cuda_fail(op, ce, "overlap_matrix");
+  API_CATCH(op)
 }
 
 int chfsi_projected_hamiltonian(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N, int64_t B, double* H_dev,
@@ -426,12 +485,17 @@ int chfsi_projected_hamiltonian(chfsi_op* op, const void* Y_dev, int64_t ldy, in
   if (rc) return rc;
   if (B < 2 || B % 2 != 0) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "chunk width B must be even and >= 2");
   if (!workspace_dev || (uintptr_t)workspace_dev % 16 != 0) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "bad workspace");
+  API_TRY
   cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
   const double* Y = reinterpret_cast<const double*>(Y_dev);
   const int64_t Bc = std::min(B, N);
   const WsLayout w = ws_layout(op, Bc);
   char* base = reinterpret_cast<char*>(workspace_dev);
   double* W = reinterpret_cast<double*>(base + w.block_off);
+  {
+    cudaError_t ce0 = order_enter(op, st);
+    if (ce0 != cudaSuccess) return cuda_fail(op, ce0, "projected_hamiltonian");
+  }
   for (int64_t j0 = 0; j0 < N; j0 += Bc) {
     const int64_t bw = std::min(Bc, N - j0);
     ApplyArgs g;                                        // W <- H~ Y[:, j0 : j0 + bw]
@@ -445,7 +509,12 @@ int chfsi_projected_hamiltonian(chfsi_op* op, const void* Y_dev, int64_t ldy, in
     if (ce == cudaSuccess) ce = launch_xty(op, Y, ldy, W, w.ldw, op->n_dofs, (int)N, (int)bw, H_dev + j0, N, st);
     if (ce != cudaSuccess) return cuda_fail(op, ce, "projected_hamiltonian");
   }
+  {
+    cudaError_t ce1 = order_leave(op, st);
+    if (ce1 != cudaSuccess) return cuda_fail(op, ce1, "projected_hamiltonian");
+  }
   return CHFSI_OK;
+  API_CATCH(op)
 }
 
 int chfsi_subspace_transform(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N, const double* Z_dev, int64_t ldz,
@@ -460,9 +529,15 @@ int chfsi_subspace_transform(chfsi_op* op, const void* Y_dev, int64_t ldy, int64
   const char* o0 = reinterpret_cast<const char*>(Out_dev);
   const size_t ybytes = (size_t)op->n_dofs * ldy * 8, obytes = (size_t)op->n_dofs * ldo * 8;
   if (y0 < o0 + obytes && o0 < y0 + ybytes) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "Y and Out must not overlap");
-  cudaError_t ce = launch_xz(op, reinterpret_cast<const double*>(Y_dev), ldy, Z_dev, ldz, op->n_dofs, (int)N, (int)N2,
-                             reinterpret_cast<double*>(Out_dev), ldo, reinterpret_cast<cudaStream_t>(cuda_stream));
+  API_TRY
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  cudaError_t ce = order_enter(op, st);
+  if (ce == cudaSuccess)
+    ce = launch_xz(op, reinterpret_cast<const double*>(Y_dev), ldy, Z_dev, ldz, op->n_dofs, (int)N, (int)N2,
+                   reinterpret_cast<double*>(Out_dev), ldo, st);
+  if (ce == cudaSuccess) ce = order_leave(op, st);
   return ce == cudaSuccess ? CHFSI_OK : cuda_fail(op, ce, "subspace_transform");
+  API_CATCH(op)
 }
 
 int64_t chfsi_launch_count(const chfsi_op* op) { return op ? op->launches : -1; }
@@ -483,6 +558,7 @@ int chfsi_set_profiling(chfsi_op* op, int enabled) {
 
 int chfsi_get_profile(chfsi_op* op, chfsi_profile* prof) {
   if (!op || !prof) return CHFSI_ERR_BAD_ARGUMENT;
+  API_TRY
   std::memset(prof, 0, sizeof(*prof));
   for (size_t i = 0; i + 3 <= op->prof_used; i += 3) {
     cudaError_t ce = cudaEventSynchronize(op->prof_events[i + 2]);
@@ -495,6 +571,7 @@ int chfsi_get_profile(chfsi_op* op, chfsi_profile* prof) {
   prof->contraction_launches = op->prof_main_launches; prof->projector_launches = op->prof_proj_launches;
   op->prof_used = 0; op->prof_main_launches = 0; op->prof_proj_launches = 0;
   return CHFSI_OK;
+  API_CATCH(op)
 }
 
 const char* chfsi_last_error(const chfsi_op* op) { return op ? op->err.c_str() : g_create_error.c_str(); }

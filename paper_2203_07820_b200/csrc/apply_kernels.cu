@@ -428,18 +428,7 @@ struct PersistDev {
   unsigned long long ticket_base;
   uint32_t epoch;
   int n_tiles;
-#ifdef CHFSI_TRACE
-  long long* trace;                         // [grid][64 tiles][2 warps][16] clock64 stamps (debug builds only)
-  int debug_flags;                          // bit 0: skip the epilogue (timing experiments only; results are wrong)
-#endif
 };
-#ifdef CHFSI_TRACE
-#define TRACE_STAMP(slot) do { if (tr) tr[slot] = clock64(); } while (0)
-#define TRACE_ADD(slot, v) do { if (tr) tr[slot] += (v); } while (0)
-#else
-#define TRACE_STAMP(slot) do { } while (0)
-#define TRACE_ADD(slot, v) do { } while (0)
-#endif
 
 __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
@@ -515,13 +504,6 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<S> a, P
   for (int iter = 0;; ++iter) {
     const long long ticket = ticket_s[iter & 1];
     if (ticket >= pd.n_tiles) break;
-#ifdef CHFSI_TRACE
-    long long* tr = nullptr;
-    if (pd.trace && lane == 0 && (warp == 0 || warp == 7) && iter < 64)
-      tr = pd.trace + (((long long)blockIdx.x * 64 + iter) * 2 + (warp ? 1 : 0)) * 16;
-    if (tr) { for (int z = 6; z < 16; ++z) tr[z] = 0; }
-    TRACE_STAMP(0);
-#endif
     const int pos = (int)(ticket / (np * nct)), part = (int)((ticket / nct) % np), jt = (int)(ticket % nct);
     const int cell = pd.pos_cell[pos];
     const int row0 = part * a.mw;                                        // first output node of this tile
@@ -540,25 +522,13 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<S> a, P
     __syncthreads();
 
     const int npanel = kt / kP2PanelK;
-#ifdef CHFSI_TRACE
-    long long* tr_p = tr;
-    if (tr) tr[4] = 0;
-#endif
-    TRACE_STAMP(1);
     // Producer duty rotates over the 8 warps (panel j is issued by lane 0 of warp j % 8, kP2Ahead iterations ahead):
     // wait for the ring slot, then one expect_tx, one bulk copy (matrix panel) and two TMA row gathers (X or P rows).
     auto produce = [&](int pj) {
       if (lane != 0) return;
       const uint32_t q = q0 + (uint32_t)pj;
       const int s = (int)(q % kP2Stages);
-#ifdef CHFSI_TRACE
-      long long te0 = clock64();
-#endif
       mbar_wait(&empty[s], ((q / kP2Stages) & 1u) ^ 1u);
-#ifdef CHFSI_TRACE
-      long long te1 = clock64();
-      if (tr_p) tr_p[4] += te1 - te0;
-#endif
       S* As = stage0 + s * stage_elems;
       S* Xs = As + a_panel_elems;
       const uint32_t a_bytes = (uint32_t)a_panel_elems * (uint32_t)sizeof(S);
@@ -570,9 +540,6 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<S> a, P
                   idx_s[k0 + 3] & 0x7fffffff, &full[s]);
       tma_gather4(Xs + 4 * kP2LdXs, tm, col0, idx_s[k0 + 4] & 0x7fffffff, idx_s[k0 + 5] & 0x7fffffff,
                   idx_s[k0 + 6] & 0x7fffffff, idx_s[k0 + 7] & 0x7fffffff, &full[s]);
-#ifdef CHFSI_TRACE
-      if (tr_p) tr_p[8] += clock64() - te1;
-#endif
     };
     if (warp < kP2Ahead && warp < npanel) produce(warp);
 
@@ -608,20 +575,11 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<S> a, P
     for (int pi = 0; pi < npanel; ++pi) {
       const uint32_t q = q0 + (uint32_t)pi;
       const int s = (int)(q % kP2Stages);
-#ifdef CHFSI_TRACE
-      long long tw0 = tr ? clock64() : 0;
-#endif
       {
         const int pj = pi + kP2Ahead;
         if (pj < npanel && (pj & 7) == warp) produce(pj);
       }
-#ifdef CHFSI_TRACE
-      long long tw1 = tr ? clock64() : 0;
-#endif
       mbar_wait(&full[s], (q / kP2Stages) & 1u);
-#ifdef CHFSI_TRACE
-      if (tr) { long long tw2 = clock64(); if (pi == 0) tr[2] = tw2; else { tr[6] += tw2 - tw1; } tr[7] += tw1 - tw0; }
-#endif
       if (active) {
         const S* As = stage0 + s * stage_elems;
         const S* Ap = As + fk * lda + mt0 * 8 + fm;
@@ -656,15 +614,9 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<S> a, P
       if (lane == 0) mbar_arrive(&empty[s]);
     }
     q0 += (uint32_t)npanel;
-    TRACE_STAMP(3);
 
     // ---- epilogue: assembly + recurrence (steps 4-5).  C fragment: row = lane/4, columns 2*(lane%4) + {0,1}
-#ifdef CHFSI_TRACE
-    const bool skip_epi = (pd.debug_flags & 1) != 0;
-#else
-    constexpr bool skip_epi = false;
-#endif
-    if (!a.atomic && !skip_epi) {
+    if (!a.atomic) {
       const int d0 = pd.dep_ptr[pos], nd = (pd.dep_ptr[pos + 1] - d0) * np;   // every block of every earlier neighbour
       for (int d = lane; d < nd; d += 32) {
         const uint32_t* f = pd.flags + ((int64_t)pd.dep_pos[d0 + d / np] * np + d % np) * nct + jt;
@@ -672,8 +624,7 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<S> a, P
       }
       __syncwarp();
     }
-    TRACE_STAMP(12);
-    if (active && !skip_epi) {
+    if (active) {
       // first contribution to a dof: plain store of alpha acc (the -beta Y_{k-2} term is already in acc); later
       // contributions: red.global.add.f64 (fire and forget); their order is fixed by the completion flags.
 #pragma unroll
@@ -696,10 +647,8 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<S> a, P
         }
       }
     }
-    TRACE_STAMP(13);
     __threadfence();
     __syncthreads();   // all stores of the tile are done and fenced; idx_s / ticket slot may be reused
-    TRACE_STAMP(14);
     if (tid == 0 && !a.atomic) st_release_gpu(pd.flags + ((int64_t)pos * np + part) * nct + jt, pd.epoch);
   }
 }
@@ -811,9 +760,6 @@ bool make_row_gather_map(CUtensorMap* tm, const void* base, int64_t rows, int64_
 }
 
 
-#ifdef CHFSI_TRACE
-long long* g_trace_buffer = nullptr;
-#endif
 
 template <typename S>
 size_t p2_smem_bytes(const Op* op) {
@@ -847,6 +793,8 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
     k_set_diag_shift<T><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(reinterpret_cast<T*>(op->mat), op->mat_off, op->idx_off,
                                                                     op->gidx, op->ktot, op->diag0, op->m_cell, op->lda, op->mw,
                                                                     op->n_cells, g.cshift);
+    const cudaError_t se = cudaGetLastError();
+    if (se != cudaSuccess) return se;           // cur_shift keeps describing what the matrices actually hold
     op->cur_shift = g.cshift;
     op->launches++;
   }
@@ -926,9 +874,6 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
       const unsigned grid = (unsigned)std::min<int64_t>(n_tiles, 2 * (int64_t)op->n_sm);
       pd.n_tiles = (int)n_tiles;
       pd.ticket_base = (unsigned long long)(g.epoch - 1) * (unsigned long long)(n_tiles + grid);
-#ifdef CHFSI_TRACE
-      pd.trace = nullptr; pd.debug_flags = 0;
-#endif
       const size_t sm = t3_smem_bytes(op);
       switch (MT16) {
         case 11: k_apply_tf32_p<11><<<grid, kP2Threads, sm, st>>>(a, pd, tmX, tmP); break;
@@ -951,15 +896,8 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
       pd.epoch = g.epoch;
       const int64_t n_tiles = op->n_cells * op->n_parts * a.n_col_tiles;
       unsigned grid = (unsigned)std::min<int64_t>(n_tiles, 2 * (int64_t)op->n_sm);
-#ifdef CHFSI_TRACE
-      if (const char* eg = getenv("CHFSI_DEBUG_GRID")) grid = (unsigned)std::min<int64_t>(n_tiles, atoi(eg));
-#endif
       pd.n_tiles = (int)n_tiles;
       pd.ticket_base = (unsigned long long)(g.epoch - 1) * (unsigned long long)(n_tiles + grid);
-#ifdef CHFSI_TRACE
-      pd.trace = g_trace_buffer;
-      pd.debug_flags = getenv("CHFSI_DEBUG_FLAGS") ? atoi(getenv("CHFSI_DEBUG_FLAGS")) : 0;
-#endif
       const size_t sm = p2_smem_bytes<T>(op);
       switch (MT) {
         case 11: k_apply_dmma_p<11, T><<<grid, kP2Threads, sm, st>>>(a, pd, tmX, tmP); break;
@@ -1007,6 +945,7 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
 
 cudaError_t init_apply_kernels(Op* op) {
   cudaError_t e;
+  if ((e = init_rr_kernels())) return e;
   size_t smem_fast = (size_t)kStages * (kPanelK * op->lda + kPanelK * kLdXs) * sizeof(double) + kStages * sizeof(uint64_t) +
                      (size_t)op->max_ktot * sizeof(int32_t);
   if (smem_fast <= 227 * 1024) {
@@ -1053,9 +992,6 @@ cudaError_t init_apply_kernels(Op* op) {
   return cudaSuccess;
 }
 
-#ifdef CHFSI_TRACE
-extern "C" void chfsi_debug_set_trace(long long* dev_buffer) { g_trace_buffer = dev_buffer; }
-#endif
 
 cudaError_t assemble_projector_rows(Op* op, const HostPlan& plan, const chfsi_mesh& mesh, cudaStream_t st) {
   op->n_pseg = 0; op->n_prow = (int64_t)plan.grow_dof.size();

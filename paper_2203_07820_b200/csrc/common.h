@@ -142,6 +142,10 @@ struct Op {
   size_t host_ws_bytes = 0;
   cudaStream_t host_st[2] = {nullptr, nullptr};
   cudaEvent_t host_done[2] = {nullptr, nullptr};
+  // cross-stream ordering of the calls on this handle (api.cu order_enter / order_leave)
+  cudaEvent_t order_ev = nullptr;
+  cudaStream_t order_stream = nullptr;
+  bool order_valid = false;
   int64_t launches = 0;
   // optional per-kernel timing (chfsi_set_profiling): event triples (start, after projector kernels, end)
   bool profiling = false;
@@ -189,7 +193,9 @@ cudaError_t launch_xty(Op* op, const double* A, int64_t lda, const double* B, in
 // Out[n_rows][ldo] = Y Z, Y [n_rows][ldy] with N columns, Z [N][ldz] with N2 columns (Alg. 2 step 3)
 cudaError_t launch_xz(Op* op, const double* Y, int64_t ldy, const double* Z, int64_t ldz, int64_t n_rows, int N, int N2,
                       double* Out, int64_t ldo, cudaStream_t stream);
-// Opts the kernels into the shared memory they need for this operator (once, at create).
+// Opts the kernels into the shared memory they need for this operator, on the CURRENT device (at every create: the
+// attribute is per device).
 cudaError_t init_apply_kernels(Op* op);
+cudaError_t init_rr_kernels();
 
 }  // namespace chfsi

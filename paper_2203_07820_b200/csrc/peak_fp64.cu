@@ -56,8 +56,12 @@ extern "C" int chfsi_measure_fp64_peak(double* dmma_tflops, double* dfma_tflops,
   const int threads = 512, grid = sms * 2, iters = 8192;
   double* out = nullptr;
   if (cudaMalloc((void**)&out, (size_t)grid * threads * sizeof(double)) != cudaSuccess) return CHFSI_ERR_OUT_OF_MEMORY;
-  cudaEvent_t e0, e1;
-  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) {
+    if (e0) cudaEventDestroy(e0);
+    cudaFree(out);
+    return CHFSI_ERR_CUDA;
+  }
   double best[2] = {0.0, 0.0};
   for (int which = 0; which < 2; ++which) {
     for (int rep = 0; rep < 6; ++rep) {   // rep 0 is the warm-up
@@ -65,7 +69,7 @@ extern "C" int chfsi_measure_fp64_peak(double* dmma_tflops, double* dfma_tflops,
       if (which == 0) k_peak_dmma<<<grid, threads, 0, st>>>(out, iters, 1.0, 1e-3);
       else k_peak_dfma<<<grid, threads, 0, st>>>(out, iters * 8, 1.0000001, 1e-3);
       cudaEventRecord(e1, st);
-      if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(out); return CHFSI_ERR_CUDA; }
+      if (cudaEventSynchronize(e1) != cudaSuccess) { cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(out); return CHFSI_ERR_CUDA; }
       float ms = 0.f;
       cudaEventElapsedTime(&ms, e0, e1);
       const double flops = which == 0 ? (double)grid * (threads / 32) * iters * kAcc * 512.0

@@ -195,17 +195,22 @@ __global__ void __launch_bounds__(256, 2) k_xz(const double* __restrict__ Y, int
   }
 }
 
+constexpr size_t xz_smem_bytes() { return (size_t)2 * (kXzM * kXzLdA + kXzK * kXzLdB) * sizeof(double); }
+constexpr size_t xty_smem_bytes() { return (size_t)kXtStages * (kXtK * kXtLdA + kXtK * kXtLdB) * sizeof(double); }
+
 }  // namespace
+
+// Shared-memory opt-in of the Rayleigh-Ritz kernels: a per-DEVICE attribute, so it is set for the current device at
+// every operator creation (init_apply_kernels), not once per process.
+cudaError_t init_rr_kernels() {
+  cudaError_t e = cudaFuncSetAttribute(k_xz, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)xz_smem_bytes());
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(k_xty, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)xty_smem_bytes());
+}
 
 cudaError_t launch_xz(Op* op, const double* Y, int64_t ldy, const double* Z, int64_t ldz, int64_t n_rows, int N, int N2,
                       double* Out, int64_t ldo, cudaStream_t st) {
-  const size_t smem = (size_t)2 * (kXzM * kXzLdA + kXzK * kXzLdB) * sizeof(double);
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(k_xz, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+  const size_t smem = xz_smem_bytes();
   dim3 grid((unsigned)((N2 + kXzN - 1) / kXzN), (unsigned)((n_rows + kXzM - 1) / kXzM));
   k_xz<<<grid, 256, smem, st>>>(Y, ldy, Z, ldz, n_rows, N, N2, Out, ldo);
   op->launches++;
@@ -238,13 +243,7 @@ cudaError_t launch_xty(Op* op, const double* A, int64_t lda, const double* B, in
     if ((e = cudaMalloc(&op->rr_scratch, need)) != cudaSuccess) return e;
     op->rr_scratch_bytes = need;
   }
-  const size_t smem = (size_t)kXtStages * (kXtK * kXtLdA + kXtK * kXtLdB) * sizeof(double);
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(k_xty, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+  const size_t smem = xty_smem_bytes();
   dim3 grid((unsigned)ti, (unsigned)tj, (unsigned)n_split);
   k_xty<<<grid, 256, smem, st>>>(A, lda, B, ldb, n_rows, N1, N2, rows_per_split, reinterpret_cast<double*>(op->rr_scratch));
   k_xty_reduce<<<(unsigned)(((int64_t)N1 * N2 + 255) / 256), 256, 0, st>>>(reinterpret_cast<const double*>(op->rr_scratch), n_split,
