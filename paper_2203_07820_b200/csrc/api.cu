@@ -50,7 +50,7 @@ void free_op(chfsi_op* op) {
   cudaFree(op->color_cells); cudaFree(op->dep_ptr); cudaFree(op->dep_pos); cudaFree(op->all_cells); cudaFree(op->pc_cells); cudaFree(op->cell_proj_ptr);
   cudaFree(op->proj_ptr); cudaFree(op->proj_pcrow); cudaFree(op->seg_ptr); cudaFree(op->grow_dof); cudaFree(op->pcoef);
   cudaFree(op->grp_seg_ptr); cudaFree(op->proj_grp); cudaFree(op->proj_slot);
-  cudaFree(op->rr_scratch);
+  cudaFree(op->rr_scratch); cudaFree(op->sf_coef); cudaFree(op->sf_sloc); cudaFree(op->crows);
   for (int i = 0; i < 2; ++i) {
     cudaFree(op->host_stage[i]);
     if (op->host_done[i]) cudaEventDestroy(op->host_done[i]);
@@ -76,7 +76,8 @@ WsLayout ws_layout(const Op* op, int64_t B) {
   w.pc_off = w.p_off + align_up((size_t)(op->n_proj + 1) * B * w.elt, 256);
   w.sync_off = w.pc_off + align_up((size_t)(op->n_pseg > 0 ? op->n_pseg : 1) * kProjGroup * B * sizeof(double), 256);
   // ticket counter (first 128 bytes) + one completion flag per (cell, 32-column tile): apply_kernels.cu, v2 kernel
-  w.sync_bytes = align_up(128 + (size_t)op->n_cells * op->n_parts * (size_t)((B + 31) / 32) * sizeof(uint32_t), 256);
+  // (16-column tiles in the sum-factorised FP64 kernel)
+  w.sync_bytes = align_up(128 + (size_t)op->n_cells * op->n_parts * (size_t)((B + 15) / 16) * sizeof(uint32_t), 256);
   w.total = w.sync_off + w.sync_bytes;
   return w;
 }
@@ -258,6 +259,8 @@ int chfsi_create(chfsi_op** out, const chfsi_mesh* mesh, const chfsi_potential* 
   CKC(cudaMalloc((void**)&op->diag0, (size_t)op->n_cells * op->m_cell * sizeof(double)), "cudaMalloc(diagonal)");
   CKC(capture_diagonal(op, st), "diagonal capture");
   CKC(init_apply_kernels(op), "kernel attribute setup");
+  CKC(init_sf_variant(op, tab, st), "sum-factorised variant setup");
+  if (op->sf_ok) CKC(build_sf_fields(op, pot->veff_q, st), "quadrature-point fields");
   CKC(cudaStreamSynchronize(st), "sync");
 #undef CKC
   } catch (const std::bad_alloc&) {
@@ -285,6 +288,11 @@ int chfsi_update_potential(chfsi_op* op, const chfsi_potential* pot, void* cuda_
   cudaError_t ce = order_enter(op, st);
   if (ce == cudaSuccess) ce = rebuild_local_matrices(op, pot->veff_q, st);
   if (ce != cudaSuccess) return cuda_fail(op, ce, "update_potential (cell matrices)");
+  if (op->sf_ok) {
+    ce = build_sf_fields(op, pot->veff_q, st);
+    if (ce != cudaSuccess) return cuda_fail(op, ce, "update_potential (quadrature-point fields)");
+    op->launches++;
+  }
   ce = capture_diagonal(op, st);      // new unshifted diagonals; the spectral shift of the last filter is gone
   if (ce == cudaSuccess) ce = cudaStreamSynchronize(st);
   if (ce != cudaSuccess) return cuda_fail(op, ce, "update_potential (diagonal)");
@@ -544,7 +552,7 @@ int64_t chfsi_launch_count(const chfsi_op* op) { return op ? op->launches : -1; 
 
 int chfsi_set_kernel_variant(chfsi_op* op, int variant) {
   if (!op) return CHFSI_ERR_BAD_ARGUMENT;
-  if (variant < 0 || variant > 3) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "variant must be 0, 1, 2 or 3");
+  if (variant < 0 || variant > 5) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "variant must be 0 .. 5");
   op->variant = variant;
   return CHFSI_OK;
 }

@@ -730,6 +730,7 @@ __global__ void __launch_bounds__(256, 2) k_proj_rows_tma(const int32_t* __restr
 }
 
 #include "apply_tf32.cuh"
+#include "apply_sf.cuh"
 
 // Tensor map of a row-major FP64 / FP32 block [rows][ld] restricted to its first `cols` columns, box = box_cols x 1
 // (tile::gather4 picks four such rows per instruction); columns beyond `cols` read as zero.
@@ -747,7 +748,8 @@ EncodeTiledFn encode_tiled_fn() {
   }();
   return fn;
 }
-bool make_row_gather_map(CUtensorMap* tm, const void* base, int64_t rows, int64_t cols, int64_t ld, int elt, int box_cols) {
+bool make_row_gather_map(CUtensorMap* tm, const void* base, int64_t rows, int64_t cols, int64_t ld, int elt, int box_cols,
+                         bool swizzle128 = false) {
   EncodeTiledFn enc = encode_tiled_fn();
   if (!enc || rows < 1 || cols < 1 || (ld * elt) % 16 != 0 || (uintptr_t)base % 16 != 0) return false;
   const cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
@@ -755,7 +757,8 @@ bool make_row_gather_map(CUtensorMap* tm, const void* base, int64_t rows, int64_
   const cuuint32_t box[2] = {(cuuint32_t)box_cols, 1};
   const cuuint32_t estr[2] = {1, 1};
   return enc(tm, elt == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<void*>(base), dims, strides, box, estr,
-             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+             CU_TENSOR_MAP_INTERLEAVE_NONE, swizzle128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
+             CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
@@ -788,7 +791,15 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
     op->prof_used += 3;
     cudaEventRecord(ev[0], st);
   }
-  if (g.cshift != op->cur_shift) {   // once per filter call: move the spectral shift onto the matrix diagonals
+  // row segments of a chunk start 16-byte aligned (TMA, vector loads / stores of the fragments)
+  constexpr int kPer16 = 16 / (int)sizeof(T);
+  const bool aligned = B % kPer16 == 0 && g.ldx % kPer16 == 0 && g.ldt % kPer16 == 0 && ((uintptr_t)g.X % 16 == 0) &&
+                       ((uintptr_t)g.T % 16 == 0) && ((uintptr_t)g.P % 16 == 0) && op->max_ktot <= kMaxKtot;
+  // variant 0 (automatic) / 5: the sum-factorised kernel (apply_sf.cuh) when the operator qualifies
+  CUtensorMap tmX, tmP;
+  const bool use_sf = op->sf_ok && aligned && (op->variant == 0 || op->variant == 5) && g.sync != nullptr && g.epoch > 0 &&
+                      make_row_gather_map(&tmX, g.X, op->n_dofs, B, g.ldx, (int)sizeof(T), sf_tile_cols<T>(), true);
+  if (!use_sf && g.cshift != op->cur_shift) {   // once per filter call: move the spectral shift onto the matrix diagonals
     const int64_t n = op->n_cells * op->m_cell;
     k_set_diag_shift<T><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(reinterpret_cast<T*>(op->mat), op->mat_off, op->idx_off,
                                                                     op->gidx, op->ktot, op->diag0, op->m_cell, op->lda, op->mw,
@@ -825,29 +836,25 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
   a.alpha = (T)g.alpha; a.beta = (T)g.beta;
   a.atomic = op->assembly;
 
-  // row segments of a chunk start 16-byte aligned (TMA, vector loads / stores of the fragments)
-  constexpr int kPer16 = 16 / (int)sizeof(T);
-  const bool aligned = B % kPer16 == 0 && g.ldx % kPer16 == 0 && g.ldt % kPer16 == 0 && ((uintptr_t)g.X % 16 == 0) &&
-                       ((uintptr_t)g.T % 16 == 0) && ((uintptr_t)g.P % 16 == 0) && op->max_ktot <= kMaxKtot;
-  // variant 0: persistent single-launch kernel (v2); variant 2: one launch per colour (v1); variant 1: generic
+  // variant 4 (and 0 when the sum-factorised kernel does not apply): persistent single-launch dense kernel;
+  // variant 2: one launch per colour; variant 1: generic
   bool fast2 = false, fast = false;
   int MT = (op->mw / 8 + 3) / 4;   // 8-row tiles per warp row: 11 (p=6), 8 (p=7, 8), 7, 4, 2, 1
   // variant 0: persistent single-launch kernel, FP64 DMMA accumulation for both storage types;
   // variant 3 (FP32 storage only, opt-in): persistent kernel with 3xTF32 products on the 32-bit tensor pipe -- 1.3x
   // faster, but the FP32 tensor accumulator truncates: |dY|/|Y| ~ 2e-6 per apply, Ritz values off by up to 4e-5 Ha,
   // i.e. inside the 1e-4 block tolerance but outside the 1e-5 Ha eigenvalue tolerance of the FP32 variant
-  CUtensorMap tmX, tmP;
   bool fast3 = false;   // 3xTF32 kernel
   const int MT16 = ((op->m_cell + 15) / 16 + 1) / 2;
   if (sizeof(T) == 4 && aligned && B % 8 == 0 && op->variant == 3 && op->n_parts == 1 && g.sync != nullptr && g.epoch > 0)
     fast3 = (MT16 == 11 || MT16 == 7 || MT16 == 4 || MT16 == 2 || MT16 == 1) && t3_smem_bytes(op) <= 113 * 1024 &&
             make_row_gather_map(&tmX, g.X, op->n_dofs, B, g.ldx, 4, kT3TileN) &&
             make_row_gather_map(&tmP, g.P, op->n_proj + 1, B, B, 4, kT3TileN);
-  if (aligned && !fast3 && op->variant == 0 && g.sync != nullptr && g.epoch > 0)
+  if (aligned && !fast3 && !use_sf && (op->variant == 0 || op->variant == 4 || op->variant == 5) && g.sync != nullptr && g.epoch > 0)
     fast2 = (MT == 11 || MT == 8 || MT == 7 || MT == 4 || MT == 2 || MT == 1) && p2_smem_bytes<T>(op) <= 113 * 1024 &&
             make_row_gather_map(&tmX, g.X, op->n_dofs, B, g.ldx, (int)sizeof(T), kP2TileN) &&
             make_row_gather_map(&tmP, g.P, op->n_proj + 1, B, B, (int)sizeof(T), kP2TileN);
-  if (sizeof(T) == 8 && aligned && B % 8 == 0 && !fast2 && op->variant != 1 && op->n_parts == 1) fast = (MT == 11 || MT == 4 || MT == 2 || MT == 7);
+  if (sizeof(T) == 8 && aligned && B % 8 == 0 && !fast2 && !use_sf && op->variant != 1 && op->n_parts == 1) fast = (MT == 11 || MT == 4 || MT == 2 || MT == 7);
   size_t smem_fast = (size_t)kStages * (kPanelK * op->lda + kPanelK * kLdXs) * sizeof(double) + kStages * sizeof(uint64_t) +
                      (size_t)op->max_ktot * sizeof(int32_t);
   if (fast && smem_fast > 227 * 1024) fast = false;
@@ -861,6 +868,31 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
     op->prof_proj_launches += op->launches - launches_before;
   }
   const int64_t launches_mid = op->launches;
+  if (use_sf) {
+    a.cells = nullptr; a.n_launch_cells = (int)op->n_cells;
+    a.n_col_tiles = (B + sf_tile_cols<T>() - 1) / sf_tile_cols<T>();
+    PersistDev pd;
+    pd.pos_cell = op->color_cells; pd.dep_ptr = op->dep_ptr; pd.dep_pos = op->dep_pos;
+    pd.counter = g.sync;
+    pd.flags = reinterpret_cast<uint32_t*>(g.sync) + kSyncFlagOffset;
+    pd.epoch = g.epoch;
+    const int64_t n_tiles = op->n_cells * a.n_col_tiles;
+    const unsigned grid = (unsigned)std::min<int64_t>(n_tiles, 2 * (int64_t)op->n_sm);
+    pd.n_tiles = (int)n_tiles;
+    pd.ticket_base = (unsigned long long)(g.epoch - 1) * (unsigned long long)(n_tiles + grid);
+    SfDev sf;
+    sf.coef = op->sf_coef; sf.sloc = op->sf_sloc; sf.crows = op->crows; sf.cell_proj_ptr = op->cell_proj_ptr;
+    sf.cshift = g.cshift;
+    switch (op->p) {
+      case 1: k_apply_sf<1, T><<<grid, kSfThreads, sf_smem_bytes<1, T>(op), st>>>(a, sf, pd, tmX); break;
+      case 2: k_apply_sf<2, T><<<grid, kSfThreads, sf_smem_bytes<2, T>(op), st>>>(a, sf, pd, tmX); break;
+      case 3: k_apply_sf<3, T><<<grid, kSfThreads, sf_smem_bytes<3, T>(op), st>>>(a, sf, pd, tmX); break;
+      case 4: k_apply_sf<4, T><<<grid, kSfThreads, sf_smem_bytes<4, T>(op), st>>>(a, sf, pd, tmX); break;
+      case 5: k_apply_sf<5, T><<<grid, kSfThreads, sf_smem_bytes<5, T>(op), st>>>(a, sf, pd, tmX); break;
+      case 6: k_apply_sf<6, T><<<grid, kSfThreads, sf_smem_bytes<6, T>(op), st>>>(a, sf, pd, tmX); break;
+    }
+    op->launches++;
+  }
   if (fast3) {
     if constexpr (sizeof(T) == 4) {
       a.cells = nullptr; a.n_launch_cells = (int)op->n_cells;
@@ -910,7 +942,7 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
       op->launches++;
     }
   }
-  const int n_launch = (fast2 || fast3) ? 0 : (op->assembly == 1 ? 1 : op->n_colors);
+  const int n_launch = (fast2 || fast3 || use_sf) ? 0 : (op->assembly == 1 ? 1 : op->n_colors);
   for (int c = 0; c < n_launch; ++c) {
     if (op->assembly == 1) { a.cells = op->all_cells; a.n_launch_cells = (int)op->n_cells; }
     else { a.cells = op->color_cells + op->color_ptr[c]; a.n_launch_cells = op->color_ptr[c + 1] - op->color_ptr[c]; }
@@ -993,6 +1025,71 @@ cudaError_t init_apply_kernels(Op* op) {
 }
 
 
+namespace {
+__global__ void __launch_bounds__(256) k_sf_sloc(const int32_t* __restrict__ gidx, const int64_t* __restrict__ idx_off,
+                                                 const double* __restrict__ mass, int m_cell, int mpad, int64_t n_cells,
+                                                 double* __restrict__ sloc) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n_cells * mpad) return;
+  const int64_t c = i / mpad;
+  const int l = (int)(i - c * mpad);
+  sloc[i] = l < m_cell ? 1.0 / sqrt(mass[gidx[idx_off[c] + l] & 0x7fffffff]) : 0.0;
+}
+template <int P>
+cudaError_t sf_set_attr(Op* op) {
+  cudaError_t e;
+  if ((e = cudaFuncSetAttribute(k_apply_sf<P, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sf_smem_bytes<P, double>(op)))) return e;
+  return cudaFuncSetAttribute(k_apply_sf<P, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sf_smem_bytes<P, float>(op));
+}
+}  // namespace
+
+cudaError_t init_sf_variant(Op* op, const Tables1D& tab, cudaStream_t st) {
+  op->sf_ok = false;
+  if (op->p > 6 || op->max_ktot - op->mpad > kSfMaxProj) return cudaSuccess;
+  const int n1 = tab.n1, nq1 = tab.nq1;
+  // Phi[q][i] = l_i(x_q): the Lagrange (GLL) basis at the Gauss points; Dh[q'][q] = derivative of the Lagrange polynomial
+  // through the GAUSS points at Gauss point q' (barycentric form, long double), both zero-padded to 8 x 8
+  double phi[64], dh[64];
+  for (int i = 0; i < 64; ++i) phi[i] = dh[i] = 0.0;
+  for (int q = 0; q < nq1; ++q)
+    for (int i = 0; i < n1; ++i) phi[q * 8 + i] = tab.phi[(size_t)q * n1 + i];
+  long double lam[8];
+  for (int j = 0; j < nq1; ++j) {
+    lam[j] = 1.0L;
+    for (int k = 0; k < nq1; ++k)
+      if (k != j) lam[j] /= ((long double)tab.gq_x[j] - (long double)tab.gq_x[k]);
+  }
+  for (int i = 0; i < nq1; ++i) {
+    long double diag = 0.0L;
+    for (int j = 0; j < nq1; ++j) {
+      if (j == i) continue;
+      const long double v = (lam[j] / lam[i]) / ((long double)tab.gq_x[i] - (long double)tab.gq_x[j]);
+      dh[i * 8 + j] = (double)v;
+      diag -= v;
+    }
+    dh[i * 8 + i] = (double)diag;
+  }
+  cudaError_t e;
+  if ((e = cudaMemcpyToSymbolAsync(c_sf_phi, phi, sizeof(phi), (size_t)op->p * sizeof(phi), cudaMemcpyHostToDevice, st))) return e;
+  if ((e = cudaMemcpyToSymbolAsync(c_sf_dhat, dh, sizeof(dh), (size_t)op->p * sizeof(dh), cudaMemcpyHostToDevice, st))) return e;
+  if ((e = cudaStreamSynchronize(st))) return e;       // phi / dh live on this stack frame
+  const int64_t n = op->n_cells * op->mpad;
+  if ((e = cudaMalloc((void**)&op->sf_sloc, (size_t)n * sizeof(double)))) return e;
+  k_sf_sloc<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(op->gidx, op->idx_off, op->mass, op->m_cell, op->mpad, op->n_cells, op->sf_sloc);
+  if ((e = cudaGetLastError())) return e;
+  switch (op->p) {
+    case 1: e = sf_set_attr<1>(op); break;
+    case 2: e = sf_set_attr<2>(op); break;
+    case 3: e = sf_set_attr<3>(op); break;
+    case 4: e = sf_set_attr<4>(op); break;
+    case 5: e = sf_set_attr<5>(op); break;
+    case 6: e = sf_set_attr<6>(op); break;
+  }
+  if (e != cudaSuccess) return e;
+  op->sf_ok = true;
+  return cudaSuccess;
+}
+
 cudaError_t assemble_projector_rows(Op* op, const HostPlan& plan, const chfsi_mesh& mesh, cudaStream_t st) {
   op->n_pseg = 0; op->n_prow = (int64_t)plan.grow_dof.size();
   const size_t elt = op->precision == 64 ? 8 : 4;
@@ -1006,6 +1103,7 @@ cudaError_t assemble_projector_rows(Op* op, const HostPlan& plan, const chfsi_me
   int32_t* d_row_cell = nullptr; double* d_rows = nullptr;
   if ((e = cudaMalloc((void**)&d_row_cell, row_cell.size() * sizeof(int32_t)))) return e;
   if ((e = cudaMalloc((void**)&d_rows, (size_t)op->nnz_cp * mc * sizeof(double)))) { cudaFree(d_row_cell); return e; }
+  op->crows = d_rows;   // kept: the sum-factorised kernel applies C~^c P from these rows (freed with the operator)
   std::vector<double> rows((size_t)op->nnz_cp * mc);
   e = cudaMemcpyAsync(d_row_cell, row_cell.data(), row_cell.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st);
   if (e == cudaSuccess) {
@@ -1019,7 +1117,7 @@ cudaError_t assemble_projector_rows(Op* op, const HostPlan& plan, const chfsi_me
   }
   if (e == cudaSuccess) e = cudaMemcpyAsync(rows.data(), d_rows, rows.size() * sizeof(double), cudaMemcpyDeviceToHost, st);
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-  cudaFree(d_row_cell); cudaFree(d_rows);
+  cudaFree(d_row_cell);
   if (e != cudaSuccess) return e;
   // 2. assembly over the cells of each projector, in the caller's CSR order (deterministic)
   std::vector<double> coef((size_t)op->n_prow * kProjGroup, 0.0);

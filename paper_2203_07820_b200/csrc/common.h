@@ -126,6 +126,13 @@ struct Op {
   // "c1 H~ + c2") and the recurrence epilogue never re-reads X.
   double* diag0 = nullptr;
   double cur_shift = 0.0;
+  // sum-factorised variant (apply_sf.cuh; FE degree <= 6): quadrature-point fields W0 = w detJ V_eff and
+  // G = 1/2 w detJ J^-1 J^-T in the kernel's lane order [n_cells][nq1][7][32][2], M^-1/2 per (cell, node)
+  // [n_cells][mpad], and the projector columns s_l C^c_{l,j} as compact FP64 rows [nnz_cp][m_cell]
+  bool sf_ok = false;
+  double* sf_coef = nullptr;
+  double* sf_sloc = nullptr;
+  double* crows = nullptr;
   // kept from create for chfsi_update_potential: cell vertices and the 1-D tables of the setup kernels
   double* setup_verts = nullptr;         // [n_cells][24]
   double* setup_pp = nullptr;            // [4][nq1][n1*n1]
@@ -165,6 +172,9 @@ cudaError_t build_cell_matrices(Op* op, const HostPlan& plan, const Tables1D& ta
 // Recomputes the Hamiltonian rows (rows 0..M_cell-1) of every cell matrix for a new V_eff (HOST pointer
 // [n_cells][(p+2)^3]); projector rows, layout and colouring are untouched.  Synchronises the stream.
 cudaError_t rebuild_local_matrices(Op* op, const double* veff_q_host, cudaStream_t stream);
+// Quadrature-point fields of the sum-factorised variant (op->sf_coef, allocated on first use) from V_eff at the Gauss
+// points (HOST pointer) and the cell geometry; op->setup_* must exist.  Synchronises the stream.
+cudaError_t build_sf_fields(Op* op, const double* veff_q_host, cudaStream_t stream);
 
 // ---- apply kernels (apply_kernels.cu) ----------------------------------------------------------------------
 struct ApplyArgs {
@@ -197,5 +207,8 @@ cudaError_t launch_xz(Op* op, const double* Y, int64_t ldy, const double* Z, int
 // attribute is per device).
 cudaError_t init_apply_kernels(Op* op);
 cudaError_t init_rr_kernels();
+// Sum-factorised variant: uploads the 1-D tables of degree tab.p to constant memory of the current device and fills
+// op->sf_sloc; sets op->sf_ok when the operator qualifies (p <= 6, at most kSfMaxProj projectors per cell).
+cudaError_t init_sf_variant(Op* op, const Tables1D& tab, cudaStream_t stream);
 
 }  // namespace chfsi

@@ -217,6 +217,29 @@ __global__ void __launch_bounds__(256) k_cell_projector(int n1, int nq1, SetupTa
   }
 }
 
+// Fields of the sum-factorised apply at the Gauss points of every cell, in the lane order of k_apply_sf:
+//   coef[c][qc][k][lane = 4 qa + qb/2][e = qb % 2],  k = 0: w detJ V_eff;  k = 1..6: 1/2 w detJ (J^-1 J^-T)_{xx,xy,xz,yy,yz,zz}
+// (the integrands of Eq. 40 / Eq. 30 term 1, before the shape functions are applied).
+__global__ void __launch_bounds__(256) k_sf_fields(int nq1, int64_t n_cells, SetupTables tb, const double* __restrict__ verts,
+                                                   const double* __restrict__ veff, double* __restrict__ coef) {
+  __shared__ double vt[24];
+  const int64_t c = blockIdx.x;
+  const int nq2 = nq1 * nq1, nq = nq1 * nq2;
+  if (threadIdx.x < 24) vt[threadIdx.x] = verts[c * 24 + threadIdx.x];
+  __syncthreads();
+  double* out = coef + c * (int64_t)nq1 * 7 * 64;
+  for (int q = threadIdx.x; q < nq; q += blockDim.x) {
+    const int qa = q % nq1, qb = (q / nq1) % nq1, qc = q / nq2;
+    const Geom g = trilinear_geom(vt, tb.gq_x[qa], tb.gq_x[qb], tb.gq_x[qc]);
+    const double wj = tb.gq_w[qa] * tb.gq_w[qb] * tb.gq_w[qc] * g.detJ;
+    const int slot = (4 * qa + (qb >> 1)) * 2 + (qb & 1);
+    double* o = out + (int64_t)qc * 7 * 64 + slot;
+    o[0] = wj * veff[c * nq + q];
+    o[64] = 0.5 * wj * g.G[0][0]; o[128] = 0.5 * wj * g.G[0][1]; o[192] = 0.5 * wj * g.G[0][2];
+    o[256] = 0.5 * wj * g.G[1][1]; o[320] = 0.5 * wj * g.G[1][2]; o[384] = 0.5 * wj * g.G[2][2];
+  }
+}
+
 template <typename U>
 cudaError_t upload(U** dst, const U* src, size_t n, cudaStream_t st) {
   *dst = nullptr;
@@ -268,6 +291,27 @@ done:
   return err;
 }
 }  // namespace
+
+cudaError_t build_sf_fields(Op* op, const double* veff_q_host, cudaStream_t stream) {
+  cudaError_t err = cudaSuccess;
+  const int nq1 = op->nq1;
+  const size_t elems = (size_t)op->n_cells * nq1 * 7 * 64;
+  double* d_veff = nullptr;
+  if (!op->sf_coef) {
+    CK(cudaMalloc((void**)&op->sf_coef, elems * sizeof(double)));
+    CK(cudaMemsetAsync(op->sf_coef, 0, elems * sizeof(double), stream));   // lanes beyond the Gauss grid (p < 6) stay zero
+  }
+  CK(upload(&d_veff, veff_q_host, (size_t)op->n_cells * op->n_q, stream));
+  {
+    SetupTables tb{op->setup_pp, op->setup_phi, op->setup_gx, op->setup_gw};
+    k_sf_fields<<<(unsigned)op->n_cells, 256, 0, stream>>>(nq1, op->n_cells, tb, op->setup_verts, d_veff, op->sf_coef);
+    CK(cudaGetLastError());
+    CK(cudaStreamSynchronize(stream));
+  }
+done:
+  cudaFree(d_veff);
+  return err;
+}
 
 cudaError_t rebuild_local_matrices(Op* op, const double* veff_q_host, cudaStream_t stream) {
   return launch_local_matrices(op, veff_q_host, stream, /*zero_tail=*/0, nullptr);
