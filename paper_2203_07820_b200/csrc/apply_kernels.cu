@@ -189,12 +189,12 @@ __global__ void __launch_bounds__(128) k_extract_proj_rows(const T* __restrict__
                                                            const int64_t* __restrict__ cell_proj_ptr,
                                                            const int32_t* __restrict__ row_cell,
                                                            const int32_t* __restrict__ ktot, int m_cell, int mpad, int lda,
-                                                           int mw, double* __restrict__ out) {
+                                                           int mw, double* __restrict__ out /*[rows][mpad]*/) {
   const int64_t r = blockIdx.x;
   const int c = row_cell[r];
   const int krow = mpad + (int)(r - cell_proj_ptr[c]);
   const T* M = mat + mat_off[c];
-  for (int l = threadIdx.x; l < m_cell; l += 128) out[r * m_cell + l] = (double)M[mat_elem(krow, l, mw, lda, ktot[c])];
+  for (int l = threadIdx.x; l < mpad; l += 128) out[r * mpad + l] = l < m_cell ? (double)M[mat_elem(krow, l, mw, lda, ktot[c])] : 0.0;
 }
 
 // Atomic assembly needs the recurrence term in place first:  T <- -beta T
@@ -1096,15 +1096,16 @@ cudaError_t assemble_projector_rows(Op* op, const HostPlan& plan, const chfsi_me
   cudaError_t e;
   if (op->n_proj == 0 || op->n_prow == 0 || op->nnz_cp == 0) return cudaSuccess;
   const int mc = op->m_cell;
-  // 1. compact FP64 copy of the projector rows of the cell matrices, on the host
+  // 1. compact FP64 copy of the projector rows of the cell matrices ([nnz_cp][mpad], zero-padded), on the host
   std::vector<int32_t> row_cell((size_t)op->nnz_cp);
   for (int64_t c = 0; c < op->n_cells; ++c)
     for (int64_t r = plan.cell_proj_ptr[c]; r < plan.cell_proj_ptr[c + 1]; ++r) row_cell[r] = (int32_t)c;
   int32_t* d_row_cell = nullptr; double* d_rows = nullptr;
   if ((e = cudaMalloc((void**)&d_row_cell, row_cell.size() * sizeof(int32_t)))) return e;
-  if ((e = cudaMalloc((void**)&d_rows, (size_t)op->nnz_cp * mc * sizeof(double)))) { cudaFree(d_row_cell); return e; }
+  const int mpad = op->mpad;
+  if ((e = cudaMalloc((void**)&d_rows, (size_t)op->nnz_cp * mpad * sizeof(double)))) { cudaFree(d_row_cell); return e; }
   op->crows = d_rows;   // kept: the sum-factorised kernel applies C~^c P from these rows (freed with the operator)
-  std::vector<double> rows((size_t)op->nnz_cp * mc);
+  std::vector<double> rows((size_t)op->nnz_cp * mpad);
   e = cudaMemcpyAsync(d_row_cell, row_cell.data(), row_cell.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st);
   if (e == cudaSuccess) {
     if (op->precision == 64)
@@ -1130,7 +1131,7 @@ cudaError_t assemble_projector_rows(Op* op, const HostPlan& plan, const chfsi_me
       for (int64_t k = plan.proj_ptr[j]; k < plan.proj_ptr[j + 1]; ++k) {
         const int64_t pr = plan.proj_pcrow[k];
         const int64_t c = row_cell[pr];
-        for (int l = 0; l < mc; ++l) coef[(size_t)loc[mesh.cell_dofs[c * mc + l]] * kProjGroup + i] += rows[(size_t)pr * mc + l];
+        for (int l = 0; l < mc; ++l) coef[(size_t)loc[mesh.cell_dofs[c * mc + l]] * kProjGroup + i] += rows[(size_t)pr * mpad + l];
       }
     }
   }
