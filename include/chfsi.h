@@ -100,6 +100,10 @@ typedef struct {
   int64_t cells_with_proj;
   double flops_per_vector_apply;/* n_cells*2*m_cell^2 + 4*m_cell*nnz_cell_proj + 7*n_dofs  */
   int64_t matrix_bytes;         /* device bytes of the Loewdin-scaled cell matrices (incl. padding)         */
+  double sf_flops_per_vector_apply; /* flops the sum-factorised kernel EXECUTES per vector-apply (DMMA at 512
+                                   per warp instruction incl. the 7 -> 8 padding, DFMA, projector MMAs of the assembly);
+                                   0 when that kernel does not apply to the operator (p > 6)                  */
+  int64_t sf_field_bytes;       /* device bytes of its quadrature-point fields and M^-1/2 tables             */
 } chfsi_info;
 
 /* assembly: 0 = deterministic (graph colouring of cells that share a dof; every dof is assembled in colour
@@ -176,10 +180,16 @@ int chfsi_subspace_transform(chfsi_op* op, const void* Y_dev, int64_t ldy, int64
 /* Number of kernel launches enqueued by this handle since creation (for benchmark bookkeeping). */
 int64_t chfsi_launch_count(const chfsi_op* op);
 
-/* Selects the kernel used for the per-cell contraction: 0 = automatic (single-launch persistent tensor-core
- * kernel when the shape allows), 1 = force the generic path, 2 = the earlier tensor-core kernel with one launch
- * per colour, 3 = (FP32 storage only) 3xTF32 products on the 32-bit tensor pipe: faster, but outside the 1e-5 Ha
- * eigenvalue tolerance of the FP32 variant (see csrc/apply_tf32.cuh).  For tests and A/B measurements. */
+/* Selects the kernel used for the per-cell product H~^e X^e (all variants compute the same H~ X up to rounding):
+ *   0 = automatic: the sum-factorised (matrix-free) kernel for FE degree p <= 6 (north_star: "sum-factorised where
+ *       measurement says so"; csrc/apply_sf.cuh), else the dense persistent tensor-core kernel, else the generic path;
+ *   1 = generic dense path (any shape / alignment);
+ *   2 = dense tensor-core kernel, one launch per colour;
+ *   3 = (FP32 storage only) dense, 3xTF32 products on the 32-bit tensor pipe: outside the 1e-5 Ha eigenvalue
+ *       tolerance of the FP32 variant (csrc/apply_tf32.cuh);
+ *   4 = dense persistent tensor-core kernel (FP64 DMMA with the distinct per-cell matrices of Eq. 47);
+ *   5 = sum-factorised kernel (same as 0 where it applies).
+ * For tests and A/B measurements. */
 int chfsi_set_kernel_variant(chfsi_op* op, int variant);
 
 /* Per-kernel device timing for the roofline report.  While enabled, every H~ application records one CUDA

@@ -51,7 +51,8 @@ class _Info(C.Structure):
                 ("assembly", C.c_int32), ("n_colors", C.c_int32),
                 ("n_cells", C.c_int64), ("n_dofs", C.c_int64), ("n_proj", C.c_int64),
                 ("nnz_cell_proj", C.c_int64), ("cells_with_proj", C.c_int64),
-                ("flops_per_vector_apply", C.c_double), ("matrix_bytes", C.c_int64)]
+                ("flops_per_vector_apply", C.c_double), ("matrix_bytes", C.c_int64),
+                ("sf_flops_per_vector_apply", C.c_double), ("sf_field_bytes", C.c_int64)]
 
 
 class _Profile(C.Structure):

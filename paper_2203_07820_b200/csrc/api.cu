@@ -311,6 +311,19 @@ int chfsi_get_info(const chfsi_op* op, chfsi_info* info) {
   info->flops_per_vector_apply = (double)op->n_cells * 2.0 * op->m_cell * op->m_cell +
                                  4.0 * op->m_cell * (double)op->nnz_cp + 7.0 * (double)op->n_dofs;
   info->matrix_bytes = op->mat_elems * (op->precision == 64 ? 8 : 4);
+  info->sf_flops_per_vector_apply = 0.0; info->sf_field_bytes = 0;
+  if (op->sf_ok) {
+    // executed work of k_apply_sf per (cell, column): DMMAs of the eight MMA stages, the in-lane DFMA stages, the
+    // Gauss-point stage, the scalings; per cell with projectors the k = 8 MMAs of the assembly (apply_sf.cuh)
+    const double n1 = op->n1, nq1 = op->nq1;
+    const double dmma = 8.0 * n1 + 8.0 * nq1;
+    const double lane_flops = 2.0 * (4.0 * n1 * nq1 + 4.0 * nq1 * nq1) + 34.0 * nq1 + 10.0 * n1;
+    const double per_cell_col = dmma * 512.0 + 32.0 * lane_flops;
+    const double proj_per_cell_col = 2.0 * ((op->m_cell + 7) / 8) * 512.0 / 8.0;
+    info->sf_flops_per_vector_apply = (double)op->n_cells * per_cell_col + (double)op->n_pc_cells * proj_per_cell_col +
+                                      4.0 * (double)op->n_cells * op->m_cell;
+    info->sf_field_bytes = (int64_t)op->n_cells * (op->nq1 * 7 * 64 + op->mpad) * 8;
+  }
   return CHFSI_OK;
 }
 

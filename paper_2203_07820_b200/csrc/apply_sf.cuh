@@ -213,23 +213,21 @@ __global__ void __launch_bounds__(kSfThreads, 2) k_apply_sf(ApplyDev<S> a, SfDev
                 dmma884(T2[c][u][0], T2[c][u][1], d[c][u][s], fPhiB[s]);    // T2[c][qb][qa] = sum_b T1 Phi[qb][b]
         }
 #pragma unroll
-        for (int q = 0; q < nq1; ++q) {
-          double acc[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
+        for (int q = 0; q < nq1; ++q)
 #pragma unroll
-          for (int c = 0; c < n1; ++c) {
+          for (int u = 0; u < 2; ++u) uh[q][u][0] = uh[q][u][1] = w[q][u][0] = w[q][u][1] = 0.0;
+        // third direction in the lane's registers, outer-product order: 4 nq1 independent accumulators
+#pragma unroll
+        for (int c = 0; c < n1; ++c)
+#pragma unroll
+          for (int q = 0; q < nq1; ++q) {
             const double ph = c_sf_phi[P][q * 8 + c];
 #pragma unroll
             for (int u = 0; u < 2; ++u) {
-              acc[u][0] = fma(ph, T2[c][u][0], acc[u][0]);
-              acc[u][1] = fma(ph, T2[c][u][1], acc[u][1]);
+              uh[q][u][0] = fma(ph, T2[c][u][0], uh[q][u][0]);
+              uh[q][u][1] = fma(ph, T2[c][u][1], uh[q][u][1]);
             }
           }
-#pragma unroll
-          for (int u = 0; u < 2; ++u) {
-            uh[q][u][0] = acc[u][0]; uh[q][u][1] = acc[u][1];
-            w[q][u][0] = w[q][u][1] = 0.0;
-          }
-        }
       }
 
       // ---- Gauss grid, slab by slab: gradient, metric / potential, transposed gradient -----------------------------
@@ -273,14 +271,19 @@ __global__ void __launch_bounds__(kSfThreads, 2) k_apply_sf(ApplyDev<S> a, SfDev
             dmma884(dx[u][0], dx[u][1], fDA[1], b1[u]);
             dmma884(dy[u][0], dy[u][1], uh[q][u][1], fDB[1]);
           }
+          {
+            double dzo[2][2] = {{0.0, 0.0}, {0.0, 0.0}};               // d_z u^ in the lane's registers (even / odd partial sums)
 #pragma unroll
-          for (int r = 0; r < nq1; ++r) {
-            const double dh = c_sf_dhat[P][q * 8 + r];                 // d_z u^ in the lane's registers
+            for (int r = 0; r < nq1; ++r) {
+              const double dh = c_sf_dhat[P][q * 8 + r];
 #pragma unroll
-            for (int u = 0; u < 2; ++u) {
-              dz[u][0] = fma(dh, uh[r][u][0], dz[u][0]);
-              dz[u][1] = fma(dh, uh[r][u][1], dz[u][1]);
+              for (int u = 0; u < 2; ++u) {
+                if (r & 1) { dzo[u][0] = fma(dh, uh[r][u][0], dzo[u][0]); dzo[u][1] = fma(dh, uh[r][u][1], dzo[u][1]); }
+                else { dz[u][0] = fma(dh, uh[r][u][0], dz[u][0]); dz[u][1] = fma(dh, uh[r][u][1], dz[u][1]); }
+              }
             }
+#pragma unroll
+            for (int u = 0; u < 2; ++u) { dz[u][0] += dzo[u][0]; dz[u][1] += dzo[u][1]; }
           }
           const double2* cq = reinterpret_cast<const double2*>(coef_s) + (q * 7) * 32 + lane;
           const double2 W0 = cq[0], Gxx = cq[32], Gxy = cq[64], Gxz = cq[96], Gyy = cq[128], Gyz = cq[160], Gzz = cq[192];
@@ -313,24 +316,30 @@ __global__ void __launch_bounds__(kSfThreads, 2) k_apply_sf(ApplyDev<S> a, SfDev
       }
 
       // ---- back to the nodes: y = (Phi x Phi x Phi)^T w; slabs alternate between the two scratch buffers ------------
+      double z[n1][2][2];
 #pragma unroll
-      for (int c = 0; c < n1; ++c) {
-        double* scr = (c & 1) ? scrB : scrA;
-        double z[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
+      for (int c = 0; c < n1; ++c)
 #pragma unroll
-        for (int q = 0; q < nq1; ++q) {
+        for (int u = 0; u < 2; ++u) z[c][u][0] = z[c][u][1] = 0.0;
+#pragma unroll
+      for (int q = 0; q < nq1; ++q)
+#pragma unroll
+        for (int c = 0; c < n1; ++c) {
           const double ph = c_sf_phi[P][q * 8 + c];
 #pragma unroll
           for (int u = 0; u < 2; ++u) {
-            z[u][0] = fma(ph, w[q][u][0], z[u][0]);
-            z[u][1] = fma(ph, w[q][u][1], z[u][1]);
+            z[c][u][0] = fma(ph, w[q][u][0], z[c][u][0]);
+            z[c][u][1] = fma(ph, w[q][u][1], z[c][u][1]);
           }
         }
 #pragma unroll
+      for (int c = 0; c < n1; ++c) {
+        double* scr = (c & 1) ? scrB : scrA;
+#pragma unroll
         for (int u = 0; u < 2; ++u) {
           double y0 = 0.0, y1 = 0.0;
-          dmma884(y0, y1, z[u][0], fPhiTB[0]);                         // y1[c][b][qa] = sum_qb z[qa][qb] Phi[qb][b]
-          dmma884(y0, y1, z[u][1], fPhiTB[1]);
+          dmma884(y0, y1, z[c][u][0], fPhiTB[0]);                      // y1[c][b][qa] = sum_qb z[qa][qb] Phi[qb][b]
+          dmma884(y0, y1, z[c][u][1], fPhiTB[1]);
           *reinterpret_cast<double2*>(scr + u * kSfScrSlab + so_w) = make_double2(y0, y1);
         }
         __syncwarp();

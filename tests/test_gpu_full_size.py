@@ -1,13 +1,16 @@
-"""GPU <-> oracle parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (chunk width B,
-degree m, stored bounds recipe B, default coloured assembly), through the C ABI.  `-m gpu`.
+"""GPU <-> oracle parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (all N columns of
+an ld = N device array filtered in chunks of B, degree m, stored bounds recipe B, default kernel and coloured
+assembly), through the C ABI.  `-m gpu`.
 
  * config 2: the whole 110,592 x 256 block against the oracle, plus the Rayleigh-Ritz values.
- * configs 3 / 4 / 5: the GPU filters one full chunk (B = 256 / 512 / 400 columns); the oracle filters SAMPLED
-   columns of that chunk one by one (columns are independent, and every column of the seeded block
-   has its own random stream), and sampled ROWS of H~X are recomputed from the definition (oracle.apply_H_rows).
+ * configs 3 / 4 / 5 (and the extra p = 7 workload 6): the GPU filters THE JOB THE BENCH TIMES -- all N = 1024 / 4096 /
+   4000 columns in 4 / 8 / 10 chunks; the oracle filters sampled columns of the FIRST, a MIDDLE and the LAST chunk
+   one by one (columns are independent; every sampled column comes from the config's seeded block, the
+   others are device-generated N(0,1) fill), and sampled ROWS of H~X are recomputed from the definition
+   (oracle.apply_H_rows).  H~X itself is compared on the sampled columns only; the rest of a chunk is covered by
+   the GPU-vs-GPU identities below.
  * properties that hold at any size: the fused filter equals the three-term recurrence driven by separate
-   apply_H calls; a column filtered inside the wide chunk (tensor-core kernel) equals the same column filtered
-   alone (generic kernel).
+   apply_H calls; a column filtered inside the wide chunk equals the same column filtered alone (generic kernel).
 """
 import numpy as np
 import pytest
@@ -37,7 +40,7 @@ def device_block(torch, random_block, n_dofs, B, seed, dtype):
 
 
 def ritz_first_order_slack(orc, oop, Fo, err):
-    """DESIGN.md reading U13.  A Ritz value is a Rayleigh quotient: for a unit Ritz vector v with residual
+    """DESIGN.md Sec. 2, reading U13.  A Ritz value is a Rayleigh quotient: for a unit Ritz vector v with residual
     r = H~v - theta v, a perturbation d of v moves theta by 2 d.r + O(|d|^2).  The sampled columns of a random block
     after ONE filter pass are far from converged (|r| is tens of Ha), so the FP32 variant's storage-level relative
     error `err` shows up in first order; north_star's 1e-5 Ha presumes (nearly) converged pairs, where r -> 0.
@@ -94,44 +97,67 @@ def config3_oracle():
     return wl, orc.operator_from_workload(wl)
 
 
-SAMPLE_COLS = {3: [0, 131, 255], 4: [0, 300, 511], 5: [0, 399], 6: [0, 131, 255]}
+# columns of the first, a middle and the last chunk of the whole job (chunk widths 256 / 512 / 400 / 256)
+SAMPLE_COLS = {3: [0, 600, 1023], 4: [0, 2000, 4095], 5: [0, 2000, 3999], 6: [0, 131, 255]}
+
+
+def whole_job_block(torch, random_block, n_dofs, N, seed, dtype, cols):
+    """[n_dofs, N] device array (ld = N): the sampled columns are the config's seeded columns, the rest N(0,1) fill."""
+    g = torch.Generator(device="cuda")
+    g.manual_seed(seed)
+    X = torch.empty((n_dofs, N), dtype=dtype, device="cuda")
+    for j0 in range(0, N, 256):
+        j1 = min(N, j0 + 256)
+        X[:, j0:j1] = torch.randn((n_dofs, j1 - j0), dtype=dtype, device="cuda", generator=g)
+    X[:, cols] = torch.from_numpy(random_block(n_dofs, cols, seed)).to("cuda", dtype)
+    return X
 
 
 @pytest.mark.parametrize("config", [3, 4])
-def test_config3_and_4_one_chunk_sampled_columns(config, config3_oracle):
-    _check_one_chunk_sampled_columns(config, *config3_oracle)
+def test_config3_and_4_whole_job_sampled_columns(config, config3_oracle):
+    _check_whole_job_sampled_columns(config, *config3_oracle)
 
 
-def test_p7_workload_one_chunk_sampled_columns():
-    """Extra workload 6 (not in BASELINE.json): config 2's box at FE degree 7, where the persistent kernel processes
-    the 512 output nodes of a cell as two tiles of 256."""
+def test_p7_workload_whole_job_sampled_columns():
+    """Extra workload 6 (not in BASELINE.json): config 2's box at FE degree 7, where the persistent dense kernel
+    processes the 512 output nodes of a cell as two tiles of 256 (the sum-factorised kernel stops at p = 6)."""
     torch, orc, Operator, CONFIGS, SEED_X, load_bounds, make_workload, random_block = _imports()
     wl = make_workload(6)
-    _check_one_chunk_sampled_columns(6, wl, orc.operator_from_workload(wl))
+    _check_whole_job_sampled_columns(6, wl, orc.operator_from_workload(wl))
 
 
-def _check_one_chunk_sampled_columns(config, wl, oop):
+def _check_whole_job_sampled_columns(config, wl, oop):
     torch, orc, Operator, CONFIGS, SEED_X, load_bounds, make_workload, random_block = _imports()
     spec = CONFIGS[config]
     a0, a, b = load_bounds(spec.bounds_key, "B")
     tol, tol_ritz = (1e-10, 1e-8) if spec.precision == 64 else (1e-4, 1e-5)
     op = Operator.from_workload(wl, precision=spec.precision)
-    Xd = device_block(torch, random_block, wl.n_dofs, spec.B, spec.seed_base + SEED_X, op.dtype)
     cols = SAMPLE_COLS[config]
-    Xs = Xd[:, cols].double().cpu().numpy()                  # FP32 variant: the input rounded once to FP32
+    X = whole_job_block(torch, random_block, wl.n_dofs, spec.N, spec.seed_base + SEED_X, op.dtype, cols)
+    assert X.stride(0) == spec.N
+    Xs = X[:, cols].double().cpu().numpy()                   # FP32 variant: the input rounded once to FP32
     if spec.precision == 64:
         assert np.array_equal(Xs, random_block(wl.n_dofs, cols, spec.seed_base + SEED_X))
-    Y = op.apply_H(Xd)
+    # H~X on the chunks that hold the sampled columns, compared on those columns
     Yr = orc.apply_H(oop, Xs)
-    assert rel_fro(Y[:, cols].double().cpu().numpy(), Yr) <= tol
-    # the fused filter == the recurrence built from apply_H (any size), then the oracle on the sampled columns
-    F = Xd.clone()
-    op.chebyshev_filter_chunked(F, spec.B, spec.m, a, b, a0)
-    R = recurrence_from_apply_H(torch, op, Xd, spec.m, a, b, a0)
-    assert float((F - R).norm() / R.norm()) <= (1e-12 if spec.precision == 64 else 1e-5)
-    del R, Y
+    for k, j in enumerate(cols):
+        j0 = (j // spec.B) * spec.B
+        Y = op.apply_H(X[:, j0:min(spec.N, j0 + spec.B)])
+        assert rel_fro(Y[:, j - j0].double().cpu().numpy(), Yr[:, k]) <= tol, (config, j)
+        del Y
+    # properties on the first chunk: fused filter == recurrence built from apply_H; column alone == column in the chunk
+    X0 = X[:, :spec.B].clone()
+    R = recurrence_from_apply_H(torch, op, X0, spec.m, a, b, a0)
+    one = X[:, cols[0]:cols[0] + 1].clone()
+    # THE JOB THE BENCH TIMES: all N columns, ld = N, chunks of B
+    op.chebyshev_filter_chunked(X, spec.B, spec.m, a, b, a0)
+    assert float((X[:, :spec.B] - R).norm() / R.norm()) <= (1e-12 if spec.precision == 64 else 1e-5)
+    del R, X0
+    op.chebyshev_filter(one, spec.m, a, b, a0)
+    assert float((one[:, 0] - X[:, cols[0]]).norm() / one.norm()) <= (1e-12 if spec.precision == 64 else 1e-5)
+    # the oracle on the sampled columns of the first, a middle and the last chunk
     Fo = orc.chebyshev_filter(oop, Xs, spec.m, a, b, a0)
-    Fs = F[:, cols].double().cpu().numpy()
+    Fs = X[:, cols].double().cpu().numpy()
     errs = []
     for k, j in enumerate(cols):
         err = rel_fro(Fs[:, k], Fo[:, k])
@@ -140,48 +166,55 @@ def _check_one_chunk_sampled_columns(config, wl, oop):
         assert np.max(np.abs(Fs[:, k] - Fo[:, k])) <= tol * np.max(np.abs(Fo[:, k]))
     th_g = orc.ritz_values_of_block(Fs, orc.apply_H(oop, Fs))
     th_o = orc.ritz_values_of_block(Fo, orc.apply_H(oop, Fo))
+    # FP64: 1e-8 Ha as stated.  FP32: the three sampled columns of a once-filtered random block are far from converged,
+    # so the storage-level error shows in first order (reading U13; the unslackened 1e-5 Ha check on a
+    # converged subspace is tests/test_gpu_parity.py::test_fp32_ritz_values_of_a_converged_subspace...)
     slack = 0.0 if spec.precision == 64 else ritz_first_order_slack(orc, oop, Fo, max(errs))
-    assert np.max(np.abs(th_g - th_o)) <= tol_ritz + slack, (np.max(np.abs(th_g - th_o)), slack)
-    # a column filtered alone (generic kernel, B = 1) == the same column inside the wide chunk
-    one = Xd[:, cols[1]:cols[1] + 1].clone()
-    op.chebyshev_filter(one, spec.m, a, b, a0)
-    assert float((one[:, 0] - F[:, cols[1]]).norm() / one.norm()) <= (1e-12 if spec.precision == 64 else 1e-5)
+    d = float(np.max(np.abs(th_g - th_o)))
+    print(f"config {config}: column errors {['%.2e' % e for e in errs]}, Ritz difference {d:.3e} Ha, first-order slack {slack:.3e}")
+    assert d <= tol_ritz + slack, (d, slack)
     op.close()
 
 
-def test_config5_one_chunk_sampled_rows_columns_and_properties():
+def test_config5_whole_job_sampled_rows_columns_and_properties():
     torch, orc, Operator, CONFIGS, SEED_X, load_bounds, make_workload, random_block = _imports()
     spec = CONFIGS[5]
     wl = make_workload(5)
     a0, a, b = load_bounds(spec.bounds_key, "B")
     op = Operator.from_workload(wl)
     assert op.info["n_dofs"] == 1728000 and op.info["n_proj"] == 1728
-    Xd = device_block(torch, random_block, wl.n_dofs, spec.B, spec.seed_base + SEED_X, op.dtype)
     cols = SAMPLE_COLS[5]
-    Xs = Xd[:, cols].cpu().numpy()
+    X = whole_job_block(torch, random_block, wl.n_dofs, spec.N, spec.seed_base + SEED_X, op.dtype, cols)   # 55.3 GB
+    Xs = X[:, cols].cpu().numpy()
     # (1) sampled rows of H~X recomputed one by one from the definition, without the whole oracle operator
     M = orc.mass_diagonal(wl.p, wl.cell_dofs, wl.cell_vertices, wl.n_dofs)
     assert np.allclose(op.mass_diag().cpu().numpy(), M, rtol=1e-12)
     near_atom = int(wl.cell_dofs[int(wl.proj_cell_idx[0]), 171])          # a dof inside a projector's support
     rows = [0, 3, 120 * 5 + 2, near_atom, wl.n_dofs - 1]
-    Y = op.apply_H(Xd)
     Yr = orc.apply_H_rows(wl, M, Xs, rows)
-    Yg = Y[rows][:, cols].cpu().numpy()
-    assert np.max(np.abs(Yg - Yr)) <= 1e-10 * float(Y.abs().max())
-    del Y
-    # (2) fused filter == recurrence from apply_H calls, at the full chunk width and degree
-    F = Xd.clone()
-    op.chebyshev_filter_chunked(F, spec.B, spec.m, a, b, a0)
-    R = recurrence_from_apply_H(torch, op, Xd, spec.m, a, b, a0)
-    assert float((F - R).norm() / R.norm()) <= 1e-12
+    for k, j in enumerate(cols):
+        j0 = (j // spec.B) * spec.B
+        Y = op.apply_H(X[:, j0:j0 + spec.B])
+        assert np.max(np.abs(Y[rows][:, j - j0].cpu().numpy() - Yr[:, k])) <= 1e-10 * float(Y.abs().max())
+        del Y
+    # (2) fused filter == recurrence from apply_H calls, at the full chunk width and degree (first chunk)
+    X0 = X[:, :spec.B].clone()
+    R = recurrence_from_apply_H(torch, op, X0, spec.m, a, b, a0)
+    del X0
+    # (3) THE JOB THE BENCH TIMES: 4,000 columns resident in HBM, ld = 4000, ten chunks of 400
+    op.chebyshev_filter_chunked(X, spec.B, spec.m, a, b, a0)
+    assert float((X[:, :spec.B] - R).norm() / R.norm()) <= 1e-12
     del R
-    # (3) the oracle proper on sampled columns of the chunk
+    Fs = X[:, cols].cpu().numpy()
+    del X
+    torch.cuda.empty_cache()
+    # (4) the oracle proper on sampled columns of the first, a middle and the last chunk
     oop = orc.operator_from_workload(wl)
     Fo = orc.chebyshev_filter(oop, Xs, spec.m, a, b, a0)
-    Fs = F[:, cols].cpu().numpy()
     for k, j in enumerate(cols):
         err = rel_fro(Fs[:, k], Fo[:, k])
         assert err <= 1e-10, f"config 5 column {j}: {err:.3e}"
+        assert np.max(np.abs(Fs[:, k] - Fo[:, k])) <= 1e-10 * np.max(np.abs(Fo[:, k]))
     th_g = orc.ritz_values_of_block(Fs, orc.apply_H(oop, Fs))
     th_o = orc.ritz_values_of_block(Fo, orc.apply_H(oop, Fo))
     assert np.max(np.abs(th_g - th_o)) <= 1e-8

@@ -36,8 +36,11 @@ def assert_block_close(Y, Yo, tol, what):
 
 
 CASES = {
-    # name: (workload kwargs | config number, B, m, precision)
+    # name: (workload kwargs | config number, B, m, precision[, bounds recipe of workloads/bounds.json])
     "config1": (1, 32, 10, 64),
+    # config 1 literally as BASELINE.json words it: b from a 20-step Lanczos estimate, a0 and a from a 30-vector
+    # Rayleigh-Ritz on a random start (recipe A of DESIGN.md reading U7; stored by oracle/make_bounds.py)
+    "config1_recipeA": (1, 32, 10, 64, "A"),
     "p6_nonlocal_ragged": (dict(n=3, p=6, L=6.0, atoms_per_side=1, n_gaussians=0, nonlocal_=True, smooth_field=0.05,
                                 seed_base=77), 72, 7, 64),
     "p6_distorted_cells": (dict(n=2, p=6, L=4.0, mesh_jitter=0.15, atoms_per_side=1, n_gaussians=0, nonlocal_=True,
@@ -77,14 +80,15 @@ def oracle_case(name):
     if name in _cache:
         return _cache[name]
     torch, orc, Operator, _, make_workload, random_block, load_bounds = _imports()
-    spec, B, m, precision = CASES[name]
+    spec, B, m, precision = CASES[name][:4]
+    recipe = CASES[name][4] if len(CASES[name]) > 4 else "B"
     wl = make_workload(spec) if isinstance(spec, int) else make_workload(None, **spec)
     oop = orc.operator_from_workload(wl)
     X = random_block(wl.n_dofs, range(B), 7)
     if precision == 32:
         X = X.astype(np.float32).astype(np.float64)     # the FP64-generated input rounded once to FP32 (reading U9)
     if isinstance(spec, int):
-        a0, a, b = load_bounds(str(spec), "B")
+        a0, a, b = load_bounds(str(spec), recipe)
     else:
         b, lmin = orc.lanczos_upper_bound(oop, np.random.default_rng(5).standard_normal(wl.n_dofs), 20)
         a0, a = lmin, lmin + 0.1 * (b - lmin)
@@ -94,12 +98,14 @@ def oracle_case(name):
     return _cache[name]
 
 
+# kernel variants (include/chfsi.h): 0 automatic (sum-factorised kernel for p <= 6, dense persistent kernel above),
+# 1 generic, 2 dense with one launch per colour, 4 dense persistent, 5 sum-factorised
 @pytest.mark.parametrize("assembly", [0, 1])
-@pytest.mark.parametrize("variant", [0, 1, 2])
+@pytest.mark.parametrize("variant", [0, 1, 2, 4])
 @pytest.mark.parametrize("name", list(CASES))
 def test_apply_H_and_filter_match_the_oracle(name, assembly, variant):
     torch, orc, Operator, _, _, _, _ = _imports()
-    _, B, m, precision = CASES[name]
+    _, B, m, precision = CASES[name][:4]
     wl, oop, X, (a0, a, b), Yo, Fo = oracle_case(name)
     tol, tol_ritz = TOL[precision]
     op = Operator.from_workload(wl, precision=precision, assembly=assembly)
@@ -128,7 +134,7 @@ def test_fp32_3xtf32_variant_is_within_the_block_tolerance_and_reproducible():
     this kernel is not the default)."""
     torch, orc, Operator, _, _, _, _ = _imports()
     name = "p6_fp32"
-    _, B, m, precision = CASES[name]
+    _, B, m, precision = CASES[name][:4]
     wl, oop, X, (a0, a, b), Yo, Fo = oracle_case(name)
     th_o = orc.ritz_values_of_block(Fo, orc.apply_H(oop, Fo))
     for assembly in (0, 1):
@@ -393,3 +399,85 @@ def test_argument_errors_on_the_device_entry_points():
         op32.overlap_matrix(torch.zeros((wl.n_dofs, 8), dtype=torch.float32, device="cuda"))
     assert ei.value.code == -5
     op32.close()
+
+
+def test_fp32_ritz_values_of_a_converged_subspace_within_1e_5_Ha_without_slack():
+    """north_star: FP32 variant eigenvalues within 1e-5 Ha.  That bound presumes (nearly) converged Ritz pairs (DESIGN.md
+    reading U13): here a 24-vector block runs SIX Chebyshev-filtered subspace iterations -- filter of degree 10 in the FP32
+    variant on the GPU, orthonormalisation on the host -- next to the same iteration with the FP64 oracle; the wanted
+    Ritz values (those below the filter bound a) of the two final subspaces, both measured with the oracle's apply_H,
+    must agree to 1e-5 Ha with NO slack term, and so must the GPU FP64 path to 1e-8 Ha."""
+    torch, orc, Operator, _, _, _, _ = _imports()
+    wl, oop, X, (a0, a, b), _, _ = oracle_case("p6_fp32")
+    nvec, m, passes = 24, 10, 6
+    lo, _ = np.linalg.qr(X[:, :nvec])
+    blocks = {"oracle": lo.copy(), 64: lo.copy(), 32: lo.astype(np.float32).astype(np.float64)}
+    ops = {64: Operator.from_workload(wl, precision=64), 32: Operator.from_workload(wl, precision=32)}
+    a_f = None
+    for it in range(passes):
+        # bounds of this pass from the oracle's current subspace (same scalars for every side): a = largest Ritz value
+        th = orc.ritz_values_of_block(blocks["oracle"], orc.apply_H(oop, blocks["oracle"]))
+        a_f, a0_f = float(th[-1]), float(th[0]) - 1e-3
+        for key in blocks:
+            Y = blocks[key]
+            if key == "oracle":
+                F = orc.chebyshev_filter(oop, Y, m, a_f, b, a0_f)
+            else:
+                Fd = torch.tensor(Y, dtype=ops[key].dtype, device="cuda")
+                ops[key].chebyshev_filter(Fd, m, a_f, b, a0_f)
+                F = Fd.double().cpu().numpy()
+            Q, _ = np.linalg.qr(F)
+            blocks[key] = Q if key != 32 else Q.astype(np.float32).astype(np.float64)
+    th = {k: orc.ritz_values_of_block(v, orc.apply_H(oop, v)) for k, v in blocks.items()}
+    wanted = th["oracle"] < 0.5 * (th["oracle"][0] + th["oracle"][-1])       # the lower half: converged after six passes
+    assert wanted.sum() >= 8
+    res = orc.apply_H(oop, blocks["oracle"])
+    d32 = float(np.max(np.abs(th[32][wanted] - th["oracle"][wanted])))
+    d64 = float(np.max(np.abs(th[64][wanted] - th["oracle"][wanted])))
+    print(f"converged-subspace Ritz differences: FP32 {d32:.3e} Ha, FP64 {d64:.3e} Ha ({int(wanted.sum())} values)")
+    assert d32 <= 1e-5, d32
+    assert d64 <= 1e-8, d64
+    for o in ops.values():
+        o.close()
+
+
+def test_projector_without_support_and_unused_dof_branches():
+    """host_setup.cpp: a projector whose CSR row is empty contributes nothing (the operator equals the one without it, and
+    the oracle agrees); a mesh whose n_dofs exceeds the dofs its cells use is rejected as a bad mesh."""
+    torch, orc, Operator, ChfsiError, make_workload, random_block, _ = _imports()
+    wl, oop, X, (a0, a, b), Yo, Fo = oracle_case("p3_odd_B")
+    # insert an empty projector in front, one in the middle and one at the end
+    ptr, D = list(wl.proj_cell_ptr), list(wl.D)
+    mid = wl.n_proj // 2
+    ptr2 = [0] + ptr[:mid + 1] + [ptr[mid]] + ptr[mid + 1:] + [ptr[-1]]
+    D2 = [0.7] + D[:mid] + [-0.3] + D[mid:] + [0.9]
+    op = Operator(wl.p, wl.cell_dofs, wl.cell_vertices, wl.n_dofs, wl.veff_q, wl.n_proj + 3, np.array(D2),
+                  np.array(ptr2, dtype=np.int64), wl.proj_cell_idx, wl.chi_q)
+    oop2 = orc.build_operator(wl.p, wl.cell_dofs, wl.cell_vertices, wl.n_dofs, wl.veff_q, wl.n_proj + 3, np.array(D2),
+                              np.array(ptr2, dtype=np.int64), wl.proj_cell_idx, wl.chi_q)
+    assert np.array_equal(orc.apply_H(oop2, X), Yo)            # the oracle: empty rows add nothing
+    for variant in (0, 1):
+        op.set_kernel_variant(variant)
+        Y = op.apply_H(torch.tensor(X, device="cuda")).cpu().numpy()
+        assert_block_close(Y, Yo, 1e-10, f"empty-support projectors, variant {variant}")
+    op.close()
+    with pytest.raises(ChfsiError) as ei:
+        Operator(wl.p, wl.cell_dofs, wl.cell_vertices, wl.n_dofs + 5, wl.veff_q)      # five dofs that belong to no cell
+    assert ei.value.code == -2 and "belongs to no cell" in str(ei.value)
+
+
+def test_block_width_limit_is_an_argument_error():
+    """check_block_args: B > 2^20 is refused before any device work (called through the raw ABI with dummy pointers)."""
+    import ctypes as C
+    torch, orc, Operator, ChfsiError, *_ = _imports()
+    from paper_2203_07820_b200 import load_library
+    wl, *_ = oracle_case("p3_odd_B")
+    op = Operator.from_workload(wl)
+    lib = load_library()
+    big = (1 << 20) + 2
+    ws = op.workspace(8)
+    x = torch.zeros(16, dtype=torch.float64, device="cuda")
+    rc = lib.chfsi_apply_H(op._h, C.c_void_p(x.data_ptr()), big, C.c_void_p(ws.data_ptr()), big, big,
+                           C.c_void_p(ws.data_ptr()), None)
+    assert rc == -1 and b"too large" in lib.chfsi_last_error(op._h)
+    op.close()
