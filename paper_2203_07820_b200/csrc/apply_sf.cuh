@@ -60,8 +60,8 @@ size_t sf_smem_bytes(const Op* op) {
   b += (size_t)nq1 * 7 * 64 * sizeof(double);                          // coefficient fields of the cell
   b += (size_t)kSfWarps * 4 * kSfScrSlab * sizeof(double);             // per-warp transposition scratch: 2 slabs x 2 columns
   b += (size_t)op->mpad * 16;                                          // {s_l, c or 0} per node
-  b += (size_t)kSfMaxProj * sf_tile_cols<S>() * sizeof(double);        // rows of P for the cell
-  b += (size_t)(op->mpad + kSfMaxProj) * sizeof(int32_t) + 64;         // index list, barriers, tickets
+  b += (size_t)2 * kSfMaxProj * sf_tile_cols<S>() * sizeof(double);    // rows of P for the cell (this tile, next tile)
+  b += (size_t)2 * (op->mpad + kSfMaxProj) * sizeof(int32_t) + 64;     // index lists (this tile, next tile), barriers, tickets
   return b;
 }
 
@@ -96,15 +96,14 @@ __global__ void __launch_bounds__(kSfThreads, 2) k_apply_sf(ApplyDev<S> a, SfDev
   double* coef_s = reinterpret_cast<double*>(xt + (size_t)mpad * 128);              // [nq1][7][32][2]
   double* scr_all = coef_s + coef_elems;                                            // [warps][4][kSfScrSlab]
   double2* tab_s = reinterpret_cast<double2*>(scr_all + kSfWarps * 4 * kSfScrSlab); // [mpad]
-  double* Ps = reinterpret_cast<double*>(tab_s + mpad);                             // [kSfMaxProj][TN]
-  uint64_t* bar = reinterpret_cast<uint64_t*>(Ps + kSfMaxProj * TN);               // [2]: tile data, projector columns
+  double* Ps_all = reinterpret_cast<double*>(tab_s + mpad);                         // [2][kSfMaxProj][TN]
+  uint64_t* bar = reinterpret_cast<uint64_t*>(Ps_all + 2 * kSfMaxProj * TN);       // [2]: tile data, projector columns
   long long* ticket_s = reinterpret_cast<long long*>(bar + 2);                      // [2]
-  int32_t* idx_s = reinterpret_cast<int32_t*>(ticket_s + 2);                        // [mpad + kSfMaxProj]
+  int32_t* idx_all = reinterpret_cast<int32_t*>(ticket_s + 2);                      // [2][mpad + kSfMaxProj]
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int g = lane >> 2, t = lane & 3;
   const int nct = a.n_col_tiles;
-  const double alpha = a.alpha, beta = a.beta;
   // scratch slabs of this warp: [buffer A | B][column u]; element (row, col) of a slab at row * pitch + col
   double* scrA = scr_all + warp * 4 * kSfScrSlab;
   double* scrB = scrA + 2 * kSfScrSlab;
@@ -134,37 +133,67 @@ __global__ void __launch_bounds__(kSfThreads, 2) k_apply_sf(ApplyDev<S> a, SfDev
   }
   __syncthreads();
 
+  // Small per-tile data: index list (dofs of the cell's nodes, then its projector ids), {M^-1/2, shift} per node, the
+  // rows of P of the cell's projectors.  Those of the NEXT tile are fetched into registers at the start of the assembly
+  // of the current tile and stored at its end, and the next tile's rows and fields are requested right after the
+  // completion flag is released: the next tile starts with a wait on the copies only.
+  constexpr int kIdxStride = (mc + 7) / 8 * 8 + kSfMaxProj;
+  constexpr int kIdxPer = (kIdxStride + kSfThreads - 1) / kSfThreads;
+  constexpr int kPsPer = kSfMaxProj * TN / kSfThreads;
+  int idx_pre[kIdxPer];
+  double sl_pre[kIdxPer], p_pre[kPsPer];
+  auto load_small = [&](long long ticket_l, int& cell_l, int& col0_l) {
+    cell_l = pd.pos_cell[(int)(ticket_l / nct)];
+    col0_l = (int)(ticket_l % nct) * TN;
+    const int32_t* gi_l = a.gidx + a.idx_off[cell_l];
+    const int np_l = (int)(sf.cell_proj_ptr[cell_l + 1] - sf.cell_proj_ptr[cell_l]);
+    const int ncols_l = min(TN, a.B - col0_l);
+#pragma unroll
+    for (int i = 0; i < kIdxPer; ++i) {
+      const int k = tid + i * kSfThreads;
+      idx_pre[i] = (k < mpad + np_l) ? gi_l[k] : 0;
+      sl_pre[i] = (k < mc) ? sf.sloc[(int64_t)cell_l * mpad + k] : 0.0;
+    }
+#pragma unroll
+    for (int i = 0; i < kPsPer; ++i) {
+      const int e = tid + i * kSfThreads, jj = e / TN, cc = e % TN;
+      p_pre[i] = (jj < np_l && cc < ncols_l) ? (double)a.P[(int64_t)gi_l[mpad + jj] * a.ldp + col0_l + cc] : 0.0;
+    }
+  };
+  auto store_small = [&](int32_t* idx_l, double* Ps_l) {
+#pragma unroll
+    for (int i = 0; i < kIdxPer; ++i) {
+      const int k = tid + i * kSfThreads;
+      if (k < kIdxStride) idx_l[k] = idx_pre[i];
+      if (k < mpad) tab_s[k] = make_double2(sl_pre[i], (idx_pre[i] < 0) ? sf.cshift : 0.0);
+    }
+#pragma unroll
+    for (int i = 0; i < kPsPer; ++i) Ps_l[tid + i * kSfThreads] = p_pre[i];
+  };
+  auto issue_tile = [&](const int32_t* idx_l, int cell_l, int col0_l) {      // warp 0, all lanes
+    if (lane == 0) {
+      mbar_expect_tx(bar, (uint32_t)mpad * 128u + (uint32_t)(coef_elems * sizeof(double)));
+      bulk_g2s(coef_s, sf.coef + (int64_t)cell_l * coef_elems, (uint32_t)(coef_elems * sizeof(double)), bar);
+    }
+    __syncwarp();
+    for (int r4 = lane; r4 < mpad / 4; r4 += 32)
+      tma_gather4(xt + (size_t)r4 * 512, &tmX, col0_l, idx_l[4 * r4] & 0x7fffffff, idx_l[4 * r4 + 1] & 0x7fffffff,
+                  idx_l[4 * r4 + 2] & 0x7fffffff, idx_l[4 * r4 + 3] & 0x7fffffff, bar);
+  };
+  if (ticket_s[0] < pd.n_tiles) {
+    int cell_f, col0_f;
+    load_small(ticket_s[0], cell_f, col0_f);
+    store_small(idx_all, Ps_all);
+    __syncthreads();
+    if (warp == 0) issue_tile(idx_all, cell_f, col0_f);
+  }
+
   uint32_t phase = 0, phase_c = 0;   // parities of the two barriers (tile data / projector columns)
   for (int iter = 0;; ++iter) {
-    const long long ticket = ticket_s[iter & 1];
-    if (ticket >= pd.n_tiles) break;
-    const int pos = (int)(ticket / nct), jt = (int)(ticket % nct);
-    const int cell = pd.pos_cell[pos];
-    const int col0 = jt * TN;
-    const int ncols = min(TN, a.B - col0);                 // even: B is a multiple of the 16-byte chunk
-    const int32_t* gi = a.gidx + a.idx_off[cell];
-    const int64_t cp0 = sf.cell_proj_ptr[cell];
-    const int np = (int)(sf.cell_proj_ptr[cell + 1] - cp0);
+    if (ticket_s[iter & 1] >= pd.n_tiles) break;
+    {
+    const int ncols = min(TN, a.B - (int)(ticket_s[iter & 1] % nct) * TN);   // even: B is a multiple of the 16-byte chunk
     if (tid == 0) ticket_s[(iter + 1) & 1] = (long long)(atomicAdd(pd.counter, 1ull) - pd.ticket_base);
-    for (int k = tid; k < mpad + np; k += kSfThreads) idx_s[k] = gi[k];
-    __syncthreads();   // idx_s visible; every thread is done with the previous tile's rows (its epilogue)
-    if (warp == 0) {
-      if (lane == 0) {
-        mbar_expect_tx(bar, (uint32_t)mpad * 128u + (uint32_t)(coef_elems * sizeof(double)));
-        bulk_g2s(coef_s, sf.coef + (int64_t)cell * coef_elems, (uint32_t)(coef_elems * sizeof(double)), bar);
-      }
-      __syncwarp();
-      for (int r4 = lane; r4 < mpad / 4; r4 += 32)
-        tma_gather4(xt + (size_t)r4 * 512, &tmX, col0, idx_s[4 * r4] & 0x7fffffff, idx_s[4 * r4 + 1] & 0x7fffffff,
-                    idx_s[4 * r4 + 2] & 0x7fffffff, idx_s[4 * r4 + 3] & 0x7fffffff, bar);
-    }
-    for (int k = tid; k < mpad; k += kSfThreads)
-      tab_s[k] = make_double2(k < mc ? sf.sloc[(int64_t)cell * mpad + k] : 0.0, (idx_s[k] < 0) ? sf.cshift : 0.0);
-    for (int e = tid; e < kSfMaxProj * TN; e += kSfThreads) {
-      const int jj = e / TN, cc = e % TN;
-      Ps[e] = (jj < np && cc < ncols) ? (double)a.P[(int64_t)idx_s[mpad + jj] * a.ldp + col0 + cc] : 0.0;
-    }
-    __syncthreads();   // tab_s / Ps visible
     mbar_wait(bar, phase);
 
     // ------------------------------------------------------------------------------------------------------------
@@ -367,10 +396,29 @@ __global__ void __launch_bounds__(kSfThreads, 2) k_apply_sf(ApplyDev<S> a, SfDev
       __syncwarp();                                                    // scratch free for the next pair of columns
     }
     __syncthreads();                                                   // the whole tile holds H~^loc X - c X [first]
+    }
+    // The tile coordinates are re-derived from the ticket in shared memory (a volatile read) instead of being kept in
+    // registers across the column loop above, which needs every register it can get.
+    {
+    const long long ticket = *reinterpret_cast<volatile long long*>(&ticket_s[iter & 1]);
+    int32_t* idx_s = idx_all + (iter & 1) * kIdxStride;
+    int32_t* idx_n = idx_all + ((iter + 1) & 1) * kIdxStride;
+    const int pos = (int)(ticket / nct), jt = (int)(ticket % nct);
+    const int cell = pd.pos_cell[pos];
+    const int col0 = jt * TN;
+    const int ncols = min(TN, a.B - col0);
+    const int64_t cp0 = sf.cell_proj_ptr[cell];
+    const int np = (int)(sf.cell_proj_ptr[cell + 1] - cp0);
+    const double alpha = a.alpha, beta = a.beta;
+    const double* Ps = Ps_all + (iter & 1) * kSfMaxProj * TN;
 
     // ---- assembly + recurrence (steps 4-5) and the projector term C~^c P (Alg. 4 step 5) -------------------------
     // The coefficient fields are dead now: the projector columns of the cell, s_l C^c_{l,j} ([np][mpad] FP64, contiguous),
     // arrive in their place by one bulk copy while the dependency flags and the old target rows are fetched.
+    const long long ticket_n = ticket_s[(iter + 1) & 1];
+    const bool has_next = ticket_n < pd.n_tiles;
+    int cell_n = 0, col0_n = 0;
+    if (has_next) load_small(ticket_n, cell_n, col0_n);
     double* crow_s = coef_s;
     const int npc = min(np, kSfCrowChunk);
     if (tid == 0 && np > 0) {
@@ -473,9 +521,12 @@ __global__ void __launch_bounds__(kSfThreads, 2) k_apply_sf(ApplyDev<S> a, SfDev
       }
     }
     phase ^= 1u;
-    __threadfence();
+    if (has_next) store_small(idx_n, Ps_all + ((iter + 1) & 1) * kSfMaxProj * TN);
+    __threadfence();                                               // (before the copies are issued: the fence would wait for them)
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic accesses to the tile rows before the next TMA writes
-    __syncthreads();
+    __syncthreads();                                               // tile assembled and fenced; next index list visible
     if (tid == 0 && !a.atomic) st_release_gpu(pd.flags + (int64_t)pos * nct + jt, pd.epoch);
+    if (has_next && warp == 0) issue_tile(idx_n, cell_n, col0_n);
+    }
   }
 }
