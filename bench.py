@@ -1,11 +1,14 @@
 #!/usr/bin/env python
 """Benchmark of the Chebyshev-filter hot path.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--assembly 0|1] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--assembly 0|1] [--variant V] [--impl reference]
+    python bench.py --all-configs            one JSON line per BASELINE.json config (profiles/r02_all_configs.md)
+    python bench.py --rr                     Rayleigh-Ritz products S, H^, Y Z on config 3's rows (Alg. 2 steps 1 and 3)
 
 One "step" = one pass of the whole hot path over one batch of synthetic input: the degree-m Chebyshev filter
-(cell extraction, per-cell contraction, non-local projectors, assembly, fused recurrence; m times) applied to
-all N vectors of the chosen BASELINE.json config in chunks of B columns.  Prints ONE JSON line.
+(cell extraction, per-cell product, non-local projectors, assembly, fused recurrence; m times) applied to
+all N vectors of the chosen BASELINE.json config in chunks of B columns.  Prints ONE JSON line.  The default workload
+is the largest single-GPU configuration, config 5 (1,728,000 dofs = the paper's Mo6x6x6 count, 4,000 vectors, m = 40).
 
 N > 1 (torchrun): the path shards over the vectors (the paper's band parallelisation): every rank
 holds a replica of the operator and filters its own N columns; there is no data-path collective (weak scaling).
@@ -26,28 +29,32 @@ if ROOT not in sys.path:
 
 METRIC = "chebyshev_filter_vector_applies_per_s"
 UNIT = "vector-applies/s"
-DEFAULT_CONFIG = 2          # BASELINE.json configs[1]
+DEFAULT_CONFIG = 5          # the largest single-GPU configuration of BASELINE.json (the metric names no config)
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the contraction kernel, from the `ncu --set full`
-# capture summarised in profiles/ (file named in the value); None until a capture exists for that key.
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the `ncu --set full` captures
+# summarised in profiles/ (one capture per (config, kernel); re-captured whenever that kernel changes); None = no capture.
 NCU_TRAFFIC_BYTES_PER_LAUNCH = {
-    (2, 0): 1.661e9,        # profiles/r01_v4_config2_config3.md: 1.334 GB read + 0.327 GB written per launch
-    (3, 0): 14.54e9,        # same file: 11.68 GB read + 2.86 GB written per launch
+    (2, "k_apply_dmma_p<double>"): 1.661e9,    # profiles/r01_v4_config2_config3.md: 1.334 GB read + 0.327 GB written
+    (3, "k_apply_dmma_p<double>"): 14.54e9,    # same file: 11.68 GB read + 2.86 GB written
 }
 
 
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=DEFAULT_CONFIG, choices=[1, 2, 3, 4, 5, 6],
                     help="BASELINE.json config 1..5; 6 = extra p=7 workload (config 2's box at FE degree 7)")
     ap.add_argument("--assembly", type=int, default=0, choices=[0, 1],
                     help="0 deterministic coloured assembly, 1 atomic assembly")
-    ap.add_argument("--variant", type=int, default=0, choices=[0, 1, 2, 3],
-                    help="contraction kernel: 0 default (persistent single launch), 1 generic, 2 one launch per colour, "
-                         "3 FP32 storage with 3xTF32 products (opt-in, looser accuracy)")
+    ap.add_argument("--variant", type=int, default=0, choices=[0, 1, 2, 3, 4, 5],
+                    help="kernel of the per-cell product: 0 automatic (sum-factorised for p <= 6, else dense persistent), "
+                         "1 generic, 2 dense one launch per colour, 3 FP32 storage with 3xTF32 products (looser accuracy), "
+                         "4 dense persistent DMMA kernel, 5 sum-factorised")
+    ap.add_argument("--all-configs", action="store_true", help="one JSON line per BASELINE.json config (1..5)")
+    ap.add_argument("--rr", action="store_true",
+                    help="Rayleigh-Ritz products (S = Y^T Y, H^ = Y^T H~ Y, Y Z) at N = 1024 on config 3's rows")
     ap.add_argument("--block-width", type=int, default=0,
                     help="override the chunk width B of the config (block-width sweep, the shape of the paper's Fig. 2a); "
                          "N becomes one chunk of that width")
@@ -179,6 +186,21 @@ def run_reference(args, spec):
 # ------------------------------------------------------------------------------------------------------------
 # the CUDA path
 # ------------------------------------------------------------------------------------------------------------
+KERNEL_NAMES = {
+    (64, 1): "k_apply_generic<double>", (64, 2): "k_apply_dmma", (64, 4): "k_apply_dmma_p<double>", (64, 5): "k_apply_sf<double>",
+    (32, 1): "k_apply_generic<float>", (32, 3): "k_apply_tf32_p", (32, 4): "k_apply_dmma_p<float>", (32, 5): "k_apply_sf<float>",
+}
+
+
+def dominant_kernel(precision, variant, info):
+    """Name of the kernel the automatic choice (variant 0) resolves to for this operator (include/chfsi.h)."""
+    if variant == 0:
+        variant = 5 if info["sf_flops_per_vector_apply"] > 0 else 4
+    if variant == 5 and not info["sf_flops_per_vector_apply"] > 0:
+        variant = 4
+    return KERNEL_NAMES.get((precision, variant), "k_apply_generic"), variant
+
+
 def run_b200(args, spec):
     import numpy as np
     import torch
@@ -194,7 +216,7 @@ def run_b200(args, spec):
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
     torch.cuda.set_device(local_rank)
-    if world > 1:
+    if world > 1 and not dist.is_initialized():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
     wl = make_workload(spec.config)
@@ -204,15 +226,16 @@ def run_b200(args, spec):
     info = op.info
     N, B, m = spec.N, spec.B, spec.m
     dtype = op.dtype
+    elt = 8 if spec.precision == 64 else 4
+    kernel, eff_variant = dominant_kernel(spec.precision, args.variant, info)
 
-    # synthetic N(0,1) block, generated on the host with a per-rank seed (band-parallel shard), pinned
-    rng = np.random.default_rng([spec.seed_base + SEED_X, rank])
-    X_host = torch.from_numpy(rng.standard_normal((wl.n_dofs, N)).astype(np.float64 if spec.precision == 64 else np.float32))
-    try:
-        X_host = X_host.pin_memory()
-    except Exception:
-        pass
-    X0 = X_host.to("cuda")
+    # synthetic N(0,1) block resident in HBM, one seeded stream per rank (band-parallel shard), generated on the device
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(1000003 * (spec.seed_base + SEED_X) + rank)
+    X0 = torch.empty((wl.n_dofs, N), dtype=dtype, device="cuda")
+    for j0 in range(0, N, 256):
+        j1 = min(N, j0 + 256)
+        X0[:, j0:j1] = torch.randn((wl.n_dofs, j1 - j0), dtype=dtype, device="cuda", generator=gen)
     X = torch.empty_like(X0)
     ws = op.workspace(min(B, N))
     peaks = measure_fp64_peak()
@@ -250,48 +273,56 @@ def run_b200(args, spec):
     value = world * N * m / (ms_per_step * 1e-3)
     flops_va = info["flops_per_vector_apply"]
 
-    # roofline of the dominant kernel (per-cell contraction incl. gather, 3d rows, assembly, recurrence)
-    elt = 8 if spec.precision == 64 else 4
-    contr_flops_per_apply = (info["n_cells"] * 2.0 * info["m_cell"] ** 2 + 2.0 * info["m_cell"] * info["nnz_cell_proj"])
-    n_apply = prof["applies"]
+    # roofline of the dominant kernel (per-cell product incl. gather, projector term, assembly, recurrence)
     cols_total = N * m * args.steps                           # column-applies covered by the profile
-    contr_tflops = contr_flops_per_apply * cols_total / (prof["contraction_ms"] * 1e-3) * 1e-12 if prof["contraction_ms"] > 0 else None
-    if spec.precision == 32 and args.variant == 3:
-        peak, bound, peak_note = 277.3 / 3.0, "tensor", \
-            "mma.sync m16n8k8 TF32 rate measured on B200 (277.3 TFLOP/s, round-1 microbenchmark) / 3 passes per FP32 product"
-    elif spec.precision == 64 or args.variant == 0:
-        # the FP32 variant stores matrices and vectors in FP32 and contracts them on the same FP64 tensor pipe
-        peak, bound, peak_note = peaks["dmma_tflops"], "tensor", \
-            "FP64 mma.sync m8n8k4 (DMMA) rate measured in this run by chfsi_measure_fp64_peak; MEASURED_PEAKS.json has no FP64 figure"
+    sf = eff_variant == 5
+    if sf:
+        # the sum-factorised kernel: EXECUTED flops; DMMA and DFMA share one FP64 pipe on B200
+        kflops_per_col = info["sf_flops_per_vector_apply"]
+        peak, bound = peaks["dmma_tflops"], "alu"
+        peak_note = ("FP64 pipe rate measured in this run by chfsi_measure_fp64_peak (mma.sync m8n8k4 f64; plain DFMA measures "
+                     "the same and the two share the pipe: a mixed stream never exceeds it, DESIGN.md Sec. 5); "
+                     "MEASURED_PEAKS.json has no FP64 figure")
     else:
-        peak, bound, peak_note = 2 * 37.2, "alu", "FP32 FFMA: 148 SMs x 128 lanes x 2 x 1.965 GHz (B200_PROFILING.md unit counts)"
-    key = (spec.config, args.assembly)
+        kflops_per_col = info["n_cells"] * 2.0 * info["m_cell"] ** 2 + 2.0 * info["m_cell"] * info["nnz_cell_proj"]
+        if spec.precision == 32 and eff_variant == 3:
+            peak, bound, peak_note = 277.3 / 3.0, "tensor", \
+                "mma.sync m16n8k8 TF32 rate measured on B200 (277.3 TFLOP/s, round-1 microbenchmark) / 3 passes per FP32 product"
+        elif eff_variant in (2, 4):
+            peak, bound, peak_note = peaks["dmma_tflops"], "tensor", \
+                "FP64 mma.sync m8n8k4 (DMMA) rate measured in this run by chfsi_measure_fp64_peak; MEASURED_PEAKS.json has no FP64 figure"
+        else:
+            peak = peaks["dfma_tflops"] * (2.0 if spec.precision == 32 else 1.0)
+            bound, peak_note = "alu", "plain FMA loop: DFMA rate measured in this run (x2 for FP32 FFMA, B200_PROFILING.md unit counts)"
+    k_tflops = kflops_per_col * cols_total / (prof["contraction_ms"] * 1e-3) * 1e-12 if prof["contraction_ms"] > 0 else None
     roofline = {
-        "kernel": ({0: "k_apply_dmma_p<double>", 1: "k_apply_generic<double>", 2: "k_apply_dmma"}[args.variant]
-                   if spec.precision == 64 else {0: "k_apply_dmma_p<float>", 3: "k_apply_tf32_p"}.get(args.variant, "k_apply_generic<float>")),
-        "bound": bound, "achieved": contr_tflops, "peak": peak, "unit": "TFLOP/s",
-        "frac": (contr_tflops / peak) if contr_tflops else None,
-        "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(key),
+        "kernel": kernel, "bound": bound, "achieved": k_tflops, "peak": peak, "unit": "TFLOP/s",
+        "frac": (k_tflops / peak) if k_tflops else None,
+        "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get((spec.config, kernel)) if args.assembly == 0 else None,
+        "flops_counted": "executed (sum-factorised kernel)" if sf else "algorithmic 2 (M_cell + N_psp) M_cell per cell and column",
         "peak_source": peak_note,
         "launches": prof["contraction_launches"],
         "avg_launch_ms": prof["contraction_ms"] / max(1, prof["contraction_launches"]),
-        "flops_per_launch": contr_flops_per_apply * cols_total / max(1, prof["contraction_launches"]),
+        "flops_per_launch": kflops_per_col * cols_total / max(1, prof["contraction_launches"]),
         "share_of_step": prof["contraction_ms"] / ms_local,
         "projector_ms_share": prof["projector_ms"] / ms_local,
         "fp64_dfma_peak": peaks["dfma_tflops"] if peaks else None,
+        "dense_equivalent_tflops": (info["n_cells"] * 2.0 * info["m_cell"] ** 2 + 2.0 * info["m_cell"] * info["nnz_cell_proj"])
+        * cols_total / (prof["contraction_ms"] * 1e-3) * 1e-12 if prof["contraction_ms"] > 0 else None,
     }
 
-    # end to end through the host-buffer entry point: H2D of every chunk, filter, D2H of the result
+    # end to end through the host-buffer entry point: H2D of every chunk, filter, D2H of the result, pinned host memory.
+    # One pinned buffer, filtered in place step after step (the cost of a step does not depend on the values).
     e2e = None
     if not args.no_e2e:
-        Xh = X_host.clone()
-        try:
-            Xh = Xh.pin_memory()
-        except Exception:
-            pass
-        n_e2e = max(1, min(args.steps, 3))
-        op.chebyshev_filter_host(Xh, B, m, a, b, a0)          # warm-up (allocations, first touch)
-        Xh.copy_(X_host)
+        del X
+        torch.cuda.empty_cache()
+        Xh = torch.empty((wl.n_dofs, N), dtype=dtype, pin_memory=True)
+        Xh.copy_(X0)
+        del X0
+        torch.cuda.empty_cache()
+        n_e2e = max(1, min(args.steps, 10))
+        op.chebyshev_filter_host(Xh, B, m, a, b, a0)          # warm-up (staging allocations, first touch)
         barrier()
         t0 = time.perf_counter()
         for _ in range(n_e2e):
@@ -301,7 +332,9 @@ def run_b200(args, spec):
         dt = aggregate_max(dt, world)
         nbytes = wl.n_dofs * N * elt
         e2e = {"value": world * N * m * n_e2e / dt, "unit": UNIT, "h2d_bytes_per_step": nbytes,
-               "d2h_bytes_per_step": nbytes, "steps": n_e2e, "timer": "host wall clock around chfsi_chebyshev_filter_host"}
+               "d2h_bytes_per_step": nbytes, "steps": n_e2e, "timer": "host wall clock around chfsi_chebyshev_filter_host",
+               "fraction_of_device_resident": world * N * m * n_e2e / dt / value}
+        del Xh
 
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -311,33 +344,113 @@ def run_b200(args, spec):
         cpu_baseline = {"value": v, "unit": UNIT, "cores": cpu_threads(), "kind": "oracle",
                         "sample": f"columns 0..{ncols - 1} of the first chunk, full degree m={spec.m}, one pass"}
 
+    line = None
     if rank == 0:
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None,
             "dtype": ("f64" if spec.precision == 64 else
-                      "f32 (3xTF32 products, f32 accumulate)" if args.variant == 3 else
-                      "f64 accumulate on f32-stored matrices and vectors"),
+                      "f32 (3xTF32 products, f32 accumulate)" if eff_variant == 3 else
+                      "f64 arithmetic on f32-stored vectors"),
             "data": "synthetic",
             "config": {"workload": workload_name(spec), "assembly": "coloured" if args.assembly == 0 else "atomic",
-                       "n_colors": info["n_colors"], "bounds": {"a0": a0, "a": a, "b": b},
+                       "kernel": kernel, "n_colors": info["n_colors"], "bounds": {"a0": a0, "a": a, "b": b},
                        "parallelism": f"band-parallel x{world} (operator replicated, no collective)",
-                       "l2": "inputs larger than L2 (cell matrices %.2f GB + vector blocks %.2f GB vs 126 MB)"
-                             % (info["matrix_bytes"] / 1e9, 2 * wl.n_dofs * min(B, N) * elt / 1e9)},
-            "tflops": value * flops_va * 1e-12,
-            "flops_per_vector_apply": flops_va,
+                       "l2": "inputs larger than L2 (vector blocks %.2f GB + operator data %.2f GB vs 126 MB)"
+                             % (2 * wl.n_dofs * min(B, N) * elt / 1e9,
+                                (info["sf_field_bytes"] if sf else info["matrix_bytes"]) / 1e9)},
+            "tflops": value * (info["sf_flops_per_vector_apply"] if sf else flops_va) * 1e-12,
+            "tflops_counted": "executed" if sf else "algorithmic",
+            "dense_equivalent_tflops": value * flops_va * 1e-12,
+            "flops_per_vector_apply": info["sf_flops_per_vector_apply"] if sf else flops_va,
             "roofline": roofline, "e2e": e2e, "cpu_baseline": cpu_baseline,
             "gpu_launches": launches, "clocks": clocks,
         }
         print(json.dumps(line), flush=True)
-    if world > 1:
-        dist.destroy_process_group()
+    op.close()
+    return line
+
+
+def run_rr(args):
+    """Rayleigh-Ritz products of Algorithm 2 at N = 1024 columns on config 3's 884,736 rows:
+    S = Y^T Y (k_xty), H^ = Y^T (H~ Y) (apply + k_xty per chunk), Out = Y Z (k_xz).  One JSON line."""
+    import torch
+
+    from paper_2203_07820_b200 import Operator, measure_fp64_peak
+    from workloads.generate import CONFIGS, make_workload
+    spec = CONFIGS[3]
+    wl = make_workload(3)
+    op = Operator.from_workload(wl)
+    info = op.info
+    N, B = 1024, 256
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(77)
+    Y = torch.randn((wl.n_dofs, N), dtype=torch.float64, device="cuda", generator=gen)
+    Z = torch.randn((N, N), dtype=torch.float64, device="cuda", generator=gen)
+    Out = torch.empty_like(Y)
+    ws = op.workspace(B)
+    peaks = measure_fp64_peak()
+    sampler = ClockSampler(torch.cuda.current_device())
+
+    def timed(fn):
+        for _ in range(args.warmup):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.steps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / args.steps
+
+    sampler.start()
+    l0 = op.launch_count()
+    ms_s = timed(lambda: op.overlap_matrix(Y))
+    ms_h = timed(lambda: op.projected_hamiltonian(Y, B=B, workspace=ws))
+    ms_z = timed(lambda: op.subspace_transform(Y, Z, Out=Out))
+    launches = op.launch_count() - l0
+    clocks = sampler.stop()
+    gemm = 2.0 * wl.n_dofs * N * N                            # flops of one tall product
+    kernel, _ = dominant_kernel(64, args.variant, info)
+    apply_flops = (info["sf_flops_per_vector_apply"] if "sf" in kernel else info["flops_per_vector_apply"]) * N
+    peak = peaks["dmma_tflops"]
+    parts = {
+        "overlap_S": {"kernel": "k_xty", "ms": ms_s, "tflops": gemm / ms_s * 1e-9, "frac": gemm / ms_s * 1e-9 / peak},
+        "projected_H": {"kernel": kernel + " + k_xty", "ms": ms_h, "tflops": (gemm + apply_flops) / ms_h * 1e-9,
+                        "frac": (gemm + apply_flops) / ms_h * 1e-9 / peak},
+        "transform_YZ": {"kernel": "k_xz", "ms": ms_z, "tflops": gemm / ms_z * 1e-9, "frac": gemm / ms_z * 1e-9 / peak},
+    }
+    total_ms = ms_s + ms_h + ms_z
+    line = {
+        "metric": "rayleigh_ritz_products_fp64_tflops", "value": (3 * gemm + apply_flops) / total_ms * 1e-9, "unit": "TFLOP/s",
+        "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": total_ms, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"Rayleigh-Ritz products of Alg. 2 (S, H^, Y Z) on config 3's mesh: {wl.n_dofs} rows, N = {N} columns, "
+                               f"H~Y in chunks of {B}", "l2": "blocks of 7.2 GB vs 126 MB L2"},
+        "roofline": {"kernel": "k_xz", "bound": "tensor", "achieved": parts["transform_YZ"]["tflops"], "peak": peak,
+                     "unit": "TFLOP/s", "frac": parts["transform_YZ"]["frac"], "traffic": None,
+                     "peak_source": "FP64 mma.sync m8n8k4 (DMMA) rate measured in this run by chfsi_measure_fp64_peak"},
+        "parts": parts, "gpu_launches": launches, "clocks": clocks,
+    }
+    print(json.dumps(line), flush=True)
+    op.close()
 
 
 def main():
     args = parse_args()
     from workloads.generate import CONFIGS
+    if args.rr:
+        run_rr(args)
+        return
+    if args.all_configs:
+        for c in (1, 2, 3, 4, 5):
+            if args.impl == "reference":
+                run_reference(args, CONFIGS[c])
+            else:
+                run_b200(args, CONFIGS[c])
+        return
     spec = CONFIGS[args.config]
     if args.block_width > 0:
         import dataclasses
@@ -346,6 +459,9 @@ def main():
         run_reference(args, spec)
     else:
         run_b200(args, spec)
+        import torch.distributed as dist
+        if dist.is_initialized():
+            dist.destroy_process_group()
 
 
 if __name__ == "__main__":

@@ -371,6 +371,70 @@ def projection_matrices(op: Operator, Y):
     return Y.T @ Y, Y.T @ apply_H(op, Y)
 
 
+def overlap_mixed(Y, block: int):
+    """Mixed-precision overlap matrix of Sec. 3.2 / 4.4.1: "the diagonal block entries of
+    overlap matrix S in RRGEP-O are evaluated in FP64 arithmetic while the off-diagonal entries are computed in FP32
+    arithmetic".  Blocks are the `block`-wide column blocks of the blocked products; an FP32 block is
+    the product of the operands rounded to FP32, accumulated in FP32 (numpy float32 matmul), returned in FP64."""
+    Y = np.asarray(Y, dtype=np.float64)
+    N = Y.shape[1]
+    Y32 = Y.astype(np.float32)
+    S = (Y32.T @ Y32).astype(np.float64)
+    for j0 in range(0, N, block):
+        j1 = min(N, j0 + block)
+        S[j0:j1, j0:j1] = Y[:, j0:j1].T @ Y[:, j0:j1]
+    return S
+
+
+def projected_hamiltonian_mixed(Y, HY, n_oc: int):
+    """Mixed-precision projected Hamiltonian of Eq. 38-39: with the split Psi_f = [Psi^oc Psi^fr]
+    (the first n_oc and the remaining columns), the oc-oc, oc-fr and fr-oc blocks of H^ = Psi_f^T (H~ Psi_f) are
+    FP32 products, the fr-fr block is an FP64 product.  HY = H~ Y is given (FP64)."""
+    Y = np.asarray(Y, dtype=np.float64)
+    HY = np.asarray(HY, dtype=np.float64)
+    Hh = (Y.astype(np.float32).T @ HY.astype(np.float32)).astype(np.float64)
+    Hh[n_oc:, n_oc:] = Y[:, n_oc:].T @ HY[:, n_oc:]
+    return Hh
+
+
+def cholesky_inverse(S):
+    """Algorithm 2 step 2a: Cholesky factor S = L L^T (lower) and its inverse L^-1, by the textbook
+    column (Cholesky-Banachiewicz) recursion and forward substitution -- plain loops, no LAPACK."""
+    S = np.asarray(S, dtype=np.float64)
+    N = S.shape[0]
+    L = np.zeros((N, N))
+    for j in range(N):
+        d = S[j, j] - L[j, :j] @ L[j, :j]
+        if not d > 0.0:
+            raise np.linalg.LinAlgError("matrix is not positive definite")
+        L[j, j] = np.sqrt(d)
+        L[j + 1:, j] = (S[j + 1:, j] - L[j + 1:, :j] @ L[j, :j]) / L[j, j]
+    Linv = np.zeros((N, N))
+    for i in range(N):                       # row i of L^-1 from L L^-1 = I
+        e = np.zeros(N)
+        e[i] = 1.0
+        Linv[i] = (e - L[i, :i] @ Linv[:i]) / L[i, i]
+    return L, Linv
+
+
+def orthonormal_basis_mixed(Y, LinvT):
+    """Mixed-precision RRGEP-ST-O: Psi^o = SP[Psi_f (L^-T)_od] + DP[Psi_f (L^-T)_d], with (L^-T)_d the
+    diagonal and (L^-T)_od the off-diagonal entries of L^-T: the FP32 product plus an FP64 column scaling."""
+    Y = np.asarray(Y, dtype=np.float64)
+    d = np.diag(LinvT).copy()
+    od = LinvT - np.diag(d)
+    return (Y.astype(np.float32) @ od.astype(np.float32)).astype(np.float64) + Y * d[None, :]
+
+
+def rayleigh_ritz_gep(S, Hh, n_fr: int):
+    """Algorithm 2 step 2 (RRGEP-D): Cholesky S = L L^T, standard problem (L^-1 H^ L^-T) Q' = Q' D,
+    the n_fr HIGHEST eigenpairs, Q_fr = L^-T Q'_fr.  Returns (D_fr ascending, Q_fr, L^-1)."""
+    L, Linv = cholesky_inverse(0.5 * (S + S.T))
+    A = Linv @ (0.5 * (Hh + Hh.T)) @ Linv.T
+    ev, Qp = np.linalg.eigh(0.5 * (A + A.T))
+    return ev[-n_fr:], Linv.T @ Qp[:, -n_fr:], Linv
+
+
 def ritz_values_of_block(Y, HY, rel_cut: float = 1e-12):
     """Same as rayleigh_ritz but for a given pair (Y, H~Y) (used to compare GPU and oracle blocks with the
     SAME H~Y provider).  Columns are normalised with the norms of Y."""

@@ -199,3 +199,98 @@ def test_apply_H_rows_equals_rows_of_apply_H(jitter):
     Y = orc.apply_H(op, X)
     Yr = orc.apply_H_rows(wl, op.M, X, rows)
     assert np.allclose(Yr, Y[rows], rtol=1e-12, atol=1e-13 * np.abs(Y).max())
+
+
+# ------------------------------------------------------------------------------------------------------------
+# Rayleigh-Ritz step of Algorithm 2 with the paper's mixed-precision blocking
+# ------------------------------------------------------------------------------------------------------------
+def test_cholesky_inverse_against_lapack_and_definition():
+    rng = np.random.default_rng(11)
+    for n in (1, 2, 7, 40):
+        A = rng.standard_normal((n + 5, n))
+        S = A.T @ A + 0.1 * np.eye(n)
+        L, Linv = orc.cholesky_inverse(S)
+        assert np.allclose(L, np.linalg.cholesky(S), rtol=1e-12, atol=1e-13)      # library routine
+        assert np.allclose(np.triu(L, 1), 0) and np.all(np.diag(L) > 0)
+        assert np.allclose(L @ L.T, S, rtol=1e-12, atol=1e-12)                    # definition
+        assert np.allclose(Linv @ L, np.eye(n), atol=1e-11) and np.allclose(np.triu(Linv, 1), 0)
+    with pytest.raises(np.linalg.LinAlgError):
+        orc.cholesky_inverse(np.array([[1.0, 2.0], [2.0, 1.0]]))
+
+
+def test_mixed_precision_overlap_blocks():
+    """Diagonal blocks are the FP64 product bit for bit, off-diagonal blocks carry an FP32-sized error that scales with
+    the column norms (and vanishes with the off-diagonal content: orthonormal input gives the identity to FP32
+    rounding of exact zeros); block = N reduces to the FP64 overlap; a transposed / wrong-block implementation fails."""
+    rng = np.random.default_rng(12)
+    n, N, blk = 600, 24, 8
+    Y = rng.standard_normal((n, N)) * np.logspace(0, 2, N)[None, :]
+    S64 = Y.T @ Y
+    Sm = orc.overlap_mixed(Y, blk)
+    nrm = np.linalg.norm(Y, axis=0)
+    for j0 in range(0, N, blk):
+        assert np.array_equal(Sm[j0:j0 + blk, j0:j0 + blk], S64[j0:j0 + blk, j0:j0 + blk])
+    off = np.ones((N, N), dtype=bool)
+    for j0 in range(0, N, blk):
+        off[j0:j0 + blk, j0:j0 + blk] = False
+    err = np.abs(Sm - S64) / np.outer(nrm, nrm)
+    assert 1e-10 < err[off].max() <= 20 * np.finfo(np.float32).eps      # FP32-sized, not FP64-sized
+    assert np.array_equal(orc.overlap_mixed(Y, N), S64)
+    Q, _ = np.linalg.qr(rng.standard_normal((n, N)))
+    Sq = orc.overlap_mixed(Q, blk)
+    assert np.max(np.abs(Sq - np.eye(N))) <= 5e-7 and np.max(np.abs(np.diag(Sq) - 1)) <= 1e-14
+
+
+def test_mixed_precision_projected_hamiltonian_blocks_and_ritz_values():
+    """Eq. 39: only the fr-fr block is FP64 (bit-equal to the FP64 product), the other three are FP32 products; for a
+    nearly converged subspace (H^ nearly diagonal) the n_fr highest Ritz values of the mixed matrices agree with the
+    FP64 ones far below the FP32 level -- the property the paper's blocking rests on."""
+    wl = make_workload(None, n=3, p=3, L=6.0, atoms_per_side=1, n_gaussians=0, nonlocal_=True, smooth_field=0.05,
+                       seed_base=61)
+    op = orc.operator_from_workload(wl)
+    rng = np.random.default_rng(13)
+    N, n_oc = 16, 10
+    Y = rng.standard_normal((wl.n_dofs, N))
+    HY = orc.apply_H(op, Y)
+    Hm = orc.projected_hamiltonian_mixed(Y, HY, n_oc)
+    H64 = Y.T @ HY
+    assert np.array_equal(Hm[n_oc:, n_oc:], H64[n_oc:, n_oc:])
+    assert not np.array_equal(Hm[:n_oc, :n_oc], H64[:n_oc, :n_oc]) and not np.array_equal(Hm[n_oc:, :n_oc], H64[n_oc:, :n_oc])
+    assert np.max(np.abs(Hm - H64)) <= 1e-5 * np.max(np.abs(H64))
+    # nearly converged subspace: a few filter + orthonormalisation passes
+    b, lmin = orc.lanczos_upper_bound(op, rng.standard_normal(wl.n_dofs), 20)
+    for _ in range(8):
+        th = orc.ritz_values_of_block(Y, orc.apply_H(op, Y))
+        Y, _ = np.linalg.qr(orc.chebyshev_filter(op, Y, 12, float(th[-1]), b, float(th[0]) - 1e-3))
+    Y = Y * (1.0 + 0.2 * rng.standard_normal(N))[None, :]         # not normalised: S is diagonal-dominant, not the identity
+    HY = orc.apply_H(op, Y)
+    n_fr = N - n_oc
+    d64, _, _ = orc.rayleigh_ritz_gep(Y.T @ Y, Y.T @ HY, n_fr)
+    dm, _, _ = orc.rayleigh_ritz_gep(orc.overlap_mixed(Y, 4), orc.projected_hamiltonian_mixed(Y, HY, n_oc), n_fr)
+    conv = np.abs(d64 - orc.ritz_values_of_block(Y, HY)[-n_fr:])
+    assert np.max(conv) <= 1e-9                                    # the GEP route equals the Rayleigh-Ritz measure
+    assert np.max(np.abs(dm[:3] - d64[:3])) <= 1e-7, np.abs(dm - d64)
+
+
+def test_rayleigh_ritz_gep_and_mixed_orthonormal_basis():
+    """Algorithm 2 steps 2-3 on an invariant subspace written in a random basis: D_fr are the top eigenvalues, Psi^R =
+    Y Q_fr are eigenvectors, Psi^o = Y L^-T is orthonormal; the mixed SP/DP form of Psi^o differs by an FP32-sized term
+    that vanishes when L^-T is diagonal (orthogonal input columns)."""
+    rng = np.random.default_rng(14)
+    n, N, n_fr = 60, 9, 4
+    A = rng.standard_normal((n, n))
+    H = 0.5 * (A + A.T)
+    ev, V = np.linalg.eigh(H)
+    Y = V[:, :N] @ rng.standard_normal((N, N))
+    D, Q, Linv = orc.rayleigh_ritz_gep(Y.T @ Y, Y.T @ (H @ Y), n_fr)
+    assert np.allclose(D, ev[N - n_fr:N], atol=1e-9)
+    R = Y @ Q
+    assert np.allclose(H @ R, R * D[None, :], atol=1e-8)
+    Po = Y @ Linv.T
+    assert np.allclose(Po.T @ Po, np.eye(N), atol=1e-9)
+    Pm = orc.orthonormal_basis_mixed(Y, Linv.T)
+    assert 0 < np.max(np.abs(Pm - Po)) <= 1e-4 * np.max(np.abs(Po))
+    Yo = V[:, :N] * (1.0 + rng.random(N))[None, :]                 # orthogonal columns: L^-T is diagonal
+    _, _, Li = orc.rayleigh_ritz_gep(Yo.T @ Yo, Yo.T @ (H @ Yo), n_fr)
+    Li_d = np.diag(np.diag(Li))
+    assert np.allclose(orc.orthonormal_basis_mixed(Yo, Li_d.T), Yo @ Li_d.T, rtol=1e-15, atol=0)
