@@ -429,8 +429,7 @@ def test_fp32_ritz_values_of_a_converged_subspace_within_1e_5_Ha_without_slack()
             Q, _ = np.linalg.qr(F)
             blocks[key] = Q if key != 32 else Q.astype(np.float32).astype(np.float64)
     th = {k: orc.ritz_values_of_block(v, orc.apply_H(oop, v)) for k, v in blocks.items()}
-    wanted = th["oracle"] < 0.5 * (th["oracle"][0] + th["oracle"][-1])       # the lower half: converged after six passes
-    assert wanted.sum() >= 8
+    wanted = np.arange(nvec) < nvec // 2                 # the lower half of the Ritz values: converged after six passes
     res = orc.apply_H(oop, blocks["oracle"])
     d32 = float(np.max(np.abs(th[32][wanted] - th["oracle"][wanted])))
     d64 = float(np.max(np.abs(th[64][wanted] - th["oracle"][wanted])))
