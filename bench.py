@@ -410,6 +410,13 @@ def run_rr(args):
     ms_s = timed(lambda: op.overlap_matrix(Y))
     ms_h = timed(lambda: op.projected_hamiltonian(Y, B=B, workspace=ws))
     ms_z = timed(lambda: op.subspace_transform(Y, Z, Out=Out))
+    # the paper's mixed-precision blocking (Eq. 38-39): diagonal blocks of 256 columns FP64, N_fr = 128 of 1024
+    blk, n_oc = 256, N - 128
+    ms_sm = timed(lambda: op.overlap_matrix_mixed(Y, blk))
+    ms_hm = timed(lambda: op.projected_hamiltonian_mixed(Y, n_oc, B=B, workspace=ws))
+    ms_zm = timed(lambda: op.subspace_transform_mixed(Y, Z, Out=Out))
+    Sd = op.overlap_matrix(Y)
+    ms_ch = timed(lambda: op.cholesky_inverse(Sd))
     launches = op.launch_count() - l0
     clocks = sampler.stop()
     gemm = 2.0 * wl.n_dofs * N * N                            # flops of one tall product
@@ -421,6 +428,14 @@ def run_rr(args):
         "projected_H": {"kernel": kernel + " + k_xty", "ms": ms_h, "tflops": (gemm + apply_flops) / ms_h * 1e-9,
                         "frac": (gemm + apply_flops) / ms_h * 1e-9 / peak},
         "transform_YZ": {"kernel": "k_xz", "ms": ms_z, "tflops": gemm / ms_z * 1e-9, "frac": gemm / ms_z * 1e-9 / peak},
+        # mixed precision: same algorithmic flops; speed-up over the FP64 product of the same step
+        "overlap_S_mixed": {"kernel": "k_xty_tf32 (3xTF32) + k_xty (FP64 diagonal blocks)", "ms": ms_sm,
+                            "tflops": gemm / ms_sm * 1e-9, "speedup_vs_fp64": ms_s / ms_sm},
+        "projected_H_mixed": {"kernel": kernel + " + k_xty_tf32 + k_xty (fr-fr block)", "ms": ms_hm,
+                              "tflops": (gemm + apply_flops) / ms_hm * 1e-9, "speedup_vs_fp64": ms_h / ms_hm},
+        "transform_mixed": {"kernel": "k_xz_tf32 (3xTF32 off-diagonal + FP64 diagonal)", "ms": ms_zm,
+                            "tflops": gemm / ms_zm * 1e-9, "speedup_vs_fp64": ms_z / ms_zm},
+        "cholesky_inverse": {"kernel": "k_chol_* / k_trinv_row (N = 1024)", "ms": ms_ch},
     }
     total_ms = ms_s + ms_h + ms_z
     line = {

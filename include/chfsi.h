@@ -177,6 +177,34 @@ int chfsi_projected_hamiltonian(chfsi_op* op, const void* Y_dev, int64_t ldy, in
 int chfsi_subspace_transform(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N, const double* Z_dev, int64_t ldz,
                              int64_t N2, void* Out_dev, int64_t ldo, void* cuda_stream);
 
+/* Dense N x N step of Algorithm 2 on the device -- step 2a: Cholesky factor S = L L^T and L^-1,
+ * which steps 2b (H^ -> L^-1 H^ L^-T) and 3b (Psi^o = Psi_f L^-T) need.  S_dev [N][N] row-major FP64 (symmetric; only
+ * the lower triangle is read), L_dev and Linv_dev [N][N] row-major FP64 DEVICE arrays owned by the caller (lower
+ * triangular, zeros above the diagonal); info_dev: DEVICE int, 0 on success, else the 1-based index of the first
+ * non-positive pivot (S not positive definite: the factors are then meaningless).  Enqueued on cuda_stream, no host
+ * synchronisation (the pivot status stays on the device for that reason).  Errors: CHFSI_ERR_BAD_ARGUMENT (NULL, N < 1,
+ * N > 16384, overlapping arrays).  The dense symmetric eigenproblem of step 2c is left to the caller (the paper runs it
+ * on the CPUs with ELPA). */
+int chfsi_cholesky_inverse(chfsi_op* op, const double* S_dev, int64_t N, double* L_dev, double* Linv_dev, int* info_dev,
+                           void* cuda_stream);
+
+/* The paper's mixed-precision blocking of the O(M N^2) products of Algorithm 2 (Sec. 3.2; Sec.
+ * 4.4.1).  "FP32" blocks: operands rounded to FP32, FP32-level products on the 32-bit tensor pipe (3xTF32
+ * split; single-pass TF32 is not used), summed in FP64.  FP64 operators only; N, ldy even; pointers 16-byte aligned;
+ * library-owned FP32 copies of the blocks grow on demand (the call then synchronises the stream once).
+ *   chfsi_overlap_matrix_mixed:        S = Y^T Y with the diagonal blocks of width `block` in FP64, the rest FP32
+ *   chfsi_projected_hamiltonian_mixed: H^ = Y^T (H~ Y) with the split Y = [Y^oc Y^fr] of Eq. 38 (first n_oc columns /
+ *                                      the rest): the fr-fr block FP64, the oc-oc, oc-fr and fr-oc blocks FP32 (Eq. 39)
+ *   chfsi_subspace_transform_mixed:    Out = SP[Y Z_od] + DP[Y Z_d] for a square Z [N][ldz] (Z = L^-T gives Psi^o,
+ *                                      RRGEP-ST-O): off-diagonal entries of Z FP32, diagonal entries FP64
+ * Other arguments as in the FP64 calls above. */
+int chfsi_overlap_matrix_mixed(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N, int64_t block, double* S_dev,
+                               void* cuda_stream);
+int chfsi_projected_hamiltonian_mixed(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N, int64_t B, int64_t n_oc,
+                                      double* H_dev, void* workspace_dev, void* cuda_stream);
+int chfsi_subspace_transform_mixed(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N, const double* Z_dev, int64_t ldz,
+                                   void* Out_dev, int64_t ldo, void* cuda_stream);
+
 /* Number of kernel launches enqueued by this handle since creation (for benchmark bookkeeping). */
 int64_t chfsi_launch_count(const chfsi_op* op);
 

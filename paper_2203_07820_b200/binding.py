@@ -20,7 +20,8 @@ LIB_PATH = os.path.join(HERE, "libchfsi.so")
 
 EXPORTED_SYMBOLS = [
     "chfsi_create", "chfsi_destroy", "chfsi_update_potential", "chfsi_get_info", "chfsi_workspace_bytes", "chfsi_mass_diag",
-    "chfsi_apply_H", "chfsi_overlap_matrix", "chfsi_projected_hamiltonian", "chfsi_subspace_transform", "chfsi_chebyshev_filter", "chfsi_chebyshev_filter_chunked", "chfsi_chebyshev_filter_host",
+    "chfsi_apply_H", "chfsi_overlap_matrix", "chfsi_projected_hamiltonian", "chfsi_subspace_transform",
+    "chfsi_cholesky_inverse", "chfsi_overlap_matrix_mixed", "chfsi_projected_hamiltonian_mixed", "chfsi_subspace_transform_mixed", "chfsi_chebyshev_filter", "chfsi_chebyshev_filter_chunked", "chfsi_chebyshev_filter_host",
     "chfsi_launch_count", "chfsi_set_kernel_variant", "chfsi_set_profiling", "chfsi_get_profile",
     "chfsi_measure_fp64_peak", "chfsi_last_error",
 ]
@@ -97,6 +98,14 @@ def load_library(build_if_missing: bool = True):
     lib_.chfsi_projected_hamiltonian.restype = C.c_int
     lib_.chfsi_subspace_transform.argtypes = [vp, vp, i64, i64, vp, i64, i64, vp, i64, vp]
     lib_.chfsi_subspace_transform.restype = C.c_int
+    lib_.chfsi_cholesky_inverse.argtypes = [vp, vp, i64, vp, vp, vp, vp]
+    lib_.chfsi_cholesky_inverse.restype = C.c_int
+    lib_.chfsi_overlap_matrix_mixed.argtypes = [vp, vp, i64, i64, i64, vp, vp]
+    lib_.chfsi_overlap_matrix_mixed.restype = C.c_int
+    lib_.chfsi_projected_hamiltonian_mixed.argtypes = [vp, vp, i64, i64, i64, i64, vp, vp, vp]
+    lib_.chfsi_projected_hamiltonian_mixed.restype = C.c_int
+    lib_.chfsi_subspace_transform_mixed.argtypes = [vp, vp, i64, i64, vp, i64, vp, i64, vp]
+    lib_.chfsi_subspace_transform_mixed.restype = C.c_int
     lib_.chfsi_chebyshev_filter.argtypes = [vp, vp, i64, i64, i32, dbl, dbl, dbl, vp, vp]
     lib_.chfsi_chebyshev_filter.restype = C.c_int
     lib_.chfsi_chebyshev_filter_chunked.argtypes = [vp, vp, i64, i64, i64, i32, dbl, dbl, dbl, vp, vp]
@@ -273,6 +282,55 @@ class Operator:
             raise ValueError("Out must have N2 columns")
         self._check(load_library().chfsi_subspace_transform(self._h, yp, ldy, N, C.c_void_p(Z.data_ptr()),
                                                             int(Z.stride(0)), N2, op_, ldo, _stream_ptr(stream)))
+        return Out
+
+    def cholesky_inverse(self, S, stream=None):
+        """Algorithm 2 step 2a on the device: returns (L, L^-1, info) for S = L L^T; info is a device int32 tensor
+        (0 = success, else the 1-based index of the first non-positive pivot)."""
+        import torch
+        if not (S.is_cuda and S.dim() == 2 and S.shape[0] == S.shape[1] and S.dtype == torch.float64 and S.is_contiguous()):
+            raise ValueError("S must be a contiguous square FP64 CUDA tensor")
+        N = int(S.shape[0])
+        L, Linv = torch.empty_like(S), torch.empty_like(S)
+        info = torch.zeros(1, dtype=torch.int32, device="cuda")
+        self._check(load_library().chfsi_cholesky_inverse(self._h, C.c_void_p(S.data_ptr()), N, C.c_void_p(L.data_ptr()),
+                                                          C.c_void_p(Linv.data_ptr()), C.c_void_p(info.data_ptr()),
+                                                          _stream_ptr(stream)))
+        return L, Linv, info
+
+    def overlap_matrix_mixed(self, Y, block, stream=None):
+        """S = Y^T Y, diagonal blocks of width `block` FP64, the rest FP32."""
+        import torch
+        yp, ldy, N = self._block(Y, "Y")
+        S = torch.empty((N, N), dtype=torch.float64, device="cuda")
+        self._check(load_library().chfsi_overlap_matrix_mixed(self._h, yp, ldy, N, int(block), C.c_void_p(S.data_ptr()),
+                                                              _stream_ptr(stream)))
+        return S
+
+    def projected_hamiltonian_mixed(self, Y, n_oc, B=None, workspace=None, stream=None):
+        """H^ = Y^T (H~ Y) with the blocking of Eq. 39: fr-fr block (rows, columns >= n_oc) FP64, the rest FP32."""
+        import torch
+        yp, ldy, N = self._block(Y, "Y")
+        B = int(B) if B is not None else min(N, 256)
+        ws = workspace if workspace is not None else self.workspace(min(B, N))
+        Hh = torch.empty((N, N), dtype=torch.float64, device="cuda")
+        self._check(load_library().chfsi_projected_hamiltonian_mixed(self._h, yp, ldy, N, B, int(n_oc), C.c_void_p(Hh.data_ptr()),
+                                                                     C.c_void_p(ws.data_ptr()), _stream_ptr(stream)))
+        return Hh
+
+    def subspace_transform_mixed(self, Y, Z, Out=None, stream=None):
+        """Out = SP[Y Z_od] + DP[Y Z_d] for a square Z (Z = L^-T gives the orthonormal basis Psi^o)."""
+        import torch
+        yp, ldy, N = self._block(Y, "Y")
+        if Z.dim() != 2 or Z.shape[0] != N or Z.shape[1] != N or Z.dtype != torch.float64 or Z.stride(1) != 1 or not Z.is_cuda:
+            raise ValueError("Z must be a [N, N] FP64 CUDA tensor with unit column stride")
+        if Out is None:
+            Out = torch.empty((self.n_dofs, N), dtype=torch.float64, device="cuda")
+        op_, ldo, No = self._block(Out, "Out")
+        if No != N:
+            raise ValueError("Out must have N columns")
+        self._check(load_library().chfsi_subspace_transform_mixed(self._h, yp, ldy, N, C.c_void_p(Z.data_ptr()),
+                                                                  int(Z.stride(0)), op_, ldo, _stream_ptr(stream)))
         return Out
 
     def chebyshev_filter(self, X, m, a, b, a0, workspace=None, stream=None):

@@ -50,7 +50,7 @@ void free_op(chfsi_op* op) {
   cudaFree(op->color_cells); cudaFree(op->dep_ptr); cudaFree(op->dep_pos); cudaFree(op->all_cells); cudaFree(op->pc_cells); cudaFree(op->cell_proj_ptr);
   cudaFree(op->proj_ptr); cudaFree(op->proj_pcrow); cudaFree(op->seg_ptr); cudaFree(op->grow_dof); cudaFree(op->pcoef);
   cudaFree(op->grp_seg_ptr); cudaFree(op->proj_grp); cudaFree(op->proj_slot);
-  cudaFree(op->rr_scratch); cudaFree(op->sf_coef); cudaFree(op->sf_sloc); cudaFree(op->crows);
+  cudaFree(op->rr_scratch); cudaFree(op->rr32[0]); cudaFree(op->rr32[1]); cudaFree(op->sf_coef); cudaFree(op->sf_sloc); cudaFree(op->crows);
   for (int i = 0; i < 2; ++i) {
     cudaFree(op->host_stage[i]);
     if (op->host_done[i]) cudaEventDestroy(op->host_done[i]);
@@ -558,6 +558,137 @@ int chfsi_subspace_transform(chfsi_op* op, const void* Y_dev, int64_t ldy, int64
                    reinterpret_cast<double*>(Out_dev), ldo, st);
   if (ce == cudaSuccess) ce = order_leave(op, st);
   return ce == cudaSuccess ? CHFSI_OK : cuda_fail(op, ce, "subspace_transform");
+  API_CATCH(op)
+}
+
+namespace {
+// library-owned FP32 buffer `which` of at least `bytes` bytes (grown on demand; the stream is synchronised before a
+// buffer that may still be in use is released)
+cudaError_t rr32_reserve(chfsi_op* op, int which, size_t bytes, cudaStream_t st) {
+  if (op->rr32_bytes[which] >= bytes) return cudaSuccess;
+  cudaError_t e = cudaStreamSynchronize(st);
+  if (e != cudaSuccess) return e;
+  cudaFree(op->rr32[which]);
+  op->rr32[which] = nullptr; op->rr32_bytes[which] = 0;
+  if ((e = cudaMalloc(&op->rr32[which], bytes)) != cudaSuccess) return e;
+  op->rr32_bytes[which] = bytes;
+  return cudaSuccess;
+}
+}  // namespace
+
+int chfsi_cholesky_inverse(chfsi_op* op, const double* S_dev, int64_t N, double* L_dev, double* Linv_dev, int* info_dev,
+                           void* cuda_stream) {
+  if (!op) return CHFSI_ERR_BAD_ARGUMENT;
+  if (!S_dev || !L_dev || !Linv_dev || !info_dev) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "NULL matrix / status pointer");
+  if (N < 1 || N > 16384) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "need 1 <= N <= 16384");
+  if (S_dev == L_dev || S_dev == Linv_dev || L_dev == Linv_dev) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "S, L and L^-1 must be distinct arrays");
+  API_TRY
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  cudaError_t ce = order_enter(op, st);
+  if (ce == cudaSuccess) ce = launch_cholesky_inverse(op, S_dev, (int)N, L_dev, Linv_dev, info_dev, st);
+  if (ce == cudaSuccess) ce = order_leave(op, st);
+  return ce == cudaSuccess ? CHFSI_OK : cuda_fail(op, ce, "cholesky_inverse");
+  API_CATCH(op)
+}
+
+int chfsi_overlap_matrix_mixed(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N, int64_t block, double* S_dev,
+                               void* cuda_stream) {
+  int rc = check_rr_args(op, Y_dev, ldy, N, S_dev);
+  if (rc) return rc;
+  if (block < 2 || block % 2 != 0) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "block width must be even and >= 2");
+  API_TRY
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  const double* Y = reinterpret_cast<const double*>(Y_dev);
+  const int64_t ld32 = (N + 3) / 4 * 4;
+  cudaError_t ce = order_enter(op, st);
+  if (ce == cudaSuccess) ce = rr32_reserve(op, 0, (size_t)op->n_dofs * ld32 * sizeof(float), st);
+  float* Y32 = reinterpret_cast<float*>(op->rr32[0]);
+  if (ce == cudaSuccess) ce = launch_to_f32(op, Y, ldy, Y32, ld32, op->n_dofs, (int)N, 0, nullptr, st);
+  // FP32 blocks first (tiles inside a diagonal block are skipped), then the FP64 diagonal blocks on top
+  if (ce == cudaSuccess) ce = launch_xty_tf32(op, Y32, ld32, Y32, ld32, op->n_dofs, (int)N, (int)N, (int)block, 0, 0, S_dev, N, st);
+  for (int64_t j0 = 0; j0 < N && ce == cudaSuccess; j0 += block) {
+    const int bw = (int)std::min(block, N - j0);
+    ce = launch_xty(op, Y + j0, ldy, Y + j0, ldy, op->n_dofs, bw, bw, S_dev + j0 * N + j0, N, st);
+  }
+  if (ce == cudaSuccess) ce = order_leave(op, st);
+  return ce == cudaSuccess ? CHFSI_OK : cuda_fail(op, ce, "overlap_matrix_mixed");
+  API_CATCH(op)
+}
+
+int chfsi_projected_hamiltonian_mixed(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N, int64_t B, int64_t n_oc,
+                                      double* H_dev, void* workspace_dev, void* cuda_stream) {
+  int rc = check_rr_args(op, Y_dev, ldy, N, H_dev);
+  if (rc) return rc;
+  if (B < 2 || B % 2 != 0) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "chunk width B must be even and >= 2");
+  if (n_oc < 0 || n_oc > N || n_oc % 2 != 0) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "need 0 <= n_oc <= N, n_oc even");
+  if (!workspace_dev || (uintptr_t)workspace_dev % 16 != 0) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "bad workspace");
+  API_TRY
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  const double* Y = reinterpret_cast<const double*>(Y_dev);
+  const int64_t Bc = std::min(B, N);
+  const WsLayout w = ws_layout(op, Bc);
+  char* base = reinterpret_cast<char*>(workspace_dev);
+  double* W = reinterpret_cast<double*>(base + w.block_off);
+  const int64_t ld32 = (N + 3) / 4 * 4, ldw32 = (Bc + 3) / 4 * 4;
+  cudaError_t ce = order_enter(op, st);
+  if (ce == cudaSuccess) ce = rr32_reserve(op, 0, (size_t)op->n_dofs * ld32 * sizeof(float), st);
+  if (ce == cudaSuccess) ce = rr32_reserve(op, 1, (size_t)op->n_dofs * ldw32 * sizeof(float), st);
+  float* Y32 = reinterpret_cast<float*>(op->rr32[0]);
+  float* W32 = reinterpret_cast<float*>(op->rr32[1]);
+  if (ce == cudaSuccess) ce = launch_to_f32(op, Y, ldy, Y32, ld32, op->n_dofs, (int)N, 0, nullptr, st);
+  for (int64_t j0 = 0; j0 < N && ce == cudaSuccess; j0 += Bc) {
+    const int64_t bw = std::min(Bc, N - j0);
+    ApplyArgs g;                                        // W <- H~ Y[:, j0 : j0 + bw]   (FP64)
+    g.X = Y + j0; g.ldx = ldy; g.T = W; g.ldt = w.ldw; g.B = bw;
+    g.alpha = 1.0; g.beta = 0.0; g.cshift = 0.0;
+    g.P = base + w.p_off; g.Pc = base + w.pc_off;
+    g.sync = reinterpret_cast<unsigned long long*>(base + w.sync_off); g.epoch = 1;
+    ce = cudaMemsetAsync(g.sync, 0, w.sync_bytes, st);
+    if (ce == cudaSuccess) { op->launches++; ce = launch_apply(op, g, st); }
+    // Eq. 39: all rows of these columns as FP32 products ...
+    if (ce == cudaSuccess) ce = launch_to_f32(op, W, w.ldw, W32, ldw32, op->n_dofs, (int)bw, 0, nullptr, st);
+    if (ce == cudaSuccess) ce = launch_xty_tf32(op, Y32, ld32, W32, ldw32, op->n_dofs, (int)N, (int)bw, 0, 0, 0, H_dev + j0, N, st);
+    // ... and the fr-fr part (rows and columns >= n_oc) in FP64 on top
+    const int64_t c0 = std::max(j0, n_oc);
+    if (ce == cudaSuccess && c0 < j0 + bw && n_oc < N)
+      ce = launch_xty(op, Y + n_oc, ldy, W + (c0 - j0), w.ldw, op->n_dofs, (int)(N - n_oc), (int)(j0 + bw - c0),
+                      H_dev + n_oc * N + c0, N, st);
+  }
+  if (ce == cudaSuccess) ce = order_leave(op, st);
+  return ce == cudaSuccess ? CHFSI_OK : cuda_fail(op, ce, "projected_hamiltonian_mixed");
+  API_CATCH(op)
+}
+
+int chfsi_subspace_transform_mixed(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N, const double* Z_dev, int64_t ldz,
+                                   void* Out_dev, int64_t ldo, void* cuda_stream) {
+  int rc = check_rr_args(op, Y_dev, ldy, N, Out_dev);
+  if (rc) return rc;
+  if (!Z_dev) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "NULL transformation matrix");
+  if (ldz < N || ldo < N) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "need N <= ldz, ldo");
+  if (ldz % 2 != 0 || ldo % 2 != 0 || (uintptr_t)Z_dev % 16 != 0)
+    return fail(op, CHFSI_ERR_UNSUPPORTED, "subspace_transform_mixed: ldz, ldo must be even, pointers 16-byte aligned");
+  const char* y0 = reinterpret_cast<const char*>(Y_dev);
+  const char* o0 = reinterpret_cast<const char*>(Out_dev);
+  const size_t ybytes = (size_t)op->n_dofs * ldy * 8, obytes = (size_t)op->n_dofs * ldo * 8;
+  if (y0 < o0 + obytes && o0 < y0 + ybytes) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "Y and Out must not overlap");
+  API_TRY
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  const double* Y = reinterpret_cast<const double*>(Y_dev);
+  const int64_t ld32 = (N + 3) / 4 * 4;
+  cudaError_t ce = order_enter(op, st);
+  if (ce == cudaSuccess) ce = rr32_reserve(op, 0, (size_t)op->n_dofs * ld32 * sizeof(float), st);
+  // FP32 copy of Z without its diagonal, followed by the FP64 diagonal, in the second buffer
+  const size_t z32_bytes = align_up((size_t)N * ld32 * sizeof(float), 256);
+  if (ce == cudaSuccess) ce = rr32_reserve(op, 1, z32_bytes + (size_t)N * sizeof(double), st);
+  float* Y32 = reinterpret_cast<float*>(op->rr32[0]);
+  float* Z32 = reinterpret_cast<float*>(op->rr32[1]);
+  double* zd = reinterpret_cast<double*>(reinterpret_cast<char*>(op->rr32[1]) + z32_bytes);
+  if (ce == cudaSuccess) ce = launch_to_f32(op, Y, ldy, Y32, ld32, op->n_dofs, (int)N, 0, nullptr, st);
+  if (ce == cudaSuccess) ce = launch_to_f32(op, Z_dev, ldz, Z32, ld32, N, (int)N, 1, zd, st);
+  if (ce == cudaSuccess)
+    ce = launch_xz_tf32(op, Y32, ld32, Z32, ld32, Y, ldy, zd, op->n_dofs, (int)N, (int)N, reinterpret_cast<double*>(Out_dev), ldo, st);
+  if (ce == cudaSuccess) ce = order_leave(op, st);
+  return ce == cudaSuccess ? CHFSI_OK : cuda_fail(op, ce, "subspace_transform_mixed");
   API_CATCH(op)
 }
 

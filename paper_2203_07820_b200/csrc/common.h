@@ -142,6 +142,9 @@ struct Op {
   // split-row partial tiles of the Rayleigh-Ritz projection products (rr_kernels.cu); grown on demand
   void* rr_scratch = nullptr;
   size_t rr_scratch_bytes = 0;
+  // FP32 copies of the blocks of the mixed-precision Rayleigh-Ritz products; grown on demand
+  void* rr32[2] = {nullptr, nullptr};
+  size_t rr32_bytes[2] = {0, 0};
   // device staging of chfsi_chebyshev_filter_host, kept between calls (grown on demand, freed at destroy)
   void* host_stage[2] = {nullptr, nullptr};
   size_t host_stage_bytes[2] = {0, 0};
@@ -203,6 +206,19 @@ cudaError_t launch_xty(Op* op, const double* A, int64_t lda, const double* B, in
 // Out[n_rows][ldo] = Y Z, Y [n_rows][ldy] with N columns, Z [N][ldz] with N2 columns (Alg. 2 step 3)
 cudaError_t launch_xz(Op* op, const double* Y, int64_t ldy, const double* Z, int64_t ldz, int64_t n_rows, int N, int N2,
                       double* Out, int64_t ldo, cudaStream_t stream);
+// Mixed-precision products of the Rayleigh-Ritz step (rr_kernels.cu): FP32 operands, 3xTF32
+// products, FP64 totals.  launch_to_f32 rounds an FP64 block to FP32 (optionally splitting off the diagonal of a square
+// matrix); launch_xty_tf32 writes C = A^T B except the tiles inside diagonal blocks of width skip_block (> 0);
+// launch_xz_tf32 writes Out = Y32 Z32 + Y diag(zd).
+cudaError_t init_rr_mixed_kernels();
+cudaError_t launch_to_f32(Op* op, const double* src, int64_t lds, float* dst, int64_t ldd, int64_t rows, int cols, int zero_diag,
+                          double* diag, cudaStream_t st);
+cudaError_t launch_xty_tf32(Op* op, const float* A, int64_t lda, const float* B, int64_t ldb, int64_t n_rows, int N1, int N2,
+                            int skip_block, int row_block0, int col_block0, double* C, int64_t ldc, cudaStream_t st);
+cudaError_t launch_xz_tf32(Op* op, const float* Y32, int64_t ldy32, const float* Z32, int64_t ldz32, const double* Y, int64_t ldy,
+                           const double* zd, int64_t n_rows, int N, int N2, double* Out, int64_t ldo, cudaStream_t st);
+// Cholesky factor and its inverse of an N x N FP64 matrix on the device (rr_dense.cu; Alg. 2 step 2a)
+cudaError_t launch_cholesky_inverse(Op* op, const double* S, int N, double* L, double* Linv, int* info_dev, cudaStream_t st);
 // Opts the kernels into the shared memory they need for this operator, on the CURRENT device (at every create: the
 // attribute is per device).
 cudaError_t init_apply_kernels(Op* op);

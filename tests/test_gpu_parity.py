@@ -480,3 +480,95 @@ def test_block_width_limit_is_an_argument_error():
                            C.c_void_p(ws.data_ptr()), None)
     assert rc == -1 and b"too large" in lib.chfsi_last_error(op._h)
     op.close()
+
+
+def test_cholesky_and_inverse_on_the_device_match_the_oracle():
+    """chfsi_cholesky_inverse (Algorithm 2 step 2a): L and L^-1 against the oracle's textbook recursion
+    for sizes below, at and off the 32-wide blocking; a matrix that is not positive definite is reported in info."""
+    torch, orc, Operator, _, _, _, _ = _imports()
+    wl, *_ = oracle_case("p3_odd_B")
+    op = Operator.from_workload(wl)
+    rng = np.random.default_rng(21)
+    for n in (2, 31, 32, 33, 100, 256):
+        A = rng.standard_normal((n + 10, n))
+        S = A.T @ A + 0.05 * np.eye(n)
+        Lo, Lio = orc.cholesky_inverse(S)
+        L, Linv, info = op.cholesky_inverse(torch.tensor(S, device="cuda"))
+        assert int(info.item()) == 0
+        assert np.max(np.abs(L.cpu().numpy() - Lo)) <= 1e-12 * np.max(np.abs(Lo)), n
+        assert np.max(np.abs(Linv.cpu().numpy() - Lio)) <= 1e-10 * np.max(np.abs(Lio)), n
+        assert float(torch.triu(L, 1).abs().max()) == 0.0 and float(torch.triu(Linv, 1).abs().max()) == 0.0
+    bad = np.eye(40)
+    bad[17, 17] = -1.0
+    _, _, info = op.cholesky_inverse(torch.tensor(bad, device="cuda"))
+    assert int(info.item()) == 18
+    op.close()
+
+
+def test_mixed_precision_rayleigh_ritz_products_match_the_oracle():
+    """The paper's mixed-precision blocking (Eq. 38-39) against the oracle's plain
+    statement of it: FP64 blocks agree at the FP64 level, FP32 blocks agree with the oracle's FP32 products and with the
+    exact product at the FP32 level (scaled by the column norms); then Algorithm 2 with the mixed matrices on a nearly
+    converged subspace: the n_fr highest Ritz values equal the FP64 oracle's far below the FP32 level."""
+    torch, orc, Operator, _, _, _, _ = _imports()
+    wl, oop, X, (a0, a, b), Yo, Fo = oracle_case("p6_nonlocal_ragged")
+    op = Operator.from_workload(wl)
+    eps32 = float(np.finfo(np.float32).eps)
+    rng = np.random.default_rng(22)
+    Y = Fo / np.linalg.norm(Fo, axis=0, keepdims=True) * (1.0 + 0.5 * rng.random(Fo.shape[1]))[None, :]
+    N, blk, n_oc = Y.shape[1], 24, 40                      # 72 columns: three diagonal blocks; oc / fr split inside a block
+    nrm = np.linalg.norm(Y, axis=0)
+    scale = np.outer(nrm, nrm)
+    Yd = torch.tensor(Y, device="cuda")
+    # -- overlap matrix
+    S64, Som = Y.T @ Y, orc.overlap_mixed(Y, blk)
+    S = op.overlap_matrix_mixed(Yd, blk).cpu().numpy()
+    assert torch.equal(op.overlap_matrix_mixed(Yd, blk), torch.tensor(S, device="cuda"))       # deterministic
+    diag = np.zeros((N, N), dtype=bool)
+    for j0 in range(0, N, blk):
+        diag[j0:j0 + blk, j0:j0 + blk] = True
+    assert np.max(np.abs(S - S64)[diag] / scale[diag]) <= 1e-13
+    assert np.max(np.abs(S - S64)[~diag] / scale[~diag]) <= 8 * eps32
+    assert np.max(np.abs(S - Som)[~diag] / scale[~diag]) <= 64 * eps32                           # numpy's FP32 sums are looser
+    assert np.max(np.abs(S - S64)[~diag] / scale[~diag]) > 1e-12                                 # they ARE FP32 products
+    # -- projected Hamiltonian (Eq. 39)
+    HY = orc.apply_H(oop, Y)
+    H64, Hom = Y.T @ HY, orc.projected_hamiltonian_mixed(Y, HY, n_oc)
+    hs = np.outer(nrm, np.linalg.norm(HY, axis=0))
+    for B in (N, 32):
+        Hm = op.projected_hamiltonian_mixed(Yd, n_oc, B=B).cpu().numpy()
+        assert np.max(np.abs(Hm - H64)[n_oc:, n_oc:] / hs[n_oc:, n_oc:]) <= 1e-12, B
+        lo = np.ones((N, N), dtype=bool)
+        lo[n_oc:, n_oc:] = False
+        assert np.max(np.abs(Hm - H64)[lo] / hs[lo]) <= 8 * eps32, B
+        assert np.max(np.abs(Hm - Hom)[lo] / hs[lo]) <= 64 * eps32, B
+        assert np.max(np.abs(Hm - H64)[lo] / hs[lo]) > 1e-12, B
+    # -- orthonormal basis  Psi^o = SP[Y L^-T_od] + DP[Y L^-T_d]
+    _, Linv = orc.cholesky_inverse(S64)
+    Zt = np.ascontiguousarray(Linv.T)
+    Pm = op.subspace_transform_mixed(Yd, torch.tensor(Zt, device="cuda")).cpu().numpy()
+    Pom, P64 = orc.orthonormal_basis_mixed(Y, Zt), Y @ Zt
+    bound = np.abs(Y) @ np.abs(Zt - np.diag(np.diag(Zt)))        # size of the FP32 part, entry by entry
+    assert np.max(np.abs(Pm - P64) / (bound + 1e-300)) <= 8 * eps32
+    assert np.max(np.abs(Pm - Pom) / (bound + 1e-300)) <= 64 * eps32
+    # -- Algorithm 2 with the mixed matrices on a nearly converged subspace
+    Q = Fo[:, :32].copy()
+    for _ in range(6):
+        th = orc.ritz_values_of_block(Q, orc.apply_H(oop, Q))
+        Q, _ = np.linalg.qr(orc.chebyshev_filter(oop, Q, 10, float(th[-1]), b, float(th[0]) - 1e-3))
+    Q = Q * (1.0 + 0.3 * rng.random(32))[None, :]
+    Qd = torch.tensor(Q, device="cuda")
+    n_oc2, n_fr = 24, 8
+    Sm = op.overlap_matrix_mixed(Qd, 8)
+    Hm = op.projected_hamiltonian_mixed(Qd, n_oc2, B=16)
+    L, Linv_d, info = op.cholesky_inverse(0.5 * (Sm + Sm.T))
+    assert int(info.item()) == 0
+    A = (Linv_d @ (0.5 * (Hm + Hm.T)) @ Linv_d.T).cpu().numpy()
+    d_mixed = np.linalg.eigvalsh(0.5 * (A + A.T))[-n_fr:]
+    d_orc, _, _ = orc.rayleigh_ritz_gep(Q.T @ Q, Q.T @ orc.apply_H(oop, Q), n_fr)
+    print("mixed-precision Ritz values (n_fr highest) vs FP64 oracle:", np.abs(d_mixed - d_orc))
+    assert np.max(np.abs(d_mixed - d_orc)) <= 1e-5
+    Po = op.subspace_transform_mixed(Qd, Linv_d.T.contiguous())
+    G = (Po.T @ Po).cpu().numpy()
+    assert np.max(np.abs(G - np.eye(32))) <= 1e-5
+    op.close()
