@@ -294,6 +294,101 @@ def apply_H(op: Operator, X):
     return s[:, None] * W
 
 
+# ---------------------------------------------------------------------------------------------------------
+# k-point variant (periodic part u_k of a Bloch wavefunction, Eq. 2-3): complex Hermitian operator
+# ---------------------------------------------------------------------------------------------------------
+
+
+@dataclass
+class OperatorK:
+    """H~^k = M^-1/2 H^k M^-1/2 with (Eq. 30; Eq. 33)
+        H^k_jl = 1/2 int grad N_j . grad N_l + int (V_eff + 1/2 |k|^2) N_j N_l - i int k . (N_j grad N_l)
+                 + sum_p C^k_pj h_p conj(C^k_pl),     C^k_pj = int sum_r e^{-i k.(x - L_r)} chi_p(x, R_a + L_r) N_j(x) dx.
+    Stored per cell: He = 1/2 K^e + V^e + 1/2 |k|^2 M_G^e (real symmetric), Ae_jl = sum_q w detJ N_j(q) (k . grad N_l)(q)
+    (real, antisymmetric after assembly), and the complex projector vectors Cc = Cr + i Ci."""
+    base: Operator                     # carries p, cell_dofs, M, He (incl. the 1/2 |k|^2 term), D, projector CSR, Cc = Cr
+    kvec: np.ndarray                   # [3]
+    Ae: np.ndarray                     # [n_cells, M_cell, M_cell]
+    Ci: np.ndarray                     # [nnz, M_cell]   imaginary parts of the projector vectors
+
+
+def cell_k_term(ref: RefCell, vertices, kvec):
+    """Ae_jl = sum_q w_q detJ_q N_j(q) (k . grad_x N_l)(q): the last term of Eq. 30 without its factor -i."""
+    J = trilinear_jacobian(vertices, ref.ref_q)
+    detJ = np.linalg.det(J)
+    Jinv = np.linalg.inv(J)
+    g = np.einsum("qdi,qdl->qil", Jinv, ref.dN)              # physical gradients [nq, 3, M_cell]
+    kg = np.einsum("i,qil->ql", np.asarray(kvec, dtype=np.float64), g)
+    return (ref.N * (ref.wq * detJ)[:, None]).T @ kg
+
+
+def build_operator_k(p, cell_dofs, cell_vertices, n_dofs, veff_q, kvec, n_proj=0, D=None, proj_cell_ptr=None,
+                     proj_cell_idx=None, chi_q=None, chi_q_im=None) -> OperatorK:
+    """chi_q + i chi_q_im are the samples of sum_r e^{-i k.(x - L_r)} chi(x, R_a + L_r) at the Gauss points."""
+    kvec = np.asarray(kvec, dtype=np.float64)
+    base = build_operator(p, cell_dofs, cell_vertices, n_dofs, veff_q + 0.5 * float(kvec @ kvec), n_proj, D,
+                          proj_cell_ptr, proj_cell_idx, chi_q)
+    ref = reference_cell(p)
+    Ae = np.zeros_like(base.He)
+    for c in range(base.n_cells):
+        Ae[c] = cell_k_term(ref, cell_vertices[c], kvec)
+    Ci = np.zeros_like(base.Cc)
+    if n_proj and chi_q_im is not None:
+        for j in range(n_proj):
+            for k in range(int(proj_cell_ptr[j]), int(proj_cell_ptr[j + 1])):
+                Ci[k] = projector_cell_vector(ref, cell_vertices[proj_cell_idx[k]], chi_q_im[k])
+    return OperatorK(base, kvec, Ae, Ci)
+
+
+def apply_H_k(opk: OperatorK, X):
+    """Y = H~^k X for a complex block X [n_dofs, B], cell by cell as apply_H (Eq. 47, Alg. 4), written on the real and
+    imaginary parts:  (He - i Ae)(Ur + i Ui) = (He Ur + Ae Ui) + i (He Ui - Ae Ur);  P = conj(C)^T U;  W += C (D P)."""
+    op = opk.base
+    X = np.asarray(X, dtype=np.complex128)
+    if X.ndim == 1:
+        return apply_H_k(opk, X[:, None])[:, 0]
+    s = 1.0 / np.sqrt(op.M)
+    Ur, Ui = s[:, None] * X.real, s[:, None] * X.imag
+    Wr, Wi = np.zeros_like(Ur), np.zeros_like(Ui)
+    for c in range(op.n_cells):
+        g = op.cell_dofs[c]
+        Wr[g] += op.He[c] @ Ur[g] + opk.Ae[c] @ Ui[g]
+        Wi[g] += op.He[c] @ Ui[g] - opk.Ae[c] @ Ur[g]
+    if op.n_proj:
+        Pr = np.zeros((op.n_proj, X.shape[1]))
+        Pi = np.zeros((op.n_proj, X.shape[1]))
+        for j in range(op.n_proj):
+            for k in range(int(op.proj_cell_ptr[j]), int(op.proj_cell_ptr[j + 1])):
+                g = op.cell_dofs[op.proj_cell_idx[k]]
+                Pr[j] += op.Cc[k] @ Ur[g] + opk.Ci[k] @ Ui[g]        # conj(C) . U
+                Pi[j] += op.Cc[k] @ Ui[g] - opk.Ci[k] @ Ur[g]
+        Pr *= op.D[:, None]
+        Pi *= op.D[:, None]
+        for j in range(op.n_proj):
+            for k in range(int(op.proj_cell_ptr[j]), int(op.proj_cell_ptr[j + 1])):
+                g = op.cell_dofs[op.proj_cell_idx[k]]
+                Wr[g] += np.outer(op.Cc[k], Pr[j]) - np.outer(opk.Ci[k], Pi[j])
+                Wi[g] += np.outer(op.Cc[k], Pi[j]) + np.outer(opk.Ci[k], Pr[j])
+    return s[:, None] * (Wr + 1j * Wi)
+
+
+def chebyshev_filter_k(opk: OperatorK, X, m: int, a: float, b: float, a0: float):
+    """chebyshev_filter for the complex Hermitian H~^k (same scaled recurrence, real scalars)."""
+    if m < 1 or not (a0 <= a < b):
+        raise ValueError("need m >= 1 and a0 <= a < b")
+    X = np.asarray(X, dtype=np.complex128)
+    e, c = (b - a) / 2, (b + a) / 2
+    sigma1 = e / (a0 - c)
+    sigma = sigma1
+    Ym2 = X
+    Ym1 = (sigma1 / e) * (apply_H_k(opk, X) - c * X)
+    for _ in range(2, m + 1):
+        sigma_new = 1.0 / (2.0 / sigma1 - sigma)
+        Y = (2 * sigma_new / e) * (apply_H_k(opk, Ym1) - c * Ym1) - (sigma * sigma_new) * Ym2
+        Ym2, Ym1, sigma = Ym1, Y, sigma_new
+    return Ym1
+
+
 def chebyshev_filter(op: Operator, X, m: int, a: float, b: float, a0: float):
     """Degree-m scaled Chebyshev filter (Eq. 37, in the scaled three-term form of ref. [86]
     (Zhou, Saad, Tiago, Chelikowsky); reading U1):

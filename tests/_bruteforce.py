@@ -70,9 +70,11 @@ def jacobian_fd(verts, ref, h=0.25):
 
 
 def dense_operator(p, cell_dofs, cell_vertices, n_dofs, veff_q, n_proj=0, D=None, proj_cell_ptr=None,
-                   proj_cell_idx=None, chi_q=None, nq1=None):
+                   proj_cell_idx=None, chi_q=None, nq1=None, kvec=None, chi_q_im=None):
     """Dense (M_diag, Hloc, C, H~) for a tiny mesh by the global formulation described in the module
-    docstring.  Returns dict with 'M' [n], 'K' [n,n], 'V' [n,n], 'C' [n,n_proj], 'Ht' [n,n]."""
+    docstring.  Returns dict with 'M' [n], 'K' [n,n], 'V' [n,n], 'C' [n,n_proj], 'Ht' [n,n].
+    With `kvec` the k-point operator of Eq. 30 / 33 is returned as a complex 'Ht':
+    H^k = 1/2 K + V + 1/2 |k|^2 M_G - i A_k + C h C^dagger, (A_k)_jl = int N_j k.grad N_l, C complex."""
     nq1 = nq1 or p + 2
     gx, gw = gll_nodes_weights(p)
     qx, qw = npleg.leggauss(nq1)
@@ -124,8 +126,25 @@ def dense_operator(p, cell_dofs, cell_vertices, n_dofs, veff_q, n_proj=0, D=None
             c = int(proj_cell_idx[k])
             C[:, j] += Phi[c].T @ (W[c] * chi_q[k])
     Hloc = 0.5 * K + V
-    H = Hloc + (C @ np.diag(np.asarray(D, dtype=np.float64)) @ C.T if n_proj else 0.0)
     s = 1 / np.sqrt(M)
+    if kvec is not None:
+        kvec = np.asarray(kvec, dtype=np.float64)
+        MG = Phi2.T @ (Wf[:, None] * Phi2)
+        A = np.zeros((n_dofs, n_dofs))
+        for d in range(3):
+            G = dPhi[:, :, d, :].reshape(n_cells * nq, n_dofs)
+            A += kvec[d] * (Phi2.T @ (Wf[:, None] * G))
+        Ck = C.astype(np.complex128)
+        if n_proj and chi_q_im is not None:
+            for j in range(n_proj):
+                for k in range(int(proj_cell_ptr[j]), int(proj_cell_ptr[j + 1])):
+                    c = int(proj_cell_idx[k])
+                    Ck[:, j] += 1j * (Phi[c].T @ (W[c] * chi_q_im[k]))
+        Hk = Hloc + 0.5 * float(kvec @ kvec) * MG - 1j * A
+        if n_proj:
+            Hk = Hk + Ck @ np.diag(np.asarray(D, dtype=np.float64)) @ Ck.conj().T
+        return dict(M=M, K=K, V=V, C=Ck, A=A, Ht=s[:, None] * Hk * s[None, :])
+    H = Hloc + (C @ np.diag(np.asarray(D, dtype=np.float64)) @ C.T if n_proj else 0.0)
     return dict(M=M, K=K, V=V, C=C, Hloc=Hloc, Ht=s[:, None] * H * s[None, :])
 
 

@@ -90,6 +90,9 @@ class Workload:
     n: int = 0
     periodic: bool = True
     atoms: np.ndarray = field(default_factory=lambda: np.zeros((0, 3)))
+    # k-point variant: kvec [3] and the imaginary parts of the projector samples (chi_q then holds the real parts)
+    kvec: Optional[np.ndarray] = None
+    chi_q_im: Optional[np.ndarray] = None
 
     @property
     def m_cell(self) -> int:
@@ -223,8 +226,9 @@ def _radial_norms(s: float, rc: float):
     return 1 / np.sqrt(n0), 1 / np.sqrt(n1)
 
 
-def _projectors(xq, centres, half_diag, atoms, L, periodic, rc):
-    """Per atom: support cells and chi values [8, n_support, nq] (l=0,1 x 2 radial widths)."""
+def _projectors(xq, centres, half_diag, atoms, L, periodic, rc, kvec=None):
+    """Per atom: support cells and chi values [8, n_support, nq] (l=0,1 x 2 radial widths).  With a k-point the values
+    are the complex samples of sum_r e^{-i k.(x - L_r)} chi(x, R_a + L_r) (Eq. 33), L_r = image shift."""
     result = []
     norms = [_radial_norms(s, rc) for s in PROJ_WIDTHS]
     for pos in atoms:
@@ -239,12 +243,13 @@ def _projectors(xq, centres, half_diag, atoms, L, periodic, rc):
             keep = np.nonzero(inside.any(axis=1))[0]
             for kk in keep:
                 c = int(cells[kk])
-                vals = np.zeros((8, xq.shape[1]))
+                vals = np.zeros((8, xq.shape[1]), dtype=np.float64 if kvec is None else np.complex128)
+                phase = 1.0 if kvec is None else np.exp(-1j * ((xq[cells[kk]] - sh[None, :]) @ np.asarray(kvec)))
                 for si, s in enumerate(PROJ_WIDTHS):
                     f = np.where(inside[kk], np.exp(-r[kk] ** 2 / (2 * s ** 2)) * (1 - (r[kk] / rc) ** 2) ** 2, 0.0)
-                    vals[4 * si + 0] = norms[si][0] * f
+                    vals[4 * si + 0] = norms[si][0] * f * phase
                     for ax in range(3):
-                        vals[4 * si + 1 + ax] = norms[si][1] * f * d[kk, :, ax]
+                        vals[4 * si + 1 + ax] = norms[si][1] * f * d[kk, :, ax] * phase
                 if c in chunks:
                     chunks[c] += vals
                 else:
@@ -265,8 +270,9 @@ def _lattice_atoms(k: int, L: float, jitter: float, seed: int) -> np.ndarray:
 
 def make_workload(config: Optional[int] = None, *, n=None, p=None, L=None, periodic=True, mesh_jitter=0.0,
                   atoms_per_side=None, n_gaussians=None, nonlocal_=None, smooth_field=None, seed_base=None,
-                  r_cut=R_CUT) -> Workload:
-    """Build the operator inputs of a BASELINE.json config (or a custom small case for tests)."""
+                  r_cut=R_CUT, kvec=None) -> Workload:
+    """Build the operator inputs of a BASELINE.json config (or a custom small case for tests).  `kvec` (bohr^-1) selects
+    the k-point variant: the projector samples then carry the Bloch phase of Eq. 33 (real and imaginary parts)."""
     spec = CONFIGS[config] if config is not None else None
     pick = lambda v, name: v if v is not None else getattr(spec, name)
     n, p, L = pick(n, "n"), pick(p, "p"), float(pick(L, "L"))
@@ -291,7 +297,7 @@ def make_workload(config: Optional[int] = None, *, n=None, p=None, L=None, perio
     wl = Workload(spec=spec, p=p, n_cells=n ** 3, n_dofs=n_dofs, cell_dofs=cell_dofs, cell_vertices=verts,
                   veff_q=np.ascontiguousarray(veff), L=L, n=n, periodic=periodic, atoms=atoms)
     if nl:
-        per_atom = _projectors(xq, centres, half_diag, atoms, L, periodic, r_cut)
+        per_atom = _projectors(xq, centres, half_diag, atoms, L, periodic, r_cut, kvec)
         ptr, idx, chi = [0], [], []
         for cells, vals in per_atom:
             for j in range(8):
@@ -302,7 +308,12 @@ def make_workload(config: Optional[int] = None, *, n=None, p=None, L=None, perio
         wl.proj_cell_ptr = np.array(ptr, dtype=np.int64)
         wl.proj_cell_idx = np.concatenate(idx).astype(np.int32) if idx else np.zeros(0, dtype=np.int32)
         wl.chi_q = np.ascontiguousarray(np.concatenate(chi, axis=0)) if chi else np.zeros((0, xq.shape[1]))
+        if kvec is not None:
+            wl.chi_q_im = np.ascontiguousarray(wl.chi_q.imag)
+            wl.chi_q = np.ascontiguousarray(wl.chi_q.real)
         wl.D = np.random.default_rng(sb + SEED_D).uniform(-1.0, 1.0, size=wl.n_proj)
+    if kvec is not None:
+        wl.kvec = np.asarray(kvec, dtype=np.float64)
     return wl
 
 
