@@ -36,6 +36,8 @@ DEFAULT_CONFIG = 5          # the largest single-GPU configuration of BASELINE.j
 NCU_TRAFFIC_BYTES_PER_LAUNCH = {
     (2, "k_apply_dmma_p<double>"): 1.661e9,    # profiles/r01_v4_config2_config3.md: 1.334 GB read + 0.327 GB written
     (3, "k_apply_dmma_p<double>"): 14.54e9,    # same file: 11.68 GB read + 2.86 GB written
+    (5, "k_apply_sf<double>"): 27.24e9,        # profiles/r02_sf_kernel.md: 18.48 GB read + 8.76 GB written
+    (3, "k_apply_sf<double>"): 8.82e9,         # same file: 5.97 GB read + 2.84 GB written
 }
 
 
