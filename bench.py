@@ -50,10 +50,10 @@ def parse_args():
                     help="BASELINE.json config 1..5; 6 = extra p=7 workload (config 2's box at FE degree 7)")
     ap.add_argument("--assembly", type=int, default=0, choices=[0, 1],
                     help="0 deterministic coloured assembly, 1 atomic assembly")
-    ap.add_argument("--variant", type=int, default=0, choices=[0, 1, 2, 3, 4, 5],
+    ap.add_argument("--variant", type=int, default=0, choices=[0, 1, 2, 3, 4, 5, 6],
                     help="kernel of the per-cell product: 0 automatic (sum-factorised for p <= 6, else dense persistent), "
                          "1 generic, 2 dense one launch per colour, 3 FP32 storage with 3xTF32 products (looser accuracy), "
-                         "4 dense persistent DMMA kernel, 5 sum-factorised")
+                         "4 dense persistent DMMA kernel, 5 sum-factorised, 6 sum-factorised warp-specialised")
     ap.add_argument("--all-configs", action="store_true", help="one JSON line per BASELINE.json config (1..5)")
     ap.add_argument("--rr", action="store_true",
                     help="Rayleigh-Ritz products (S = Y^T Y, H^ = Y^T H~ Y, Y Z) at N = 1024 on config 3's rows")
@@ -190,6 +190,7 @@ def run_reference(args, spec):
 # ------------------------------------------------------------------------------------------------------------
 KERNEL_NAMES = {
     (64, 1): "k_apply_generic<double>", (64, 2): "k_apply_dmma", (64, 4): "k_apply_dmma_p<double>", (64, 5): "k_apply_sf<double>",
+    (64, 6): "k_apply_sf_ws<double>", (32, 6): "k_apply_sf_ws<float>",
     (32, 1): "k_apply_generic<float>", (32, 3): "k_apply_tf32_p", (32, 4): "k_apply_dmma_p<float>", (32, 5): "k_apply_sf<float>",
 }
 
@@ -198,7 +199,7 @@ def dominant_kernel(precision, variant, info):
     """Name of the kernel the automatic choice (variant 0) resolves to for this operator (include/chfsi.h)."""
     if variant == 0:
         variant = 5 if info["sf_flops_per_vector_apply"] > 0 else 4
-    if variant == 5 and not info["sf_flops_per_vector_apply"] > 0:
+    if variant in (5, 6) and not info["sf_flops_per_vector_apply"] > 0:
         variant = 4
     return KERNEL_NAMES.get((precision, variant), "k_apply_generic"), variant
 
@@ -277,7 +278,7 @@ def run_b200(args, spec):
 
     # roofline of the dominant kernel (per-cell product incl. gather, projector term, assembly, recurrence)
     cols_total = N * m * args.steps                           # column-applies covered by the profile
-    sf = eff_variant == 5
+    sf = eff_variant in (5, 6)
     if sf:
         # the sum-factorised kernel: EXECUTED flops; DMMA and DFMA share one FP64 pipe on B200
         kflops_per_col = info["sf_flops_per_vector_apply"]

@@ -109,18 +109,45 @@ int filter_block(chfsi_op* op, void* X, int64_t ldx, int64_t B, int32_t m, doubl
   double sigma = sigma1;
   void* cur = X; int64_t ldcur = ldx;      // Y_{k-1}
   void* tgt = W; int64_t ldtgt = w.ldw;    // Y_{k-2} -> Y_k
+  // Scaled form of the recurrence for kernels that only add into the target block (ApplyArgs::accumulate): the blocks
+  // hold W_k = s_k Y_k with s_0 = s_1 = 1 and s_k = -s_{k-2} / beta_k, so that
+  //   Y_k = alpha_k (H~ - c) Y_{k-1} - beta_k Y_{k-2}   <=>   W_k = W_{k-2} + (s_k alpha_k / s_{k-1}) (H~ - c) W_{k-1},
+  // and the result is W_m / s_m.  |s_k| = T_k(t0) / T_{k mod 2}(t0) (the unnormalised Chebyshev polynomials at
+  // t0 = (a0 - c) / e): when that leaves the range of the storage type the three-term form is used instead.
+  g.X = cur; g.ldx = ldcur; g.T = tgt; g.ldt = ldtgt;
+  bool scaled = m >= 2 && apply_accumulates(op, g);
+  if (scaled) {
+    const double limit = op->precision == 64 ? 1e200 : 1e25;
+    double s2 = 1.0, s1 = 1.0, sg = sigma1;
+    for (int k = 2; k <= m && scaled; ++k) {
+      const double sn = 1.0 / (2.0 / sigma1 - sg);
+      const double sk = -s2 / (sg * sn);
+      if (!(std::fabs(sk) < limit && std::fabs(sk) > 1.0 / limit)) scaled = false;
+      s2 = s1; s1 = sk; sg = sn;
+    }
+  }
+  double s_km2 = 1.0, s_km1 = 1.0;         // s_{k-2}, s_{k-1}
   for (int k = 1; k <= m; ++k) {
     g.X = cur; g.ldx = ldcur; g.T = tgt; g.ldt = ldtgt; g.cshift = c; g.epoch = (uint32_t)k;
+    g.accumulate = false;
     if (k == 1) { g.alpha = sigma1 / e; g.beta = 0.0; }
     else {
       const double sigma_new = 1.0 / (2.0 / sigma1 - sigma);
       g.alpha = 2.0 * sigma_new / e; g.beta = sigma * sigma_new; sigma = sigma_new;
+      if (scaled) {
+        const double s_k = -s_km2 / g.beta;
+        g.alpha = s_k * g.alpha / s_km1; g.beta = 0.0; g.accumulate = true;
+        s_km2 = s_km1; s_km1 = s_k;
+      }
     }
     cudaError_t ce = launch_apply(op, g, st);
     if (ce != cudaSuccess) return cuda_fail(op, ce, "chebyshev_filter launch");
     std::swap(cur, tgt); std::swap(ldcur, ldtgt);
   }
-  if (cur != X) {   // odd m: result sits in the workspace block
+  if (scaled) {     // X <- W_m / s_m (from the workspace block when m is odd, in place when m is even)
+    cudaError_t ce = launch_scale_block(op, X, ldx, cur, ldcur, B, 1.0 / s_km1, st);
+    if (ce != cudaSuccess) return cuda_fail(op, ce, "chebyshev_filter rescale");
+  } else if (cur != X) {   // odd m: result sits in the workspace block
     cudaError_t ce = cudaMemcpy2DAsync(X, (size_t)ldx * w.elt, W, (size_t)w.ldw * w.elt, (size_t)B * w.elt,
                                        (size_t)op->n_dofs, cudaMemcpyDeviceToDevice, st);
     if (ce != cudaSuccess) return cuda_fail(op, ce, "chebyshev_filter copy-back");
@@ -696,7 +723,7 @@ int64_t chfsi_launch_count(const chfsi_op* op) { return op ? op->launches : -1; 
 
 int chfsi_set_kernel_variant(chfsi_op* op, int variant) {
   if (!op) return CHFSI_ERR_BAD_ARGUMENT;
-  if (variant < 0 || variant > 5) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "variant must be 0 .. 5");
+  if (variant < 0 || variant > 6) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "variant must be 0 .. 6");
   op->variant = variant;
   return CHFSI_OK;
 }

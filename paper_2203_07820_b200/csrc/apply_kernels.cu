@@ -39,6 +39,7 @@ struct ApplyDev {
   int B;
   T alpha, beta;                       // T <- alpha (H~ - c) X - beta T ; the shift c sits on the matrix diagonals
   int atomic;                          // 1: red.add into a pre-filled target
+  int accumulate;                      // 1: T <- T + alpha (H~ - c) X (k_apply_sf_ws; common.h ApplyArgs::accumulate)
 };
 
 __device__ __forceinline__ void red_add(double* p, double v) { atomicAdd(p, v); }
@@ -731,6 +732,7 @@ __global__ void __launch_bounds__(256, 2) k_proj_rows_tma(const int32_t* __restr
 
 #include "apply_tf32.cuh"
 #include "apply_sf.cuh"
+#include "apply_sf_ws.cuh"
 
 // Tensor map of a row-major FP64 / FP32 block [rows][ld] restricted to its first `cols` columns, box = box_cols x 1
 // (tile::gather4 picks four such rows per instruction); columns beyond `cols` read as zero.
@@ -797,8 +799,14 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
                        ((uintptr_t)g.T % 16 == 0) && ((uintptr_t)g.P % 16 == 0) && op->max_ktot <= kMaxKtot;
   // variant 0 (automatic) / 5: the sum-factorised kernel (apply_sf.cuh) when the operator qualifies
   CUtensorMap tmX, tmP;
-  const bool use_sf = op->sf_ok && aligned && (op->variant == 0 || op->variant == 5) && g.sync != nullptr && g.epoch > 0 &&
-                      make_row_gather_map(&tmX, g.X, op->n_dofs, B, g.ldx, (int)sizeof(T), sf_tile_cols<T>(), true);
+  CUtensorMap tmPs;
+  bool use_sf = op->sf_ok && aligned && (op->variant == 0 || op->variant == 5 || op->variant == 6) && g.sync != nullptr && g.epoch > 0 &&
+                make_row_gather_map(&tmX, g.X, op->n_dofs, B, g.ldx, (int)sizeof(T), sf_tile_cols<T>(), true);
+  // variant 6: the warp-specialised form (apply_sf_ws.cuh).  It never reads the target block: T = alpha (..) or, with
+  // g.accumulate, T += alpha (..); a three-term update with beta != 0 goes to k_apply_sf.
+  const bool use_ws = use_sf && op->variant == 6 && (g.accumulate || g.beta == 0.0) &&
+                      make_row_gather_map(&tmPs, g.P, op->n_proj + 1, B, B, (int)sizeof(T), sf_tile_cols<T>(), false);
+  if (g.accumulate && !use_ws) return cudaErrorNotSupported;   // the caller asks apply_accumulates() first
   if (!use_sf && g.cshift != op->cur_shift) {   // once per filter call: move the spectral shift onto the matrix diagonals
     const int64_t n = op->n_cells * op->m_cell;
     k_set_diag_shift<T><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(reinterpret_cast<T*>(op->mat), op->mat_off, op->idx_off,
@@ -835,6 +843,7 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
   a.X = X; a.ldx = g.ldx; a.Tg = Tg; a.ldt = g.ldt; a.P = P; a.ldp = B; a.B = B;
   a.alpha = (T)g.alpha; a.beta = (T)g.beta;
   a.atomic = op->assembly;
+  a.accumulate = g.accumulate ? 1 : 0;
 
   // variant 4 (and 0 when the sum-factorised kernel does not apply): persistent single-launch dense kernel;
   // variant 2: one launch per colour; variant 1: generic
@@ -859,7 +868,7 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
                      (size_t)op->max_ktot * sizeof(int32_t);
   if (fast && smem_fast > 227 * 1024) fast = false;
 
-  if (op->assembly == 1) {
+  if (op->assembly == 1 && !g.accumulate) {
     k_prefill<T><<<148 * 8, 256, 0, st>>>(Tg, g.ldt, op->n_dofs, B, a.beta);
     op->launches++;
   }
@@ -883,6 +892,18 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
     SfDev sf;
     sf.coef = op->sf_coef; sf.sloc = op->sf_sloc; sf.crows = op->crows; sf.cell_proj_ptr = op->cell_proj_ptr;
     sf.cshift = g.cshift;
+    if (use_ws) {
+      const unsigned gws = (unsigned)std::min<int64_t>(n_tiles, (int64_t)op->n_sm);
+      pd.ticket_base = (unsigned long long)(g.epoch - 1) * (unsigned long long)(n_tiles + gws);
+      switch (op->p) {
+        case 1: k_apply_sf_ws<1, T><<<gws, kWsThreads, WsSmem<1, T>::bytes, st>>>(a, sf, pd, tmX, tmPs); break;
+        case 2: k_apply_sf_ws<2, T><<<gws, kWsThreads, WsSmem<2, T>::bytes, st>>>(a, sf, pd, tmX, tmPs); break;
+        case 3: k_apply_sf_ws<3, T><<<gws, kWsThreads, WsSmem<3, T>::bytes, st>>>(a, sf, pd, tmX, tmPs); break;
+        case 4: k_apply_sf_ws<4, T><<<gws, kWsThreads, WsSmem<4, T>::bytes, st>>>(a, sf, pd, tmX, tmPs); break;
+        case 5: k_apply_sf_ws<5, T><<<gws, kWsThreads, WsSmem<5, T>::bytes, st>>>(a, sf, pd, tmX, tmPs); break;
+        case 6: k_apply_sf_ws<6, T><<<gws, kWsThreads, WsSmem<6, T>::bytes, st>>>(a, sf, pd, tmX, tmPs); break;
+      }
+    } else
     switch (op->p) {
       case 1: k_apply_sf<1, T><<<grid, kSfThreads, sf_smem_bytes<1, T>(op), st>>>(a, sf, pd, tmX); break;
       case 2: k_apply_sf<2, T><<<grid, kSfThreads, sf_smem_bytes<2, T>(op), st>>>(a, sf, pd, tmX); break;
@@ -1039,6 +1060,8 @@ template <int P>
 cudaError_t sf_set_attr(Op* op) {
   cudaError_t e;
   if ((e = cudaFuncSetAttribute(k_apply_sf<P, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sf_smem_bytes<P, double>(op)))) return e;
+  if ((e = cudaFuncSetAttribute(k_apply_sf_ws<P, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, WsSmem<P, double>::bytes))) return e;
+  if ((e = cudaFuncSetAttribute(k_apply_sf_ws<P, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, WsSmem<P, float>::bytes))) return e;
   return cudaFuncSetAttribute(k_apply_sf<P, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sf_smem_bytes<P, float>(op));
 }
 }  // namespace
@@ -1160,6 +1183,42 @@ cudaError_t capture_diagonal(Op* op, cudaStream_t st) {
     k_capture_diag<float><<<grid, 256, 0, st>>>(reinterpret_cast<const float*>(op->mat), op->mat_off, op->ktot, op->diag0,
                                                 op->m_cell, op->lda, op->mw, op->n_cells);
   op->cur_shift = 0.0;
+  return cudaGetLastError();
+}
+
+namespace {
+template <typename T>
+bool block_aligned(const Op* op, const ApplyArgs& g) {
+  constexpr int kPer16 = 16 / (int)sizeof(T);
+  return g.B % kPer16 == 0 && g.ldx % kPer16 == 0 && g.ldt % kPer16 == 0 && ((uintptr_t)g.X % 16 == 0) &&
+         ((uintptr_t)g.T % 16 == 0) && ((uintptr_t)g.P % 16 == 0) && op->max_ktot <= kMaxKtot;
+}
+template <typename T>
+__global__ void __launch_bounds__(256) k_scale_block(T* __restrict__ dst, int64_t ldd, const T* __restrict__ src, int64_t lds,
+                                                     int64_t n_dofs, int B, double factor) {
+  const int64_t n = n_dofs * B;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t g = i / B; const int col = (int)(i - g * B);
+    dst[g * ldd + col] = (T)(factor * (double)src[g * lds + col]);
+  }
+}
+}  // namespace
+
+bool apply_accumulates(const Op* op, const ApplyArgs& g) {
+  if (!(op->sf_ok && op->variant == 6 && g.sync != nullptr && encode_tiled_fn() != nullptr)) return false;
+  return op->precision == 64 ? block_aligned<double>(op, g) : block_aligned<float>(op, g);
+}
+
+cudaError_t launch_scale_block(Op* op, void* dst, int64_t ldd, const void* src, int64_t lds, int64_t B, double factor,
+                               cudaStream_t st) {
+  const unsigned grid = (unsigned)(op->n_sm * 8);
+  if (op->precision == 64)
+    k_scale_block<double><<<grid, 256, 0, st>>>(reinterpret_cast<double*>(dst), ldd, reinterpret_cast<const double*>(src), lds,
+                                                op->n_dofs, (int)B, factor);
+  else
+    k_scale_block<float><<<grid, 256, 0, st>>>(reinterpret_cast<float*>(dst), ldd, reinterpret_cast<const float*>(src), lds,
+                                               op->n_dofs, (int)B, factor);
+  op->launches++;
   return cudaGetLastError();
 }
 

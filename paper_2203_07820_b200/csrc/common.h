@@ -191,7 +191,16 @@ struct ApplyArgs {
   // completion flags, zeroed by the caller of launch_apply before epoch 1; epoch increases by one per launch
   unsigned long long* sync = nullptr;
   uint32_t epoch = 0;
+  // accumulate: T <- T + alpha (H~ X - cshift X); beta is ignored and the target block is never read by the kernel
+  // (every contribution is a red.add).  Only the warp-specialised sum-factorised kernel takes it: ask
+  // apply_accumulates() first.  The filter loop then runs the recurrence in scaled blocks (api.cu filter_block).
+  bool accumulate = false;
 };
+// True when launch_apply would run these arguments (X, ldx, T, ldt, P, B, sync set) with accumulate = true.
+bool apply_accumulates(const Op* op, const ApplyArgs& a);
+// dst[g][0..B) = factor * src[g][0..B) for all dofs g (element type per op->precision; dst may equal src).
+cudaError_t launch_scale_block(Op* op, void* dst, int64_t ldd, const void* src, int64_t lds, int64_t B, double factor,
+                               cudaStream_t stream);
 // Enqueues one fused H~ application + recurrence update.  Returns cudaGetLastError().
 cudaError_t launch_apply(Op* op, const ApplyArgs& a, cudaStream_t stream);
 // Builds op->pcoef: the projector rows of the cell matrices summed over the cells of each dof (once, at create,

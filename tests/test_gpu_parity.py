@@ -99,9 +99,10 @@ def oracle_case(name):
 
 
 # kernel variants (include/chfsi.h): 0 automatic (sum-factorised kernel for p <= 6, dense persistent kernel above),
-# 1 generic, 2 dense with one launch per colour, 4 dense persistent, 5 sum-factorised
+# 1 generic, 2 dense with one launch per colour, 4 dense persistent, 5 sum-factorised (one CTA = column loop + hand-over),
+# 6 sum-factorised warp-specialised
 @pytest.mark.parametrize("assembly", [0, 1])
-@pytest.mark.parametrize("variant", [0, 1, 2, 4])
+@pytest.mark.parametrize("variant", [0, 1, 2, 4, 5, 6])
 @pytest.mark.parametrize("name", list(CASES))
 def test_apply_H_and_filter_match_the_oracle(name, assembly, variant):
     torch, orc, Operator, _, _, _, _ = _imports()
@@ -304,6 +305,34 @@ def test_single_launch_ordering_equals_per_colour_launches_bit_for_bit():
     assert torch.equal(app[0][0], app[2][0])
     assert torch.equal(out[0][0], out[0][1])
     assert rel_fro(out[2][0].cpu().numpy(), out[0][0].cpu().numpy()) <= 1e-13
+    op.close()
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+def test_warp_specialised_kernel_equals_the_plain_sum_factorised_kernel_bit_for_bit(precision):
+    """k_apply_sf_ws (variant 6) runs the arithmetic of k_apply_sf (variant 5) with the tile hand-over moved to helper
+    warps; the column arithmetic and the colour-order assembly are the same, so H~X must agree to the last bit, run to
+    run and between the two kernels (a lost dependency, a buffer handed over too early or a stale index list would
+    show up here).  In the filter the warp-specialised kernel runs the recurrence in scaled blocks (every contribution a
+    red.add, csrc/api.cu filter_block): equal to rounding, and bit-reproducible run to run.  Mesh large enough that
+    every SM holds a CTA and tiles queue up behind flags."""
+    torch, orc, Operator, _, make_workload, random_block, _ = _imports()
+    wl = make_workload(None, n=6, p=6, L=12.0, atoms_per_side=1, n_gaussians=0, nonlocal_=True, smooth_field=0.05,
+                       seed_base=92)
+    op = Operator.from_workload(wl, precision=precision, assembly=0)
+    assert op.info["sf_flops_per_vector_apply"] > 0, "the operator must qualify for the sum-factorised kernels"
+    X = torch.tensor(random_block(wl.n_dofs, range(136), 3), dtype=op.dtype, device="cuda")  # full column tiles + a ragged one
+    out, app = {}, {}
+    for variant in (5, 6, 6):
+        op.set_kernel_variant(variant)
+        app.setdefault(variant, []).append(op.apply_H(X))
+        F = X.clone()
+        op.chebyshev_filter(F, 7, 0.5, 400.0, 0.1)
+        out.setdefault(variant, []).append(F)
+    assert torch.equal(app[6][0], app[6][1]) and torch.equal(out[6][0], out[6][1])
+    assert torch.equal(app[5][0], app[6][0])
+    tol = 1e-13 if precision == 64 else 1e-5
+    assert rel_fro(out[6][0].double().cpu().numpy(), out[5][0].double().cpu().numpy()) <= tol
     op.close()
 
 
