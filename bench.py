@@ -51,7 +51,7 @@ def parse_args():
     ap.add_argument("--assembly", type=int, default=0, choices=[0, 1],
                     help="0 deterministic coloured assembly, 1 atomic assembly")
     ap.add_argument("--variant", type=int, default=0, choices=[0, 1, 2, 3, 4, 5, 6],
-                    help="kernel of the per-cell product: 0 automatic (sum-factorised for p <= 6, else dense persistent), "
+                    help="kernel of the per-cell product: 0 automatic (warp-specialised sum-factorised for p <= 6, else dense persistent), "
                          "1 generic, 2 dense one launch per colour, 3 FP32 storage with 3xTF32 products (looser accuracy), "
                          "4 dense persistent DMMA kernel, 5 sum-factorised, 6 sum-factorised warp-specialised")
     ap.add_argument("--all-configs", action="store_true", help="one JSON line per BASELINE.json config (1..5)")
@@ -198,7 +198,7 @@ KERNEL_NAMES = {
 def dominant_kernel(precision, variant, info):
     """Name of the kernel the automatic choice (variant 0) resolves to for this operator (include/chfsi.h)."""
     if variant == 0:
-        variant = 5 if info["sf_flops_per_vector_apply"] > 0 else 4
+        variant = 6 if info["sf_flops_per_vector_apply"] > 0 else 4
     if variant in (5, 6) and not info["sf_flops_per_vector_apply"] > 0:
         variant = 4
     return KERNEL_NAMES.get((precision, variant), "k_apply_generic"), variant

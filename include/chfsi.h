@@ -209,14 +209,18 @@ int chfsi_subspace_transform_mixed(chfsi_op* op, const void* Y_dev, int64_t ldy,
 int64_t chfsi_launch_count(const chfsi_op* op);
 
 /* Selects the kernel used for the per-cell product H~^e X^e (all variants compute the same H~ X up to rounding):
- *   0 = automatic: the sum-factorised (matrix-free) kernel for FE degree p <= 6 (north_star: "sum-factorised where
- *       measurement says so"; csrc/apply_sf.cuh), else the dense persistent tensor-core kernel, else the generic path;
+ *   0 = automatic: the warp-specialised sum-factorised (matrix-free) kernel for FE degree p <= 6 (north_star:
+ *       "sum-factorised where measurement says so"; csrc/apply_sf_ws.cuh; a three-term update with beta != 0 asked for
+ *       outside chfsi_chebyshev_filter goes to the kernel of variant 5), else the dense persistent tensor-core kernel,
+ *       else the generic path;
  *   1 = generic dense path (any shape / alignment);
  *   2 = dense tensor-core kernel, one launch per colour;
  *   3 = (FP32 storage only) dense, 3xTF32 products on the 32-bit tensor pipe: outside the 1e-5 Ha eigenvalue
  *       tolerance of the FP32 variant (csrc/apply_tf32.cuh);
  *   4 = dense persistent tensor-core kernel (FP64 DMMA with the distinct per-cell matrices of Eq. 47);
- *   5 = sum-factorised kernel (same as 0 where it applies).
+ *   5 = sum-factorised kernel, one CTA = column loop + tile hand-over (csrc/apply_sf.cuh; the round-2 predecessor of 6);
+ *   6 = warp-specialised sum-factorised kernel (same as 0 where it applies): the filter runs its recurrence in scaled
+ *       blocks so that every contribution to the target block is an addition (csrc/api.cu filter_block).
  * For tests and A/B measurements. */
 int chfsi_set_kernel_variant(chfsi_op* op, int variant);
 

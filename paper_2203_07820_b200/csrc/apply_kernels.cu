@@ -802,9 +802,9 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
   CUtensorMap tmPs;
   bool use_sf = op->sf_ok && aligned && (op->variant == 0 || op->variant == 5 || op->variant == 6) && g.sync != nullptr && g.epoch > 0 &&
                 make_row_gather_map(&tmX, g.X, op->n_dofs, B, g.ldx, (int)sizeof(T), sf_tile_cols<T>(), true);
-  // variant 6: the warp-specialised form (apply_sf_ws.cuh).  It never reads the target block: T = alpha (..) or, with
+  // variants 0 and 6: the warp-specialised form (apply_sf_ws.cuh).  It never reads the target block: T = alpha (..) or, with
   // g.accumulate, T += alpha (..); a three-term update with beta != 0 goes to k_apply_sf.
-  const bool use_ws = use_sf && op->variant == 6 && (g.accumulate || g.beta == 0.0) &&
+  const bool use_ws = use_sf && op->variant != 5 && (g.accumulate || g.beta == 0.0) &&
                       make_row_gather_map(&tmPs, g.P, op->n_proj + 1, B, B, (int)sizeof(T), sf_tile_cols<T>(), false);
   if (g.accumulate && !use_ws) return cudaErrorNotSupported;   // the caller asks apply_accumulates() first
   if (!use_sf && g.cshift != op->cur_shift) {   // once per filter call: move the spectral shift onto the matrix diagonals
@@ -859,7 +859,7 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
     fast3 = (MT16 == 11 || MT16 == 7 || MT16 == 4 || MT16 == 2 || MT16 == 1) && t3_smem_bytes(op) <= 113 * 1024 &&
             make_row_gather_map(&tmX, g.X, op->n_dofs, B, g.ldx, 4, kT3TileN) &&
             make_row_gather_map(&tmP, g.P, op->n_proj + 1, B, B, 4, kT3TileN);
-  if (aligned && !fast3 && !use_sf && (op->variant == 0 || op->variant == 4 || op->variant == 5) && g.sync != nullptr && g.epoch > 0)
+  if (aligned && !fast3 && !use_sf && (op->variant == 0 || op->variant >= 4) && g.sync != nullptr && g.epoch > 0)
     fast2 = (MT == 11 || MT == 8 || MT == 7 || MT == 4 || MT == 2 || MT == 1) && p2_smem_bytes<T>(op) <= 113 * 1024 &&
             make_row_gather_map(&tmX, g.X, op->n_dofs, B, g.ldx, (int)sizeof(T), kP2TileN) &&
             make_row_gather_map(&tmP, g.P, op->n_proj + 1, B, B, (int)sizeof(T), kP2TileN);
@@ -1205,7 +1205,7 @@ __global__ void __launch_bounds__(256) k_scale_block(T* __restrict__ dst, int64_
 }  // namespace
 
 bool apply_accumulates(const Op* op, const ApplyArgs& g) {
-  if (!(op->sf_ok && op->variant == 6 && g.sync != nullptr && encode_tiled_fn() != nullptr)) return false;
+  if (!(op->sf_ok && (op->variant == 0 || op->variant == 6) && g.sync != nullptr && encode_tiled_fn() != nullptr)) return false;
   return op->precision == 64 ? block_aligned<double>(op, g) : block_aligned<float>(op, g);
 }
 

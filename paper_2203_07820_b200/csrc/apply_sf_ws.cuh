@@ -31,8 +31,10 @@ constexpr int kWsComputeWarps = 8;
 constexpr int kWsHelperWarps = 4;                 // warp 8: producer; warps 9-11: assemblers
 constexpr int kWsAsmWarps = kWsHelperWarps - 1;
 constexpr int kWsThreads = 32 * (kWsComputeWarps + kWsHelperWarps);
-constexpr int kWsRegsCompute = 224;               // 256 x 224 + 128 x 56 = 64,512 registers = 384 x 168 (the launch allocation)
-constexpr int kWsRegsHelper = 56;
+// registers after setmaxnreg: 256 x 224 + 128 x 56 = 256 x 232 + 128 x 40 = 64,512 = 384 x 168 (the launch allocation).
+// FP64 tiles (one column pair per compute warp) need the faster assembler; FP32 tiles (two pairs per warp) leave it slack.
+template <typename S> __host__ __device__ constexpr int ws_regs_compute() { return sizeof(S) == 8 ? 224 : 232; }
+template <typename S> __host__ __device__ constexpr int ws_regs_helper() { return sizeof(S) == 8 ? 56 : 40; }
 
 template <int P, typename S>
 struct WsSmem {
@@ -95,7 +97,7 @@ __global__ void __launch_bounds__(kWsThreads, 1) k_apply_sf_ws(ApplyDev<S> a, Sf
     // =============================================================================================================
     // compute warps: the column loop of apply_sf.cuh on tile j in buffer j & 1
     // =============================================================================================================
-    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kWsRegsCompute));
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(ws_regs_compute<S>()));
     double* scrA = reinterpret_cast<double*>(smem_dyn + L::off_scr) + warp * 4 * kSfScrSlab;
     double* scrB = scrA + 2 * kSfScrSlab;
     const int so_w = g * kSfScrPitch + 2 * t;
@@ -326,7 +328,7 @@ __global__ void __launch_bounds__(kWsThreads, 1) k_apply_sf_ws(ApplyDev<S> a, Sf
       set = (set == 2) ? 0 : set + 1;
     }
   } else {
-    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kWsRegsHelper));
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(ws_regs_helper<S>()));
     if (warp == kWsComputeWarps) {
       // ===========================================================================================================
       // producer warp
@@ -437,7 +439,7 @@ __global__ void __launch_bounds__(kWsThreads, 1) k_apply_sf_ws(ApplyDev<S> a, Sf
           // 8 nt + 2t + {0, 1} of every 8-column block nt; two such steps are in flight per warp (the chain LDS -> DMMA ->
           // DMMA -> scale -> red of one step is pure latency).
           constexpr int nmt = (mc + 7) / 8;
-          constexpr int kU = 2;
+          constexpr int kU = NT == 2 ? 2 : 1;               // FP32 tiles (32 columns) have four blocks per step already
 #pragma unroll 1
           for (int mt0 = aw; mt0 < nmt; mt0 += kU * kWsAsmWarps) {
             double v[kU][NT][2], ca[kU][4];
