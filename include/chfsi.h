@@ -116,6 +116,25 @@ int chfsi_create(chfsi_op** out, const chfsi_mesh* mesh, const chfsi_potential* 
                  int assembly /* 0 | 1 */, void* cuda_stream);
 int chfsi_destroy(chfsi_op* op);
 
+/* k-point variant: the operator that acts on the cell-periodic part u_k of a Bloch wavefunction (Eq. 2-3),
+ *   H^k_jl = 1/2 int grad N_j . grad N_l + int (V_eff + 1/2 |k|^2) N_j N_l - i int N_j (k . grad N_l)
+ *            + sum_p C^k_pj h_p conj(C^k_pl)                                   (Eq. 30; Eq. 33),
+ * complex Hermitian after the Loewdin scaling H~^k = M^-1/2 H^k M^-1/2 (Eq. 34).  The projector samples
+ * carry the Bloch phase of Eq. 33: chi_q of `nl` holds the real parts and chi_q_im the imaginary parts of
+ *   sum_r e^{-i k.(x - L_r)} chi_p(x, R_a + L_r)  at the Gauss points (same [nnz][(p+2)^3] layout; HOST pointer, copied).
+ * A handle made here takes COMPLEX blocks in every block entry point below (chfsi_workspace_bytes, chfsi_apply_H,
+ * chfsi_chebyshev_filter, _chunked, _host): element = two FP64 values (re, im), [n_dofs][ld] complex elements with the
+ * vector index fastest, B / N / ld counted in complex columns; a0, a, b stay real (the spectrum is real).
+ * FE degree p <= 6 and FP64 only (CHFSI_ERR_UNSUPPORTED otherwise); the Rayleigh-Ritz
+ * entry points do not take such a handle.  k = 0 with chi_q_im = 0 gives the real operator on both parts. */
+typedef struct {
+  double k[3];                  /* Bloch wave vector, bohr^-1                                              */
+  const double* chi_q_im;       /* [nnz][(p+2)^3]; may be NULL when there are no projectors                */
+} chfsi_kpoint;
+int chfsi_create_k(chfsi_op** out, const chfsi_mesh* mesh, const chfsi_potential* pot,
+                   const chfsi_nonlocal* nl /* nullable */, const chfsi_kpoint* kpoint, int assembly /* 0 | 1 */,
+                   void* cuda_stream);
+
 /* New V_eff on the same mesh and projectors: recomputes the Hamiltonian part of every cell matrix,
  *   H^e_jk = 1/2 K^e_jk + sum_q w_q detJ_q V_eff(q) N_j(q) N_k(q)     (Eq. 30 terms 1-2; Eq. 40,
  *   PAPER.md:462-464), Loewdin-scaled (Eq. 34),

@@ -19,7 +19,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libchfsi.so")
 
 EXPORTED_SYMBOLS = [
-    "chfsi_create", "chfsi_destroy", "chfsi_update_potential", "chfsi_get_info", "chfsi_workspace_bytes", "chfsi_mass_diag",
+    "chfsi_create", "chfsi_create_k", "chfsi_destroy", "chfsi_update_potential", "chfsi_get_info", "chfsi_workspace_bytes", "chfsi_mass_diag",
     "chfsi_apply_H", "chfsi_overlap_matrix", "chfsi_projected_hamiltonian", "chfsi_subspace_transform",
     "chfsi_cholesky_inverse", "chfsi_overlap_matrix_mixed", "chfsi_projected_hamiltonian_mixed", "chfsi_subspace_transform_mixed", "chfsi_chebyshev_filter", "chfsi_chebyshev_filter_chunked", "chfsi_chebyshev_filter_host",
     "chfsi_launch_count", "chfsi_set_kernel_variant", "chfsi_set_profiling", "chfsi_get_profile",
@@ -31,6 +31,10 @@ class ChfsiError(RuntimeError):
     def __init__(self, code: int, msg: str):
         super().__init__(f"libchfsi error {code}: {msg}")
         self.code = code
+
+
+class _KPoint(C.Structure):
+    _fields_ = [("k", C.c_double * 3), ("chi_q_im", C.c_void_p)]
 
 
 class _Mesh(C.Structure):
@@ -80,6 +84,9 @@ def load_library(build_if_missing: bool = True):
     lib_.chfsi_create.argtypes = [C.POINTER(vp), C.POINTER(_Mesh), C.POINTER(_Potential), C.POINTER(_Nonlocal),
                                   C.c_int, C.c_int, vp]
     lib_.chfsi_create.restype = C.c_int
+    lib_.chfsi_create_k.argtypes = [C.POINTER(vp), C.POINTER(_Mesh), C.POINTER(_Potential), C.POINTER(_Nonlocal),
+                                    C.POINTER(_KPoint), C.c_int, vp]
+    lib_.chfsi_create_k.restype = C.c_int
     lib_.chfsi_destroy.argtypes = [vp]
     lib_.chfsi_destroy.restype = C.c_int
     lib_.chfsi_update_potential.argtypes = [vp, C.POINTER(_Potential), vp]
@@ -155,8 +162,11 @@ class Operator:
     """Owns one `chfsi_op` handle.  Inputs are host NumPy arrays (copied by the library during the call)."""
 
     def __init__(self, p, cell_dofs, cell_vertices, n_dofs, veff_q, n_proj=0, D=None, proj_cell_ptr=None,
-                 proj_cell_idx=None, chi_q=None, precision=64, assembly=0, stream=None):
+                 proj_cell_idx=None, chi_q=None, precision=64, assembly=0, stream=None, kvec=None, chi_q_im=None):
+        """kvec (3 floats, bohr^-1) selects the k-point variant (chfsi_create_k): blocks are then complex128 tensors and
+        chi_q / chi_q_im hold the real / imaginary parts of the Bloch-phased projector samples."""
         self._h = None
+        self.kpoint = kvec is not None
         L = load_library()
         import torch
         if not torch.cuda.is_available():
@@ -176,8 +186,19 @@ class Operator:
             keep += [D, ptr, idx, chi]
             nlp = C.pointer(_Nonlocal(int(n_proj), _np_ptr(D), _np_ptr(ptr), _np_ptr(idx), _np_ptr(chi)))
         h = C.c_void_p()
-        rc = L.chfsi_create(C.byref(h), C.byref(mesh), C.byref(pot), nlp, int(precision), int(assembly),
-                            _stream_ptr(stream))
+        if self.kpoint:
+            kp = _KPoint()
+            for i in range(3):
+                kp.k[i] = float(kvec[i])
+            if n_proj:
+                chi_im = np.ascontiguousarray(chi_q_im if chi_q_im is not None else np.zeros_like(chi), dtype=np.float64)
+                keep.append(chi_im)
+                kp.chi_q_im = chi_im.ctypes.data
+            rc = L.chfsi_create_k(C.byref(h), C.byref(mesh), C.byref(pot), nlp, C.byref(kp), int(assembly),
+                                  _stream_ptr(stream))
+        else:
+            rc = L.chfsi_create(C.byref(h), C.byref(mesh), C.byref(pot), nlp, int(precision), int(assembly),
+                                _stream_ptr(stream))
         if rc != 0:
             raise ChfsiError(rc, (L.chfsi_last_error(None) or b"").decode())
         self._h = h
@@ -191,8 +212,10 @@ class Operator:
 
     @classmethod
     def from_workload(cls, wl, precision=64, assembly=0, stream=None):
+        """wl.kvec set (workloads.generate.make_workload(kvec=...)): the k-point variant."""
         return cls(wl.p, wl.cell_dofs, wl.cell_vertices, wl.n_dofs, wl.veff_q, wl.n_proj, wl.D, wl.proj_cell_ptr,
-                   wl.proj_cell_idx, wl.chi_q, precision=precision, assembly=assembly, stream=stream)
+                   wl.proj_cell_idx, wl.chi_q, precision=precision, assembly=assembly, stream=stream,
+                   kvec=getattr(wl, "kvec", None), chi_q_im=getattr(wl, "chi_q_im", None))
 
     # -- helpers ------------------------------------------------------------------------------------------
     def _check(self, rc: int):
@@ -202,6 +225,8 @@ class Operator:
     @property
     def dtype(self):
         import torch
+        if self.kpoint:
+            return torch.complex128
         return torch.float64 if self.precision == 64 else torch.float32
 
     def _block(self, X, name):
@@ -360,7 +385,7 @@ class Operator:
                 raise TypeError("X_host: expected a 2-D CPU tensor of the operator's precision, vector index fastest")
             ptr, ld, N, rows = X_host.data_ptr(), X_host.stride(0), X_host.shape[1], X_host.shape[0]
         else:
-            want = np.float64 if self.precision == 64 else np.float32
+            want = np.complex128 if self.kpoint else np.float64 if self.precision == 64 else np.float32
             if X_host.dtype != want or X_host.ndim != 2 or X_host.strides[1] != X_host.itemsize:
                 raise TypeError("X_host: expected a 2-D array of the operator's precision, vector index fastest")
             ptr, ld, N, rows = X_host.ctypes.data, X_host.strides[0] // X_host.itemsize, X_host.shape[1], X_host.shape[0]

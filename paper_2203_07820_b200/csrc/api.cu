@@ -51,6 +51,7 @@ void free_op(chfsi_op* op) {
   cudaFree(op->proj_ptr); cudaFree(op->proj_pcrow); cudaFree(op->seg_ptr); cudaFree(op->grow_dof); cudaFree(op->pcoef);
   cudaFree(op->grp_seg_ptr); cudaFree(op->proj_grp); cudaFree(op->proj_slot);
   cudaFree(op->rr_scratch); cudaFree(op->rr32[0]); cudaFree(op->rr32[1]); cudaFree(op->sf_coef); cudaFree(op->sf_sloc); cudaFree(op->crows);
+  cudaFree(op->pcoef_im); cudaFree(op->seg_slot_proj); cudaFree(op->back_segs);
   for (int i = 0; i < 2; ++i) {
     cudaFree(op->host_stage[i]);
     if (op->host_done[i]) cudaEventDestroy(op->host_done[i]);
@@ -126,6 +127,8 @@ int filter_block(chfsi_op* op, void* X, int64_t ldx, int64_t B, int32_t m, doubl
       s2 = s1; s1 = sk; sg = sn;
     }
   }
+  if (op->kpoint && m >= 2 && !scaled)
+    return fail(op, CHFSI_ERR_UNSUPPORTED, "k-point filter: block not aligned for the sum-factorised kernel, or T_m(t0) out of range");
   double s_km2 = 1.0, s_km1 = 1.0;         // s_{k-2}, s_{k-1}
   for (int k = 1; k <= m; ++k) {
     g.X = cur; g.ldx = ldcur; g.T = tgt; g.ldt = ldtgt; g.cshift = c; g.epoch = (uint32_t)k;
@@ -189,14 +192,20 @@ int check_filter_scalars(chfsi_op* op, int32_t m, double a, double b, double a0)
 
 }  // namespace
 
-extern "C" {
+namespace {
+// columns of the real block behind one column of the caller's block: 2 for the complex blocks of a k-point handle
+inline int64_t col_width(const chfsi_op* op) { return op->kpoint ? 2 : 1; }
 
-int chfsi_create(chfsi_op** out, const chfsi_mesh* mesh, const chfsi_potential* pot, const chfsi_nonlocal* nl,
-                 int precision, int assembly, void* cuda_stream) {
+int create_impl(chfsi_op** out, const chfsi_mesh* mesh, const chfsi_potential* pot_in, const chfsi_nonlocal* nl,
+                const chfsi_kpoint* kp, int precision, int assembly, void* cuda_stream) {
   if (!out) return fail(nullptr, CHFSI_ERR_BAD_ARGUMENT, "out == NULL");
   *out = nullptr;
-  if (!mesh || !pot || !mesh->cell_dofs || !mesh->cell_vertices || !pot->veff_q)
+  if (!mesh || !pot_in || !mesh->cell_dofs || !mesh->cell_vertices || !pot_in->veff_q)
     return fail(nullptr, CHFSI_ERR_BAD_ARGUMENT, "NULL mesh / potential pointer");
+  if (kp && (mesh->p > 6 || precision != 64))
+    return fail(nullptr, CHFSI_ERR_UNSUPPORTED, "the k-point variant needs FE degree p <= 6 and precision 64");
+  if (kp && !(std::isfinite(kp->k[0]) && std::isfinite(kp->k[1]) && std::isfinite(kp->k[2])))
+    return fail(nullptr, CHFSI_ERR_BAD_ARGUMENT, "non-finite k vector");
   if (mesh->p < 1 || mesh->p > 8) return fail(nullptr, CHFSI_ERR_UNSUPPORTED, "FE degree p must be in 1..8");
   if (precision != 64 && precision != 32) return fail(nullptr, CHFSI_ERR_UNSUPPORTED, "precision must be 64 or 32");
   if (assembly != 0 && assembly != 1) return fail(nullptr, CHFSI_ERR_BAD_ARGUMENT, "assembly must be 0 or 1");
@@ -213,9 +222,24 @@ int chfsi_create(chfsi_op** out, const chfsi_mesh* mesh, const chfsi_potential* 
                                              (ce != cudaSuccess ? cudaGetErrorString(ce) : "device count 0"));
   cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
 
+  if (kp && has_nl && !kp->chi_q_im) return fail(nullptr, CHFSI_ERR_BAD_ARGUMENT, "NULL chi_q_im with projectors");
   chfsi_op* op = new (std::nothrow) chfsi_op();
   if (!op) return fail(nullptr, CHFSI_ERR_OUT_OF_MEMORY, "host allocation failed");
   try {
+  // k-point variant: the term 1/2 |k|^2 of Eq. 30 joins V_eff at the Gauss points
+  std::vector<double> veff_k;
+  chfsi_potential pot_k = *pot_in;
+  const chfsi_potential* pot = pot_in;
+  if (kp) {
+    op->kpoint = true;
+    for (int i = 0; i < 3; ++i) op->kvec[i] = kp->k[i];
+    const int64_t nq = (int64_t)(mesh->p + 2) * (mesh->p + 2) * (mesh->p + 2);
+    const double half_k2 = 0.5 * (kp->k[0] * kp->k[0] + kp->k[1] * kp->k[1] + kp->k[2] * kp->k[2]);
+    veff_k.resize((size_t)(mesh->n_cells * nq));
+    for (size_t i = 0; i < veff_k.size(); ++i) veff_k[i] = pot_in->veff_q[i] + half_k2;
+    pot_k.veff_q = veff_k.data();
+    pot = &pot_k;
+  }
   op->p = mesh->p; op->n1 = mesh->p + 1; op->nq1 = mesh->p + 2;
   op->m_cell = op->n1 * op->n1 * op->n1; op->n_q = op->nq1 * op->nq1 * op->nq1;
   op->mpad = (op->m_cell + 7) / 8 * 8;
@@ -288,6 +312,16 @@ int chfsi_create(chfsi_op** out, const chfsi_mesh* mesh, const chfsi_potential* 
   CKC(init_apply_kernels(op), "kernel attribute setup");
   CKC(init_sf_variant(op, tab, st), "sum-factorised variant setup");
   if (op->sf_ok) CKC(build_sf_fields(op, pot->veff_q, st), "quadrature-point fields");
+  if (kp) {
+    if (!op->sf_ok) {
+      free_op(op);
+      return fail(nullptr, CHFSI_ERR_UNSUPPORTED, "the k-point variant needs the sum-factorised kernel");
+    }
+    if (has_nl && op->nnz_cp > 0) {   // imaginary parts of the projector coefficients: the same path on chi_q_im
+      CKC(build_cell_projectors(op, plan, kp->chi_q_im, st), "cell projectors (imaginary parts)");
+      CKC(assemble_projector_rows_imag(op, plan, *mesh, st), "projector-row assembly (imaginary parts)");
+    }
+  }
   CKC(cudaStreamSynchronize(st), "sync");
 #undef CKC
   } catch (const std::bad_alloc&) {
@@ -301,6 +335,21 @@ int chfsi_create(chfsi_op** out, const chfsi_mesh* mesh, const chfsi_potential* 
   return CHFSI_OK;
 }
 
+}  // namespace
+
+extern "C" {
+
+int chfsi_create(chfsi_op** out, const chfsi_mesh* mesh, const chfsi_potential* pot, const chfsi_nonlocal* nl,
+                 int precision, int assembly, void* cuda_stream) {
+  return create_impl(out, mesh, pot, nl, nullptr, precision, assembly, cuda_stream);
+}
+
+int chfsi_create_k(chfsi_op** out, const chfsi_mesh* mesh, const chfsi_potential* pot, const chfsi_nonlocal* nl,
+                   const chfsi_kpoint* kpoint, int assembly, void* cuda_stream) {
+  if (!kpoint) return fail(nullptr, CHFSI_ERR_BAD_ARGUMENT, "kpoint == NULL");
+  return create_impl(out, mesh, pot, nl, kpoint, 64, assembly, cuda_stream);
+}
+
 int chfsi_destroy(chfsi_op* op) {
   if (!op) return CHFSI_ERR_BAD_ARGUMENT;
   free_op(op);
@@ -312,11 +361,19 @@ int chfsi_update_potential(chfsi_op* op, const chfsi_potential* pot, void* cuda_
   if (!pot || !pot->veff_q) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "NULL potential pointer");
   API_TRY
   cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  std::vector<double> veff_k;
+  const double* veff_q = pot->veff_q;
+  if (op->kpoint) {   // V_eff + 1/2 |k|^2 (Eq. 30), as at creation
+    const double half_k2 = 0.5 * (op->kvec[0] * op->kvec[0] + op->kvec[1] * op->kvec[1] + op->kvec[2] * op->kvec[2]);
+    veff_k.resize((size_t)(op->n_cells * op->n_q));
+    for (size_t i = 0; i < veff_k.size(); ++i) veff_k[i] = pot->veff_q[i] + half_k2;
+    veff_q = veff_k.data();
+  }
   cudaError_t ce = order_enter(op, st);
-  if (ce == cudaSuccess) ce = rebuild_local_matrices(op, pot->veff_q, st);
+  if (ce == cudaSuccess && !op->kpoint) ce = rebuild_local_matrices(op, veff_q, st);   // (k handles have no dense path)
   if (ce != cudaSuccess) return cuda_fail(op, ce, "update_potential (cell matrices)");
   if (op->sf_ok) {
-    ce = build_sf_fields(op, pot->veff_q, st);
+    ce = build_sf_fields(op, veff_q, st);
     if (ce != cudaSuccess) return cuda_fail(op, ce, "update_potential (quadrature-point fields)");
     op->launches++;
   }
@@ -356,7 +413,7 @@ int chfsi_get_info(const chfsi_op* op, chfsi_info* info) {
 
 int chfsi_workspace_bytes(const chfsi_op* op, int64_t B, size_t* bytes) {
   if (!op || !bytes || B < 1) return CHFSI_ERR_BAD_ARGUMENT;
-  *bytes = ws_layout(op, B).total;
+  *bytes = ws_layout(op, B * col_width(op)).total;
   return CHFSI_OK;
 }
 
@@ -369,6 +426,7 @@ int chfsi_mass_diag(const chfsi_op* op, double* M_dev, void* cuda_stream) {
 
 int chfsi_apply_H(chfsi_op* op, const void* X_dev, int64_t ldx, void* Y_dev, int64_t ldy, int64_t B,
                   void* workspace_dev, void* cuda_stream) {
+  if (op) { ldx *= col_width(op); ldy *= col_width(op); B *= col_width(op); }    // complex columns = pairs of real columns
   int rc = check_block_args(op, X_dev, ldx, B, workspace_dev);
   if (rc) return rc;
   if (!Y_dev) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "NULL output block");
@@ -396,6 +454,7 @@ int chfsi_apply_H(chfsi_op* op, const void* X_dev, int64_t ldx, void* Y_dev, int
 
 int chfsi_chebyshev_filter(chfsi_op* op, void* X_dev, int64_t ldx, int64_t B, int32_t m, double a, double b,
                            double a0, void* workspace_dev, void* cuda_stream) {
+  if (op) { ldx *= col_width(op); B *= col_width(op); }
   int rc = check_block_args(op, X_dev, ldx, B, workspace_dev);
   if (rc) return rc;
   if ((rc = check_filter_scalars(op, m, a, b, a0))) return rc;
@@ -412,6 +471,7 @@ int chfsi_chebyshev_filter(chfsi_op* op, void* X_dev, int64_t ldx, int64_t B, in
 
 int chfsi_chebyshev_filter_chunked(chfsi_op* op, void* X_dev, int64_t ldx, int64_t N, int64_t B, int32_t m,
                                    double a, double b, double a0, void* workspace_dev, void* cuda_stream) {
+  if (op) { ldx *= col_width(op); B *= col_width(op); N *= col_width(op); }
   int rc = check_block_args(op, X_dev, ldx, B, workspace_dev);
   if (rc) return rc;
   if (N < 1 || ldx < N) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "need 1 <= N <= ld");
@@ -435,6 +495,7 @@ int chfsi_chebyshev_filter_host(chfsi_op* op, void* X_host, int64_t ldx, int64_t
                                 double b, double a0) {
   if (!op) return CHFSI_ERR_BAD_ARGUMENT;
   if (!X_host) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "NULL host block");
+  ldx *= col_width(op); N *= col_width(op); B *= col_width(op);
   if (B < 1 || N < 1 || ldx < N) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "need B >= 1 and 1 <= N <= ld");
   int rc = check_filter_scalars(op, m, a, b, a0);
   if (rc) return rc;
@@ -515,6 +576,7 @@ int check_rr_args(chfsi_op* op, const void* Y, int64_t ldy, int64_t N, const voi
 }  // namespace
 
 int chfsi_overlap_matrix(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N, double* S_dev, void* cuda_stream) {
+  if (op && op->kpoint) return fail(op, CHFSI_ERR_UNSUPPORTED, "real-block entry point called on a k-point handle");
   int rc = check_rr_args(op, Y_dev, ldy, N, S_dev);
   if (rc) return rc;
   API_TRY
@@ -529,6 +591,7 @@ int chfsi_overlap_matrix(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N
 
 int chfsi_projected_hamiltonian(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N, int64_t B, double* H_dev,
                                 void* workspace_dev, void* cuda_stream) {
+  if (op && op->kpoint) return fail(op, CHFSI_ERR_UNSUPPORTED, "real-block entry point called on a k-point handle");
   int rc = check_rr_args(op, Y_dev, ldy, N, H_dev);
   if (rc) return rc;
   if (B < 2 || B % 2 != 0) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "chunk width B must be even and >= 2");
@@ -567,6 +630,7 @@ int chfsi_projected_hamiltonian(chfsi_op* op, const void* Y_dev, int64_t ldy, in
 
 int chfsi_subspace_transform(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N, const double* Z_dev, int64_t ldz,
                              int64_t N2, void* Out_dev, int64_t ldo, void* cuda_stream) {
+  if (op && op->kpoint) return fail(op, CHFSI_ERR_UNSUPPORTED, "real-block entry point called on a k-point handle");
   int rc = check_rr_args(op, Y_dev, ldy, N, Out_dev);
   if (rc) return rc;
   if (!Z_dev) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "NULL transformation matrix");
@@ -620,6 +684,7 @@ int chfsi_cholesky_inverse(chfsi_op* op, const double* S_dev, int64_t N, double*
 
 int chfsi_overlap_matrix_mixed(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N, int64_t block, double* S_dev,
                                void* cuda_stream) {
+  if (op && op->kpoint) return fail(op, CHFSI_ERR_UNSUPPORTED, "real-block entry point called on a k-point handle");
   int rc = check_rr_args(op, Y_dev, ldy, N, S_dev);
   if (rc) return rc;
   if (block < 2 || block % 2 != 0) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "block width must be even and >= 2");
@@ -644,6 +709,7 @@ int chfsi_overlap_matrix_mixed(chfsi_op* op, const void* Y_dev, int64_t ldy, int
 
 int chfsi_projected_hamiltonian_mixed(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N, int64_t B, int64_t n_oc,
                                       double* H_dev, void* workspace_dev, void* cuda_stream) {
+  if (op && op->kpoint) return fail(op, CHFSI_ERR_UNSUPPORTED, "real-block entry point called on a k-point handle");
   int rc = check_rr_args(op, Y_dev, ldy, N, H_dev);
   if (rc) return rc;
   if (B < 2 || B % 2 != 0) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "chunk width B must be even and >= 2");
@@ -688,6 +754,7 @@ int chfsi_projected_hamiltonian_mixed(chfsi_op* op, const void* Y_dev, int64_t l
 
 int chfsi_subspace_transform_mixed(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N, const double* Z_dev, int64_t ldz,
                                    void* Out_dev, int64_t ldo, void* cuda_stream) {
+  if (op && op->kpoint) return fail(op, CHFSI_ERR_UNSUPPORTED, "real-block entry point called on a k-point handle");
   int rc = check_rr_args(op, Y_dev, ldy, N, Out_dev);
   if (rc) return rc;
   if (!Z_dev) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "NULL transformation matrix");

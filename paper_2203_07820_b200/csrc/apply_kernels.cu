@@ -663,25 +663,33 @@ __global__ void __launch_bounds__(kP2Threads, 2) k_apply_dmma_p(ApplyDev<S> a, P
 // -------------------------------------------------------------------------------------------------------------
 constexpr int kPTRows = 8, kPTStages = 6, kPTAhead = kPTStages - 2;
 template <typename T>
-size_t pt_smem_bytes() {
-  return (size_t)kPTStages * kPTRows * kPRCols * sizeof(T) + (size_t)kProjSegRows * kProjGroup * sizeof(T) +
+size_t pt_smem_bytes(bool cplx = false) {
+  return (size_t)kPTStages * kPTRows * kPRCols * sizeof(T) + (size_t)(cplx ? 2 : 1) * kProjSegRows * kProjGroup * sizeof(T) +
          (size_t)(kProjSegRows + 8) * sizeof(int32_t) + 2 * kPTStages * sizeof(uint64_t);
 }
-template <typename T>
+// CPLX (k-point variant): the columns are (re, im) pairs and the coefficients complex, P = conj(C)^T X (Eq. 33 with the
+// Bloch phases): the thread of a real column adds  cr x_own + ci x_partner  (even column: Re P = cr xr + ci xi;
+// odd column: Im P = cr xi - ci xr).
+template <typename T, bool CPLX>
 __global__ void __launch_bounds__(256, 2) k_proj_rows_tma(const int32_t* __restrict__ seg_ptr, const int32_t* __restrict__ grow_dof,
-                                                          const T* __restrict__ pcoef, double* __restrict__ Pc, int B,
+                                                          const T* __restrict__ pcoef, const T* __restrict__ pcoef_im,
+                                                          double* __restrict__ Pc, int B,
                                                           const __grid_constant__ CUtensorMap tmX) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   T* ring = reinterpret_cast<T*>(smem_raw);                                        // [stages][8 rows][256 columns]
-  T* cs = ring + kPTStages * kPTRows * kPRCols;                                    // [128][8]
-  int32_t* dofs = reinterpret_cast<int32_t*>(cs + kProjSegRows * kProjGroup);     // [128 + 8]
+  T* cs = ring + kPTStages * kPTRows * kPRCols;                                    // [128][8] (+ [128][8] imaginary parts)
+  T* csi = cs + kProjSegRows * kProjGroup;
+  int32_t* dofs = reinterpret_cast<int32_t*>(cs + (CPLX ? 2 : 1) * kProjSegRows * kProjGroup);     // [128 + 8]
   uint64_t* full = reinterpret_cast<uint64_t*>(dofs + kProjSegRows + 8);
   uint64_t* empty = full + kPTStages;
   const int seg = blockIdx.x;
   const int r0 = seg_ptr[seg], nr = seg_ptr[seg + 1] - r0;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int col0 = blockIdx.y * kPRCols;
-  for (int e = tid; e < nr * kProjGroup; e += 256) cs[e] = pcoef[(int64_t)r0 * kProjGroup + e];
+  for (int e = tid; e < nr * kProjGroup; e += 256) {
+    cs[e] = pcoef[(int64_t)r0 * kProjGroup + e];
+    if (CPLX) csi[e] = pcoef_im[(int64_t)r0 * kProjGroup + e];
+  }
   for (int e = tid; e < kProjSegRows + 8; e += 256) dofs[e] = grow_dof[r0 + min(e, nr - 1)];   // tail: any valid row
   if (tid == 0) {
     for (int s = 0; s < kPTStages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 8); }
@@ -719,6 +727,12 @@ __global__ void __launch_bounds__(256, 2) k_proj_rows_tma(const int32_t* __restr
       const double x = (double)xs[r * kPRCols];
 #pragma unroll
       for (int i = 0; i < kProjGroup; ++i) acc[i] = fma((double)cp[r * kProjGroup + i], x, acc[i]);
+      if (CPLX) {
+        const double xp = (tid & 1) ? -(double)xs[r * kPRCols - 1] : (double)xs[r * kPRCols + 1];   // partner column of the pair
+        const T* ci = csi + (pi * kPTRows + r) * kProjGroup;
+#pragma unroll
+        for (int i = 0; i < kProjGroup; ++i) acc[i] = fma((double)ci[i], xp, acc[i]);
+      }
     }
     __syncwarp();
     if (lane == 0) mbar_arrive(&empty[s]);
@@ -727,6 +741,45 @@ __global__ void __launch_bounds__(256, 2) k_proj_rows_tma(const int32_t* __restr
   if (col < B) {
 #pragma unroll
     for (int i = 0; i < kProjGroup; ++i) Pc[((int64_t)seg * kProjGroup + i) * B + col] = acc[i];
+  }
+}
+
+// k-point variant, Alg. 4 steps 5-6 dof by dof: T[g] += alpha sum_j C~_{g,j} (D P)_j with complex
+// coefficients C~ = cr + i ci and complex P (column pairs re, im):  re: cr Pr - ci Pi,  im: cr Pi + ci Pr.  One CTA =
+// (segment of <= 128 rows of one projector group, 256 real columns); the segments of one launch belong to groups of one
+// colour, so no two CTAs of a launch touch the same row and a plain read-modify-write is race-free and ordered.
+template <typename T>
+__global__ void __launch_bounds__(256) k_proj_back(const int32_t* __restrict__ segs, const int32_t* __restrict__ seg_ptr,
+                                                   const int32_t* __restrict__ grow_dof, const T* __restrict__ pcoef,
+                                                   const T* __restrict__ pcoef_im, const int32_t* __restrict__ seg_slot_proj,
+                                                   const T* __restrict__ P, int B, T* __restrict__ Tg, int64_t ldt, double alpha) {
+  __shared__ T cs[kProjSegRows * kProjGroup], csi[kProjSegRows * kProjGroup];
+  __shared__ int32_t dofs[kProjSegRows];
+  const int seg = segs[blockIdx.x];
+  const int r0 = seg_ptr[seg], nr = seg_ptr[seg + 1] - r0;
+  const int tid = threadIdx.x;
+  for (int e = tid; e < nr * kProjGroup; e += 256) {
+    cs[e] = pcoef[(int64_t)r0 * kProjGroup + e];
+    csi[e] = pcoef_im[(int64_t)r0 * kProjGroup + e];
+  }
+  for (int e = tid; e < nr; e += 256) dofs[e] = grow_dof[r0 + e];
+  __syncthreads();
+  const int col = blockIdx.y * 256 + tid;
+  if (col >= B) return;
+  double pr[kProjGroup], pp[kProjGroup];
+  const double sgn = (col & 1) ? 1.0 : -1.0;
+#pragma unroll
+  for (int i = 0; i < kProjGroup; ++i) {
+    const int j = seg_slot_proj[seg * kProjGroup + i];
+    pr[i] = j >= 0 ? (double)P[(int64_t)j * B + col] : 0.0;
+    pp[i] = j >= 0 ? sgn * (double)P[(int64_t)j * B + (col ^ 1)] : 0.0;
+  }
+  for (int r = 0; r < nr; ++r) {
+    double v = 0.0;
+#pragma unroll
+    for (int i = 0; i < kProjGroup; ++i) v = fma((double)cs[r * kProjGroup + i], pr[i], fma((double)csi[r * kProjGroup + i], pp[i], v));
+    T* tp = Tg + (int64_t)dofs[r] * ldt + col;
+    *tp = (T)((double)*tp + alpha * v);
   }
 }
 
@@ -807,6 +860,7 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
   const bool use_ws = use_sf && op->variant != 5 && (g.accumulate || g.beta == 0.0) &&
                       make_row_gather_map(&tmPs, g.P, op->n_proj + 1, B, B, (int)sizeof(T), sf_tile_cols<T>(), false);
   if (g.accumulate && !use_ws) return cudaErrorNotSupported;   // the caller asks apply_accumulates() first
+  if (op->kpoint && !(use_ws && sizeof(T) == 8)) return cudaErrorNotSupported;   // the k-point variant has this one kernel
   if (!use_sf && g.cshift != op->cur_shift) {   // once per filter call: move the spectral shift onto the matrix diagonals
     const int64_t n = op->n_cells * op->m_cell;
     k_set_diag_shift<T><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(reinterpret_cast<T*>(op->mat), op->mat_off, op->idx_off,
@@ -824,9 +878,14 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
     dim3 g1((unsigned)op->n_pseg, (unsigned)((B + kPRCols - 1) / kPRCols));
     CUtensorMap tmXp;
     if (op->variant != 1 && make_row_gather_map(&tmXp, g.X, op->n_dofs, B, g.ldx, (int)sizeof(T), kPRCols)) {
-      k_proj_rows_tma<T><<<g1, 256, pt_smem_bytes<T>(), st>>>(op->seg_ptr, op->grow_dof, reinterpret_cast<const T*>(op->pcoef), Pc,
-                                                             B, tmXp);
+      if (op->kpoint)
+        k_proj_rows_tma<T, true><<<g1, 256, pt_smem_bytes<T>(true), st>>>(op->seg_ptr, op->grow_dof, reinterpret_cast<const T*>(op->pcoef),
+                                                                          reinterpret_cast<const T*>(op->pcoef_im), Pc, B, tmXp);
+      else
+        k_proj_rows_tma<T, false><<<g1, 256, pt_smem_bytes<T>(), st>>>(op->seg_ptr, op->grow_dof, reinterpret_cast<const T*>(op->pcoef),
+                                                                       nullptr, Pc, B, tmXp);
     } else {
+      if (op->kpoint) return cudaErrorNotSupported;
       const int vec_ok = (g.ldx % 2 == 0 && (uintptr_t)g.X % 16 == 0) ? 1 : 0;
       k_proj_rows<T><<<g1, 256, 0, st>>>(op->seg_ptr, op->grow_dof, reinterpret_cast<const T*>(op->pcoef), X, g.ldx, Pc, B, vec_ok);
     }
@@ -895,13 +954,36 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
     if (use_ws) {
       const unsigned gws = (unsigned)std::min<int64_t>(n_tiles, (int64_t)op->n_sm);
       pd.ticket_base = (unsigned long long)(g.epoch - 1) * (unsigned long long)(n_tiles + gws);
+      if (op->kpoint) {
+        if constexpr (sizeof(T) == 8) {
+          switch (op->p) {
+            case 1: k_apply_sf_ws<1, T, true><<<gws, kWsThreads, WsSmem<1, T, true>::bytes, st>>>(a, sf, pd, tmX, tmPs); break;
+            case 2: k_apply_sf_ws<2, T, true><<<gws, kWsThreads, WsSmem<2, T, true>::bytes, st>>>(a, sf, pd, tmX, tmPs); break;
+            case 3: k_apply_sf_ws<3, T, true><<<gws, kWsThreads, WsSmem<3, T, true>::bytes, st>>>(a, sf, pd, tmX, tmPs); break;
+            case 4: k_apply_sf_ws<4, T, true><<<gws, kWsThreads, WsSmem<4, T, true>::bytes, st>>>(a, sf, pd, tmX, tmPs); break;
+            case 5: k_apply_sf_ws<5, T, true><<<gws, kWsThreads, WsSmem<5, T, true>::bytes, st>>>(a, sf, pd, tmX, tmPs); break;
+            case 6: k_apply_sf_ws<6, T, true><<<gws, kWsThreads, WsSmem<6, T, true>::bytes, st>>>(a, sf, pd, tmX, tmPs); break;
+          }
+        }
+      } else
       switch (op->p) {
-        case 1: k_apply_sf_ws<1, T><<<gws, kWsThreads, WsSmem<1, T>::bytes, st>>>(a, sf, pd, tmX, tmPs); break;
-        case 2: k_apply_sf_ws<2, T><<<gws, kWsThreads, WsSmem<2, T>::bytes, st>>>(a, sf, pd, tmX, tmPs); break;
-        case 3: k_apply_sf_ws<3, T><<<gws, kWsThreads, WsSmem<3, T>::bytes, st>>>(a, sf, pd, tmX, tmPs); break;
-        case 4: k_apply_sf_ws<4, T><<<gws, kWsThreads, WsSmem<4, T>::bytes, st>>>(a, sf, pd, tmX, tmPs); break;
-        case 5: k_apply_sf_ws<5, T><<<gws, kWsThreads, WsSmem<5, T>::bytes, st>>>(a, sf, pd, tmX, tmPs); break;
-        case 6: k_apply_sf_ws<6, T><<<gws, kWsThreads, WsSmem<6, T>::bytes, st>>>(a, sf, pd, tmX, tmPs); break;
+        case 1: k_apply_sf_ws<1, T, false><<<gws, kWsThreads, WsSmem<1, T>::bytes, st>>>(a, sf, pd, tmX, tmPs); break;
+        case 2: k_apply_sf_ws<2, T, false><<<gws, kWsThreads, WsSmem<2, T>::bytes, st>>>(a, sf, pd, tmX, tmPs); break;
+        case 3: k_apply_sf_ws<3, T, false><<<gws, kWsThreads, WsSmem<3, T>::bytes, st>>>(a, sf, pd, tmX, tmPs); break;
+        case 4: k_apply_sf_ws<4, T, false><<<gws, kWsThreads, WsSmem<4, T>::bytes, st>>>(a, sf, pd, tmX, tmPs); break;
+        case 5: k_apply_sf_ws<5, T, false><<<gws, kWsThreads, WsSmem<5, T>::bytes, st>>>(a, sf, pd, tmX, tmPs); break;
+        case 6: k_apply_sf_ws<6, T, false><<<gws, kWsThreads, WsSmem<6, T>::bytes, st>>>(a, sf, pd, tmX, tmPs); break;
+      }
+      if (op->kpoint && op->n_pseg > 0) {
+        for (size_t c = 0; c + 1 < op->back_color_ptr.size(); ++c) {
+          const int n_seg_c = op->back_color_ptr[c + 1] - op->back_color_ptr[c];
+          if (n_seg_c == 0) continue;
+          dim3 gb((unsigned)n_seg_c, (unsigned)((B + 255) / 256));
+          k_proj_back<T><<<gb, 256, 0, st>>>(op->back_segs + op->back_color_ptr[c], op->seg_ptr, op->grow_dof,
+                                             reinterpret_cast<const T*>(op->pcoef), reinterpret_cast<const T*>(op->pcoef_im),
+                                             op->seg_slot_proj, P, B, Tg, g.ldt, g.alpha);
+          op->launches++;
+        }
       }
     } else
     switch (op->p) {
@@ -1036,8 +1118,9 @@ cudaError_t init_apply_kernels(Op* op) {
       if ((e = cudaFuncSetAttribute(k_apply_tf32_p<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_t3))) return e;
     }
   }
-  if ((e = cudaFuncSetAttribute(k_proj_rows_tma<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pt_smem_bytes<double>()))) return e;
-  if ((e = cudaFuncSetAttribute(k_proj_rows_tma<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pt_smem_bytes<float>()))) return e;
+  if ((e = cudaFuncSetAttribute(k_proj_rows_tma<double, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pt_smem_bytes<double>()))) return e;
+  if ((e = cudaFuncSetAttribute(k_proj_rows_tma<float, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pt_smem_bytes<float>()))) return e;
+  if ((e = cudaFuncSetAttribute(k_proj_rows_tma<double, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pt_smem_bytes<double>(true)))) return e;
   size_t smem_gen = (size_t)op->max_ktot * 32 * 8;
   if (smem_gen > 227 * 1024) return cudaErrorInvalidValue;
   if ((e = cudaFuncSetAttribute(k_apply_generic<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_gen))) return e;
@@ -1060,15 +1143,16 @@ template <int P>
 cudaError_t sf_set_attr(Op* op) {
   cudaError_t e;
   if ((e = cudaFuncSetAttribute(k_apply_sf<P, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sf_smem_bytes<P, double>(op)))) return e;
-  if ((e = cudaFuncSetAttribute(k_apply_sf_ws<P, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, WsSmem<P, double>::bytes))) return e;
-  if ((e = cudaFuncSetAttribute(k_apply_sf_ws<P, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, WsSmem<P, float>::bytes))) return e;
+  if ((e = cudaFuncSetAttribute(k_apply_sf_ws<P, double, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, WsSmem<P, double>::bytes))) return e;
+  if ((e = cudaFuncSetAttribute(k_apply_sf_ws<P, float, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, WsSmem<P, float>::bytes))) return e;
+  if ((e = cudaFuncSetAttribute(k_apply_sf_ws<P, double, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, WsSmem<P, double, true>::bytes))) return e;
   return cudaFuncSetAttribute(k_apply_sf<P, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sf_smem_bytes<P, float>(op));
 }
 }  // namespace
 
 cudaError_t init_sf_variant(Op* op, const Tables1D& tab, cudaStream_t st) {
   op->sf_ok = false;
-  if (op->p > 6 || op->max_ktot - op->mpad > kSfMaxProj) return cudaSuccess;
+  if (op->p > 6 || (!op->kpoint && op->max_ktot - op->mpad > kSfMaxProj)) return cudaSuccess;   // (k-point variant: no projector data in the kernel)
   const int n1 = tab.n1, nq1 = tab.nq1;
   // Phi[q][i] = l_i(x_q): the Lagrange (GLL) basis at the Gauss points; Dh[q'][q] = derivative of the Lagrange polynomial
   // through the GAUSS points at Gauss point q' (barycentric form, long double), both zero-padded to 8 x 8
@@ -1113,11 +1197,13 @@ cudaError_t init_sf_variant(Op* op, const Tables1D& tab, cudaStream_t st) {
   return cudaSuccess;
 }
 
-cudaError_t assemble_projector_rows(Op* op, const HostPlan& plan, const chfsi_mesh& mesh, cudaStream_t st) {
-  op->n_pseg = 0; op->n_prow = (int64_t)plan.grow_dof.size();
-  const size_t elt = op->precision == 64 ? 8 : 4;
+namespace {
+// Dof-centric projector coefficients coef[row][slot] = sum over the cells of the row's dof of the projector rows that the
+// cell matrices hold right now (Alg. 4's assembly over cells applied to C once, in the caller's CSR order: deterministic).
+// *d_rows_out (optional) receives the compact device copy [nnz_cp][mpad] of those rows; the caller owns it.
+cudaError_t projector_coefficients(Op* op, const HostPlan& plan, const chfsi_mesh& mesh, cudaStream_t st,
+                                   std::vector<double>* coef_out, double** d_rows_out) {
   cudaError_t e;
-  if (op->n_proj == 0 || op->n_prow == 0 || op->nnz_cp == 0) return cudaSuccess;
   const int mc = op->m_cell;
   // 1. compact FP64 copy of the projector rows of the cell matrices ([nnz_cp][mpad], zero-padded), on the host
   std::vector<int32_t> row_cell((size_t)op->nnz_cp);
@@ -1127,7 +1213,6 @@ cudaError_t assemble_projector_rows(Op* op, const HostPlan& plan, const chfsi_me
   if ((e = cudaMalloc((void**)&d_row_cell, row_cell.size() * sizeof(int32_t)))) return e;
   const int mpad = op->mpad;
   if ((e = cudaMalloc((void**)&d_rows, (size_t)op->nnz_cp * mpad * sizeof(double)))) { cudaFree(d_row_cell); return e; }
-  op->crows = d_rows;   // kept: the sum-factorised kernel applies C~^c P from these rows (freed with the operator)
   std::vector<double> rows((size_t)op->nnz_cp * mpad);
   e = cudaMemcpyAsync(d_row_cell, row_cell.data(), row_cell.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st);
   if (e == cudaSuccess) {
@@ -1142,9 +1227,12 @@ cudaError_t assemble_projector_rows(Op* op, const HostPlan& plan, const chfsi_me
   if (e == cudaSuccess) e = cudaMemcpyAsync(rows.data(), d_rows, rows.size() * sizeof(double), cudaMemcpyDeviceToHost, st);
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);
   cudaFree(d_row_cell);
+  if (e != cudaSuccess || !d_rows_out) cudaFree(d_rows);
   if (e != cudaSuccess) return e;
+  if (d_rows_out) *d_rows_out = d_rows;
   // 2. assembly over the cells of each projector, in the caller's CSR order (deterministic)
-  std::vector<double> coef((size_t)op->n_prow * kProjGroup, 0.0);
+  std::vector<double>& coef = *coef_out;
+  coef.assign((size_t)op->n_prow * kProjGroup, 0.0);
   std::vector<int32_t> loc((size_t)op->n_dofs, -1);
   for (int grp = 0; grp < plan.n_groups; ++grp) {
     for (int32_t r = plan.grp_row_ptr[grp]; r < plan.grp_row_ptr[grp + 1]; ++r) loc[plan.grow_dof[r]] = r;
@@ -1158,19 +1246,75 @@ cudaError_t assemble_projector_rows(Op* op, const HostPlan& plan, const chfsi_me
       }
     }
   }
-  // 3. upload in the operator's storage type
-  if ((e = cudaMalloc(&op->pcoef, coef.size() * elt))) return e;
+  return cudaSuccess;
+}
+// upload in the operator's storage type
+cudaError_t upload_coefficients(Op* op, const std::vector<double>& coef, void** dst, cudaStream_t st) {
+  const size_t elt = op->precision == 64 ? 8 : 4;
+  cudaError_t e;
+  if ((e = cudaMalloc(dst, coef.size() * elt))) return e;
   if (op->precision == 64) {
-    e = cudaMemcpyAsync(op->pcoef, coef.data(), coef.size() * sizeof(double), cudaMemcpyHostToDevice, st);
+    e = cudaMemcpyAsync(*dst, coef.data(), coef.size() * sizeof(double), cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
   } else {
     std::vector<float> cf(coef.begin(), coef.end());
-    e = cudaMemcpyAsync(op->pcoef, cf.data(), cf.size() * sizeof(float), cudaMemcpyHostToDevice, st);
+    e = cudaMemcpyAsync(*dst, cf.data(), cf.size() * sizeof(float), cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
   }
+  return e;
+}
+}  // namespace
+
+cudaError_t assemble_projector_rows(Op* op, const HostPlan& plan, const chfsi_mesh& mesh, cudaStream_t st) {
+  op->n_pseg = 0; op->n_prow = (int64_t)plan.grow_dof.size();
+  if (op->n_proj == 0 || op->n_prow == 0 || op->nnz_cp == 0) return cudaSuccess;
+  std::vector<double> coef;
+  // the compact rows are kept: the sum-factorised kernels apply C~^c P from them (freed with the operator)
+  cudaError_t e = projector_coefficients(op, plan, mesh, st, &coef, &op->crows);
   if (e != cudaSuccess) return e;
+  if ((e = upload_coefficients(op, coef, &op->pcoef, st))) return e;
   op->n_pseg = (int64_t)plan.seg_ptr.size() - 1;
   return cudaSuccess;
+}
+
+cudaError_t assemble_projector_rows_imag(Op* op, const HostPlan& plan, const chfsi_mesh& mesh, cudaStream_t st) {
+  if (op->n_pseg == 0) return cudaSuccess;
+  std::vector<double> coef;
+  cudaError_t e = projector_coefficients(op, plan, mesh, st, &coef, nullptr);
+  if (e != cudaSuccess) return e;
+  if ((e = upload_coefficients(op, coef, &op->pcoef_im, st))) return e;
+  // projector of every (segment, slot), and the segments ordered by a colouring of the groups in which two groups that
+  // share a dof differ: the back-projection adds into the target block one colour per launch, so that every dof is
+  // summed in one fixed order
+  const int n_seg = (int)op->n_pseg;
+  std::vector<int32_t> seg_slot((size_t)n_seg * kProjGroup, -1), seg_color((size_t)n_seg, 0);
+  std::vector<uint32_t> used((size_t)op->n_dofs, 0u);
+  int n_colors = 0;
+  for (int grp = 0; grp < plan.n_groups; ++grp) {
+    uint32_t mask = 0;
+    for (int32_t r = plan.grp_row_ptr[grp]; r < plan.grp_row_ptr[grp + 1]; ++r) mask |= used[plan.grow_dof[r]];
+    int col = 0;
+    while (col < 31 && (mask >> col & 1u)) ++col;
+    for (int32_t r = plan.grp_row_ptr[grp]; r < plan.grp_row_ptr[grp + 1]; ++r) used[plan.grow_dof[r]] |= 1u << col;
+    n_colors = std::max(n_colors, col + 1);
+    for (int32_t sg = plan.grp_seg_ptr[grp]; sg < plan.grp_seg_ptr[grp + 1]; ++sg) {
+      seg_color[sg] = col;
+      for (int i = 0; i < kProjGroup; ++i) seg_slot[(size_t)sg * kProjGroup + i] = plan.grp_proj[(size_t)grp * kProjGroup + i];
+    }
+  }
+  std::vector<int32_t> order;
+  op->back_color_ptr.assign(1, 0);
+  for (int col = 0; col < n_colors; ++col) {
+    for (int sg = 0; sg < n_seg; ++sg)
+      if (seg_color[sg] == col) order.push_back(sg);
+    op->back_color_ptr.push_back((int32_t)order.size());
+  }
+  if ((e = cudaMalloc((void**)&op->seg_slot_proj, seg_slot.size() * sizeof(int32_t)))) return e;
+  if ((e = cudaMalloc((void**)&op->back_segs, order.size() * sizeof(int32_t)))) return e;
+  e = cudaMemcpyAsync(op->seg_slot_proj, seg_slot.data(), seg_slot.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(op->back_segs, order.data(), order.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  return e;
 }
 
 cudaError_t capture_diagonal(Op* op, cudaStream_t st) {

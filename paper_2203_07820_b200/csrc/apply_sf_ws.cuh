@@ -36,15 +36,18 @@ constexpr int kWsThreads = 32 * (kWsComputeWarps + kWsHelperWarps);
 template <typename S> __host__ __device__ constexpr int ws_regs_compute() { return sizeof(S) == 8 ? 224 : 232; }
 template <typename S> __host__ __device__ constexpr int ws_regs_helper() { return sizeof(S) == 8 ? 56 : 40; }
 
-template <int P, typename S>
+// KP = k-point variant: a column pair is one complex column (re, im); ten fields per Gauss point (the last three carry
+// w detJ J^-1 k); no projector data here -- the back-projection C (D P) is k_proj_back's.
+template <int P, typename S, bool KP = false>
 struct WsSmem {
   static constexpr int n1 = P + 1, nq1 = P + 2, mc = n1 * n1 * n1, mpad = (mc + 7) / 8 * 8;
   static constexpr int TN = sf_tile_cols<S>();
   static constexpr int tile_bytes = (mpad * 128 + 1023) / 1024 * 1024;      // TMA swizzle atoms: 1024-byte aligned buffers
-  static constexpr int coef_elems = nq1 * 7 * 64;
+  static constexpr int NF = KP ? 10 : 7;                                    // fields per Gauss point
+  static constexpr int coef_elems = nq1 * NF * 64;
   static constexpr int coef_bytes = coef_elems * 8;
-  static constexpr int crow_bytes = (kSfCrowChunk * mpad * 8 + 127) / 128 * 128;
-  static constexpr int ps_bytes = kSfMaxProj * 128;                         // [kSfMaxProj][TN] of S: 128-byte rows
+  static constexpr int crow_bytes = KP ? 0 : (kSfCrowChunk * mpad * 8 + 127) / 128 * 128;
+  static constexpr int ps_bytes = KP ? 0 : kSfMaxProj * 128;                         // [kSfMaxProj][TN] of S: 128-byte rows
   static constexpr int idx_stride = mpad + kSfMaxProj;
   static constexpr int small_bytes = (idx_stride * 4 + mpad * 8 + 127) / 128 * 128;   // index list, then M^-1/2 (doubles)
   static constexpr int off_xt = 0;                                          // [2][tile_bytes]
@@ -61,11 +64,12 @@ struct WsSmem {
 
 __device__ __forceinline__ void ws_asm_sync() { asm volatile("bar.sync 1, %0;" ::"n"(32 * kWsAsmWarps) : "memory"); }
 
-template <int P, typename S>
+template <int P, typename S, bool KP>
 __global__ void __launch_bounds__(kWsThreads, 1) k_apply_sf_ws(ApplyDev<S> a, SfDev sf, PersistDev pd,
                                                                const __grid_constant__ CUtensorMap tmX,
                                                                const __grid_constant__ CUtensorMap tmP) {
-  using L = WsSmem<P, S>;
+  using L = WsSmem<P, S, KP>;
+  constexpr int NF = L::NF;
   constexpr int n1 = L::n1, nq1 = L::nq1, nn = n1 * n1, mc = L::mc, mpad = L::mpad;
   constexpr int TN = L::TN;
   constexpr int NT = TN / 8;
@@ -239,8 +243,19 @@ __global__ void __launch_bounds__(kWsThreads, 1) k_apply_sf_ws(ApplyDev<S> a, Sf
 #pragma unroll
               for (int u = 0; u < 2; ++u) { dz[u][0] += dzo[u][0]; dz[u][1] += dzo[u][1]; }
             }
-            const double2* cq = reinterpret_cast<const double2*>(coef_s) + (q * 7) * 32 + lane;
+            const double2* cq = reinterpret_cast<const double2*>(coef_s) + (q * NF) * 32 + lane;
             const double2 W0 = cq[0], Gxx = cq[32], Gxy = cq[64], Gxz = cq[96], Gyy = cq[128], Gyz = cq[160], Gzz = cq[192];
+            if (KP) {
+              // -i int N_j k.grad u (Eq. 30 last term) on (re, im) = (u = 0, u = 1):  re += kap.grad u_im,
+              // im -= kap.grad u_re  with kap = w detJ J^-1 k
+              const double2 Kx = cq[224], Ky = cq[256], Kz = cq[288];
+              const double r0 = fma(Kx.x, dx[0][0], fma(Ky.x, dy[0][0], Kz.x * dz[0][0]));
+              const double r1 = fma(Kx.y, dx[0][1], fma(Ky.y, dy[0][1], Kz.y * dz[0][1]));
+              const double i0 = fma(Kx.x, dx[1][0], fma(Ky.x, dy[1][0], Kz.x * dz[1][0]));
+              const double i1 = fma(Kx.y, dx[1][1], fma(Ky.y, dy[1][1], Kz.y * dz[1][1]));
+              w[q][0][0] += i0; w[q][0][1] += i1;
+              w[q][1][0] -= r0; w[q][1][1] -= r1;
+            }
             double gz[2][2];
 #pragma unroll
             for (int u = 0; u < 2; ++u) {
@@ -337,7 +352,7 @@ __global__ void __launch_bounds__(kWsThreads, 1) k_apply_sf_ws(ApplyDev<S> a, Sf
       auto issue_small = [&](long long tk, int s) {
         const int cell_l = pd.pos_cell[(int)(tk / nct)];
         unsigned char* dst = smem_dyn + L::off_small + s * L::small_bytes;
-        const uint32_t nb = (uint32_t)a.ktot[cell_l] * 4u;                       // mpad + round8(projectors of the cell) entries
+        const uint32_t nb = KP ? (uint32_t)mpad * 4u : (uint32_t)a.ktot[cell_l] * 4u;   // mpad + round8(projectors of the cell) entries
         mbar_expect_tx(bar_small + s, nb + (uint32_t)mpad * 8u);
         bulk_g2s(dst, a.gidx + a.idx_off[cell_l], nb, bar_small + s);
         bulk_g2s(dst + L::idx_stride * 4, sf.sloc + (int64_t)cell_l * mpad, (uint32_t)mpad * 8u, bar_small + s);
@@ -360,7 +375,7 @@ __global__ void __launch_bounds__(kWsThreads, 1) k_apply_sf_ws(ApplyDev<S> a, Sf
         const int cell_l = pd.pos_cell[(int)(tk / nct)];
         const int col0_l = (int)(tk % nct) * TN;
         const int64_t cp0 = sf.cell_proj_ptr[cell_l];
-        const int np = (int)(sf.cell_proj_ptr[cell_l + 1] - cp0);
+        const int np = KP ? 0 : (int)(sf.cell_proj_ptr[cell_l + 1] - cp0);
         const int npc = min(np, kSfCrowChunk), np8 = (np + 7) / 8 * 8;
         mbar_wait(bar_small + set, (uint32_t)(iter / 3) & 1u);
         const int32_t* idx_l = reinterpret_cast<const int32_t*>(smem_dyn + L::off_small + set * L::small_bytes);
@@ -410,7 +425,7 @@ __global__ void __launch_bounds__(kWsThreads, 1) k_apply_sf_ws(ApplyDev<S> a, Sf
         const int col0 = jt * TN;
         const int ncols = min(TN, a.B - col0);
         const int64_t cp0 = sf.cell_proj_ptr[cell];
-        const int np = (int)(sf.cell_proj_ptr[cell + 1] - cp0);
+        const int np = KP ? 0 : (int)(sf.cell_proj_ptr[cell + 1] - cp0);
         const int npc = min(np, kSfCrowChunk);
         const unsigned char* xt = smem_dyn + L::off_xt + b * L::tile_bytes;
         const double* crow_s = reinterpret_cast<const double*>(smem_dyn + L::off_crow + b * L::crow_bytes);

@@ -130,6 +130,15 @@ struct Op {
   // G = 1/2 w detJ J^-1 J^-T in the kernel's lane order [n_cells][nq1][7][32][2], M^-1/2 per (cell, node)
   // [n_cells][mpad], and the projector columns s_l C^c_{l,j} as compact FP64 rows [nnz_cp][m_cell]
   bool sf_ok = false;
+  // k-point variant (chfsi_create_k): vector blocks are complex (FP64 pairs re, im = two adjacent real columns), the
+  // fields carry w detJ J^-1 k, the projector coefficients are complex (pcoef = real parts, pcoef_im = imaginary parts) and
+  // the back-projection C (D P) runs as its own dof-centric kernel (k_proj_back), one launch per colour of the projector groups
+  bool kpoint = false;
+  double kvec[3] = {0.0, 0.0, 0.0};
+  void* pcoef_im = nullptr;              // [n_prow][8]
+  int32_t* seg_slot_proj = nullptr;      // [n_pseg][8] projector (row of P) of slot i of the segment's group, -1 if empty
+  int32_t* back_segs = nullptr;          // segments ordered by the colour of their group
+  std::vector<int32_t> back_color_ptr;   // [n_back_colors + 1] into back_segs
   double* sf_coef = nullptr;
   double* sf_sloc = nullptr;
   double* crows = nullptr;
@@ -178,6 +187,8 @@ cudaError_t rebuild_local_matrices(Op* op, const double* veff_q_host, cudaStream
 // Quadrature-point fields of the sum-factorised variant (op->sf_coef, allocated on first use) from V_eff at the Gauss
 // points (HOST pointer) and the cell geometry; op->setup_* must exist.  Synchronises the stream.
 cudaError_t build_sf_fields(Op* op, const double* veff_q_host, cudaStream_t stream);
+// Projector rows of the cell matrices from projector samples at the Gauss points (HOST pointer); see setup_kernels.cu.
+cudaError_t build_cell_projectors(Op* op, const HostPlan& plan, const double* chi_host, cudaStream_t stream);
 
 // ---- apply kernels (apply_kernels.cu) ----------------------------------------------------------------------
 struct ApplyArgs {
@@ -206,6 +217,9 @@ cudaError_t launch_apply(Op* op, const ApplyArgs& a, cudaStream_t stream);
 // Builds op->pcoef: the projector rows of the cell matrices summed over the cells of each dof (once, at create,
 // after build_cell_matrices; deterministic host summation in the caller's CSR order).
 cudaError_t assemble_projector_rows(Op* op, const HostPlan& plan, const chfsi_mesh& mesh, cudaStream_t stream);
+// k-point variant: the same assembly for the imaginary parts (the cell matrices then hold them in their projector rows)
+// into op->pcoef_im, and the group / colour tables of the back-projection kernel.
+cudaError_t assemble_projector_rows_imag(Op* op, const HostPlan& plan, const chfsi_mesh& mesh, cudaStream_t stream);
 // Copies the diagonal of every cell matrix into op->diag0 (once, at create, after build_cell_matrices).
 cudaError_t capture_diagonal(Op* op, cudaStream_t stream);
 // C[N1][ldc] = A^T B over n_rows rows of two FP64 blocks [n_rows][ld] (Alg. 2 step 1); enqueued on

@@ -24,6 +24,7 @@ constexpr int kMaxNq1 = 10;
 struct Geom {
   double detJ;
   double G[3][3];  // sum_i Jinv[a][i] Jinv[b][i]
+  double Ji[3][3]; // Jinv[d][i] = d xi_d / d x_i
 };
 
 __device__ inline Geom trilinear_geom(const double* vt /*[8][3]*/, double x, double y, double z) {
@@ -57,7 +58,10 @@ __device__ inline Geom trilinear_geom(const double* vt /*[8][3]*/, double x, dou
 #pragma unroll
   for (int a = 0; a < 3; ++a)
 #pragma unroll
-    for (int b = 0; b < 3; ++b) r.G[a][b] = Ji[a][0] * Ji[b][0] + Ji[a][1] * Ji[b][1] + Ji[a][2] * Ji[b][2];
+    for (int b = 0; b < 3; ++b) {
+      r.G[a][b] = Ji[a][0] * Ji[b][0] + Ji[a][1] * Ji[b][1] + Ji[a][2] * Ji[b][2];
+      r.Ji[a][b] = Ji[a][b];
+    }
   return r;
 }
 
@@ -219,24 +223,32 @@ __global__ void __launch_bounds__(256) k_cell_projector(int n1, int nq1, SetupTa
 
 // Fields of the sum-factorised apply at the Gauss points of every cell, in the lane order of k_apply_sf:
 //   coef[c][qc][k][lane = 4 qa + qb/2][e = qb % 2],  k = 0: w detJ V_eff;  k = 1..6: 1/2 w detJ (J^-1 J^-T)_{xx,xy,xz,yy,yz,zz}
-// (the integrands of Eq. 40 / Eq. 30 term 1, before the shape functions are applied).
-__global__ void __launch_bounds__(256) k_sf_fields(int nq1, int64_t n_cells, SetupTables tb, const double* __restrict__ verts,
-                                                   const double* __restrict__ veff, double* __restrict__ coef) {
+// (the integrands of Eq. 40 / Eq. 30 term 1, before the shape functions are applied).  k-point variant
+// (nf = 10): k = 7..9: w detJ (J^-1 kvec)_d, the integrand of the last term of Eq. 30 without its factor -i:
+// k . grad_x u = sum_d (J^-1 kvec)_d d u / d xi_d.
+__global__ void __launch_bounds__(256) k_sf_fields(int nq1, int nf, int64_t n_cells, SetupTables tb, const double* __restrict__ verts,
+                                                   const double* __restrict__ veff, double kx, double ky, double kz,
+                                                   double* __restrict__ coef) {
   __shared__ double vt[24];
   const int64_t c = blockIdx.x;
   const int nq2 = nq1 * nq1, nq = nq1 * nq2;
   if (threadIdx.x < 24) vt[threadIdx.x] = verts[c * 24 + threadIdx.x];
   __syncthreads();
-  double* out = coef + c * (int64_t)nq1 * 7 * 64;
+  double* out = coef + c * (int64_t)nq1 * nf * 64;
   for (int q = threadIdx.x; q < nq; q += blockDim.x) {
     const int qa = q % nq1, qb = (q / nq1) % nq1, qc = q / nq2;
     const Geom g = trilinear_geom(vt, tb.gq_x[qa], tb.gq_x[qb], tb.gq_x[qc]);
     const double wj = tb.gq_w[qa] * tb.gq_w[qb] * tb.gq_w[qc] * g.detJ;
     const int slot = (4 * qa + (qb >> 1)) * 2 + (qb & 1);
-    double* o = out + (int64_t)qc * 7 * 64 + slot;
+    double* o = out + (int64_t)qc * nf * 64 + slot;
     o[0] = wj * veff[c * nq + q];
     o[64] = 0.5 * wj * g.G[0][0]; o[128] = 0.5 * wj * g.G[0][1]; o[192] = 0.5 * wj * g.G[0][2];
     o[256] = 0.5 * wj * g.G[1][1]; o[320] = 0.5 * wj * g.G[1][2]; o[384] = 0.5 * wj * g.G[2][2];
+    if (nf == 10) {
+      o[448] = wj * (g.Ji[0][0] * kx + g.Ji[0][1] * ky + g.Ji[0][2] * kz);
+      o[512] = wj * (g.Ji[1][0] * kx + g.Ji[1][1] * ky + g.Ji[1][2] * kz);
+      o[576] = wj * (g.Ji[2][0] * kx + g.Ji[2][1] * ky + g.Ji[2][2] * kz);
+    }
   }
 }
 
@@ -295,7 +307,8 @@ done:
 cudaError_t build_sf_fields(Op* op, const double* veff_q_host, cudaStream_t stream) {
   cudaError_t err = cudaSuccess;
   const int nq1 = op->nq1;
-  const size_t elems = (size_t)op->n_cells * nq1 * 7 * 64;
+  const int nf = op->kpoint ? 10 : 7;
+  const size_t elems = (size_t)op->n_cells * nq1 * nf * 64;
   double* d_veff = nullptr;
   if (!op->sf_coef) {
     CK(cudaMalloc((void**)&op->sf_coef, elems * sizeof(double)));
@@ -304,7 +317,8 @@ cudaError_t build_sf_fields(Op* op, const double* veff_q_host, cudaStream_t stre
   CK(upload(&d_veff, veff_q_host, (size_t)op->n_cells * op->n_q, stream));
   {
     SetupTables tb{op->setup_pp, op->setup_phi, op->setup_gx, op->setup_gw};
-    k_sf_fields<<<(unsigned)op->n_cells, 256, 0, stream>>>(nq1, op->n_cells, tb, op->setup_verts, d_veff, op->sf_coef);
+    k_sf_fields<<<(unsigned)op->n_cells, 256, 0, stream>>>(nq1, nf, op->n_cells, tb, op->setup_verts, d_veff, op->kvec[0], op->kvec[1],
+                                                           op->kvec[2], op->sf_coef);
     CK(cudaGetLastError());
     CK(cudaStreamSynchronize(stream));
   }
@@ -317,36 +331,20 @@ cudaError_t rebuild_local_matrices(Op* op, const double* veff_q_host, cudaStream
   return launch_local_matrices(op, veff_q_host, stream, /*zero_tail=*/0, nullptr);
 }
 
-cudaError_t build_cell_matrices(Op* op, const HostPlan& plan, const Tables1D& tab, const chfsi_mesh& mesh,
-                                const chfsi_potential& pot, const chfsi_nonlocal* nl, cudaStream_t stream,
-                                bool* bad_jacobian) {
+// Projector rows of the cell matrices, C^c_{l,j} = sum_q w detJ chi_j(q) N_l(q) (Eq. 33), from the samples
+// chi (HOST pointer [nnz][(p+2)^3]); op->setup_* must exist.  The k-point variant calls it a second time with the
+// imaginary parts of the samples.  Synchronises the stream.
+cudaError_t build_cell_projectors(Op* op, const HostPlan& plan, const double* chi_host, cudaStream_t stream) {
   cudaError_t err = cudaSuccess;
-  const int n1 = tab.n1, nq1 = tab.nq1, nn = n1 * n1, nq = nq1 * nq1 * nq1;
-  const int64_t nc = op->n_cells;
+  const int n1 = op->n1, nq1 = op->nq1, nn = n1 * n1, nq = nq1 * nq1 * nq1;
   double* d_chi = nullptr;
   int64_t* d_row_src = nullptr; int32_t* d_row_cell = nullptr;
-  std::vector<double> pp((size_t)4 * nq1 * nn);
-  for (int idx = 0; idx < 4; ++idx)
-    for (int q = 0; q < nq1; ++q)
-      for (int a = 0; a < n1; ++a)
-        for (int a2 = 0; a2 < n1; ++a2) {
-          double f = (idx & 1) ? tab.dphi[q * n1 + a] : tab.phi[q * n1 + a];
-          double g = (idx & 2) ? tab.dphi[q * n1 + a2] : tab.phi[q * n1 + a2];
-          pp[((size_t)idx * nq1 + q) * nn + a * n1 + a2] = f * g;
-        }
   std::vector<int32_t> row_cell(plan.cell_proj_idx.size());
-  for (int64_t c = 0; c < nc; ++c)
+  for (int64_t c = 0; c < op->n_cells; ++c)
     for (int64_t r = plan.cell_proj_ptr[c]; r < plan.cell_proj_ptr[c + 1]; ++r) row_cell[r] = (int32_t)c;
-
-  CK(upload(&op->setup_pp, pp.data(), pp.size(), stream));
-  CK(upload(&op->setup_phi, tab.phi.data(), tab.phi.size(), stream));
-  CK(upload(&op->setup_gx, tab.gq_x.data(), tab.gq_x.size(), stream));
-  CK(upload(&op->setup_gw, tab.gq_w.data(), tab.gq_w.size(), stream));
-  CK(upload(&op->setup_verts, mesh.cell_vertices, (size_t)nc * 24, stream));
-  CK(launch_local_matrices(op, pot.veff_q, stream, /*zero_tail=*/1, bad_jacobian));
-  if (op->nnz_cp > 0) {
+  {
     SetupTables tb{op->setup_pp, op->setup_phi, op->setup_gx, op->setup_gw};
-    CK(upload(&d_chi, nl->chi_q, (size_t)op->nnz_cp * nq, stream));
+    CK(upload(&d_chi, chi_host, (size_t)op->nnz_cp * nq, stream));
     CK(upload(&d_row_src, plan.cell_proj_src.data(), plan.cell_proj_src.size(), stream));
     CK(upload(&d_row_cell, row_cell.data(), row_cell.size(), stream));
     size_t smem2 = ((size_t)nq + (size_t)n1 * nq1 * nq1 + (size_t)nn * nq1 + (size_t)nq1 * n1 + 24) * sizeof(double);
@@ -363,6 +361,32 @@ cudaError_t build_cell_matrices(Op* op, const HostPlan& plan, const Tables1D& ta
   }
 done:
   cudaFree(d_chi); cudaFree(d_row_src); cudaFree(d_row_cell);
+  return err;
+}
+
+cudaError_t build_cell_matrices(Op* op, const HostPlan& plan, const Tables1D& tab, const chfsi_mesh& mesh,
+                                const chfsi_potential& pot, const chfsi_nonlocal* nl, cudaStream_t stream,
+                                bool* bad_jacobian) {
+  cudaError_t err = cudaSuccess;
+  const int n1 = tab.n1, nq1 = tab.nq1, nn = n1 * n1, nq = nq1 * nq1 * nq1;
+  const int64_t nc = op->n_cells;
+  std::vector<double> pp((size_t)4 * nq1 * nn);
+  for (int idx = 0; idx < 4; ++idx)
+    for (int q = 0; q < nq1; ++q)
+      for (int a = 0; a < n1; ++a)
+        for (int a2 = 0; a2 < n1; ++a2) {
+          double f = (idx & 1) ? tab.dphi[q * n1 + a] : tab.phi[q * n1 + a];
+          double g = (idx & 2) ? tab.dphi[q * n1 + a2] : tab.phi[q * n1 + a2];
+          pp[((size_t)idx * nq1 + q) * nn + a * n1 + a2] = f * g;
+        }
+  CK(upload(&op->setup_pp, pp.data(), pp.size(), stream));
+  CK(upload(&op->setup_phi, tab.phi.data(), tab.phi.size(), stream));
+  CK(upload(&op->setup_gx, tab.gq_x.data(), tab.gq_x.size(), stream));
+  CK(upload(&op->setup_gw, tab.gq_w.data(), tab.gq_w.size(), stream));
+  CK(upload(&op->setup_verts, mesh.cell_vertices, (size_t)nc * 24, stream));
+  CK(launch_local_matrices(op, pot.veff_q, stream, /*zero_tail=*/1, bad_jacobian));
+  if (op->nnz_cp > 0) CK(build_cell_projectors(op, plan, nl->chi_q, stream));
+done:
   return err;
 }
 
