@@ -4,6 +4,7 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--assembly 0|1] [--variant V] [--impl reference]
     python bench.py --all-configs            one JSON line per BASELINE.json config (profiles/r02_all_configs.md)
     python bench.py --rr                     Rayleigh-Ritz products S, H^, Y Z on config 3's rows (Alg. 2 steps 1 and 3)
+    python bench.py --kpoint                 k-point variant (complex Hermitian H~^k) on config 3's mesh, 512 complex vectors
 
 One "step" = one pass of the whole hot path over one batch of synthetic input: the degree-m Chebyshev filter
 (cell extraction, per-cell product, non-local projectors, assembly, fused recurrence; m times) applied to
@@ -38,6 +39,8 @@ NCU_TRAFFIC_BYTES_PER_LAUNCH = {
     (3, "k_apply_dmma_p<double>"): 14.54e9,    # same file: 11.68 GB read + 2.86 GB written
     (5, "k_apply_sf<double>"): 27.24e9,        # profiles/r02_sf_kernel.md: 18.48 GB read + 8.76 GB written
     (3, "k_apply_sf<double>"): 8.82e9,         # same file: 5.97 GB read + 2.84 GB written
+    (5, "k_apply_sf_ws<double>"): 27.28e9,     # profiles/r02b_ws_kernel.md: 18.49 GB read + 8.79 GB written
+    (3, "k_apply_sf_ws<double>"): 8.83e9,      # same file: 5.97 GB read + 2.86 GB written
 }
 
 
@@ -57,6 +60,8 @@ def parse_args():
     ap.add_argument("--all-configs", action="store_true", help="one JSON line per BASELINE.json config (1..5)")
     ap.add_argument("--rr", action="store_true",
                     help="Rayleigh-Ritz products (S = Y^T Y, H^ = Y^T H~ Y, Y Z) at N = 1024 on config 3's rows")
+    ap.add_argument("--kpoint", action="store_true",
+                    help="k-point variant (chfsi_create_k) on config 3's mesh: 512 complex vectors in chunks of 128, m = 30")
     ap.add_argument("--block-width", type=int, default=0,
                     help="override the chunk width B of the config (block-width sweep, the shape of the paper's Fig. 2a); "
                          "N becomes one chunk of that width")
@@ -456,11 +461,79 @@ def run_rr(args):
     op.close()
 
 
+def run_kpoint(args):
+    """Chebyshev filter of the k-point variant (Eq. 30 k-terms PAPER.md:309-311; the paper's best CF speed-up is on its
+    k-point benchmark, Table 5) on config 3's mesh and potential: 512 complex vectors (= 1,024 real columns, the
+    same bytes as config 3) in chunks of 128, m = 30.  One JSON line; value counts COMPLEX vector-applies."""
+    import torch
+
+    from paper_2203_07820_b200 import Operator, measure_fp64_peak
+    from workloads.generate import CONFIGS, load_bounds, make_workload
+    spec = CONFIGS[3]
+    kvec = [0.05, 0.03, -0.04]
+    wl = make_workload(3, kvec=kvec)
+    a0, a, b = load_bounds(spec.bounds_key, "B")
+    b = 1.05 * b + 1.0                                  # the k-terms widen the spectrum slightly
+    op = Operator.from_workload(wl)
+    info = op.info
+    N, B, m = 512, 128, spec.m
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(4242)
+    X0 = torch.view_as_complex(torch.randn((wl.n_dofs, N, 2), dtype=torch.float64, device="cuda", generator=gen))
+    X = torch.empty_like(X0)
+    ws = op.workspace(B)
+    peaks = measure_fp64_peak()
+
+    def step():
+        X.copy_(X0)
+        op.chebyshev_filter_chunked(X, B, m, a, b, a0, workspace=ws)
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(torch.cuda.current_device())
+    op.set_profiling(True)
+    l0 = op.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler.start()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms = e0.elapsed_time(e1)
+    prof = op.get_profile()
+    launches = op.launch_count() - l0 + args.steps
+    value = N * m * args.steps / (ms * 1e-3)
+    flops_col = 2.0 * info["sf_flops_per_vector_apply"]           # a complex column = two real columns (+ 12 flop per Gauss point)
+    k_tflops = flops_col * N * m * args.steps / (prof["contraction_ms"] * 1e-3) * 1e-12
+    line = {
+        "metric": "chebyshev_filter_complex_vector_applies_per_s", "value": value, "unit": "complex vector-applies/s",
+        "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64 (complex)", "data": "synthetic",
+        "config": {"workload": f"k-point variant on config 3's mesh: {wl.n_dofs} dofs, N={N} complex vectors in chunks of B={B}, "
+                               f"m={m}, k={kvec}", "kernel": "k_apply_sf_ws<double, k-point> + k_proj_back",
+                   "l2": "inputs larger than L2"},
+        "real_equivalent_vector_applies_per_s": 2.0 * value,
+        "roofline": {"kernel": "k_apply_sf_ws<double, k-point> (+ k_proj_back)", "bound": "alu", "achieved": k_tflops,
+                     "peak": peaks["dmma_tflops"], "unit": "TFLOP/s", "frac": k_tflops / peaks["dmma_tflops"], "traffic": None,
+                     "flops_counted": "executed: 2 x the real sum-factorised count per complex column",
+                     "share_of_step": prof["contraction_ms"] / ms, "projector_ms_share": prof["projector_ms"] / ms},
+        "gpu_launches": launches, "clocks": clocks,
+    }
+    print(json.dumps(line), flush=True)
+    op.close()
+
+
 def main():
     args = parse_args()
     from workloads.generate import CONFIGS
     if args.rr:
         run_rr(args)
+        return
+    if args.kpoint:
+        run_kpoint(args)
         return
     if args.all_configs:
         for c in (1, 2, 3, 4, 5):
