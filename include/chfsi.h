@@ -224,6 +224,43 @@ int chfsi_projected_hamiltonian_mixed(chfsi_op* op, const void* Y_dev, int64_t l
 int chfsi_subspace_transform_mixed(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N, const double* Z_dev, int64_t ldz,
                                    void* Out_dev, int64_t ldo, void* cuda_stream);
 
+/* ---- Cell-partitioned operation (the paper's domain decomposition over MPI tasks / GPUs; boundary sums and
+ * FP32 boundary traffic; Alg. 4 step 3 across parts) ------------------------------------------
+ * A PART is an operator on a subset of the cells of a mesh, with its own dense numbering of the dofs those cells touch.
+ * H~ X of the whole mesh is the sum of the parts' results on the dofs they share, provided every part (i) scales with the
+ * diagonal mass of the WHOLE mesh and (ii) uses projector coefficients P summed over all parts.  The library gives the pieces;
+ * the exchange between the parts (NCCL all-reduce / send-recv) belongs to the caller (paper_2203_07820_b200/partition.py):
+ *
+ *   chfsi_mesh_mass        host only, no device: diagonal GLL mass M_g = sum_cells w_a w_b w_c detJ of `mesh`
+ *                          into mass_host[n_dofs]; a part's partial masses are then summed over the parts by the caller.
+ *   chfsi_create_part      chfsi_create with the mass of the whole mesh at the part's dofs given (dof_mass[n_dofs], HOST).
+ *   chfsi_projector_coefficients      steps 3a-3c of the path on the part's cells: P_dev[n_proj][B] (operator's storage type,
+ *                          vector index fastest) = D (C^T X) restricted to the part's cells; summing it over the parts gives P.
+ *   chfsi_apply_H_with_coefficients   chfsi_apply_H with steps 3a-3c replaced by the given P_dev[n_proj][B]: Y = the part's
+ *                          contribution to H~ X (complete on interior dofs, partial on shared ones).
+ *   chfsi_pack_rows / chfsi_unpack_rows   buf[s(i)][0..B) = X[rows[i]][0..B) and back, s(i) = slots_dev[i] (or i when slots_dev is
+ *                          NULL; the slots let every part write into one buffer laid out over all shared dofs); buf is a
+ *                          dense [.][B] array; buf_precision = the operator's precision, or 32 for the paper's FP32
+ *                          boundary payload; X is any [rows][ld] block of the operator's type; rows_dev / slots_dev are
+ *                          DEVICE int32 arrays.
+ *   chfsi_recurrence_update            T <- alpha (HX - c X) - beta T on whole blocks: one degree of the scaled recurrence
+ *                          (Eq. 37) once HX is complete on every dof.
+ * All device work is enqueued on the stream; same block conventions and error codes as above.  Not for k-point handles. */
+int chfsi_mesh_mass(const chfsi_mesh* mesh, double* mass_host);
+int chfsi_create_part(chfsi_op** out, const chfsi_mesh* mesh, const chfsi_potential* pot, const chfsi_nonlocal* nl /* nullable */,
+                      const double* dof_mass, int precision /* 64 | 32 */, int assembly /* 0 | 1 */, void* cuda_stream);
+int chfsi_projector_coefficients(chfsi_op* op, const void* X_dev, int64_t ldx, int64_t B, void* P_dev, void* workspace_dev,
+                                 void* cuda_stream);
+int chfsi_apply_H_with_coefficients(chfsi_op* op, const void* X_dev, int64_t ldx, void* Y_dev, int64_t ldy, int64_t B,
+                                    const void* P_dev, void* workspace_dev, void* cuda_stream);
+int chfsi_pack_rows(chfsi_op* op, const void* X_dev, int64_t ldx, int64_t B, const int32_t* rows_dev,
+                    const int32_t* slots_dev /* nullable */, int64_t n_rows, void* buf_dev, int buf_precision, void* cuda_stream);
+int chfsi_unpack_rows(chfsi_op* op, const void* buf_dev, int buf_precision, const int32_t* rows_dev,
+                      const int32_t* slots_dev /* nullable */, int64_t n_rows, void* X_dev, int64_t ldx, int64_t B,
+                      void* cuda_stream);
+int chfsi_recurrence_update(chfsi_op* op, const void* HX_dev, int64_t ldh, const void* X_dev, int64_t ldx, void* T_dev,
+                            int64_t ldt, int64_t B, double alpha, double beta, double c, void* cuda_stream);
+
 /* Number of kernel launches enqueued by this handle since creation (for benchmark bookkeeping). */
 int64_t chfsi_launch_count(const chfsi_op* op);
 

@@ -4,6 +4,6 @@ Everything on the path runs in the CUDA kernels behind the C ABI of `include/chf
 marshals arguments (ctypes) and uses PyTorch for device memory and streams.  There is no CPU fallback: the
 import works without a GPU (so the symbols can be checked), any compute call without one raises.
 """
-from .binding import (ChfsiError, Operator, lib, load_library, measure_fp64_peak, EXPORTED_SYMBOLS)  # noqa: F401
+from .binding import (ChfsiError, Operator, lib, load_library, measure_fp64_peak, mesh_mass, EXPORTED_SYMBOLS)  # noqa: F401
 
-__all__ = ["ChfsiError", "Operator", "lib", "load_library", "measure_fp64_peak", "EXPORTED_SYMBOLS"]
+__all__ = ["ChfsiError", "Operator", "lib", "load_library", "measure_fp64_peak", "mesh_mass", "EXPORTED_SYMBOLS"]

@@ -19,7 +19,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libchfsi.so")
 
 EXPORTED_SYMBOLS = [
-    "chfsi_create", "chfsi_create_k", "chfsi_destroy", "chfsi_update_potential", "chfsi_get_info", "chfsi_workspace_bytes", "chfsi_mass_diag",
+    "chfsi_create", "chfsi_create_k", "chfsi_create_part", "chfsi_mesh_mass", "chfsi_projector_coefficients",
+    "chfsi_apply_H_with_coefficients", "chfsi_pack_rows", "chfsi_unpack_rows", "chfsi_recurrence_update", "chfsi_destroy", "chfsi_update_potential", "chfsi_get_info", "chfsi_workspace_bytes", "chfsi_mass_diag",
     "chfsi_apply_H", "chfsi_overlap_matrix", "chfsi_projected_hamiltonian", "chfsi_subspace_transform",
     "chfsi_cholesky_inverse", "chfsi_overlap_matrix_mixed", "chfsi_projected_hamiltonian_mixed", "chfsi_subspace_transform_mixed", "chfsi_chebyshev_filter", "chfsi_chebyshev_filter_chunked", "chfsi_chebyshev_filter_host",
     "chfsi_launch_count", "chfsi_set_kernel_variant", "chfsi_set_profiling", "chfsi_get_profile",
@@ -87,6 +88,21 @@ def load_library(build_if_missing: bool = True):
     lib_.chfsi_create_k.argtypes = [C.POINTER(vp), C.POINTER(_Mesh), C.POINTER(_Potential), C.POINTER(_Nonlocal),
                                     C.POINTER(_KPoint), C.c_int, vp]
     lib_.chfsi_create_k.restype = C.c_int
+    lib_.chfsi_create_part.argtypes = [C.POINTER(vp), C.POINTER(_Mesh), C.POINTER(_Potential), C.POINTER(_Nonlocal), vp,
+                                       C.c_int, C.c_int, vp]
+    lib_.chfsi_create_part.restype = C.c_int
+    lib_.chfsi_mesh_mass.argtypes = [C.POINTER(_Mesh), vp]
+    lib_.chfsi_mesh_mass.restype = C.c_int
+    lib_.chfsi_projector_coefficients.argtypes = [vp, vp, i64, i64, vp, vp, vp]
+    lib_.chfsi_projector_coefficients.restype = C.c_int
+    lib_.chfsi_apply_H_with_coefficients.argtypes = [vp, vp, i64, vp, i64, i64, vp, vp, vp]
+    lib_.chfsi_apply_H_with_coefficients.restype = C.c_int
+    lib_.chfsi_pack_rows.argtypes = [vp, vp, i64, i64, vp, vp, i64, vp, C.c_int, vp]
+    lib_.chfsi_pack_rows.restype = C.c_int
+    lib_.chfsi_unpack_rows.argtypes = [vp, vp, C.c_int, vp, vp, i64, vp, i64, i64, vp]
+    lib_.chfsi_unpack_rows.restype = C.c_int
+    lib_.chfsi_recurrence_update.argtypes = [vp, vp, i64, vp, i64, vp, i64, i64, dbl, dbl, dbl, vp]
+    lib_.chfsi_recurrence_update.restype = C.c_int
     lib_.chfsi_destroy.argtypes = [vp]
     lib_.chfsi_destroy.restype = C.c_int
     lib_.chfsi_update_potential.argtypes = [vp, C.POINTER(_Potential), vp]
@@ -158,13 +174,27 @@ def measure_fp64_peak(stream=None) -> dict:
     return {"dmma_tflops": a.value, "dfma_tflops": b.value}
 
 
+def mesh_mass(p, cell_dofs, cell_vertices, n_dofs) -> np.ndarray:
+    """chfsi_mesh_mass: diagonal GLL mass of a mesh (or of a part of one: the partial sums over its cells).  Host only."""
+    cell_dofs = np.ascontiguousarray(cell_dofs, dtype=np.int32)
+    cell_vertices = np.ascontiguousarray(cell_vertices, dtype=np.float64)
+    mesh = _Mesh(int(p), int(cell_dofs.shape[0]), int(n_dofs), _np_ptr(cell_dofs), _np_ptr(cell_vertices))
+    M = np.empty(int(n_dofs), dtype=np.float64)
+    rc = load_library().chfsi_mesh_mass(C.byref(mesh), M.ctypes.data)
+    if rc != 0:
+        raise ChfsiError(rc, (load_library().chfsi_last_error(None) or b"").decode())
+    return M
+
+
 class Operator:
     """Owns one `chfsi_op` handle.  Inputs are host NumPy arrays (copied by the library during the call)."""
 
     def __init__(self, p, cell_dofs, cell_vertices, n_dofs, veff_q, n_proj=0, D=None, proj_cell_ptr=None,
-                 proj_cell_idx=None, chi_q=None, precision=64, assembly=0, stream=None, kvec=None, chi_q_im=None):
+                 proj_cell_idx=None, chi_q=None, precision=64, assembly=0, stream=None, kvec=None, chi_q_im=None,
+                 dof_mass=None):
         """kvec (3 floats, bohr^-1) selects the k-point variant (chfsi_create_k): blocks are then complex128 tensors and
-        chi_q / chi_q_im hold the real / imaginary parts of the Bloch-phased projector samples."""
+        chi_q / chi_q_im hold the real / imaginary parts of the Bloch-phased projector samples.  dof_mass ([n_dofs], the
+        diagonal mass of the whole mesh at these dofs) makes the handle a PART of a larger mesh (chfsi_create_part)."""
         self._h = None
         self.kpoint = kvec is not None
         L = load_library()
@@ -196,6 +226,12 @@ class Operator:
                 kp.chi_q_im = chi_im.ctypes.data
             rc = L.chfsi_create_k(C.byref(h), C.byref(mesh), C.byref(pot), nlp, C.byref(kp), int(assembly),
                                   _stream_ptr(stream))
+        elif dof_mass is not None:
+            dm = np.ascontiguousarray(dof_mass, dtype=np.float64)
+            if dm.shape != (int(n_dofs),):
+                raise ValueError("dof_mass must have n_dofs entries")
+            rc = L.chfsi_create_part(C.byref(h), C.byref(mesh), C.byref(pot), nlp, dm.ctypes.data, int(precision),
+                                     int(assembly), _stream_ptr(stream))
         else:
             rc = L.chfsi_create(C.byref(h), C.byref(mesh), C.byref(pot), nlp, int(precision), int(assembly),
                                 _stream_ptr(stream))
@@ -272,6 +308,74 @@ class Operator:
         self._check(load_library().chfsi_apply_H(self._h, xp, ldx, yp, ldy, B, C.c_void_p(ws.data_ptr()),
                                                  _stream_ptr(stream)))
         return Y
+
+    # -- cell-partitioned operation (include/chfsi.h "Cell-partitioned operation") --------------------------------
+    def projector_coefficients(self, X, P=None, workspace=None, stream=None):
+        """P[n_proj, B] = D (C^T X) over this operator's cells (steps 3a-3c); a device tensor of the operator's dtype."""
+        import torch
+        xp, ldx, B = self._block(X, "X")
+        n_proj = int(self.info["n_proj"])
+        if P is None:
+            P = torch.zeros((n_proj, B), dtype=self.dtype, device="cuda")
+        if tuple(P.shape) != (n_proj, B) or not P.is_contiguous() or P.dtype != self.dtype:
+            raise ValueError("P must be a contiguous [n_proj, B] tensor of the operator's dtype")
+        ws = workspace if workspace is not None else self.workspace(B)
+        self._check(load_library().chfsi_projector_coefficients(self._h, xp, ldx, B, C.c_void_p(P.data_ptr()),
+                                                                C.c_void_p(ws.data_ptr()), _stream_ptr(stream)))
+        return P
+
+    def apply_H_with_coefficients(self, X, P, Y=None, workspace=None, stream=None):
+        """This operator's contribution to H~ X with the projector coefficients P[n_proj, B] given."""
+        import torch
+        xp, ldx, B = self._block(X, "X")
+        if Y is None:
+            Y = torch.empty((self.n_dofs, B), dtype=self.dtype, device="cuda")
+        yp, ldy, By = self._block(Y, "Y")
+        n_proj = int(self.info["n_proj"])
+        if By != B or tuple(P.shape) != (n_proj, B) or not P.is_contiguous() or P.dtype != self.dtype:
+            raise ValueError("need Y [n_dofs, B] and a contiguous P [n_proj, B] of the operator's dtype")
+        ws = workspace if workspace is not None else self.workspace(B)
+        self._check(load_library().chfsi_apply_H_with_coefficients(self._h, xp, ldx, yp, ldy, B, C.c_void_p(P.data_ptr()),
+                                                                   C.c_void_p(ws.data_ptr()), _stream_ptr(stream)))
+        return Y
+
+    def _rows_block(self, X, name):
+        import torch
+        if not (isinstance(X, torch.Tensor) and X.is_cuda and X.dim() == 2 and X.dtype == self.dtype and X.stride(1) == 1):
+            raise TypeError(f"{name}: expected a 2-D CUDA tensor of the operator's dtype, vector index fastest")
+        return C.c_void_p(X.data_ptr()), int(X.stride(0)), int(X.shape[1])
+
+    def pack_rows(self, X, rows, buf, slots=None, stream=None):
+        """buf[s(i)] = X[rows[i]], s(i) = slots[i] or i (rows, slots: int32 device tensors; buf: contiguous [., B] of X's dtype
+        or float32)."""
+        import torch
+        xp, ldx, B = self._rows_block(X, "X")
+        bp = 32 if buf.dtype == torch.float32 else 64
+        sp = C.c_void_p(slots.data_ptr()) if slots is not None else None
+        self._check(load_library().chfsi_pack_rows(self._h, xp, ldx, B, C.c_void_p(rows.data_ptr()), sp, int(rows.numel()),
+                                                   C.c_void_p(buf.data_ptr()), bp, _stream_ptr(stream)))
+        return buf
+
+    def unpack_rows(self, buf, rows, X, slots=None, stream=None):
+        """X[rows[i]] = buf[s(i)]."""
+        import torch
+        xp, ldx, B = self._rows_block(X, "X")
+        bp = 32 if buf.dtype == torch.float32 else 64
+        sp = C.c_void_p(slots.data_ptr()) if slots is not None else None
+        self._check(load_library().chfsi_unpack_rows(self._h, C.c_void_p(buf.data_ptr()), bp, C.c_void_p(rows.data_ptr()), sp,
+                                                     int(rows.numel()), xp, ldx, B, _stream_ptr(stream)))
+        return X
+
+    def recurrence_update(self, HX, X, T, alpha, beta, c, stream=None):
+        """T <- alpha (HX - c X) - beta T on whole blocks."""
+        hp, ldh, B = self._block(HX, "HX")
+        xp, ldx, Bx = self._block(X, "X")
+        tp, ldt, Bt = self._block(T, "T")
+        if not (B == Bx == Bt):
+            raise ValueError("HX, X and T must have the same number of columns")
+        self._check(load_library().chfsi_recurrence_update(self._h, hp, ldh, xp, ldx, tp, ldt, B, float(alpha), float(beta),
+                                                           float(c), _stream_ptr(stream)))
+        return T
 
     def overlap_matrix(self, Y, stream=None):
         """S = Y^T Y (Algorithm 2 step 1a); returns a [N, N] FP64 device tensor."""

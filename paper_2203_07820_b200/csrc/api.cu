@@ -197,7 +197,7 @@ namespace {
 inline int64_t col_width(const chfsi_op* op) { return op->kpoint ? 2 : 1; }
 
 int create_impl(chfsi_op** out, const chfsi_mesh* mesh, const chfsi_potential* pot_in, const chfsi_nonlocal* nl,
-                const chfsi_kpoint* kp, int precision, int assembly, void* cuda_stream) {
+                const chfsi_kpoint* kp, const double* dof_mass, int precision, int assembly, void* cuda_stream) {
   if (!out) return fail(nullptr, CHFSI_ERR_BAD_ARGUMENT, "out == NULL");
   *out = nullptr;
   if (!mesh || !pot_in || !mesh->cell_dofs || !mesh->cell_vertices || !pot_in->veff_q)
@@ -259,6 +259,14 @@ int create_impl(chfsi_op** out, const chfsi_mesh* mesh, const chfsi_potential* p
   HostPlan plan;
   std::string msg = analyse_mesh(*mesh, has_nl ? nl : nullptr, tab, op->lda, op->n_parts, &plan);
   if (!msg.empty()) { free_op(op); return fail(nullptr, CHFSI_ERR_BAD_MESH, msg); }
+  if (dof_mass) {   // a part of a larger mesh: the diagonal mass of the WHOLE mesh at these dofs (chfsi_create_part)
+    for (int64_t g = 0; g < mesh->n_dofs; ++g)
+      if (!(dof_mass[g] > 0.0) || !std::isfinite(dof_mass[g])) {
+        free_op(op);
+        return fail(nullptr, CHFSI_ERR_BAD_ARGUMENT, "dof_mass must be positive and finite");
+      }
+    plan.mass.assign(dof_mass, dof_mass + mesh->n_dofs);
+  }
 
   op->n_colors = plan.n_colors; op->color_ptr = plan.color_ptr;
   op->nnz_cp = (int64_t)plan.cell_proj_idx.size();
@@ -341,13 +349,36 @@ extern "C" {
 
 int chfsi_create(chfsi_op** out, const chfsi_mesh* mesh, const chfsi_potential* pot, const chfsi_nonlocal* nl,
                  int precision, int assembly, void* cuda_stream) {
-  return create_impl(out, mesh, pot, nl, nullptr, precision, assembly, cuda_stream);
+  return create_impl(out, mesh, pot, nl, nullptr, nullptr, precision, assembly, cuda_stream);
 }
 
 int chfsi_create_k(chfsi_op** out, const chfsi_mesh* mesh, const chfsi_potential* pot, const chfsi_nonlocal* nl,
                    const chfsi_kpoint* kpoint, int assembly, void* cuda_stream) {
   if (!kpoint) return fail(nullptr, CHFSI_ERR_BAD_ARGUMENT, "kpoint == NULL");
-  return create_impl(out, mesh, pot, nl, kpoint, 64, assembly, cuda_stream);
+  return create_impl(out, mesh, pot, nl, kpoint, nullptr, 64, assembly, cuda_stream);
+}
+
+int chfsi_create_part(chfsi_op** out, const chfsi_mesh* mesh, const chfsi_potential* pot, const chfsi_nonlocal* nl,
+                      const double* dof_mass, int precision, int assembly, void* cuda_stream) {
+  if (!dof_mass) return fail(nullptr, CHFSI_ERR_BAD_ARGUMENT, "dof_mass == NULL");
+  return create_impl(out, mesh, pot, nl, nullptr, dof_mass, precision, assembly, cuda_stream);
+}
+
+int chfsi_mesh_mass(const chfsi_mesh* mesh, double* mass_host) {
+  if (!mesh || !mass_host || !mesh->cell_dofs || !mesh->cell_vertices) return CHFSI_ERR_BAD_ARGUMENT;
+  if (mesh->p < 1 || mesh->p > 8) return CHFSI_ERR_UNSUPPORTED;
+  if (mesh->n_cells < 1 || mesh->n_dofs < 1) return CHFSI_ERR_BAD_ARGUMENT;
+  try {
+    Tables1D tab;
+    build_tables(mesh->p, &tab);
+    std::vector<double> m;
+    const std::string msg = mesh_mass(*mesh, tab, &m);
+    if (!msg.empty()) { g_create_error = msg; return CHFSI_ERR_BAD_MESH; }
+    std::copy(m.begin(), m.end(), mass_host);
+    return CHFSI_OK;
+  } catch (...) {
+    return CHFSI_ERR_OUT_OF_MEMORY;
+  }
 }
 
 int chfsi_destroy(chfsi_op* op) {
@@ -450,6 +481,100 @@ int chfsi_apply_H(chfsi_op* op, const void* X_dev, int64_t ldx, void* Y_dev, int
   if (ce != cudaSuccess) return cuda_fail(op, ce, "apply_H launch");
   return CHFSI_OK;
   API_CATCH(op)
+}
+
+namespace {
+// chfsi_apply_H in phases (ApplyArgs::phase): the projector coefficients of this operator's cells, or H~X with given ones
+int apply_phase(chfsi_op* op, const void* X_dev, int64_t ldx, void* Y_dev, int64_t ldy, int64_t B, void* P_dev, int phase,
+                void* workspace_dev, void* cuda_stream) {
+  int rc = check_block_args(op, X_dev, ldx, B, workspace_dev);
+  if (rc) return rc;
+  if (op->kpoint) return fail(op, CHFSI_ERR_UNSUPPORTED, "phased application of a k-point handle");
+  if (op->n_proj > 0 && !P_dev) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "NULL coefficient block");
+  if (phase == 2) {
+    if (!Y_dev) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "NULL output block");
+    if (ldy < B) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "ldy < B");
+    if (X_dev == Y_dev) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "X and Y must not overlap");
+  }
+  API_TRY
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  const WsLayout w = ws_layout(op, B);
+  char* base = reinterpret_cast<char*>(workspace_dev);
+  ApplyArgs g;
+  g.X = X_dev; g.ldx = ldx; g.T = phase == 2 ? Y_dev : const_cast<void*>(X_dev); g.ldt = phase == 2 ? ldy : ldx; g.B = B;
+  g.alpha = 1.0; g.beta = 0.0; g.cshift = 0.0; g.phase = phase;
+  g.P = base + w.p_off; g.Pc = base + w.pc_off;
+  g.sync = reinterpret_cast<unsigned long long*>(base + w.sync_off); g.epoch = 1;
+  const size_t p_bytes = (size_t)op->n_proj * B * w.elt;
+  cudaError_t ce = order_enter(op, st);
+  if (ce == cudaSuccess) ce = cudaMemsetAsync(g.sync, 0, w.sync_bytes, st);
+  if (ce == cudaSuccess && phase == 2) {   // rows 0 .. n_proj-1 from the caller, the all-zero row n_proj behind them
+    if (p_bytes) ce = cudaMemcpyAsync(g.P, P_dev, p_bytes, cudaMemcpyDeviceToDevice, st);
+    if (ce == cudaSuccess) ce = cudaMemsetAsync(reinterpret_cast<char*>(g.P) + p_bytes, 0, (size_t)B * w.elt, st);
+  }
+  if (ce != cudaSuccess) return cuda_fail(op, ce, "phased apply_H setup");
+  op->launches++;
+  ce = launch_apply(op, g, st);
+  if (ce == cudaSuccess && phase == 1 && p_bytes) ce = cudaMemcpyAsync(P_dev, g.P, p_bytes, cudaMemcpyDeviceToDevice, st);
+  if (ce == cudaSuccess) ce = order_leave(op, st);
+  if (ce != cudaSuccess) return cuda_fail(op, ce, "phased apply_H launch");
+  return CHFSI_OK;
+  API_CATCH(op)
+}
+}  // namespace
+
+int chfsi_projector_coefficients(chfsi_op* op, const void* X_dev, int64_t ldx, int64_t B, void* P_dev, void* workspace_dev,
+                                 void* cuda_stream) {
+  return apply_phase(op, X_dev, ldx, nullptr, 0, B, P_dev, 1, workspace_dev, cuda_stream);
+}
+
+int chfsi_apply_H_with_coefficients(chfsi_op* op, const void* X_dev, int64_t ldx, void* Y_dev, int64_t ldy, int64_t B,
+                                    const void* P_dev, void* workspace_dev, void* cuda_stream) {
+  return apply_phase(op, X_dev, ldx, Y_dev, ldy, B, const_cast<void*>(P_dev), 2, workspace_dev, cuda_stream);
+}
+
+int chfsi_recurrence_update(chfsi_op* op, const void* HX_dev, int64_t ldh, const void* X_dev, int64_t ldx, void* T_dev,
+                            int64_t ldt, int64_t B, double alpha, double beta, double c, void* cuda_stream) {
+  if (!op) return CHFSI_ERR_BAD_ARGUMENT;
+  if (!HX_dev || !X_dev || !T_dev) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "NULL block");
+  if (B < 1 || ldh < B || ldx < B || ldt < B) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "need B >= 1 and ld >= B");
+  if (op->kpoint) return fail(op, CHFSI_ERR_UNSUPPORTED, "recurrence_update on a k-point handle");
+  API_TRY
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  cudaError_t ce = order_enter(op, st);
+  if (ce == cudaSuccess) ce = launch_recurrence(op, HX_dev, ldh, X_dev, ldx, T_dev, ldt, B, alpha, beta, c, st);
+  if (ce == cudaSuccess) ce = order_leave(op, st);
+  return ce == cudaSuccess ? CHFSI_OK : cuda_fail(op, ce, "recurrence_update");
+  API_CATCH(op)
+}
+
+namespace {
+int pack_rows(chfsi_op* op, const void* X_dev, int64_t ldx, int64_t B, const int32_t* rows_dev, const int32_t* slots_dev,
+              int64_t n_rows, void* buf_dev, int buf_precision, bool unpack, void* cuda_stream) {
+  if (!op) return CHFSI_ERR_BAD_ARGUMENT;
+  if (n_rows < 0 || B < 1 || ldx < B) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "need n_rows >= 0, B >= 1, ld >= B");
+  if (n_rows > 0 && (!X_dev || !rows_dev || !buf_dev)) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "NULL pointer");
+  if (buf_precision != op->precision && buf_precision != 32)
+    return fail(op, CHFSI_ERR_BAD_ARGUMENT, "buf_precision must be the operator's precision or 32");
+  if (op->kpoint) return fail(op, CHFSI_ERR_UNSUPPORTED, "pack / unpack on a k-point handle");
+  API_TRY
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  cudaError_t ce = order_enter(op, st);
+  if (ce == cudaSuccess) ce = launch_pack_rows(op, X_dev, ldx, B, rows_dev, slots_dev, n_rows, buf_dev, buf_precision, unpack, st);
+  if (ce == cudaSuccess) ce = order_leave(op, st);
+  return ce == cudaSuccess ? CHFSI_OK : cuda_fail(op, ce, unpack ? "unpack_rows" : "pack_rows");
+  API_CATCH(op)
+}
+}  // namespace
+
+int chfsi_pack_rows(chfsi_op* op, const void* X_dev, int64_t ldx, int64_t B, const int32_t* rows_dev, const int32_t* slots_dev,
+                    int64_t n_rows, void* buf_dev, int buf_precision, void* cuda_stream) {
+  return pack_rows(op, X_dev, ldx, B, rows_dev, slots_dev, n_rows, buf_dev, buf_precision, false, cuda_stream);
+}
+
+int chfsi_unpack_rows(chfsi_op* op, const void* buf_dev, int buf_precision, const int32_t* rows_dev, const int32_t* slots_dev,
+                      int64_t n_rows, void* X_dev, int64_t ldx, int64_t B, void* cuda_stream) {
+  return pack_rows(op, X_dev, ldx, B, rows_dev, slots_dev, n_rows, const_cast<void*>(buf_dev), buf_precision, true, cuda_stream);
 }
 
 int chfsi_chebyshev_filter(chfsi_op* op, void* X_dev, int64_t ldx, int64_t B, int32_t m, double a, double b,

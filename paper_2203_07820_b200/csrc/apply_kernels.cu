@@ -833,7 +833,8 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
   T* Tg = reinterpret_cast<T*>(g.T);
   const T* mat = reinterpret_cast<const T*>(op->mat);
   cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
-  if (op->profiling) {
+  const bool profiling = op->profiling && g.phase == 0;
+  if (profiling) {
     if (op->prof_used + 3 > op->prof_events.size()) {
       for (int i = 0; i < 3; ++i) {
         cudaEvent_t e;
@@ -874,7 +875,7 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
   const int64_t launches_before = op->launches;
   // steps 3a-3c
   double* Pc = reinterpret_cast<double*>(g.Pc);
-  if (op->n_pseg > 0) {
+  if (op->n_pseg > 0 && g.phase != 2) {
     dim3 g1((unsigned)op->n_pseg, (unsigned)((B + kPRCols - 1) / kPRCols));
     CUtensorMap tmXp;
     if (op->variant != 1 && make_row_gather_map(&tmXp, g.X, op->n_dofs, B, g.ldx, (int)sizeof(T), kPRCols)) {
@@ -891,11 +892,12 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
     }
     op->launches++;
   }
-  {
+  if (g.phase != 2) {
     dim3 g2((unsigned)(op->n_proj + 1), (unsigned)((B + 127) / 128));
     k_proj_reduce<T><<<g2, 128, 0, st>>>(Pc, op->grp_seg_ptr, op->proj_grp, op->proj_slot, op->D, op->n_proj, P, B);
     op->launches++;
   }
+  if (g.phase == 1) return cudaGetLastError();
   ApplyDev<T> a;
   a.mat = mat; a.mat_off = op->mat_off; a.idx_off = op->idx_off; a.ktot = op->ktot; a.gidx = op->gidx;
   a.m_cell = op->m_cell; a.mpad = op->mpad; a.lda = op->lda; a.mw = op->mw; a.n_parts = op->n_parts;
@@ -931,7 +933,7 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
     k_prefill<T><<<148 * 8, 256, 0, st>>>(Tg, g.ldt, op->n_dofs, B, a.beta);
     op->launches++;
   }
-  if (op->profiling) {
+  if (profiling) {
     cudaEventRecord(ev[1], st);
     op->prof_proj_launches += op->launches - launches_before;
   }
@@ -1069,7 +1071,7 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
     }
     op->launches++;
   }
-  if (op->profiling) {
+  if (profiling) {
     cudaEventRecord(ev[2], st);
     op->prof_main_launches += op->launches - launches_mid;
   }

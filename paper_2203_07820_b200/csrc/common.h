@@ -81,6 +81,8 @@ struct HostPlan {
 // Returns "" on success, else an error message (bad mesh).
 std::string analyse_mesh(const chfsi_mesh& mesh, const chfsi_nonlocal* nl, const Tables1D& tab, int lda, int n_parts,
                          HostPlan* plan);
+// Diagonal GLL mass of a mesh on the host; returns an error text or "".
+std::string mesh_mass(const chfsi_mesh& mesh, const Tables1D& tab, std::vector<double>* mass);
 
 // ---- device operator ----------------------------------------------------------------------------------------
 struct Op {
@@ -206,7 +208,17 @@ struct ApplyArgs {
   // (every contribution is a red.add).  Only the warp-specialised sum-factorised kernel takes it: ask
   // apply_accumulates() first.  The filter loop then runs the recurrence in scaled blocks (api.cu filter_block).
   bool accumulate = false;
+  // phase: 0 = the whole application; 1 = steps 3a-3c only (the D-scaled projector coefficients P of this operator's cells
+  // are left in the workspace rows `P`); 2 = everything but steps 3a-3c (`P` is given).  Phases 1 and 2 let a caller
+  // that holds only a part of the mesh sum P over the parts in between (Alg. 4 step 3).
+  int phase = 0;
 };
+// Helpers of the cell-partitioned filter (part_kernels.cu): rows of a block to / from a packed buffer of the block's own
+// type (buf_precision == op->precision) or FP32, and one degree of the three-term recurrence on whole blocks.
+cudaError_t launch_pack_rows(Op* op, const void* X, int64_t ldx, int64_t B, const int32_t* rows, const int32_t* slots,
+                             int64_t n_rows, void* buf, int buf_precision, bool unpack, cudaStream_t stream);
+cudaError_t launch_recurrence(Op* op, const void* HX, int64_t ldh, const void* X, int64_t ldx, void* T, int64_t ldt, int64_t B,
+                              double alpha, double beta, double c, cudaStream_t stream);
 // True when launch_apply would run these arguments (X, ldx, T, ldt, P, B, sync set) with accumulate = true.
 bool apply_accumulates(const Op* op, const ApplyArgs& a);
 // dst[g][0..B) = factor * src[g][0..B) for all dofs g (element type per op->precision; dst may equal src).

@@ -120,6 +120,27 @@ double trilinear_detJ(const double* verts, double x, double y, double z) {
 }
 }  // namespace
 
+// M_g = sum over the cells of dof g of w_a w_b w_c detJ at the node: GLL quadrature makes the mass diagonal.
+// Dofs and Jacobians are assumed valid as far as analyse_mesh checks them first; a non-positive Jacobian is reported.
+std::string mesh_mass(const chfsi_mesh& mesh, const Tables1D& tab, std::vector<double>* mass) {
+  const int n1 = tab.n1, mc = n1 * n1 * n1;
+  mass->assign((size_t)mesh.n_dofs, 0.0);
+  for (int64_t c = 0; c < mesh.n_cells; ++c) {
+    const int32_t* cd = mesh.cell_dofs + c * mc;
+    const double* vt = mesh.cell_vertices + c * 24;
+    for (int k = 0; k < n1; ++k)
+      for (int j = 0; j < n1; ++j)
+        for (int i = 0; i < n1; ++i) {
+          const int32_t g = cd[i + n1 * (j + n1 * k)];
+          if (g < 0 || g >= mesh.n_dofs) return "cell " + std::to_string(c) + ": dof index out of range";
+          double dj = trilinear_detJ(vt, tab.gll_x[i], tab.gll_x[j], tab.gll_x[k]);
+          if (!(dj > 0.0)) return "cell " + std::to_string(c) + ": non-positive Jacobian";
+          (*mass)[g] += tab.gll_w[i] * tab.gll_w[j] * tab.gll_w[k] * dj;
+        }
+  }
+  return "";
+}
+
 std::string analyse_mesh(const chfsi_mesh& mesh, const chfsi_nonlocal* nl, const Tables1D& tab, int lda, int n_parts,
                          HostPlan* plan) {
   const int n1 = tab.n1, mc = n1 * n1 * n1;
@@ -142,17 +163,9 @@ std::string analyse_mesh(const chfsi_mesh& mesh, const chfsi_nonlocal* nl, const
     if (deg[g] == 0) return "dof " + std::to_string(g) + " belongs to no cell";
 
   // ---- diagonal GLL mass, deterministic cell order ------------------------------------------
-  plan->mass.assign(nd, 0.0);
-  for (int64_t c = 0; c < nc; ++c) {
-    const int32_t* cd = mesh.cell_dofs + c * mc;
-    const double* vt = mesh.cell_vertices + c * 24;
-    for (int k = 0; k < n1; ++k)
-      for (int j = 0; j < n1; ++j)
-        for (int i = 0; i < n1; ++i) {
-          double dj = trilinear_detJ(vt, tab.gll_x[i], tab.gll_x[j], tab.gll_x[k]);
-          if (!(dj > 0.0)) return "cell " + std::to_string(c) + ": non-positive Jacobian";
-          plan->mass[cd[i + n1 * (j + n1 * k)]] += tab.gll_w[i] * tab.gll_w[j] * tab.gll_w[k] * dj;
-        }
+  {
+    const std::string mm = mesh_mass(mesh, tab, &plan->mass);
+    if (!mm.empty()) return mm;
   }
 
   // ---- greedy colouring of the cell graph (cells adjacent when they share a dof) ---------------------------

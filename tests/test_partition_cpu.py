@@ -1,0 +1,108 @@
+"""Host logic of the cell-partitioned (multi-GPU) form (paper_2203_07820_b200/partition.py),
+`-m "not gpu"`: the partition bookkeeping, the mass of the whole mesh assembled from the parts over a world-size-2 gloo
+group, and the algebra of the boundary sum (parts' contributions on shared dofs add up to H~ X of the whole mesh) with the
+ORACLE standing in for the part operators."""
+import multiprocessing as mp
+import os
+
+import numpy as np
+import pytest
+
+from workloads.generate import make_workload
+
+
+def small_workload(nonlocal_=True, n=4, p=2, jitter=0.1):
+    return make_workload(None, n=n, p=p, L=2.0 * n, mesh_jitter=jitter, atoms_per_side=2, n_gaussians=0, nonlocal_=nonlocal_,
+                         smooth_field=0.05, seed_base=55, r_cut=2.2)
+
+
+@pytest.mark.parametrize("world", [1, 2, 3, 4])
+def test_partition_covers_the_mesh_and_maps_back(world):
+    from paper_2203_07820_b200.partition import CellPartition
+    wl = small_workload()
+    cp = CellPartition(wl, world)
+    cd = np.asarray(wl.cell_dofs)
+    counts = np.bincount(cp.owner, minlength=world)
+    assert counts.sum() == cd.shape[0] and counts.min() >= cd.shape[0] // world           # balanced, every cell once
+    touched = np.zeros(wl.n_dofs, dtype=int)
+    n_q = wl.veff_q.shape[1]
+    proj_cells_seen = 0
+    for r in range(world):
+        lp = cp.local(r)
+        assert np.array_equal(lp.dofs[lp.cell_dofs], cd[lp.cells])                          # local ids map back
+        assert np.array_equal(lp.cell_vertices.reshape(-1, 24), np.asarray(wl.cell_vertices).reshape(-1, 24)[lp.cells])
+        touched[lp.dofs] += 1
+        assert np.array_equal(lp.dofs[lp.shared_rows], cp.shared_dofs[lp.shared_slots])     # rows <-> slots of shared dofs
+        # projectors: the local CSR is the global one restricted to this rank's cells, samples and couplings carried along
+        for jl, j in enumerate(lp.proj_ids):
+            assert lp.D[jl] == wl.D[j]
+            glob = {int(wl.proj_cell_idx[k]): k for k in range(int(wl.proj_cell_ptr[j]), int(wl.proj_cell_ptr[j + 1]))}
+            for kl in range(int(lp.proj_cell_ptr[jl]), int(lp.proj_cell_ptr[jl + 1])):
+                gc = int(lp.cells[lp.proj_cell_idx[kl]])
+                assert gc in glob and np.array_equal(lp.chi_q[kl], wl.chi_q[glob[gc]])
+                proj_cells_seen += 1
+        assert lp.chi_q.shape == (len(lp.proj_cell_idx), n_q)
+    assert touched.min() >= 1
+    assert np.array_equal(np.nonzero(touched >= 2)[0], cp.shared_dofs)
+    assert proj_cells_seen == len(wl.proj_cell_idx)                                         # every (projector, cell) pair once
+    if world == 1:
+        assert len(cp.shared_dofs) == 0
+
+
+def test_mesh_mass_of_the_library_equals_the_oracle_and_the_volume():
+    from oracle import chfsi_oracle as orc
+    from paper_2203_07820_b200 import mesh_mass
+    wl = small_workload(p=3)
+    M = mesh_mass(wl.p, wl.cell_dofs, wl.cell_vertices, wl.n_dofs)
+    assert np.allclose(M, orc.mass_diagonal(wl.p, wl.cell_dofs, wl.cell_vertices, wl.n_dofs), rtol=1e-13, atol=0)
+    assert abs(M.sum() - 8.0 ** 3) <= 1e-10 * 8.0 ** 3                                      # sum M = volume of the periodic box
+
+
+def _rank_main(rank, world, port, q):
+    """One gloo rank: mass of the whole mesh at its dofs, and its (oracle) contribution to H~ X with the boundary sum."""
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    import torch
+    import torch.distributed as dist
+    from oracle import chfsi_oracle as orc
+    from paper_2203_07820_b200.partition import CellPartition, TorchComm, global_mass_at
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        wl = small_workload(nonlocal_=False)
+        comm = TorchComm()
+        cp = CellPartition(wl, world)
+        lp = cp.local(rank)
+        mass = global_mass_at(lp, cp, wl.p, comm)
+        # the part as an oracle operator with the mass of the whole mesh; its apply_H is the part's contribution
+        oop = orc.build_operator(wl.p, lp.cell_dofs, lp.cell_vertices, len(lp.dofs), lp.veff_q)
+        oop.M = mass
+        X = np.random.default_rng(3).standard_normal((wl.n_dofs, 5))
+        Y = orc.apply_H(oop, X[lp.dofs])
+        buf = torch.zeros((len(cp.shared_dofs), 5), dtype=torch.float64)
+        buf[torch.from_numpy(lp.shared_slots.astype(np.int64))] = torch.from_numpy(Y[lp.shared_rows])
+        comm.all_reduce(buf)
+        Y[lp.shared_rows] = buf.numpy()[lp.shared_slots]
+        q.put((rank, lp.dofs, mass, Y))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_world_size_2_gloo_mass_and_boundary_sum_reproduce_the_whole_mesh():
+    from oracle import chfsi_oracle as orc
+    from paper_2203_07820_b200 import mesh_mass
+    world, port = 2, 29500 + os.getpid() % 2000
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_rank_main, args=(r, world, port, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = [q.get(timeout=240) for _ in range(world)]
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    wl = small_workload(nonlocal_=False)
+    Mg = mesh_mass(wl.p, wl.cell_dofs, wl.cell_vertices, wl.n_dofs)
+    X = np.random.default_rng(3).standard_normal((wl.n_dofs, 5))
+    Yg = orc.apply_H(orc.operator_from_workload(wl), X)
+    for rank, dofs, mass, Y in res:
+        assert np.allclose(mass, Mg[dofs], rtol=1e-14, atol=0)
+        assert np.max(np.abs(Y - Yg[dofs])) <= 1e-12 * np.max(np.abs(Yg))
