@@ -60,6 +60,10 @@ def parse_args():
     ap.add_argument("--all-configs", action="store_true", help="one JSON line per BASELINE.json config (1..5)")
     ap.add_argument("--rr", action="store_true",
                     help="Rayleigh-Ritz products (S = Y^T Y, H^ = Y^T H~ Y, Y Z) at N = 1024 on config 3's rows")
+    ap.add_argument("--partition", action="store_true",
+                    help="cell-partitioned filter (paper's domain decomposition, PAPER.md:649): the mesh of --config (default 3) is "
+                         "split over the --gpus ranks, boundary rows summed by NCCL all-reduce once per H~ application (strong scaling)")
+    ap.add_argument("--boundary-fp32", action="store_true", help="with --partition: FP32 boundary payload (PAPER.md:536)")
     ap.add_argument("--kpoint", action="store_true",
                     help="k-point variant (chfsi_create_k) on config 3's mesh: 512 complex vectors in chunks of 128, m = 30")
     ap.add_argument("--block-width", type=int, default=0,
@@ -526,9 +530,78 @@ def run_kpoint(args):
     op.close()
 
 
+def run_partition(args, spec):
+    """Strong scaling over cells: every rank holds a slab of the mesh (partition.py) and the rows of its dofs for ALL N vectors;
+    per H~ application one all-reduce of the projector coefficients and one of the shared rows.  N = 1 measures the same
+    unfused sequence (phased apply + recurrence kernel) without any exchange."""
+    import torch
+    import torch.distributed as dist
+
+    from paper_2203_07820_b200.partition import PartitionedOperator, SingleComm, TorchComm
+    from paper_2203_07820_b200.sharding import aggregate_max
+    from workloads.generate import load_bounds, make_workload
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    if world > 1 and not dist.is_initialized():
+        dist.init_process_group("nccl", device_id=torch.device("cuda", torch.cuda.current_device()))
+    wl = make_workload(spec.config)
+    a0, a, b = load_bounds(spec.bounds_key, "B")
+    part = PartitionedOperator(wl, comm=TorchComm() if world > 1 else SingleComm(), precision=spec.precision,
+                               boundary_fp32=args.boundary_fp32)
+    N, B, m = spec.N, spec.B, spec.m
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(99)                                      # same seed on every rank; only the timing matters here
+    X0 = torch.randn((part.n_local_dofs, N), dtype=part.dtype, device="cuda", generator=gen)
+    X = torch.empty_like(X0)
+    ws = part.op.workspace(min(B, N))
+
+    def step():
+        X.copy_(X0)
+        part.chebyshev_filter_chunked(X, B, m, a, b, a0, workspace=ws)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(torch.cuda.current_device())
+    l0 = part.op.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler.start()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    clocks = sampler.stop()
+    ms = aggregate_max(e0.elapsed_time(e1), world) / args.steps
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": N * m / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+            "dtype": "f64" if spec.precision == 64 else "f64 arithmetic on f32-stored vectors", "data": "synthetic",
+            "config": {"workload": workload_name(spec), "parallelism": f"cell partition x{world} (slabs), all-reduce of the "
+                       f"projector coefficients and of the shared rows per H~ application, payload "
+                       f"{'FP32' if args.boundary_fp32 else 'block precision'}",
+                       "shared_dofs": int(part.n_shared), "local_dofs_rank0": int(part.n_local_dofs),
+                       "l2": "inputs larger than L2"},
+            "gpu_launches": part.op.launch_count() - l0 + args.steps, "clocks": clocks}), flush=True)
+    part.close()
+    if dist.is_initialized():
+        dist.destroy_process_group()
+
+
 def main():
     args = parse_args()
     from workloads.generate import CONFIGS
+    if args.partition:
+        run_partition(args, CONFIGS[args.config if args.config != DEFAULT_CONFIG else 3])
+        return
     if args.rr:
         run_rr(args)
         return
