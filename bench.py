@@ -64,6 +64,10 @@ def parse_args():
                     help="cell-partitioned filter (paper's domain decomposition, PAPER.md:649): the mesh of --config (default 3) is "
                          "split over the --gpus ranks, boundary rows summed by NCCL all-reduce once per H~ application (strong scaling)")
     ap.add_argument("--boundary-fp32", action="store_true", help="with --partition: FP32 boundary payload (PAPER.md:536)")
+    ap.add_argument("--soak", type=float, default=0.0,
+                    help="soak run of SECONDS per case on config 2's operator: degree-9 filters repeated at several block widths, "
+                         "FP64 and FP32 storage, every result compared bit for bit with the first one (flag-ordered assembly, "
+                         "buffer hand-over of the persistent kernels); prints one JSON line")
     ap.add_argument("--kpoint", action="store_true",
                     help="k-point variant (chfsi_create_k) on config 3's mesh: 512 complex vectors in chunks of 128, m = 30")
     ap.add_argument("--block-width", type=int, default=0,
@@ -596,9 +600,46 @@ def run_partition(args, spec):
         dist.destroy_process_group()
 
 
+def run_soak(args):
+    import torch
+
+    from paper_2203_07820_b200 import Operator
+    from workloads.generate import load_bounds, make_workload
+    wl = make_workload(2)
+    a0, a, b = load_bounds("2", "B")
+    cases, total_filters, total_launches = [], 0, 0
+    for precision in (64, 32):
+        op = Operator.from_workload(wl, precision=precision)
+        for B in (256, 200, 72, 32, 16):
+            gen = torch.Generator(device="cuda")
+            gen.manual_seed(7 + B)
+            X0 = torch.randn((wl.n_dofs, B), dtype=op.dtype, device="cuda", generator=gen)
+            ws = op.workspace(B)
+            ref, n, l0, t0 = None, 0, op.launch_count(), time.perf_counter()
+            while time.perf_counter() - t0 < args.soak:
+                for _ in range(20):
+                    X = X0.clone()
+                    op.chebyshev_filter(X, 9, a, b, a0, workspace=ws)
+                    if ref is None:
+                        ref = X
+                    elif not torch.equal(X, ref):
+                        raise RuntimeError(f"soak: result differs from the first run (precision {precision}, B = {B}, filter {n})")
+                    n += 1
+                torch.cuda.synchronize()
+            cases.append({"precision": precision, "B": B, "filters": n})
+            total_filters += n
+            total_launches += op.launch_count() - l0
+        op.close()
+    print(json.dumps({"soak": "bit-identical throughout, no hang", "seconds_per_case": args.soak, "filters": total_filters,
+                      "kernel_launches": total_launches, "cases": cases}), flush=True)
+
+
 def main():
     args = parse_args()
     from workloads.generate import CONFIGS
+    if args.soak > 0:
+        run_soak(args)
+        return
     if args.partition:
         run_partition(args, CONFIGS[args.config if args.config != DEFAULT_CONFIG else 3])
         return
