@@ -58,7 +58,8 @@ struct WsSmem {
   static constexpr int off_scr = off_small + 3 * small_bytes;               // [8 warps][4][kSfScrSlab] doubles
   static constexpr int off_bar = off_scr + kWsComputeWarps * 4 * kSfScrSlab * 8;   // full[2], done[2], free[2], small[3], crow2
   static constexpr int off_ticket = off_bar + 10 * 8;                        // [4] long long
-  static constexpr int bytes = off_ticket + 4 * 8;
+  static constexpr int off_frag = (off_ticket + 4 * 8 + 15) / 16 * 16;      // [16][32] doubles: per-lane fragments of the 1-D matrices
+  static constexpr int bytes = off_frag + 16 * 32 * 8;
   static_assert(idx_stride * 4 % 16 == 0, "M^-1/2 follows the index list 16-byte aligned");
 };
 
@@ -106,18 +107,33 @@ __global__ void __launch_bounds__(kWsThreads, 1) k_apply_sf_ws(ApplyDev<S> a, Sf
     double* scrB = scrA + 2 * kSfScrSlab;
     const int so_w = g * kSfScrPitch + 2 * t;
     const int so_r0 = t * kSfScrPitch + g, so_r1 = (4 + t) * kSfScrPitch + g;
-    double fPhiA[2], fPhiB[2], fDA[2], fDB[2], fDtA[2], fDtB[2], fPhiTA[2], fPhiTB[2];
+    // constant fragments of the 1-D matrices (k-step s: contraction index 4s + t for "matrix x data", 2t + s for "data x
+    // matrix"), one 4 KB table in shared memory for all warps: sixteen doubles per lane that would otherwise be spilled
+    // and come back from L2 at the start of every column pair
+    double* frag_s = reinterpret_cast<double*>(smem_dyn + L::off_frag);
+    if (warp == 0) {
 #pragma unroll
-    for (int s = 0; s < 2; ++s) {
-      fPhiA[s] = c_sf_phi[P][g * 8 + 4 * s + t];
-      fPhiB[s] = c_sf_phi[P][g * 8 + 2 * t + s];
-      fDA[s] = c_sf_dhat[P][g * 8 + 4 * s + t];
-      fDB[s] = c_sf_dhat[P][g * 8 + 2 * t + s];
-      fDtA[s] = c_sf_dhat[P][(4 * s + t) * 8 + g];
-      fDtB[s] = c_sf_dhat[P][(2 * t + s) * 8 + g];
-      fPhiTA[s] = c_sf_phi[P][(4 * s + t) * 8 + g];
-      fPhiTB[s] = c_sf_phi[P][(2 * t + s) * 8 + g];
+      for (int s = 0; s < 2; ++s) {
+        frag_s[(0 + s) * 32 + lane] = c_sf_phi[P][g * 8 + 4 * s + t];           // PhiA:  Phi[qa = g][a = 4s + t]
+        frag_s[(2 + s) * 32 + lane] = c_sf_phi[P][g * 8 + 2 * t + s];           // PhiB:  Phi[qb = g][b = 2t + s]
+        frag_s[(4 + s) * 32 + lane] = c_sf_dhat[P][g * 8 + 4 * s + t];          // DA:    Dh[qa' = g][qa = 4s + t]
+        frag_s[(6 + s) * 32 + lane] = c_sf_dhat[P][g * 8 + 2 * t + s];          // DB:    Dh[qb' = g][qb = 2t + s]
+        frag_s[(8 + s) * 32 + lane] = c_sf_dhat[P][(4 * s + t) * 8 + g];        // DtA:   Dh[qa = 4s + t][qa'' = g]
+        frag_s[(10 + s) * 32 + lane] = c_sf_dhat[P][(2 * t + s) * 8 + g];       // DtB:   Dh[qb = 2t + s][qb'' = g]
+        frag_s[(12 + s) * 32 + lane] = c_sf_phi[P][(4 * s + t) * 8 + g];        // PhiTA: Phi[qa = 4s + t][a = g]
+        frag_s[(14 + s) * 32 + lane] = c_sf_phi[P][(2 * t + s) * 8 + g];        // PhiTB: Phi[qb = 2t + s][b = g]
+      }
     }
+    asm volatile("bar.sync 2, %0;" ::"n"(32 * kWsComputeWarps) : "memory");
+    const double* fr = frag_s + lane;
+#define fPhiA(s) fr[(0 + (s)) * 32]
+#define fPhiB(s) fr[(2 + (s)) * 32]
+#define fDA(s) fr[(4 + (s)) * 32]
+#define fDB(s) fr[(6 + (s)) * 32]
+#define fDtA(s) fr[(8 + (s)) * 32]
+#define fDtB(s) fr[(10 + (s)) * 32]
+#define fPhiTA(s) fr[(12 + (s)) * 32]
+#define fPhiTB(s) fr[(14 + (s)) * 32]
     const double cshift = sf.cshift;
     int set = 0;                                                      // j % 3
     for (int iter = 0;; ++iter) {
@@ -159,7 +175,7 @@ __global__ void __launch_bounds__(kWsThreads, 1) k_apply_sf_ws(ApplyDev<S> a, Sf
 #pragma unroll
                 for (int u = 0; u < 2; ++u) {
                   if (s == 0) d[c][u][0] = d[c][u][1] = 0.0;
-                  dmma884(d[c][u][0], d[c][u][1], fPhiA[s], bv[c][u]);
+                  dmma884(d[c][u][0], d[c][u][1], fPhiA(s), bv[c][u]);
                 }
             }
 #pragma unroll
@@ -171,7 +187,7 @@ __global__ void __launch_bounds__(kWsThreads, 1) k_apply_sf_ws(ApplyDev<S> a, Sf
 #pragma unroll
               for (int c = 0; c < n1; ++c)
 #pragma unroll
-                for (int u = 0; u < 2; ++u) dmma884(T2[c][u][0], T2[c][u][1], d[c][u][s], fPhiB[s]);
+                for (int u = 0; u < 2; ++u) dmma884(T2[c][u][0], T2[c][u][1], d[c][u][s], fPhiB(s));
           }
 #pragma unroll
           for (int q = 0; q < nq1; ++q)
@@ -212,8 +228,8 @@ __global__ void __launch_bounds__(kWsThreads, 1) k_apply_sf_ws(ApplyDev<S> a, Sf
           if (q > 0) {
 #pragma unroll
             for (int u = 0; u < 2; ++u) {
-              dmma884(w[q - 1][u][0], w[q - 1][u][1], fDtA[0], c0[u]);
-              dmma884(w[q - 1][u][0], w[q - 1][u][1], fDtA[1], c1[u]);
+              dmma884(w[q - 1][u][0], w[q - 1][u][1], fDtA(0), c0[u]);
+              dmma884(w[q - 1][u][0], w[q - 1][u][1], fDtA(1), c1[u]);
             }
           }
           if (q < nq1) {
@@ -221,13 +237,13 @@ __global__ void __launch_bounds__(kWsThreads, 1) k_apply_sf_ws(ApplyDev<S> a, Sf
 #pragma unroll
             for (int u = 0; u < 2; ++u) {
               dx[u][0] = dx[u][1] = dy[u][0] = dy[u][1] = dz[u][0] = dz[u][1] = 0.0;
-              dmma884(dx[u][0], dx[u][1], fDA[0], b0[u]);
-              dmma884(dy[u][0], dy[u][1], uh[q][u][0], fDB[0]);
+              dmma884(dx[u][0], dx[u][1], fDA(0), b0[u]);
+              dmma884(dy[u][0], dy[u][1], uh[q][u][0], fDB(0));
             }
 #pragma unroll
             for (int u = 0; u < 2; ++u) {
-              dmma884(dx[u][0], dx[u][1], fDA[1], b1[u]);
-              dmma884(dy[u][0], dy[u][1], uh[q][u][1], fDB[1]);
+              dmma884(dx[u][0], dx[u][1], fDA(1), b1[u]);
+              dmma884(dy[u][0], dy[u][1], uh[q][u][1], fDB(1));
             }
             {
               double dzo[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
@@ -268,8 +284,8 @@ __global__ void __launch_bounds__(kWsThreads, 1) k_apply_sf_ws(ApplyDev<S> a, Sf
               gz[u][1] = fma(Gxz.y, dx[u][1], fma(Gyz.y, dy[u][1], Gzz.y * dz[u][1]));
               w[q][u][0] = fma(W0.x, uh[q][u][0], w[q][u][0]);
               w[q][u][1] = fma(W0.y, uh[q][u][1], w[q][u][1]);
-              dmma884(w[q][u][0], w[q][u][1], gy0, fDtB[0]);
-              dmma884(w[q][u][0], w[q][u][1], gy1, fDtB[1]);
+              dmma884(w[q][u][0], w[q][u][1], gy0, fDtB(0));
+              dmma884(w[q][u][0], w[q][u][1], gy1, fDtB(1));
               *reinterpret_cast<double2*>(scrB + u * kSfScrSlab + so_w) = make_double2(gx0, gx1);
             }
 #pragma unroll
@@ -307,8 +323,8 @@ __global__ void __launch_bounds__(kWsThreads, 1) k_apply_sf_ws(ApplyDev<S> a, Sf
 #pragma unroll
           for (int u = 0; u < 2; ++u) {
             double y0 = 0.0, y1 = 0.0;
-            dmma884(y0, y1, z[c][u][0], fPhiTB[0]);
-            dmma884(y0, y1, z[c][u][1], fPhiTB[1]);
+            dmma884(y0, y1, z[c][u][0], fPhiTB(0));
+            dmma884(y0, y1, z[c][u][1], fPhiTB(1));
             *reinterpret_cast<double2*>(scr + u * kSfScrSlab + so_w) = make_double2(y0, y1);
           }
           __syncwarp();
@@ -317,8 +333,8 @@ __global__ void __launch_bounds__(kWsThreads, 1) k_apply_sf_ws(ApplyDev<S> a, Sf
           for (int u = 0; u < 2; ++u) {
             const double b0 = scr[u * kSfScrSlab + so_r0], b1 = scr[u * kSfScrSlab + so_r1];
             y[u][0] = y[u][1] = 0.0;
-            dmma884(y[u][0], y[u][1], fPhiTA[0], b0);
-            dmma884(y[u][0], y[u][1], fPhiTA[1], b1);
+            dmma884(y[u][0], y[u][1], fPhiTA(0), b0);
+            dmma884(y[u][0], y[u][1], fPhiTA(1), b1);
           }
           // lane (g, t): nodes (a = g, b = 2t + e, c); the result overwrites the two columns:  s_l y_l - c x_l [first]
 #pragma unroll
@@ -342,6 +358,14 @@ __global__ void __launch_bounds__(kWsThreads, 1) k_apply_sf_ws(ApplyDev<S> a, Sf
       if (lane == 0) mbar_arrive(bar_done + b);
       set = (set == 2) ? 0 : set + 1;
     }
+#undef fPhiA
+#undef fPhiB
+#undef fDA
+#undef fDB
+#undef fDtA
+#undef fDtB
+#undef fPhiTA
+#undef fPhiTB
   } else {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(ws_regs_helper<S>()));
     if (warp == kWsComputeWarps) {
