@@ -952,7 +952,7 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
     pd.ticket_base = (unsigned long long)(g.epoch - 1) * (unsigned long long)(n_tiles + grid);
     SfDev sf;
     sf.coef = op->sf_coef; sf.sloc = op->sf_sloc; sf.crows = op->crows; sf.cell_proj_ptr = op->cell_proj_ptr;
-    sf.cshift = g.cshift;
+    sf.cshift = g.cshift; sf.zero = 0;
     if (use_ws) {
       const unsigned gws = (unsigned)std::min<int64_t>(n_tiles, (int64_t)op->n_sm);
       pd.ticket_base = (unsigned long long)(g.epoch - 1) * (unsigned long long)(n_tiles + gws);

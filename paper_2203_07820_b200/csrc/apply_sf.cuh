@@ -51,6 +51,7 @@ struct SfDev {
   const double* __restrict__ crows;          // [nnz_cell_proj][mpad]  s_l C^c_{l,j} (rows padded with zeros)
   const int64_t* __restrict__ cell_proj_ptr; // [n_cells + 1]
   double cshift;                             // spectral shift c of the running filter (0 for apply_H)
+  int zero;                                  // 0 (k_apply_sf_ws: keeps the 1-D table addresses out of ptxas's hoisting)
 };
 
 template <int P, typename S>

@@ -135,6 +135,9 @@ __global__ void __launch_bounds__(kWsThreads, 1) k_apply_sf_ws(ApplyDev<S> a, Sf
 #define fPhiTA(s) fr[(12 + (s)) * 32]
 #define fPhiTB(s) fr[(14 + (s)) * 32]
     const double cshift = sf.cshift;
+    // a run-time zero in the index of the 1-D tables: with compile-time addresses ptxas hoists a few dozen table entries
+    // into registers for the whole kernel and spills them; this way every use is a uniform constant load next to its DFMAs
+    const int zo = sf.zero;
     int set = 0;                                                      // j % 3
     for (int iter = 0;; ++iter) {
       const int b = iter & 1;
@@ -197,7 +200,7 @@ __global__ void __launch_bounds__(kWsThreads, 1) k_apply_sf_ws(ApplyDev<S> a, Sf
           for (int c = 0; c < n1; ++c)
 #pragma unroll
             for (int q = 0; q < nq1; ++q) {
-              const double ph = c_sf_phi[P][q * 8 + c];
+              const double ph = c_sf_phi[P][q * 8 + c + zo];
 #pragma unroll
               for (int u = 0; u < 2; ++u) {
                 uh[q][u][0] = fma(ph, T2[c][u][0], uh[q][u][0]);
@@ -249,7 +252,7 @@ __global__ void __launch_bounds__(kWsThreads, 1) k_apply_sf_ws(ApplyDev<S> a, Sf
               double dzo[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
 #pragma unroll
               for (int r = 0; r < nq1; ++r) {
-                const double dh = c_sf_dhat[P][q * 8 + r];
+                const double dh = c_sf_dhat[P][q * 8 + r + zo];
 #pragma unroll
                 for (int u = 0; u < 2; ++u) {
                   if (r & 1) { dzo[u][0] = fma(dh, uh[r][u][0], dzo[u][0]); dzo[u][1] = fma(dh, uh[r][u][1], dzo[u][1]); }
@@ -290,7 +293,7 @@ __global__ void __launch_bounds__(kWsThreads, 1) k_apply_sf_ws(ApplyDev<S> a, Sf
             }
 #pragma unroll
             for (int r = 0; r < nq1; ++r) {
-              const double dh = c_sf_dhat[P][q * 8 + r];
+              const double dh = c_sf_dhat[P][q * 8 + r + zo];
 #pragma unroll
               for (int u = 0; u < 2; ++u) {
                 w[r][u][0] = fma(dh, gz[u][0], w[r][u][0]);
@@ -310,7 +313,7 @@ __global__ void __launch_bounds__(kWsThreads, 1) k_apply_sf_ws(ApplyDev<S> a, Sf
         for (int q = 0; q < nq1; ++q)
 #pragma unroll
           for (int c = 0; c < n1; ++c) {
-            const double ph = c_sf_phi[P][q * 8 + c];
+            const double ph = c_sf_phi[P][q * 8 + c + zo];
 #pragma unroll
             for (int u = 0; u < 2; ++u) {
               z[c][u][0] = fma(ph, w[q][u][0], z[c][u][0]);
