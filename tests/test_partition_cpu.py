@@ -106,3 +106,37 @@ def test_world_size_2_gloo_mass_and_boundary_sum_reproduce_the_whole_mesh():
     for rank, dofs, mass, Y in res:
         assert np.allclose(mass, Mg[dofs], rtol=1e-14, atol=0)
         assert np.max(np.abs(Y - Yg[dofs])) <= 1e-12 * np.max(np.abs(Yg))
+
+
+def test_part_entry_points_report_argument_errors_without_a_device():
+    import ctypes as C
+    from paper_2203_07820_b200 import load_library
+    from paper_2203_07820_b200.binding import _KPoint, _Mesh, _Potential
+    lib = load_library()
+    M = np.zeros(8)
+    assert lib.chfsi_mesh_mass(None, M.ctypes.data) == -1
+    cd = np.arange(8, dtype=np.int32).reshape(1, 8)
+    cv = np.zeros((1, 8, 3))                                                 # degenerate cell: non-positive Jacobian
+    mesh = _Mesh(1, 1, 8, cd.ctypes.data, cv.ctypes.data)
+    assert lib.chfsi_mesh_mass(C.byref(mesh), M.ctypes.data) == -2
+    assert b"Jacobian" in lib.chfsi_last_error(None)
+    mesh9 = _Mesh(9, 1, 8, cd.ctypes.data, cv.ctypes.data)
+    assert lib.chfsi_mesh_mass(C.byref(mesh9), M.ctypes.data) == -5
+    h = C.c_void_p()
+    vq = np.zeros((1, 27))
+    pot = _Potential(vq.ctypes.data)
+    assert lib.chfsi_create_part(C.byref(h), C.byref(mesh), C.byref(pot), None, None, 64, 0, None) == -1     # dof_mass == NULL
+    assert lib.chfsi_create_k(C.byref(h), C.byref(mesh), C.byref(pot), None, None, 0, None) == -1           # kpoint == NULL
+    kp = _KPoint()
+    kp.k[0], kp.k[1], kp.k[2] = float("nan"), 0.0, 0.0
+    assert lib.chfsi_create_k(C.byref(h), C.byref(mesh), C.byref(pot), None, C.byref(kp), 0, None) == -1    # non-finite k
+    mesh7 = _Mesh(7, 1, 512, cd.ctypes.data, cv.ctypes.data)
+    kp.k[0] = 0.1
+    assert lib.chfsi_create_k(C.byref(h), C.byref(mesh7), C.byref(pot), None, C.byref(kp), 0, None) == -5   # p = 7
+    assert h.value is None
+    for fn, args in ((lib.chfsi_projector_coefficients, (None, None, 0, 0, None, None, None)),
+                     (lib.chfsi_apply_H_with_coefficients, (None, None, 0, None, 0, 0, None, None, None)),
+                     (lib.chfsi_pack_rows, (None, None, 0, 0, None, None, 0, None, 64, None)),
+                     (lib.chfsi_unpack_rows, (None, None, 64, None, None, 0, None, 0, 0, None)),
+                     (lib.chfsi_recurrence_update, (None, None, 0, None, 0, None, 0, 0, 1.0, 0.0, 0.0, None))):
+        assert fn(*args) == -1
