@@ -433,6 +433,23 @@ def run_rr(args):
     ms_zm = timed(lambda: op.subspace_transform_mixed(Y, Z, Out=Out))
     Sd = op.overlap_matrix(Y)
     ms_ch = timed(lambda: op.cholesky_inverse(Sd))
+    # DHM step of an SCF iteration (chfsi_update_potential, Alg. 1 step 4): host wall clock incl. the H2D copy of the samples
+    import numpy as _np
+    veff_new = _np.ascontiguousarray(wl.veff_q * 0.99)
+
+    def timed_host(fn, n=5):
+        fn()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(n):
+            fn()
+        torch.cuda.synchronize()
+        return (time.perf_counter() - t0) / n * 1e3
+
+    ms_dhm_sf = timed_host(lambda: op.update_potential(veff_new))
+    op.set_kernel_variant(4)
+    ms_dhm_dense = timed_host(lambda: (op.update_potential(veff_new), op.apply_H(Y[:, :32])))
+    op.set_kernel_variant(args.variant)
     launches = op.launch_count() - l0
     clocks = sampler.stop()
     gemm = 2.0 * wl.n_dofs * N * N                            # flops of one tall product
@@ -452,6 +469,9 @@ def run_rr(args):
         "transform_mixed": {"kernel": "k_xz_tf32 (3xTF32 off-diagonal + FP64 diagonal)", "ms": ms_zm,
                             "tflops": gemm / ms_zm * 1e-9, "speedup_vs_fp64": ms_z / ms_zm},
         "cholesky_inverse": {"kernel": "k_chol_* / k_trinv_row (N = 1024)", "ms": ms_ch},
+        "update_potential": {"kernel": "k_sf_fields (default: quadrature-point fields only; 17 MB of samples H2D)", "ms": ms_dhm_sf},
+        "update_potential_dense": {"kernel": "k_sf_fields + k_cell_matrix (lazy rebuild of the 3.9 GB of dense cell matrices, "
+                                             "variant 4) + one 32-column apply", "ms": ms_dhm_dense},
     }
     total_ms = ms_s + ms_h + ms_z
     line = {

@@ -139,6 +139,9 @@ int chfsi_create_k(chfsi_op** out, const chfsi_mesh* mesh, const chfsi_potential
  *   H^e_jk = 1/2 K^e_jk + sum_q w_q detJ_q V_eff(q) N_j(q) N_k(q)     (Eq. 30 terms 1-2; Eq. 40,
  *   PAPER.md:462-464), Loewdin-scaled (Eq. 34),
  * which is the DHM step of every SCF iteration (Algorithm 1 step 4: V_eff changes with the density).
+ * Where the sum-factorised kernel is the operator's default (p <= 6) its operator data are the quadrature-point fields
+ * w detJ V_eff(q): the call uploads the samples (kept on the device) and rebuilds those fields in one small kernel; the dense
+ * cell matrices are brought up to date from the device copy only when a dense kernel variant is used afterwards.
  * pot->veff_q is a HOST pointer [n_cells][(p+2)^3] (x fastest), copied during the call; projector rows, mesh
  * analysis, colouring and all buffers are reused.  The work is enqueued on cuda_stream and the call returns after
  * synchronising it (the host array may be released).  Must not overlap an apply / filter running on the same

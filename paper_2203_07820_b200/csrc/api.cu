@@ -51,7 +51,7 @@ void free_op(chfsi_op* op) {
   cudaFree(op->proj_ptr); cudaFree(op->proj_pcrow); cudaFree(op->seg_ptr); cudaFree(op->grow_dof); cudaFree(op->pcoef);
   cudaFree(op->grp_seg_ptr); cudaFree(op->proj_grp); cudaFree(op->proj_slot);
   cudaFree(op->rr_scratch); cudaFree(op->rr32[0]); cudaFree(op->rr32[1]); cudaFree(op->sf_coef); cudaFree(op->sf_sloc); cudaFree(op->crows);
-  cudaFree(op->pcoef_im); cudaFree(op->seg_slot_proj); cudaFree(op->back_segs);
+  cudaFree(op->pcoef_im); cudaFree(op->seg_slot_proj); cudaFree(op->back_segs); cudaFree(op->veff_dev);
   for (int i = 0; i < 2; ++i) {
     cudaFree(op->host_stage[i]);
     if (op->host_done[i]) cudaEventDestroy(op->host_done[i]);
@@ -401,17 +401,26 @@ int chfsi_update_potential(chfsi_op* op, const chfsi_potential* pot, void* cuda_
     veff_q = veff_k.data();
   }
   cudaError_t ce = order_enter(op, st);
-  if (ce == cudaSuccess && !op->kpoint) ce = rebuild_local_matrices(op, veff_q, st);   // (k handles have no dense path)
-  if (ce != cudaSuccess) return cuda_fail(op, ce, "update_potential (cell matrices)");
+  if (ce != cudaSuccess) return cuda_fail(op, ce, "update_potential");
   if (op->sf_ok) {
-    ce = build_sf_fields(op, veff_q, st);
+    // the default kernel is sum-factorised: its operator data are the quadrature-point fields, rebuilt in one small kernel
+    // from the samples; the dense cell matrices (other kernel variants) follow lazily from the device copy of the samples
+    const size_t bytes = (size_t)op->n_cells * op->n_q * sizeof(double);
+    if (!op->veff_dev) ce = cudaMalloc((void**)&op->veff_dev, bytes);
+    if (ce == cudaSuccess) ce = cudaMemcpyAsync(op->veff_dev, veff_q, bytes, cudaMemcpyHostToDevice, st);
+    if (ce == cudaSuccess) ce = build_sf_fields_dev(op, op->veff_dev, st);
+    if (ce == cudaSuccess) ce = cudaStreamSynchronize(st);      // veff_q (caller's / veff_k) may go away after the call
     if (ce != cudaSuccess) return cuda_fail(op, ce, "update_potential (quadrature-point fields)");
-    op->launches++;
+    op->dense_stale = !op->kpoint;
+    op->launches += 1;
+  } else {
+    ce = rebuild_local_matrices(op, veff_q, st);
+    if (ce != cudaSuccess) return cuda_fail(op, ce, "update_potential (cell matrices)");
+    ce = capture_diagonal(op, st);      // new unshifted diagonals; the spectral shift of the last filter is gone
+    if (ce == cudaSuccess) ce = cudaStreamSynchronize(st);
+    if (ce != cudaSuccess) return cuda_fail(op, ce, "update_potential (diagonal)");
+    op->launches += 2;
   }
-  ce = capture_diagonal(op, st);      // new unshifted diagonals; the spectral shift of the last filter is gone
-  if (ce == cudaSuccess) ce = cudaStreamSynchronize(st);
-  if (ce != cudaSuccess) return cuda_fail(op, ce, "update_potential (diagonal)");
-  op->launches += 2;
   op->order_valid = false;             // the stream was synchronised: nothing of this handle is in flight
   return CHFSI_OK;
   API_CATCH(op)

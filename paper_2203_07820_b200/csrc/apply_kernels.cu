@@ -862,6 +862,10 @@ cudaError_t launch_apply_t(Op* op, const ApplyArgs& g, cudaStream_t st) {
                       make_row_gather_map(&tmPs, g.P, op->n_proj + 1, B, B, (int)sizeof(T), sf_tile_cols<T>(), false);
   if (g.accumulate && !use_ws) return cudaErrorNotSupported;   // the caller asks apply_accumulates() first
   if (op->kpoint && !(use_ws && sizeof(T) == 8)) return cudaErrorNotSupported;   // the k-point variant has this one kernel
+  if (!use_sf && op->dense_stale) {             // a dense kernel after chfsi_update_potential refreshed only the fields
+    const cudaError_t re = refresh_dense_matrices(op, st);
+    if (re != cudaSuccess) return re;
+  }
   if (!use_sf && g.cshift != op->cur_shift) {   // once per filter call: move the spectral shift onto the matrix diagonals
     const int64_t n = op->n_cells * op->m_cell;
     k_set_diag_shift<T><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(reinterpret_cast<T*>(op->mat), op->mat_off, op->idx_off,

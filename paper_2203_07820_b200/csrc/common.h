@@ -132,6 +132,11 @@ struct Op {
   // G = 1/2 w detJ J^-1 J^-T in the kernel's lane order [n_cells][nq1][7][32][2], M^-1/2 per (cell, node)
   // [n_cells][mpad], and the projector columns s_l C^c_{l,j} as compact FP64 rows [nnz_cp][m_cell]
   bool sf_ok = false;
+  // chfsi_update_potential on an operator whose default kernel is sum-factorised only refreshes the quadrature-point fields
+  // (veff_dev keeps the samples on the device); the dense cell matrices are rebuilt from veff_dev the first time a dense
+  // kernel variant is asked for afterwards
+  double* veff_dev = nullptr;            // [n_cells][n_q], set by the first chfsi_update_potential
+  bool dense_stale = false;
   // k-point variant (chfsi_create_k): vector blocks are complex (FP64 pairs re, im = two adjacent real columns), the
   // fields carry w detJ J^-1 k, the projector coefficients are complex (pcoef = real parts, pcoef_im = imaginary parts) and
   // the back-projection C (D P) runs as its own dof-centric kernel (k_proj_back), one launch per colour of the projector groups
@@ -186,9 +191,13 @@ cudaError_t build_cell_matrices(Op* op, const HostPlan& plan, const Tables1D& ta
 // Recomputes the Hamiltonian rows (rows 0..M_cell-1) of every cell matrix for a new V_eff (HOST pointer
 // [n_cells][(p+2)^3]); projector rows, layout and colouring are untouched.  Synchronises the stream.
 cudaError_t rebuild_local_matrices(Op* op, const double* veff_q_host, cudaStream_t stream);
+// The same from op->veff_dev, followed by capture_diagonal: brings stale dense matrices up to date (op->dense_stale).
+cudaError_t refresh_dense_matrices(Op* op, cudaStream_t stream);
 // Quadrature-point fields of the sum-factorised variant (op->sf_coef, allocated on first use) from V_eff at the Gauss
 // points (HOST pointer) and the cell geometry; op->setup_* must exist.  Synchronises the stream.
 cudaError_t build_sf_fields(Op* op, const double* veff_q_host, cudaStream_t stream);
+// The same from samples already on the device; enqueues only (no synchronisation).
+cudaError_t build_sf_fields_dev(Op* op, const double* veff_q_dev, cudaStream_t stream);
 // Projector rows of the cell matrices from projector samples at the Gauss points (HOST pointer); see setup_kernels.cu.
 cudaError_t build_cell_projectors(Op* op, const HostPlan& plan, const double* chi_host, cudaStream_t stream);
 

@@ -268,14 +268,16 @@ cudaError_t upload(U** dst, const U* src, size_t n, cudaStream_t st) {
 
 namespace {
 // Hamiltonian rows of all cell matrices from V_eff at the Gauss points (host pointer); op->setup_* must exist.
-cudaError_t launch_local_matrices(Op* op, const double* veff_host, cudaStream_t stream, int zero_tail, bool* bad_jacobian) {
+cudaError_t launch_local_matrices(Op* op, const double* veff_host, cudaStream_t stream, int zero_tail, bool* bad_jacobian,
+                                  const double* veff_dev = nullptr) {
   cudaError_t err = cudaSuccess;
   const int n1 = op->n1, nq1 = op->nq1, nn = n1 * n1, nq = nq1 * nq1 * nq1, mc = n1 * nn;
   const int64_t nc = op->n_cells;
-  double *d_veff = nullptr, *d_scratch = nullptr;
+  double *d_veff = nullptr, *d_scratch = nullptr, *d_veff_own = nullptr;
   int* d_bad = nullptr;
   int h_bad = 0;
-  CK(upload(&d_veff, veff_host, (size_t)nc * nq, stream));
+  if (veff_dev) d_veff = const_cast<double*>(veff_dev);
+  else { CK(upload(&d_veff_own, veff_host, (size_t)nc * nq, stream)); d_veff = d_veff_own; }
   CK(upload(&d_bad, &h_bad, 1, stream));
   {
     SetupTables tb{op->setup_pp, op->setup_phi, op->setup_gx, op->setup_gw};
@@ -299,32 +301,49 @@ cudaError_t launch_local_matrices(Op* op, const double* veff_host, cudaStream_t 
     if (bad_jacobian) *bad_jacobian = (h_bad != 0);
   }
 done:
-  cudaFree(d_veff); cudaFree(d_scratch); cudaFree(d_bad);
+  cudaFree(d_veff_own); cudaFree(d_scratch); cudaFree(d_bad);
   return err;
 }
 }  // namespace
 
-cudaError_t build_sf_fields(Op* op, const double* veff_q_host, cudaStream_t stream) {
+cudaError_t build_sf_fields_dev(Op* op, const double* veff_q_dev, cudaStream_t stream) {
   cudaError_t err = cudaSuccess;
   const int nq1 = op->nq1;
   const int nf = op->kpoint ? 10 : 7;
   const size_t elems = (size_t)op->n_cells * nq1 * nf * 64;
-  double* d_veff = nullptr;
   if (!op->sf_coef) {
     CK(cudaMalloc((void**)&op->sf_coef, elems * sizeof(double)));
     CK(cudaMemsetAsync(op->sf_coef, 0, elems * sizeof(double), stream));   // lanes beyond the Gauss grid (p < 6) stay zero
   }
-  CK(upload(&d_veff, veff_q_host, (size_t)op->n_cells * op->n_q, stream));
   {
     SetupTables tb{op->setup_pp, op->setup_phi, op->setup_gx, op->setup_gw};
-    k_sf_fields<<<(unsigned)op->n_cells, 256, 0, stream>>>(nq1, nf, op->n_cells, tb, op->setup_verts, d_veff, op->kvec[0], op->kvec[1],
-                                                           op->kvec[2], op->sf_coef);
+    k_sf_fields<<<(unsigned)op->n_cells, 256, 0, stream>>>(nq1, nf, op->n_cells, tb, op->setup_verts, veff_q_dev, op->kvec[0],
+                                                           op->kvec[1], op->kvec[2], op->sf_coef);
     CK(cudaGetLastError());
-    CK(cudaStreamSynchronize(stream));
   }
+done:
+  return err;
+}
+
+cudaError_t build_sf_fields(Op* op, const double* veff_q_host, cudaStream_t stream) {
+  cudaError_t err = cudaSuccess;
+  double* d_veff = nullptr;
+  CK(upload(&d_veff, veff_q_host, (size_t)op->n_cells * op->n_q, stream));
+  CK(build_sf_fields_dev(op, d_veff, stream));
+  CK(cudaStreamSynchronize(stream));
 done:
   cudaFree(d_veff);
   return err;
+}
+
+cudaError_t refresh_dense_matrices(Op* op, cudaStream_t stream) {
+  if (!op->dense_stale) return cudaSuccess;
+  cudaError_t e = launch_local_matrices(op, nullptr, stream, /*zero_tail=*/0, nullptr, op->veff_dev);
+  if (e != cudaSuccess) return e;
+  if ((e = capture_diagonal(op, stream))) return e;
+  op->dense_stale = false;
+  op->launches += 2;
+  return cudaSuccess;
 }
 
 cudaError_t rebuild_local_matrices(Op* op, const double* veff_q_host, cudaStream_t stream) {

@@ -168,23 +168,29 @@ def test_update_potential_equals_a_fresh_operator_and_the_oracle():
     veff2 = 0.6 * wl.veff_q - 0.25 + 0.05 * rng.standard_normal(wl.veff_q.shape)
     wl2 = dataclasses.replace(wl, veff_q=veff2)
     oop2 = orc.operator_from_workload(wl2)
+    # variant 0: the sum-factorised default (the update refreshes the quadrature-point fields only); 4 and 1: dense kernels,
+    # whose cell matrices are rebuilt lazily from the device copy of the samples the first time they are asked for
     for precision, tol in ((64, 1e-10), (32, 1e-4)):
         Xr = X.astype(np.float32).astype(np.float64) if precision == 32 else X
-        op = Operator.from_workload(wl, precision=precision)
-        Xd = torch.tensor(Xr, dtype=op.dtype, device="cuda")
-        F = Xd.clone()
-        op.chebyshev_filter(F, 4, a, b, a0)                   # leaves the shift c on the diagonals
-        op.update_potential(veff2)
-        Y_upd = op.apply_H(Xd)
-        fresh = Operator.from_workload(wl2, precision=precision)
-        Y_new = fresh.apply_H(Xd)
-        assert torch.equal(Y_upd, Y_new)
-        assert_block_close(Y_upd.double().cpu().numpy(), orc.apply_H(oop2, Xr), tol, f"update_potential FP{precision}")
-        F1, F2 = Xd.clone(), Xd.clone()
-        op.chebyshev_filter(F1, 5, a, b + 1.0, a0)
-        fresh.chebyshev_filter(F2, 5, a, b + 1.0, a0)
-        assert torch.equal(F1, F2)
-        op.close(); fresh.close()
+        for variants in ((0, 0), (4, 4), (0, 4), (1, 1)):         # (variant before the update, variant after it)
+            op = Operator.from_workload(wl, precision=precision)
+            op.set_kernel_variant(variants[0])
+            Xd = torch.tensor(Xr, dtype=op.dtype, device="cuda")
+            F = Xd.clone()
+            op.chebyshev_filter(F, 4, a, b, a0)                   # leaves the shift c on the diagonals of the dense matrices
+            op.update_potential(veff2)
+            op.set_kernel_variant(variants[1])
+            Y_upd = op.apply_H(Xd)
+            fresh = Operator.from_workload(wl2, precision=precision)
+            fresh.set_kernel_variant(variants[1])
+            Y_new = fresh.apply_H(Xd)
+            assert torch.equal(Y_upd, Y_new), variants
+            assert_block_close(Y_upd.double().cpu().numpy(), orc.apply_H(oop2, Xr), tol, f"update_potential FP{precision} {variants}")
+            F1, F2 = Xd.clone(), Xd.clone()
+            op.chebyshev_filter(F1, 5, a, b + 1.0, a0)
+            fresh.chebyshev_filter(F2, 5, a, b + 1.0, a0)
+            assert torch.equal(F1, F2), variants
+            op.close(); fresh.close()
 
 
 @pytest.mark.parametrize("name", ["p6_nonlocal_ragged", "config1"])
