@@ -39,8 +39,8 @@ NCU_TRAFFIC_BYTES_PER_LAUNCH = {
     (3, "k_apply_dmma_p<double>"): 14.54e9,    # same file: 11.68 GB read + 2.86 GB written
     (5, "k_apply_sf<double>"): 27.24e9,        # profiles/r02_sf_kernel.md: 18.48 GB read + 8.76 GB written
     (3, "k_apply_sf<double>"): 8.82e9,         # same file: 5.97 GB read + 2.84 GB written
-    (5, "k_apply_sf_ws<double>"): 27.28e9,     # profiles/r02b_ws_kernel.md: 18.49 GB read + 8.79 GB written
-    (3, "k_apply_sf_ws<double>"): 8.83e9,      # same file: 5.97 GB read + 2.86 GB written
+    (5, "k_apply_sf_ws<double>"): 27.22e9,     # profiles/r02c_ws_kernel.md: 18.48 GB read + 8.74 GB written
+    (3, "k_apply_sf_ws<double>"): 8.80e9,      # same file: 5.97 GB read + 2.83 GB written
 }
 
 
