@@ -283,6 +283,11 @@ int64_t chfsi_launch_count(const chfsi_op* op);
  * For tests and A/B measurements. */
 int chfsi_set_kernel_variant(chfsi_op* op, int variant);
 
+/* Kernel of the FP32 blocks of the mixed-precision Rayleigh-Ritz products S and H^ (3xTF32 products, FP64 totals):
+ *   0 = automatic = 1;  1 = tcgen05.mma kind::tf32 with TMEM accumulators, operands by TMA (csrc/rr_umma.cu);
+ *   2 = mma.sync m16n8k8 (csrc/rr_kernels.cu k_xty_tf32).  Same results up to the rounding of the FP32 partial sums. */
+int chfsi_set_rr_variant(chfsi_op* op, int variant);
+
 /* Per-kernel device timing for the roofline report.  While enabled, every H~ application records one CUDA
  * event pair on the launching stream around its per-cell contraction launches (the dominant kernel; steps 1,
  * 2, 3d, 4, 5 of the path) and one around its projector launches (steps 3a-3c).  chfsi_get_profile waits for

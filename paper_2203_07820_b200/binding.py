@@ -23,7 +23,7 @@ EXPORTED_SYMBOLS = [
     "chfsi_apply_H_with_coefficients", "chfsi_pack_rows", "chfsi_unpack_rows", "chfsi_recurrence_update", "chfsi_destroy", "chfsi_update_potential", "chfsi_get_info", "chfsi_workspace_bytes", "chfsi_mass_diag",
     "chfsi_apply_H", "chfsi_overlap_matrix", "chfsi_projected_hamiltonian", "chfsi_subspace_transform",
     "chfsi_cholesky_inverse", "chfsi_overlap_matrix_mixed", "chfsi_projected_hamiltonian_mixed", "chfsi_subspace_transform_mixed", "chfsi_chebyshev_filter", "chfsi_chebyshev_filter_chunked", "chfsi_chebyshev_filter_host",
-    "chfsi_launch_count", "chfsi_set_kernel_variant", "chfsi_set_profiling", "chfsi_get_profile",
+    "chfsi_launch_count", "chfsi_set_kernel_variant", "chfsi_set_rr_variant", "chfsi_set_profiling", "chfsi_get_profile",
     "chfsi_measure_fp64_peak", "chfsi_last_error",
 ]
 
@@ -139,6 +139,8 @@ def load_library(build_if_missing: bool = True):
     lib_.chfsi_launch_count.restype = i64
     lib_.chfsi_set_kernel_variant.argtypes = [vp, C.c_int]
     lib_.chfsi_set_kernel_variant.restype = C.c_int
+    lib_.chfsi_set_rr_variant.argtypes = [vp, C.c_int]
+    lib_.chfsi_set_rr_variant.restype = C.c_int
     lib_.chfsi_set_profiling.argtypes = [vp, C.c_int]
     lib_.chfsi_set_profiling.restype = C.c_int
     lib_.chfsi_get_profile.argtypes = [vp, C.POINTER(_Profile)]
@@ -510,6 +512,9 @@ class Operator:
 
     def set_kernel_variant(self, variant: int):
         self._check(load_library().chfsi_set_kernel_variant(self._h, int(variant)))
+
+    def set_rr_variant(self, variant: int):
+        self._check(load_library().chfsi_set_rr_variant(self._h, int(variant)))
 
     def set_profiling(self, enabled: bool):
         self._check(load_library().chfsi_set_profiling(self._h, int(bool(enabled))))

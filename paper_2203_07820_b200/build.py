@@ -15,7 +15,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libchfsi.so")
-SOURCES = ["api.cu", "apply_kernels.cu", "rr_kernels.cu", "rr_dense.cu", "part_kernels.cu", "setup_kernels.cu", "host_setup.cpp", "peak_fp64.cu"]
+SOURCES = ["api.cu", "apply_kernels.cu", "rr_kernels.cu", "rr_dense.cu", "rr_umma.cu", "part_kernels.cu", "setup_kernels.cu", "host_setup.cpp", "peak_fp64.cu"]
 HEADERS = sorted(os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".h", ".cuh"))) + \
     [os.path.join(HERE, "..", "include", "chfsi.h")]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]

@@ -929,6 +929,13 @@ int chfsi_set_kernel_variant(chfsi_op* op, int variant) {
   return CHFSI_OK;
 }
 
+int chfsi_set_rr_variant(chfsi_op* op, int variant) {
+  if (!op) return CHFSI_ERR_BAD_ARGUMENT;
+  if (variant < 0 || variant > 2) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "rr variant must be 0 .. 2");
+  op->rr_variant = variant;
+  return CHFSI_OK;
+}
+
 int chfsi_set_profiling(chfsi_op* op, int enabled) {
   if (!op) return CHFSI_ERR_BAD_ARGUMENT;
   op->profiling = enabled != 0;

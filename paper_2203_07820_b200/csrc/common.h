@@ -92,6 +92,7 @@ struct Op {
   // kernel is (cell, part, column tile), so the accumulators of 8 warps always fit the register file.
   int n_parts = 1, mw = 0;
   int precision = 64, assembly = 0, variant = 0;
+  int rr_variant = 0;                    // FP32 blocks of the mixed Rayleigh-Ritz products: 0 / 1 tcgen05 (rr_umma.cu), 2 mma.sync
   int64_t n_cells = 0, n_dofs = 0, n_proj = 0, nnz_cp = 0, n_pc_cells = 0;
   int n_colors = 0;
   std::vector<int32_t> color_ptr;        // host copy
@@ -257,6 +258,11 @@ cudaError_t launch_xz(Op* op, const double* Y, int64_t ldy, const double* Z, int
 cudaError_t init_rr_mixed_kernels();
 cudaError_t launch_to_f32(Op* op, const double* src, int64_t lds, float* dst, int64_t ldd, int64_t rows, int cols, int zero_diag,
                           double* diag, cudaStream_t st);
+// tcgen05 form of the same product (rr_umma.cu): partial sums of the row splits into Cpart[n_split][N1][N2]; false when the
+// tensor maps cannot be encoded (the caller then runs k_xty_tf32).  init_umma_kernels: per-device kernel attributes.
+cudaError_t init_umma_kernels();
+bool launch_xty_umma(const float* A, int64_t lda, const float* B, int64_t ldb, int64_t n_rows, int N1, int N2, int n_split,
+                     int64_t rows_per_split, int skip_block, int row_block0, int col_block0, double* Cpart, cudaStream_t stream);
 cudaError_t launch_xty_tf32(Op* op, const float* A, int64_t lda, const float* B, int64_t ldb, int64_t n_rows, int N1, int N2,
                             int skip_block, int row_block0, int col_block0, double* C, int64_t ldc, cudaStream_t st);
 cudaError_t launch_xz_tf32(Op* op, const float* Y32, int64_t ldy32, const float* Z32, int64_t ldz32, const double* Y, int64_t ldy,

@@ -545,7 +545,9 @@ constexpr size_t xz32_smem_bytes() { return (size_t)2 * (kZ32M * kZ32LdA + kZ32K
 }  // namespace
 
 cudaError_t init_rr_mixed_kernels() {
-  cudaError_t e = cudaFuncSetAttribute(k_xty_tf32, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)xty32_smem_bytes());
+  cudaError_t e = init_umma_kernels();
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(k_xty_tf32, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)xty32_smem_bytes());
   if (e != cudaSuccess) return e;
   return cudaFuncSetAttribute(k_xz_tf32, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)xz32_smem_bytes());
 }
@@ -577,8 +579,12 @@ cudaError_t launch_xty_tf32(Op* op, const float* A, int64_t lda, const float* B,
     op->rr_scratch_bytes = need;
   }
   dim3 grid((unsigned)ti, (unsigned)tj, (unsigned)n_split);
-  k_xty_tf32<<<grid, 256, xty32_smem_bytes(), st>>>(A, lda, B, ldb, n_rows, N1, N2, rows_per_split, skip_block, row_block0,
-                                                    col_block0, reinterpret_cast<double*>(op->rr_scratch));
+  // rr_variant 0 / 1: the tcgen05 kernel (rr_umma.cu); 2, or no tensor maps: the mma.sync kernel below.  Same partial sums layout.
+  if (op->rr_variant == 2 ||
+      !launch_xty_umma(A, lda, B, ldb, n_rows, N1, N2, n_split, rows_per_split, skip_block, row_block0, col_block0,
+                       reinterpret_cast<double*>(op->rr_scratch), st))
+    k_xty_tf32<<<grid, 256, xty32_smem_bytes(), st>>>(A, lda, B, ldb, n_rows, N1, N2, rows_per_split, skip_block, row_block0,
+                                                      col_block0, reinterpret_cast<double*>(op->rr_scratch));
   k_xty_reduce_masked<<<(unsigned)(((int64_t)N1 * N2 + 255) / 256), 256, 0, st>>>(
       reinterpret_cast<const double*>(op->rr_scratch), n_split, N1, N2, skip_block, row_block0, col_block0, C, ldc);
   op->launches += 2;

@@ -1,0 +1,288 @@
+// C = A^T B of two tall FP32 blocks on the 5th-generation tensor cores (tcgen05.mma kind::tf32, accumulators in TMEM):
+// the FP32 blocks of the paper's mixed-precision Rayleigh-Ritz products (Sec. 3.2 / 4.4.1: Eq. 38-39, PAPER.md:426-440;
+// PAPER.md:564 "FP32 off-diagonal blocks").  Drop-in for k_xty_tf32 (rr_kernels.cu): same tiles (128 x 64), same split-row
+// partial sums Cpart[z][N1][N2] in FP64, same masked reduction.
+//
+//   * an FP32 product is a 3xTF32 split, a b ~ a_hi b_lo + a_lo b_hi + a_hi b_hi: hi = the value as the tensor core reads it
+//     (kind::tf32 ignores the low 13 mantissa bits), lo = x - hi (exact in FP32) computed by four "split" warps from the
+//     tile that the TMA has put into shared memory, written into a second tile of the same layout;
+//   * both operands are MN-major (the stored layout [rows][columns] has the output index fastest and the contraction
+//     index = rows).  For MN-major 32-bit operands the tensor core takes ONE shared-memory layout, the 128-byte swizzle with
+//     32-byte atoms (SWIZZLE_128B_BASE32B: atoms of 32 columns x 4 rows), which is what a TMA box {32 columns, 32 rows}
+//     with CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B writes; one tcgen05.mma (M = 128, N = 64, K = 8) consumes two such atoms;
+//   * the FP32 accumulator of the tensor pipe does not round to nearest, so an accumulation chain is ONE 32-row stage
+//     (12 MMAs from zero) in one of two 64-column TMEM buffers; eight epilogue warps drain it (tcgen05.ld), add the stage
+//     sums in FP32 registers with round-to-nearest for 16 stages and then into FP64 totals -- while the next stage's MMAs
+//     run into the other buffer;
+//   * roles: 8 epilogue warps, 4 split warps, 1 TMA producer warp, 1 MMA warp (one elected lane issues); 4-stage ring.
+#include <cuda.h>
+
+#include <algorithm>
+
+#include "common.h"
+
+namespace chfsi {
+namespace {
+
+constexpr int kUM = 128, kUN = 64, kUK = 32, kUStages = 4;
+constexpr int kUEpiWarps = 8, kUSplitWarps = 4;
+constexpr int kUThreads = 32 * (kUEpiWarps + kUSplitWarps + 2);
+constexpr int kUABytes = kUK * kUM * 4, kUBBytes = kUK * kUN * 4;              // 16 KB, 8 KB
+constexpr int kUStageBytes = 2 * (kUABytes + kUBBytes);                          // hi + lo tiles of A and B: 48 KB
+constexpr int kUFlush = 16;                                                      // stages per FP32 -> FP64 flush
+constexpr size_t kUSmemBytes = (size_t)kUStages * kUStageBytes + 1024 + 256;
+
+__device__ __forceinline__ uint32_t u_smem(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void u_mbar_init(uint64_t* bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(u_smem(bar)), "r"(count));
+}
+__device__ __forceinline__ void u_mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(u_smem(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void u_mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(u_smem(bar)) : "memory");
+}
+__device__ __forceinline__ void u_mbar_wait(uint64_t* bar, uint32_t parity) {
+  uint32_t done;
+  do {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(done)
+        : "r"(u_smem(bar)), "r"(parity)
+        : "memory");
+  } while (!done);
+}
+// box {32 columns, 32 rows} of a 2-D FP32 tensor at (column c0, row r0) -> dst (32 rows of 128 bytes, 128B-swizzled)
+__device__ __forceinline__ void u_tma_load(void* dst, const CUtensorMap* tm, int c0, int r0, uint64_t* bar) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];" ::"r"(
+                   u_smem(dst)),
+               "l"(tm), "r"(u_smem(bar)), "r"(c0), "r"(r0)
+               : "memory");
+}
+// shared-memory matrix descriptor of an MN-major operand in the 128B / 32B-atom swizzle: atoms of 32 columns x 4 rows (512
+// bytes); leading byte offset = distance between atoms along MN, stride byte offset = distance between atoms along K
+__device__ __forceinline__ uint64_t u_desc(uint32_t smem_addr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
+  uint64_t d = 0;
+  d |= (uint64_t)((smem_addr >> 4) & 0x3fff);
+  d |= (uint64_t)((lbo_bytes >> 4) & 0x3fff) << 16;
+  d |= (uint64_t)((sbo_bytes >> 4) & 0x3fff) << 32;
+  d |= (uint64_t)1 << 46;                                  // descriptor version of sm_100
+  d |= (uint64_t)1 << 61;                                  // SWIZZLE_128B_BASE32B: the one layout of MN-major 32-bit operands
+  return d;
+}
+// instruction descriptor: D = F32, A = B = TF32, both MN-major, N = 64, M = 128, dense, no negation
+constexpr uint32_t kUIdesc = (1u << 4) | (2u << 7) | (2u << 10) | (1u << 15) | (1u << 16) | ((uint32_t)(kUN >> 3) << 17) |
+                             ((uint32_t)(kUM >> 4) << 24);
+__device__ __forceinline__ void u_mma(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "setp.ne.b32 p, %4, 0;\n"
+      "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n"
+      "}\n" ::"r"(tmem_d),
+      "l"(adesc), "l"(bdesc), "r"(kUIdesc), "r"(accumulate)
+      : "memory");
+}
+__device__ __forceinline__ void u_commit(uint64_t* bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(u_smem(bar)) : "memory");
+}
+// 32 consecutive TMEM columns of this thread's lane (32x32b shape: lane = 32 (warp % 4) + lane id)
+__device__ __forceinline__ void u_tmem_ld32(uint32_t taddr, float (&v)[32]) {
+  uint32_t r[32];
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, %17, "
+      "%18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]),
+        "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]), "=r"(r[17]), "=r"(r[18]),
+        "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]),
+        "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+      : "r"(taddr)
+      : "memory");
+  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+  for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
+}
+
+__global__ void __launch_bounds__(kUThreads, 1) k_xty_umma(const __grid_constant__ CUtensorMap tmA,
+                                                           const __grid_constant__ CUtensorMap tmB, int64_t n_rows, int N1, int N2,
+                                                           int64_t rows_per_split, int skip_block, int row_block0, int col_block0,
+                                                           double* __restrict__ Cpart) {
+  const int i0 = blockIdx.x * kUM, j0 = blockIdx.y * kUN;
+  if (skip_block > 0) {                                        // tiles inside an FP64 diagonal block: not ours (k_xty_tf32's rule)
+    const int bi0 = (row_block0 + i0) / skip_block, bi1 = (row_block0 + min(i0 + kUM, N1) - 1) / skip_block;
+    const int bj0 = (col_block0 + j0) / skip_block, bj1 = (col_block0 + min(j0 + kUN, N2) - 1) / skip_block;
+    if (bi0 == bi1 && bj0 == bj1 && bi0 == bj0) return;
+  }
+  extern __shared__ unsigned char u_raw[];
+  unsigned char* sm = reinterpret_cast<unsigned char*>(((uintptr_t)u_raw + 1023) & ~(uintptr_t)1023);   // swizzle atoms: 1024-byte aligned
+  uint64_t* bars = reinterpret_cast<uint64_t*>(sm + (size_t)kUStages * kUStageBytes);
+  uint64_t* full_raw = bars;                     // [stages] TMA landed
+  uint64_t* full_split = bars + kUStages;        // [stages] lo tiles written
+  uint64_t* empty = bars + 2 * kUStages;         // [stages] MMAs that read the stage are done
+  uint64_t* acc_full = bars + 3 * kUStages;      // [2] accumulator holds a finished stage sum
+  uint64_t* acc_empty = acc_full + 2;            // [2] accumulator drained
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_empty + 2);
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int64_t g0 = (int64_t)blockIdx.z * rows_per_split, g1 = min(n_rows, g0 + rows_per_split);
+  const int nstage = (int)((g1 - g0 + kUK - 1) / kUK);
+
+  if (tid == 0) {
+    for (int s = 0; s < kUStages; ++s) { u_mbar_init(full_raw + s, 1); u_mbar_init(full_split + s, kUSplitWarps); u_mbar_init(empty + s, 1); }
+    for (int a = 0; a < 2; ++a) { u_mbar_init(acc_full + a, 1); u_mbar_init(acc_empty + a, kUEpiWarps); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == kUEpiWarps + kUSplitWarps + 1) {                 // the MMA warp owns the tensor memory: two 64-column accumulators
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(u_smem(tmem_slot)), "n"(2 * kUN) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  const uint32_t tmem = *reinterpret_cast<volatile uint32_t*>(tmem_slot);
+
+  if (warp < kUEpiWarps) {
+    // ---- epilogue warps: lane quarter q = warp % 4 (rows 32 q + lane of the tile), column half h = warp / 4 --------------
+    const int q = warp & 3, h = warp >> 2;
+    float p32[32];
+    double tot[32];
+#pragma unroll
+    for (int j = 0; j < 32; ++j) { p32[j] = 0.0f; tot[j] = 0.0; }
+    for (int it = 0; it < nstage; ++it) {
+      const int a = it & 1;
+      u_mbar_wait(acc_full + a, (uint32_t)(it >> 1) & 1u);
+      asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+      float v[32];
+      u_tmem_ld32(tmem + ((uint32_t)(32 * q) << 16) + (uint32_t)(a * kUN + 32 * h), v);
+      asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+      __syncwarp();
+      if (lane == 0) u_mbar_arrive(acc_empty + a);
+#pragma unroll
+      for (int j = 0; j < 32; ++j) p32[j] += v[j];                              // round-to-nearest FP32 adds of stage sums
+      if ((it % kUFlush) == kUFlush - 1 || it == nstage - 1) {
+#pragma unroll
+        for (int j = 0; j < 32; ++j) { tot[j] += (double)p32[j]; p32[j] = 0.0f; }
+      }
+    }
+    const int r = i0 + 32 * q + lane;
+    if (r < N1) {
+      double* Cp = Cpart + (int64_t)blockIdx.z * N1 * N2 + (int64_t)r * N2 + j0 + 32 * h;
+#pragma unroll
+      for (int j = 0; j < 32; ++j)
+        if (j0 + 32 * h + j < N2) Cp[j] = tot[j];
+    }
+  } else if (warp < kUEpiWarps + kUSplitWarps) {
+    // ---- split warps: lo = x - tf32(x) for the stage's A and B tiles (same offsets: the swizzle is element-wise transparent) ---
+    const int st = tid - 32 * kUEpiWarps;
+    for (int it = 0; it < nstage; ++it) {
+      const int s = it % kUStages;
+      unsigned char* base = sm + (size_t)s * kUStageBytes;
+      u_mbar_wait(full_raw + s, (uint32_t)(it / kUStages) & 1u);
+      auto split = [](const float4* src, float4* dst, int n4, int t0) {
+        for (int e = t0; e < n4; e += 32 * kUSplitWarps) {
+          const float4 x = src[e];
+          float4 l;
+          l.x = x.x - __uint_as_float(__float_as_uint(x.x) & 0xffffe000u);
+          l.y = x.y - __uint_as_float(__float_as_uint(x.y) & 0xffffe000u);
+          l.z = x.z - __uint_as_float(__float_as_uint(x.z) & 0xffffe000u);
+          l.w = x.w - __uint_as_float(__float_as_uint(x.w) & 0xffffe000u);
+          dst[e] = l;
+        }
+      };
+      split(reinterpret_cast<const float4*>(base), reinterpret_cast<float4*>(base + kUABytes), kUABytes / 16, st);
+      split(reinterpret_cast<const float4*>(base + 2 * kUABytes), reinterpret_cast<float4*>(base + 2 * kUABytes + kUBBytes),
+            kUBBytes / 16, st);
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic writes of the lo tiles before the tensor core reads them
+      __syncwarp();
+      if (lane == 0) u_mbar_arrive(full_split + s);
+    }
+  } else if (warp == kUEpiWarps + kUSplitWarps) {
+    // ---- TMA producer ---------------------------------------------------------------------------------------------------
+    if (lane == 0) {
+      for (int it = 0; it < nstage; ++it) {
+        const int s = it % kUStages;
+        unsigned char* base = sm + (size_t)s * kUStageBytes;
+        u_mbar_wait(empty + s, ((uint32_t)(it / kUStages) & 1u) ^ 1u);
+        u_mbar_expect_tx(full_raw + s, (uint32_t)(kUABytes + kUBBytes));
+        const int r0 = (int)(g0 + (int64_t)it * kUK);
+#pragma unroll
+        for (int m = 0; m < kUM / 32; ++m) u_tma_load(base + m * 4096, &tmA, i0 + 32 * m, r0, full_raw + s);
+#pragma unroll
+        for (int m = 0; m < kUN / 32; ++m) u_tma_load(base + 2 * kUABytes + m * 4096, &tmB, j0 + 32 * m, r0, full_raw + s);
+      }
+    }
+  } else {
+    // ---- MMA warp: one lane issues; per stage 4 k-atoms x (hi lo + lo hi + hi hi) from zero into accumulator it & 1 --------
+    if (lane == 0) {
+      for (int it = 0; it < nstage; ++it) {
+        const int s = it % kUStages, a = it & 1;
+        const uint32_t sbase = u_smem(sm + (size_t)s * kUStageBytes);
+        u_mbar_wait(acc_empty + a, ((uint32_t)(it >> 1) & 1u) ^ 1u);
+        u_mbar_wait(full_split + s, (uint32_t)(it / kUStages) & 1u);
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        const uint32_t d = tmem + (uint32_t)(a * kUN);
+#pragma unroll
+        for (int ka = 0; ka < kUK / 8; ++ka) {
+          const uint64_t ahi = u_desc(sbase + ka * 1024, 4096, 512), alo = u_desc(sbase + kUABytes + ka * 1024, 4096, 512);
+          const uint64_t bhi = u_desc(sbase + 2 * kUABytes + ka * 1024, 4096, 512);
+          const uint64_t blo = u_desc(sbase + 2 * kUABytes + kUBBytes + ka * 1024, 4096, 512);
+          u_mma(d, ahi, blo, ka > 0 ? 1u : 0u);
+          u_mma(d, alo, bhi, 1u);
+          u_mma(d, ahi, bhi, 1u);
+        }
+        u_commit(empty + s);          // the stage may be refilled once these MMAs have read it
+        u_commit(acc_full + a);       // ... and the accumulator holds the stage sum
+      }
+    }
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  if (warp == kUEpiWarps + kUSplitWarps + 1)
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(2 * kUN) : "memory");
+}
+
+using UEncodeFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                               const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                               CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+UEncodeFn u_encode_fn() {
+  static UEncodeFn fn = [] {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess)
+      p = nullptr;
+    return reinterpret_cast<UEncodeFn>(p);
+  }();
+  return fn;
+}
+// FP32 block [rows][ld] restricted to `cols` columns; box = 32 columns x 32 rows, 128-byte swizzle, zero fill outside
+bool u_make_map(CUtensorMap* tm, const float* base, int64_t rows, int64_t cols, int64_t ld) {
+  UEncodeFn enc = u_encode_fn();
+  if (!enc || rows < 1 || cols < 1 || (ld * 4) % 16 != 0 || (uintptr_t)base % 16 != 0) return false;
+  const cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
+  const cuuint64_t strides[1] = {(cuuint64_t)ld * 4};
+  const cuuint32_t box[2] = {32, (cuuint32_t)kUK};
+  const cuuint32_t estr[2] = {1, 1};
+  return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+             CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+}  // namespace
+
+cudaError_t init_umma_kernels() {
+  return cudaFuncSetAttribute(k_xty_umma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kUSmemBytes);
+}
+
+// Cpart[z][N1][N2] (FP64) = per-split sums of A^T B; returns false when the tensor maps cannot be built (caller falls back)
+bool launch_xty_umma(const float* A, int64_t lda, const float* B, int64_t ldb, int64_t n_rows, int N1, int N2, int n_split,
+                     int64_t rows_per_split, int skip_block, int row_block0, int col_block0, double* Cpart, cudaStream_t st) {
+  CUtensorMap tmA, tmB;
+  if (!u_make_map(&tmA, A, n_rows, N1, lda) || !u_make_map(&tmB, B, n_rows, N2, ldb)) return false;
+  dim3 grid((unsigned)((N1 + kUM - 1) / kUM), (unsigned)((N2 + kUN - 1) / kUN), (unsigned)n_split);
+  k_xty_umma<<<grid, kUThreads, kUSmemBytes, st>>>(tmA, tmB, n_rows, N1, N2, rows_per_split, skip_block, row_block0, col_block0, Cpart);
+  return true;
+}
+
+}  // namespace chfsi
