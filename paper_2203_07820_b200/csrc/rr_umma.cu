@@ -10,9 +10,9 @@
 //     index = rows).  For MN-major 32-bit operands the tensor core takes ONE shared-memory layout, the 128-byte swizzle with
 //     32-byte atoms (SWIZZLE_128B_BASE32B: atoms of 32 columns x 4 rows), which is what a TMA box {32 columns, 32 rows}
 //     with CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B writes; one tcgen05.mma (M = 128, N = 64, K = 8) consumes two such atoms;
-//   * the FP32 accumulator of the tensor pipe does not round to nearest, so an accumulation chain is ONE 32-row stage
-//     (12 MMAs from zero) in one of two 64-column TMEM buffers; eight epilogue warps drain it (tcgen05.ld), add the stage
-//     sums in FP32 registers with round-to-nearest for 16 stages and then into FP64 totals -- while the next stage's MMAs
+//   * the FP32 accumulator of the tensor pipe does not round to nearest, so an accumulation chain is kept to TWO 32-row stages
+//     (24 MMAs from zero) in one of two 64-column TMEM buffers; eight epilogue warps drain it (tcgen05.ld), add the chain
+//     sums in FP32 registers with round-to-nearest for 8 chains and then into FP64 totals -- while the next stage's MMAs
 //     run into the other buffer;
 //   * roles: 8 epilogue warps, 4 split warps, 1 TMA producer warp, 1 MMA warp (one elected lane issues); 4-stage ring.
 #include <cuda.h>
@@ -29,7 +29,8 @@ constexpr int kUEpiWarps = 8, kUSplitWarps = 4;
 constexpr int kUThreads = 32 * (kUEpiWarps + kUSplitWarps + 2);
 constexpr int kUABytes = kUK * kUM * 4, kUBBytes = kUK * kUN * 4;              // 16 KB, 8 KB
 constexpr int kUStageBytes = 2 * (kUABytes + kUBBytes);                          // hi + lo tiles of A and B: 48 KB
-constexpr int kUFlush = 16;                                                      // stages per FP32 -> FP64 flush
+constexpr int kUChain = 2;                                                       // stages per accumulation chain in TMEM
+constexpr int kUFlush = 8;                                                       // chains per FP32 -> FP64 flush
 constexpr size_t kUSmemBytes = (size_t)kUStages * kUStageBytes + 1024 + 256;
 
 __device__ __forceinline__ uint32_t u_smem(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -151,7 +152,8 @@ __global__ void __launch_bounds__(kUThreads, 1) k_xty_umma(const __grid_constant
     double tot[32];
 #pragma unroll
     for (int j = 0; j < 32; ++j) { p32[j] = 0.0f; tot[j] = 0.0; }
-    for (int it = 0; it < nstage; ++it) {
+    const int nchain = (nstage + kUChain - 1) / kUChain;
+    for (int it = 0; it < nchain; ++it) {
       const int a = it & 1;
       u_mbar_wait(acc_full + a, (uint32_t)(it >> 1) & 1u);
       asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
@@ -161,8 +163,8 @@ __global__ void __launch_bounds__(kUThreads, 1) k_xty_umma(const __grid_constant
       __syncwarp();
       if (lane == 0) u_mbar_arrive(acc_empty + a);
 #pragma unroll
-      for (int j = 0; j < 32; ++j) p32[j] += v[j];                              // round-to-nearest FP32 adds of stage sums
-      if ((it % kUFlush) == kUFlush - 1 || it == nstage - 1) {
+      for (int j = 0; j < 32; ++j) p32[j] += v[j];                              // round-to-nearest FP32 adds of chain sums
+      if ((it % kUFlush) == kUFlush - 1 || it == nchain - 1) {
 #pragma unroll
         for (int j = 0; j < 32; ++j) { tot[j] += (double)p32[j]; p32[j] = 0.0f; }
       }
@@ -218,9 +220,10 @@ __global__ void __launch_bounds__(kUThreads, 1) k_xty_umma(const __grid_constant
     // ---- MMA warp: one lane issues; per stage 4 k-atoms x (hi lo + lo hi + hi hi) from zero into accumulator it & 1 --------
     if (lane == 0) {
       for (int it = 0; it < nstage; ++it) {
-        const int s = it % kUStages, a = it & 1;
+        const int s = it % kUStages, ch = it / kUChain, a = ch & 1;
+        const bool first = it % kUChain == 0, last = it % kUChain == kUChain - 1 || it == nstage - 1;
         const uint32_t sbase = u_smem(sm + (size_t)s * kUStageBytes);
-        u_mbar_wait(acc_empty + a, ((uint32_t)(it >> 1) & 1u) ^ 1u);
+        if (first) u_mbar_wait(acc_empty + a, ((uint32_t)(ch >> 1) & 1u) ^ 1u);
         u_mbar_wait(full_split + s, (uint32_t)(it / kUStages) & 1u);
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         const uint32_t d = tmem + (uint32_t)(a * kUN);
@@ -229,12 +232,12 @@ __global__ void __launch_bounds__(kUThreads, 1) k_xty_umma(const __grid_constant
           const uint64_t ahi = u_desc(sbase + ka * 1024, 4096, 512), alo = u_desc(sbase + kUABytes + ka * 1024, 4096, 512);
           const uint64_t bhi = u_desc(sbase + 2 * kUABytes + ka * 1024, 4096, 512);
           const uint64_t blo = u_desc(sbase + 2 * kUABytes + kUBBytes + ka * 1024, 4096, 512);
-          u_mma(d, ahi, blo, ka > 0 ? 1u : 0u);
+          u_mma(d, ahi, blo, (ka > 0 || !first) ? 1u : 0u);
           u_mma(d, alo, bhi, 1u);
           u_mma(d, ahi, bhi, 1u);
         }
         u_commit(empty + s);          // the stage may be refilled once these MMAs have read it
-        u_commit(acc_full + a);       // ... and the accumulator holds the stage sum
+        if (last) u_commit(acc_full + a);   // ... and the accumulator holds the sum of the chain
       }
     }
   }
