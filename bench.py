@@ -462,11 +462,11 @@ def run_rr(args):
                         "frac": (gemm + apply_flops) / ms_h * 1e-9 / peak},
         "transform_YZ": {"kernel": "k_xz", "ms": ms_z, "tflops": gemm / ms_z * 1e-9, "frac": gemm / ms_z * 1e-9 / peak},
         # mixed precision: same algorithmic flops; speed-up over the FP64 product of the same step
-        "overlap_S_mixed": {"kernel": "k_xty_tf32 (3xTF32) + k_xty (FP64 diagonal blocks)", "ms": ms_sm,
+        "overlap_S_mixed": {"kernel": "k_umma<xty> (tcgen05 kind::tf32, 3xTF32) + k_xty (FP64 diagonal blocks)", "ms": ms_sm,
                             "tflops": gemm / ms_sm * 1e-9, "speedup_vs_fp64": ms_s / ms_sm},
-        "projected_H_mixed": {"kernel": kernel + " + k_xty_tf32 + k_xty (fr-fr block)", "ms": ms_hm,
+        "projected_H_mixed": {"kernel": kernel + " + k_umma<xty> (tcgen05) + k_xty (fr-fr block)", "ms": ms_hm,
                               "tflops": (gemm + apply_flops) / ms_hm * 1e-9, "speedup_vs_fp64": ms_h / ms_hm},
-        "transform_mixed": {"kernel": "k_xz_tf32 (3xTF32 off-diagonal + FP64 diagonal)", "ms": ms_zm,
+        "transform_mixed": {"kernel": "k_umma<xz> (tcgen05 kind::tf32, 3xTF32 off-diagonal + FP64 diagonal)", "ms": ms_zm,
                             "tflops": gemm / ms_zm * 1e-9, "speedup_vs_fp64": ms_z / ms_zm},
         "cholesky_inverse": {"kernel": "k_chol_* / k_trinv_row (N = 1024)", "ms": ms_ch},
         "update_potential": {"kernel": "k_sf_fields (default: quadrature-point fields only; 17 MB of samples H2D)", "ms": ms_dhm_sf},

@@ -263,6 +263,8 @@ cudaError_t launch_to_f32(Op* op, const double* src, int64_t lds, float* dst, in
 cudaError_t init_umma_kernels();
 bool launch_xty_umma(const float* A, int64_t lda, const float* B, int64_t ldb, int64_t n_rows, int N1, int N2, int n_split,
                      int64_t rows_per_split, int skip_block, int row_block0, int col_block0, double* Cpart, cudaStream_t stream);
+bool launch_xz_umma(const float* Y32, int64_t ldy32, const float* Z32, int64_t ldz32, const double* Y, int64_t ldy, const double* zd,
+                    int64_t n_rows, int N, int N2, double* Out, int64_t ldo, cudaStream_t stream);
 cudaError_t launch_xty_tf32(Op* op, const float* A, int64_t lda, const float* B, int64_t ldb, int64_t n_rows, int N1, int N2,
                             int skip_block, int row_block0, int col_block0, double* C, int64_t ldc, cudaStream_t st);
 cudaError_t launch_xz_tf32(Op* op, const float* Y32, int64_t ldy32, const float* Z32, int64_t ldz32, const double* Y, int64_t ldy,

@@ -594,7 +594,8 @@ cudaError_t launch_xty_tf32(Op* op, const float* A, int64_t lda, const float* B,
 cudaError_t launch_xz_tf32(Op* op, const float* Y32, int64_t ldy32, const float* Z32, int64_t ldz32, const double* Y, int64_t ldy,
                            const double* zd, int64_t n_rows, int N, int N2, double* Out, int64_t ldo, cudaStream_t st) {
   dim3 grid((unsigned)((N2 + kZ32N - 1) / kZ32N), (unsigned)((n_rows + kZ32M - 1) / kZ32M));
-  k_xz_tf32<<<grid, 256, xz32_smem_bytes(), st>>>(Y32, ldy32, Z32, ldz32, Y, ldy, zd, n_rows, N, N2, Out, ldo);
+  if (op->rr_variant == 2 || !launch_xz_umma(Y32, ldy32, Z32, ldz32, Y, ldy, zd, n_rows, N, N2, Out, ldo, st))   // tcgen05 first
+    k_xz_tf32<<<grid, 256, xz32_smem_bytes(), st>>>(Y32, ldy32, Z32, ldz32, Y, ldy, zd, n_rows, N, N2, Out, ldo);
   op->launches++;
   return cudaGetLastError();
 }

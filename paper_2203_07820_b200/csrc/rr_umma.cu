@@ -3,9 +3,9 @@
 // PAPER.md:564 "FP32 off-diagonal blocks").  Drop-in for k_xty_tf32 (rr_kernels.cu): same tiles (128 x 64), same split-row
 // partial sums Cpart[z][N1][N2] in FP64, same masked reduction.
 //
-//   * an FP32 product is a 3xTF32 split, a b ~ a_hi b_lo + a_lo b_hi + a_hi b_hi: hi = the value as the tensor core reads it
-//     (kind::tf32 ignores the low 13 mantissa bits), lo = x - hi (exact in FP32) computed by four "split" warps from the
-//     tile that the TMA has put into shared memory, written into a second tile of the same layout;
+//   * an FP32 product is a 3xTF32 split, a b ~ a_hi b_lo + a_lo b_hi + a_hi b_hi: hi = x rounded to TF32 (cvt.rna), lo = x - hi
+//     (exact in FP32), both computed by four "split" warps from the tile that the TMA has put into shared memory: hi replaces
+//     the tile in place, lo goes to a second tile of the same layout (the swizzle is element-wise transparent);
 //   * both operands are MN-major (the stored layout [rows][columns] has the output index fastest and the contraction
 //     index = rows).  For MN-major 32-bit operands the tensor core takes ONE shared-memory layout, the 128-byte swizzle with
 //     32-byte atoms (SWIZZLE_128B_BASE32B: atoms of 32 columns x 4 rows), which is what a TMA box {32 columns, 32 rows}
@@ -66,26 +66,28 @@ __device__ __forceinline__ void u_tma_load(void* dst, const CUtensorMap* tm, int
 }
 // shared-memory matrix descriptor of an MN-major operand in the 128B / 32B-atom swizzle: atoms of 32 columns x 4 rows (512
 // bytes); leading byte offset = distance between atoms along MN, stride byte offset = distance between atoms along K
-__device__ __forceinline__ uint64_t u_desc(uint32_t smem_addr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
+__device__ __forceinline__ uint64_t u_desc(uint32_t smem_addr, uint32_t lbo_bytes, uint32_t sbo_bytes, uint32_t layout_type = 1) {
   uint64_t d = 0;
   d |= (uint64_t)((smem_addr >> 4) & 0x3fff);
   d |= (uint64_t)((lbo_bytes >> 4) & 0x3fff) << 16;
   d |= (uint64_t)((sbo_bytes >> 4) & 0x3fff) << 32;
   d |= (uint64_t)1 << 46;                                  // descriptor version of sm_100
-  d |= (uint64_t)1 << 61;                                  // SWIZZLE_128B_BASE32B: the one layout of MN-major 32-bit operands
+  d |= (uint64_t)layout_type << 61;                        // 1 = SWIZZLE_128B_BASE32B (the one layout of MN-major 32-bit operands), 2 = SWIZZLE_128B
   return d;
 }
 // instruction descriptor: D = F32, A = B = TF32, both MN-major, N = 64, M = 128, dense, no negation
-constexpr uint32_t kUIdesc = (1u << 4) | (2u << 7) | (2u << 10) | (1u << 15) | (1u << 16) | ((uint32_t)(kUN >> 3) << 17) |
-                             ((uint32_t)(kUM >> 4) << 24);
-__device__ __forceinline__ void u_mma(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t accumulate) {
+__host__ __device__ constexpr uint32_t u_idesc(bool a_mn_major) {
+  return (1u << 4) | (2u << 7) | (2u << 10) | ((a_mn_major ? 1u : 0u) << 15) | (1u << 16) | ((uint32_t)(kUN >> 3) << 17) |
+         ((uint32_t)(kUM >> 4) << 24);
+}
+__device__ __forceinline__ void u_mma(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t accumulate, uint32_t idesc) {
   asm volatile(
       "{\n"
       ".reg .pred p;\n"
       "setp.ne.b32 p, %4, 0;\n"
       "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n"
       "}\n" ::"r"(tmem_d),
-      "l"(adesc), "l"(bdesc), "r"(kUIdesc), "r"(accumulate)
+      "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
       : "memory");
 }
 __device__ __forceinline__ void u_commit(uint64_t* bar) {
@@ -108,12 +110,18 @@ __device__ __forceinline__ void u_tmem_ld32(uint32_t taddr, float (&v)[32]) {
   for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
 }
 
-__global__ void __launch_bounds__(kUThreads, 1) k_xty_umma(const __grid_constant__ CUtensorMap tmA,
-                                                           const __grid_constant__ CUtensorMap tmB, int64_t n_rows, int N1, int N2,
-                                                           int64_t rows_per_split, int skip_block, int row_block0, int col_block0,
-                                                           double* __restrict__ Cpart) {
-  const int i0 = blockIdx.x * kUM, j0 = blockIdx.y * kUN;
-  if (skip_block > 0) {                                        // tiles inside an FP64 diagonal block: not ours (k_xty_tf32's rule)
+// XZ = false:  Cpart[z] = A^T B over the rows of split z (A, B: [rows][columns], both MN-major; tile = 128 columns of A x 64 of B)
+// XZ = true:   Out[g][j] = sum_i Y32[g][i] Z32[i][j] + Y[g][j] zd[j]  (subspace transformation with the FP64 diagonal part,
+//              PAPER.md:564): A = Y32 tile of 128 ROWS, K-major (the contraction index i is contiguous: plain 128-byte swizzle),
+//              B = Z32 panel, MN-major; blockIdx.x = column tile, blockIdx.y = row block; N1 = number of contraction indices
+template <bool XZ>
+__global__ void __launch_bounds__(kUThreads, 1) k_umma(const __grid_constant__ CUtensorMap tmA,
+                                                       const __grid_constant__ CUtensorMap tmB, int64_t n_rows, int N1, int N2,
+                                                       int64_t rows_per_split, int skip_block, int row_block0, int col_block0,
+                                                       double* __restrict__ Cpart, const double* __restrict__ Yd, int64_t ldy,
+                                                       const double* __restrict__ zd, int64_t ldo) {
+  const int i0 = XZ ? 0 : blockIdx.x * kUM, j0 = (XZ ? blockIdx.x : blockIdx.y) * kUN;
+  if (!XZ && skip_block > 0) {                                        // tiles inside an FP64 diagonal block: not ours (k_xty_tf32's rule)
     const int bi0 = (row_block0 + i0) / skip_block, bi1 = (row_block0 + min(i0 + kUM, N1) - 1) / skip_block;
     const int bj0 = (col_block0 + j0) / skip_block, bj1 = (col_block0 + min(j0 + kUN, N2) - 1) / skip_block;
     if (bi0 == bi1 && bj0 == bj1 && bi0 == bj0) return;
@@ -128,8 +136,9 @@ __global__ void __launch_bounds__(kUThreads, 1) k_xty_umma(const __grid_constant
   uint64_t* acc_empty = acc_full + 2;            // [2] accumulator drained
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_empty + 2);
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int64_t g0 = (int64_t)blockIdx.z * rows_per_split, g1 = min(n_rows, g0 + rows_per_split);
-  const int nstage = (int)((g1 - g0 + kUK - 1) / kUK);
+  const int64_t g0 = XZ ? (int64_t)blockIdx.y * kUM : (int64_t)blockIdx.z * rows_per_split;
+  const int64_t g1 = min(n_rows, g0 + (XZ ? (int64_t)kUM : rows_per_split));
+  const int nstage = XZ ? (N1 + kUK - 1) / kUK : (int)((g1 - g0 + kUK - 1) / kUK);
 
   if (tid == 0) {
     for (int s = 0; s < kUStages; ++s) { u_mbar_init(full_raw + s, 1); u_mbar_init(full_split + s, kUSplitWarps); u_mbar_init(empty + s, 1); }
@@ -169,12 +178,23 @@ __global__ void __launch_bounds__(kUThreads, 1) k_xty_umma(const __grid_constant
         for (int j = 0; j < 32; ++j) { tot[j] += (double)p32[j]; p32[j] = 0.0f; }
       }
     }
-    const int r = i0 + 32 * q + lane;
-    if (r < N1) {
-      double* Cp = Cpart + (int64_t)blockIdx.z * N1 * N2 + (int64_t)r * N2 + j0 + 32 * h;
+    if (XZ) {
+      const int64_t r = g0 + 32 * q + lane;                                     // Out = FP32 off-diagonal part + FP64 diagonal part
+      if (r < n_rows) {
+        double* op_ = Cpart + r * ldo + j0 + 32 * h;
+        const double* yp = Yd + r * ldy + j0 + 32 * h;
 #pragma unroll
-      for (int j = 0; j < 32; ++j)
-        if (j0 + 32 * h + j < N2) Cp[j] = tot[j];
+        for (int j = 0; j < 32; ++j)
+          if (j0 + 32 * h + j < N2) op_[j] = fma(yp[j], zd[j0 + 32 * h + j], tot[j]);
+      }
+    } else {
+      const int r = i0 + 32 * q + lane;
+      if (r < N1) {
+        double* Cp = Cpart + (int64_t)blockIdx.z * N1 * N2 + (int64_t)r * N2 + j0 + 32 * h;
+#pragma unroll
+        for (int j = 0; j < 32; ++j)
+          if (j0 + 32 * h + j < N2) Cp[j] = tot[j];
+      }
     }
   } else if (warp < kUEpiWarps + kUSplitWarps) {
     // ---- split warps: lo = x - tf32(x) for the stage's A and B tiles (same offsets: the swizzle is element-wise transparent) ---
@@ -183,19 +203,23 @@ __global__ void __launch_bounds__(kUThreads, 1) k_xty_umma(const __grid_constant
       const int s = it % kUStages;
       unsigned char* base = sm + (size_t)s * kUStageBytes;
       u_mbar_wait(full_raw + s, (uint32_t)(it / kUStages) & 1u);
-      auto split = [](const float4* src, float4* dst, int n4, int t0) {
+      auto rna = [](float x) {                               // x rounded to TF32 (round to nearest, ties away), as an FP32 value
+        uint32_t r;
+        asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(x));
+        return __uint_as_float(r);
+      };
+      auto split = [&](float4* src, float4* dst, int n4, int t0) {     // src <- hi = tf32(x), dst <- lo = x - hi (exact)
         for (int e = t0; e < n4; e += 32 * kUSplitWarps) {
           const float4 x = src[e];
-          float4 l;
-          l.x = x.x - __uint_as_float(__float_as_uint(x.x) & 0xffffe000u);
-          l.y = x.y - __uint_as_float(__float_as_uint(x.y) & 0xffffe000u);
-          l.z = x.z - __uint_as_float(__float_as_uint(x.z) & 0xffffe000u);
-          l.w = x.w - __uint_as_float(__float_as_uint(x.w) & 0xffffe000u);
+          float4 hv, l;
+          hv.x = rna(x.x); hv.y = rna(x.y); hv.z = rna(x.z); hv.w = rna(x.w);
+          l.x = x.x - hv.x; l.y = x.y - hv.y; l.z = x.z - hv.z; l.w = x.w - hv.w;
+          src[e] = hv;
           dst[e] = l;
         }
       };
-      split(reinterpret_cast<const float4*>(base), reinterpret_cast<float4*>(base + kUABytes), kUABytes / 16, st);
-      split(reinterpret_cast<const float4*>(base + 2 * kUABytes), reinterpret_cast<float4*>(base + 2 * kUABytes + kUBBytes),
+      split(reinterpret_cast<float4*>(base), reinterpret_cast<float4*>(base + kUABytes), kUABytes / 16, st);
+      split(reinterpret_cast<float4*>(base + 2 * kUABytes), reinterpret_cast<float4*>(base + 2 * kUABytes + kUBBytes),
             kUBBytes / 16, st);
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic writes of the lo tiles before the tensor core reads them
       __syncwarp();
@@ -209,9 +233,13 @@ __global__ void __launch_bounds__(kUThreads, 1) k_xty_umma(const __grid_constant
         unsigned char* base = sm + (size_t)s * kUStageBytes;
         u_mbar_wait(empty + s, ((uint32_t)(it / kUStages) & 1u) ^ 1u);
         u_mbar_expect_tx(full_raw + s, (uint32_t)(kUABytes + kUBBytes));
-        const int r0 = (int)(g0 + (int64_t)it * kUK);
+        const int r0 = XZ ? it * kUK : (int)(g0 + (int64_t)it * kUK);             // first contraction index of the stage
+        if (XZ) {
+          u_tma_load(base, &tmA, r0, (int)g0, full_raw + s);                     // 128 rows x 32 contraction indices (K-major)
+        } else {
 #pragma unroll
-        for (int m = 0; m < kUM / 32; ++m) u_tma_load(base + m * 4096, &tmA, i0 + 32 * m, r0, full_raw + s);
+          for (int m = 0; m < kUM / 32; ++m) u_tma_load(base + m * 4096, &tmA, i0 + 32 * m, r0, full_raw + s);
+        }
 #pragma unroll
         for (int m = 0; m < kUN / 32; ++m) u_tma_load(base + 2 * kUABytes + m * 4096, &tmB, j0 + 32 * m, r0, full_raw + s);
       }
@@ -229,12 +257,14 @@ __global__ void __launch_bounds__(kUThreads, 1) k_xty_umma(const __grid_constant
         const uint32_t d = tmem + (uint32_t)(a * kUN);
 #pragma unroll
         for (int ka = 0; ka < kUK / 8; ++ka) {
-          const uint64_t ahi = u_desc(sbase + ka * 1024, 4096, 512), alo = u_desc(sbase + kUABytes + ka * 1024, 4096, 512);
+          // A: MN-major atoms (X^T Y), or K-major rows of 128 bytes in 8-row groups of 1024 bytes, 32 bytes per k-step (Y Z)
+          const uint64_t ahi = XZ ? u_desc(sbase + ka * 32, 16, 1024, 2) : u_desc(sbase + ka * 1024, 4096, 512);
+          const uint64_t alo = XZ ? u_desc(sbase + kUABytes + ka * 32, 16, 1024, 2) : u_desc(sbase + kUABytes + ka * 1024, 4096, 512);
           const uint64_t bhi = u_desc(sbase + 2 * kUABytes + ka * 1024, 4096, 512);
           const uint64_t blo = u_desc(sbase + 2 * kUABytes + kUBBytes + ka * 1024, 4096, 512);
-          u_mma(d, ahi, blo, (ka > 0 || !first) ? 1u : 0u);
-          u_mma(d, alo, bhi, 1u);
-          u_mma(d, ahi, bhi, 1u);
+          u_mma(d, ahi, blo, (ka > 0 || !first) ? 1u : 0u, u_idesc(!XZ));
+          u_mma(d, alo, bhi, 1u, u_idesc(!XZ));
+          u_mma(d, ahi, bhi, 1u, u_idesc(!XZ));
         }
         u_commit(empty + s);          // the stage may be refilled once these MMAs have read it
         if (last) u_commit(acc_full + a);   // ... and the accumulator holds the sum of the chain
@@ -261,21 +291,25 @@ UEncodeFn u_encode_fn() {
   return fn;
 }
 // FP32 block [rows][ld] restricted to `cols` columns; box = 32 columns x 32 rows, 128-byte swizzle, zero fill outside
-bool u_make_map(CUtensorMap* tm, const float* base, int64_t rows, int64_t cols, int64_t ld) {
+// (k_major: box = 32 columns x 128 rows in the plain 128-byte swizzle: the K-major A operand of the Y Z product)
+bool u_make_map(CUtensorMap* tm, const float* base, int64_t rows, int64_t cols, int64_t ld, bool k_major = false) {
   UEncodeFn enc = u_encode_fn();
   if (!enc || rows < 1 || cols < 1 || (ld * 4) % 16 != 0 || (uintptr_t)base % 16 != 0) return false;
   const cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
   const cuuint64_t strides[1] = {(cuuint64_t)ld * 4};
-  const cuuint32_t box[2] = {32, (cuuint32_t)kUK};
+  const cuuint32_t box[2] = {32, (cuuint32_t)(k_major ? kUM : kUK)};
   const cuuint32_t estr[2] = {1, 1};
   return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-             CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+             k_major ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 }  // namespace
 
 cudaError_t init_umma_kernels() {
-  return cudaFuncSetAttribute(k_xty_umma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kUSmemBytes);
+  cudaError_t e = cudaFuncSetAttribute(k_umma<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kUSmemBytes);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(k_umma<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kUSmemBytes);
 }
 
 // Cpart[z][N1][N2] (FP64) = per-split sums of A^T B; returns false when the tensor maps cannot be built (caller falls back)
@@ -284,7 +318,18 @@ bool launch_xty_umma(const float* A, int64_t lda, const float* B, int64_t ldb, i
   CUtensorMap tmA, tmB;
   if (!u_make_map(&tmA, A, n_rows, N1, lda) || !u_make_map(&tmB, B, n_rows, N2, ldb)) return false;
   dim3 grid((unsigned)((N1 + kUM - 1) / kUM), (unsigned)((N2 + kUN - 1) / kUN), (unsigned)n_split);
-  k_xty_umma<<<grid, kUThreads, kUSmemBytes, st>>>(tmA, tmB, n_rows, N1, N2, rows_per_split, skip_block, row_block0, col_block0, Cpart);
+  k_umma<false><<<grid, kUThreads, kUSmemBytes, st>>>(tmA, tmB, n_rows, N1, N2, rows_per_split, skip_block, row_block0, col_block0, Cpart,
+                                                      nullptr, 0, nullptr, 0);
+  return true;
+}
+
+// Out[g][j] = sum_i Y32[g][i] Z32[i][j] (3xTF32) + Y[g][j] zd[j] (FP64), g < n_rows, i < N, j < N2; false: no tensor maps
+bool launch_xz_umma(const float* Y32, int64_t ldy32, const float* Z32, int64_t ldz32, const double* Y, int64_t ldy, const double* zd,
+                    int64_t n_rows, int N, int N2, double* Out, int64_t ldo, cudaStream_t st) {
+  CUtensorMap tmA, tmB;
+  if (!u_make_map(&tmA, Y32, n_rows, N, ldy32, true) || !u_make_map(&tmB, Z32, N, N2, ldz32)) return false;
+  dim3 grid((unsigned)((N2 + kUN - 1) / kUN), (unsigned)((n_rows + kUM - 1) / kUM));
+  k_umma<true><<<grid, kUThreads, kUSmemBytes, st>>>(tmA, tmB, n_rows, N, N2, 0, 0, 0, 0, Out, Y, ldy, zd, ldo);
   return true;
 }
 
