@@ -540,6 +540,37 @@ def test_cholesky_and_inverse_on_the_device_match_the_oracle():
     op.close()
 
 
+@pytest.mark.parametrize("N,blk", [(200, 40), (256, 64), (72, 24)])
+def test_tcgen05_and_mma_sync_kernels_of_the_fp32_blocks_agree(N, blk):
+    """The FP32 blocks of the mixed products run on tcgen05 (rr variant 1, csrc/rr_umma.cu: TMA + TMEM, MN-major TF32 operands)
+    or on mma.sync (variant 2): both are 3xTF32 products with FP64 totals, so both sit within 8 eps_FP32 of the FP64 product
+    (relative to the norm products) and within that of each other; each is deterministic.  Sizes span several 128 x 64 tiles,
+    ragged N, a ragged last 32-row stage (5,832 rows) and several row splits."""
+    torch, orc, Operator, _, _, _, _ = _imports()
+    wl, *_ = oracle_case("p6_nonlocal_ragged")
+    op = Operator.from_workload(wl)
+    eps32 = float(np.finfo(np.float32).eps)
+    g = torch.Generator(device="cuda")
+    g.manual_seed(N)
+    Y = torch.randn((wl.n_dofs, N), dtype=torch.float64, device="cuda", generator=g)
+    Z = torch.randn((N, N), dtype=torch.float64, device="cuda", generator=g).triu()
+    S64, P64 = Y.T @ Y, Y @ Z
+    nrm = Y.norm(dim=0)
+    s_scale, p_scale = torch.outer(nrm, nrm), torch.outer(Y.norm(dim=1), Z.norm(dim=0))
+    res = {}
+    for variant in (1, 2):
+        op.set_rr_variant(variant)
+        S, P = op.overlap_matrix_mixed(Y, blk), op.subspace_transform_mixed(Y, Z)
+        assert torch.equal(S, op.overlap_matrix_mixed(Y, blk)) and torch.equal(P, op.subspace_transform_mixed(Y, Z))
+        assert float(((S - S64).abs() / s_scale).max()) <= 8 * eps32, variant
+        assert float(((P - P64).abs() / p_scale).max()) <= 8 * eps32, variant
+        res[variant] = (S, P)
+    assert float(((res[1][0] - res[2][0]).abs() / s_scale).max()) <= 8 * eps32
+    assert float(((res[1][1] - res[2][1]).abs() / p_scale).max()) <= 8 * eps32
+    assert not torch.equal(res[1][0], res[2][0])                 # two different kernels did run
+    op.close()
+
+
 def test_mixed_precision_rayleigh_ritz_products_match_the_oracle():
     """The paper's mixed-precision blocking (Eq. 38-39) against the oracle's plain
     statement of it: FP64 blocks agree at the FP64 level, FP32 blocks agree with the oracle's FP32 products and with the
