@@ -203,11 +203,9 @@ __global__ void __launch_bounds__(kUThreads, 1) k_umma(const __grid_constant__ C
       const int s = it % kUStages;
       unsigned char* base = sm + (size_t)s * kUStageBytes;
       u_mbar_wait(full_raw + s, (uint32_t)(it / kUStages) & 1u);
-      auto rna = [](float x) {                               // x rounded to TF32 (round to nearest, ties away), as an FP32 value
-        uint32_t r;
-        asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(x));
-        return __uint_as_float(r);
-      };
+      // x rounded to TF32 (round to nearest, ties away from zero) as an FP32 value: integer add + mask on the bit pattern
+      // (full-rate ALU instructions; cvt.rna.tf32.f32 runs on the slow conversion pipe and made these warps the bottleneck)
+      auto rna = [](float x) { return __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xffffe000u); };
       auto split = [&](float4* src, float4* dst, int n4, int t0) {     // src <- hi = tf32(x), dst <- lo = x - hi (exact)
         for (int e = t0; e < n4; e += 32 * kUSplitWarps) {
           const float4 x = src[e];
