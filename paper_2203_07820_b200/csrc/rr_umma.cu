@@ -3,7 +3,7 @@
 // PAPER.md:564 "FP32 off-diagonal blocks").  Drop-in for k_xty_tf32 (rr_kernels.cu): same tiles (128 x 64), same split-row
 // partial sums Cpart[z][N1][N2] in FP64, same masked reduction.
 //
-//   * an FP32 product is a 3xTF32 split, a b ~ a_hi b_lo + a_lo b_hi + a_hi b_hi: hi = x rounded to TF32 (cvt.rna), lo = x - hi
+//   * an FP32 product is a 3xTF32 split, a b ~ a_hi b_lo + a_lo b_hi + a_hi b_hi: hi = x rounded to TF32 (nearest; integer add + mask), lo = x - hi
 //     (exact in FP32), both computed by four "split" warps from the tile that the TMA has put into shared memory: hi replaces
 //     the tile in place, lo goes to a second tile of the same layout (the swizzle is element-wise transparent);
 //   * both operands are MN-major (the stored layout [rows][columns] has the output index fastest and the contraction
