@@ -31,10 +31,12 @@ constexpr int kWsComputeWarps = 8;
 constexpr int kWsHelperWarps = 4;                 // warp 8: producer; warps 9-11: assemblers
 constexpr int kWsAsmWarps = kWsHelperWarps - 1;
 constexpr int kWsThreads = 32 * (kWsComputeWarps + kWsHelperWarps);
-// registers after setmaxnreg: 256 x 224 + 128 x 56 = 256 x 232 + 128 x 40 = 64,512 = 384 x 168 (the launch allocation).
-// FP64 tiles (one column pair per compute warp) need the faster assembler; FP32 tiles (two pairs per warp) leave it slack.
-template <typename S> __host__ __device__ constexpr int ws_regs_compute() { return sizeof(S) == 8 ? 224 : 232; }
-template <typename S> __host__ __device__ constexpr int ws_regs_helper() { return sizeof(S) == 8 ? 56 : 40; }
+// registers after setmaxnreg: 256 x 216 + 128 x 72 = 256 x 232 + 128 x 40 = 64,512 = 384 x 168 (the launch allocation).
+// FP64 tiles (one column pair per compute warp) need the faster assembler: at 72 registers its two m-tiles in flight are
+// spill-free and the column loop still is at 216 (measured: 224 / 56 -> 216 / 72 +2 % at config 5, 208 / 88 no further gain);
+// FP32 tiles (two pairs per warp) leave the assembler slack.
+template <typename S> __host__ __device__ constexpr int ws_regs_compute() { return sizeof(S) == 8 ? 216 : 232; }
+template <typename S> __host__ __device__ constexpr int ws_regs_helper() { return sizeof(S) == 8 ? 72 : 40; }
 
 // KP = k-point variant: a column pair is one complex column (re, im); ten fields per Gauss point (the last three carry
 // w detJ J^-1 k); no projector data here -- the back-projection C (D P) is k_proj_back's.
