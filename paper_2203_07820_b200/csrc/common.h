@@ -261,6 +261,8 @@ cudaError_t launch_to_f32(Op* op, const double* src, int64_t lds, float* dst, in
 // tcgen05 form of the same product (rr_umma.cu): partial sums of the row splits into Cpart[n_split][N1][N2]; false when the
 // tensor maps cannot be encoded (the caller then runs k_xty_tf32).  init_umma_kernels: per-device kernel attributes.
 cudaError_t init_umma_kernels();
+void umma_xty_plan(int n_sm, int64_t n_rows, int N1, int N2, int skip_block, int row_block0, int col_block0, int* n_split,
+                   int64_t* rows_per_split);          // row splits for launch_xty_umma (rows per split: a multiple of 32)
 bool launch_xty_umma(const float* A, int64_t lda, const float* B, int64_t ldb, int64_t n_rows, int N1, int N2, int n_split,
                      int64_t rows_per_split, int skip_block, int row_block0, int col_block0, double* Cpart, cudaStream_t stream);
 bool launch_xz_umma(const float* Y32, int64_t ldy32, const float* Z32, int64_t ldz32, const double* Y, int64_t ldy, const double* zd,

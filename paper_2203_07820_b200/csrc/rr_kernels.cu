@@ -569,6 +569,8 @@ cudaError_t launch_xty_tf32(Op* op, const float* A, int64_t lda, const float* B,
   int n_split = std::min(ns_max, std::max(1, (3 * cap + tiles - 1) / tiles));
   int64_t rows_per_split = ((n_rows + n_split - 1) / n_split + kT32K - 1) / kT32K * kT32K;
   n_split = (int)((n_rows + rows_per_split - 1) / rows_per_split);
+  if (op->rr_variant != 2)                                   // the tcgen05 kernel has its own tile shape and occupancy
+    umma_xty_plan(op->n_sm, n_rows, N1, N2, skip_block, row_block0, col_block0, &n_split, &rows_per_split);
   const size_t need = (size_t)n_split * N1 * N2 * sizeof(double);
   if (need > op->rr_scratch_bytes) {
     cudaError_t e = cudaStreamSynchronize(st);
@@ -578,8 +580,8 @@ cudaError_t launch_xty_tf32(Op* op, const float* A, int64_t lda, const float* B,
     if ((e = cudaMalloc(&op->rr_scratch, need)) != cudaSuccess) return e;
     op->rr_scratch_bytes = need;
   }
-  dim3 grid((unsigned)ti, (unsigned)tj, (unsigned)n_split);
   // rr_variant 0 / 1: the tcgen05 kernel (rr_umma.cu); 2, or no tensor maps: the mma.sync kernel below.  Same partial sums layout.
+  dim3 grid((unsigned)ti, (unsigned)tj, (unsigned)n_split);
   if (op->rr_variant == 2 ||
       !launch_xty_umma(A, lda, B, ldb, n_rows, N1, N2, n_split, rows_per_split, skip_block, row_block0, col_block0,
                        reinterpret_cast<double*>(op->rr_scratch), st))

@@ -1,7 +1,9 @@
 // C = A^T B of two tall FP32 blocks on the 5th-generation tensor cores (tcgen05.mma kind::tf32, accumulators in TMEM):
 // the FP32 blocks of the paper's mixed-precision Rayleigh-Ritz products (Sec. 3.2 / 4.4.1: Eq. 38-39, PAPER.md:426-440;
-// PAPER.md:564 "FP32 off-diagonal blocks").  Drop-in for k_xty_tf32 (rr_kernels.cu): same tiles (128 x 64), same split-row
-// partial sums Cpart[z][N1][N2] in FP64, same masked reduction.
+// PAPER.md:564 "FP32 off-diagonal blocks").  Drop-in for k_xty_tf32 (rr_kernels.cu): same split-row partial sums
+// Cpart[z][N1][N2] in FP64, same masked reduction; output tiles are 128 x 128 (every MMA reads its operands from shared memory,
+// the split warps read and write the same tiles again: at 128 x 64 the kernel was bound by shared-memory bandwidth at 0.27 of
+// the TF32 peak, a square tile moves a third less per flop).
 //
 //   * an FP32 product is a 3xTF32 split, a b ~ a_hi b_lo + a_lo b_hi + a_hi b_hi: hi = x rounded to TF32 (nearest; integer add + mask), lo = x - hi
 //     (exact in FP32), both computed by four "split" warps from the tile that the TMA has put into shared memory: hi replaces
@@ -9,12 +11,13 @@
 //   * both operands are MN-major (the stored layout [rows][columns] has the output index fastest and the contraction
 //     index = rows).  For MN-major 32-bit operands the tensor core takes ONE shared-memory layout, the 128-byte swizzle with
 //     32-byte atoms (SWIZZLE_128B_BASE32B: atoms of 32 columns x 4 rows), which is what a TMA box {32 columns, 32 rows}
-//     with CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B writes; one tcgen05.mma (M = 128, N = 64, K = 8) consumes two such atoms;
+//     with CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B writes; one tcgen05.mma (M = 128, N = 128, K = 8) consumes two such atoms per 32 columns;
 //   * the FP32 accumulator of the tensor pipe does not round to nearest, so an accumulation chain is kept to TWO 32-row stages
-//     (24 MMAs from zero) in one of two 64-column TMEM buffers; eight epilogue warps drain it (tcgen05.ld), add the chain
-//     sums in FP32 registers with round-to-nearest for 8 chains and then into FP64 totals -- while the next stage's MMAs
+//     (24 MMAs from zero) in one of two 128-column TMEM buffers; eight epilogue warps drain it (tcgen05.ld) and add the chain
+//     sums to FP64 totals in registers (64 per thread: these warps run at 208 registers, setmaxnreg) -- while the next stage's MMAs
 //     run into the other buffer;
-//   * roles: 8 epilogue warps, 4 split warps, 1 TMA producer warp, 1 MMA warp (one elected lane issues); 4-stage ring.
+//   * roles: 8 epilogue warps, 4 split warps, 1 TMA producer warp, 1 MMA warp (one elected lane issues), 2 idle warps that complete
+//     the fourth warpgroup for setmaxnreg; 3-stage ring of 64 KB (hi and lo tiles of A and B).
 #include <cuda.h>
 
 #include <algorithm>
@@ -24,13 +27,13 @@
 namespace chfsi {
 namespace {
 
-constexpr int kUM = 128, kUN = 64, kUK = 32, kUStages = 4;
+constexpr int kUM = 128, kUN = 128, kUK = 32, kUStages = 3;
 constexpr int kUEpiWarps = 8, kUSplitWarps = 4;
-constexpr int kUThreads = 32 * (kUEpiWarps + kUSplitWarps + 2);
-constexpr int kUABytes = kUK * kUM * 4, kUBBytes = kUK * kUN * 4;              // 16 KB, 8 KB
-constexpr int kUStageBytes = 2 * (kUABytes + kUBBytes);                          // hi + lo tiles of A and B: 48 KB
+constexpr int kUThreads = 32 * (kUEpiWarps + kUSplitWarps + 4);                  // + TMA warp, MMA warp, two idle warps (whole warpgroups)
+constexpr int kUABytes = kUK * kUM * 4, kUBBytes = kUK * kUN * 4;              // 16 KB, 16 KB
+constexpr int kUStageBytes = 2 * (kUABytes + kUBBytes);                          // hi + lo tiles of A and B: 64 KB
 constexpr int kUChain = 2;                                                       // stages per accumulation chain in TMEM
-constexpr int kUFlush = 8;                                                       // chains per FP32 -> FP64 flush
+constexpr int kURegsEpi = 208, kURegsOther = 48;                                 // setmaxnreg: 8 x 32 x 208 + 8 x 32 x 48 = 64 K registers
 constexpr size_t kUSmemBytes = (size_t)kUStages * kUStageBytes + 1024 + 256;
 
 __device__ __forceinline__ uint32_t u_smem(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -145,7 +148,7 @@ __global__ void __launch_bounds__(kUThreads, 1) k_umma(const __grid_constant__ C
     for (int a = 0; a < 2; ++a) { u_mbar_init(acc_full + a, 1); u_mbar_init(acc_empty + a, kUEpiWarps); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  if (warp == kUEpiWarps + kUSplitWarps + 1) {                 // the MMA warp owns the tensor memory: two 64-column accumulators
+  if (warp == kUEpiWarps + kUSplitWarps + 1) {                 // the MMA warp owns the tensor memory: two 128-column accumulators
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(u_smem(tmem_slot)), "n"(2 * kUN) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
   }
@@ -156,47 +159,48 @@ __global__ void __launch_bounds__(kUThreads, 1) k_umma(const __grid_constant__ C
 
   if (warp < kUEpiWarps) {
     // ---- epilogue warps: lane quarter q = warp % 4 (rows 32 q + lane of the tile), column half h = warp / 4 --------------
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kURegsEpi));
     const int q = warp & 3, h = warp >> 2;
-    float p32[32];
-    double tot[32];
+    constexpr int kHalf = kUN / 2;                                              // 64 columns per thread, FP64 totals in registers
+    double tot[kHalf];
 #pragma unroll
-    for (int j = 0; j < 32; ++j) { p32[j] = 0.0f; tot[j] = 0.0; }
+    for (int j = 0; j < kHalf; ++j) tot[j] = 0.0;
     const int nchain = (nstage + kUChain - 1) / kUChain;
     for (int it = 0; it < nchain; ++it) {
       const int a = it & 1;
       u_mbar_wait(acc_full + a, (uint32_t)(it >> 1) & 1u);
       asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-      float v[32];
-      u_tmem_ld32(tmem + ((uint32_t)(32 * q) << 16) + (uint32_t)(a * kUN + 32 * h), v);
+#pragma unroll
+      for (int c = 0; c < kHalf / 32; ++c) {
+        float v[32];
+        u_tmem_ld32(tmem + ((uint32_t)(32 * q) << 16) + (uint32_t)(a * kUN + kHalf * h + 32 * c), v);
+#pragma unroll
+        for (int j = 0; j < 32; ++j) tot[32 * c + j] += (double)v[j];           // chain sums (64 rows) are added in FP64
+      }
       asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
       __syncwarp();
       if (lane == 0) u_mbar_arrive(acc_empty + a);
-#pragma unroll
-      for (int j = 0; j < 32; ++j) p32[j] += v[j];                              // round-to-nearest FP32 adds of chain sums
-      if ((it % kUFlush) == kUFlush - 1 || it == nchain - 1) {
-#pragma unroll
-        for (int j = 0; j < 32; ++j) { tot[j] += (double)p32[j]; p32[j] = 0.0f; }
-      }
     }
     if (XZ) {
       const int64_t r = g0 + 32 * q + lane;                                     // Out = FP32 off-diagonal part + FP64 diagonal part
       if (r < n_rows) {
-        double* op_ = Cpart + r * ldo + j0 + 32 * h;
-        const double* yp = Yd + r * ldy + j0 + 32 * h;
+        double* op_ = Cpart + r * ldo + j0 + kHalf * h;
+        const double* yp = Yd + r * ldy + j0 + kHalf * h;
 #pragma unroll
-        for (int j = 0; j < 32; ++j)
-          if (j0 + 32 * h + j < N2) op_[j] = fma(yp[j], zd[j0 + 32 * h + j], tot[j]);
+        for (int j = 0; j < kHalf; ++j)
+          if (j0 + kHalf * h + j < N2) op_[j] = fma(yp[j], zd[j0 + kHalf * h + j], tot[j]);
       }
     } else {
       const int r = i0 + 32 * q + lane;
       if (r < N1) {
-        double* Cp = Cpart + (int64_t)blockIdx.z * N1 * N2 + (int64_t)r * N2 + j0 + 32 * h;
+        double* Cp = Cpart + (int64_t)blockIdx.z * N1 * N2 + (int64_t)r * N2 + j0 + kHalf * h;
 #pragma unroll
-        for (int j = 0; j < 32; ++j)
-          if (j0 + 32 * h + j < N2) Cp[j] = tot[j];
+        for (int j = 0; j < kHalf; ++j)
+          if (j0 + kHalf * h + j < N2) Cp[j] = tot[j];
       }
     }
   } else if (warp < kUEpiWarps + kUSplitWarps) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kURegsOther));
     // ---- split warps: lo = x - tf32(x) for the stage's A and B tiles (same offsets: the swizzle is element-wise transparent) ---
     const int st = tid - 32 * kUEpiWarps;
     for (int it = 0; it < nstage; ++it) {
@@ -223,7 +227,9 @@ __global__ void __launch_bounds__(kUThreads, 1) k_umma(const __grid_constant__ C
       __syncwarp();
       if (lane == 0) u_mbar_arrive(full_split + s);
     }
-  } else if (warp == kUEpiWarps + kUSplitWarps) {
+  } else {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kURegsOther));   // warps 12 .. 15: one warpgroup (TMA, MMA, two idle)
+    if (warp == kUEpiWarps + kUSplitWarps) {
     // ---- TMA producer ---------------------------------------------------------------------------------------------------
     if (lane == 0) {
       for (int it = 0; it < nstage; ++it) {
@@ -242,7 +248,7 @@ __global__ void __launch_bounds__(kUThreads, 1) k_umma(const __grid_constant__ C
         for (int m = 0; m < kUN / 32; ++m) u_tma_load(base + 2 * kUABytes + m * 4096, &tmB, j0 + 32 * m, r0, full_raw + s);
       }
     }
-  } else {
+    } else if (warp == kUEpiWarps + kUSplitWarps + 1) {
     // ---- MMA warp: one lane issues; per stage 4 k-atoms x (hi lo + lo hi + hi hi) from zero into accumulator it & 1 --------
     if (lane == 0) {
       for (int it = 0; it < nstage; ++it) {
@@ -267,6 +273,7 @@ __global__ void __launch_bounds__(kUThreads, 1) k_umma(const __grid_constant__ C
         u_commit(empty + s);          // the stage may be refilled once these MMAs have read it
         if (last) u_commit(acc_full + a);   // ... and the accumulator holds the sum of the chain
       }
+    }
     }
   }
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -308,6 +315,36 @@ cudaError_t init_umma_kernels() {
   cudaError_t e = cudaFuncSetAttribute(k_umma<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kUSmemBytes);
   if (e != cudaSuccess) return e;
   return cudaFuncSetAttribute(k_umma<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kUSmemBytes);
+}
+
+// Row splits of the X^T Y product for this kernel: one CTA per SM, equal work per CTA, so the split count is the one whose CTA
+// count (tiles that are not skipped x splits) fills its last wave best, among 2 .. 8 waves and >= 2,048 rows per split.
+void umma_xty_plan(int n_sm, int64_t n_rows, int N1, int N2, int skip_block, int row_block0, int col_block0, int* n_split,
+                   int64_t* rows_per_split) {
+  int tiles = 0;
+  for (int i0 = 0; i0 < N1; i0 += kUM)
+    for (int j0 = 0; j0 < N2; j0 += kUN) {
+      bool skip = false;
+      if (skip_block > 0) {
+        const int bi0 = (row_block0 + i0) / skip_block, bi1 = (row_block0 + std::min(i0 + kUM, N1) - 1) / skip_block;
+        const int bj0 = (col_block0 + j0) / skip_block, bj1 = (col_block0 + std::min(j0 + kUN, N2) - 1) / skip_block;
+        skip = bi0 == bi1 && bj0 == bj1 && bi0 == bj0;
+      }
+      tiles += skip ? 0 : 1;
+    }
+  tiles = std::max(tiles, 1);
+  const int ns_max = (int)std::max<int64_t>(1, n_rows / 2048);
+  const int ns_lo = std::min(ns_max, std::max(1, (2 * n_sm + tiles - 1) / tiles));
+  const int ns_hi = std::min(ns_max, std::max(ns_lo, 8 * n_sm / tiles));
+  int best_ns = ns_lo;
+  double best = 0.0;
+  for (int ns = ns_lo; ns <= ns_hi; ++ns) {
+    const int64_t ctas = (int64_t)tiles * ns;
+    const double eff = (double)ctas / (double)(((ctas + n_sm - 1) / n_sm) * n_sm);
+    if (eff > best + 1e-9) { best = eff; best_ns = ns; }
+  }
+  *rows_per_split = ((n_rows + best_ns - 1) / best_ns + kUK - 1) / kUK * kUK;
+  *n_split = (int)((n_rows + *rows_per_split - 1) / *rows_per_split);
 }
 
 // Cpart[z][N1][N2] (FP64) = per-split sums of A^T B; returns false when the tensor maps cannot be built (caller falls back)

@@ -540,11 +540,12 @@ def test_cholesky_and_inverse_on_the_device_match_the_oracle():
     op.close()
 
 
-@pytest.mark.parametrize("N,blk", [(200, 40), (256, 64), (72, 24)])
+@pytest.mark.parametrize("N,blk", [(200, 40), (256, 64), (72, 24), (384, 128)])
 def test_tcgen05_and_mma_sync_kernels_of_the_fp32_blocks_agree(N, blk):
     """The FP32 blocks of the mixed products run on tcgen05 (rr variant 1, csrc/rr_umma.cu: TMA + TMEM, MN-major TF32 operands)
     or on mma.sync (variant 2): both are 3xTF32 products with FP64 totals, so both sit within 8 eps_FP32 of the FP64 product
-    (relative to the norm products) and within that of each other; each is deterministic.  Sizes span several 128 x 64 tiles,
+    (relative to the norm products) and within that of each other; each is deterministic.  Sizes span several 128 x 128 tiles
+    (384 with block 128: tiles inside a diagonal block are skipped),
     ragged N, a ragged last 32-row stage (5,832 rows) and several row splits."""
     torch, orc, Operator, _, _, _, _ = _imports()
     wl, *_ = oracle_case("p6_nonlocal_ragged")
