@@ -183,8 +183,10 @@ int chfsi_chebyshev_filter_host(chfsi_op* op, void* X_host, int64_t ldx, int64_t
  * S_dev / H_dev are DEVICE arrays [N][N], row-major, FP64, owned by the caller.  N, ldy and B must be even and the
  * pointers 16-byte aligned (CHFSI_ERR_UNSUPPORTED otherwise).  workspace_dev: chfsi_workspace_bytes(op, min(B, N)).
  * Work is enqueued on cuda_stream; the row-split partial sums live in a library-owned scratch buffer that grows on
- * demand (the call then synchronises the stream once).  Both matrices are computed in full (symmetric up to rounding:
- * H^ is not symmetrised).  The Cholesky / eigen-decomposition of step 2 is left to the caller (N x N, dense). */
+ * demand (the call then synchronises the stream once).  Both matrices are Hermitian and only their lower triangle is
+ * computed (tiles strictly above the diagonal are skipped; for H^ chunk j0 gives the rows >= j0 of its columns);
+ * the entries above the diagonal are copies, [r][c] = [c][r], so both triangles are valid and the result is exactly
+ * symmetric.  The Cholesky / eigen-decomposition of step 2 is left to the caller (N x N, dense). */
 int chfsi_overlap_matrix(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N, double* S_dev, void* cuda_stream);
 int chfsi_projected_hamiltonian(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N, int64_t B, double* H_dev,
                                 void* workspace_dev, void* cuda_stream);
@@ -219,7 +221,8 @@ int chfsi_cholesky_inverse(chfsi_op* op, const double* S_dev, int64_t N, double*
  *                                      the rest): the fr-fr block FP64, the oc-oc, oc-fr and fr-oc blocks FP32 (Eq. 39)
  *   chfsi_subspace_transform_mixed:    Out = SP[Y Z_od] + DP[Y Z_d] for a square Z [N][ldz] (Z = L^-T gives Psi^o,
  *                                      RRGEP-ST-O): off-diagonal entries of Z FP32, diagonal entries FP64
- * Other arguments as in the FP64 calls above. */
+ * Other arguments as in the FP64 calls above; S and H^ are again computed as lower triangles and mirrored (exactly
+ * symmetric; the FP32 oc-fr block is the mirror of the fr-oc block). */
 int chfsi_overlap_matrix_mixed(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N, int64_t block, double* S_dev,
                                void* cuda_stream);
 int chfsi_projected_hamiltonian_mixed(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N, int64_t B, int64_t n_oc,

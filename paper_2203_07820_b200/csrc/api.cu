@@ -717,7 +717,9 @@ int chfsi_overlap_matrix(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N
   const double* Y = reinterpret_cast<const double*>(Y_dev);
   cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
   cudaError_t ce = order_enter(op, st);
-  if (ce == cudaSuccess) ce = launch_xty(op, Y, ldy, Y, ldy, op->n_dofs, (int)N, (int)N, S_dev, N, st);
+  // S is Hermitian: lower triangle computed, upper mirrored
+  if (ce == cudaSuccess) ce = launch_xty(op, Y, ldy, Y, ldy, op->n_dofs, (int)N, (int)N, S_dev, N, st, 1);
+  if (ce == cudaSuccess) ce = launch_mirror_lower(op, S_dev, (int)N, N, st);
   if (ce == cudaSuccess) ce = order_leave(op, st);
   return ce == cudaSuccess ? CHFSI_OK : cuda_fail(op, ce, "overlap_matrix");
   API_CATCH(op)
@@ -750,12 +752,14 @@ int chfsi_projected_hamiltonian(chfsi_op* op, const void* Y_dev, int64_t ldy, in
     g.sync = reinterpret_cast<unsigned long long*>(base + w.sync_off); g.epoch = 1;
     cudaError_t ce = cudaMemsetAsync(g.sync, 0, w.sync_bytes, st);
     if (ce == cudaSuccess) { op->launches++; ce = launch_apply(op, g, st); }
-    // H^[:, j0 : j0 + bw] = Y^T W
-    if (ce == cudaSuccess) ce = launch_xty(op, Y, ldy, W, w.ldw, op->n_dofs, (int)N, (int)bw, H_dev + j0, N, st);
+    // H^[j0 :, j0 : j0 + bw] = Y[:, j0 :]^T W: the rows from the chunk's diagonal block down (H^ is Hermitian)
+    if (ce == cudaSuccess)
+      ce = launch_xty(op, Y + j0, ldy, W, w.ldw, op->n_dofs, (int)(N - j0), (int)bw, H_dev + j0 * N + j0, N, st, 1);
     if (ce != cudaSuccess) return cuda_fail(op, ce, "projected_hamiltonian");
   }
   {
-    cudaError_t ce1 = order_leave(op, st);
+    cudaError_t ce1 = launch_mirror_lower(op, H_dev, (int)N, N, st);
+    if (ce1 == cudaSuccess) ce1 = order_leave(op, st);
     if (ce1 != cudaSuccess) return cuda_fail(op, ce1, "projected_hamiltonian");
   }
   return CHFSI_OK;
@@ -831,11 +835,13 @@ int chfsi_overlap_matrix_mixed(chfsi_op* op, const void* Y_dev, int64_t ldy, int
   float* Y32 = reinterpret_cast<float*>(op->rr32[0]);
   if (ce == cudaSuccess) ce = launch_to_f32(op, Y, ldy, Y32, ld32, op->n_dofs, (int)N, 0, nullptr, st);
   // FP32 blocks first (tiles inside a diagonal block are skipped), then the FP64 diagonal blocks on top
-  if (ce == cudaSuccess) ce = launch_xty_tf32(op, Y32, ld32, Y32, ld32, op->n_dofs, (int)N, (int)N, (int)block, 0, 0, S_dev, N, st);
+  // (lower triangle only, mirrored at the end: PAPER.md:558)
+  if (ce == cudaSuccess) ce = launch_xty_tf32(op, Y32, ld32, Y32, ld32, op->n_dofs, (int)N, (int)N, (int)block, 0, 0, S_dev, N, st, 1);
   for (int64_t j0 = 0; j0 < N && ce == cudaSuccess; j0 += block) {
     const int bw = (int)std::min(block, N - j0);
-    ce = launch_xty(op, Y + j0, ldy, Y + j0, ldy, op->n_dofs, bw, bw, S_dev + j0 * N + j0, N, st);
+    ce = launch_xty(op, Y + j0, ldy, Y + j0, ldy, op->n_dofs, bw, bw, S_dev + j0 * N + j0, N, st, 1);
   }
+  if (ce == cudaSuccess) ce = launch_mirror_lower(op, S_dev, (int)N, N, st);
   if (ce == cudaSuccess) ce = order_leave(op, st);
   return ce == cudaSuccess ? CHFSI_OK : cuda_fail(op, ce, "overlap_matrix_mixed");
   API_CATCH(op)
@@ -874,13 +880,18 @@ int chfsi_projected_hamiltonian_mixed(chfsi_op* op, const void* Y_dev, int64_t l
     if (ce == cudaSuccess) { op->launches++; ce = launch_apply(op, g, st); }
     // Eq. 39: all rows of these columns as FP32 products ...
     if (ce == cudaSuccess) ce = launch_to_f32(op, W, w.ldw, W32, ldw32, op->n_dofs, (int)bw, 0, nullptr, st);
-    if (ce == cudaSuccess) ce = launch_xty_tf32(op, Y32, ld32, W32, ldw32, op->n_dofs, (int)N, (int)bw, 0, 0, 0, H_dev + j0, N, st);
+    // (rows from the chunk's diagonal block down: H^ is Hermitian; the first row is rounded down to a multiple
+    // of 4 for the 16-byte alignment of the FP32 operand, so up to two rows above the diagonal block are computed as well)
+    const int64_t r0 = j0 / 4 * 4;
+    if (ce == cudaSuccess)
+      ce = launch_xty_tf32(op, Y32 + r0, ld32, W32, ldw32, op->n_dofs, (int)(N - r0), (int)bw, 0, 0, 0, H_dev + r0 * N + j0, N, st, 1);
     // ... and the fr-fr part (rows and columns >= n_oc) in FP64 on top
     const int64_t c0 = std::max(j0, n_oc);
     if (ce == cudaSuccess && c0 < j0 + bw && n_oc < N)
-      ce = launch_xty(op, Y + n_oc, ldy, W + (c0 - j0), w.ldw, op->n_dofs, (int)(N - n_oc), (int)(j0 + bw - c0),
-                      H_dev + n_oc * N + c0, N, st);
+      ce = launch_xty(op, Y + c0, ldy, W + (c0 - j0), w.ldw, op->n_dofs, (int)(N - c0), (int)(j0 + bw - c0),
+                      H_dev + c0 * N + c0, N, st, 1);
   }
+  if (ce == cudaSuccess) ce = launch_mirror_lower(op, H_dev, (int)N, N, st);
   if (ce == cudaSuccess) ce = order_leave(op, st);
   return ce == cudaSuccess ? CHFSI_OK : cuda_fail(op, ce, "projected_hamiltonian_mixed");
   API_CATCH(op)

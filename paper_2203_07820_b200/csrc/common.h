@@ -246,8 +246,11 @@ cudaError_t assemble_projector_rows_imag(Op* op, const HostPlan& plan, const chf
 cudaError_t capture_diagonal(Op* op, cudaStream_t stream);
 // C[N1][ldc] = A^T B over n_rows rows of two FP64 blocks [n_rows][ld] (Alg. 2 step 1); enqueued on
 // the stream; may grow op->rr_scratch (then it synchronises the stream once).
+// lower != 0: the result is the lower triangle (r >= c, local indices) of a Hermitian matrix: tiles strictly above the diagonal
+// are not computed and entries above it are not written; launch_mirror_lower then fills C[r][c] = C[c][r], c > r.
 cudaError_t launch_xty(Op* op, const double* A, int64_t lda, const double* B, int64_t ldb, int64_t n_rows, int N1, int N2,
-                       double* C, int64_t ldc, cudaStream_t stream);
+                       double* C, int64_t ldc, cudaStream_t stream, int lower = 0);
+cudaError_t launch_mirror_lower(Op* op, double* C, int N, int64_t ldc, cudaStream_t stream);
 // Out[n_rows][ldo] = Y Z, Y [n_rows][ldy] with N columns, Z [N][ldz] with N2 columns (Alg. 2 step 3)
 cudaError_t launch_xz(Op* op, const double* Y, int64_t ldy, const double* Z, int64_t ldz, int64_t n_rows, int N, int N2,
                       double* Out, int64_t ldo, cudaStream_t stream);
@@ -261,14 +264,15 @@ cudaError_t launch_to_f32(Op* op, const double* src, int64_t lds, float* dst, in
 // tcgen05 form of the same product (rr_umma.cu): partial sums of the row splits into Cpart[n_split][N1][N2]; false when the
 // tensor maps cannot be encoded (the caller then runs k_xty_tf32).  init_umma_kernels: per-device kernel attributes.
 cudaError_t init_umma_kernels();
-void umma_xty_plan(int n_sm, int64_t n_rows, int N1, int N2, int skip_block, int row_block0, int col_block0, int* n_split,
-                   int64_t* rows_per_split);          // row splits for launch_xty_umma (rows per split: a multiple of 32)
+void umma_xty_plan(int n_sm, int64_t n_rows, int N1, int N2, int skip_block, int row_block0, int col_block0, int lower,
+                   int* n_split, int64_t* rows_per_split);          // row splits for launch_xty_umma (rows per split: a multiple of 32)
 bool launch_xty_umma(const float* A, int64_t lda, const float* B, int64_t ldb, int64_t n_rows, int N1, int N2, int n_split,
-                     int64_t rows_per_split, int skip_block, int row_block0, int col_block0, double* Cpart, cudaStream_t stream);
+                     int64_t rows_per_split, int skip_block, int row_block0, int col_block0, int lower, double* Cpart,
+                     cudaStream_t stream);
 bool launch_xz_umma(const float* Y32, int64_t ldy32, const float* Z32, int64_t ldz32, const double* Y, int64_t ldy, const double* zd,
                     int64_t n_rows, int N, int N2, double* Out, int64_t ldo, cudaStream_t stream);
 cudaError_t launch_xty_tf32(Op* op, const float* A, int64_t lda, const float* B, int64_t ldb, int64_t n_rows, int N1, int N2,
-                            int skip_block, int row_block0, int col_block0, double* C, int64_t ldc, cudaStream_t st);
+                            int skip_block, int row_block0, int col_block0, double* C, int64_t ldc, cudaStream_t st, int lower = 0);
 cudaError_t launch_xz_tf32(Op* op, const float* Y32, int64_t ldy32, const float* Z32, int64_t ldz32, const double* Y, int64_t ldy,
                            const double* zd, int64_t n_rows, int N, int N2, double* Out, int64_t ldo, cudaStream_t st);
 // Cholesky factor and its inverse of an N x N FP64 matrix on the device (rr_dense.cu; Alg. 2 step 2a)

@@ -31,13 +31,14 @@ __device__ __forceinline__ void cp_async16_zfill(void* dst, const void* src, int
 }
 
 __global__ void __launch_bounds__(256, 2) k_xty(const double* __restrict__ A, int64_t lda, const double* __restrict__ B,
-                                                int64_t ldb, int64_t n_rows, int N1, int N2, int64_t rows_per_split,
+                                                int64_t ldb, int64_t n_rows, int N1, int N2, int64_t rows_per_split, int lower,
                                                 double* __restrict__ Cpart /*[gridDim.z][N1][N2]*/) {
   extern __shared__ __align__(16) double xs[];
   constexpr int stage_elems = kXtK * kXtLdA + kXtK * kXtLdB;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int wm = warp >> 1, wn = warp & 1, fk = lane & 3, fm = lane >> 2;
   const int i0 = blockIdx.x * kXtM, j0 = blockIdx.y * kXtN;
+  if (lower && j0 > i0 + kXtM - 1) return;              // Hermitian result: tiles strictly above the diagonal are not computed
   const int64_t g0 = (int64_t)blockIdx.z * rows_per_split, g1 = min(n_rows, g0 + rows_per_split);
   const int npanel = (int)((g1 - g0 + kXtK - 1) / kXtK);
 
@@ -106,10 +107,11 @@ __global__ void __launch_bounds__(256, 2) k_xty(const double* __restrict__ A, in
 }
 
 // C[i][j] = sum over the row splits, in split order
-__global__ void __launch_bounds__(256) k_xty_reduce(const double* __restrict__ Cpart, int n_split, int N1, int N2,
+__global__ void __launch_bounds__(256) k_xty_reduce(const double* __restrict__ Cpart, int n_split, int N1, int N2, int lower,
                                                     double* __restrict__ C, int64_t ldc) {
   const int64_t e = (int64_t)blockIdx.x * 256 + threadIdx.x;
   if (e >= (int64_t)N1 * N2) return;
+  if (lower && e % N2 > e / N2) return;                  // above the diagonal: filled by k_mirror_lower
   double s = 0.0;
   for (int k = 0; k < n_split; ++k) s += Cpart[(int64_t)k * N1 * N2 + e];
   C[(e / N2) * ldc + (e % N2)] = s;
@@ -218,12 +220,34 @@ cudaError_t launch_xz(Op* op, const double* Y, int64_t ldy, const double* Z, int
   return cudaGetLastError();
 }
 
+// Tiles of a TM x TN tiling of an N1 x N2 result that a kernel computes when only the lower triangle is wanted
+int lower_tiles(int N1, int N2, int TM, int TN, int lower) {
+  int n = 0;
+  for (int i0 = 0; i0 < N1; i0 += TM)
+    for (int j0 = 0; j0 < N2; j0 += TN) n += (lower && j0 > i0 + TM - 1) ? 0 : 1;
+  return std::max(n, 1);
+}
+
+__global__ void __launch_bounds__(256) k_mirror_lower(double* __restrict__ C, int N, int64_t ldc) {
+  const int64_t e = (int64_t)blockIdx.x * 256 + threadIdx.x;
+  if (e >= (int64_t)N * N) return;
+  const int r = (int)(e / N), c = (int)(e % N);
+  if (c > r) C[(int64_t)r * ldc + c] = C[(int64_t)c * ldc + r];
+}
+
+// C[r][c] <- C[c][r] for c > r (only the lower triangle of the Hermitian S and H^ is computed)
+cudaError_t launch_mirror_lower(Op* op, double* C, int N, int64_t ldc, cudaStream_t st) {
+  k_mirror_lower<<<(unsigned)(((int64_t)N * N + 255) / 256), 256, 0, st>>>(C, N, ldc);
+  op->launches++;
+  return cudaGetLastError();
+}
+
 cudaError_t launch_xty(Op* op, const double* A, int64_t lda, const double* B, int64_t ldb, int64_t n_rows, int N1, int N2,
-                       double* C, int64_t ldc, cudaStream_t st) {
+                       double* C, int64_t ldc, cudaStream_t st, int lower) {
   const int ti = (N1 + kXtM - 1) / kXtM, tj = (N2 + kXtN - 1) / kXtN;
   // Row splits: at least ~3 waves of 2 CTAs per SM and at least 512 rows per split; among the candidates the one
   // whose CTA count fills its last wave best (128 tiles x 7 splits = 3.03 waves would idle a quarter of the GPU).
-  const int cap = 2 * op->n_sm, tiles = ti * tj;
+  const int cap = 2 * op->n_sm, tiles = lower_tiles(N1, N2, kXtM, kXtN, lower);
   const int ns_max = (int)std::max<int64_t>(1, (n_rows + 511) / 512);
   const int ns_lo = std::min(ns_max, std::max(1, (3 * cap + tiles - 1) / tiles));
   int n_split = ns_lo;
@@ -246,9 +270,9 @@ cudaError_t launch_xty(Op* op, const double* A, int64_t lda, const double* B, in
   }
   const size_t smem = xty_smem_bytes();
   dim3 grid((unsigned)ti, (unsigned)tj, (unsigned)n_split);
-  k_xty<<<grid, 256, smem, st>>>(A, lda, B, ldb, n_rows, N1, N2, rows_per_split, reinterpret_cast<double*>(op->rr_scratch));
+  k_xty<<<grid, 256, smem, st>>>(A, lda, B, ldb, n_rows, N1, N2, rows_per_split, lower, reinterpret_cast<double*>(op->rr_scratch));
   k_xty_reduce<<<(unsigned)(((int64_t)N1 * N2 + 255) / 256), 256, 0, st>>>(reinterpret_cast<const double*>(op->rr_scratch), n_split,
-                                                                          N1, N2, C, ldc);
+                                                                          N1, N2, lower, C, ldc);
   op->launches += 2;
   return cudaGetLastError();
 }
@@ -310,7 +334,7 @@ constexpr int kT32LdA = kT32M + 8, kT32LdB = kT32N + 8;       // k-major panels:
 // tiles that lie entirely inside a diagonal block of width `skip_block` (> 0) are skipped: those entries are FP64 products
 __global__ void __launch_bounds__(256, 1) k_xty_tf32(const float* __restrict__ A, int64_t lda, const float* __restrict__ B,
                                                      int64_t ldb, int64_t n_rows, int N1, int N2, int64_t rows_per_split,
-                                                     int skip_block, int row_block0, int col_block0,
+                                                     int skip_block, int row_block0, int col_block0, int lower,
                                                      double* __restrict__ Cpart) {
   extern __shared__ __align__(16) float fs[];
   constexpr int stage_elems = kT32K * kT32LdA + kT32K * kT32LdB;
@@ -318,6 +342,7 @@ __global__ void __launch_bounds__(256, 1) k_xty_tf32(const float* __restrict__ A
   const int wm = warp >> 1, wn = warp & 1, g = lane >> 2, t = lane & 3;
   const int i0 = blockIdx.x * kT32M, j0 = blockIdx.y * kT32N;
   double* Cp = Cpart + (int64_t)blockIdx.z * N1 * N2;
+  if (lower && j0 > i0 + kT32M - 1) return;                     // strictly above the diagonal
   if (skip_block > 0) {
     const int bi0 = (row_block0 + i0) / skip_block, bi1 = (row_block0 + min(i0 + kT32M, N1) - 1) / skip_block;
     const int bj0 = (col_block0 + j0) / skip_block, bj1 = (col_block0 + min(j0 + kT32N, N2) - 1) / skip_block;
@@ -418,11 +443,12 @@ __global__ void __launch_bounds__(256, 1) k_xty_tf32(const float* __restrict__ A
 
 // C[r][c] = sum over splits; entries of tiles skipped above are left untouched (mask by the same rule)
 __global__ void __launch_bounds__(256) k_xty_reduce_masked(const double* __restrict__ Cpart, int n_split, int N1, int N2,
-                                                           int skip_block, int row_block0, int col_block0,
+                                                           int skip_block, int row_block0, int col_block0, int lower,
                                                            double* __restrict__ C, int64_t ldc) {
   const int64_t e = (int64_t)blockIdx.x * 256 + threadIdx.x;
   if (e >= (int64_t)N1 * N2) return;
   const int r = (int)(e / N2), c = (int)(e % N2);
+  if (lower && c > r) return;
   if (skip_block > 0) {
     const int i0 = r / kT32M * kT32M, j0 = c / kT32N * kT32N;
     const int bi0 = (row_block0 + i0) / skip_block, bi1 = (row_block0 + min(i0 + kT32M, N1) - 1) / skip_block;
@@ -562,15 +588,15 @@ cudaError_t launch_to_f32(Op* op, const double* src, int64_t lds, float* dst, in
 }
 
 cudaError_t launch_xty_tf32(Op* op, const float* A, int64_t lda, const float* B, int64_t ldb, int64_t n_rows, int N1, int N2,
-                            int skip_block, int row_block0, int col_block0, double* C, int64_t ldc, cudaStream_t st) {
+                            int skip_block, int row_block0, int col_block0, double* C, int64_t ldc, cudaStream_t st, int lower) {
   const int ti = (N1 + kT32M - 1) / kT32M, tj = (N2 + kT32N - 1) / kT32N;
-  const int cap = 2 * op->n_sm, tiles = ti * tj;
+  const int cap = 2 * op->n_sm, tiles = lower_tiles(N1, N2, kT32M, kT32N, lower);
   const int ns_max = (int)std::max<int64_t>(1, (n_rows + 1023) / 1024);
   int n_split = std::min(ns_max, std::max(1, (3 * cap + tiles - 1) / tiles));
   int64_t rows_per_split = ((n_rows + n_split - 1) / n_split + kT32K - 1) / kT32K * kT32K;
   n_split = (int)((n_rows + rows_per_split - 1) / rows_per_split);
   if (op->rr_variant != 2)                                   // the tcgen05 kernel has its own tile shape and occupancy
-    umma_xty_plan(op->n_sm, n_rows, N1, N2, skip_block, row_block0, col_block0, &n_split, &rows_per_split);
+    umma_xty_plan(op->n_sm, n_rows, N1, N2, skip_block, row_block0, col_block0, lower, &n_split, &rows_per_split);
   const size_t need = (size_t)n_split * N1 * N2 * sizeof(double);
   if (need > op->rr_scratch_bytes) {
     cudaError_t e = cudaStreamSynchronize(st);
@@ -583,12 +609,12 @@ cudaError_t launch_xty_tf32(Op* op, const float* A, int64_t lda, const float* B,
   // rr_variant 0 / 1: the tcgen05 kernel (rr_umma.cu); 2, or no tensor maps: the mma.sync kernel below.  Same partial sums layout.
   dim3 grid((unsigned)ti, (unsigned)tj, (unsigned)n_split);
   if (op->rr_variant == 2 ||
-      !launch_xty_umma(A, lda, B, ldb, n_rows, N1, N2, n_split, rows_per_split, skip_block, row_block0, col_block0,
+      !launch_xty_umma(A, lda, B, ldb, n_rows, N1, N2, n_split, rows_per_split, skip_block, row_block0, col_block0, lower,
                        reinterpret_cast<double*>(op->rr_scratch), st))
     k_xty_tf32<<<grid, 256, xty32_smem_bytes(), st>>>(A, lda, B, ldb, n_rows, N1, N2, rows_per_split, skip_block, row_block0,
-                                                      col_block0, reinterpret_cast<double*>(op->rr_scratch));
+                                                      col_block0, lower, reinterpret_cast<double*>(op->rr_scratch));
   k_xty_reduce_masked<<<(unsigned)(((int64_t)N1 * N2 + 255) / 256), 256, 0, st>>>(
-      reinterpret_cast<const double*>(op->rr_scratch), n_split, N1, N2, skip_block, row_block0, col_block0, C, ldc);
+      reinterpret_cast<const double*>(op->rr_scratch), n_split, N1, N2, skip_block, row_block0, col_block0, lower, C, ldc);
   op->launches += 2;
   return cudaGetLastError();
 }

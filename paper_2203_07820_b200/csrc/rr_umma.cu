@@ -121,9 +121,10 @@ template <bool XZ>
 __global__ void __launch_bounds__(kUThreads, 1) k_umma(const __grid_constant__ CUtensorMap tmA,
                                                        const __grid_constant__ CUtensorMap tmB, int64_t n_rows, int N1, int N2,
                                                        int64_t rows_per_split, int skip_block, int row_block0, int col_block0,
-                                                       double* __restrict__ Cpart, const double* __restrict__ Yd, int64_t ldy,
+                                                       int lower, double* __restrict__ Cpart, const double* __restrict__ Yd, int64_t ldy,
                                                        const double* __restrict__ zd, int64_t ldo) {
   const int i0 = XZ ? 0 : blockIdx.x * kUM, j0 = (XZ ? blockIdx.x : blockIdx.y) * kUN;
+  if (!XZ && lower && j0 > i0 + kUM - 1) return;                      // strictly above the diagonal of a Hermitian result
   if (!XZ && skip_block > 0) {                                        // tiles inside an FP64 diagonal block: not ours (k_xty_tf32's rule)
     const int bi0 = (row_block0 + i0) / skip_block, bi1 = (row_block0 + min(i0 + kUM, N1) - 1) / skip_block;
     const int bj0 = (col_block0 + j0) / skip_block, bj1 = (col_block0 + min(j0 + kUN, N2) - 1) / skip_block;
@@ -319,13 +320,13 @@ cudaError_t init_umma_kernels() {
 
 // Row splits of the X^T Y product for this kernel: one CTA per SM, equal work per CTA, so the split count is the one whose CTA
 // count (tiles that are not skipped x splits) fills its last wave best, among 2 .. 8 waves and >= 2,048 rows per split.
-void umma_xty_plan(int n_sm, int64_t n_rows, int N1, int N2, int skip_block, int row_block0, int col_block0, int* n_split,
-                   int64_t* rows_per_split) {
+void umma_xty_plan(int n_sm, int64_t n_rows, int N1, int N2, int skip_block, int row_block0, int col_block0, int lower,
+                   int* n_split, int64_t* rows_per_split) {
   int tiles = 0;
   for (int i0 = 0; i0 < N1; i0 += kUM)
     for (int j0 = 0; j0 < N2; j0 += kUN) {
-      bool skip = false;
-      if (skip_block > 0) {
+      bool skip = lower && j0 > i0 + kUM - 1;
+      if (!skip && skip_block > 0) {
         const int bi0 = (row_block0 + i0) / skip_block, bi1 = (row_block0 + std::min(i0 + kUM, N1) - 1) / skip_block;
         const int bj0 = (col_block0 + j0) / skip_block, bj1 = (col_block0 + std::min(j0 + kUN, N2) - 1) / skip_block;
         skip = bi0 == bi1 && bj0 == bj1 && bi0 == bj0;
@@ -349,12 +350,13 @@ void umma_xty_plan(int n_sm, int64_t n_rows, int N1, int N2, int skip_block, int
 
 // Cpart[z][N1][N2] (FP64) = per-split sums of A^T B; returns false when the tensor maps cannot be built (caller falls back)
 bool launch_xty_umma(const float* A, int64_t lda, const float* B, int64_t ldb, int64_t n_rows, int N1, int N2, int n_split,
-                     int64_t rows_per_split, int skip_block, int row_block0, int col_block0, double* Cpart, cudaStream_t st) {
+                     int64_t rows_per_split, int skip_block, int row_block0, int col_block0, int lower, double* Cpart,
+                     cudaStream_t st) {
   CUtensorMap tmA, tmB;
   if (!u_make_map(&tmA, A, n_rows, N1, lda) || !u_make_map(&tmB, B, n_rows, N2, ldb)) return false;
   dim3 grid((unsigned)((N1 + kUM - 1) / kUM), (unsigned)((N2 + kUN - 1) / kUN), (unsigned)n_split);
-  k_umma<false><<<grid, kUThreads, kUSmemBytes, st>>>(tmA, tmB, n_rows, N1, N2, rows_per_split, skip_block, row_block0, col_block0, Cpart,
-                                                      nullptr, 0, nullptr, 0);
+  k_umma<false><<<grid, kUThreads, kUSmemBytes, st>>>(tmA, tmB, n_rows, N1, N2, rows_per_split, skip_block, row_block0, col_block0, lower,
+                                                      Cpart, nullptr, 0, nullptr, 0);
   return true;
 }
 
@@ -364,7 +366,7 @@ bool launch_xz_umma(const float* Y32, int64_t ldy32, const float* Z32, int64_t l
   CUtensorMap tmA, tmB;
   if (!u_make_map(&tmA, Y32, n_rows, N, ldy32, true) || !u_make_map(&tmB, Z32, N, N2, ldz32)) return false;
   dim3 grid((unsigned)((N2 + kUN - 1) / kUN), (unsigned)((n_rows + kUM - 1) / kUM));
-  k_umma<true><<<grid, kUThreads, kUSmemBytes, st>>>(tmA, tmB, n_rows, N, N2, 0, 0, 0, 0, Out, Y, ldy, zd, ldo);
+  k_umma<true><<<grid, kUThreads, kUSmemBytes, st>>>(tmA, tmB, n_rows, N, N2, 0, 0, 0, 0, 0, Out, Y, ldy, zd, ldo);
   return true;
 }
 

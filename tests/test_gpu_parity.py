@@ -208,9 +208,11 @@ def test_rayleigh_ritz_projection_matrices_match_the_oracle(name):
     N = Y.shape[1]
     S = op.overlap_matrix(Yd)
     assert torch.equal(S, op.overlap_matrix(Yd))
+    assert torch.equal(S, S.T)                                  # lower triangle computed, upper mirrored
     assert np.max(np.abs(S.cpu().numpy() - So)) <= 1e-12 * np.max(np.abs(So))
     for B in (N, 24 if N > 24 else 16):
         Hh = op.projected_hamiltonian(Yd, B=B).cpu().numpy()
+        assert np.array_equal(Hh, Hh.T)
         assert np.max(np.abs(Hh - Ho)) <= 1e-11 * np.max(np.abs(Ho)), (name, B)
     Ss, Hs = S.cpu().numpy(), 0.5 * (Hh + Hh.T)
     th_g = scipy.linalg.eigh(Hs, 0.5 * (Ss + Ss.T), eigvals_only=True)
@@ -569,6 +571,47 @@ def test_tcgen05_and_mma_sync_kernels_of_the_fp32_blocks_agree(N, blk):
     assert float(((res[1][0] - res[2][0]).abs() / s_scale).max()) <= 8 * eps32
     assert float(((res[1][1] - res[2][1]).abs() / p_scale).max()) <= 8 * eps32
     assert not torch.equal(res[1][0], res[2][0])                 # two different kernels did run
+    op.close()
+
+
+@pytest.mark.parametrize("rr_variant", [1, 2])
+def test_lower_triangle_products_span_several_tiles(rr_variant):
+    """S and H^ are Hermitian and only their lower triangle is computed: tiles strictly above the diagonal are
+    skipped, the upper triangle is a mirror.  N = 328 spans three 128-wide tiles (ragged), chunks of 90 columns start at
+    columns that are not multiples of 4 (the FP32 operand of the mixed H^ then starts up to two rows early) and n_oc = 100
+    splits a chunk.  References: FP64 products of torch on the device (S) and of the library's own H~Y (H^: this test
+    is about the arrangement of the products, the operator itself is compared with the oracle elsewhere)."""
+    torch, orc, Operator, _, _, _, _ = _imports()
+    wl, *_ = oracle_case("p6_nonlocal_ragged")
+    op = Operator.from_workload(wl)
+    op.set_rr_variant(rr_variant)
+    eps32 = float(np.finfo(np.float32).eps)
+    g = torch.Generator(device="cuda")
+    g.manual_seed(7)
+    N, B, n_oc = 328, 90, 100
+    Y = torch.randn((wl.n_dofs, N), dtype=torch.float64, device="cuda", generator=g)
+    W = op.apply_H(Y)
+    S64, H64 = Y.T @ Y, Y.T @ W
+    H64 = 0.5 * (H64 + H64.T)
+    nY, nW = Y.norm(dim=0), W.norm(dim=0)
+    s_scale, h_scale = torch.outer(nY, nY), torch.maximum(torch.outer(nY, nW), torch.outer(nW, nY))
+    S = op.overlap_matrix(Y)
+    assert torch.equal(S, S.T) and float(((S - S64).abs() / s_scale).max()) <= 1e-13
+    for chunk in (B, N, 64):
+        Hh = op.projected_hamiltonian(Y, B=chunk)
+        assert torch.equal(Hh, Hh.T) and float(((Hh - H64).abs() / h_scale).max()) <= 1e-13, chunk
+    Sm = op.overlap_matrix_mixed(Y, 82)
+    assert torch.equal(Sm, Sm.T) and float(((Sm - S64).abs() / s_scale).max()) <= 8 * eps32
+    blocks = torch.zeros((N, N), dtype=torch.bool, device="cuda")
+    for j0 in range(0, N, 82):
+        blocks[j0:j0 + 82, j0:j0 + 82] = True
+    assert float(((Sm - S64).abs() / s_scale)[blocks].max()) <= 1e-13            # diagonal blocks are FP64 products
+    for chunk in (B, N):
+        Hm = op.projected_hamiltonian_mixed(Y, n_oc, B=chunk)
+        err = (Hm - H64).abs() / h_scale
+        assert torch.equal(Hm, Hm.T) and float(err.max()) <= 8 * eps32, chunk
+        assert float(err[n_oc:, n_oc:].max()) <= 1e-13, chunk                   # the fr-fr block is an FP64 product
+        assert float(err[:n_oc, :].max()) > 1e-12                               # the rest ARE FP32 products
     op.close()
 
 
