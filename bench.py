@@ -438,6 +438,9 @@ def run_rr(args):
     ms_sm = timed(lambda: op.overlap_matrix_mixed(Y, blk))
     ms_hm = timed(lambda: op.projected_hamiltonian_mixed(Y, n_oc, B=B, workspace=ws))
     ms_zm = timed(lambda: op.subspace_transform_mixed(Y, Z, Out=Out))
+    Zu = Z.triu()                                             # Z = L^-T of step 3b is upper triangular: zero panels are skipped
+    ms_zu = timed(lambda: op.subspace_transform(Y, Zu, Out=Out))
+    ms_zum = timed(lambda: op.subspace_transform_mixed(Y, Zu, Out=Out))
     Sd = op.overlap_matrix(Y)
     ms_ch = timed(lambda: op.cholesky_inverse(Sd))
     # DHM step of an SCF iteration (chfsi_update_potential, Alg. 1 step 4): host wall clock incl. the H2D copy of the samples
@@ -478,6 +481,10 @@ def run_rr(args):
                               "tflops": (gemm_low + apply_flops) / ms_hm * 1e-9, "speedup_vs_fp64": ms_h / ms_hm},
         "transform_mixed": {"kernel": "k_umma<xz> (tcgen05 kind::tf32, 3xTF32 off-diagonal + FP64 diagonal)", "ms": ms_zm,
                             "tflops": gemm / ms_zm * 1e-9, "speedup_vs_fp64": ms_z / ms_zm},
+        "transform_YZ_upper": {"kernel": "k_xz, upper-triangular Z (detected on the device)", "ms": ms_zu,
+                               "tflops": gemm_low / ms_zu * 1e-9, "frac": gemm_low / ms_zu * 1e-9 / peak},
+        "transform_mixed_upper": {"kernel": "k_umma<xz>, upper-triangular Z", "ms": ms_zum, "tflops": gemm_low / ms_zum * 1e-9,
+                                  "speedup_vs_fp64": ms_zu / ms_zum},
         "cholesky_inverse": {"kernel": "k_chol_* / k_trinv_row (N = 1024)", "ms": ms_ch},
         "update_potential": {"kernel": "k_sf_fields (default: quadrature-point fields only; 17 MB of samples H2D)", "ms": ms_dhm_sf},
         "update_potential_dense": {"kernel": "k_sf_fields + k_cell_matrix (lazy rebuild of the 3.9 GB of dense cell matrices, "

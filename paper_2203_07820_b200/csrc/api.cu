@@ -50,7 +50,7 @@ void free_op(chfsi_op* op) {
   cudaFree(op->color_cells); cudaFree(op->dep_ptr); cudaFree(op->dep_pos); cudaFree(op->all_cells); cudaFree(op->pc_cells); cudaFree(op->cell_proj_ptr);
   cudaFree(op->proj_ptr); cudaFree(op->proj_pcrow); cudaFree(op->seg_ptr); cudaFree(op->grow_dof); cudaFree(op->pcoef);
   cudaFree(op->grp_seg_ptr); cudaFree(op->proj_grp); cudaFree(op->proj_slot);
-  cudaFree(op->rr_scratch); cudaFree(op->rr32[0]); cudaFree(op->rr32[1]); cudaFree(op->sf_coef); cudaFree(op->sf_sloc); cudaFree(op->crows);
+  cudaFree(op->rr_scratch); cudaFree(op->rr_flag); cudaFree(op->rr32[0]); cudaFree(op->rr32[1]); cudaFree(op->sf_coef); cudaFree(op->sf_sloc); cudaFree(op->crows);
   cudaFree(op->pcoef_im); cudaFree(op->seg_slot_proj); cudaFree(op->back_segs); cudaFree(op->veff_dev);
   for (int i = 0; i < 2; ++i) {
     cudaFree(op->host_stage[i]);

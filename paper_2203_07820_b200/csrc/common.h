@@ -158,6 +158,7 @@ struct Op {
   double* setup_gw = nullptr;            // [nq1]
   // split-row partial tiles of the Rayleigh-Ritz projection products (rr_kernels.cu); grown on demand
   void* rr_scratch = nullptr;
+  int* rr_flag = nullptr;             // device word: != 0 when the Z of the current Y Z product has a nonzero below its diagonal
   size_t rr_scratch_bytes = 0;
   // FP32 copies of the blocks of the mixed-precision Rayleigh-Ritz products; grown on demand
   void* rr32[2] = {nullptr, nullptr};
@@ -270,7 +271,7 @@ bool launch_xty_umma(const float* A, int64_t lda, const float* B, int64_t ldb, i
                      int64_t rows_per_split, int skip_block, int row_block0, int col_block0, int lower, double* Cpart,
                      cudaStream_t stream);
 bool launch_xz_umma(const float* Y32, int64_t ldy32, const float* Z32, int64_t ldz32, const double* Y, int64_t ldy, const double* zd,
-                    int64_t n_rows, int N, int N2, double* Out, int64_t ldo, cudaStream_t stream);
+                    int64_t n_rows, int N, int N2, double* Out, int64_t ldo, const int* lower_nonzero, cudaStream_t stream);
 cudaError_t launch_xty_tf32(Op* op, const float* A, int64_t lda, const float* B, int64_t ldb, int64_t n_rows, int N1, int N2,
                             int skip_block, int row_block0, int col_block0, double* C, int64_t ldc, cudaStream_t st, int lower = 0);
 cudaError_t launch_xz_tf32(Op* op, const float* Y32, int64_t ldy32, const float* Z32, int64_t ldz32, const double* Y, int64_t ldy,

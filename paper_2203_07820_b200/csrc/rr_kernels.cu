@@ -123,19 +123,44 @@ __global__ void __launch_bounds__(256) k_xty_reduce(const double* __restrict__ C
 // Rows are independent, so there is no reduction across CTAs: CTA tile = 128 rows x 64 columns, K = N streamed in
 // 32-column panels of Y / 32-row panels of Z through a 2-stage cp.async ring; 8 warps as 4 x 2, 4 x 4 DMMA tiles each.
 // ---------------------------------------------------------------------------------------------------------------
+// *flag |= 1 when Z [N][ld] (N2 columns) has a nonzero entry below its diagonal (row i > column j)
+template <typename T>
+__global__ void __launch_bounds__(256) k_lower_nonzero(const T* __restrict__ Z, int64_t ld, int N, int N2, int* __restrict__ flag) {
+  const int64_t e = (int64_t)blockIdx.x * 256 + threadIdx.x;
+  bool nz = false;
+  if (e < (int64_t)N * N2) {
+    const int i = (int)(e / N2), j = (int)(e % N2);
+    nz = i > j && Z[(int64_t)i * ld + j] != T(0);
+  }
+  if (__syncthreads_or(nz) && threadIdx.x == 0) atomicOr(flag, 1);
+}
+template <typename T>
+cudaError_t detect_lower_nonzero(Op* op, const T* Z, int64_t ld, int N, int N2, cudaStream_t st) {
+  if (!op->rr_flag) {
+    cudaError_t e = cudaMalloc(&op->rr_flag, sizeof(int));
+    if (e != cudaSuccess) return e;
+  }
+  cudaError_t e = cudaMemsetAsync(op->rr_flag, 0, sizeof(int), st);
+  if (e != cudaSuccess) return e;
+  k_lower_nonzero<T><<<(unsigned)(((int64_t)N * N2 + 255) / 256), 256, 0, st>>>(Z, ld, N, N2, op->rr_flag);
+  return cudaGetLastError();
+}
+
 constexpr int kXzM = 128, kXzN = 64, kXzK = 32;
 constexpr int kXzLdA = kXzK + 4, kXzLdB = kXzN + 4;   // 36, 68: pitch mod 16 == 4
 
 __global__ void __launch_bounds__(256, 2) k_xz(const double* __restrict__ Y, int64_t ldy, const double* __restrict__ Z,
                                                int64_t ldz, int64_t n_rows, int N, int N2, double* __restrict__ Out,
-                                               int64_t ldo) {
+                                               int64_t ldo, const int* __restrict__ lower_nonzero) {
   extern __shared__ __align__(16) double xs[];
   constexpr int stage_elems = kXzM * kXzLdA + kXzK * kXzLdB;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int wm = warp >> 1, wn = warp & 1, fk = lane & 3, fm = lane >> 2;
   const int j0 = blockIdx.x * kXzN;
   const int64_t g0 = (int64_t)blockIdx.y * kXzM;
-  const int npanel = (N + kXzK - 1) / kXzK;
+  // upper-triangular Z (Z = L^-T of step 3b): rows i > j of column j are zero, the panels below this tile's columns are skipped
+  const int Keff = (*lower_nonzero == 0) ? min(N, j0 + kXzN) : N;
+  const int npanel = (Keff + kXzK - 1) / kXzK;
 
   auto load_panel = [&](int pi) {
     double* As = xs + (pi & 1) * stage_elems;
@@ -215,8 +240,10 @@ cudaError_t launch_xz(Op* op, const double* Y, int64_t ldy, const double* Z, int
                       double* Out, int64_t ldo, cudaStream_t st) {
   const size_t smem = xz_smem_bytes();
   dim3 grid((unsigned)((N2 + kXzN - 1) / kXzN), (unsigned)((n_rows + kXzM - 1) / kXzM));
-  k_xz<<<grid, 256, smem, st>>>(Y, ldy, Z, ldz, n_rows, N, N2, Out, ldo);
-  op->launches++;
+  cudaError_t e = detect_lower_nonzero(op, Z, ldz, N, N2, st);
+  if (e != cudaSuccess) return e;
+  k_xz<<<grid, 256, smem, st>>>(Y, ldy, Z, ldz, n_rows, N, N2, Out, ldo, op->rr_flag);
+  op->launches += 2;
   return cudaGetLastError();
 }
 
@@ -466,14 +493,15 @@ constexpr int kZ32LdA = kZ32K + 4, kZ32LdB = kZ32N + 8;      // A row-major (m x
 __global__ void __launch_bounds__(256, 1) k_xz_tf32(const float* __restrict__ Y32, int64_t ldy32, const float* __restrict__ Z32,
                                                     int64_t ldz32, const double* __restrict__ Y, int64_t ldy,
                                                     const double* __restrict__ zd, int64_t n_rows, int N, int N2,
-                                                    double* __restrict__ Out, int64_t ldo) {
+                                                    double* __restrict__ Out, int64_t ldo, const int* __restrict__ lower_nonzero) {
   extern __shared__ __align__(16) float fs[];
   constexpr int stage_elems = kZ32M * kZ32LdA + kZ32K * kZ32LdB;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int wm = warp >> 1, wn = warp & 1, g = lane >> 2, t = lane & 3;
   const int j0 = blockIdx.x * kZ32N;
   const int64_t g0 = (int64_t)blockIdx.y * kZ32M;
-  const int npanel = (N + kZ32K - 1) / kZ32K;
+  const int Keff = (*lower_nonzero == 0) ? min(N, j0 + kZ32N) : N;      // upper-triangular Z: zero panels skipped (k_xz)
+  const int npanel = (Keff + kZ32K - 1) / kZ32K;
   auto load_panel = [&](int pi) {
     float* As = fs + (pi & 1) * stage_elems;
     float* Bs = As + kZ32M * kZ32LdA;
@@ -622,9 +650,11 @@ cudaError_t launch_xty_tf32(Op* op, const float* A, int64_t lda, const float* B,
 cudaError_t launch_xz_tf32(Op* op, const float* Y32, int64_t ldy32, const float* Z32, int64_t ldz32, const double* Y, int64_t ldy,
                            const double* zd, int64_t n_rows, int N, int N2, double* Out, int64_t ldo, cudaStream_t st) {
   dim3 grid((unsigned)((N2 + kZ32N - 1) / kZ32N), (unsigned)((n_rows + kZ32M - 1) / kZ32M));
-  if (op->rr_variant == 2 || !launch_xz_umma(Y32, ldy32, Z32, ldz32, Y, ldy, zd, n_rows, N, N2, Out, ldo, st))   // tcgen05 first
-    k_xz_tf32<<<grid, 256, xz32_smem_bytes(), st>>>(Y32, ldy32, Z32, ldz32, Y, ldy, zd, n_rows, N, N2, Out, ldo);
-  op->launches++;
+  cudaError_t e = detect_lower_nonzero(op, Z32, ldz32, N, N2, st);
+  if (e != cudaSuccess) return e;
+  if (op->rr_variant == 2 || !launch_xz_umma(Y32, ldy32, Z32, ldz32, Y, ldy, zd, n_rows, N, N2, Out, ldo, op->rr_flag, st))   // tcgen05 first
+    k_xz_tf32<<<grid, 256, xz32_smem_bytes(), st>>>(Y32, ldy32, Z32, ldz32, Y, ldy, zd, n_rows, N, N2, Out, ldo, op->rr_flag);
+  op->launches += 2;
   return cudaGetLastError();
 }
 

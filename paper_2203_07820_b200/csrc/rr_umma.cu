@@ -122,7 +122,7 @@ __global__ void __launch_bounds__(kUThreads, 1) k_umma(const __grid_constant__ C
                                                        const __grid_constant__ CUtensorMap tmB, int64_t n_rows, int N1, int N2,
                                                        int64_t rows_per_split, int skip_block, int row_block0, int col_block0,
                                                        int lower, double* __restrict__ Cpart, const double* __restrict__ Yd, int64_t ldy,
-                                                       const double* __restrict__ zd, int64_t ldo) {
+                                                       const double* __restrict__ zd, int64_t ldo, const int* __restrict__ lower_nonzero) {
   const int i0 = XZ ? 0 : blockIdx.x * kUM, j0 = (XZ ? blockIdx.x : blockIdx.y) * kUN;
   if (!XZ && lower && j0 > i0 + kUM - 1) return;                      // strictly above the diagonal of a Hermitian result
   if (!XZ && skip_block > 0) {                                        // tiles inside an FP64 diagonal block: not ours (k_xty_tf32's rule)
@@ -142,7 +142,8 @@ __global__ void __launch_bounds__(kUThreads, 1) k_umma(const __grid_constant__ C
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int64_t g0 = XZ ? (int64_t)blockIdx.y * kUM : (int64_t)blockIdx.z * rows_per_split;
   const int64_t g1 = min(n_rows, g0 + (XZ ? (int64_t)kUM : rows_per_split));
-  const int nstage = XZ ? (N1 + kUK - 1) / kUK : (int)((g1 - g0 + kUK - 1) / kUK);
+  // Y Z with an upper-triangular Z (Z = L^-T): the contraction stops at the last column of the tile (the rest of Z is zero)
+  const int nstage = XZ ? (((*lower_nonzero == 0) ? min(N1, j0 + kUN) : N1) + kUK - 1) / kUK : (int)((g1 - g0 + kUK - 1) / kUK);
 
   if (tid == 0) {
     for (int s = 0; s < kUStages; ++s) { u_mbar_init(full_raw + s, 1); u_mbar_init(full_split + s, kUSplitWarps); u_mbar_init(empty + s, 1); }
@@ -356,17 +357,17 @@ bool launch_xty_umma(const float* A, int64_t lda, const float* B, int64_t ldb, i
   if (!u_make_map(&tmA, A, n_rows, N1, lda) || !u_make_map(&tmB, B, n_rows, N2, ldb)) return false;
   dim3 grid((unsigned)((N1 + kUM - 1) / kUM), (unsigned)((N2 + kUN - 1) / kUN), (unsigned)n_split);
   k_umma<false><<<grid, kUThreads, kUSmemBytes, st>>>(tmA, tmB, n_rows, N1, N2, rows_per_split, skip_block, row_block0, col_block0, lower,
-                                                      Cpart, nullptr, 0, nullptr, 0);
+                                                      Cpart, nullptr, 0, nullptr, 0, nullptr);
   return true;
 }
 
 // Out[g][j] = sum_i Y32[g][i] Z32[i][j] (3xTF32) + Y[g][j] zd[j] (FP64), g < n_rows, i < N, j < N2; false: no tensor maps
 bool launch_xz_umma(const float* Y32, int64_t ldy32, const float* Z32, int64_t ldz32, const double* Y, int64_t ldy, const double* zd,
-                    int64_t n_rows, int N, int N2, double* Out, int64_t ldo, cudaStream_t st) {
+                    int64_t n_rows, int N, int N2, double* Out, int64_t ldo, const int* lower_nonzero, cudaStream_t st) {
   CUtensorMap tmA, tmB;
   if (!u_make_map(&tmA, Y32, n_rows, N, ldy32, true) || !u_make_map(&tmB, Z32, N, N2, ldz32)) return false;
   dim3 grid((unsigned)((N2 + kUN - 1) / kUN), (unsigned)((n_rows + kUM - 1) / kUM));
-  k_umma<true><<<grid, kUThreads, kUSmemBytes, st>>>(tmA, tmB, n_rows, N, N2, 0, 0, 0, 0, 0, Out, Y, ldy, zd, ldo);
+  k_umma<true><<<grid, kUThreads, kUSmemBytes, st>>>(tmA, tmB, n_rows, N, N2, 0, 0, 0, 0, 0, Out, Y, ldy, zd, ldo, lower_nonzero);
   return true;
 }
 

@@ -612,6 +612,22 @@ def test_lower_triangle_products_span_several_tiles(rr_variant):
         assert torch.equal(Hm, Hm.T) and float(err.max()) <= 8 * eps32, chunk
         assert float(err[n_oc:, n_oc:].max()) <= 1e-13, chunk                   # the fr-fr block is an FP64 product
         assert float(err[:n_oc, :].max()) > 1e-12                               # the rest ARE FP32 products
+    # Y Z: an upper-triangular Z (Z = L^-T, Algorithm 2 step 3b) is detected on the device and the zero panels are skipped;
+    # a dense Z, and one with a single nonzero in the last row of the first column, take the full contraction
+    Zd = torch.randn((N, N), dtype=torch.float64, device="cuda", generator=g)
+    Zu = Zd.triu()
+    Z1 = Zu.clone()
+    Z1[N - 1, 0] = 0.5
+    for Z in (Zd, Zu, Z1):
+        P64 = Y @ Z
+        p_scale = torch.outer(Y.norm(dim=1), Z.norm(dim=0))
+        P = op.subspace_transform(Y, Z)
+        assert torch.equal(P, op.subspace_transform(Y, Z)) and float(((P - P64).abs() / p_scale).max()) <= 1e-13
+        Pm = op.subspace_transform_mixed(Y, Z)
+        assert float(((Pm - P64).abs() / p_scale).max()) <= 8 * eps32
+    Zr = torch.randn((N, 100), dtype=torch.float64, device="cuda", generator=g).triu()      # N2 < N, upper trapezoidal
+    P = op.subspace_transform(Y, Zr)
+    assert float(((P - Y @ Zr).abs() / torch.outer(Y.norm(dim=1), Zr.norm(dim=0))).max()) <= 1e-13
     op.close()
 
 
