@@ -191,6 +191,27 @@ int chfsi_overlap_matrix(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N
 int chfsi_projected_hamiltonian(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N, int64_t B, double* H_dev,
                                 void* workspace_dev, void* cuda_stream);
 
+/* Allocation-free variant of chfsi_overlap_matrix, for callers that cannot call cudaMalloc (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid it): S = Y^T Y (Algorithm 2 step 1a; lower triangle computed,
+ * upper mirrored) with the row-split partial sums in a STATIC device array of the library instead of the
+ * scratch buffer that chfsi_overlap_matrix grows on demand.  The call makes no cudaMalloc / cudaFree, creates no event or
+ * stream and calls no allocating library routine: it enqueues three kernels on cuda_stream and returns.
+ *   limit:   N <= CHFSI_NOALLOC_MAX_N (512) columns; a larger N is CHFSI_ERR_BAD_ARGUMENT with a message that names the
+ *            limit.  Any number of rows.  The static array holds CHFSI_NOALLOC_SPLITS x MAX_N x MAX_N doubles = 16 MiB of
+ *            device memory on every GPU that loads the library, until the process exits.
+ *   sharing: ALL calls on a device (any handle, any stream) use the same array, which keeps the last call's contents;
+ *            nothing in it has to start at zero (every partial sum that is read is written by the same call), but two
+ *            calls that overlap on the GPU RACE on it: the caller orders them (same stream, or an event between them).
+ *            The handle's cross-stream ordering of the other entry points does not cover this call.
+ *   device:  the current device must be the one the handle was created on (CHFSI_ERR_CUDA otherwise); the device
+ *            address of the array is looked up at chfsi_create*, once per device.
+ * Arguments, layout, alignment rules and result as chfsi_overlap_matrix (FP64 operators, real handles; N, ldy even,
+ * pointers 16-byte aligned); the sums are split over the rows as there, so the two results agree to rounding (bit for bit
+ * when both choose the same number of row splits). */
+#define CHFSI_NOALLOC_MAX_N 512
+#define CHFSI_NOALLOC_SPLITS 8
+int chfsi_overlap_matrix_noalloc(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N, double* S_dev, void* cuda_stream);
+
 /* Subspace transformation  Out = Y Z  -- Algorithm 2 step 3 (RRGEP-ST; the blocked "X_p Z"
  * products of PAPER.md:560): with Z = Q_fr it gives the Ritz vectors Psi_fr^R = Psi_f Q_fr (step 3a), with
  * Z = L^-T (S = L L^T) the orthonormal basis Psi^o = Psi_f L^-T (step 3b).  FP64 operators only.

@@ -21,7 +21,7 @@ LIB_PATH = os.path.join(HERE, "libchfsi.so")
 EXPORTED_SYMBOLS = [
     "chfsi_create", "chfsi_create_k", "chfsi_create_part", "chfsi_mesh_mass", "chfsi_projector_coefficients",
     "chfsi_apply_H_with_coefficients", "chfsi_pack_rows", "chfsi_unpack_rows", "chfsi_recurrence_update", "chfsi_destroy", "chfsi_update_potential", "chfsi_get_info", "chfsi_workspace_bytes", "chfsi_mass_diag",
-    "chfsi_apply_H", "chfsi_overlap_matrix", "chfsi_projected_hamiltonian", "chfsi_subspace_transform",
+    "chfsi_apply_H", "chfsi_overlap_matrix", "chfsi_overlap_matrix_noalloc", "chfsi_projected_hamiltonian", "chfsi_subspace_transform",
     "chfsi_cholesky_inverse", "chfsi_overlap_matrix_mixed", "chfsi_projected_hamiltonian_mixed", "chfsi_subspace_transform_mixed", "chfsi_chebyshev_filter", "chfsi_chebyshev_filter_chunked", "chfsi_chebyshev_filter_host",
     "chfsi_launch_count", "chfsi_set_kernel_variant", "chfsi_set_rr_variant", "chfsi_set_profiling", "chfsi_get_profile",
     "chfsi_measure_fp64_peak", "chfsi_last_error",
@@ -117,6 +117,8 @@ def load_library(build_if_missing: bool = True):
     lib_.chfsi_apply_H.restype = C.c_int
     lib_.chfsi_overlap_matrix.argtypes = [vp, vp, i64, i64, vp, vp]
     lib_.chfsi_overlap_matrix.restype = C.c_int
+    lib_.chfsi_overlap_matrix_noalloc.argtypes = [vp, vp, i64, i64, vp, vp]
+    lib_.chfsi_overlap_matrix_noalloc.restype = C.c_int
     lib_.chfsi_projected_hamiltonian.argtypes = [vp, vp, i64, i64, i64, vp, vp, vp]
     lib_.chfsi_projected_hamiltonian.restype = C.c_int
     lib_.chfsi_subspace_transform.argtypes = [vp, vp, i64, i64, vp, i64, i64, vp, i64, vp]
@@ -386,6 +388,17 @@ class Operator:
         S = torch.empty((N, N), dtype=torch.float64, device="cuda")
         self._check(load_library().chfsi_overlap_matrix(self._h, yp, ldy, N, C.c_void_p(S.data_ptr()),
                                                         _stream_ptr(stream)))
+        return S
+
+    def overlap_matrix_noalloc(self, Y, S, stream=None):
+        """S <- Y^T Y through chfsi_overlap_matrix_noalloc: the library allocates nothing (static scratch, N <= 512; calls
+        that overlap on the GPU race on it).  `S` is the caller's contiguous [N, N] FP64 device tensor."""
+        import torch
+        yp, ldy, N = self._block(Y, "Y")
+        if not (isinstance(S, torch.Tensor) and S.is_cuda and S.dtype == torch.float64 and S.shape == (N, N) and S.is_contiguous()):
+            raise TypeError("S: expected a contiguous [N, N] float64 CUDA tensor")
+        self._check(load_library().chfsi_overlap_matrix_noalloc(self._h, yp, ldy, N, C.c_void_p(S.data_ptr()),
+                                                                _stream_ptr(stream)))
         return S
 
     def projected_hamiltonian(self, Y, B=None, workspace=None, stream=None):

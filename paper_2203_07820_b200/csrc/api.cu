@@ -725,6 +725,24 @@ int chfsi_overlap_matrix(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N
   API_CATCH(op)
 }
 
+int chfsi_overlap_matrix_noalloc(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N, double* S_dev, void* cuda_stream) {
+  if (op && op->kpoint) return fail(op, CHFSI_ERR_UNSUPPORTED, "real-block entry point called on a k-point handle");
+  int rc = check_rr_args(op, Y_dev, ldy, N, S_dev);
+  if (rc) return rc;
+  if (N > CHFSI_NOALLOC_MAX_N)
+    return fail(op, CHFSI_ERR_BAD_ARGUMENT,
+                "overlap_matrix_noalloc: N = " + std::to_string(N) + " exceeds CHFSI_NOALLOC_MAX_N = " +
+                    std::to_string(CHFSI_NOALLOC_MAX_N) + " (static scratch of 16 MiB); use chfsi_overlap_matrix");
+  API_TRY
+  // no order_enter / order_leave (the latter may create an event): the caller orders calls that share the static array
+  cudaError_t ce = launch_xty_static(op, reinterpret_cast<const double*>(Y_dev), ldy, op->n_dofs, (int)N, S_dev, N,
+                                     reinterpret_cast<cudaStream_t>(cuda_stream));
+  if (ce == cudaErrorInvalidDevice)
+    return fail(op, CHFSI_ERR_CUDA, "overlap_matrix_noalloc: the current device is not the one this handle was created on");
+  return ce == cudaSuccess ? CHFSI_OK : cuda_fail(op, ce, "overlap_matrix_noalloc");
+  API_CATCH(op)
+}
+
 int chfsi_projected_hamiltonian(chfsi_op* op, const void* Y_dev, int64_t ldy, int64_t N, int64_t B, double* H_dev,
                                 void* workspace_dev, void* cuda_stream) {
   if (op && op->kpoint) return fail(op, CHFSI_ERR_UNSUPPORTED, "real-block entry point called on a k-point handle");

@@ -252,6 +252,10 @@ cudaError_t capture_diagonal(Op* op, cudaStream_t stream);
 cudaError_t launch_xty(Op* op, const double* A, int64_t lda, const double* B, int64_t ldb, int64_t n_rows, int N1, int N2,
                        double* C, int64_t ldc, cudaStream_t stream, int lower = 0);
 cudaError_t launch_mirror_lower(Op* op, double* C, int N, int64_t ldc, cudaStream_t stream);
+// Allocation-free S = Y^T Y (chfsi_overlap_matrix_noalloc): partial sums in a file-scope __device__ array of rr_kernels.cu
+// whose device address resolve_xty_static() looks up once per device (called by init_rr_kernels with that device current).
+cudaError_t resolve_xty_static();
+cudaError_t launch_xty_static(Op* op, const double* Y, int64_t ldy, int64_t n_rows, int N, double* S, int64_t lds, cudaStream_t stream);
 // Out[n_rows][ldo] = Y Z, Y [n_rows][ldy] with N columns, Z [N][ldz] with N2 columns (Alg. 2 step 3)
 cudaError_t launch_xz(Op* op, const double* Y, int64_t ldy, const double* Z, int64_t ldz, int64_t n_rows, int N, int N2,
                       double* Out, int64_t ldo, cudaStream_t stream);

@@ -10,6 +10,7 @@
 // tiles of mma.sync.m8n8k4.f64; the row range is split over gridDim.z CTAs whose partial tiles are summed in split
 // order by k_xty_reduce: deterministic.  Rows stream through a 2-stage cp.async ring of 32-row panels.
 #include <algorithm>
+#include <mutex>
 
 #include "common.h"
 
@@ -233,6 +234,7 @@ cudaError_t init_rr_kernels() {
   cudaError_t e = cudaFuncSetAttribute(k_xz, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)xz_smem_bytes());
   if (e != cudaSuccess) return e;
   if ((e = cudaFuncSetAttribute(k_xty, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)xty_smem_bytes()))) return e;
+  if ((e = resolve_xty_static())) return e;              // device address of the static scratch of the allocation-free S
   return init_rr_mixed_kernels();
 }
 
@@ -301,6 +303,91 @@ cudaError_t launch_xty(Op* op, const double* A, int64_t lda, const double* B, in
   k_xty_reduce<<<(unsigned)(((int64_t)N1 * N2 + 255) / 256), 256, 0, st>>>(reinterpret_cast<const double*>(op->rr_scratch), n_split,
                                                                           N1, N2, lower, C, ldc);
   op->launches += 2;
+  return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Allocation-free S = Y^T Y (chfsi_overlap_matrix_noalloc, include/chfsi.h): k_xty's row-split partial sums go to a
+// file-scope array in device memory instead of the cudaMalloc'ed op->rr_scratch, for callers that cannot allocate
+// (CUDA graph capture, serving loops).  Every device that loads the library holds the kXtyStaticBytes of the array until
+// the process exits.  In HOST code `g_xty_static` is only a stand-in for the symbol: its device address is looked up by
+// cudaGetSymbolAddress once per device (resolve_xty_static, called with that device current at operator creation) and
+// THAT pointer is what k_xty is given; device code (k_xty_reduce_static) names the array directly.
+// The array is shared by every call on a device and keeps the last call's contents.  Nothing in it has to start at zero:
+// every partial sum the reduction reads (splits 0 .. n_split-1, entries r >= c) is stored by the k_xty launch of the same
+// call.  Two calls that overlap on the GPU (different streams, no dependency) race on it.
+// ---------------------------------------------------------------------------------------------------------------
+namespace {
+constexpr size_t kXtyStaticDoubles = (size_t)CHFSI_NOALLOC_SPLITS * CHFSI_NOALLOC_MAX_N * CHFSI_NOALLOC_MAX_N;   // 2 Mi doubles
+constexpr size_t kXtyStaticBytes = kXtyStaticDoubles * sizeof(double);                                          // 16 MiB
+static __device__ __align__(256) double g_xty_static[kXtyStaticDoubles];
+
+constexpr int kMaxDevices = 64;
+double* g_xty_static_ptr[kMaxDevices] = {};         // device address of g_xty_static on device d (nullptr: not looked up yet)
+std::mutex g_xty_static_mutex;
+
+// C[r][c] (r >= c) = sum over the row splits, in split order, of the partial sums in g_xty_static
+__global__ void __launch_bounds__(256) k_xty_reduce_static(int n_split, int N, double* __restrict__ C, int64_t ldc) {
+  const int64_t e = (int64_t)blockIdx.x * 256 + threadIdx.x;
+  if (e >= (int64_t)N * N) return;
+  if (e % N > e / N) return;                            // above the diagonal: filled by k_mirror_lower
+  double s = 0.0;
+  for (int k = 0; k < n_split; ++k) s += g_xty_static[(int64_t)k * N * N + e];
+  C[(e / N) * ldc + (e % N)] = s;
+}
+}  // namespace
+
+// Once per device, with that device current (init_rr_kernels at operator creation): the device address of the array.
+cudaError_t resolve_xty_static() {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(g_xty_static_mutex);
+  if (g_xty_static_ptr[dev]) return cudaSuccess;
+  double* ptr = nullptr;
+  e = cudaGetSymbolAddress((void**)&ptr, g_xty_static);
+  if (e != cudaSuccess) return e;
+  if (!ptr) return cudaErrorInvalidSymbol;
+  g_xty_static_ptr[dev] = ptr;
+  return cudaSuccess;
+}
+
+// S[N][N] = Y^T Y, lower triangle computed and mirrored as in chfsi_overlap_matrix.  No cudaMalloc / cudaFree / event or
+// stream creation: three kernel launches on `st`.  cudaErrorInvalidValue: N beyond CHFSI_NOALLOC_MAX_N;
+// cudaErrorInvalidDevice: the current device is not one an operator was created on (no looked-up address).
+cudaError_t launch_xty_static(Op* op, const double* Y, int64_t ldy, int64_t n_rows, int N, double* S, int64_t lds, cudaStream_t st) {
+  if (N < 1 || N > CHFSI_NOALLOC_MAX_N) return cudaErrorInvalidValue;
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  double* scratch = nullptr;
+  if (dev >= 0 && dev < kMaxDevices) {
+    std::lock_guard<std::mutex> lock(g_xty_static_mutex);
+    scratch = g_xty_static_ptr[dev];
+  }
+  if (!scratch) return cudaErrorInvalidDevice;         // no operator was created with this device current
+  const int ti = (N + kXtM - 1) / kXtM, tj = (N + kXtN - 1) / kXtN;
+  // row splits as in launch_xty, but never more than fit into the array (>= CHFSI_NOALLOC_SPLITS by construction)
+  const int cap = 2 * op->n_sm, tiles = lower_tiles(N, N, kXtM, kXtN, 1);
+  const int ns_fit = (int)std::min<size_t>(kXtyStaticDoubles / ((size_t)N * N), 1u << 20);
+  const int ns_max = std::min(ns_fit, (int)std::max<int64_t>(1, (n_rows + 511) / 512));
+  const int ns_lo = std::min(ns_max, std::max(1, (3 * cap + tiles - 1) / tiles));
+  int n_split = ns_lo;
+  double best = 0.0;
+  for (int ns = ns_lo; ns <= std::min(ns_max, 3 * ns_lo + 2); ++ns) {
+    const int64_t ctas = (int64_t)tiles * ns;
+    const double eff = (double)ctas / (double)(((ctas + cap - 1) / cap) * cap);
+    if (eff > best + 1e-9) { best = eff; n_split = ns; }
+  }
+  const int64_t rows_per_split = ((n_rows + n_split - 1) / n_split + kXtK - 1) / kXtK * kXtK;
+  n_split = (int)((n_rows + rows_per_split - 1) / rows_per_split);
+  if ((size_t)n_split * N * N > kXtyStaticDoubles) return cudaErrorInvalidValue;      // cannot happen: n_split <= ns_fit
+  dim3 grid((unsigned)ti, (unsigned)tj, (unsigned)n_split);
+  k_xty<<<grid, 256, xty_smem_bytes(), st>>>(Y, ldy, Y, ldy, n_rows, N, N, rows_per_split, 1, scratch);
+  k_xty_reduce_static<<<(unsigned)(((int64_t)N * N + 255) / 256), 256, 0, st>>>(n_split, N, S, lds);
+  k_mirror_lower<<<(unsigned)(((int64_t)N * N + 255) / 256), 256, 0, st>>>(S, N, lds);
+  op->launches += 3;
   return cudaGetLastError();
 }
 
