@@ -574,7 +574,7 @@ def run_kpoint(args):
 def run_partition(args, spec):
     """Strong scaling over cells: every rank holds a slab of the mesh (partition.py) and the rows of its dofs for ALL N vectors;
     per H~ application one all-reduce of the projector coefficients and one of the shared rows.  N = 1 measures the same
-    unfused sequence (phased apply + recurrence kernel) without any exchange."""
+    sequence (phased, accumulating apply in scaled blocks; shared-row fix-up) without any exchange."""
     import torch
     import torch.distributed as dist
 

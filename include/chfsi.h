@@ -288,6 +288,36 @@ int chfsi_unpack_rows(chfsi_op* op, const void* buf_dev, int buf_precision, cons
 int chfsi_recurrence_update(chfsi_op* op, const void* HX_dev, int64_t ldh, const void* X_dev, int64_t ldx, void* T_dev,
                             int64_t ldt, int64_t B, double alpha, double beta, double c, void* cuda_stream);
 
+/* The same exchange for the filter in SCALED blocks (the accumulate-only recurrence W_k = W_{k-2} + gamma_k (H~ - c) W_{k-1} of
+ * chfsi_chebyshev_filter, U14), which saves the separate recurrence pass over the block: the part's cell kernel adds
+ * its contribution straight into the block that holds W_{k-2}, and only the rows of the shared dofs are fixed up afterwards.
+ *   chfsi_accumulate_supported   *supported = 1 when chfsi_apply_shifted_with_coefficients can ADD for these blocks (the
+ *                          sum-factorised kernel: p <= 6, kernel variant 0 or 6, 16-byte aligned blocks); else 0 and the caller
+ *                          stays with chfsi_apply_H_with_coefficients + chfsi_recurrence_update.  No device work.
+ *   chfsi_apply_shifted_with_coefficients   T = alpha (H~_part - c) X  (accumulate = 0: the part's first contribution to a dof is
+ *                          a store, T need not be initialised) or  T += alpha (H~_part - c) X  (accumulate = 1;
+ *                          CHFSI_ERR_UNSUPPORTED where chfsi_accumulate_supported says 0), projector coefficients P_dev given.
+ *                          EVERY part subtracts c X once on each dof it holds, shared or not.
+ *   chfsi_pack_rows_delta  buf[s(i)] = T[rows[i]] - base[i] + corr X[rows[i]] (1 - owner[i]): the part's contribution to its
+ *                          shared rows.  base_dev [n_rows][B] (dense, operator's type) = those rows of T as packed by
+ *                          chfsi_pack_rows BEFORE the accumulating application (NULL after a storing one: 0); owner_dev[n_rows]
+ *                          (DEVICE bytes) = 1 on the one part that owns the dof, 0 on the others, which put the shift back:
+ *                          corr = alpha c.  Summed over the parts, buf is alpha (H~ - c) X on the shared dofs.
+ *   chfsi_unpack_rows_sum  T[rows[i]] = base[i] + buf[s(i)]  (base_dev NULL: 0), the sums back in place.
+ * buf, slots, precisions and error codes as in chfsi_pack_rows / chfsi_unpack_rows. */
+int chfsi_accumulate_supported(chfsi_op* op, const void* X_dev, int64_t ldx, const void* T_dev, int64_t ldt, int64_t B,
+                               void* workspace_dev, int* supported);
+int chfsi_apply_shifted_with_coefficients(chfsi_op* op, const void* X_dev, int64_t ldx, void* T_dev, int64_t ldt, int64_t B,
+                                          double alpha, double c, int accumulate, const void* P_dev, void* workspace_dev,
+                                          void* cuda_stream);
+int chfsi_pack_rows_delta(chfsi_op* op, const void* T_dev, int64_t ldt, const void* base_dev /* nullable */, const void* X_dev,
+                          int64_t ldx, const uint8_t* owner_dev, double corr, int64_t B, const int32_t* rows_dev,
+                          const int32_t* slots_dev /* nullable */, int64_t n_rows, void* buf_dev, int buf_precision,
+                          void* cuda_stream);
+int chfsi_unpack_rows_sum(chfsi_op* op, const void* buf_dev, int buf_precision, const void* base_dev /* nullable */,
+                          const int32_t* rows_dev, const int32_t* slots_dev /* nullable */, int64_t n_rows, void* T_dev,
+                          int64_t ldt, int64_t B, void* cuda_stream);
+
 /* Number of kernel launches enqueued by this handle since creation (for benchmark bookkeeping). */
 int64_t chfsi_launch_count(const chfsi_op* op);
 

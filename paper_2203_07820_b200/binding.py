@@ -20,7 +20,8 @@ LIB_PATH = os.path.join(HERE, "libchfsi.so")
 
 EXPORTED_SYMBOLS = [
     "chfsi_create", "chfsi_create_k", "chfsi_create_part", "chfsi_mesh_mass", "chfsi_projector_coefficients",
-    "chfsi_apply_H_with_coefficients", "chfsi_pack_rows", "chfsi_unpack_rows", "chfsi_recurrence_update", "chfsi_destroy", "chfsi_update_potential", "chfsi_get_info", "chfsi_workspace_bytes", "chfsi_mass_diag",
+    "chfsi_apply_H_with_coefficients", "chfsi_pack_rows", "chfsi_unpack_rows", "chfsi_recurrence_update", "chfsi_accumulate_supported", "chfsi_apply_shifted_with_coefficients",
+    "chfsi_pack_rows_delta", "chfsi_unpack_rows_sum", "chfsi_destroy", "chfsi_update_potential", "chfsi_get_info", "chfsi_workspace_bytes", "chfsi_mass_diag",
     "chfsi_apply_H", "chfsi_overlap_matrix", "chfsi_overlap_matrix_noalloc", "chfsi_projected_hamiltonian", "chfsi_subspace_transform",
     "chfsi_cholesky_inverse", "chfsi_overlap_matrix_mixed", "chfsi_projected_hamiltonian_mixed", "chfsi_subspace_transform_mixed", "chfsi_chebyshev_filter", "chfsi_chebyshev_filter_chunked", "chfsi_chebyshev_filter_host",
     "chfsi_launch_count", "chfsi_set_kernel_variant", "chfsi_set_rr_variant", "chfsi_set_profiling", "chfsi_get_profile",
@@ -103,6 +104,14 @@ def load_library(build_if_missing: bool = True):
     lib_.chfsi_unpack_rows.restype = C.c_int
     lib_.chfsi_recurrence_update.argtypes = [vp, vp, i64, vp, i64, vp, i64, i64, dbl, dbl, dbl, vp]
     lib_.chfsi_recurrence_update.restype = C.c_int
+    lib_.chfsi_accumulate_supported.argtypes = [vp, vp, i64, vp, i64, i64, vp, C.POINTER(C.c_int)]
+    lib_.chfsi_accumulate_supported.restype = C.c_int
+    lib_.chfsi_apply_shifted_with_coefficients.argtypes = [vp, vp, i64, vp, i64, i64, dbl, dbl, C.c_int, vp, vp, vp]
+    lib_.chfsi_apply_shifted_with_coefficients.restype = C.c_int
+    lib_.chfsi_pack_rows_delta.argtypes = [vp, vp, i64, vp, vp, i64, vp, dbl, i64, vp, vp, i64, vp, C.c_int, vp]
+    lib_.chfsi_pack_rows_delta.restype = C.c_int
+    lib_.chfsi_unpack_rows_sum.argtypes = [vp, vp, C.c_int, vp, vp, vp, i64, vp, i64, i64, vp]
+    lib_.chfsi_unpack_rows_sum.restype = C.c_int
     lib_.chfsi_destroy.argtypes = [vp]
     lib_.chfsi_destroy.restype = C.c_int
     lib_.chfsi_update_potential.argtypes = [vp, C.POINTER(_Potential), vp]
@@ -379,6 +388,63 @@ class Operator:
             raise ValueError("HX, X and T must have the same number of columns")
         self._check(load_library().chfsi_recurrence_update(self._h, hp, ldh, xp, ldx, tp, ldt, B, float(alpha), float(beta),
                                                            float(c), _stream_ptr(stream)))
+        return T
+
+    # -- the exchange of the filter in scaled (accumulate-only) blocks: include/chfsi.h ----------------------------
+    def accumulate_supported(self, X, T, workspace=None) -> bool:
+        """True when apply_shifted_with_coefficients(..., accumulate=True) is available for these blocks."""
+        xp, ldx, B = self._block(X, "X")
+        tp, ldt, Bt = self._block(T, "T")
+        if B != Bt:
+            raise ValueError("X and T must have the same number of columns")
+        ws = workspace if workspace is not None else self.workspace(B)
+        yes = C.c_int(0)
+        self._check(load_library().chfsi_accumulate_supported(self._h, xp, ldx, tp, ldt, B, C.c_void_p(ws.data_ptr()), C.byref(yes)))
+        return bool(yes.value)
+
+    def apply_shifted_with_coefficients(self, X, P, T, alpha, c, accumulate, workspace=None, stream=None):
+        """T = alpha (H~_part - c) X (accumulate False) or T += alpha (H~_part - c) X, projector coefficients P given."""
+        xp, ldx, B = self._block(X, "X")
+        tp, ldt, Bt = self._block(T, "T")
+        n_proj = int(self.info["n_proj"])
+        if Bt != B or tuple(P.shape) != (n_proj, B) or not P.is_contiguous() or P.dtype != self.dtype:
+            raise ValueError("need T [n_dofs, B] and a contiguous P [n_proj, B] of the operator's dtype")
+        ws = workspace if workspace is not None else self.workspace(B)
+        self._check(load_library().chfsi_apply_shifted_with_coefficients(
+            self._h, xp, ldx, tp, ldt, B, float(alpha), float(c), 1 if accumulate else 0, C.c_void_p(P.data_ptr()),
+            C.c_void_p(ws.data_ptr()), _stream_ptr(stream)))
+        return T
+
+    def pack_rows_delta(self, T, base, X, owner, corr, rows, buf, slots=None, stream=None):
+        """buf[s(i)] = T[rows[i]] - base[i] + corr X[rows[i]] (1 - owner[i]); base: contiguous [n_rows, B] or None; owner: uint8."""
+        import torch
+        tp, ldt, B = self._rows_block(T, "T")
+        xp, ldx, Bx = self._rows_block(X, "X")
+        n = int(rows.numel())
+        if Bx != B or owner.dtype != torch.uint8 or int(owner.numel()) != n:
+            raise ValueError("need X with T's columns and one uint8 owner flag per row")
+        if base is not None and not (base.is_contiguous() and tuple(base.shape) == (n, B) and base.dtype == T.dtype):
+            raise ValueError("base: contiguous [n_rows, B] of T's dtype")
+        bp = 32 if buf.dtype == torch.float32 else 64
+        sp = C.c_void_p(slots.data_ptr()) if slots is not None else None
+        bs = C.c_void_p(base.data_ptr()) if base is not None else None
+        self._check(load_library().chfsi_pack_rows_delta(self._h, tp, ldt, bs, xp, ldx, C.c_void_p(owner.data_ptr()), float(corr), B,
+                                                         C.c_void_p(rows.data_ptr()), sp, n, C.c_void_p(buf.data_ptr()), bp,
+                                                         _stream_ptr(stream)))
+        return buf
+
+    def unpack_rows_sum(self, buf, base, rows, T, slots=None, stream=None):
+        """T[rows[i]] = base[i] + buf[s(i)] (base None: 0)."""
+        import torch
+        tp, ldt, B = self._rows_block(T, "T")
+        n = int(rows.numel())
+        if base is not None and not (base.is_contiguous() and tuple(base.shape) == (n, B) and base.dtype == T.dtype):
+            raise ValueError("base: contiguous [n_rows, B] of T's dtype")
+        bp = 32 if buf.dtype == torch.float32 else 64
+        sp = C.c_void_p(slots.data_ptr()) if slots is not None else None
+        bs = C.c_void_p(base.data_ptr()) if base is not None else None
+        self._check(load_library().chfsi_unpack_rows_sum(self._h, C.c_void_p(buf.data_ptr()), bp, bs, C.c_void_p(rows.data_ptr()), sp, n,
+                                                         tp, ldt, B, _stream_ptr(stream)))
         return T
 
     def overlap_matrix(self, Y, stream=None):

@@ -495,7 +495,8 @@ int chfsi_apply_H(chfsi_op* op, const void* X_dev, int64_t ldx, void* Y_dev, int
 namespace {
 // chfsi_apply_H in phases (ApplyArgs::phase): the projector coefficients of this operator's cells, or H~X with given ones
 int apply_phase(chfsi_op* op, const void* X_dev, int64_t ldx, void* Y_dev, int64_t ldy, int64_t B, void* P_dev, int phase,
-                void* workspace_dev, void* cuda_stream) {
+                void* workspace_dev, void* cuda_stream, double alpha = 1.0, double cshift = 0.0, bool accumulate = false,
+                int* query = nullptr) {
   int rc = check_block_args(op, X_dev, ldx, B, workspace_dev);
   if (rc) return rc;
   if (op->kpoint) return fail(op, CHFSI_ERR_UNSUPPORTED, "phased application of a k-point handle");
@@ -511,9 +512,12 @@ int apply_phase(chfsi_op* op, const void* X_dev, int64_t ldx, void* Y_dev, int64
   char* base = reinterpret_cast<char*>(workspace_dev);
   ApplyArgs g;
   g.X = X_dev; g.ldx = ldx; g.T = phase == 2 ? Y_dev : const_cast<void*>(X_dev); g.ldt = phase == 2 ? ldy : ldx; g.B = B;
-  g.alpha = 1.0; g.beta = 0.0; g.cshift = 0.0; g.phase = phase;
+  g.alpha = alpha; g.beta = 0.0; g.cshift = cshift; g.phase = phase; g.accumulate = accumulate;
   g.P = base + w.p_off; g.Pc = base + w.pc_off;
   g.sync = reinterpret_cast<unsigned long long*>(base + w.sync_off); g.epoch = 1;
+  if (query) { *query = apply_accumulates(op, g) ? 1 : 0; return CHFSI_OK; }
+  if (accumulate && !apply_accumulates(op, g))
+    return fail(op, CHFSI_ERR_UNSUPPORTED, "accumulating application: needs the sum-factorised kernel (p <= 6, variant 0 or 6) and aligned blocks");
   const size_t p_bytes = (size_t)op->n_proj * B * w.elt;
   cudaError_t ce = order_enter(op, st);
   if (ce == cudaSuccess) ce = cudaMemsetAsync(g.sync, 0, w.sync_bytes, st);
@@ -540,6 +544,20 @@ int chfsi_projector_coefficients(chfsi_op* op, const void* X_dev, int64_t ldx, i
 int chfsi_apply_H_with_coefficients(chfsi_op* op, const void* X_dev, int64_t ldx, void* Y_dev, int64_t ldy, int64_t B,
                                     const void* P_dev, void* workspace_dev, void* cuda_stream) {
   return apply_phase(op, X_dev, ldx, Y_dev, ldy, B, const_cast<void*>(P_dev), 2, workspace_dev, cuda_stream);
+}
+
+int chfsi_apply_shifted_with_coefficients(chfsi_op* op, const void* X_dev, int64_t ldx, void* T_dev, int64_t ldt, int64_t B,
+                                          double alpha, double c, int accumulate, const void* P_dev, void* workspace_dev,
+                                          void* cuda_stream) {
+  if (op && !(std::isfinite(alpha) && std::isfinite(c))) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "alpha, c must be finite");
+  return apply_phase(op, X_dev, ldx, T_dev, ldt, B, const_cast<void*>(P_dev), 2, workspace_dev, cuda_stream, alpha, c, accumulate != 0);
+}
+
+int chfsi_accumulate_supported(chfsi_op* op, const void* X_dev, int64_t ldx, const void* T_dev, int64_t ldt, int64_t B,
+                               void* workspace_dev, int* supported) {
+  if (op && !supported) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "NULL result pointer");
+  int dummy = 0;   // P_dev is not dereferenced by the query
+  return apply_phase(op, X_dev, ldx, const_cast<void*>(T_dev), ldt, B, &dummy, 2, workspace_dev, nullptr, 1.0, 0.0, true, supported);
 }
 
 int chfsi_recurrence_update(chfsi_op* op, const void* HX_dev, int64_t ldh, const void* X_dev, int64_t ldx, void* T_dev,
@@ -584,6 +602,43 @@ int chfsi_pack_rows(chfsi_op* op, const void* X_dev, int64_t ldx, int64_t B, con
 int chfsi_unpack_rows(chfsi_op* op, const void* buf_dev, int buf_precision, const int32_t* rows_dev, const int32_t* slots_dev,
                       int64_t n_rows, void* X_dev, int64_t ldx, int64_t B, void* cuda_stream) {
   return pack_rows(op, X_dev, ldx, B, rows_dev, slots_dev, n_rows, const_cast<void*>(buf_dev), buf_precision, true, cuda_stream);
+}
+
+namespace {
+int rows_delta(chfsi_op* op, void* T_dev, int64_t ldt, const void* base_dev, const void* X_dev, int64_t ldx, const uint8_t* owner_dev,
+               double corr, int64_t B, const int32_t* rows_dev, const int32_t* slots_dev, int64_t n_rows, void* buf_dev,
+               int buf_precision, bool unpack, void* cuda_stream) {
+  if (!op) return CHFSI_ERR_BAD_ARGUMENT;
+  if (n_rows < 0 || B < 1 || ldt < B) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "need n_rows >= 0, B >= 1, ld >= B");
+  if (n_rows > 0 && (!T_dev || !rows_dev || !buf_dev)) return fail(op, CHFSI_ERR_BAD_ARGUMENT, "NULL pointer");
+  if (n_rows > 0 && !unpack && (!X_dev || !owner_dev || ldx < B || !std::isfinite(corr)))
+    return fail(op, CHFSI_ERR_BAD_ARGUMENT, "pack_rows_delta: need X (ldx >= B), the owner flags and a finite correction factor");
+  if (buf_precision != op->precision && buf_precision != 32)
+    return fail(op, CHFSI_ERR_BAD_ARGUMENT, "buf_precision must be the operator's precision or 32");
+  if (op->kpoint) return fail(op, CHFSI_ERR_UNSUPPORTED, "pack / unpack on a k-point handle");
+  API_TRY
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  cudaError_t ce = order_enter(op, st);
+  if (ce == cudaSuccess)
+    ce = launch_rows_delta(op, T_dev, ldt, base_dev, X_dev, ldx, owner_dev, corr, B, rows_dev, slots_dev, n_rows, buf_dev,
+                           buf_precision, unpack, st);
+  if (ce == cudaSuccess) ce = order_leave(op, st);
+  return ce == cudaSuccess ? CHFSI_OK : cuda_fail(op, ce, unpack ? "unpack_rows_sum" : "pack_rows_delta");
+  API_CATCH(op)
+}
+}  // namespace
+
+int chfsi_pack_rows_delta(chfsi_op* op, const void* T_dev, int64_t ldt, const void* base_dev, const void* X_dev, int64_t ldx,
+                          const uint8_t* owner_dev, double corr, int64_t B, const int32_t* rows_dev, const int32_t* slots_dev,
+                          int64_t n_rows, void* buf_dev, int buf_precision, void* cuda_stream) {
+  return rows_delta(op, const_cast<void*>(T_dev), ldt, base_dev, X_dev, ldx, owner_dev, corr, B, rows_dev, slots_dev, n_rows, buf_dev,
+                    buf_precision, false, cuda_stream);
+}
+
+int chfsi_unpack_rows_sum(chfsi_op* op, const void* buf_dev, int buf_precision, const void* base_dev, const int32_t* rows_dev,
+                          const int32_t* slots_dev, int64_t n_rows, void* T_dev, int64_t ldt, int64_t B, void* cuda_stream) {
+  return rows_delta(op, T_dev, ldt, base_dev, nullptr, 0, nullptr, 0.0, B, rows_dev, slots_dev, n_rows, const_cast<void*>(buf_dev),
+                    buf_precision, true, cuda_stream);
 }
 
 int chfsi_chebyshev_filter(chfsi_op* op, void* X_dev, int64_t ldx, int64_t B, int32_t m, double a, double b,

@@ -228,6 +228,11 @@ struct ApplyArgs {
 // type (buf_precision == op->precision) or FP32, and one degree of the three-term recurrence on whole blocks.
 cudaError_t launch_pack_rows(Op* op, const void* X, int64_t ldx, int64_t B, const int32_t* rows, const int32_t* slots,
                              int64_t n_rows, void* buf, int buf_precision, bool unpack, cudaStream_t stream);
+// accumulate-only exchange: pack  buf[s(i)] = T[rows[i]] - base[i] + corr X[rows[i]] (1 - owner[i])  /  unpack
+// T[rows[i]] = base[i] + buf[s(i)]   (base [n_rows][B] contiguous or nullptr; part_kernels.cu)
+cudaError_t launch_rows_delta(Op* op, void* T, int64_t ldt, const void* base, const void* X, int64_t ldx, const uint8_t* owner,
+                              double corr, int64_t B, const int32_t* rows, const int32_t* slots, int64_t n_rows, void* buf,
+                              int buf_precision, bool unpack, cudaStream_t stream);
 cudaError_t launch_recurrence(Op* op, const void* HX, int64_t ldh, const void* X, int64_t ldx, void* T, int64_t ldt, int64_t B,
                               double alpha, double beta, double c, cudaStream_t stream);
 // True when launch_apply would run these arguments (X, ldx, T, ldt, P, B, sync set) with accumulate = true.

@@ -43,6 +43,7 @@ class LocalPart:
     chi_q: np.ndarray              # [nnz_local, n_q]
     shared_rows: np.ndarray        # [n_shared_here] local rows of the dofs shared with other ranks, ascending
     shared_slots: np.ndarray       # [n_shared_here] their positions in the global list of shared dofs
+    shared_owner: np.ndarray       # [n_shared_here] uint8: 1 where this rank is the lowest rank that holds the dof (its owner)
 
 
 class CellPartition:
@@ -98,7 +99,8 @@ class CellPartition:
             proj_cell_ptr=np.asarray(ptr, dtype=np.int64), proj_cell_idx=np.asarray(idx, dtype=np.int32),
             chi_q=np.asarray(chi, dtype=np.float64).reshape(len(idx), n_q),
             shared_rows=np.searchsorted(dofs, shared_here).astype(np.int32),
-            shared_slots=np.searchsorted(self.shared_dofs, shared_here).astype(np.int32))
+            shared_slots=np.searchsorted(self.shared_dofs, shared_here).astype(np.int32),
+            shared_owner=(np.argmax(self._touch[shared_here], axis=1) == rank).astype(np.uint8))
 
 
 # ------------------------------------------------------------------------------------------------------------
@@ -178,6 +180,7 @@ class PartitionedOperator:
         dev = "cuda"
         self._rows = torch.from_numpy(pt.shared_rows).to(dev)
         self._slots = torch.from_numpy(pt.shared_slots).to(dev)
+        self._owner = torch.from_numpy(pt.shared_owner).to(dev)
         self._proj_rows = torch.arange(len(pt.proj_ids), dtype=torch.int32, device=dev)
         self._proj_slots = torch.from_numpy(pt.proj_ids.astype(np.int32)).to(dev)
 
@@ -246,21 +249,77 @@ class PartitionedOperator:
         """In place on the local rows of a block (all ranks call it together)."""
         return self.chebyshev_filter_chunked(X, int(X.shape[1]), m, a, b, a0, workspace)
 
-    def chebyshev_filter_chunked(self, X, B, m, a, b, a0, workspace=None):
+    @staticmethod
+    def scaled_scalars(m, a, b, a0, precision=64):
+        """The recurrence in scaled blocks W_k = s_k Y_k (U14; csrc/api.cu filter_block): W_1 = g_1 (H~ - c) W_0 and
+        W_k = W_{k-2} + g_k (H~ - c) W_{k-1}; returns ([g_1 .. g_m], 1 / s_m, c), or None when |s_k| leaves the range of the
+        storage type (the three-term form is used then)."""
+        e, c = 0.5 * (b - a), 0.5 * (b + a)
+        s1 = e / (a0 - c)
+        limit = 1e200 if precision == 64 else 1e25
+        gam, sg, s_km2, s_km1 = [s1 / e], s1, 1.0, 1.0
+        for _ in range(2, m + 1):
+            sn = 1.0 / (2.0 / s1 - sg)
+            alpha, beta = 2.0 * sn / e, sg * sn
+            sg = sn
+            s_k = -s_km2 / beta
+            if not (1.0 / limit < abs(s_k) < limit):
+                return None
+            gam.append(s_k * alpha / s_km1)
+            s_km2, s_km1 = s_km1, s_k
+        return gam, 1.0 / s_km1, c
+
+    def chebyshev_filter_chunked(self, X, B, m, a, b, a0, workspace=None, scaled=True):
         """All N columns in chunks of B, TWO chunks in flight: while the shared rows of one chunk are on the wire (async
-        all-reduce), the cell kernel of the other chunk runs."""
+        all-reduce), the cell kernel of the other chunk runs.  scaled (default, where the part's kernel can add into its
+        target block): the recurrence runs in scaled blocks, the cell kernel accumulates this part's contribution straight
+        into W_{k-2} and only the shared rows are fixed up (pack_rows_delta / unpack_rows_sum) -- no recurrence pass over
+        the block; otherwise H~X, the exchange and chfsi_recurrence_update."""
         import torch
         if m < 1 or not (a0 <= a < b):
             raise ValueError("need m >= 1 and a0 <= a < b")
         N = int(X.shape[1])
         B = min(int(B), N)
         scal, c = self.recurrence_scalars(m, a, b, a0)
+        sc = self.scaled_scalars(m, a, b, a0, self.op.precision) if (scaled and m >= 2) else None
         ws = workspace if workspace is not None else self.op.workspace(B)
         chunks = [(j0, min(N, j0 + B)) for j0 in range(0, N, B)]
+        n_here = int(self._rows.numel())
         for i0 in range(0, len(chunks), 2):
             pair = chunks[i0:i0 + 2]
             cur = [X[:, j0:j1] for j0, j1 in pair]                      # Y_{k-1}
             tgt = [torch.empty((self.n_local_dofs, j1 - j0), dtype=self.dtype, device="cuda") for j0, j1 in pair]   # Y_{k-2} -> Y_k
+            if sc is not None and all(self.op.accumulate_supported(cur[q], tgt[q], ws) for q in range(len(pair))):
+                gam, inv_sm, _ = sc
+                for k, g in enumerate(gam, start=1):
+                    bufs, works, bases = [], [], []
+                    for q in range(len(pair)):
+                        Bq = int(cur[q].shape[1])
+                        Pg = self.coefficients_partial(cur[q], ws)
+                        self.comm.all_reduce(Pg)
+                        P = torch.empty((len(self.part.proj_ids), Bq), dtype=self.dtype, device="cuda")
+                        if len(self.part.proj_ids):
+                            self.op.unpack_rows(Pg, self._proj_rows, P, slots=self._proj_slots)
+                        base = None
+                        if k >= 2 and n_here:                             # the shared rows of W_{k-2} before this part adds to them
+                            base = torch.empty((n_here, Bq), dtype=self.dtype, device="cuda")
+                            self.op.pack_rows(tgt[q], self._rows, base)
+                        self.op.apply_shifted_with_coefficients(cur[q], P, tgt[q], g, c, k >= 2, workspace=ws)
+                        buf = torch.zeros((max(self.n_shared, 1), Bq), dtype=self.payload_dtype, device="cuda")
+                        if n_here:
+                            self.op.pack_rows_delta(tgt[q], base, cur[q], self._owner, g * c, self._rows, buf, slots=self._slots)
+                        works.append(self.comm.all_reduce(buf, async_op=True))
+                        bufs.append(buf); bases.append(base)
+                    for q in range(len(pair)):
+                        if works[q] is not None:
+                            works[q].wait()
+                        if n_here:
+                            self.op.unpack_rows_sum(bufs[q], bases[q], self._rows, tgt[q], slots=self._slots)
+                        cur[q], tgt[q] = tgt[q], cur[q]
+                for q, (j0, j1) in enumerate(pair):                      # X <- W_m / s_m (in place when m is even)
+                    out = X[:, j0:j1]
+                    self.op.recurrence_update(cur[q], cur[q], out, inv_sm, 0.0, 0.0)
+                continue
             HX = [torch.empty_like(t) for t in tgt]
             for alpha, beta in scal:
                 bufs, works = [], []

@@ -77,19 +77,23 @@ def run_ranks(world, fn):
     return out
 
 
-def workload(p=4, n=4):
+def workload(p=4, n=4, atoms_per_side=2):
     from workloads.generate import make_workload
-    return make_workload(None, n=n, p=p, L=2.0 * n, mesh_jitter=0.1, atoms_per_side=2, n_gaussians=0, nonlocal_=True,
+    return make_workload(None, n=n, p=p, L=2.0 * n, mesh_jitter=0.1, atoms_per_side=atoms_per_side, n_gaussians=0, nonlocal_=True,
                          smooth_field=0.05, seed_base=56, r_cut=2.2)
 
 
-@pytest.mark.parametrize("world,p,fp32", [(2, 4, False), (3, 6, False), (4, 3, False), (2, 6, True)])
-def test_partitioned_apply_and_filter_match_the_oracle_on_the_whole_mesh(world, p, fp32):
+# aps = atoms per side.  With one atom every cell has at most 8 projectors, the parts run the sum-factorised kernel and the
+# filter goes through the accumulate-only exchange (asserted); with 2^3 atoms some cells see more than 16 projectors, the
+# parts run the dense kernel and the filter takes H~X + exchange + recurrence pass.
+@pytest.mark.parametrize("world,p,fp32,aps", [(2, 4, False, 2), (3, 6, False, 2), (4, 3, False, 2), (2, 6, True, 2),
+                                              (2, 6, False, 1), (3, 4, True, 1), (4, 5, False, 1)])
+def test_partitioned_apply_and_filter_match_the_oracle_on_the_whole_mesh(world, p, fp32, aps):
     import torch
     from oracle import chfsi_oracle as orc
     from paper_2203_07820_b200.partition import CellPartition, PartitionedOperator
     from workloads.generate import random_block
-    wl = workload(p=p, n=4 if p <= 4 else 3)
+    wl = workload(p=p, n=4 if p <= 4 else 3, atoms_per_side=aps)
     oop = orc.operator_from_workload(wl)
     B, m = 24, 6
     X = random_block(wl.n_dofs, range(B), 9)
@@ -110,6 +114,12 @@ def test_partitioned_apply_and_filter_match_the_oracle_on_the_whole_mesh(world, 
         Y = part.apply_H(Xl)
         F = Xl.clone()
         part.chebyshev_filter_chunked(F, 8, m, a, b, a0)            # three chunks: a pair in flight, then a single one
+        if aps == 1:
+            assert part.op.accumulate_supported(F[:, :8], Xl[:, :8])     # ... in scaled blocks (the cell kernel accumulates)
+        F3 = Xl.clone()
+        part.chebyshev_filter_chunked(F3, 8, m, a, b, a0, scaled=False)   # H~X, exchange, separate recurrence pass
+        err3 = float((F3 - F).norm() / F.norm())
+        assert err3 <= (1e-5 if fp32 else 1e-12), err3
         torch.cuda.synchronize()
         res = (part.part.dofs, Y.cpu().numpy(), F.cpu().numpy(), part.op.launch_count())
         part.close()
@@ -132,13 +142,15 @@ def test_partitioned_apply_and_filter_match_the_oracle_on_the_whole_mesh(world, 
         assert err <= tol and emax <= tol, f"world {world} {what}: rel Frobenius {err:.3e}, max-norm {emax:.3e}"
 
 
-def test_single_part_equals_the_plain_operator():
-    """world = 1: the phased application (coefficients, then H~X with given coefficients) is the plain chfsi_apply_H."""
+@pytest.mark.parametrize("aps", [1, 2])
+def test_single_part_equals_the_plain_operator(aps):
+    """world = 1: the phased application (coefficients, then H~X with given coefficients) is the plain chfsi_apply_H, and the
+    filter (aps = 1: through the accumulate-only path, like chfsi_chebyshev_filter itself) is the plain filter."""
     import torch
     from paper_2203_07820_b200 import Operator
     from paper_2203_07820_b200.partition import PartitionedOperator
     from workloads.generate import random_block
-    wl = workload(p=6, n=3)
+    wl = workload(p=6, n=3, atoms_per_side=aps)
     part = PartitionedOperator(wl)
     op = Operator.from_workload(wl)
     assert np.allclose(part.mass, op.mass_diag().cpu().numpy(), rtol=1e-14, atol=0)
@@ -148,4 +160,8 @@ def test_single_part_equals_the_plain_operator():
     part.chebyshev_filter(F1, 5, 0.5, 300.0, 0.1)
     op.chebyshev_filter(F2, 5, 0.5, 300.0, 0.1)
     assert float((F1 - F2).norm() / F2.norm()) <= 1e-13
+    F3, F4 = X.clone(), X.clone()                                   # even degree: the final rescale is in place
+    part.chebyshev_filter(F3, 6, 0.5, 300.0, 0.1)
+    op.chebyshev_filter(F4, 6, 0.5, 300.0, 0.1)
+    assert float((F3 - F4).norm() / F4.norm()) <= 1e-13
     part.close(); op.close()

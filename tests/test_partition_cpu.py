@@ -33,6 +33,7 @@ def test_partition_covers_the_mesh_and_maps_back(world):
         assert np.array_equal(lp.cell_vertices.reshape(-1, 24), np.asarray(wl.cell_vertices).reshape(-1, 24)[lp.cells])
         touched[lp.dofs] += 1
         assert np.array_equal(lp.dofs[lp.shared_rows], cp.shared_dofs[lp.shared_slots])     # rows <-> slots of shared dofs
+        assert lp.shared_owner.dtype == np.uint8 and lp.shared_owner.shape == lp.shared_rows.shape
         # projectors: the local CSR is the global one restricted to this rank's cells, samples and couplings carried along
         for jl, j in enumerate(lp.proj_ids):
             assert lp.D[jl] == wl.D[j]
@@ -44,9 +45,61 @@ def test_partition_covers_the_mesh_and_maps_back(world):
         assert lp.chi_q.shape == (len(lp.proj_cell_idx), n_q)
     assert touched.min() >= 1
     assert np.array_equal(np.nonzero(touched >= 2)[0], cp.shared_dofs)
+    owners = np.zeros(len(cp.shared_dofs), dtype=int)                                       # every shared dof has ONE owner
+    for r in range(world):
+        lp = cp.local(r)
+        np.add.at(owners, lp.shared_slots, lp.shared_owner)
+    assert np.all(owners == 1)
     assert proj_cells_seen == len(wl.proj_cell_idx)                                         # every (projector, cell) pair once
     if world == 1:
         assert len(cp.shared_dofs) == 0
+
+
+def test_scaled_scalars_reproduce_the_three_term_recurrence():
+    """W_k = s_k Y_k with W_k = W_{k-2} + g_k (H~ - c) W_{k-1} (U14) on scalars: for an eigenvalue lam the classic
+    recurrence gives y_m, the scaled one w_m / s_m: equal; and the guard returns None when s_k leaves the FP32 range."""
+    from paper_2203_07820_b200.partition import PartitionedOperator as PO
+    m, a, b, a0 = 12, 0.4, 30.0, -0.3
+    scal, c = PO.recurrence_scalars(m, a, b, a0)
+    gam, inv_sm, c2 = PO.scaled_scalars(m, a, b, a0)
+    assert c2 == c and len(gam) == m
+    for lam in (-0.3, 0.1, 5.0, 29.0):
+        y0, y1 = 1.0, scal[0][0] * (lam - c)
+        w0, w1 = 1.0, gam[0] * (lam - c)
+        for k in range(1, m):
+            y0, y1 = y1, scal[k][0] * (lam - c) * y1 - scal[k][1] * y0
+            w0, w1 = w1, w0 + gam[k] * (lam - c) * w1
+        assert abs(w1 * inv_sm - y1) <= 1e-12 * max(1.0, abs(y1))
+    assert PO.scaled_scalars(60, 0.4, 30.0, -30.0, precision=32) is None and PO.scaled_scalars(60, 0.4, 30.0, -30.0) is not None
+
+
+def test_delta_exchange_with_owner_correction_sums_to_the_whole_mesh_update():
+    """The accumulate-only exchange (include/chfsi.h: chfsi_pack_rows_delta / chfsi_unpack_rows_sum) with the ORACLE as the part
+    operators: every part adds g (H~_part - c) X to its copy of W, subtracting c X once per dof it holds; what travels is
+    W_new - W_old on the shared rows, with g c X put back by the parts that do not own the dof; base + sum = W + g (H~ - c) X."""
+    from oracle import chfsi_oracle as orc
+    from paper_2203_07820_b200 import mesh_mass
+    from paper_2203_07820_b200.partition import CellPartition
+    wl = small_workload(nonlocal_=False)
+    world, g, c = 3, -0.37, 1.9
+    cp = CellPartition(wl, world)
+    Mg = mesh_mass(wl.p, wl.cell_dofs, wl.cell_vertices, wl.n_dofs)
+    rng = np.random.default_rng(8)
+    X, W = rng.standard_normal((wl.n_dofs, 4)), rng.standard_normal((wl.n_dofs, 4))
+    want = W + g * (orc.apply_H(orc.operator_from_workload(wl), X) - c * X)
+    buf = np.zeros((len(cp.shared_dofs), 4))
+    locals_ = []
+    for r in range(world):
+        lp = cp.local(r)
+        oop = orc.build_operator(wl.p, lp.cell_dofs, lp.cell_vertices, len(lp.dofs), lp.veff_q)
+        oop.M = Mg[lp.dofs]
+        Wl = W[lp.dofs] + g * (orc.apply_H(oop, X[lp.dofs]) - c * X[lp.dofs])               # what the part's kernel leaves
+        base = W[lp.dofs][lp.shared_rows]
+        buf[lp.shared_slots] += Wl[lp.shared_rows] - base + g * c * X[lp.dofs][lp.shared_rows] * (1 - lp.shared_owner)[:, None]
+        locals_.append((lp, Wl, base))
+    for lp, Wl, base in locals_:
+        Wl[lp.shared_rows] = base + buf[lp.shared_slots]
+        assert np.max(np.abs(Wl - want[lp.dofs])) <= 1e-12 * np.max(np.abs(want))
 
 
 def test_mesh_mass_of_the_library_equals_the_oracle_and_the_volume():
@@ -138,5 +191,9 @@ def test_part_entry_points_report_argument_errors_without_a_device():
                      (lib.chfsi_apply_H_with_coefficients, (None, None, 0, None, 0, 0, None, None, None)),
                      (lib.chfsi_pack_rows, (None, None, 0, 0, None, None, 0, None, 64, None)),
                      (lib.chfsi_unpack_rows, (None, None, 64, None, None, 0, None, 0, 0, None)),
-                     (lib.chfsi_recurrence_update, (None, None, 0, None, 0, None, 0, 0, 1.0, 0.0, 0.0, None))):
+                     (lib.chfsi_recurrence_update, (None, None, 0, None, 0, None, 0, 0, 1.0, 0.0, 0.0, None)),
+                     (lib.chfsi_accumulate_supported, (None, None, 0, None, 0, 0, None, None)),
+                     (lib.chfsi_apply_shifted_with_coefficients, (None, None, 0, None, 0, 0, 1.0, 0.0, 1, None, None, None)),
+                     (lib.chfsi_pack_rows_delta, (None, None, 0, None, None, 0, None, 0.0, 0, None, None, 0, None, 64, None)),
+                     (lib.chfsi_unpack_rows_sum, (None, None, 64, None, None, None, 0, None, 0, 0, None))):
         assert fn(*args) == -1
