@@ -165,3 +165,41 @@ def test_single_part_equals_the_plain_operator(aps):
     op.chebyshev_filter(F4, 6, 0.5, 300.0, 0.1)
     assert float((F3 - F4).norm() / F4.norm()) <= 1e-13
     part.close(); op.close()
+
+
+_NCCL_WORLD1 = r"""
+import os, sys
+import torch, torch.distributed as dist
+torch.cuda.set_device(0)
+dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", 0))
+from paper_2203_07820_b200 import Operator
+from paper_2203_07820_b200.partition import PartitionedOperator, TorchComm
+from workloads.generate import make_workload, random_block
+wl = make_workload(None, n=3, p=6, L=6.0, mesh_jitter=0.1, atoms_per_side=1, n_gaussians=0, nonlocal_=True, smooth_field=0.05,
+                   seed_base=56, r_cut=2.2)
+part = PartitionedOperator(wl, comm=TorchComm())
+op = Operator.from_workload(wl)
+X = torch.tensor(random_block(wl.n_dofs, range(32), 2), device="cuda")
+assert torch.equal(part.apply_H(X), op.apply_H(X))
+F1, F2, F3 = X.clone(), X.clone(), X.clone()
+part.chebyshev_filter_chunked(F1, 8, 7, 0.5, 300.0, 0.1)                  # async all-reduces, two chunks in flight
+op.chebyshev_filter(F2, 7, 0.5, 300.0, 0.1)
+part.chebyshev_filter_chunked(F3, 8, 7, 0.5, 300.0, 0.1, scaled=False)
+torch.cuda.synchronize()
+assert float((F1 - F2).norm() / F2.norm()) <= 1e-13 and float((F3 - F2).norm() / F2.norm()) <= 1e-13
+dist.destroy_process_group()
+print("NCCL-WORLD1-OK")
+"""
+
+
+def test_torch_distributed_communicator_over_nccl_with_one_rank():
+    """TorchComm on the NCCL backend (the communicator `bench.py --gpus N --partition` uses), world size 1, in a process of its
+    own: process-group set-up with a device id, the host all-reduce of the mass through a device tensor, synchronous and
+    asynchronous device all-reduces ordered against the library's kernels on torch's current stream.  More ranks need more GPUs."""
+    import os
+    import subprocess
+    import sys
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1", MASTER_PORT=str(29600 + os.getpid() % 300), RANK="0", WORLD_SIZE="1")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, "-c", _NCCL_WORLD1], cwd=root, env=env, capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0 and "NCCL-WORLD1-OK" in r.stdout, r.stdout[-2000:] + r.stderr[-4000:]
