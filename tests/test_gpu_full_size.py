@@ -11,6 +11,8 @@ assembly), through the C ABI.  `-m gpu`.
    the GPU-vs-GPU identities below.
  * properties that hold at any size: the fused filter equals the three-term recurrence driven by separate
    apply_H calls; a column filtered inside the wide chunk equals the same column filtered alone (generic kernel).
+ * the Rayleigh-Ritz products of Algorithm 2 at the size `bench.py --rr` times (config 3's rows, N = 1024): sampled columns
+   of S and H^ (H~ of those columns by the oracle) and sampled rows of Y Z against cuBLAS products, FP64 and mixed.
 """
 import numpy as np
 import pytest
@@ -176,6 +178,66 @@ def _check_whole_job_sampled_columns(config, wl, oop):
     d = float(np.max(np.abs(th_g - th_o)))
     print(f"config {config}: column errors {['%.2e' % e for e in errs]}, Ritz difference {d:.3e} Ha, first-order slack {slack:.3e}")
     assert d <= tol_ritz + slack, (d, slack)
+    op.close()
+
+
+def test_config3_rayleigh_ritz_products_at_the_size_bench_rr_times(config3_oracle):
+    """Algorithm 2's O(M N^2) products in the launch configuration `bench.py --rr` times: config 3's 884,736 rows, N = 1024
+    columns, H~Y in chunks of 256, mixed blocking with FP64 diagonal blocks of 256 and N_fr = 128.  Sampled COLUMNS of S and H^
+    against cuBLAS products of torch (for H^ with the ORACLE's H~ on those columns), sampled ROWS of Y Z against torch, for
+    a dense and an upper-triangular Z; plus what holds at any size: exact symmetry (lower triangle computed),
+    diag S = squared column norms, FP64 entries of the mixed matrices where Eq. 38-39 put them."""
+    torch, orc, Operator, CONFIGS, SEED_X, load_bounds, make_workload, random_block = _imports()
+    wl, oop = config3_oracle
+    op = Operator.from_workload(wl)
+    N, B, blk, n_fr = 1024, 256, 256, 128
+    n_oc = N - n_fr
+    eps32 = float(np.finfo(np.float32).eps)
+    cols = [0, 600, 1023]
+    g = torch.Generator(device="cuda")
+    g.manual_seed(2203)
+    Y = torch.empty((wl.n_dofs, N), dtype=torch.float64, device="cuda")
+    for j0 in range(0, N, 256):
+        Y[:, j0:j0 + 256] = torch.randn((wl.n_dofs, 256), dtype=torch.float64, device="cuda", generator=g)
+    Y *= (1.0 + 0.5 * torch.rand(N, dtype=torch.float64, device="cuda", generator=g)) / np.sqrt(wl.n_dofs)
+    nY = Y.norm(dim=0)
+    # -- S
+    S = op.overlap_matrix(Y)
+    assert torch.equal(S, S.T)
+    Sc = Y.T @ Y[:, cols]
+    sc_scale = torch.outer(nY, nY[cols])
+    assert float(((S[:, cols] - Sc).abs() / sc_scale).max()) <= 1e-12
+    assert float(((S.diagonal() - nY * nY).abs() / (nY * nY)).max()) <= 1e-12
+    Sm = op.overlap_matrix_mixed(Y, blk)
+    assert torch.equal(Sm, Sm.T)
+    err = (Sm - S).abs() / torch.outer(nY, nY)
+    inblk = (torch.arange(N, device="cuda")[:, None] // blk) == (torch.arange(N, device="cuda")[None, :] // blk)
+    assert float(err[inblk].max()) <= 1e-13 and float(err[~inblk].max()) <= 8 * eps32 and float(err[~inblk].max()) > 1e-12
+    # -- H^ (the oracle's H~ on the sampled columns)
+    Wo = torch.from_numpy(orc.apply_H(oop, Y[:, cols].cpu().numpy())).to("cuda")
+    nW = Wo.norm(dim=0)
+    Hc = Y.T @ Wo
+    hc_scale = torch.outer(nY, nW)
+    ws = op.workspace(B)
+    Hh = op.projected_hamiltonian(Y, B=B, workspace=ws)
+    assert torch.equal(Hh, Hh.T)
+    assert float(((Hh[:, cols] - Hc).abs() / hc_scale).max()) <= 1e-11
+    Hm = op.projected_hamiltonian_mixed(Y, n_oc, B=B, workspace=ws)
+    assert torch.equal(Hm, Hm.T)
+    errm = (Hm[:, cols] - Hc).abs() / hc_scale
+    assert float(errm.max()) <= 8 * eps32
+    assert float(errm[n_oc:, 2].max()) <= 1e-11                   # column 1023 is in the fr block: its fr rows are FP64 products
+    # -- Y Z on sampled rows: the first and a middle 128-row tile, and the last rows
+    rows = torch.cat([torch.arange(0, 128), torch.arange(442368, 442368 + 128), torch.arange(wl.n_dofs - 64, wl.n_dofs)]).to("cuda")
+    Zd = torch.randn((N, N), dtype=torch.float64, device="cuda", generator=g) / np.sqrt(N)
+    Out = torch.empty_like(Y)
+    for Z in (Zd, Zd.triu()):
+        ref = Y[rows] @ Z
+        scale = torch.outer(Y[rows].norm(dim=1), Z.norm(dim=0))
+        op.subspace_transform(Y, Z, Out=Out)
+        assert float(((Out[rows] - ref).abs() / scale).max()) <= 1e-13
+        op.subspace_transform_mixed(Y, Z, Out=Out)
+        assert float(((Out[rows] - ref).abs() / scale).max()) <= 8 * eps32
     op.close()
 
 
