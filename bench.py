@@ -41,6 +41,8 @@ NCU_TRAFFIC_BYTES_PER_LAUNCH = {
     (3, "k_apply_sf<double>"): 8.82e9,         # same file: 5.97 GB read + 2.84 GB written
     (5, "k_apply_sf_ws<double>"): 27.22e9,     # profiles/r02c_ws_kernel.md: 18.48 GB read + 8.74 GB written
     (3, "k_apply_sf_ws<double>"): 8.80e9,      # same file: 5.97 GB read + 2.83 GB written
+    (2, "k_apply_sf_ws<double>"): 0.943e9,     # profiles/r02d_final.md: 0.661 GB read + 0.282 GB written
+    (4, "k_apply_sf_ws<float>"): 8.80e9,       # same file: 5.97 GB read + 2.83 GB written (32-column tiles of FP32 rows)
 }
 
 
